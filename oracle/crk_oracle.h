@@ -1,0 +1,79 @@
+/* crk_oracle.h -- CPU ORACLE for the CRKSPH short-range gas pipeline.  TEST INFRASTRUCTURE ONLY.
+ *
+ * A plain, slow, obviously-correct FP64 implementation of what the hot path computes, written from
+ * /root/reference/PAPER.md (arxiv 2202.02840) section 2.2, Eqs. 12-18 and 24-32, with the readings
+ * listed in DESIGN.md ("Readings of the paper").  Neighbours are found by a brute-force O(N^2) periodic
+ * minimum-image scan; sums run over exactly those sets.  No cells, no tiles, no fusion.
+ *
+ * It shares NO code with the CUDA library (paper_2202_02840_b200/csrc) and neither includes the other.
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may use it.
+ *
+ * All pointers are HOST pointers.  Inputs are the same float32 arrays the CUDA library receives; every
+ * value is promoted to double -- except the neighbour predicate, which is evaluated in prescribed FP32
+ * (reading S3) so that neighbour sets are a bit-exact contract rather than a rounding accident.
+ *
+ * Pin status (tests/test_oracle_pins.py): kernel, volumes, moments, A, B, gradA, gradB, RK gradient,
+ * grad v, limiter, viscosity switch-off, momentum/energy pair antisymmetry are pinned.  PARITY UNPINNED
+ * (fixed by DESIGN.md readings only): Eq. 18 P_j-vs-P_i choice (S6), rho = m/V for unequal masses (S2),
+ * c_s clamp max(u,0) (S12).
+ */
+#ifndef CRK_ORACLE_H
+#define CRK_ORACLE_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct crk_oracle_ctx crk_oracle_ctx;
+
+typedef struct {
+    double box;    /* cubic periodic box side L, positions in [0,L)                         */
+    double gamma;  /* adiabatic index, Eq. 4                                                */
+    double n_h;    /* hhat = h/n_h (Eq. 25); eta_crit = 1/n_h, eta_fold = 0.2/n_h (l.179)   */
+    double C_l, C_q; /* (2,1)                                                 */
+    double eps;    /* 0.1, enters as eps^2 * hhat^2 in Eq. 25                               */
+} crk_oracle_params;
+
+crk_oracle_ctx* crk_oracle_create(const crk_oracle_params* p);
+void            crk_oracle_destroy(crk_oracle_ctx* c);
+void            crk_oracle_set_threads(int nthreads);   /* 0 = all cores */
+int             crk_oracle_get_threads(void);
+
+/* neighbour search (brute force, periodic): returns 0, or -1 on bad input (h<=0, h>=L/2, x outside [0,L)) */
+int crk_oracle_build(crk_oracle_ctx* c, int64_t n, const float* x, const float* y, const float* z, const float* h);
+/* Eq. 14 + S2: V = 1/sum_j W(r_ij,h_i) (self included), rho = m/V; nbr_count = #{j!=i : r_ij < h_i}      */
+int crk_oracle_volumes(crk_oracle_ctx* c, const float* m, double* V, double* rho, uint32_t* nbr_count);
+/* PAPER.md:116 constraints: A[n], B[3][n], gradA[3][n] (d_c A), gradB[9][n] (index 3*c+a = d_c B^a)    */
+int crk_oracle_rk_coefficients(crk_oracle_ctx* c, double* A, double* B, double* gradA, double* gradB);
+/* Eqs. 26, 27-32, 24-25, 17-18: a = dv/dt [n] x3, dudt [n]; pair_count = #{j!=i : r_ij < max(h_i,h_j)}    */
+int crk_oracle_hydro_derivs(crk_oracle_ctx* c, const float* vx, const float* vy, const float* vz, const float* u,
+                            double* ax, double* ay, double* az, double* dudt, uint32_t* pair_count);
+/* the four calls above in order */
+int crk_oracle_step_derivs(crk_oracle_ctx* c, int64_t n, const float* x, const float* y, const float* z,
+                           const float* h, const float* vx, const float* vy, const float* vz, const float* m,
+                           const float* u, double* ax, double* ay, double* az, double* dudt);
+
+/* ---- diagnostics used by the pins (tests only) ---- */
+double crk_oracle_W(double r, double h);        /* Eq. 12                                   */
+double crk_oracle_dWdr(double r, double h);     /* its radial derivative                    */
+/* raw moments after crk_oracle_rk_coefficients: m0[n], m1[3][n], m2[9][n] (index 3*a+b); any may be NULL */
+int crk_oracle_get_moments(crk_oracle_ctx* c, double* m0, double* m1, double* m2);
+/* after crk_oracle_hydro_derivs */
+int crk_oracle_get_gradv(crk_oracle_ctx* c, double* gradv /* [9][n], index 3*alpha+beta = d_beta v^alpha */);
+/* S0_i = sum_j V_j WR_ij ; S1_i = sum_j V_j x_ij WR_ij ; G0_i = sum_j V_j grad WR_ij ;
+ * G1_i[3*a+c] = sum_j V_j x_ij^a (grad WR_ij)^c   (sums over the gather set incl. self)                */
+int crk_oracle_rk_sums(crk_oracle_ctx* c, double* S0, double* S1, double* G0, double* G1);
+/* A, B of the reproducing kernel centred at an arbitrary point p with support h, sources = all particles with
+ * their V_j held fixed (reading S5); brute force over all particles                                     */
+int crk_oracle_eval_AB_at(crk_oracle_ctx* c, const double p[3], double h, double* A, double B[3]);
+/* contribution of neighbour j to particle i in Eqs. 17/18: out = { m_i a_{i<-j} (3), m_i du_{i<-j} }       */
+int crk_oracle_pair_term(crk_oracle_ctx* c, int64_t i, int64_t j, double out[4]);
+/* limiter phi_ij and viscous pressures Q_i, Q_j of a pair (Eqs. 24-32): out = {phi, Q_i, Q_j, mu_i, mu_j}  */
+int crk_oracle_pair_visc(crk_oracle_ctx* c, int64_t i, int64_t j, double out[5]);
+/* neighbour list of i: entries j | flags (bit31: r<h_i, bit30: r<h_j); returns count (may exceed cap)    */
+int64_t crk_oracle_neighbors(crk_oracle_ctx* c, int64_t i, uint32_t* buf, int64_t cap);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

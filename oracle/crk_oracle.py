@@ -1,0 +1,207 @@
+"""ctypes front end of the CPU oracle (oracle/crk_oracle.cpp).  TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs import this.
+It never imports the CUDA package.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import sys
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, _HERE)
+import build as _build  # noqa: E402  (oracle/build.py)
+sys.path.pop(0)
+
+
+class _Params(C.Structure):
+    _fields_ = [("box", C.c_double), ("gamma", C.c_double), ("n_h", C.c_double),
+                ("C_l", C.c_double), ("C_q", C.c_double), ("eps", C.c_double)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(_build.build())
+        fp, dp, up = C.POINTER(C.c_float), C.POINTER(C.c_double), C.POINTER(C.c_uint32)
+        L.crk_oracle_create.restype = C.c_void_p
+        L.crk_oracle_create.argtypes = [C.POINTER(_Params)]
+        L.crk_oracle_destroy.argtypes = [C.c_void_p]
+        L.crk_oracle_set_threads.argtypes = [C.c_int]
+        L.crk_oracle_get_threads.restype = C.c_int
+        L.crk_oracle_build.argtypes = [C.c_void_p, C.c_int64, fp, fp, fp, fp]
+        L.crk_oracle_volumes.argtypes = [C.c_void_p, fp, dp, dp, up]
+        L.crk_oracle_rk_coefficients.argtypes = [C.c_void_p, dp, dp, dp, dp]
+        L.crk_oracle_hydro_derivs.argtypes = [C.c_void_p, fp, fp, fp, fp, dp, dp, dp, dp, up]
+        L.crk_oracle_W.restype = C.c_double
+        L.crk_oracle_W.argtypes = [C.c_double, C.c_double]
+        L.crk_oracle_dWdr.restype = C.c_double
+        L.crk_oracle_dWdr.argtypes = [C.c_double, C.c_double]
+        L.crk_oracle_get_moments.argtypes = [C.c_void_p, dp, dp, dp]
+        L.crk_oracle_get_gradv.argtypes = [C.c_void_p, dp]
+        L.crk_oracle_rk_sums.argtypes = [C.c_void_p, dp, dp, dp, dp]
+        L.crk_oracle_eval_AB_at.argtypes = [C.c_void_p, dp, C.c_double, dp, dp]
+        L.crk_oracle_pair_term.argtypes = [C.c_void_p, C.c_int64, C.c_int64, dp]
+        L.crk_oracle_pair_visc.argtypes = [C.c_void_p, C.c_int64, C.c_int64, dp]
+        L.crk_oracle_neighbors.restype = C.c_int64
+        L.crk_oracle_neighbors.argtypes = [C.c_void_p, C.c_int64, up, C.c_int64]
+        _lib = L
+    return _lib
+
+
+def _f(a):
+    a = np.ascontiguousarray(a, dtype=np.float32)
+    return a, a.ctypes.data_as(C.POINTER(C.c_float))
+
+
+def _d(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def _u(a):
+    return a.ctypes.data_as(C.POINTER(C.c_uint32))
+
+
+def kernel_W(r, h):
+    return lib().crk_oracle_W(float(r), float(h))
+
+
+def kernel_dWdr(r, h):
+    return lib().crk_oracle_dWdr(float(r), float(h))
+
+
+def set_threads(n: int):
+    lib().crk_oracle_set_threads(int(n))
+
+
+def get_threads() -> int:
+    return int(lib().crk_oracle_get_threads())
+
+
+class Oracle:
+    """Call-by-call mirror of the C-ABI library: build -> volumes -> rk_coefficients -> hydro_derivs."""
+
+    def __init__(self, box=1.0, gamma=5.0 / 3.0, n_h=2.4, C_l=2.0, C_q=1.0, eps=0.1):
+        self.params = _Params(box, gamma, n_h, C_l, C_q, eps)
+        self._c = lib().crk_oracle_create(C.byref(self.params))
+        self.n = 0
+        self._keep = []
+
+    def __del__(self):
+        if getattr(self, "_c", None):
+            lib().crk_oracle_destroy(self._c)
+            self._c = None
+
+    def build(self, x, y, z, h):
+        (x, px), (y, py), (z, pz), (h, ph) = _f(x), _f(y), _f(z), _f(h)
+        self.n = x.shape[0]
+        rc = lib().crk_oracle_build(self._c, self.n, px, py, pz, ph)
+        if rc:
+            raise ValueError("crk_oracle_build: bad input (h<=0, h>=L/2 or position outside [0,L))")
+
+    def volumes(self, m):
+        m, pm = _f(m)
+        n = self.n
+        V, rho, cnt = np.empty(n), np.empty(n), np.empty(n, dtype=np.uint32)
+        rc = lib().crk_oracle_volumes(self._c, pm, _d(V), _d(rho), _u(cnt))
+        assert rc == 0
+        return V, rho, cnt
+
+    def rk_coefficients(self):
+        n = self.n
+        A, B, gA, gB = np.empty(n), np.empty((3, n)), np.empty((3, n)), np.empty((9, n))
+        rc = lib().crk_oracle_rk_coefficients(self._c, _d(A), _d(B), _d(gA), _d(gB))
+        assert rc == 0
+        return A, B, gA, gB
+
+    def hydro_derivs(self, vx, vy, vz, u):
+        (vx, p1), (vy, p2), (vz, p3), (u, p4) = _f(vx), _f(vy), _f(vz), _f(u)
+        n = self.n
+        ax, ay, az, du = np.empty(n), np.empty(n), np.empty(n), np.empty(n)
+        cnt = np.empty(n, dtype=np.uint32)
+        rc = lib().crk_oracle_hydro_derivs(self._c, p1, p2, p3, p4, _d(ax), _d(ay), _d(az), _d(du), _u(cnt))
+        assert rc == 0
+        return ax, ay, az, du, cnt
+
+    def step_derivs(self, ps):
+        """ps: crk_workloads.ParticleSet (or anything with x,y,z,h,vx,vy,vz,m,u). Returns dict of all outputs."""
+        self.build(ps.x, ps.y, ps.z, ps.h)
+        V, rho, nbr = self.volumes(ps.m)
+        A, B, gA, gB = self.rk_coefficients()
+        ax, ay, az, du, pc = self.hydro_derivs(ps.vx, ps.vy, ps.vz, ps.u)
+        return dict(V=V, rho=rho, nbr_count=nbr, A=A, B=B, gradA=gA, gradB=gB,
+                    ax=ax, ay=ay, az=az, dudt=du, pair_count=pc)
+
+    # ---- diagnostics for the pins
+    def moments(self):
+        n = self.n
+        m0, m1, m2 = np.empty(n), np.empty((3, n)), np.empty((9, n))
+        assert lib().crk_oracle_get_moments(self._c, _d(m0), _d(m1), _d(m2)) == 0
+        return m0, m1, m2
+
+    def gradv(self):
+        g = np.empty((9, self.n))
+        assert lib().crk_oracle_get_gradv(self._c, _d(g)) == 0
+        return g
+
+    def rk_sums(self):
+        n = self.n
+        S0, S1, G0, G1 = np.empty(n), np.empty((3, n)), np.empty((3, n)), np.empty((9, n))
+        assert lib().crk_oracle_rk_sums(self._c, _d(S0), _d(S1), _d(G0), _d(G1)) == 0
+        return S0, S1, G0, G1
+
+    def eval_AB_at(self, p, h):
+        p = np.ascontiguousarray(p, dtype=np.float64)
+        A = C.c_double()
+        B = np.empty(3)
+        assert lib().crk_oracle_eval_AB_at(self._c, _d(p), float(h), C.byref(A), _d(B)) == 0
+        return A.value, B
+
+    def pair_term(self, i, j):
+        out = np.empty(4)
+        assert lib().crk_oracle_pair_term(self._c, int(i), int(j), _d(out)) == 0
+        return out
+
+    def pair_visc(self, i, j):
+        out = np.empty(5)
+        assert lib().crk_oracle_pair_visc(self._c, int(i), int(j), _d(out)) == 0
+        return out
+
+    def neighbors(self, i):
+        cnt = lib().crk_oracle_neighbors(self._c, int(i), None, 0)
+        buf = np.empty(max(cnt, 1), dtype=np.uint32)
+        lib().crk_oracle_neighbors(self._c, int(i), _u(buf), cnt)
+        buf = buf[:cnt]
+        return buf & np.uint32(0x3fffffff), (buf >> np.uint32(31)).astype(bool), ((buf >> np.uint32(30)) & 1).astype(bool)
+
+
+def euler_steps(ps, n_steps: int, dt: float, oracle: Oracle | None = None):
+    """Step 12 of DESIGN.md (BASELINE config 2): forward Euler in FP64 on the oracle's derivatives.
+    Yields (step, state_f32 ParticleSet-like dict, derivs dict) BEFORE each update, so a caller can
+    teacher-force another implementation on the same FP32 state.  h and m stay fixed."""
+    import copy
+    o = oracle or Oracle(ps.box, ps.gamma, ps.n_h)
+    st = {k: np.asarray(getattr(ps, k), dtype=np.float64).copy() for k in ("x", "y", "z", "vx", "vy", "vz", "u")}
+    L = ps.box
+    for step in range(n_steps + 1):
+        cur = copy.copy(ps)
+        for k in st:
+            setattr(cur, k, st[k].astype(np.float32))
+        for k in ("x", "y", "z"):           # the float32 cast may round up to L
+            a = getattr(cur, k)
+            a[a >= np.float32(L)] = np.float32(0.0)
+        d = o.step_derivs(cur)
+        yield step, cur, d
+        if step == n_steps:
+            break
+        for k, v, a in (("x", "vx", "ax"), ("y", "vy", "ay"), ("z", "vz", "az")):
+            p = st[k] + st[v] * dt
+            st[k] = p - np.floor(p / L) * L          # re-wrap with floor (reading S12)
+            st[v] = st[v] + d[a] * dt
+        st["u"] = st["u"] + d["dudt"] * dt
