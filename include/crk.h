@@ -1,0 +1,113 @@
+/* crk.h -- C ABI of libcrk: the CRKSPH short-range gas interaction pipeline of CRK-HACC (arxiv 2202.02840) on one
+ * NVIDIA B200 (sm_100a).  Hand-written CUDA kernels behind plain pointers; no torch types cross this boundary.
+ *
+ * What the library computes (citations are lines of /root/reference/PAPER.md; readings S1..S15 are in DESIGN.md):
+ *   crk_build_cells      neighbour search structure: space-filling-curve sort, 32-particle leaf buckets with
+ *                        bounding boxes extended by the leaf's maximal smoothing length, and the leaf interaction
+ *                        list that every hydro kernel reuses (section 3.3), periodic box.
+ *   crk_volumes          V_i^-1 = n_i = sum_j W(|x_i-x_j|, h_i)            Eq. 14, Wendland C4 Eq. 12
+ *                        rho_i = m_i / V_i (S2); neighbour count #{j != i : r_ij < h_i}
+ *   crk_rk_coefficients  A_i, B_i and their gradients from  sum_j V_j WR_ij = 1,  sum_j V_j x_ij WR_ij = 0
+ *                         with WR_ij = A_i (1 + B_i.x_ij) W_ij    Eqs. 15-16
+ *   crk_hydro_derivs     grad v_i (Eq. 26), limiter phi_ij (Eqs. 28-32), viscous pressure Q (Eqs. 24-25 with the
+ *                        midpoint projection of Eq. 27), then dv_i/dt (Eq. 17) and du_i/dt (Eq. 18) with P -> P+Q
+ *                        (PAPER.md:120-122, 151); non-cosmological natural units a = 1, adot = 0
+ *   crk_step_derivs      the four calls above in order (one "hydro sub-cycle" derivative evaluation)
+ *
+ * Conventions
+ *   - h is the SUPPORT radius: W = 0 for |x| >= h.  n_h relates it to the inter-particle spacing.
+ *   - Every array pointer is a DEVICE pointer owned by the caller (except in crk_step_derivs_host), SoA, length n,
+ *     float32 / uint32.  Inputs are never modified.  Outputs are written in the caller's particle order.
+ *   - Calls are asynchronous on the stream given to crk_create and ordered on it, except that crk_build_cells
+ *     synchronises once (it must learn the interaction-list size before allocating it).
+ *   - State flows build -> volumes -> rk_coefficients -> hydro_derivs inside the context; calling out of order
+ *     returns CRK_ESTATE.  The context owns all scratch memory (cudaMalloc, grown on demand, freed by crk_destroy).
+ *   - Errors: every call returns CRK_OK (0) or a negative code; nothing aborts or throws across the boundary; there
+ *     is no host fallback.  crk_last_error gives a message for the last failure on that context.
+ *   - Neighbour predicate (bit-exact contract, S3): d = x_i - x_j in float, wrapped by -+L if |d| > L/2,
+ *     r2 = fmaf(dz,dz,fmaf(dy,dy,dx*dx)); j is a neighbour of i iff r2 < h_i*h_i; the pair interacts in
+ *     crk_hydro_derivs iff r2 < max(h_i*h_i, h_j*h_j).
+ */
+#ifndef CRK_H
+#define CRK_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CRK_OK       0
+#define CRK_EINVAL  -1   /* null pointer, negative n, bad parameter                                            */
+#define CRK_ERANGE  -2   /* some h <= 0 or h >= L/2, or a position outside [0, L)  (checked on the device)    */
+#define CRK_ENOMEM  -3   /* device allocation failed                                                          */
+#define CRK_ECUDA   -4   /* a CUDA call or kernel failed; see crk_last_error                                  */
+#define CRK_ESTATE  -5   /* calls made out of order                                                           */
+
+typedef struct crk_ctx crk_ctx;   /* opaque */
+
+typedef struct {
+    float box;        /* cubic periodic box side L; positions in [0, L)                                       */
+    float gamma;      /* adiabatic index of Eq. 4                                                             */
+    float n_h;        /* particles per support radius: hhat = h/n_h (Eq. 25), eta_crit = 1/n_h,
+                         eta_fold = 0.2/n_h.  Paper default 4; the BASELINE configs use 2.4    */
+    float C_l, C_q;   /* linear / quadratic viscosity coefficients, (2, 1) in the paper        */
+    float eps;        /* 0.1; enters Eq. 25 as eps^2 * hhat^2                                                 */
+    int   leaf_size;  /* particles per leaf bucket; must be 32 in this version (one warp lane per particle)   */
+    int   flags;      /* reserved, 0                                                                          */
+} crk_params;
+
+typedef struct {
+    int64_t  n;               /* particles in the last build                                                  */
+    int64_t  n_leaves;        /* leaf buckets                                                                 */
+    int64_t  n_leaf_pairs;    /* entries of the leaf interaction list (symmetric criterion)                   */
+    int64_t  n_leaf_pairs_gather; /* of which satisfy the one-sided (gather) criterion                        */
+    int64_t  launches;        /* kernels launched by this context since crk_create / crk_reset_stats          */
+    int64_t  scratch_bytes;   /* device memory currently owned by the context                                 */
+    float    ms_build, ms_volumes, ms_rk, ms_hydro;   /* device time of the last call of each entry point,
+                                                         valid when timing is on (crk_set_timing)             */
+    float    ms_sort, ms_tree, ms_gradv, ms_forces;   /* finer split: sort+pack | leaves+list | Eq.26 | Eqs.17-18 */
+} crk_stats;
+
+/* stream: a cudaStream_t (0 = default stream).  Returns CRK_OK and *out, or an error.                       */
+int  crk_create(crk_ctx** out, const crk_params* params, void* cuda_stream);
+void crk_destroy(crk_ctx* c);
+
+/* x, y, z, h: device float[n].  Builds the sorted particle order, leaves and the leaf interaction list.     */
+int  crk_build_cells(crk_ctx* c, int64_t n, const float* x, const float* y, const float* z, const float* h);
+/* m: device float[n].  V, rho: device float[n] or NULL.  nbr_count: device uint32[n] or NULL.               */
+int  crk_volumes(crk_ctx* c, const float* m, float* V, float* rho, uint32_t* nbr_count);
+/* A: float[n]; B: float[3][n]; gradA: float[3][n] (index c: d_c A); gradB: float[9][n] (index 3*c+a: d_c B^a).
+ * Any may be NULL (the coefficients are kept inside the context for crk_hydro_derivs either way).           */
+int  crk_rk_coefficients(crk_ctx* c, float* A, float* B, float* gradA, float* gradB);
+/* vx, vy, vz, u: device float[n] (u = specific internal energy).  ax, ay, az = dv/dt, dudt = du/dt: device
+ * float[n].  pair_count: device uint32[n] or NULL = #{j != i : r_ij < max(h_i, h_j)}.                        */
+int  crk_hydro_derivs(crk_ctx* c, const float* vx, const float* vy, const float* vz, const float* u,
+                      float* ax, float* ay, float* az, float* dudt, uint32_t* pair_count);
+/* build_cells + volumes + rk_coefficients + hydro_derivs.  All device pointers.                             */
+int  crk_step_derivs(crk_ctx* c, int64_t n, const float* x, const float* y, const float* z, const float* h,
+                     const float* vx, const float* vy, const float* vz, const float* m, const float* u,
+                     float* ax, float* ay, float* az, float* dudt);
+/* Same, with HOST pointers (pinned memory recommended): copies the nine inputs to the device, evaluates, copies
+ * the four outputs back and synchronises the stream.  This is the end-to-end entry bench.py's `e2e` times.  */
+int  crk_step_derivs_host(crk_ctx* c, int64_t n, const float* x, const float* y, const float* z, const float* h,
+                          const float* vx, const float* vy, const float* vz, const float* m, const float* u,
+                          float* ax, float* ay, float* az, float* dudt);
+
+/* ---- diagnostics ---- */
+const char* crk_last_error(const crk_ctx* c);
+int  crk_get_perm(crk_ctx* c, int32_t* perm);        /* device int32[n]: perm[k] = caller index of sorted slot k   */
+int  crk_get_gradv(crk_ctx* c, float* gradv);         /* device float[9][n], index 3*a+b = d_b v^a (Eq. 26), caller order */
+int  crk_get_stats(crk_ctx* c, crk_stats* out);       /* host struct                                                */
+int  crk_reset_stats(crk_ctx* c);
+int  crk_set_timing(crk_ctx* c, int on);              /* record CUDA events around each pass (adds stream syncs when read) */
+/* leaf interaction list of leaf `leaf` (host buffer): entries leaf_index | bit31 (gather) | bit30 (periodic wrap);
+ * returns the number of entries (may exceed cap) or a negative error.  Synchronises.                         */
+int64_t crk_get_leaf_list(crk_ctx* c, int64_t leaf, uint32_t* host_buf, int64_t cap);
+
+/* Measurement aid (not part of the method): runs a register-resident FFMA loop on every SM and returns the achieved
+ * FP32 rate in flop/s (FMA = 2 flops) for bench.py's roofline denominator; *ms_out receives the kernel time.  */
+double crk_measure_fp32_peak(void* cuda_stream, int repeats, float* ms_out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

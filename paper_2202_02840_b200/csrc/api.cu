@@ -1,0 +1,289 @@
+// api.cu -- the C ABI declared in include/crk.h: context, call ordering, error reporting, timing, host-buffer entry.
+#include "crk_internal.cuh"
+
+namespace {
+
+enum { EV_BUILD0 = 0, EV_SORTED, EV_BUILD1, EV_VOL0, EV_VOL1, EV_RK0, EV_GV0, EV_GV1, EV_F1, EV_RK1, EV_HY0, EV_N };
+
+void rec(crk_ctx* c, int e) {
+    if (c->timing) cudaEventRecord(c->ev[e], c->stream);
+}
+
+__global__ void k_fp32_peak(float* out, int iters, float b, float cc) {
+    float a0 = threadIdx.x * 1e-3f, a1 = a0 + 1.f, a2 = a0 + 2.f, a3 = a0 + 3.f, a4 = a0 + 4.f, a5 = a0 + 5.f,
+          a6 = a0 + 6.f, a7 = a0 + 7.f;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int u = 0; u < 16; ++u) {
+            a0 = fmaf(a0, b, cc); a1 = fmaf(a1, b, cc); a2 = fmaf(a2, b, cc); a3 = fmaf(a3, b, cc);
+            a4 = fmaf(a4, b, cc); a5 = fmaf(a5, b, cc); a6 = fmaf(a6, b, cc); a7 = fmaf(a7, b, cc);
+        }
+    }
+    const float s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
+    if (s == 12345.678f) out[0] = s;   // keep the chain alive
+}
+
+}  // namespace
+
+extern "C" {
+
+int crk_create(crk_ctx** out, const crk_params* p, void* cuda_stream) {
+    if (!out || !p) return CRK_EINVAL;
+    *out = nullptr;
+    if (!(p->box > 0.f) || !(p->gamma > 1.f) || !(p->n_h > 0.f) || p->leaf_size != CRK_LEAF) return CRK_EINVAL;
+    crk_ctx* c = new crk_ctx();
+    c->prm = *p;
+    c->stream = (cudaStream_t)cuda_stream;
+    c->err[0] = 0;
+    memset(&c->st, 0, sizeof(c->st));
+    if (cudaMalloc(&c->flag.p, 64) != cudaSuccess || cudaMallocHost((void**)&c->h_flag, 64) != cudaSuccess) {
+        cudaGetLastError();
+        delete c;
+        return CRK_ENOMEM;
+    }
+    c->flag.cap = 64;
+    c->scratch_bytes = 64;
+    for (int e = 0; e < EV_N; ++e) cudaEventCreate(&c->ev[e]);
+    c->ev_ok = true;
+    *out = c;
+    return CRK_OK;
+}
+
+void crk_destroy(crk_ctx* c) {
+    if (!c) return;
+    cudaStreamSynchronize(c->stream);
+    DevBuf* bufs[] = {&c->keys[0], &c->keys[1], &c->vals[0], &c->vals[1], &c->hist, &c->scan_tmp, &c->posh_orig,
+                      &c->posh, &c->leaf_lo, &c->leaf_hi, &c->nbr_cnt, &c->nbr_off, &c->nbr_list, &c->nbr_gcnt,
+                      &c->posV, &c->rho_s, &c->coef, &c->velV, &c->thermo, &c->gv, &c->vel_orig, &c->m_s, &c->flag,
+                      &c->host_stage};
+    for (DevBuf* b : bufs)
+        if (b->p) cudaFree(b->p);
+    if (c->h_flag) cudaFreeHost(c->h_flag);
+    if (c->ev_ok)
+        for (int e = 0; e < EV_N; ++e) cudaEventDestroy(c->ev[e]);
+    delete c;
+}
+
+const char* crk_last_error(const crk_ctx* c) { return c ? c->err : "null context"; }
+
+int crk_build_cells(crk_ctx* c, int64_t n, const float* x, const float* y, const float* z, const float* h) {
+    if (!c) return CRK_EINVAL;
+    c->stage = 0;
+    if (n < 0 || n >= (int64_t)1 << 31 || (n > 0 && (!x || !y || !z || !h))) {
+        snprintf(c->err, sizeof(c->err), "crk_build_cells: null pointer or n out of range");
+        return CRK_EINVAL;
+    }
+    c->n = n;
+    c->nl = (n + CRK_LEAF - 1) / CRK_LEAF;
+    c->n_pairs = c->n_pairs_gather = 0;
+    if (n == 0) {
+        c->stage = 1;
+        return CRK_OK;
+    }
+    rec(c, EV_BUILD0);
+    CRK_TRY(crk_sort_particles(c, x, y, z, h));
+    rec(c, EV_SORTED);
+    CRK_TRY(crk_build_tree_and_list(c));
+    rec(c, EV_BUILD1);
+    c->stage = 1;
+    return CRK_OK;
+}
+
+int crk_volumes(crk_ctx* c, const float* m, float* V, float* rho, uint32_t* nbr_count) {
+    if (!c) return CRK_EINVAL;
+    if (c->stage < 1) {
+        snprintf(c->err, sizeof(c->err), "crk_volumes called before crk_build_cells");
+        return CRK_ESTATE;
+    }
+    if (c->n > 0 && !m) return CRK_EINVAL;
+    if (c->n > 0) {
+        rec(c, EV_VOL0);
+        CRK_TRY(crk_launch_volumes(c, m, V, rho, nbr_count));
+        rec(c, EV_VOL1);
+    }
+    c->stage = 2;
+    return CRK_OK;
+}
+
+int crk_rk_coefficients(crk_ctx* c, float* A, float* B, float* gradA, float* gradB) {
+    if (!c) return CRK_EINVAL;
+    if (c->stage < 2) {
+        snprintf(c->err, sizeof(c->err), "crk_rk_coefficients called before crk_volumes");
+        return CRK_ESTATE;
+    }
+    if (c->n > 0) {
+        rec(c, EV_RK0);
+        CRK_TRY(crk_launch_moments(c, A, B, gradA, gradB));
+        rec(c, EV_RK1);
+    }
+    c->stage = 3;
+    return CRK_OK;
+}
+
+int crk_hydro_derivs(crk_ctx* c, const float* vx, const float* vy, const float* vz, const float* u, float* ax,
+                     float* ay, float* az, float* dudt, uint32_t* pair_count) {
+    if (!c) return CRK_EINVAL;
+    if (c->stage < 3) {
+        snprintf(c->err, sizeof(c->err), "crk_hydro_derivs called before crk_rk_coefficients");
+        return CRK_ESTATE;
+    }
+    if (c->n > 0 && (!vx || !vy || !vz || !u || !ax || !ay || !az || !dudt)) return CRK_EINVAL;
+    if (c->n > 0) {
+        rec(c, EV_HY0);
+        CRK_TRY(crk_launch_hydro(c, vx, vy, vz, u, ax, ay, az, dudt, pair_count));
+    }
+    c->stage = 4;
+    return CRK_OK;
+}
+
+int crk_step_derivs(crk_ctx* c, int64_t n, const float* x, const float* y, const float* z, const float* h,
+                    const float* vx, const float* vy, const float* vz, const float* m, const float* u, float* ax,
+                    float* ay, float* az, float* dudt) {
+    CRK_TRY(crk_build_cells(c, n, x, y, z, h));
+    CRK_TRY(crk_volumes(c, m, nullptr, nullptr, nullptr));
+    CRK_TRY(crk_rk_coefficients(c, nullptr, nullptr, nullptr, nullptr));
+    return crk_hydro_derivs(c, vx, vy, vz, u, ax, ay, az, dudt, nullptr);
+}
+
+int crk_step_derivs_host(crk_ctx* c, int64_t n, const float* x, const float* y, const float* z, const float* h,
+                         const float* vx, const float* vy, const float* vz, const float* m, const float* u, float* ax,
+                         float* ay, float* az, float* dudt) {
+    if (!c || n < 0) return CRK_EINVAL;
+    if (n == 0) return crk_step_derivs(c, 0, x, y, z, h, vx, vy, vz, m, u, ax, ay, az, dudt);
+    if (!x || !y || !z || !h || !vx || !vy || !vz || !m || !u || !ax || !ay || !az || !dudt) return CRK_EINVAL;
+    const size_t stride = ((size_t)n + 63) & ~(size_t)63;
+    CRK_TRY(crk_ensure(c, c->host_stage, 13 * stride * sizeof(float)));
+    float* d = (float*)c->host_stage.p;
+    const float* in[9] = {x, y, z, h, vx, vy, vz, m, u};
+    for (int q = 0; q < 9; ++q)
+        CRK_CUDA(c, cudaMemcpyAsync(d + q * stride, in[q], (size_t)n * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    float* o = d + 9 * stride;
+    CRK_TRY(crk_step_derivs(c, n, d, d + stride, d + 2 * stride, d + 3 * stride, d + 4 * stride, d + 5 * stride,
+                            d + 6 * stride, d + 7 * stride, d + 8 * stride, o, o + stride, o + 2 * stride,
+                            o + 3 * stride));
+    float* out[4] = {ax, ay, az, dudt};
+    for (int q = 0; q < 4; ++q)
+        CRK_CUDA(c, cudaMemcpyAsync(out[q], o + q * stride, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+    CRK_CUDA(c, cudaStreamSynchronize(c->stream));
+    return CRK_OK;
+}
+
+int crk_get_perm(crk_ctx* c, int32_t* perm) {
+    if (!c || !perm) return CRK_EINVAL;
+    if (c->stage < 1) return CRK_ESTATE;
+    if (c->n == 0) return CRK_OK;
+    CRK_CUDA(c, cudaMemcpyAsync(perm, c->perm, (size_t)c->n * sizeof(int32_t), cudaMemcpyDeviceToDevice, c->stream));
+    return CRK_OK;
+}
+
+__global__ void k_scatter_gradv(const float4* __restrict__ gv, const int32_t* __restrict__ perm, int64_t n, int64_t np,
+                                float* __restrict__ out) {
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const float4 a = gv[k], b = gv[np + k], cc = gv[2 * np + k];
+    const int32_t p = perm[k];
+    const float g[9] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w, cc.x};
+#pragma unroll
+    for (int q = 0; q < 9; ++q) out[q * n + p] = g[q];
+}
+
+int crk_get_gradv(crk_ctx* c, float* gradv) {
+    if (!c || !gradv) return CRK_EINVAL;
+    if (c->stage < 4) return CRK_ESTATE;
+    if (c->n == 0) return CRK_OK;
+    k_scatter_gradv<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>((const float4*)c->gv.p, c->perm, c->n,
+                                                                           c->nl * CRK_LEAF, gradv);
+    return crk_check_launch(c, "k_scatter_gradv");
+}
+
+int crk_set_timing(crk_ctx* c, int on) {
+    if (!c) return CRK_EINVAL;
+    c->timing = on ? 1 : 0;
+    return CRK_OK;
+}
+
+int crk_reset_stats(crk_ctx* c) {
+    if (!c) return CRK_EINVAL;
+    c->launches = 0;
+    return CRK_OK;
+}
+
+int crk_get_stats(crk_ctx* c, crk_stats* out) {
+    if (!c || !out) return CRK_EINVAL;
+    memset(out, 0, sizeof(*out));
+    out->n = c->n;
+    out->n_leaves = c->nl;
+    out->n_leaf_pairs = c->n_pairs;
+    out->n_leaf_pairs_gather = c->n_pairs_gather;
+    out->launches = c->launches;
+    out->scratch_bytes = (int64_t)c->scratch_bytes;
+    if (c->timing && c->stage >= 4 && c->n > 0) {
+        CRK_CUDA(c, cudaStreamSynchronize(c->stream));
+        auto el = [&](int a, int b) {
+            float ms = 0.f;
+            if (cudaEventElapsedTime(&ms, c->ev[a], c->ev[b]) != cudaSuccess) { cudaGetLastError(); ms = -1.f; }
+            return ms;
+        };
+        out->ms_sort = el(EV_BUILD0, EV_SORTED);
+        out->ms_tree = el(EV_SORTED, EV_BUILD1);
+        out->ms_build = el(EV_BUILD0, EV_BUILD1);
+        out->ms_volumes = el(EV_VOL0, EV_VOL1);
+        out->ms_rk = el(EV_RK0, EV_RK1);
+        out->ms_hydro = el(EV_HY0, EV_F1);
+        out->ms_gradv = el(EV_GV0, EV_GV1);
+        out->ms_forces = el(EV_GV1, EV_F1);
+    }
+    return CRK_OK;
+}
+
+int64_t crk_get_leaf_list(crk_ctx* c, int64_t leaf, uint32_t* host_buf, int64_t cap) {
+    if (!c || leaf < 0) return CRK_EINVAL;
+    if (c->stage < 1) return CRK_ESTATE;
+    if (leaf >= c->nl) return CRK_EINVAL;
+    uint32_t o[2];
+    if (cudaMemcpyAsync(o, (uint32_t*)c->nbr_off.p + leaf, 2 * sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
+        return CRK_ECUDA;
+    cudaStreamSynchronize(c->stream);
+    const int64_t cnt = (int64_t)o[1] - (int64_t)o[0];
+    const int64_t ncopy = cnt < cap ? cnt : cap;
+    if (ncopy > 0 && host_buf) {
+        if (cudaMemcpyAsync(host_buf, (uint32_t*)c->nbr_list.p + o[0], (size_t)ncopy * sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
+            return CRK_ECUDA;
+        cudaStreamSynchronize(c->stream);
+    }
+    return cnt;
+}
+
+double crk_measure_fp32_peak(void* cuda_stream, int repeats, float* ms_out) {
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    int dev = 0, sms = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    float* d = nullptr;
+    if (cudaMalloc(&d, 64) != cudaSuccess) return -1.0;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    const int iters = 4096, threads = 256, blocks = sms * 8;
+    k_fp32_peak<<<blocks, threads, 0, s>>>(d, 64, 1.0001f, 0.5f);   // warm-up
+    float best = 1e30f;
+    if (repeats < 1) repeats = 1;
+    for (int r = 0; r < repeats; ++r) {
+        cudaEventRecord(e0, s);
+        k_fp32_peak<<<blocks, threads, 0, s>>>(d, iters, 1.0001f, 0.5f);
+        cudaEventRecord(e1, s);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        if (ms < best) best = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(d);
+    if (cudaGetLastError() != cudaSuccess) return -1.0;
+    if (ms_out) *ms_out = best;
+    const double flops = 2.0 * 8.0 * 16.0 * (double)iters * (double)threads * (double)blocks;
+    return flops / ((double)best * 1e-3);
+}
+
+}  // extern "C"

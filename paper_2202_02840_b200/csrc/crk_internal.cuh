@@ -1,0 +1,117 @@
+// crk_internal.cuh -- context, buffers and launch helpers shared by the translation units of libcrk.
+// Product code (CUDA, sm_100a).  Shares nothing with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+#include "../../include/crk.h"
+
+#define CRK_LEAF 32              // particles per leaf bucket = one warp lane per particle
+#define CRK_BVH_FAN 32           // children per node of the implicit wide tree over leaves
+#define CRK_MAX_LEVELS 8
+#define CRK_KEY_BITS 16          // space-filling-curve bits per dimension (48-bit keys)
+
+#define CRK_FLAG_GATHER 0x80000000u   // leaf-list entry: gap(a,b) < hmax(a)   (one-sided passes use it)
+#define CRK_FLAG_WRAP   0x40000000u   // leaf pair may straddle the periodic boundary
+#define CRK_LEAF_MASK   0x0fffffffu
+
+struct DevBuf {
+    void* p = nullptr;
+    size_t cap = 0;
+};
+
+struct crk_ctx {
+    crk_params prm;
+    cudaStream_t stream = 0;
+    int64_t n = 0, nl = 0;
+    int stage = 0;                 // 0 none, 1 built, 2 volumes, 3 coefficients, 4 hydro
+    char err[256];
+    int64_t launches = 0;
+    size_t scratch_bytes = 0;
+    int timing = 0;
+    cudaEvent_t ev[12];
+    bool ev_ok = false;
+    crk_stats st;
+
+    // sort
+    DevBuf keys[2], vals[2], hist, scan_tmp;
+    DevBuf posh_orig;              // float4 (x,y,z,h) in caller order
+    DevBuf posh;                   // float4 (x,y,z,h) in sorted order
+    int32_t* perm = nullptr;       // alias into vals[] after the sort
+    // leaves + tree
+    DevBuf leaf_lo, leaf_hi;       // float4 per node, all levels concatenated; lo.w = hmax of the subtree
+    int n_levels = 0;
+    int64_t level_off[CRK_MAX_LEVELS + 1];
+    int64_t level_cnt[CRK_MAX_LEVELS + 1];
+    DevBuf nbr_cnt, nbr_off, nbr_list, nbr_gcnt;
+    int64_t n_pairs = 0, n_pairs_gather = 0;
+    // per-particle state in sorted order
+    DevBuf posV;                   // float4 (x,y,z,V)
+    DevBuf rho_s;                  // float
+    DevBuf coef;                   // 4 planes float4[n]: (A,Bx,By,Bz) (cx,cy,cz,M00) (M01,M02,M10,M11) (M12,M20,M21,M22)
+    DevBuf velV;                   // float4 (vx,vy,vz,V)
+    DevBuf thermo;                 // float4 (P, rho, c_s, 1/h)
+    DevBuf gv;                     // 3 planes float4[n]: (g00,g01,g02,g10) (g11,g12,g20,g21) (g22, sigma/h^3, hhat, hhat^2 eps^2)
+    DevBuf vel_orig;               // float4 (vx,vy,vz,u) caller order (packed for a 16-byte gather)
+    DevBuf m_s;                    // float, sorted
+    DevBuf flag;                   // int[4] device error / status flags
+    DevBuf host_stage;             // device staging for crk_step_derivs_host (13 float arrays)
+    int* h_flag = nullptr;         // pinned host mirror
+};
+
+#define CRK_CUDA(c, call)                                                                          \
+    do {                                                                                           \
+        cudaError_t e__ = (call);                                                                  \
+        if (e__ != cudaSuccess) {                                                                  \
+            snprintf((c)->err, sizeof((c)->err), "%s:%d %s: %s", __FILE__, __LINE__, #call,        \
+                     cudaGetErrorString(e__));                                                     \
+            return CRK_ECUDA;                                                                      \
+        }                                                                                          \
+    } while (0)
+
+#define CRK_TRY(expr)                \
+    do {                             \
+        int rc__ = (expr);           \
+        if (rc__ != CRK_OK) return rc__; \
+    } while (0)
+
+static inline int crk_ensure(crk_ctx* c, DevBuf& b, size_t bytes) {
+    if (bytes <= b.cap && b.p) return CRK_OK;
+    if (b.p) {
+        cudaFree(b.p);
+        c->scratch_bytes -= b.cap;
+        b.p = nullptr;
+        b.cap = 0;
+    }
+    size_t want = bytes + bytes / 16 + 256;
+    cudaError_t e = cudaMalloc(&b.p, want);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        snprintf(c->err, sizeof(c->err), "cudaMalloc(%zu bytes) failed: %s", want, cudaGetErrorString(e));
+        b.p = nullptr;
+        return CRK_ENOMEM;
+    }
+    b.cap = want;
+    c->scratch_bytes += want;
+    return CRK_OK;
+}
+
+static inline int crk_check_launch(crk_ctx* c, const char* what) {
+    c->launches++;
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) {
+        snprintf(c->err, sizeof(c->err), "launch of %s failed: %s", what, cudaGetErrorString(e));
+        return CRK_ECUDA;
+    }
+    return CRK_OK;
+}
+
+// ---- translation-unit entry points (host side) ----
+int crk_sort_particles(crk_ctx* c, const float* x, const float* y, const float* z, const float* h);   // sort.cu
+int crk_exclusive_scan_u32(crk_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, DevBuf& tmp);    // sort.cu
+int crk_build_tree_and_list(crk_ctx* c);                                                               // tree.cu
+int crk_launch_volumes(crk_ctx* c, const float* m, float* V, float* rho, uint32_t* nbr_count);        // pairs.cu
+int crk_launch_moments(crk_ctx* c, float* A, float* B, float* gradA, float* gradB);                   // pairs.cu
+int crk_launch_hydro(crk_ctx* c, const float* vx, const float* vy, const float* vz, const float* u,
+                     float* ax, float* ay, float* az, float* dudt, uint32_t* pair_count);             // pairs.cu

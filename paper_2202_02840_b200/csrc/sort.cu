@@ -1,0 +1,311 @@
+// sort.cu -- step a0 (first half): space-filling-curve keys, LSD radix sort, packed sorted state.
+//
+// PAPER.md:292 sorts particles into chaining-mesh bins and cuts RCB leaves of N_ppl particles; here the same
+// locality is obtained by sorting on a 48-bit Hilbert key (16 bits per axis) and cutting the sorted sequence into
+// contiguous 32-particle leaves (tree.cu).  HBM-bound: every kernel here streams keys/payload once per pass.
+#include "crk_internal.cuh"
+
+namespace {
+
+constexpr int SORT_THREADS = 256;
+constexpr int SORT_ROUNDS = 16;                       // keys per lane
+constexpr int SORT_TILE = SORT_THREADS * SORT_ROUNDS; // 4096 keys per block
+constexpr int SORT_WARPS = SORT_THREADS / 32;
+constexpr int RADIX_BITS = 8;
+constexpr int RADIX = 1 << RADIX_BITS;
+
+// ---- 3-D Hilbert index (Skilling's transpose form), 16 bits per axis -> 48-bit key --------------------------
+__device__ __forceinline__ uint64_t spread3(uint32_t v) {
+    uint64_t x = v & 0x1fffffu;
+    x = (x | x << 32) & 0x1f00000000ffffull;
+    x = (x | x << 16) & 0x1f0000ff0000ffull;
+    x = (x | x << 8) & 0x100f00f00f00f00full;
+    x = (x | x << 4) & 0x10c30c30c30c30c3ull;
+    x = (x | x << 2) & 0x1249249249249249ull;
+    return x;
+}
+
+__device__ __forceinline__ uint64_t hilbert_key(uint32_t X0, uint32_t X1, uint32_t X2) {
+    const uint32_t M = 1u << (CRK_KEY_BITS - 1);
+#pragma unroll
+    for (uint32_t Q = M; Q > 1; Q >>= 1) {
+        const uint32_t P = Q - 1;
+        // axis 0
+        if (X0 & Q) X0 ^= P;
+        // axis 1
+        if (X1 & Q) X0 ^= P;
+        else { uint32_t t = (X0 ^ X1) & P; X0 ^= t; X1 ^= t; }
+        // axis 2
+        if (X2 & Q) X0 ^= P;
+        else { uint32_t t = (X0 ^ X2) & P; X0 ^= t; X2 ^= t; }
+    }
+    X1 ^= X0;
+    X2 ^= X1;
+    uint32_t t = 0;
+#pragma unroll
+    for (uint32_t Q = M; Q > 1; Q >>= 1)
+        if (X2 & Q) t ^= Q - 1;
+    X0 ^= t; X1 ^= t; X2 ^= t;
+    return (spread3(X0) << 2) | (spread3(X1) << 1) | spread3(X2);
+}
+
+// validate (S13), key, and pack (x,y,z,h) so the later permutation gather moves 16-byte words
+__global__ void __launch_bounds__(256) k_keys_pack(const float* __restrict__ x, const float* __restrict__ y,
+                                                   const float* __restrict__ z, const float* __restrict__ h,
+                                                   int64_t n, float L, uint64_t* __restrict__ keys,
+                                                   uint32_t* __restrict__ vals, float4* __restrict__ posh_orig,
+                                                   int* __restrict__ flag) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float xi = x[i], yi = y[i], zi = z[i], hi = h[i];
+    const bool ok = (xi >= 0.f) && (xi < L) && (yi >= 0.f) && (yi < L) && (zi >= 0.f) && (zi < L) && (hi > 0.f) &&
+                    (hi < 0.5f * L);
+    if (!ok) atomicOr(flag, 1);
+    const float s = (float)(1u << CRK_KEY_BITS) / L;
+    const uint32_t cmax = (1u << CRK_KEY_BITS) - 1u;
+    const uint32_t ix = min((uint32_t)fmaxf(xi * s, 0.f), cmax);
+    const uint32_t iy = min((uint32_t)fmaxf(yi * s, 0.f), cmax);
+    const uint32_t iz = min((uint32_t)fmaxf(zi * s, 0.f), cmax);
+    keys[i] = hilbert_key(ix, iy, iz);
+    vals[i] = (uint32_t)i;
+    posh_orig[i] = make_float4(xi, yi, zi, hi);
+}
+
+// per-tile digit histogram, stored digit-major so that one exclusive scan yields global stable offsets
+__global__ void __launch_bounds__(SORT_THREADS) k_radix_hist(const uint64_t* __restrict__ keys, int64_t n, int shift,
+                                                             uint32_t* __restrict__ hist, int nblk) {
+    __shared__ uint32_t cnt[RADIX];
+    cnt[threadIdx.x] = 0;
+    __syncthreads();
+    const int64_t base = (int64_t)blockIdx.x * SORT_TILE;
+#pragma unroll
+    for (int r = 0; r < SORT_ROUNDS; ++r) {
+        const int64_t idx = base + r * SORT_THREADS + threadIdx.x;
+        if (idx < n) atomicAdd(&cnt[(uint32_t)(keys[idx] >> shift) & (RADIX - 1)], 1u);
+    }
+    __syncthreads();
+    hist[(int64_t)threadIdx.x * nblk + blockIdx.x] = cnt[threadIdx.x];
+}
+
+// stable scatter: each warp owns 512 consecutive keys (16 rounds of 32), ranks them with match_any
+__global__ void __launch_bounds__(SORT_THREADS) k_radix_scatter(const uint64_t* __restrict__ keys_in,
+                                                                const uint32_t* __restrict__ vals_in,
+                                                                uint64_t* __restrict__ keys_out,
+                                                                uint32_t* __restrict__ vals_out, int64_t n, int shift,
+                                                                const uint32_t* __restrict__ offs, int nblk) {
+    __shared__ uint32_t wcnt[SORT_WARPS][RADIX];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    for (int q = threadIdx.x; q < SORT_WARPS * RADIX; q += SORT_THREADS) (&wcnt[0][0])[q] = 0;
+    __syncthreads();
+    const int64_t wbase = (int64_t)blockIdx.x * SORT_TILE + (int64_t)w * (32 * SORT_ROUNDS);
+    uint64_t k[SORT_ROUNDS];
+    uint32_t v[SORT_ROUNDS];
+    uint32_t rk[SORT_ROUNDS];
+    const uint32_t lt = (1u << lane) - 1u;
+#pragma unroll
+    for (int r = 0; r < SORT_ROUNDS; ++r) {
+        const int64_t idx = wbase + r * 32 + lane;
+        const bool valid = idx < n;
+        k[r] = valid ? keys_in[idx] : 0ull;
+        v[r] = valid ? vals_in[idx] : 0u;
+        const uint32_t d = valid ? ((uint32_t)(k[r] >> shift) & (RADIX - 1)) : (uint32_t)RADIX;
+        const uint32_t peers = __match_any_sync(0xffffffffu, d);
+        const uint32_t rank = __popc(peers & lt);
+        uint32_t prev = 0;
+        if (valid) prev = wcnt[w][d];
+        __syncwarp();
+        if (valid && rank == 0) wcnt[w][d] = prev + __popc(peers);
+        __syncwarp();
+        rk[r] = prev + rank;
+    }
+    __syncthreads();
+    {
+        const int d = threadIdx.x;   // 256 threads <-> 256 digits
+        uint32_t run = offs[(int64_t)d * nblk + blockIdx.x];
+#pragma unroll
+        for (int ww = 0; ww < SORT_WARPS; ++ww) {
+            const uint32_t cc = wcnt[ww][d];
+            wcnt[ww][d] = run;
+            run += cc;
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < SORT_ROUNDS; ++r) {
+        const int64_t idx = wbase + r * 32 + lane;
+        if (idx < n) {
+            const uint32_t d = (uint32_t)(k[r] >> shift) & (RADIX - 1);
+            const uint32_t pos = wcnt[w][d] + rk[r];
+            keys_out[pos] = k[r];
+            vals_out[pos] = v[r];
+        }
+    }
+}
+
+// ---- exclusive scan (u32), out has n+1 entries, out[n] = total ------------------------------------------------
+constexpr int SCAN_THREADS = 256;
+constexpr int SCAN_ITEMS = 8;
+constexpr int SCAN_TILE = SCAN_THREADS * SCAN_ITEMS;
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_block(const uint32_t* __restrict__ in, uint32_t* __restrict__ out,
+                                                             int64_t n_in, int64_t n_out, uint32_t* __restrict__ sums) {
+    __shared__ uint32_t wsum[SCAN_THREADS / 32];
+    const int64_t base = (int64_t)blockIdx.x * SCAN_TILE + (int64_t)threadIdx.x * SCAN_ITEMS;
+    uint32_t v[SCAN_ITEMS];
+    uint32_t tot = 0;
+#pragma unroll
+    for (int q = 0; q < SCAN_ITEMS; ++q) {
+        const int64_t i = base + q;
+        v[q] = (i < n_in) ? in[i] : 0u;
+        tot += v[q];
+    }
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    uint32_t inc = tot;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) wsum[w] = inc;
+    __syncthreads();
+    uint32_t woff = 0;
+    for (int q = 0; q < w; ++q) woff += wsum[q];
+    uint32_t run = woff + inc - tot;
+#pragma unroll
+    for (int q = 0; q < SCAN_ITEMS; ++q) {
+        const int64_t i = base + q;
+        if (i < n_out) out[i] = run;
+        run += v[q];
+    }
+    if (threadIdx.x == SCAN_THREADS - 1 && sums) sums[blockIdx.x] = woff + inc;
+}
+
+__global__ void __launch_bounds__(SCAN_THREADS) k_scan_add(uint32_t* __restrict__ out, int64_t n_out,
+                                                           const uint32_t* __restrict__ sums_scanned) {
+    const uint32_t add = sums_scanned[blockIdx.x];
+    const int64_t base = (int64_t)blockIdx.x * SCAN_TILE;
+    for (int q = threadIdx.x; q < SCAN_TILE; q += SCAN_THREADS) {
+        const int64_t i = base + q;
+        if (i < n_out) out[i] += add;
+    }
+}
+
+int scan_rec(crk_ctx* c, const uint32_t* in, uint32_t* out, int64_t n_in, int64_t n_out, uint32_t* tmp) {
+    const int64_t nblk = (n_out + SCAN_TILE - 1) / SCAN_TILE;
+    if (nblk <= 1) {
+        k_scan_block<<<1, SCAN_THREADS, 0, c->stream>>>(in, out, n_in, n_out, nullptr);
+        return crk_check_launch(c, "k_scan_block");
+    }
+    uint32_t* sums = tmp;
+    uint32_t* sums_scanned = tmp + nblk;                 // nblk + 1 entries
+    k_scan_block<<<(unsigned)nblk, SCAN_THREADS, 0, c->stream>>>(in, out, n_in, n_out, sums);
+    CRK_TRY(crk_check_launch(c, "k_scan_block"));
+    CRK_TRY(scan_rec(c, sums, sums_scanned, nblk, nblk + 1, sums_scanned + nblk + 1));
+    k_scan_add<<<(unsigned)nblk, SCAN_THREADS, 0, c->stream>>>(out, n_out, sums_scanned);
+    return crk_check_launch(c, "k_scan_add");
+}
+
+// sorted (x,y,z,h) by a 16-byte gather through the permutation, and the leaf bounding boxes in the same pass
+__global__ void __launch_bounds__(256) k_gather_leaves(const float4* __restrict__ posh_orig,
+                                                       const uint32_t* __restrict__ perm, int64_t n, int64_t nl,
+                                                       float4* __restrict__ posh, float4* __restrict__ leaf_lo,
+                                                       float4* __restrict__ leaf_hi) {
+    const int lane = threadIdx.x & 31;
+    const int64_t leaf = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (leaf >= nl) return;
+    const int64_t k = leaf * CRK_LEAF + lane;
+    const float inf = __int_as_float(0x7f800000);
+    float4 lo = make_float4(inf, inf, inf, 0.f), hi = make_float4(-inf, -inf, -inf, inf);
+    if (k < n) {
+        const float4 p = posh_orig[perm[k]];
+        posh[k] = p;
+        lo = make_float4(p.x, p.y, p.z, p.w);
+        hi = make_float4(p.x, p.y, p.z, p.w);
+    } else {
+        posh[k] = make_float4(3.0e30f, 3.0e30f, 3.0e30f, 0.0f);   // padding lanes of the last leaf: never a neighbour
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        lo.x = fminf(lo.x, __shfl_xor_sync(0xffffffffu, lo.x, o));
+        lo.y = fminf(lo.y, __shfl_xor_sync(0xffffffffu, lo.y, o));
+        lo.z = fminf(lo.z, __shfl_xor_sync(0xffffffffu, lo.z, o));
+        lo.w = fmaxf(lo.w, __shfl_xor_sync(0xffffffffu, lo.w, o));   // hmax
+        hi.x = fmaxf(hi.x, __shfl_xor_sync(0xffffffffu, hi.x, o));
+        hi.y = fmaxf(hi.y, __shfl_xor_sync(0xffffffffu, hi.y, o));
+        hi.z = fmaxf(hi.z, __shfl_xor_sync(0xffffffffu, hi.z, o));
+        hi.w = fminf(hi.w, __shfl_xor_sync(0xffffffffu, hi.w, o));   // hmin
+    }
+    if (lane == 0) {
+        leaf_lo[leaf] = lo;
+        leaf_hi[leaf] = hi;
+    }
+}
+
+}  // namespace
+
+int crk_exclusive_scan_u32(crk_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, DevBuf& tmp) {
+    // scratch: sum over levels of (2*nblk + 2)
+    size_t need = 0;
+    for (int64_t m = n + 1; m > 1;) {
+        const int64_t nblk = (m + SCAN_TILE - 1) / SCAN_TILE;
+        need += (size_t)(2 * nblk + 2);
+        if (nblk <= 1) break;
+        m = nblk + 1;
+    }
+    CRK_TRY(crk_ensure(c, tmp, need * sizeof(uint32_t) + 64));
+    return scan_rec(c, in, out, n, n + 1, (uint32_t*)tmp.p);
+}
+
+int crk_sort_particles(crk_ctx* c, const float* x, const float* y, const float* z, const float* h) {
+    const int64_t n = c->n;
+    const int64_t nl = c->nl;
+    for (int q = 0; q < 2; ++q) {
+        CRK_TRY(crk_ensure(c, c->keys[q], (size_t)n * sizeof(uint64_t)));
+        CRK_TRY(crk_ensure(c, c->vals[q], (size_t)n * sizeof(uint32_t)));
+    }
+    CRK_TRY(crk_ensure(c, c->posh_orig, (size_t)n * sizeof(float4)));
+    CRK_TRY(crk_ensure(c, c->posh, (size_t)nl * CRK_LEAF * sizeof(float4)));
+    const int nblk = (int)((n + SORT_TILE - 1) / SORT_TILE);
+    CRK_TRY(crk_ensure(c, c->hist, ((size_t)RADIX * nblk + 1) * 2 * sizeof(uint32_t)));
+    uint32_t* hist = (uint32_t*)c->hist.p;
+    uint32_t* offs = hist + (size_t)RADIX * nblk + 1;
+
+    CRK_CUDA(c, cudaMemsetAsync(c->flag.p, 0, 4 * sizeof(int), c->stream));
+    k_keys_pack<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(x, y, z, h, n, c->prm.box, (uint64_t*)c->keys[0].p,
+                                                                    (uint32_t*)c->vals[0].p, (float4*)c->posh_orig.p,
+                                                                    (int*)c->flag.p);
+    CRK_TRY(crk_check_launch(c, "k_keys_pack"));
+    int cur = 0;
+    for (int shift = 0; shift < 3 * CRK_KEY_BITS; shift += RADIX_BITS) {
+        k_radix_hist<<<nblk, SORT_THREADS, 0, c->stream>>>((const uint64_t*)c->keys[cur].p, n, shift, hist, nblk);
+        CRK_TRY(crk_check_launch(c, "k_radix_hist"));
+        CRK_TRY(crk_exclusive_scan_u32(c, hist, offs, (int64_t)RADIX * nblk, c->scan_tmp));
+        k_radix_scatter<<<nblk, SORT_THREADS, 0, c->stream>>>((const uint64_t*)c->keys[cur].p,
+                                                              (const uint32_t*)c->vals[cur].p,
+                                                              (uint64_t*)c->keys[cur ^ 1].p,
+                                                              (uint32_t*)c->vals[cur ^ 1].p, n, shift, offs, nblk);
+        CRK_TRY(crk_check_launch(c, "k_radix_scatter"));
+        cur ^= 1;
+    }
+    c->perm = (int32_t*)c->vals[cur].p;
+
+    // leaves (level 0 of the tree) are written by the gather; tree.cu sizes the node arrays
+    int64_t total = 0, cnt = nl;
+    int lev = 0;
+    while (true) {
+        c->level_off[lev] = total;
+        c->level_cnt[lev] = cnt;
+        total += cnt;
+        if (cnt <= CRK_BVH_FAN || lev + 1 >= CRK_MAX_LEVELS) break;
+        cnt = (cnt + CRK_BVH_FAN - 1) / CRK_BVH_FAN;
+        ++lev;
+    }
+    c->n_levels = lev + 1;
+    CRK_TRY(crk_ensure(c, c->leaf_lo, (size_t)total * sizeof(float4)));
+    CRK_TRY(crk_ensure(c, c->leaf_hi, (size_t)total * sizeof(float4)));
+    const int wpb = 8;
+    k_gather_leaves<<<(unsigned)((nl + wpb - 1) / wpb), wpb * 32, 0, c->stream>>>(
+        (const float4*)c->posh_orig.p, (const uint32_t*)c->perm, n, nl, (float4*)c->posh.p, (float4*)c->leaf_lo.p,
+        (float4*)c->leaf_hi.p);
+    return crk_check_launch(c, "k_gather_leaves");
+}

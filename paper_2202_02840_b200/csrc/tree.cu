@@ -1,0 +1,177 @@
+// tree.cu -- step a0 (second half): implicit 32-ary tree over the sorted leaves and the leaf interaction list.
+//
+// "leaf metadata includes a baryon interaction domain, calculated by extending the bounding box to
+// enclose the maximal smoothing length of the particles within the leaf ... all hydro operators utilize the same
+// interaction list, which need only be assembled once per hydro subcycle, and reused for each kernel."
+// Here the list of leaf a holds every leaf b whose periodic box-to-box gap is below max(hmax(a), hmax(b)); a flag
+// marks the entries that also satisfy the one-sided criterion gap < hmax(a) used by the gather passes.
+// The gap is evaluated with the same float operation sequence as the particle predicate (S3), so by
+// monotonicity of IEEE rounding the list is an exact superset of the interacting particle pairs.
+#include "crk_internal.cuh"
+
+namespace {
+
+struct Levels {
+    int n_levels;
+    int64_t off[CRK_MAX_LEVELS + 1];
+    int64_t cnt[CRK_MAX_LEVELS + 1];
+};
+
+__global__ void __launch_bounds__(256) k_tree_level(float4* __restrict__ lo, float4* __restrict__ hi, int64_t in_off,
+                                                    int64_t in_cnt, int64_t out_off, int64_t out_cnt) {
+    const int lane = threadIdx.x & 31;
+    const int64_t node = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (node >= out_cnt) return;
+    const int64_t ch = node * CRK_BVH_FAN + lane;
+    const float inf = __int_as_float(0x7f800000);
+    float4 a = make_float4(inf, inf, inf, 0.f), b = make_float4(-inf, -inf, -inf, inf);
+    if (ch < in_cnt) {
+        a = lo[in_off + ch];
+        b = hi[in_off + ch];
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a.x = fminf(a.x, __shfl_xor_sync(0xffffffffu, a.x, o));
+        a.y = fminf(a.y, __shfl_xor_sync(0xffffffffu, a.y, o));
+        a.z = fminf(a.z, __shfl_xor_sync(0xffffffffu, a.z, o));
+        a.w = fmaxf(a.w, __shfl_xor_sync(0xffffffffu, a.w, o));
+        b.x = fmaxf(b.x, __shfl_xor_sync(0xffffffffu, b.x, o));
+        b.y = fmaxf(b.y, __shfl_xor_sync(0xffffffffu, b.y, o));
+        b.z = fmaxf(b.z, __shfl_xor_sync(0xffffffffu, b.z, o));
+        b.w = fminf(b.w, __shfl_xor_sync(0xffffffffu, b.w, o));
+    }
+    if (lane == 0) {
+        lo[out_off + node] = a;
+        hi[out_off + node] = b;
+    }
+}
+
+// lower bound of |wrap(x_i - x_j)| on one axis for x_i in [qlo,qhi], x_j in [blo,bhi]
+__device__ __forceinline__ float axis_gap(float qlo, float qhi, float blo, float bhi, float L, float half, bool& wrap) {
+    const float dmin = __fsub_rn(qlo, bhi);
+    const float dmax = __fsub_rn(qhi, blo);
+    wrap = wrap || (dmin < -half) || (dmax > half);
+    const float g0 = fmaxf(0.f, fmaxf(dmin, -dmax));
+    const float gp = fmaxf(0.f, fmaxf(__fsub_rn(L, dmax), __fsub_rn(dmin, L)));
+    const float gm = fmaxf(0.f, fmaxf(__fadd_rn(dmin, L), __fsub_rn(-L, dmax)));
+    return fminf(g0, fminf(gp, gm));
+}
+
+constexpr int NBR_WARPS = 8;
+constexpr int NBR_STACK = 32 * (CRK_MAX_LEVELS + 1);
+
+template <bool FILL>
+__global__ void __launch_bounds__(NBR_WARPS * 32) k_leaf_list(const float4* __restrict__ lo, const float4* __restrict__ hi,
+                                                              Levels lv, float L, uint32_t* __restrict__ cnt,
+                                                              uint32_t* __restrict__ gcnt,
+                                                              const uint32_t* __restrict__ off,
+                                                              uint32_t* __restrict__ list) {
+    __shared__ uint32_t stack[NBR_WARPS][NBR_STACK];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int64_t q = (int64_t)blockIdx.x * NBR_WARPS + w;
+    if (q >= lv.cnt[0]) return;
+    const float4 qlo = lo[q], qhi = hi[q];
+    const float hq2 = __fmul_rn(qlo.w, qlo.w);
+    const float half = 0.5f * L;
+    const uint32_t lt = (1u << lane) - 1u;
+    uint32_t n_out = 0, n_gather = 0;
+    const uint32_t base = FILL ? off[q] : 0u;
+    int sp = 0;
+    if (lane == 0) stack[w][0] = ((uint32_t)lv.n_levels << 28);   // pseudo-root: children = all nodes of the top level
+    sp = 1;
+    __syncwarp();
+    while (sp > 0) {
+        const uint32_t e = stack[w][sp - 1];
+        --sp;
+        __syncwarp();
+        const int clev = (int)(e >> 28) - 1;
+        const int64_t child = (int64_t)(e & CRK_LEAF_MASK) * CRK_BVH_FAN + lane;
+        bool pass = false, gather = false, wrap = false;
+        if (child < lv.cnt[clev]) {
+            const float4 blo = lo[lv.off[clev] + child], bhi = hi[lv.off[clev] + child];
+            const float gx = axis_gap(qlo.x, qhi.x, blo.x, bhi.x, L, half, wrap);
+            const float gy = axis_gap(qlo.y, qhi.y, blo.y, bhi.y, L, half, wrap);
+            const float gz = axis_gap(qlo.z, qhi.z, blo.z, bhi.z, L, half, wrap);
+            const float g2 = __fmaf_rn(gz, gz, __fmaf_rn(gy, gy, __fmul_rn(gx, gx)));
+            const float hb2 = __fmul_rn(blo.w, blo.w);
+            gather = g2 < hq2;
+            pass = g2 < fmaxf(hq2, hb2);
+        }
+        const uint32_t m = __ballot_sync(0xffffffffu, pass);
+        if (clev == 0) {
+            const uint32_t mg = __ballot_sync(0xffffffffu, gather);
+            if (FILL && pass) {
+                const uint32_t pos = base + n_out + __popc(m & lt);
+                list[pos] = (uint32_t)child | (gather ? CRK_FLAG_GATHER : 0u) | (wrap ? CRK_FLAG_WRAP : 0u);
+            }
+            n_out += __popc(m);
+            n_gather += __popc(mg);
+        } else {
+            // push in descending order so that the lowest child is popped first (list comes out ascending)
+            if (pass) stack[w][sp + __popc(m & ~lt & ~(1u << lane))] = ((uint32_t)clev << 28) | (uint32_t)child;
+            sp += __popc(m);
+            __syncwarp();
+        }
+    }
+    if (!FILL && lane == 0) {
+        cnt[q] = n_out;
+        gcnt[q] = n_gather;
+    }
+}
+
+__global__ void k_sum_u32(const uint32_t* __restrict__ a, int64_t n, unsigned long long* __restrict__ out) {
+    unsigned long long s = 0;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) s += a[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+    if ((threadIdx.x & 31) == 0) atomicAdd(out, s);
+}
+
+}  // namespace
+
+int crk_build_tree_and_list(crk_ctx* c) {
+    float4* lo = (float4*)c->leaf_lo.p;
+    float4* hi = (float4*)c->leaf_hi.p;
+    Levels lv;
+    lv.n_levels = c->n_levels;
+    for (int l = 0; l <= CRK_MAX_LEVELS; ++l) {
+        lv.off[l] = l < c->n_levels ? c->level_off[l] : 0;
+        lv.cnt[l] = l < c->n_levels ? c->level_cnt[l] : 0;
+    }
+    for (int l = 1; l < c->n_levels; ++l) {
+        const int wpb = 8;
+        k_tree_level<<<(unsigned)((lv.cnt[l] + wpb - 1) / wpb), wpb * 32, 0, c->stream>>>(lo, hi, lv.off[l - 1],
+                                                                                          lv.cnt[l - 1], lv.off[l],
+                                                                                          lv.cnt[l]);
+        CRK_TRY(crk_check_launch(c, "k_tree_level"));
+    }
+    const int64_t nl = c->nl;
+    CRK_TRY(crk_ensure(c, c->nbr_cnt, (size_t)(nl + 1) * sizeof(uint32_t)));
+    CRK_TRY(crk_ensure(c, c->nbr_gcnt, (size_t)(nl + 1) * sizeof(uint32_t)));
+    CRK_TRY(crk_ensure(c, c->nbr_off, (size_t)(nl + 2) * sizeof(uint32_t)));
+    const unsigned grid = (unsigned)((nl + NBR_WARPS - 1) / NBR_WARPS);
+    k_leaf_list<false><<<grid, NBR_WARPS * 32, 0, c->stream>>>(lo, hi, lv, c->prm.box, (uint32_t*)c->nbr_cnt.p,
+                                                               (uint32_t*)c->nbr_gcnt.p, nullptr, nullptr);
+    CRK_TRY(crk_check_launch(c, "k_leaf_list<count>"));
+    CRK_TRY(crk_exclusive_scan_u32(c, (const uint32_t*)c->nbr_cnt.p, (uint32_t*)c->nbr_off.p, nl, c->scan_tmp));
+    // totals -> host (the one synchronisation of crk_build_cells): [1] = error flag, [2..3] = gather pair count
+    unsigned long long* d_sum = (unsigned long long*)((int*)c->flag.p + 2);
+    k_sum_u32<<<148, 256, 0, c->stream>>>((const uint32_t*)c->nbr_gcnt.p, nl, d_sum);
+    CRK_TRY(crk_check_launch(c, "k_sum_u32"));
+    CRK_CUDA(c, cudaMemcpyAsync(c->h_flag, c->flag.p, 4 * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CRK_CUDA(c, cudaMemcpyAsync(c->h_flag + 4, (uint32_t*)c->nbr_off.p + nl, sizeof(uint32_t), cudaMemcpyDeviceToHost,
+                                c->stream));
+    CRK_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (c->h_flag[0] & 1) {
+        snprintf(c->err, sizeof(c->err), "input out of range: need 0 <= x,y,z < box and 0 < h < box/2");
+        return CRK_ERANGE;
+    }
+    c->n_pairs = (int64_t)(uint32_t)c->h_flag[4];
+    unsigned long long g;
+    memcpy(&g, c->h_flag + 2, sizeof(g));
+    c->n_pairs_gather = (int64_t)g;
+    CRK_TRY(crk_ensure(c, c->nbr_list, (size_t)(c->n_pairs + 1) * sizeof(uint32_t)));
+    k_leaf_list<true><<<grid, NBR_WARPS * 32, 0, c->stream>>>(lo, hi, lv, c->prm.box, nullptr, nullptr,
+                                                              (const uint32_t*)c->nbr_off.p, (uint32_t*)c->nbr_list.p);
+    return crk_check_launch(c, "k_leaf_list<fill>");
+}

@@ -1,0 +1,285 @@
+"""GPU parity: the CUDA library (through its C ABI / thin binding) against the FP64 CPU oracle, element by element,
+on identical seeded inputs.  Bars (BASELINE.json north_star):
+  * neighbour counts / pair counts: bit-exact
+  * V, rho, A: <= 2e-6 relative;  B, grad A, grad B: <= 1e-4 relative L2 (normalised by rms)
+  * dv/dt, du/dt: <= 1e-4 relative L2 (normalised by rms); conservation invariants <= 1e-5
+Run with `pytest -m gpu` on a B200.
+"""
+import numpy as np
+import pytest
+
+import crk_workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+TOL_DERIV = 1e-4
+TOL_INV = 1e-5
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+def rel_l2(a, b):
+    a = np.asarray(a, dtype=np.float64); b = np.asarray(b, dtype=np.float64)
+    return float(np.sqrt(((a - b) ** 2).sum() / max((b ** 2).sum(), 1e-300)))
+
+
+def gpu_eval(ps, stages=False):
+    """Evaluate the full path on the GPU through the binding; returns numpy arrays in caller order."""
+    torch = _torch()
+    from paper_2202_02840_b200 import Crk
+    dev = torch.device("cuda:0")
+    t = {k: torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).to(dev) for k in
+         ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")}
+    ctx = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h)
+    ctx.build_cells(t["x"], t["y"], t["z"], t["h"])
+    V, rho, cnt = ctx.volumes(t["m"])
+    A, B, gA, gB = ctx.rk_coefficients()
+    ax, ay, az, du, pc = ctx.hydro_derivs(t["vx"], t["vy"], t["vz"], t["u"])
+    gv = ctx.gradv()
+    perm = ctx.perm()
+    torch.cuda.synchronize()
+    out = dict(V=V, rho=rho, nbr_count=cnt, A=A, B=B, gradA=gA, gradB=gB, ax=ax, ay=ay, az=az, dudt=du,
+               pair_count=pc, gradv=gv, perm=perm)
+    out = {k: v.cpu().numpy() for k, v in out.items()}
+    out["stats"] = ctx.stats()
+    out["ctx"] = ctx
+    return out
+
+
+def check_parity(ps, g, o, oracle_gv=None, mask=None, label=""):
+    """g: GPU outputs, o: oracle outputs (dicts).  mask: compare only these particles (windowed oracle)."""
+    sel = slice(None) if mask is None else mask
+    assert np.array_equal(g["nbr_count"][sel].astype(np.int64), o["nbr_count"][sel].astype(np.int64)), label + " nbr_count"
+    assert np.array_equal(g["pair_count"][sel].astype(np.int64), o["pair_count"][sel].astype(np.int64)), label + " pair_count"
+    assert np.max(np.abs(g["V"][sel] / o["V"][sel] - 1)) < 2e-6, label + " V"
+    assert np.max(np.abs(g["rho"][sel] / o["rho"][sel] - 1)) < 2e-6, label + " rho"
+    assert np.max(np.abs(g["A"][sel] / o["A"][sel] - 1)) < 2e-5, label + " A"
+    for k in ("B", "gradA", "gradB"):
+        e = rel_l2(g[k][:, sel], o[k][:, sel])
+        assert e < TOL_DERIV, f"{label} {k} rel L2 {e:.3e}"
+    if oracle_gv is not None:
+        e = rel_l2(g["gradv"][:, sel], oracle_gv[:, sel])
+        assert e < TOL_DERIV, f"{label} gradv rel L2 {e:.3e}"
+    acc_g = np.stack([g["ax"][sel], g["ay"][sel], g["az"][sel]]); acc_o = np.stack([o["ax"][sel], o["ay"][sel], o["az"][sel]])
+    e_a = rel_l2(acc_g, acc_o)
+    e_u = rel_l2(g["dudt"][sel], o["dudt"][sel])
+    assert e_a < TOL_DERIV, f"{label} dv/dt rel L2 {e_a:.3e}"
+    assert e_u < TOL_DERIV, f"{label} du/dt rel L2 {e_u:.3e}"
+    return e_a, e_u
+
+
+def check_invariants(ps, g, label=""):
+    m = ps.m.astype(np.float64)
+    a = [g[k].astype(np.float64) for k in ("ax", "ay", "az")]
+    v = [ps.vx.astype(np.float64), ps.vy.astype(np.float64), ps.vz.astype(np.float64)]
+    mom = max(abs((m * a[q]).sum()) for q in range(3)) / (m * np.sqrt(a[0] ** 2 + a[1] ** 2 + a[2] ** 2)).sum()
+    du = g["dudt"].astype(np.float64)
+    work = m * (v[0] * a[0] + v[1] * a[1] + v[2] * a[2])
+    en = abs((work + m * du).sum()) / ((m * np.abs(du)).sum() + np.abs(work).sum() + 1e-300)
+    assert mom < TOL_INV, f"{label} momentum residual {mom:.3e}"
+    assert en < TOL_INV, f"{label} energy residual {en:.3e}"
+    return mom, en
+
+
+# ------------------------------------------------------------------------------------------------ structure
+def test_sort_tree_and_leaf_lists_cover_every_neighbour(oracle_mod):
+    ps = wl.clustered_plummer(n_side=20)
+    g = gpu_eval(ps)
+    n = ps.n
+    perm = g["perm"].astype(np.int64)
+    assert np.array_equal(np.sort(perm), np.arange(n)), "perm is not a permutation"
+    slot = np.empty(n, dtype=np.int64); slot[perm] = np.arange(n)
+    o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+    o.build(ps.x, ps.y, ps.z, ps.h)
+    ctx = g["ctx"]
+    st = g["stats"]
+    assert st["n_leaves"] == (n + 31) // 32
+    rng = np.random.default_rng(0)
+    for leaf in rng.integers(0, st["n_leaves"], 60):
+        lst = ctx.leaf_list(int(leaf))
+        ids = (lst & np.uint32(0x0fffffff)).astype(np.int64)
+        assert np.all(np.diff(ids) > 0), "leaf list not strictly ascending"
+        gather = set(ids[(lst >> np.uint32(31)) == 1].tolist()); allb = set(ids.tolist())
+        for k in range(leaf * 32, min(leaf * 32 + 32, n)):
+            js, fi, fj = o.neighbors(perm[k])
+            lj = slot[js.astype(np.int64)] // 32
+            assert set(lj.tolist()) <= allb, "a symmetric neighbour's leaf is missing from the list"
+            assert set(lj[fi].tolist()) <= gather, "a gather neighbour's leaf lacks the gather flag"
+
+
+# ------------------------------------------------------------------------------------------------ small configs
+@pytest.mark.parametrize("name,n_side", [("tiny_uniform", 16), ("blast_wave", 24), ("clustered", 24), ("cosmo", 32)])
+def test_parity_small(name, n_side, oracle_mod):
+    ps = wl.make_config(name, n_side)
+    o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+    od = o.step_derivs(ps)
+    g = gpu_eval(ps)
+    e_a, e_u = check_parity(ps, g, od, oracle_gv=o.gradv(), label=name)
+    mom, en = check_invariants(ps, g, label=name)
+    print(f"[parity] {name} n={ps.n}: dv/dt {e_a:.2e} du/dt {e_u:.2e} momentum {mom:.2e} energy {en:.2e}")
+
+
+def test_parity_ragged_sizes(oracle_mod):
+    """N not a multiple of the 32-particle leaf, including a single leaf and a single particle"""
+    base = wl.tiny_uniform(n_side=10)
+    for n in (1, 2, 31, 33, 257, 999):
+        ps = base.subset(np.arange(n))
+        ps.h = np.full(n, 0.2, np.float32)
+        o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+        od = o.step_derivs(ps)
+        g = gpu_eval(ps)
+        assert np.array_equal(g["nbr_count"].astype(np.int64), od["nbr_count"].astype(np.int64))
+        assert np.array_equal(g["pair_count"].astype(np.int64), od["pair_count"].astype(np.int64))
+        assert np.max(np.abs(g["V"] / od["V"] - 1)) < 2e-6
+        if n >= 257:
+            check_parity(ps, g, od, label=f"ragged{n}")
+
+
+def test_step_derivs_and_host_entry_match_staged_calls():
+    torch = _torch()
+    from paper_2202_02840_b200 import Crk
+    ps = wl.tiny_uniform()
+    g = gpu_eval(ps)
+    dev = torch.device("cuda:0")
+    names = ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")
+    t = [torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).to(dev) for k in names]
+    ctx = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h)
+    out = ctx.step_derivs(*t)
+    torch.cuda.synchronize()
+    for o, k in zip(out, ("ax", "ay", "az", "dudt")):
+        assert np.array_equal(o.cpu().numpy(), g[k]), k
+    th = [torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).pin_memory() for k in names]
+    oh = [torch.empty(ps.n).pin_memory() for _ in range(4)]
+    ctx.step_derivs_host(*th, oh)
+    for o, k in zip(oh, ("ax", "ay", "az", "dudt")):
+        assert np.array_equal(o.numpy(), g[k]), k
+    # determinism: a second evaluation gives identical bits
+    out2 = ctx.step_derivs(*t)
+    torch.cuda.synchronize()
+    for a, b in zip(out, out2):
+        assert torch.equal(a, b)
+
+
+def test_errors_and_empty_input():
+    torch = _torch()
+    from paper_2202_02840_b200 import Crk, CrkError
+    dev = torch.device("cuda:0")
+    ctx = Crk()
+    e = torch.empty(0, device=dev)
+    out = ctx.step_derivs(e, e, e, e, e, e, e, e, e)
+    assert all(o.numel() == 0 for o in out)
+    one = torch.full((4,), 0.5, device=dev)
+    with pytest.raises(CrkError) as ei:
+        ctx.build_cells(one, one, one, torch.full((4,), 0.5, device=dev))       # h >= L/2
+    assert ei.value.code == -2
+    with pytest.raises(CrkError) as ei:
+        ctx.build_cells(torch.full((4,), 1.0, device=dev), one, one, torch.full((4,), 0.1, device=dev))
+    assert ei.value.code == -2
+    ctx2 = Crk()
+    with pytest.raises(CrkError) as ei:
+        ctx2.volumes(one)
+    assert ei.value.code == -5
+    ctx2.build_cells(torch.rand(4, device=dev), torch.rand(4, device=dev), torch.rand(4, device=dev),
+                     torch.full((4,), 0.1, device=dev))
+    with pytest.raises(CrkError) as ei:
+        ctx2.hydro_derivs(one, one, one, one)
+    assert ei.value.code == -5
+
+
+# ------------------------------------------------------------------------------------------------ config 2 multi-step
+def test_blast_wave_teacher_forced_euler_steps(oracle_mod):
+    """BASELINE config 2 protocol at reduced size (S12): at each Euler step the GPU evaluates derivatives on the
+    oracle's FP32 state and must meet the bar; states come from oracle/crk_oracle.py:euler_steps (FP64 update)."""
+    ps = wl.blast_wave(n_side=24)
+    worst = 0.0
+    for step, cur, od in oracle_mod.euler_steps(ps, 6, 1e-4 * (64 / 24) ** 0 * 0.25):
+        g = gpu_eval(cur)
+        e_a, e_u = check_parity(cur, g, od, label=f"blast step {step}")
+        worst = max(worst, e_a, e_u)
+    print(f"[parity] blast teacher-forced worst rel L2 {worst:.2e}")
+
+
+# ------------------------------------------------------------------------------------------------ BASELINE sizes
+def _pick_window(ps, c, half, cap=120000):
+    """Padded window such that every quantity of the core particles is determined inside it: hop 1 = symmetric set
+    (r < max(h_i,h_j): a far particle with a large h_j can reach the core), hops 2-3 = gather sets of radius <= hmax."""
+    cc = np.asarray(c, dtype=np.float64)
+    off = np.zeros(ps.n)
+    for a_, k in enumerate(("x", "y", "z")):
+        d = getattr(ps, k).astype(np.float64) - cc[a_]
+        d -= np.round(d)
+        off = np.maximum(off, np.abs(d))
+    dist = np.maximum(off - half, 0.0)                     # Chebyshev distance to the core box (<= Euclidean)
+    h = ps.h.astype(np.float64)
+    core = off <= half
+    if not core.any():
+        return None
+    hc = h[core].max()
+    partners = dist < np.maximum(h, hc)                    # superset of the hop-1 partners of the core
+    r1 = dist[partners].max()
+    pad = r1 + 2.0 * h[partners].max()
+    for _ in range(8):
+        inside = off <= half + pad
+        need = r1 + 2.0 * h[inside & (dist <= r1 + h[inside].max())].max()
+        if need <= pad * (1 + 1e-9):
+            break
+        pad = need
+    inside = off <= half + pad
+    if inside.sum() > cap:
+        return None
+    idx = np.nonzero(inside)[0]
+    return idx, core[idx]
+
+
+def _window_check(ps, oracle_mod, centres, half_in_h=2.5, label=""):
+    """windowed brute force: the oracle gets every particle of a padded window; only
+    the un-padded core is compared."""
+    g = gpu_eval(ps)
+    check_invariants(ps, g, label=label)
+    done = 0
+    for c in centres:
+        idx0, _ = wl.select_window(ps, c, 0.03, 0.0)
+        if len(idx0) == 0:
+            continue
+        half = half_in_h * float(np.median(ps.h[idx0]))
+        win = _pick_window(ps, c, half)
+        if win is None:
+            print(f"[parity] {label} window@{np.round(c, 3)} skipped (too many particles in the padded window)")
+            continue
+        idxp, corep = win
+        sub = ps.subset(idxp)
+        o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+        od = o.step_derivs(sub)
+        gs = {k: (v[idxp] if v.ndim == 1 else v[:, idxp]) for k, v in g.items() if isinstance(v, np.ndarray) and k != "perm"}
+        e_a, e_u = check_parity(sub, gs, od, oracle_gv=o.gradv(), mask=corep, label=f"{label} window@{np.round(c, 3)}")
+        print(f"[parity] {label} window n={len(idxp)} core={int(corep.sum())}: dv/dt {e_a:.2e} du/dt {e_u:.2e}")
+        done += 1
+    assert done >= 1
+    return g
+
+
+def test_parity_config2_blast_full(oracle_mod):
+    ps = wl.make_config("blast_wave")
+    c = [(0.5, 0.5, 0.5), (0.1, 0.9, 0.3)]
+    _window_check(ps, oracle_mod, c, half_in_h=3.0, label="blast64")
+
+
+def test_parity_config3_clustered_full(oracle_mod):
+    ps = wl.make_config("clustered")
+    rng = np.random.default_rng(1)
+    dens = np.argsort(ps.h)[:3]                      # densest cores
+    centres = [(float(ps.x[i]), float(ps.y[i]), float(ps.z[i])) for i in dens] + [tuple(rng.random(3)) for _ in range(3)]
+    _window_check(ps, oracle_mod, centres, half_in_h=2.0, label="clustered128")
+
+
+def test_parity_config4_cosmo_full(oracle_mod):
+    ps = wl.make_config("cosmo")
+    centres = [(0.5, 0.5, 0.5), (0.001, 0.999, 0.5), (0.25, 0.75, 0.1)]
+    g = _window_check(ps, oracle_mod, centres, half_in_h=3.0, label="cosmo256")
+    st = g["stats"]
+    print(f"[stats] cosmo256 leaves={st['n_leaves']} leaf_pairs={st['n_leaf_pairs']} launches={st['launches']}")
