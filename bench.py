@@ -1,0 +1,287 @@
+#!/usr/bin/env python
+"""bench.py -- CRKSPH pair-interactions/s on one (or N independent) B200(s).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config cosmo] [--n-side 256] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (crk_step_derivs: sort + leaves + interaction list, volumes, RK moments +
+3x3 solve, grad v, momentum/energy) over one synthetic particle set (BASELINE.json configs[3]: 256^3 = 16.8 M
+Zel'dovich-displaced particles, recipe in DESIGN.md).  Prints ONE JSON line (contract in the task statement):
+  value     pair-interactions/s = accepted ordered pairs summed over the four sweeps / step time, inputs resident in HBM
+  e2e       the same through crk_step_derivs_host (pinned HOST buffers, H2D + D2H inside the timed region)
+  roofline  dominant kernel (k_forces, Eqs. 17-18) algorithmic FP32 flop rate against the FP32 FMA-pipe peak
+  cpu_baseline  the FP64 brute-force oracle, as it stands, on a bounded window of the same workload
+With --impl reference the oracle itself is the timed arm.  N > 1: one process per GPU, each with its own seeded box
+(weak scaling, no data-path collective); rank 0 prints the aggregate.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import crk_workloads as wl  # noqa: E402
+
+METRIC = "CRKSPH pair-interactions/sec"
+UNIT = "pair-interactions/s"
+# canonical algorithmic FP32 flops per accepted ordered pair (restated in DESIGN.md)
+FLOPS_PER_PAIR = {"volumes": 16.0, "moments": 100.0, "gradv": 90.0, "forces": 250.0}
+FP32_PEAK_THEORETICAL = 148 * 128 * 2 * 1.965e9     # SMs x FP32 lanes x 2 (FMA) x max SM clock
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0}, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region"""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons = [], None, set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.lines:
+            f = [t.strip() for t in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax = float(f[1])
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": smax, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_sample(ps, target_particles=30000):
+    """bounded window of the workload for the CPU oracle: a cube around the box centre holding ~target particles"""
+    half = 0.5 * (target_particles / ps.n) ** (1.0 / 3.0)
+    idx, _ = wl.select_window(ps, (0.5, 0.5, 0.5), half, 0.0)
+    return ps.subset(idx), half
+
+
+def time_oracle(sub):
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    import crk_oracle
+    o = crk_oracle.Oracle(sub.box, sub.gamma, sub.n_h)
+    t0 = time.perf_counter()
+    d = o.step_derivs(sub)
+    dt = time.perf_counter() - t0
+    pairs = 3.0 * float(d["nbr_count"].astype(np.int64).sum()) + float(d["pair_count"].astype(np.int64).sum())
+    return pairs, dt, crk_oracle.get_threads()
+
+
+def run_reference(args, rank, world):
+    """--impl reference: the oracle (oracle/crk_oracle.cpp, FP64 brute force) timed as it stands on the host cores,
+    each step a bounded window of the same workload."""
+    if rank != 0:
+        return
+    ps = wl.make_config(args.config, args.n_side)
+    sub, half = oracle_sample(ps, args.oracle_particles)
+    for _ in range(args.warmup if args.warmup < 2 else 1):
+        time_oracle(sub)
+    tot_pairs, tot_t, cores = 0.0, 0.0, 0
+    for _ in range(args.steps):
+        pairs, dt, cores = time_oracle(sub)
+        tot_pairs += pairs; tot_t += dt
+    value = tot_pairs / tot_t
+    sample = f"cube of half-width {half:.4f} at the box centre of {ps.name} n_side={ps.meta['n_side']}: {sub.n} particles, brute-force O(n^2) neighbours"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"{ps.name} n_side={ps.meta['n_side']} (bounded sample)", "particles": sub.n},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2202_02840_b200 import Crk, crk_measure_fp32_peak
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    # each rank owns an independent seeded box of the same recipe (weak scaling; the path has no exchange step on one box)
+    base_seed = {"tiny_uniform": 1001, "blast_wave": 1002, "clustered": 1003, "cosmo": 1004, "cosmo_large": 1005}[args.config]
+    ps = wl.make_config(args.config, args.n_side, seed=base_seed + 7919 * rank)
+    names = ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")
+    host = [torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).pin_memory() for k in names]
+    t = [h.to(dev, non_blocking=True) for h in host]
+    out = [torch.empty(ps.n, device=dev) for _ in range(4)]
+    ctx = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h)
+
+    # accepted ordered pairs per sweep (exact counts from the staged API, outside the timed region)
+    ctx.build_cells(*t[:4])
+    _, _, cnt = ctx.volumes(t[7])
+    ctx.rk_coefficients(want=False)
+    res = ctx.hydro_derivs(t[4], t[5], t[6], t[8])
+    gather_pairs = float(cnt.to(torch.int64).sum().item())
+    sym_pairs = float(res[4].to(torch.int64).sum().item())
+    pairs_per_step = 3.0 * gather_pairs + sym_pairs
+    del cnt, res
+
+    ctx.set_timing(True)
+    for _ in range(max(args.warmup, 3)):
+        ctx.step_derivs(*t, out=out)
+    torch.cuda.synchronize()
+    ctx.reset_stats()
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.25)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        ctx.step_derivs(*t, out=out)
+    e1.record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    ms = e0.elapsed_time(e1)
+    st = ctx.stats()
+    clocks = sampler.stop() if rank == 0 else None
+    launches = st["launches"]
+
+    # end to end through the host-pointer C ABI entry (pinned host inputs -> device -> compute -> host outputs)
+    oh = [torch.empty(ps.n).pin_memory() for _ in range(4)]
+    ctx.set_timing(False)
+    ctx.step_derivs_host(*host, oh)
+    torch.cuda.synchronize()
+    k2 = max(1, min(args.steps, 5))
+    t0 = time.perf_counter()
+    for _ in range(k2):
+        ctx.step_derivs_host(*host, oh)
+    torch.cuda.synchronize()
+    e2e_ms = 1e3 * (time.perf_counter() - t0) / k2
+
+    tot = torch.tensor([ms, e2e_ms], device=dev, dtype=torch.float64)
+    work = torch.tensor([pairs_per_step, float(ps.n)], device=dev, dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(tot, op=dist.ReduceOp.MAX)
+        dist.all_reduce(work, op=dist.ReduceOp.SUM)
+    ms_all, e2e_all = float(tot[0]), float(tot[1])
+    pairs_all, n_all = float(work[0]), float(work[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    ms_per_step = ms_all / args.steps
+    value = pairs_all / (ms_per_step * 1e-3)
+    peaks, peak_kind = load_peaks()
+    fp32_meas, _ = crk_measure_fp32_peak(5)
+    forces_ms = st["ms_forces"]
+    forces_flops = FLOPS_PER_PAIR["forces"] * sym_pairs
+    achieved = forces_flops / (forces_ms * 1e-3) / 1e12 if forces_ms > 0 else None
+    roofline = {"bound": "alu", "kernel": "k_forces (Eqs. 17-18 + limited viscosity)",
+                "achieved": achieved, "peak": FP32_PEAK_THEORETICAL / 1e12, "unit": "TFLOP/s",
+                "frac": (achieved / (FP32_PEAK_THEORETICAL / 1e12)) if achieved else None,
+                "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md); FFMA micro-benchmark measured "
+                               f"{fp32_meas / 1e12:.1f} TFLOP/s in this run",
+                "flops_per_pair": FLOPS_PER_PAIR["forces"], "pairs_per_launch": sym_pairs, "kernel_ms": forces_ms,
+                "traffic": None}
+    passes = {k: st[k] for k in ("ms_sort", "ms_tree", "ms_volumes", "ms_rk", "ms_gradv", "ms_forces")}
+    alg_flops = (FLOPS_PER_PAIR["volumes"] + FLOPS_PER_PAIR["moments"] + FLOPS_PER_PAIR["gradv"]) * gather_pairs + forces_flops
+    sweeps_ms = st["ms_volumes"] + st["ms_rk"] + st["ms_gradv"] + st["ms_forces"]
+    sort_bytes = ps.n * (6 * 32.0 + 16 + 12 + 32 + 16)    # radix passes + pack + gather
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": f"{ps.name} n_side={ps.meta['n_side']} ({ps.n} particles per GPU, ~{gather_pairs / ps.n:.1f} neighbours)",
+                   "particles": int(n_all), "pairs_per_step": pairs_all,
+                   "l2": "inputs and per-step state exceed the 126 MB L2 (no flush needed)" if ps.n * 200 > 126e6
+                         else "state fits in L2 (small config; not the headline)"},
+        "particle_updates_per_s": n_all / (ms_per_step * 1e-3),
+        "passes_ms": passes, "timed_steps": st["timed_steps"],
+        "fp32_frac_pair_passes": alg_flops / (sweeps_ms * 1e-3) / FP32_PEAK_THEORETICAL if sweeps_ms > 0 else None,
+        "sort_gbs": sort_bytes / (st["ms_sort"] * 1e-3) / 1e9 if st["ms_sort"] > 0 else None,
+        "hbm_peak_gbs": peaks.get("hbm_gbs"), "peaks": peak_kind,
+        "e2e": {"value": pairs_all / (e2e_all * 1e-3), "unit": UNIT, "ms_per_step": e2e_all,
+                "h2d_bytes_per_step": int(9 * 4 * n_all), "d2h_bytes_per_step": int(4 * 4 * n_all)},
+        "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        sub, half = oracle_sample(ps, args.oracle_particles)
+        pairs, dt, cores = time_oracle(sub)
+        line["cpu_baseline"] = {"value": pairs / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "seconds": dt,
+                                "sample": f"cube of half-width {half:.4f} at the box centre: {sub.n} of {ps.n} particles, "
+                                          "FP64 brute-force O(n^2) neighbours (oracle/crk_oracle.cpp as it stands)"}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", default="cosmo", choices=list(wl.CONFIG_NAMES))
+    ap.add_argument("--n-side", type=int, default=None)
+    ap.add_argument("--oracle-particles", type=int, default=80000)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -180,14 +180,14 @@ def zeldovich(n_side: int = 256, seed: int = 1004, rms_disp: float = 0.3, k_cut:
     dk[:, :, -1] = 0.0
     kvec = (kx, ky, kz)
     shape = (n_side, n_side, n_side)
-    psi = [np.fft.irfftn(1j * kvec[a] * dk, s=shape) for a in range(3)]
+    psi = [np.fft.irfftn(1j * kvec[a] * dk, s=shape, axes=(0, 1, 2)) for a in range(3)]
     rms = np.sqrt(sum(float((p * p).mean()) for p in psi))
     scale = rms_disp * d / rms
     # deformation tensor d psi_a / d q_b = -k_a k_b delta_k / k^2   (symmetric)
     T = {}
     for a in range(3):
         for b in range(a, 3):
-            T[(a, b)] = scale * np.fft.irfftn(-(kvec[a] * kvec[b]) * dk, s=shape)
+            T[(a, b)] = scale * np.fft.irfftn(-(kvec[a] * kvec[b]) * dk, s=shape, axes=(0, 1, 2))
     del dk
     a00 = 1.0 + T[(0, 0)]; a11 = 1.0 + T[(1, 1)]; a22 = 1.0 + T[(2, 2)]
     a01 = T[(0, 1)]; a02 = T[(0, 2)]; a12 = T[(1, 2)]

@@ -3,11 +3,7 @@
 
 namespace {
 
-enum { EV_BUILD0 = 0, EV_SORTED, EV_BUILD1, EV_VOL0, EV_VOL1, EV_RK0, EV_GV0, EV_GV1, EV_F1, EV_RK1, EV_HY0, EV_N };
-
-void rec(crk_ctx* c, int e) {
-    if (c->timing) cudaEventRecord(c->ev[e], c->stream);
-}
+void rec(crk_ctx* c, int e) { crk_rec(c, e); }
 
 __global__ void k_fp32_peak(float* out, int iters, float b, float cc) {
     float a0 = threadIdx.x * 1e-3f, a1 = a0 + 1.f, a2 = a0 + 2.f, a3 = a0 + 3.f, a4 = a0 + 4.f, a5 = a0 + 5.f,
@@ -43,7 +39,10 @@ int crk_create(crk_ctx** out, const crk_params* p, void* cuda_stream) {
     }
     c->flag.cap = 64;
     c->scratch_bytes = 64;
-    for (int e = 0; e < EV_N; ++e) cudaEventCreate(&c->ev[e]);
+    for (int r = 0; r < CRK_EV_RING; ++r) {
+        c->ev_done[r] = false;
+        for (int e = 0; e < CRK_EV_N; ++e) cudaEventCreate(&c->ev[r][e]);
+    }
     c->ev_ok = true;
     *out = c;
     return CRK_OK;
@@ -60,7 +59,8 @@ void crk_destroy(crk_ctx* c) {
         if (b->p) cudaFree(b->p);
     if (c->h_flag) cudaFreeHost(c->h_flag);
     if (c->ev_ok)
-        for (int e = 0; e < EV_N; ++e) cudaEventDestroy(c->ev[e]);
+        for (int r = 0; r < CRK_EV_RING; ++r)
+            for (int e = 0; e < CRK_EV_N; ++e) cudaEventDestroy(c->ev[r][e]);
     delete c;
 }
 
@@ -79,6 +79,11 @@ int crk_build_cells(crk_ctx* c, int64_t n, const float* x, const float* y, const
     if (n == 0) {
         c->stage = 1;
         return CRK_OK;
+    }
+    if (c->timing) {
+        c->ev_slot = (int)(c->ev_steps % CRK_EV_RING);
+        c->ev_done[c->ev_slot] = false;
+        c->ev_steps++;
     }
     rec(c, EV_BUILD0);
     CRK_TRY(crk_sort_particles(c, x, y, z, h));
@@ -131,6 +136,7 @@ int crk_hydro_derivs(crk_ctx* c, const float* vx, const float* vy, const float* 
     if (c->n > 0) {
         rec(c, EV_HY0);
         CRK_TRY(crk_launch_hydro(c, vx, vy, vz, u, ax, ay, az, dudt, pair_count));
+        if (c->timing) c->ev_done[c->ev_slot] = true;
     }
     c->stage = 4;
     return CRK_OK;
@@ -205,6 +211,8 @@ int crk_set_timing(crk_ctx* c, int on) {
 int crk_reset_stats(crk_ctx* c) {
     if (!c) return CRK_EINVAL;
     c->launches = 0;
+    c->ev_steps = 0;
+    for (int r = 0; r < CRK_EV_RING; ++r) c->ev_done[r] = false;
     return CRK_OK;
 }
 
@@ -217,21 +225,29 @@ int crk_get_stats(crk_ctx* c, crk_stats* out) {
     out->n_leaf_pairs_gather = c->n_pairs_gather;
     out->launches = c->launches;
     out->scratch_bytes = (int64_t)c->scratch_bytes;
-    if (c->timing && c->stage >= 4 && c->n > 0) {
+    if (c->timing && c->n > 0) {
+        // mean over the completed steps still held in the event ring (all steps since crk_reset_stats if <= 64)
         CRK_CUDA(c, cudaStreamSynchronize(c->stream));
-        auto el = [&](int a, int b) {
-            float ms = 0.f;
-            if (cudaEventElapsedTime(&ms, c->ev[a], c->ev[b]) != cudaSuccess) { cudaGetLastError(); ms = -1.f; }
-            return ms;
-        };
-        out->ms_sort = el(EV_BUILD0, EV_SORTED);
-        out->ms_tree = el(EV_SORTED, EV_BUILD1);
-        out->ms_build = el(EV_BUILD0, EV_BUILD1);
-        out->ms_volumes = el(EV_VOL0, EV_VOL1);
-        out->ms_rk = el(EV_RK0, EV_RK1);
-        out->ms_hydro = el(EV_HY0, EV_F1);
-        out->ms_gradv = el(EV_GV0, EV_GV1);
-        out->ms_forces = el(EV_GV1, EV_F1);
+        double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        int cnt = 0;
+        for (int r = 0; r < CRK_EV_RING; ++r) {
+            if (!c->ev_done[r]) continue;
+            auto el = [&](int a, int b) {
+                float ms = 0.f;
+                if (cudaEventElapsedTime(&ms, c->ev[r][a], c->ev[r][b]) != cudaSuccess) { cudaGetLastError(); ms = 0.f; }
+                return (double)ms;
+            };
+            acc[0] += el(EV_BUILD0, EV_SORTED); acc[1] += el(EV_SORTED, EV_BUILD1); acc[2] += el(EV_BUILD0, EV_BUILD1);
+            acc[3] += el(EV_VOL0, EV_VOL1); acc[4] += el(EV_RK0, EV_RK1); acc[5] += el(EV_HY0, EV_F1);
+            acc[6] += el(EV_GV0, EV_GV1); acc[7] += el(EV_GV1, EV_F1);
+            ++cnt;
+        }
+        if (cnt > 0) {
+            out->ms_sort = (float)(acc[0] / cnt); out->ms_tree = (float)(acc[1] / cnt); out->ms_build = (float)(acc[2] / cnt);
+            out->ms_volumes = (float)(acc[3] / cnt); out->ms_rk = (float)(acc[4] / cnt); out->ms_hydro = (float)(acc[5] / cnt);
+            out->ms_gradv = (float)(acc[6] / cnt); out->ms_forces = (float)(acc[7] / cnt);
+        }
+        out->timed_steps = cnt;
     }
     return CRK_OK;
 }

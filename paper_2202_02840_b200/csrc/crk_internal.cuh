@@ -12,6 +12,10 @@
 #define CRK_MAX_LEVELS 8
 #define CRK_KEY_BITS 16          // space-filling-curve bits per dimension (48-bit keys)
 
+#define CRK_EV_RING 64
+#define CRK_EV_N 12
+enum { EV_BUILD0 = 0, EV_SORTED, EV_BUILD1, EV_VOL0, EV_VOL1, EV_RK0, EV_GV0, EV_GV1, EV_F1, EV_RK1, EV_HY0 };
+
 #define CRK_FLAG_GATHER 0x80000000u   // leaf-list entry: gap(a,b) < hmax(a)   (one-sided passes use it)
 #define CRK_FLAG_WRAP   0x40000000u   // leaf pair may straddle the periodic boundary
 #define CRK_LEAF_MASK   0x0fffffffu
@@ -30,7 +34,10 @@ struct crk_ctx {
     int64_t launches = 0;
     size_t scratch_bytes = 0;
     int timing = 0;
-    cudaEvent_t ev[12];
+    cudaEvent_t ev[CRK_EV_RING][CRK_EV_N];   // one event set per step, so a timed loop can be read back afterwards
+    bool ev_done[CRK_EV_RING];
+    int ev_slot = 0;
+    int64_t ev_steps = 0;
     bool ev_ok = false;
     crk_stats st;
 
@@ -75,6 +82,10 @@ struct crk_ctx {
         int rc__ = (expr);           \
         if (rc__ != CRK_OK) return rc__; \
     } while (0)
+
+static inline void crk_rec(crk_ctx* c, int e) {
+    if (c->timing) cudaEventRecord(c->ev[c->ev_slot][e], c->stream);
+}
 
 static inline int crk_ensure(crk_ctx* c, DevBuf& b, size_t bytes) {
     if (bytes <= b.cap && b.p) return CRK_OK;

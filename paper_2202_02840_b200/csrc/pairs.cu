@@ -94,13 +94,13 @@ __device__ __forceinline__ int test_chunk(const SweepArgs& a, uint32_t e0, uint3
 #pragma unroll 4
             for (int k = 0; k < 32; ++k) {
                 const float4 pj = t[k];
-                const float dx = wrap1(__fsub_rn(xi, pj.x), a.L, a.half);
-                const float dy = wrap1(__fsub_rn(yi, pj.y), a.L, a.half);
-                const float dz = wrap1(__fsub_rn(zi, pj.z), a.L, a.half);
+                const float dx0 = __fsub_rn(xi, pj.x), dy0 = __fsub_rn(yi, pj.y), dz0 = __fsub_rn(zi, pj.z);
+                const float dx = wrap1(dx0, a.L, a.half), dy = wrap1(dy0, a.L, a.half), dz = wrap1(dz0, a.L, a.half);
                 const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
                 const float lim = SYM ? fmaxf(hi2, __fmul_rn(pj.w, pj.w)) : hi2;
                 if (r2 < lim && k != self_k) {
-                    *qp = (uint8_t)(c * 32 + k);
+                    const bool wrapped = (dx != dx0) || (dy != dy0) || (dz != dz0);
+                    *qp = (uint8_t)((c * 32 + k) | (wrapped ? 0x80 : 0));    // bit 7: pair crosses the periodic boundary
                     qp += 32;
                 }
             }
@@ -124,17 +124,33 @@ __device__ __forceinline__ float wendland_w(float eta) {
     return t2 * t2 * t2 * fmaf(eta, fmaf(eta, C35_3, 6.0f), 1.0f);
 }
 
-// min-image separation of an accepted pair (same float sequence as the predicate)
-__device__ __forceinline__ void sep3(const SweepArgs& a, float xi, float yi, float zi, const float4& pj, float& dx,
-                                     float& dy, float& dz, float& r2) {
-    dx = wrap1(__fsub_rn(xi, pj.x), a.L, a.half);
-    dy = wrap1(__fsub_rn(yi, pj.y), a.L, a.half);
-    dz = wrap1(__fsub_rn(zi, pj.z), a.L, a.half);
+// Separation of an accepted pair for the VALUES (the set membership was decided by the prescribed predicate above).
+// Plain pairs: d = x_i - x_j.  Pairs that cross the periodic boundary (queue bit 7): shift the coordinate that lies in
+// the upper half of the box by -L first (exact, Sterbenz) and subtract afterwards, so that the rounding error is
+// relative to |d| and not to L  (fl(x_i - x_j) ~ 1 - 1e-3 would lose 1e-5 of a 4e-3 separation).
+__device__ __forceinline__ float sep1_wrapped(float xi, float xj, float L, float half) {
+    const float d = __fsub_rn(xi, xj);
+    if (d > half) return __fsub_rn(__fsub_rn(xi, L), xj);
+    if (d < -half) return __fsub_rn(xi, __fsub_rn(xj, L));
+    return d;
+}
+__device__ __forceinline__ void sep3(const SweepArgs& a, bool wrapped, float xi, float yi, float zi, const float4& pj,
+                                     float& dx, float& dy, float& dz, float& r2) {
+    if (!wrapped) {
+        dx = __fsub_rn(xi, pj.x);
+        dy = __fsub_rn(yi, pj.y);
+        dz = __fsub_rn(zi, pj.z);
+    } else {
+        dx = sep1_wrapped(xi, pj.x, a.L, a.half);
+        dy = sep1_wrapped(yi, pj.y, a.L, a.half);
+        dz = sep1_wrapped(zi, pj.z, a.L, a.half);
+    }
     r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
 }
 
 template <int CH, int PLANES>
 struct Smem {
+    static_assert(CH * 32 <= 128, "queue entries keep bit 7 for the periodic-wrap mark");
     static constexpr int TILE_F4 = PLANES * CH * 32;
     static constexpr int QUEUE_B = CH * 32 * 32;
     static constexpr int PER_WARP = TILE_F4 * 16 + QUEUE_B;
@@ -168,9 +184,10 @@ __global__ void __launch_bounds__(WPC * 32) k_volumes(SweepArgs a) {
         const int maxc = __reduce_max_sync(0xffffffffu, cnt);
         for (int s = 0; s < maxc; ++s) {
             if (s < cnt) {
-                const float4 pj = tile[queue[s * 32 + lane]];
+                const int qe = queue[s * 32 + lane];
+                const float4 pj = tile[qe & 0x7f];
                 float dx, dy, dz, r2;
-                sep3(a, xi, yi, zi, pj, dx, dy, dz, r2);
+                sep3(a, (qe & 0x80) != 0, xi, yi, zi, pj, dx, dy, dz, r2);
                 const float r = r2 * rsqrtf(fmaxf(r2, R2_TINY));
                 acc += wendland_w(r * inv_h);
             }
@@ -233,9 +250,10 @@ __global__ void __launch_bounds__(WPC * 32) k_moments(SweepArgs a) {
         const int maxc = __reduce_max_sync(0xffffffffu, cnt);
         for (int s = 0; s < maxc; ++s) {
             if (s < cnt) {
-                const float4 pj = tile[queue[s * 32 + lane]];
+                const int qe = queue[s * 32 + lane];
+                const float4 pj = tile[qe & 0x7f];
                 float dx, dy, dz, r2;
-                sep3(a, xi, yi, zi, pj, dx, dy, dz, r2);
+                sep3(a, (qe & 0x80) != 0, xi, yi, zi, pj, dx, dy, dz, r2);
                 const float r = r2 * rsqrtf(fmaxf(r2, R2_TINY));
                 float Wt, Dt;
                 wendland(r * inv_h, Wt, Dt);
@@ -441,11 +459,12 @@ __global__ void __launch_bounds__(WPC * 32) k_gradv(SweepArgs a) {
         const int maxc = __reduce_max_sync(0xffffffffu, cnt);
         for (int s = 0; s < maxc; ++s) {
             if (s < cnt) {
-                const int jj = queue[s * 32 + lane];
+                const int qe = queue[s * 32 + lane];
+                const int jj = qe & 0x7f;
                 const float4 pj = tile[jj];
                 const float4 vj = tile[CH4 * 32 + jj];
                 float dx, dy, dz, r2;
-                sep3(a, xi, yi, zi, pj, dx, dy, dz, r2);
+                sep3(a, (qe & 0x80) != 0, xi, yi, zi, pj, dx, dy, dz, r2);
                 const float r = r2 * rsqrtf(fmaxf(r2, R2_TINY));
                 float W, D, gx, gy, gz;
                 wendland_dim(r, ih, k3, W, D);
@@ -505,14 +524,15 @@ __global__ void __launch_bounds__(WPC * 32) k_forces(SweepArgs a) {
         const int maxc = __reduce_max_sync(0xffffffffu, cnt);
         for (int s = 0; s < maxc; ++s) {
             if (s < cnt) {
-                const int jj = queue[s * 32 + lane];
+                const int qe = queue[s * 32 + lane];
+                const int jj = qe & 0x7f;
                 const float4 pj = tile[jj];
                 const float4 vj = tile[PS + jj];
                 const float4 tj = tile[2 * PS + jj];
                 const Coef cj = load_coef(tile[3 * PS + jj], tile[4 * PS + jj], tile[5 * PS + jj], tile[6 * PS + jj]);
                 const float4 h0 = tile[7 * PS + jj], h1 = tile[8 * PS + jj], h2 = tile[9 * PS + jj];
                 float dx, dy, dz, r2;
-                sep3(a, xi, yi, zi, pj, dx, dy, dz, r2);
+                sep3(a, (qe & 0x80) != 0, xi, yi, zi, pj, dx, dy, dz, r2);
                 const float r = __fmul_rn(r2, rsqrtf(fmaxf(r2, R2_TINY)));
                 float Wi, Di, Wj, Dj;
                 wendland_dim(r, ti.w, k3i, Wi, Di);
@@ -642,14 +662,14 @@ int crk_launch_hydro(crk_ctx* c, const float* vx, const float* vy, const float* 
     SweepArgs a = make_args(c);
     k_hydro_prep<<<(unsigned)((np + 255) / 256), 256, 0, c->stream>>>(a, (const float4*)c->vel_orig.p);
     CRK_TRY(crk_check_launch(c, "k_hydro_prep"));
-    if (c->timing) cudaEventRecord(c->ev[6], c->stream);
+    crk_rec(c, EV_GV0);
     {
         const int smem = WPC * Smem<CH4, 2>::PER_WARP;
         CRK_TRY(set_smem(c, k_gradv, smem));
         k_gradv<<<(unsigned)((c->nl + WPC - 1) / WPC), WPC * 32, smem, c->stream>>>(a);
         CRK_TRY(crk_check_launch(c, "k_gradv"));
     }
-    if (c->timing) cudaEventRecord(c->ev[7], c->stream);
+    crk_rec(c, EV_GV1);
     a.o0 = ax; a.o1 = ay; a.o2 = az; a.o3 = dudt; a.ocnt = pair_count;
     {
         const int smem = WPC * Smem<CH5, PL5>::PER_WARP;
@@ -657,6 +677,6 @@ int crk_launch_hydro(crk_ctx* c, const float* vx, const float* vy, const float* 
         k_forces<<<(unsigned)((c->nl + WPC - 1) / WPC), WPC * 32, smem, c->stream>>>(a);
         CRK_TRY(crk_check_launch(c, "k_forces"));
     }
-    if (c->timing) cudaEventRecord(c->ev[8], c->stream);
+    crk_rec(c, EV_F1);
     return CRK_OK;
 }
