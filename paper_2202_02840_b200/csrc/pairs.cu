@@ -1,12 +1,15 @@
 // pairs.cu -- steps a1..a5: the four pair sweeps of one CRKSPH derivative evaluation (FP32 pair math on the FMA pipes).
 //
 // Common structure (one warp = one 32-particle leaf, one lane = one particle i, state of i in registers):
-//   for each chunk of CH neighbour leaves from the leaf interaction list (tree.cu):
-//     stage   the chunk's particle state into warp-private shared memory (coalesced 16-byte loads)
+//   for each neighbour leaf b of the leaf interaction list (tree.cu):
+//     cull    lane l takes particle l of b and tests it against the bounding box of the warp's own leaf (point-to-box gap
+//             vs the leaf's hmax, same monotone float sequence as the predicate, so nothing is lost); survivors are
+//             compacted (ballot + prefix popc) into a warp-private shared-memory tile of CAP slots, all planes
+//   when the tile is full (and at the end):
 //     test    every staged j against the lane's i with the prescribed FP32 predicate (S3); all lanes read the
-//             same j (shared-memory broadcast); accepted j are appended to a per-lane byte queue
-//     drain   each lane walks its own queue and evaluates the pair math only for accepted pairs (lane-divergence is
-//             limited to the spread of queue lengths inside one chunk instead of the ~6% acceptance rate)
+//             same j (shared-memory broadcast); accepted slots are appended to a per-lane byte queue
+//     drain   each lane walks its own queue and evaluates the pair math only for accepted pairs (lane divergence is
+//             limited to the spread of queue lengths over one tile instead of the few-% acceptance rate)
 // Equation numbers refer to /root/reference/PAPER.md; the closed forms of A, B, grad A, grad B are derived in DESIGN.md.
 #include "crk_internal.cuh"
 
@@ -25,6 +28,8 @@ struct SweepArgs {
     const uint32_t* __restrict__ list;    // entries: leaf | flags
     const int32_t* __restrict__ perm;     // sorted slot -> caller index
     const float4* __restrict__ posh;      // (x,y,z,h)
+    const float4* __restrict__ leaf_lo;   // per leaf: (xlo,ylo,zlo,hmax)
+    const float4* __restrict__ leaf_hi;   // per leaf: (xhi,yhi,zhi,hmin)
     float4* __restrict__ posV;            // (x,y,z,V)
     float4* __restrict__ velV;            // (vx,vy,vz,V)
     float4* __restrict__ thermo;          // (P,rho,cs,1/h)
@@ -43,70 +48,117 @@ __device__ __forceinline__ float wrap1(float d, float L, float half) {
     return d > half ? __fsub_rn(d, L) : (d < -half ? __fadd_rn(d, L) : d);
 }
 
-// ---- staging: CH leaves x PLANES float4 planes into warp-private smem; returns per-chunk flags -------------------
-template <int CH, int PLANES>
-__device__ __forceinline__ void stage_chunk(const SweepArgs& a, const float4* const (&planes)[PLANES], uint32_t e0,
-                                            uint32_t e1, int lane, float4* tile) {
-    uint32_t ent[CH];
-#pragma unroll
-    for (int c = 0; c < CH; ++c) {
-        const uint32_t e = e0 + c;
-        ent[c] = (e < e1) ? a.list[e] : 0xffffffffu;      // all-ones = padding entry
-    }
-#pragma unroll
-    for (int c = 0; c < CH; ++c) {
-        if (ent[c] != 0xffffffffu) {
-            const int64_t g = (int64_t)(ent[c] & CRK_LEAF_MASK) * CRK_LEAF + lane;
-#pragma unroll
-            for (int p = 0; p < PLANES; ++p) tile[(p * CH + c) * 32 + lane] = planes[p][g];
-        }
-    }
+// ---- culling helpers: lower bound of |wrap(x_i - x_j)| on one axis for x_i in [lo,hi] (monotone float ops) -------
+__device__ __forceinline__ float gap1(float lo, float hi, float x) {
+    return fmaxf(0.f, fmaxf(__fsub_rn(lo, x), __fsub_rn(x, hi)));
+}
+__device__ __forceinline__ float gap1_wrap(float lo, float hi, float x, float L) {
+    const float dmin = __fsub_rn(lo, x), dmax = __fsub_rn(hi, x);     // d = x_i - x_j ranges over [dmin, dmax]
+    const float g0 = fmaxf(0.f, fmaxf(dmin, -dmax));
+    const float gp = fmaxf(0.f, fmaxf(__fsub_rn(L, dmax), __fsub_rn(dmin, L)));
+    const float gm = fmaxf(0.f, fmaxf(__fadd_rn(dmin, L), __fsub_rn(-L, dmax)));
+    return fminf(g0, fminf(gp, gm));
 }
 
-// ---- test phase: append accepted local indices (c*32+k) to the lane's byte queue; returns queue length ----------
+// ---- test phase: append accepted slots to the lane's byte queue; returns queue length -------------------------------
 // SYM = false: gather predicate r2 < h_i^2 (Eqs. 13-14: W_ij = W(|x_i-x_j|, h_i));   SYM = true: r2 < max(h_i^2,h_j^2)
-template <int CH, bool SYM>
-__device__ __forceinline__ int test_chunk(const SweepArgs& a, uint32_t e0, uint32_t e1, int64_t self_leaf, int lane,
-                                          float xi, float yi, float zi, float hi2, const float4* tile,
-                                          uint8_t* queue) {
+template <bool SYM>
+__device__ __forceinline__ int test_slots(const SweepArgs& a, int fill4, bool wrap, int self_slot, int lane, float xi,
+                                          float yi, float zi, float hi2, const float4* tile, uint8_t* queue) {
     uint8_t* qp = queue + lane;
+    if (!wrap) {
 #pragma unroll 1
-    for (int c = 0; c < CH; ++c) {
-        if (e0 + c >= e1) break;
-        const uint32_t e = a.list[e0 + c];
-        if (!SYM && !(e & CRK_FLAG_GATHER)) continue;
-        const bool wrap = (e & CRK_FLAG_WRAP) != 0;
-        const int self_k = ((int64_t)(e & CRK_LEAF_MASK) == self_leaf) ? lane : -1;
-        const float4* t = tile + c * 32;
-        if (!wrap) {
-#pragma unroll 8
-            for (int k = 0; k < 32; ++k) {
-                const float4 pj = t[k];
+        for (int s = 0; s < fill4; s += 4) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                const float4 pj = tile[s + u];
                 const float dx = __fsub_rn(xi, pj.x), dy = __fsub_rn(yi, pj.y), dz = __fsub_rn(zi, pj.z);
                 const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
                 const float lim = SYM ? fmaxf(hi2, __fmul_rn(pj.w, pj.w)) : hi2;
-                if (r2 < lim && k != self_k) {
-                    *qp = (uint8_t)(c * 32 + k);
+                if (r2 < lim && (s + u) != self_slot) {
+                    *qp = (uint8_t)(s + u);
                     qp += 32;
                 }
             }
-        } else {
-#pragma unroll 4
-            for (int k = 0; k < 32; ++k) {
-                const float4 pj = t[k];
-                const float dx0 = __fsub_rn(xi, pj.x), dy0 = __fsub_rn(yi, pj.y), dz0 = __fsub_rn(zi, pj.z);
-                const float dx = wrap1(dx0, a.L, a.half), dy = wrap1(dy0, a.L, a.half), dz = wrap1(dz0, a.L, a.half);
-                const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-                const float lim = SYM ? fmaxf(hi2, __fmul_rn(pj.w, pj.w)) : hi2;
-                if (r2 < lim && k != self_k) {
-                    const bool wrapped = (dx != dx0) || (dy != dy0) || (dz != dz0);
-                    *qp = (uint8_t)((c * 32 + k) | (wrapped ? 0x80 : 0));    // bit 7: pair crosses the periodic boundary
-                    qp += 32;
-                }
+        }
+    } else {
+#pragma unroll 1
+        for (int s = 0; s < fill4; ++s) {
+            const float4 pj = tile[s];
+            const float dx0 = __fsub_rn(xi, pj.x), dy0 = __fsub_rn(yi, pj.y), dz0 = __fsub_rn(zi, pj.z);
+            const float dx = wrap1(dx0, a.L, a.half), dy = wrap1(dy0, a.L, a.half), dz = wrap1(dz0, a.L, a.half);
+            const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+            const float lim = SYM ? fmaxf(hi2, __fmul_rn(pj.w, pj.w)) : hi2;
+            if (r2 < lim && s != self_slot) {
+                const bool wrapped = (dx != dx0) || (dy != dy0) || (dz != dz0);
+                *qp = (uint8_t)(s | (wrapped ? 0x80 : 0));    // bit 7: pair crosses the periodic boundary
+                qp += 32;
             }
         }
     }
     return (int)(qp - (queue + lane)) >> 5;
+}
+
+// ---- the sweep: cull + compact survivors of each neighbour leaf into the tile, test + drain when it fills ---------
+template <int CAP, int PLANES, bool SYM, typename Drain>
+__device__ __forceinline__ void sweep_loop(const SweepArgs& a, const float4* const (&planes)[PLANES], int64_t leaf,
+                                           int lane, float xi, float yi, float zi, float hi2, float4* tile,
+                                           uint8_t* queue, Drain drain) {
+    static_assert(CAP <= 128 && CAP % 32 == 0, "queue entries keep bit 7 for the periodic-wrap mark");
+    const float4 blo = a.leaf_lo[leaf], bhi = a.leaf_hi[leaf];
+    const float hq2 = __fmul_rn(blo.w, blo.w);
+    const uint32_t lt = (1u << lane) - 1u;
+    int fill = 0, self_slot = -1;
+    bool cwrap = false;
+    const uint32_t e0 = a.off[leaf], e1 = a.off[leaf + 1];
+    auto flush = [&]() {
+        const int fill4 = (fill + 3) & ~3;
+        if (lane < fill4 - fill) tile[fill + lane] = make_float4(3.0e30f, 3.0e30f, 3.0e30f, 0.0f);   // never accepted
+        __syncwarp();
+        const int cnt = test_slots<SYM>(a, fill4, cwrap, self_slot, lane, xi, yi, zi, hi2, tile, queue);
+        drain(cnt);
+        __syncwarp();
+        fill = 0;
+        self_slot = -1;
+        cwrap = false;
+    };
+    uint32_t ent = (e0 < e1) ? a.list[e0] : 0u;
+    float4 pj = (e0 < e1) ? planes[0][(int64_t)(ent & CRK_LEAF_MASK) * CRK_LEAF + lane] : make_float4(0, 0, 0, 0);
+    for (uint32_t e = e0; e < e1; ++e) {
+        const uint32_t cur = ent;
+        const float4 pc = pj;
+        if (e + 1 < e1) {   // prefetch the next leaf's positions
+            ent = a.list[e + 1];
+            pj = planes[0][(int64_t)(ent & CRK_LEAF_MASK) * CRK_LEAF + lane];
+        }
+        if (!SYM && !(cur & CRK_FLAG_GATHER)) continue;
+        const int64_t b = (int64_t)(cur & CRK_LEAF_MASK);
+        const int64_t g = b * CRK_LEAF + lane;
+        const bool wrap = (cur & CRK_FLAG_WRAP) != 0;
+        float gx, gy, gz;
+        if (!wrap) {
+            gx = gap1(blo.x, bhi.x, pc.x); gy = gap1(blo.y, bhi.y, pc.y); gz = gap1(blo.z, bhi.z, pc.z);
+        } else {
+            gx = gap1_wrap(blo.x, bhi.x, pc.x, a.L); gy = gap1_wrap(blo.y, bhi.y, pc.y, a.L); gz = gap1_wrap(blo.z, bhi.z, pc.z, a.L);
+        }
+        const float g2 = __fmaf_rn(gz, gz, __fmaf_rn(gy, gy, __fmul_rn(gx, gx)));
+        const float lim = SYM ? fmaxf(hq2, __fmul_rn(pc.w, pc.w)) : hq2;
+        const bool surv = g2 < lim;
+        const uint32_t m = __ballot_sync(0xffffffffu, surv);
+        const int cnt = __popc(m);
+        if (cnt == 0) continue;
+        if (fill + cnt > CAP) flush();
+        const int slot = fill + __popc(m & lt);
+        if (surv) {
+            tile[slot] = pc;
+#pragma unroll
+            for (int p = 1; p < PLANES; ++p) tile[p * CAP + slot] = planes[p][g];
+        }
+        if (b == leaf) self_slot = surv ? slot : -1;
+        cwrap = cwrap || wrap;
+        fill += cnt;
+    }
+    if (fill > 0) flush();
 }
 
 // Wendland C4 (Eq. 12) without its sigma/h^3 prefactor, and D~ with W'/r = sigma h^-5 D~:
@@ -148,17 +200,16 @@ __device__ __forceinline__ void sep3(const SweepArgs& a, bool wrapped, float xi,
     r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
 }
 
-template <int CH, int PLANES>
+template <int CAP, int PLANES>
 struct Smem {
-    static_assert(CH * 32 <= 128, "queue entries keep bit 7 for the periodic-wrap mark");
-    static constexpr int TILE_F4 = PLANES * CH * 32;
-    static constexpr int QUEUE_B = CH * 32 * 32;
+    static constexpr int TILE_F4 = PLANES * CAP;
+    static constexpr int QUEUE_B = CAP * 32;
     static constexpr int PER_WARP = TILE_F4 * 16 + QUEUE_B;
 };
 
 // =================================================================================================== a1: volumes
 // Eq. 14: V_i^-1 = n_i = sum_j W(|x_i - x_j|, h_i), self term included (S4); rho_i = m_i / V_i (S2).
-constexpr int CH1 = 4;
+constexpr int CH1 = 128;   // tile capacity (slots)
 __global__ void __launch_bounds__(WPC * 32) k_volumes(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     using S = Smem<CH1, 1>;
@@ -176,11 +227,7 @@ __global__ void __launch_bounds__(WPC * 32) k_volumes(SweepArgs a) {
     float acc = 0.0f;
     uint32_t count = 0;
     const float4* const planes[1] = {a.posh};
-    const uint32_t e0 = a.off[leaf], e1 = a.off[leaf + 1];
-    for (uint32_t e = e0; e < e1; e += CH1) {
-        stage_chunk<CH1, 1>(a, planes, e, e1, lane, tile);
-        __syncwarp();
-        const int cnt = test_chunk<CH1, false>(a, e, e1, leaf, lane, xi, yi, zi, hi2, tile, queue);
+    sweep_loop<CH1, 1, false>(a, planes, leaf, lane, xi, yi, zi, hi2, tile, queue, [&](int cnt) {
         const int maxc = __reduce_max_sync(0xffffffffu, cnt);
         for (int s = 0; s < maxc; ++s) {
             if (s < cnt) {
@@ -193,8 +240,7 @@ __global__ void __launch_bounds__(WPC * 32) k_volumes(SweepArgs a) {
             }
         }
         count += cnt;
-        __syncwarp();
-    }
+    });
     if (valid) {
         const float k3 = SIGMA_C4 * inv_h * inv_h * inv_h;
         const float ni = k3 * (acc + 1.0f);              // self term W~(0) = 1
@@ -220,7 +266,7 @@ __global__ void __launch_bounds__(WPC * 32) k_volumes(SweepArgs a) {
 //   (g = V_j W'_ij / r):   B = -m2^-1 m1,  A = 1/(m0 + B.m1),
 //   d_c A = -A^2 (d_c m0 + 2 B.d_c m1 + B^T d_c m2 B),  d_c B = -m2^-1 (d_c m1 + d_c m2 B).
 // 29 FP32 sums per particle in eta-normalised units, then an FP64 3x3 solve per particle.
-constexpr int CH2 = 4;
+constexpr int CH2 = 128;
 __global__ void __launch_bounds__(WPC * 32) k_moments(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     using S = Smem<CH2, 1>;
@@ -242,11 +288,7 @@ __global__ void __launch_bounds__(WPC * 32) k_moments(SweepArgs a) {
     float txx = 0.f, txy = 0.f, txz = 0.f, tyy = 0.f, tyz = 0.f, tzz = 0.f;
     float c0 = 0.f, c1 = 0.f, c2 = 0.f, c3 = 0.f, c4 = 0.f, c5 = 0.f, c6 = 0.f, c7 = 0.f, c8 = 0.f, c9 = 0.f;
     const float4* const planes[1] = {a.posV};
-    const uint32_t e0 = a.off[leaf], e1 = a.off[leaf + 1];
-    for (uint32_t e = e0; e < e1; e += CH2) {
-        stage_chunk<CH2, 1>(a, planes, e, e1, lane, tile);
-        __syncwarp();
-        const int cnt = test_chunk<CH2, false>(a, e, e1, leaf, lane, xi, yi, zi, hi2, tile, queue);
+    sweep_loop<CH2, 1, false>(a, planes, leaf, lane, xi, yi, zi, hi2, tile, queue, [&](int cnt) {
         const int maxc = __reduce_max_sync(0xffffffffu, cnt);
         for (int s = 0; s < maxc; ++s) {
             if (s < cnt) {
@@ -273,8 +315,7 @@ __global__ void __launch_bounds__(WPC * 32) k_moments(SweepArgs a) {
                 c9 = fmaf(gv, zz * z, c9);
             }
         }
-        __syncwarp();
-    }
+    });
     float4 o0 = make_float4(0, 0, 0, 0), o1 = o0, o2 = o0, o3 = o0;
     if (valid) {
         // ---- a3: FP64 solve (dimensional quantities; k3 = sigma/h^3)
@@ -431,7 +472,7 @@ __device__ __forceinline__ void wendland_dim(float r, float ih, float k3, float&
 
 // =============================================================================================== a4: velocity gradient
 // Eq. 26: grad v_i = - sum_j V_j (v_i - v_j) (x) grad WR_ij   over the gather set; index [3a+b] = d_b v^a
-constexpr int CH4 = 4;
+constexpr int CH4 = 128;
 __global__ void __launch_bounds__(WPC * 32) k_gradv(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     using S = Smem<CH4, 2>;
@@ -451,18 +492,14 @@ __global__ void __launch_bounds__(WPC * 32) k_gradv(SweepArgs a) {
     const Coef ci = load_coef(a.coef[i], a.coef[a.np + i], a.coef[2 * a.np + i], a.coef[3 * a.np + i]);
     float g[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
     const float4* const planes[2] = {a.posh, a.velV};
-    const uint32_t e0 = a.off[leaf], e1 = a.off[leaf + 1];
-    for (uint32_t e = e0; e < e1; e += CH4) {
-        stage_chunk<CH4, 2>(a, planes, e, e1, lane, tile);
-        __syncwarp();
-        const int cnt = test_chunk<CH4, false>(a, e, e1, leaf, lane, xi, yi, zi, hi2, tile, queue);
+    sweep_loop<CH4, 2, false>(a, planes, leaf, lane, xi, yi, zi, hi2, tile, queue, [&](int cnt) {
         const int maxc = __reduce_max_sync(0xffffffffu, cnt);
         for (int s = 0; s < maxc; ++s) {
             if (s < cnt) {
                 const int qe = queue[s * 32 + lane];
                 const int jj = qe & 0x7f;
                 const float4 pj = tile[jj];
-                const float4 vj = tile[CH4 * 32 + jj];
+                const float4 vj = tile[CH4 + jj];
                 float dx, dy, dz, r2;
                 sep3(a, (qe & 0x80) != 0, xi, yi, zi, pj, dx, dy, dz, r2);
                 const float r = r2 * rsqrtf(fmaxf(r2, R2_TINY));
@@ -476,8 +513,7 @@ __global__ void __launch_bounds__(WPC * 32) k_gradv(SweepArgs a) {
                 g[6] = fmaf(-uz, gx, g[6]); g[7] = fmaf(-uz, gy, g[7]); g[8] = fmaf(-uz, gz, g[8]);
             }
         }
-        __syncwarp();
-    }
+    });
     const float hhat = hi / a.n_h;
     a.gv[i] = make_float4(g[0], g[1], g[2], g[3]);
     a.gv[a.np + i] = make_float4(g[4], g[5], g[6], g[7]);
@@ -489,7 +525,7 @@ __global__ void __launch_bounds__(WPC * 32) k_gradv(SweepArgs a) {
 // Eq. 18:  m_i du_i/dt = sum_j (1/2) V_i V_j (P_j+Q_j) (v_j - v_i).(grad WR_ji - grad WR_ij)       (S6)
 // Q from Eqs. 24-25 with the limited midpoint projection of Eqs. 27-32 (S7: division-free van Leer form).
 // Sums over all j != i with r2 < max(h_i^2, h_j^2); each ordered pair is evaluated by the lane that owns i.
-constexpr int CH5 = 2;
+constexpr int CH5 = 64;
 constexpr int PL5 = 10;
 __global__ void __launch_bounds__(WPC * 32) k_forces(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -515,12 +551,8 @@ __global__ void __launch_bounds__(WPC * 32) k_forces(SweepArgs a) {
     uint32_t count = 0;
     const float4* const planes[PL5] = {a.posh, a.velV, a.thermo, a.coef, a.coef + a.np, a.coef + 2 * a.np,
                                        a.coef + 3 * a.np, a.gv, a.gv + a.np, a.gv + 2 * a.np};
-    const uint32_t e0 = a.off[leaf], e1 = a.off[leaf + 1];
-    constexpr int PS = CH5 * 32;   // plane stride in the tile
-    for (uint32_t e = e0; e < e1; e += CH5) {
-        stage_chunk<CH5, PL5>(a, planes, e, e1, lane, tile);
-        __syncwarp();
-        const int cnt = valid ? test_chunk<CH5, true>(a, e, e1, leaf, lane, xi, yi, zi, hi2, tile, queue) : 0;
+    constexpr int PS = CH5;        // plane stride in the tile
+    sweep_loop<CH5, PL5, true>(a, planes, leaf, lane, xi, yi, zi, hi2, tile, queue, [&](int cnt) {
         const int maxc = __reduce_max_sync(0xffffffffu, cnt);
         for (int s = 0; s < maxc; ++s) {
             if (s < cnt) {
@@ -582,8 +614,7 @@ __global__ void __launch_bounds__(WPC * 32) k_forces(SweepArgs a) {
             }
         }
         count += cnt;
-        __syncwarp();
-    }
+    });
     if (valid) {
         const float im = 1.0f / a.m_s[i];
         const int32_t p = a.perm[i];
@@ -608,6 +639,7 @@ SweepArgs make_args(crk_ctx* c) {
     a.L = c->prm.box; a.half = 0.5f * c->prm.box;
     a.off = (const uint32_t*)c->nbr_off.p; a.list = (const uint32_t*)c->nbr_list.p;
     a.perm = c->perm;
+    a.leaf_lo = (const float4*)c->leaf_lo.p; a.leaf_hi = (const float4*)c->leaf_hi.p;
     a.posh = (const float4*)c->posh.p; a.posV = (float4*)c->posV.p; a.velV = (float4*)c->velV.p;
     a.thermo = (float4*)c->thermo.p; a.coef = (float4*)c->coef.p; a.gv = (float4*)c->gv.p;
     a.rho_s = (float*)c->rho_s.p; a.m_s = (const float*)c->m_s.p;
