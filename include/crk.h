@@ -62,11 +62,12 @@ typedef struct {
     int64_t  n_leaf_pairs_gather; /* of which satisfy the one-sided (gather) criterion                        */
     int64_t  launches;        /* kernels launched by this context since crk_create / crk_reset_stats          */
     int64_t  scratch_bytes;   /* device memory currently owned by the context                                 */
+    int64_t  list_bytes;      /* bytes of per-particle neighbour lists written by the last build              */
     float    ms_build, ms_volumes, ms_rk, ms_hydro;   /* mean device time per call of each entry point over the
                                                          steps since crk_reset_stats, when timing is on          */
-    float    ms_sort, ms_tree, ms_gradv, ms_forces;   /* finer split: sort+pack | leaves+list | Eq.26 | Eqs.17-18 */
+    float    ms_sort, ms_tree, ms_gradv, ms_forces;   /* finer split: sort+pack | leaves+leaf list | Eq.26 | Eqs.17-18 */
+    float    ms_lists;        /* per-particle neighbour lists (third part of crk_build_cells)                  */
     int32_t  timed_steps;     /* number of completed steps the ms_* fields average over (event ring of 64)    */
-    int32_t  reserved;
 } crk_stats;
 
 /* stream: a cudaStream_t (0 = default stream).  Returns CRK_OK and *out, or an error.                       */

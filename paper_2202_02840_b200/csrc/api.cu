@@ -53,8 +53,8 @@ void crk_destroy(crk_ctx* c) {
     cudaStreamSynchronize(c->stream);
     DevBuf* bufs[] = {&c->keys[0], &c->keys[1], &c->vals[0], &c->vals[1], &c->hist, &c->scan_tmp, &c->posh_orig,
                       &c->posh, &c->leaf_lo, &c->leaf_hi, &c->nbr_cnt, &c->nbr_off, &c->nbr_list, &c->nbr_gcnt,
-                      &c->posV, &c->rho_s, &c->coef, &c->velV, &c->thermo, &c->gv, &c->vel_orig, &c->m_s, &c->flag,
-                      &c->host_stage};
+                      &c->posV, &c->rho_s, &c->coef, &c->fst, &c->u_s, &c->vel_orig, &c->m_s, &c->flag,
+                      &c->host_stage, &c->arena, &c->seg_first};
     for (DevBuf* b : bufs)
         if (b->p) cudaFree(b->p);
     if (c->h_flag) cudaFreeHost(c->h_flag);
@@ -89,6 +89,8 @@ int crk_build_cells(crk_ctx* c, int64_t n, const float* x, const float* y, const
     CRK_TRY(crk_sort_particles(c, x, y, z, h));
     rec(c, EV_SORTED);
     CRK_TRY(crk_build_tree_and_list(c));
+    rec(c, EV_TREE1);
+    CRK_TRY(crk_build_nbr_lists(c));
     rec(c, EV_BUILD1);
     c->stage = 1;
     return CRK_OK;
@@ -182,13 +184,14 @@ int crk_get_perm(crk_ctx* c, int32_t* perm) {
     return CRK_OK;
 }
 
-__global__ void k_scatter_gradv(const float4* __restrict__ gv, const int32_t* __restrict__ perm, int64_t n, int64_t np,
+// grad v sits in planes 6 (w), 7 and 8 of the force-sweep state
+__global__ void k_scatter_gradv(const float4* __restrict__ fst, const int32_t* __restrict__ perm, int64_t n, int64_t np,
                                 float* __restrict__ out) {
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n) return;
-    const float4 a = gv[k], b = gv[np + k], cc = gv[2 * np + k];
+    const float4 a = fst[6 * np + k], b = fst[7 * np + k], cc = fst[8 * np + k];
     const int32_t p = perm[k];
-    const float g[9] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w, cc.x};
+    const float g[9] = {a.w, b.x, b.y, b.z, b.w, cc.x, cc.y, cc.z, cc.w};
 #pragma unroll
     for (int q = 0; q < 9; ++q) out[q * n + p] = g[q];
 }
@@ -197,7 +200,7 @@ int crk_get_gradv(crk_ctx* c, float* gradv) {
     if (!c || !gradv) return CRK_EINVAL;
     if (c->stage < 4) return CRK_ESTATE;
     if (c->n == 0) return CRK_OK;
-    k_scatter_gradv<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>((const float4*)c->gv.p, c->perm, c->n,
+    k_scatter_gradv<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>((const float4*)c->fst.p, c->perm, c->n,
                                                                            c->nl * CRK_LEAF, gradv);
     return crk_check_launch(c, "k_scatter_gradv");
 }
@@ -225,10 +228,11 @@ int crk_get_stats(crk_ctx* c, crk_stats* out) {
     out->n_leaf_pairs_gather = c->n_pairs_gather;
     out->launches = c->launches;
     out->scratch_bytes = (int64_t)c->scratch_bytes;
+    out->list_bytes = c->arena_units * 16;
     if (c->timing && c->n > 0) {
         // mean over the completed steps still held in the event ring (all steps since crk_reset_stats if <= 64)
         CRK_CUDA(c, cudaStreamSynchronize(c->stream));
-        double acc[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        double acc[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
         int cnt = 0;
         for (int r = 0; r < CRK_EV_RING; ++r) {
             if (!c->ev_done[r]) continue;
@@ -237,7 +241,8 @@ int crk_get_stats(crk_ctx* c, crk_stats* out) {
                 if (cudaEventElapsedTime(&ms, c->ev[r][a], c->ev[r][b]) != cudaSuccess) { cudaGetLastError(); ms = 0.f; }
                 return (double)ms;
             };
-            acc[0] += el(EV_BUILD0, EV_SORTED); acc[1] += el(EV_SORTED, EV_BUILD1); acc[2] += el(EV_BUILD0, EV_BUILD1);
+            acc[0] += el(EV_BUILD0, EV_SORTED); acc[1] += el(EV_SORTED, EV_TREE1); acc[2] += el(EV_BUILD0, EV_BUILD1);
+            acc[8] += el(EV_TREE1, EV_BUILD1);
             acc[3] += el(EV_VOL0, EV_VOL1); acc[4] += el(EV_RK0, EV_RK1); acc[5] += el(EV_HY0, EV_F1);
             acc[6] += el(EV_GV0, EV_GV1); acc[7] += el(EV_GV1, EV_F1);
             ++cnt;
@@ -246,6 +251,7 @@ int crk_get_stats(crk_ctx* c, crk_stats* out) {
             out->ms_sort = (float)(acc[0] / cnt); out->ms_tree = (float)(acc[1] / cnt); out->ms_build = (float)(acc[2] / cnt);
             out->ms_volumes = (float)(acc[3] / cnt); out->ms_rk = (float)(acc[4] / cnt); out->ms_hydro = (float)(acc[5] / cnt);
             out->ms_gradv = (float)(acc[6] / cnt); out->ms_forces = (float)(acc[7] / cnt);
+            out->ms_lists = (float)(acc[8] / cnt);
         }
         out->timed_steps = cnt;
     }

@@ -13,8 +13,21 @@
 #define CRK_KEY_BITS 16          // space-filling-curve bits per dimension (48-bit keys)
 
 #define CRK_EV_RING 64
-#define CRK_EV_N 12
-enum { EV_BUILD0 = 0, EV_SORTED, EV_BUILD1, EV_VOL0, EV_VOL1, EV_RK0, EV_GV0, EV_GV1, EV_F1, EV_RK1, EV_HY0 };
+#define CRK_EV_N 13
+enum { EV_BUILD0 = 0, EV_SORTED, EV_TREE1, EV_BUILD1, EV_VOL0, EV_VOL1, EV_RK0, EV_GV0, EV_GV1, EV_F1, EV_RK1, EV_HY0 };
+
+// ---- neighbour lists (lists.cu): per leaf a chain of segments in one arena of 16-byte units --------------------------
+//   segment = header (9 units) | cand[C] u32, padded to 4 | ell[K][32] u16
+//   header unit 0: {next segment (arena unit, 0 = none), C | Kg << 16, K, 0}; units 1-4: cnt_g[32] u16; units 5-8: cnt[32] u16
+//   cand[c]   = sorted-order index of candidate c (only candidates accepted by at least one lane of the leaf)
+//   ell[k][l] = k-th entry of lane l: candidate index | bit 15 (pair crosses the periodic boundary); lane l owns
+//               cnt_g[l] gather entries (r2 < h_i^2) followed by cnt[l] - cnt_g[l] entries that are symmetric-only
+#define CRK_CCAP 640             // candidates per segment (tile capacity of the sweeps)
+#define CRK_QCAP 160             // entries per lane per segment
+#define CRK_TCULL 64             // cull tile of the list builder
+#define CRK_SEG_HDR_UNITS 9
+#define CRK_ELL_WRAP 0x8000u
+#define CRK_ELL_MASK 0x7fffu
 
 #define CRK_FLAG_GATHER 0x80000000u   // leaf-list entry: gap(a,b) < hmax(a)   (one-sided passes use it)
 #define CRK_FLAG_WRAP   0x40000000u   // leaf pair may straddle the periodic boundary
@@ -53,13 +66,14 @@ struct crk_ctx {
     int64_t level_cnt[CRK_MAX_LEVELS + 1];
     DevBuf nbr_cnt, nbr_off, nbr_list, nbr_gcnt;
     int64_t n_pairs = 0, n_pairs_gather = 0;
+    DevBuf arena, seg_first;       // neighbour-list arena (16-byte units) and first-segment unit per leaf
+    int64_t arena_units = 0;       // units used by the last build
     // per-particle state in sorted order
     DevBuf posV;                   // float4 (x,y,z,V)
     DevBuf rho_s;                  // float
     DevBuf coef;                   // 4 planes float4[n]: (A,Bx,By,Bz) (cx,cy,cz,M00) (M01,M02,M10,M11) (M12,M20,M21,M22)
-    DevBuf velV;                   // float4 (vx,vy,vz,V)
-    DevBuf thermo;                 // float4 (P, rho, c_s, 1/h)
-    DevBuf gv;                     // 3 planes float4[n]: (g00,g01,g02,g10) (g11,g12,g20,g21) (g22, sigma/h^3, hhat, hhat^2 eps^2)
+    DevBuf fst;                    // force-sweep state, 9 planes float4[np] (layout at k_forces in pairs.cu)
+    DevBuf u_s;                    // float, specific internal energy in sorted order
     DevBuf vel_orig;               // float4 (vx,vy,vz,u) caller order (packed for a 16-byte gather)
     DevBuf m_s;                    // float, sorted
     DevBuf flag;                   // int[4] device error / status flags
@@ -122,6 +136,7 @@ static inline int crk_check_launch(crk_ctx* c, const char* what) {
 int crk_sort_particles(crk_ctx* c, const float* x, const float* y, const float* z, const float* h);   // sort.cu
 int crk_exclusive_scan_u32(crk_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, DevBuf& tmp);    // sort.cu
 int crk_build_tree_and_list(crk_ctx* c);                                                               // tree.cu
+int crk_build_nbr_lists(crk_ctx* c);                                                                   // lists.cu
 int crk_launch_volumes(crk_ctx* c, const float* m, float* V, float* rho, uint32_t* nbr_count);        // pairs.cu
 int crk_launch_moments(crk_ctx* c, float* A, float* B, float* gradA, float* gradB);                   // pairs.cu
 int crk_launch_hydro(crk_ctx* c, const float* vx, const float* vy, const float* vz, const float* u,

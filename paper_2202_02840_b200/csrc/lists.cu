@@ -1,0 +1,220 @@
+// lists.cu -- step a0 (third part): per-particle neighbour lists, built once per crk_build_cells and reused by all four
+// pair sweeps ("all hydro operators utilize the same interaction list, which need only be assembled once per hydro
+// subcycle, and reused for each kernel", PAPER.md:302 -- here taken down to particle pairs).
+//
+// One warp = one 32-particle leaf, one lane = one particle i.  For every neighbour leaf of the leaf interaction list
+// (tree.cu) lane l takes particle l of that leaf and culls it against the query leaf's box; survivors go to a small tile;
+// every staged j is then tested against every lane's i with the prescribed FP32 predicate (S3).  A candidate
+// accepted by at least one lane receives the next candidate index c of the current segment; lane i appends c to its
+// gather entries (r2 < h_i^2) or to its symmetric-only entries (h_i^2 <= r2 < h_j^2).  A segment is written to the arena
+// as  header | cand[C] | ell[K][32]  (layout in crk_internal.cuh); it is cut when the candidate or entry capacity would
+// overflow, so leaves in strongly clustered regions own a chain of segments.
+#include "crk_internal.cuh"
+
+namespace {
+
+constexpr int LW = 2;   // warps (= leaves) per CTA
+
+struct ListArgs {
+    int64_t n, nl;
+    float L, half;
+    const uint32_t* __restrict__ off;
+    const uint32_t* __restrict__ list;
+    const float4* __restrict__ posh;
+    const float4* __restrict__ leaf_lo;
+    const float4* __restrict__ leaf_hi;
+    uint4* arena;
+    unsigned long long arena_cap;          // units
+    unsigned long long* counter;           // next free unit (unit 0 is reserved as "none")
+    uint32_t* __restrict__ seg_first;
+};
+
+struct WarpSmem {
+    float4 tile[CRK_TCULL];
+    uint32_t tidx[CRK_TCULL];
+    uint32_t cand[CRK_CCAP];
+    uint16_t queue[CRK_QCAP][32];
+};
+
+__device__ __forceinline__ float wrap1(float d, float L, float half) {
+    return d > half ? __fsub_rn(d, L) : (d < -half ? __fadd_rn(d, L) : d);
+}
+// lower bound of |wrap(x_i - x_j)| on one axis for x_i in [lo,hi] (monotone float ops, so nothing is lost)
+__device__ __forceinline__ float gap1(float lo, float hi, float x) {
+    return fmaxf(0.f, fmaxf(__fsub_rn(lo, x), __fsub_rn(x, hi)));
+}
+__device__ __forceinline__ float gap1_wrap(float lo, float hi, float x, float L) {
+    const float dmin = __fsub_rn(lo, x), dmax = __fsub_rn(hi, x);
+    const float g0 = fmaxf(0.f, fmaxf(dmin, -dmax));
+    const float gp = fmaxf(0.f, fmaxf(__fsub_rn(L, dmax), __fsub_rn(dmin, L)));
+    const float gm = fmaxf(0.f, fmaxf(__fadd_rn(dmin, L), __fsub_rn(-L, dmax)));
+    return fminf(g0, fminf(gp, gm));
+}
+
+// test every staged candidate against the lane's particle; returns the new candidate count of the segment
+template <bool WRAP>
+__device__ __forceinline__ int test_tile(WarpSmem& S, int fill, int C, int& g, int& s, int lane, uint32_t self, float xi,
+                                         float yi, float zi, float hi2, float L, float half) {
+#pragma unroll 2
+    for (int t = 0; t < fill; ++t) {
+        const float4 pj = S.tile[t];
+        const uint32_t jidx = S.tidx[t];
+        float dx = __fsub_rn(xi, pj.x), dy = __fsub_rn(yi, pj.y), dz = __fsub_rn(zi, pj.z);
+        bool wrapped = false;
+        if (WRAP) {
+            const float wx = wrap1(dx, L, half), wy = wrap1(dy, L, half), wz = wrap1(dz, L, half);
+            wrapped = (wx != dx) || (wy != dy) || (wz != dz);
+            dx = wx; dy = wy; dz = wz;
+        }
+        const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+        const bool notself = jidx != self;
+        const bool ag = (r2 < hi2) && notself;                                       // gather: Eqs. 13-14
+        const bool as = (r2 < fmaxf(hi2, __fmul_rn(pj.w, pj.w))) && notself;         // symmetric: Eqs. 17-18
+        if (__any_sync(0xffffffffu, as)) {
+            if (lane == 0) S.cand[C] = jidx;
+            const uint16_t e = (uint16_t)(C | (wrapped ? CRK_ELL_WRAP : 0u));
+            if (ag) S.queue[g++][lane] = e;
+            else if (as) S.queue[CRK_QCAP - 1 - (s++)][lane] = e;
+            ++C;
+        }
+    }
+    return C;
+}
+
+__global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
+    __shared__ WarpSmem sm[LW];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int64_t leaf = (int64_t)blockIdx.x * LW + w;
+    if (leaf >= a.nl) return;
+    WarpSmem& S = sm[w];
+    const int64_t i = leaf * CRK_LEAF + lane;
+    const float4 pi = a.posh[i];
+    const float xi = pi.x, yi = pi.y, zi = pi.z;
+    const float hi2 = __fmul_rn(pi.w, pi.w);
+    const float4 blo = a.leaf_lo[leaf], bhi = a.leaf_hi[leaf];
+    const float hq2 = __fmul_rn(blo.w, blo.w);
+    const uint32_t lt = (1u << lane) - 1u;
+    int C = 0, g = 0, s = 0, fill = 0;
+    bool cwrap = false;
+    uint32_t prev = 0;   // arena unit of the previous segment header of this leaf
+
+    auto emit = [&]() {
+        const int Kg = __reduce_max_sync(0xffffffffu, g);
+        const int K = __reduce_max_sync(0xffffffffu, g + s);
+        const unsigned long long units = CRK_SEG_HDR_UNITS + (unsigned long long)((C + 3) >> 2) + 4ull * K;
+        unsigned long long base = 0;
+        if (lane == 0) base = atomicAdd(a.counter, units);
+        base = __shfl_sync(0xffffffffu, base, 0);
+        __syncwarp();
+        if (base + units <= a.arena_cap) {
+            uint4* hdr = a.arena + base;
+            if (lane == 0) hdr[0] = make_uint4(0u, (uint32_t)C | ((uint32_t)Kg << 16), (uint32_t)K, 0u);
+            ((uint16_t*)(hdr + 1))[lane] = (uint16_t)g;
+            ((uint16_t*)(hdr + 5))[lane] = (uint16_t)(g + s);
+            uint32_t* cd = (uint32_t*)(hdr + CRK_SEG_HDR_UNITS);
+            for (int c = lane; c < C; c += 32) cd[c] = S.cand[c];
+            uint16_t* el = (uint16_t*)(hdr + CRK_SEG_HDR_UNITS + ((C + 3) >> 2));
+            for (int k = 0; k < K; ++k) {
+                uint16_t v = 0xffffu;
+                if (k < g) v = S.queue[k][lane];
+                else if (k < g + s) v = S.queue[CRK_QCAP - 1 - (k - g)][lane];
+                el[k * 32 + lane] = v;
+            }
+            if (lane == 0) {
+                if (prev == 0) a.seg_first[leaf] = (uint32_t)base;
+                else ((uint32_t*)(a.arena + prev))[0] = (uint32_t)base;
+            }
+            prev = (uint32_t)base;
+        }
+        C = 0; g = 0; s = 0;
+        __syncwarp();
+    };
+    auto flush = [&]() {
+        const int maxlen = __reduce_max_sync(0xffffffffu, g + s);
+        if (C + fill > CRK_CCAP || maxlen + fill > CRK_QCAP) emit();
+        __syncwarp();
+        if (cwrap) C = test_tile<true>(S, fill, C, g, s, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
+        else C = test_tile<false>(S, fill, C, g, s, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
+        fill = 0;
+        cwrap = false;
+        __syncwarp();
+    };
+
+    const uint32_t e0 = a.off[leaf], e1 = a.off[leaf + 1];
+    uint32_t ent = (e0 < e1) ? a.list[e0] : 0u;
+    float4 pj = (e0 < e1) ? a.posh[(int64_t)(ent & CRK_LEAF_MASK) * CRK_LEAF + lane] : make_float4(0, 0, 0, 0);
+    for (uint32_t e = e0; e < e1; ++e) {
+        const uint32_t cur = ent;
+        const float4 pc = pj;
+        if (e + 1 < e1) {   // prefetch the next leaf's positions
+            ent = a.list[e + 1];
+            pj = a.posh[(int64_t)(ent & CRK_LEAF_MASK) * CRK_LEAF + lane];
+        }
+        const int64_t b = (int64_t)(cur & CRK_LEAF_MASK);
+        const bool wrap = (cur & CRK_FLAG_WRAP) != 0;
+        float gx, gy, gz;
+        if (!wrap) {
+            gx = gap1(blo.x, bhi.x, pc.x); gy = gap1(blo.y, bhi.y, pc.y); gz = gap1(blo.z, bhi.z, pc.z);
+        } else {
+            gx = gap1_wrap(blo.x, bhi.x, pc.x, a.L); gy = gap1_wrap(blo.y, bhi.y, pc.y, a.L); gz = gap1_wrap(blo.z, bhi.z, pc.z, a.L);
+        }
+        const float g2 = __fmaf_rn(gz, gz, __fmaf_rn(gy, gy, __fmul_rn(gx, gx)));
+        const bool surv = g2 < fmaxf(hq2, __fmul_rn(pc.w, pc.w));
+        const uint32_t m = __ballot_sync(0xffffffffu, surv);
+        const int cnt = __popc(m);
+        if (cnt == 0) continue;
+        if (fill + cnt > CRK_TCULL) flush();
+        const int slot = fill + __popc(m & lt);
+        if (surv) {
+            S.tile[slot] = pc;
+            S.tidx[slot] = (uint32_t)(b * CRK_LEAF + lane);
+        }
+        cwrap = cwrap || wrap;
+        fill += cnt;
+    }
+    if (fill > 0) flush();
+    if (C > 0) emit();
+    if (prev == 0 && lane == 0) a.seg_first[leaf] = 0u;
+}
+
+__global__ void k_set_u64(unsigned long long* p, unsigned long long v) { *p = v; }
+
+}  // namespace
+
+int crk_build_nbr_lists(crk_ctx* c) {
+    const int64_t nl = c->nl;
+    CRK_TRY(crk_ensure(c, c->seg_first, (size_t)(nl + 1) * sizeof(uint32_t)));
+    // first guess: ~7 KB per leaf at ~60 neighbours; grown to the exact need if the builder reports more
+    if (!c->arena.p) CRK_TRY(crk_ensure(c, c->arena, (size_t)nl * 9216 + 65536));
+    unsigned long long* d_counter = (unsigned long long*)((char*)c->flag.p + 32);
+    unsigned long long* h_counter = (unsigned long long*)((char*)c->h_flag + 32);
+    for (int attempt = 0; attempt < 3; ++attempt) {
+        ListArgs a;
+        a.n = c->n; a.nl = nl; a.L = c->prm.box; a.half = 0.5f * c->prm.box;
+        a.off = (const uint32_t*)c->nbr_off.p; a.list = (const uint32_t*)c->nbr_list.p;
+        a.posh = (const float4*)c->posh.p; a.leaf_lo = (const float4*)c->leaf_lo.p; a.leaf_hi = (const float4*)c->leaf_hi.p;
+        a.arena = (uint4*)c->arena.p;
+        a.arena_cap = (unsigned long long)(c->arena.cap / 16);
+        if (a.arena_cap > 0xffffffffull) a.arena_cap = 0xffffffffull;      // segment links are 32-bit unit indices (64 GB)
+        a.counter = d_counter;
+        a.seg_first = (uint32_t*)c->seg_first.p;
+        k_set_u64<<<1, 1, 0, c->stream>>>(d_counter, 1ull);
+        CRK_TRY(crk_check_launch(c, "k_set_u64"));
+        k_nbr_lists<<<(unsigned)((nl + LW - 1) / LW), LW * 32, 0, c->stream>>>(a);
+        CRK_TRY(crk_check_launch(c, "k_nbr_lists"));
+        CRK_CUDA(c, cudaMemcpyAsync(h_counter, d_counter, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
+        CRK_CUDA(c, cudaStreamSynchronize(c->stream));
+        const unsigned long long used = *h_counter;
+        if (used <= a.arena_cap) {
+            c->arena_units = (int64_t)used;
+            return CRK_OK;
+        }
+        if (used > 0xffffffffull) {
+            snprintf(c->err, sizeof(c->err), "neighbour lists need %llu 16-byte units (> 2^32): too many pairs for one context", used);
+            return CRK_ENOMEM;
+        }
+        CRK_TRY(crk_ensure(c, c->arena, (size_t)used * 16 + 65536));
+    }
+    snprintf(c->err, sizeof(c->err), "neighbour-list arena did not converge");
+    return CRK_ECUDA;
+}

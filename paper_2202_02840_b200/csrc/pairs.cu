@@ -1,40 +1,34 @@
 // pairs.cu -- steps a1..a5: the four pair sweeps of one CRKSPH derivative evaluation (FP32 pair math on the FMA pipes).
 //
-// Common structure (one warp = one 32-particle leaf, one lane = one particle i, state of i in registers):
-//   for each neighbour leaf b of the leaf interaction list (tree.cu):
-//     cull    lane l takes particle l of b and tests it against the bounding box of the warp's own leaf (point-to-box gap
-//             vs the leaf's hmax, same monotone float sequence as the predicate, so nothing is lost); survivors are
-//             compacted (ballot + prefix popc) into a warp-private shared-memory tile of CAP slots, all planes
-//   when the tile is full (and at the end):
-//     test    every staged j against the lane's i with the prescribed FP32 predicate (S3); all lanes read the
-//             same j (shared-memory broadcast); accepted slots are appended to a per-lane byte queue
-//     drain   each lane walks its own queue and evaluates the pair math only for accepted pairs (lane divergence is
-//             limited to the spread of queue lengths over one tile instead of the few-% acceptance rate)
+// All sweeps walk the neighbour lists built once per crk_build_cells (lists.cu).  A leaf (32 particles) is served by WPL
+// warps; lane l of each of them holds particle i = 32*leaf + l in registers.  Per segment of the leaf's chain:
+//   stage   the WPL warps copy the j-state planes of the segment's C candidates into a shared-memory tile, slot = candidate
+//   drain   warp wl takes rows wl, wl+WPL, ... of the ELL block; row k holds the k-th entry of every lane, so each lane
+//           evaluates one accepted pair per row with j-state fetched from the tile (entries are prefetched 4 rows ahead)
+// and at the end the WPL partial sums of a lane are added in fixed warp order (deterministic) before the epilogue.
+// No candidate is tested here: set membership was decided by the builder with the prescribed predicate (S3).
 // Equation numbers refer to /root/reference/PAPER.md; the closed forms of A, B, grad A, grad B are derived in DESIGN.md.
 #include "crk_internal.cuh"
 
 namespace {
 
-constexpr int WPC = 4;                       // warps (= leaves) per CTA
 constexpr float SIGMA_C4 = 4.923856051905513f;     // 495 / (32 pi), Eq. 12
 constexpr float C35_3 = 35.0f / 3.0f;
 constexpr float C56_3 = 56.0f / 3.0f;
 constexpr float R2_TINY = 1.0e-37f;
+constexpr int FPL = 9;                             // j-state planes of the force sweep
 
 struct SweepArgs {
     int64_t n, nl;
     float L, half;
-    const uint32_t* __restrict__ off;     // leaf list CSR offsets [nl+1]
-    const uint32_t* __restrict__ list;    // entries: leaf | flags
+    const uint4* __restrict__ arena;      // neighbour-list segments
+    const uint32_t* __restrict__ seg_first;
     const int32_t* __restrict__ perm;     // sorted slot -> caller index
     const float4* __restrict__ posh;      // (x,y,z,h)
-    const float4* __restrict__ leaf_lo;   // per leaf: (xlo,ylo,zlo,hmax)
-    const float4* __restrict__ leaf_hi;   // per leaf: (xhi,yhi,zhi,hmin)
     float4* __restrict__ posV;            // (x,y,z,V)
     float4* __restrict__ velV;            // (vx,vy,vz,V)
-    float4* __restrict__ thermo;          // (P,rho,cs,1/h)
-    float4* __restrict__ coef;            // 4 planes, stride np
-    float4* __restrict__ gv;              // 3 planes, stride np
+    float4* __restrict__ coef;            // 4 planes, stride np: (A,B) (c,M0) (M1..M4) (M5..M8)
+    float4* __restrict__ fst;             // FPL planes, stride np: force-sweep state (layout at k_forces)
     float* __restrict__ rho_s;
     const float* __restrict__ m_s;
     int64_t np;                           // padded particle count nl*32 (plane stride)
@@ -44,131 +38,122 @@ struct SweepArgs {
     uint32_t* __restrict__ ocnt;
 };
 
-__device__ __forceinline__ float wrap1(float d, float L, float half) {
-    return d > half ? __fsub_rn(d, L) : (d < -half ? __fadd_rn(d, L) : d);
+struct Seg {
+    const uint32_t* cand;
+    const uint16_t* ell;
+    int C, Kg, K, cg, ct;
+    uint32_t next;
+};
+__device__ __forceinline__ Seg load_seg(const uint4* __restrict__ arena, uint32_t unit, int lane) {
+    const uint4* hdr = arena + unit;
+    const uint4 h0 = __ldg(hdr);
+    Seg s;
+    s.next = h0.x;
+    s.C = (int)(h0.y & 0xffffu);
+    s.Kg = (int)(h0.y >> 16);
+    s.K = (int)h0.z;
+    s.cg = (int)__ldg((const uint16_t*)(hdr + 1) + lane);
+    s.ct = (int)__ldg((const uint16_t*)(hdr + 5) + lane);
+    s.cand = (const uint32_t*)(hdr + CRK_SEG_HDR_UNITS);
+    s.ell = (const uint16_t*)(hdr + CRK_SEG_HDR_UNITS + ((s.C + 3) >> 2));
+    return s;
 }
 
-// ---- culling helpers: lower bound of |wrap(x_i - x_j)| on one axis for x_i in [lo,hi] (monotone float ops) -------
-__device__ __forceinline__ float gap1(float lo, float hi, float x) {
-    return fmaxf(0.f, fmaxf(__fsub_rn(lo, x), __fsub_rn(x, hi)));
-}
-__device__ __forceinline__ float gap1_wrap(float lo, float hi, float x, float L) {
-    const float dmin = __fsub_rn(lo, x), dmax = __fsub_rn(hi, x);     // d = x_i - x_j ranges over [dmin, dmax]
-    const float g0 = fmaxf(0.f, fmaxf(dmin, -dmax));
-    const float gp = fmaxf(0.f, fmaxf(__fsub_rn(L, dmax), __fsub_rn(dmin, L)));
-    const float gm = fmaxf(0.f, fmaxf(__fadd_rn(dmin, L), __fsub_rn(-L, dmax)));
-    return fminf(g0, fminf(gp, gm));
+template <int WPL>
+__device__ __forceinline__ void group_sync(int lg) {
+    if (WPL == 1) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" ::"r"(lg + 1), "r"(WPL * 32) : "memory");
 }
 
-// ---- test phase: append accepted slots to the lane's byte queue; returns queue length -------------------------------
-// SYM = false: gather predicate r2 < h_i^2 (Eqs. 13-14: W_ij = W(|x_i-x_j|, h_i));   SYM = true: r2 < max(h_i^2,h_j^2)
-template <bool SYM>
-__device__ __forceinline__ int test_slots(const SweepArgs& a, int fill4, bool wrap, int self_slot, int lane, float xi,
-                                          float yi, float zi, float hi2, const float4* tile, uint8_t* queue) {
-    uint8_t* qp = queue + lane;
-    if (!wrap) {
-#pragma unroll 1
-        for (int s = 0; s < fill4; s += 4) {
+// ---- the sweep over one leaf's segment chain -------------------------------------------------------------------------
+// SYM = false: rows [0, Kg), lane active while k < cnt_g (gather set, Eqs. 13-14);  SYM = true: rows [0, K), k < cnt.
+// pair(slot, crosses_boundary) evaluates one accepted pair; returns the number of entries the lane owns (= its count).
+template <int WPL, int PLANES, bool SYM, typename Pair>
+__device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4* const* planes, int64_t leaf, int lg, int wl,
+                                               int lane, float4* tile, Pair pair) {
+    constexpr int NQ = (PLANES >= 4) ? 1 : 4;                  // candidates per thread in flight while staging
+    uint32_t count = 0;
+    const int tg = wl * 32 + lane;
+    for (uint32_t unit = __ldg(a.seg_first + leaf); unit != 0u;) {
+        const Seg s = load_seg(a.arena, unit, lane);
+        group_sync<WPL>(lg);                                   // the previous segment's drain is finished
+        for (int c0 = 0; c0 < s.C; c0 += WPL * 32 * NQ) {
+            uint32_t j[NQ];
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                const float4 pj = tile[s + u];
-                const float dx = __fsub_rn(xi, pj.x), dy = __fsub_rn(yi, pj.y), dz = __fsub_rn(zi, pj.z);
-                const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-                const float lim = SYM ? fmaxf(hi2, __fmul_rn(pj.w, pj.w)) : hi2;
-                if (r2 < lim && (s + u) != self_slot) {
-                    *qp = (uint8_t)(s + u);
-                    qp += 32;
+            for (int q = 0; q < NQ; ++q) {
+                const int c = c0 + q * WPL * 32 + tg;
+                j[q] = (c < s.C) ? __ldg(s.cand + c) : 0u;
+            }
+            float4 v[NQ][PLANES];
+#pragma unroll
+            for (int q = 0; q < NQ; ++q)
+#pragma unroll
+                for (int p = 0; p < PLANES; ++p) v[q][p] = __ldg(planes[p] + j[q]);
+#pragma unroll
+            for (int q = 0; q < NQ; ++q) {
+                const int c = c0 + q * WPL * 32 + tg;
+                if (c < s.C) {
+#pragma unroll
+                    for (int p = 0; p < PLANES; ++p) tile[p * CRK_CCAP + c] = v[q][p];
                 }
             }
         }
-    } else {
-#pragma unroll 1
-        for (int s = 0; s < fill4; ++s) {
-            const float4 pj = tile[s];
-            const float dx0 = __fsub_rn(xi, pj.x), dy0 = __fsub_rn(yi, pj.y), dz0 = __fsub_rn(zi, pj.z);
-            const float dx = wrap1(dx0, a.L, a.half), dy = wrap1(dy0, a.L, a.half), dz = wrap1(dz0, a.L, a.half);
-            const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-            const float lim = SYM ? fmaxf(hi2, __fmul_rn(pj.w, pj.w)) : hi2;
-            if (r2 < lim && s != self_slot) {
-                const bool wrapped = (dx != dx0) || (dy != dy0) || (dz != dz0);
-                *qp = (uint8_t)(s | (wrapped ? 0x80 : 0));    // bit 7: pair crosses the periodic boundary
-                qp += 32;
-            }
+        group_sync<WPL>(lg);
+        const int rows = SYM ? s.K : s.Kg;
+        const int mine = SYM ? s.ct : s.cg;
+        const uint16_t* ep = s.ell + lane;
+        uint32_t e[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int k = wl + q * WPL;
+            e[q] = (k < rows) ? (uint32_t)__ldg(ep + k * 32) : 0u;
         }
+        for (int k0 = wl; k0 < rows; k0 += 4 * WPL) {
+            uint32_t nx[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int k = k0 + (4 + q) * WPL;
+                nx[q] = (k < rows) ? (uint32_t)__ldg(ep + k * 32) : 0u;
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int k = k0 + q * WPL;
+                if (k < mine) pair((int)(e[q] & CRK_ELL_MASK), (e[q] & CRK_ELL_WRAP) != 0u);
+            }
+#pragma unroll
+            for (int q = 0; q < 4; ++q) e[q] = nx[q];
+        }
+        count += (uint32_t)mine;
+        unit = s.next;
     }
-    return (int)(qp - (queue + lane)) >> 5;
+    return count;
 }
 
-// ---- the sweep: cull + compact survivors of each neighbour leaf into the tile, test + drain when it fills ---------
-template <int CAP, int PLANES, bool SYM, typename Drain>
-__device__ __forceinline__ void sweep_loop(const SweepArgs& a, const float4* const (&planes)[PLANES], int64_t leaf,
-                                           int lane, float xi, float yi, float zi, float hi2, float4* tile,
-                                           uint8_t* queue, Drain drain) {
-    static_assert(CAP <= 128 && CAP % 32 == 0, "queue entries keep bit 7 for the periodic-wrap mark");
-    const float4 blo = a.leaf_lo[leaf], bhi = a.leaf_hi[leaf];
-    const float hq2 = __fmul_rn(blo.w, blo.w);
-    const uint32_t lt = (1u << lane) - 1u;
-    int fill = 0, self_slot = -1;
-    bool cwrap = false;
-    const uint32_t e0 = a.off[leaf], e1 = a.off[leaf + 1];
-    auto flush = [&]() {
-        const int fill4 = (fill + 3) & ~3;
-        if (lane < fill4 - fill) tile[fill + lane] = make_float4(3.0e30f, 3.0e30f, 3.0e30f, 0.0f);   // never accepted
-        __syncwarp();
-        const int cnt = test_slots<SYM>(a, fill4, cwrap, self_slot, lane, xi, yi, zi, hi2, tile, queue);
-        drain(cnt);
-        __syncwarp();
-        fill = 0;
-        self_slot = -1;
-        cwrap = false;
-    };
-    uint32_t ent = (e0 < e1) ? a.list[e0] : 0u;
-    float4 pj = (e0 < e1) ? planes[0][(int64_t)(ent & CRK_LEAF_MASK) * CRK_LEAF + lane] : make_float4(0, 0, 0, 0);
-    for (uint32_t e = e0; e < e1; ++e) {
-        const uint32_t cur = ent;
-        const float4 pc = pj;
-        if (e + 1 < e1) {   // prefetch the next leaf's positions
-            ent = a.list[e + 1];
-            pj = planes[0][(int64_t)(ent & CRK_LEAF_MASK) * CRK_LEAF + lane];
-        }
-        if (!SYM && !(cur & CRK_FLAG_GATHER)) continue;
-        const int64_t b = (int64_t)(cur & CRK_LEAF_MASK);
-        const int64_t g = b * CRK_LEAF + lane;
-        const bool wrap = (cur & CRK_FLAG_WRAP) != 0;
-        float gx, gy, gz;
-        if (!wrap) {
-            gx = gap1(blo.x, bhi.x, pc.x); gy = gap1(blo.y, bhi.y, pc.y); gz = gap1(blo.z, bhi.z, pc.z);
-        } else {
-            gx = gap1_wrap(blo.x, bhi.x, pc.x, a.L); gy = gap1_wrap(blo.y, bhi.y, pc.y, a.L); gz = gap1_wrap(blo.z, bhi.z, pc.z, a.L);
-        }
-        const float g2 = __fmaf_rn(gz, gz, __fmaf_rn(gy, gy, __fmul_rn(gx, gx)));
-        const float lim = SYM ? fmaxf(hq2, __fmul_rn(pc.w, pc.w)) : hq2;
-        const bool surv = g2 < lim;
-        const uint32_t m = __ballot_sync(0xffffffffu, surv);
-        const int cnt = __popc(m);
-        if (cnt == 0) continue;
-        if (fill + cnt > CAP) flush();
-        const int slot = fill + __popc(m & lt);
-        if (surv) {
-            tile[slot] = pc;
+// add the WPL partial sums of each lane in warp order; the result lands in warp 0 of the group
+template <int WPL, int NACC>
+__device__ __forceinline__ void group_reduce(float (&acc)[NACC], int lg, int wl, int lane, float* red) {
+    if (WPL == 1) return;
+    group_sync<WPL>(lg);                                       // the tile is no longer read: reuse it
+    if (wl > 0) {
 #pragma unroll
-            for (int p = 1; p < PLANES; ++p) tile[p * CAP + slot] = planes[p][g];
-        }
-        if (b == leaf) self_slot = surv ? slot : -1;
-        cwrap = cwrap || wrap;
-        fill += cnt;
+        for (int q = 0; q < NACC; ++q) red[((wl - 1) * NACC + q) * 32 + lane] = acc[q];
     }
-    if (fill > 0) flush();
+    group_sync<WPL>(lg);
+    if (wl == 0) {
+        for (int w2 = 1; w2 < WPL; ++w2)
+#pragma unroll
+            for (int q = 0; q < NACC; ++q) acc[q] += red[((w2 - 1) * NACC + q) * 32 + lane];
+    }
 }
 
 // Wendland C4 (Eq. 12) without its sigma/h^3 prefactor, and D~ with W'/r = sigma h^-5 D~:
 //   W~ = (1-eta)^6 (1 + 6 eta + 35/3 eta^2),   D~ = -(56/3) (1-eta)^5 (1 + 5 eta)
 __device__ __forceinline__ void wendland(float eta, float& Wt, float& Dt) {
-    const float t = fmaxf(1.0f - eta, 0.0f);
-    const float t2 = t * t;
-    const float t5 = t2 * t2 * t;
-    Wt = t5 * t * fmaf(eta, fmaf(eta, C35_3, 6.0f), 1.0f);
-    Dt = -C56_3 * t5 * fmaf(5.0f, eta, 1.0f);
+    const float t = fmaxf(__fsub_rn(1.0f, eta), 0.0f);
+    const float t2 = __fmul_rn(t, t);
+    const float t5 = __fmul_rn(__fmul_rn(t2, t2), t);
+    Wt = __fmul_rn(__fmul_rn(t5, t), __fmaf_rn(eta, __fmaf_rn(eta, C35_3, 6.0f), 1.0f));
+    Dt = __fmul_rn(__fmul_rn(-C56_3, t5), __fmaf_rn(5.0f, eta, 1.0f));
 }
 __device__ __forceinline__ float wendland_w(float eta) {
     const float t = fmaxf(1.0f - eta, 0.0f);
@@ -176,8 +161,8 @@ __device__ __forceinline__ float wendland_w(float eta) {
     return t2 * t2 * t2 * fmaf(eta, fmaf(eta, C35_3, 6.0f), 1.0f);
 }
 
-// Separation of an accepted pair for the VALUES (the set membership was decided by the prescribed predicate above).
-// Plain pairs: d = x_i - x_j.  Pairs that cross the periodic boundary (queue bit 7): shift the coordinate that lies in
+// Separation of an accepted pair for the VALUES (the set membership was decided by the prescribed predicate).
+// Plain pairs: d = x_i - x_j.  Pairs that cross the periodic boundary (entry bit 15): shift the coordinate that lies in
 // the upper half of the box by -L first (exact, Sterbenz) and subtract afterwards, so that the rounding error is
 // relative to |d| and not to L  (fl(x_i - x_j) ~ 1 - 1e-3 would lose 1e-5 of a 4e-3 separation).
 __device__ __forceinline__ float sep1_wrapped(float xi, float xj, float L, float half) {
@@ -200,46 +185,28 @@ __device__ __forceinline__ void sep3(const SweepArgs& a, bool wrapped, float xi,
     r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
 }
 
-template <int CAP, int PLANES>
-struct Smem {
-    static constexpr int TILE_F4 = PLANES * CAP;
-    static constexpr int QUEUE_B = CAP * 32;
-    static constexpr int PER_WARP = TILE_F4 * 16 + QUEUE_B;
-};
-
 // =================================================================================================== a1: volumes
 // Eq. 14: V_i^-1 = n_i = sum_j W(|x_i - x_j|, h_i), self term included (S4); rho_i = m_i / V_i (S2).
-constexpr int CH1 = 128;   // tile capacity (slots)
-__global__ void __launch_bounds__(WPC * 32) k_volumes(SweepArgs a) {
+constexpr int W1_WPC = 4;
+__global__ void __launch_bounds__(W1_WPC * 32) k_volumes(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    using S = Smem<CH1, 1>;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int64_t leaf = (int64_t)blockIdx.x * WPC + w;
+    const int64_t leaf = (int64_t)blockIdx.x * W1_WPC + w;
     if (leaf >= a.nl) return;
-    float4* tile = (float4*)(smem_raw + (size_t)w * S::PER_WARP);
-    uint8_t* queue = (uint8_t*)(tile + S::TILE_F4);
+    float4* tile = (float4*)smem_raw + (size_t)w * CRK_CCAP;
     const int64_t i = leaf * CRK_LEAF + lane;
     const bool valid = i < a.n;
     const float4 pi = a.posh[i];
     const float xi = pi.x, yi = pi.y, zi = pi.z, hi = pi.w;
-    const float hi2 = __fmul_rn(hi, hi);
     const float inv_h = valid ? 1.0f / hi : 0.0f;
     float acc = 0.0f;
-    uint32_t count = 0;
     const float4* const planes[1] = {a.posh};
-    sweep_loop<CH1, 1, false>(a, planes, leaf, lane, xi, yi, zi, hi2, tile, queue, [&](int cnt) {
-        const int maxc = __reduce_max_sync(0xffffffffu, cnt);
-        for (int s = 0; s < maxc; ++s) {
-            if (s < cnt) {
-                const int qe = queue[s * 32 + lane];
-                const float4 pj = tile[qe & 0x7f];
-                float dx, dy, dz, r2;
-                sep3(a, (qe & 0x80) != 0, xi, yi, zi, pj, dx, dy, dz, r2);
-                const float r = r2 * rsqrtf(fmaxf(r2, R2_TINY));
-                acc += wendland_w(r * inv_h);
-            }
-        }
-        count += cnt;
+    const uint32_t count = leaf_sweep<1, 1, false>(a, planes, leaf, w, 0, lane, tile, [&](int c, bool wrapped) {
+        const float4 pj = tile[c];
+        float dx, dy, dz, r2;
+        sep3(a, wrapped, xi, yi, zi, pj, dx, dy, dz, r2);
+        const float r = r2 * rsqrtf(fmaxf(r2, R2_TINY));
+        acc += wendland_w(r * inv_h);
     });
     if (valid) {
         const float k3 = SIGMA_C4 * inv_h * inv_h * inv_h;
@@ -266,20 +233,17 @@ __global__ void __launch_bounds__(WPC * 32) k_volumes(SweepArgs a) {
 //   (g = V_j W'_ij / r):   B = -m2^-1 m1,  A = 1/(m0 + B.m1),
 //   d_c A = -A^2 (d_c m0 + 2 B.d_c m1 + B^T d_c m2 B),  d_c B = -m2^-1 (d_c m1 + d_c m2 B).
 // 29 FP32 sums per particle in eta-normalised units, then an FP64 3x3 solve per particle.
-constexpr int CH2 = 128;
-__global__ void __launch_bounds__(WPC * 32) k_moments(SweepArgs a) {
+constexpr int W2_WPC = 4;
+__global__ void __launch_bounds__(W2_WPC * 32) k_moments(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    using S = Smem<CH2, 1>;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int64_t leaf = (int64_t)blockIdx.x * WPC + w;
+    const int64_t leaf = (int64_t)blockIdx.x * W2_WPC + w;
     if (leaf >= a.nl) return;
-    float4* tile = (float4*)(smem_raw + (size_t)w * S::PER_WARP);
-    uint8_t* queue = (uint8_t*)(tile + S::TILE_F4);
+    float4* tile = (float4*)smem_raw + (size_t)w * CRK_CCAP;
     const int64_t i = leaf * CRK_LEAF + lane;
     const bool valid = i < a.n;
     const float4 ph = a.posh[i];
     const float xi = ph.x, yi = ph.y, zi = ph.z, hi = ph.w;
-    const float hi2 = __fmul_rn(hi, hi);
     const float inv_h = valid ? 1.0f / hi : 0.0f;
     // accumulators: s0; s1[3]; s2[6] (xx,xy,xz,yy,yz,zz); t0[3]; t1[6]; t2[10] (xxx,xxy,xxz,xyy,xyz,xzz,yyy,yyz,yzz,zzz)
     float s0 = 0.f, s1x = 0.f, s1y = 0.f, s1z = 0.f;
@@ -288,33 +252,27 @@ __global__ void __launch_bounds__(WPC * 32) k_moments(SweepArgs a) {
     float txx = 0.f, txy = 0.f, txz = 0.f, tyy = 0.f, tyz = 0.f, tzz = 0.f;
     float c0 = 0.f, c1 = 0.f, c2 = 0.f, c3 = 0.f, c4 = 0.f, c5 = 0.f, c6 = 0.f, c7 = 0.f, c8 = 0.f, c9 = 0.f;
     const float4* const planes[1] = {a.posV};
-    sweep_loop<CH2, 1, false>(a, planes, leaf, lane, xi, yi, zi, hi2, tile, queue, [&](int cnt) {
-        const int maxc = __reduce_max_sync(0xffffffffu, cnt);
-        for (int s = 0; s < maxc; ++s) {
-            if (s < cnt) {
-                const int qe = queue[s * 32 + lane];
-                const float4 pj = tile[qe & 0x7f];
-                float dx, dy, dz, r2;
-                sep3(a, (qe & 0x80) != 0, xi, yi, zi, pj, dx, dy, dz, r2);
-                const float r = r2 * rsqrtf(fmaxf(r2, R2_TINY));
-                float Wt, Dt;
-                wendland(r * inv_h, Wt, Dt);
-                const float wv = pj.w * Wt, gv = pj.w * Dt;
-                const float x = dx * inv_h, y = dy * inv_h, z = dz * inv_h;
-                const float xx = x * x, xy = x * y, xz = x * z, yy = y * y, yz = y * z, zz = z * z;
-                s0 += wv;
-                s1x = fmaf(wv, x, s1x); s1y = fmaf(wv, y, s1y); s1z = fmaf(wv, z, s1z);
-                sxx = fmaf(wv, xx, sxx); sxy = fmaf(wv, xy, sxy); sxz = fmaf(wv, xz, sxz);
-                syy = fmaf(wv, yy, syy); syz = fmaf(wv, yz, syz); szz = fmaf(wv, zz, szz);
-                t0x = fmaf(gv, x, t0x); t0y = fmaf(gv, y, t0y); t0z = fmaf(gv, z, t0z);
-                txx = fmaf(gv, xx, txx); txy = fmaf(gv, xy, txy); txz = fmaf(gv, xz, txz);
-                tyy = fmaf(gv, yy, tyy); tyz = fmaf(gv, yz, tyz); tzz = fmaf(gv, zz, tzz);
-                c0 = fmaf(gv, xx * x, c0); c1 = fmaf(gv, xx * y, c1); c2 = fmaf(gv, xx * z, c2);
-                c3 = fmaf(gv, xy * y, c3); c4 = fmaf(gv, xy * z, c4); c5 = fmaf(gv, xz * z, c5);
-                c6 = fmaf(gv, yy * y, c6); c7 = fmaf(gv, yy * z, c7); c8 = fmaf(gv, yz * z, c8);
-                c9 = fmaf(gv, zz * z, c9);
-            }
-        }
+    leaf_sweep<1, 1, false>(a, planes, leaf, w, 0, lane, tile, [&](int c, bool wrapped) {
+        const float4 pj = tile[c];
+        float dx, dy, dz, r2;
+        sep3(a, wrapped, xi, yi, zi, pj, dx, dy, dz, r2);
+        const float r = r2 * rsqrtf(fmaxf(r2, R2_TINY));
+        float Wt, Dt;
+        wendland(r * inv_h, Wt, Dt);
+        const float wv = pj.w * Wt, gv = pj.w * Dt;
+        const float x = dx * inv_h, y = dy * inv_h, z = dz * inv_h;
+        const float xx = x * x, xy = x * y, xz = x * z, yy = y * y, yz = y * z, zz = z * z;
+        s0 += wv;
+        s1x = fmaf(wv, x, s1x); s1y = fmaf(wv, y, s1y); s1z = fmaf(wv, z, s1z);
+        sxx = fmaf(wv, xx, sxx); sxy = fmaf(wv, xy, sxy); sxz = fmaf(wv, xz, sxz);
+        syy = fmaf(wv, yy, syy); syz = fmaf(wv, yz, syz); szz = fmaf(wv, zz, szz);
+        t0x = fmaf(gv, x, t0x); t0y = fmaf(gv, y, t0y); t0z = fmaf(gv, z, t0z);
+        txx = fmaf(gv, xx, txx); txy = fmaf(gv, xy, txy); txz = fmaf(gv, xz, txz);
+        tyy = fmaf(gv, yy, tyy); tyz = fmaf(gv, yz, tyz); tzz = fmaf(gv, zz, tzz);
+        c0 = fmaf(gv, xx * x, c0); c1 = fmaf(gv, xx * y, c1); c2 = fmaf(gv, xx * z, c2);
+        c3 = fmaf(gv, xy * y, c3); c4 = fmaf(gv, xy * z, c4); c5 = fmaf(gv, xz * z, c5);
+        c6 = fmaf(gv, yy * y, c6); c7 = fmaf(gv, yy * z, c7); c8 = fmaf(gv, yz * z, c8);
+        c9 = fmaf(gv, zz * z, c9);
     });
     float4 o0 = make_float4(0, 0, 0, 0), o1 = o0, o2 = o0, o3 = o0;
     if (valid) {
@@ -408,27 +366,26 @@ __global__ void __launch_bounds__(WPC * 32) k_moments(SweepArgs a) {
     a.coef[3 * a.np + i] = o3;
 }
 
-// ---- hydro preparation: sorted (vx,vy,vz,V) and (P, rho, c_s, 1/h) ------------------------------------------------
+// ---- hydro preparation: sorted (vx,vy,vz,V), and force-sweep plane 0 = (x,y,z,1/h) -----------------------------------
 __global__ void __launch_bounds__(256) k_pack_vel(const float* __restrict__ vx, const float* __restrict__ vy,
                                                   const float* __restrict__ vz, const float* __restrict__ u, int64_t n,
                                                   float4* __restrict__ out) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) out[i] = make_float4(vx[i], vy[i], vz[i], u[i]);
 }
-// Eq. 4: P = (gamma-1) rho u (unclamped);  c_s = sqrt(gamma P / rho) = sqrt(gamma (gamma-1) max(u,0))  (S12)
-__global__ void __launch_bounds__(256) k_hydro_prep(SweepArgs a, const float4* __restrict__ vel_orig) {
+__global__ void __launch_bounds__(256) k_hydro_prep(SweepArgs a, const float4* __restrict__ vel_orig, float* __restrict__ u_s) {
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= a.np) return;
+    const float4 ph = a.posh[k];
     if (k < a.n) {
         const float4 v = vel_orig[a.perm[k]];
-        const float V = a.posV[k].w;
-        const float rho = a.rho_s[k];
-        const float g = a.gamma;
-        a.velV[k] = make_float4(v.x, v.y, v.z, V);
-        a.thermo[k] = make_float4((g - 1.0f) * rho * v.w, rho, sqrtf(g * (g - 1.0f) * fmaxf(v.w, 0.0f)), 1.0f / a.posh[k].w);
+        a.velV[k] = make_float4(v.x, v.y, v.z, a.posV[k].w);
+        u_s[k] = v.w;
+        a.fst[k] = make_float4(ph.x, ph.y, ph.z, 1.0f / ph.w);
     } else {
         a.velV[k] = make_float4(0, 0, 0, 0);
-        a.thermo[k] = make_float4(0, 0, 0, 0);
+        u_s[k] = 0.0f;
+        a.fst[k] = make_float4(ph.x, ph.y, ph.z, 0.0f);
     }
 }
 
@@ -462,166 +419,177 @@ __device__ __forceinline__ void rk_grad(const Coef& k, float x, float y, float z
 __device__ __forceinline__ float visc_Q(float rho, float cs, float mu, float Cl, float Cq) {
     return __fmul_rn(__fmul_rn(rho, mu), __fmaf_rn(Cq, mu, -__fmul_rn(Cl, cs)));
 }
-// dimensional W and D = W'/r for support h (k3 = sigma/h^3, ih = 1/h)
-__device__ __forceinline__ void wendland_dim(float r, float ih, float k3, float& W, float& D) {
+// dimensional W and D = W'/r for support h:  k3 = sigma/h^3, k5 = sigma/h^5, ih = 1/h
+__device__ __forceinline__ void wendland_dim(float r, float ih, float k3, float k5, float& W, float& D) {
     float Wt, Dt;
     wendland(__fmul_rn(r, ih), Wt, Dt);
     W = __fmul_rn(k3, Wt);
-    D = __fmul_rn(__fmul_rn(__fmul_rn(k3, ih), ih), Dt);
+    D = __fmul_rn(k5, Dt);
 }
 
 // =============================================================================================== a4: velocity gradient
-// Eq. 26: grad v_i = - sum_j V_j (v_i - v_j) (x) grad WR_ij   over the gather set; index [3a+b] = d_b v^a
-constexpr int CH4 = 128;
-__global__ void __launch_bounds__(WPC * 32) k_gradv(SweepArgs a) {
+// Eq. 26: grad v_i = - sum_j V_j (v_i - v_j) (x) grad WR_ij   over the gather set; index [3a+b] = d_b v^a.
+// The epilogue also forms P = (gamma-1) rho u (Eq. 4, unclamped) and c_s = sqrt(gamma (gamma-1) max(u,0)) (S12) and writes
+// the packed force-sweep state of the particle.
+constexpr int W4_WPL = 2, W4_LPC = 2;
+__global__ void __launch_bounds__(W4_WPL * W4_LPC * 32) k_gradv(SweepArgs a, const float* __restrict__ u_s) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    using S = Smem<CH4, 2>;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int64_t leaf = (int64_t)blockIdx.x * WPC + w;
+    const int lg = w / W4_WPL, wl = w % W4_WPL;
+    const int64_t leaf = (int64_t)blockIdx.x * W4_LPC + lg;
     if (leaf >= a.nl) return;
-    float4* tile = (float4*)(smem_raw + (size_t)w * S::PER_WARP);
-    uint8_t* queue = (uint8_t*)(tile + S::TILE_F4);
+    float4* tile = (float4*)smem_raw + (size_t)lg * 2 * CRK_CCAP;
     const int64_t i = leaf * CRK_LEAF + lane;
     const bool valid = i < a.n;
     const float4 ph = a.posh[i];
     const float xi = ph.x, yi = ph.y, zi = ph.z, hi = ph.w;
-    const float hi2 = __fmul_rn(hi, hi);
     const float ih = valid ? 1.0f / hi : 0.0f;
     const float k3 = SIGMA_C4 * ih * ih * ih;
+    const float k5 = k3 * ih * ih;
     const float4 vi = a.velV[i];
-    const Coef ci = load_coef(a.coef[i], a.coef[a.np + i], a.coef[2 * a.np + i], a.coef[3 * a.np + i]);
+    const float4 q0 = a.coef[i], q1 = a.coef[a.np + i], q2 = a.coef[2 * a.np + i], q3 = a.coef[3 * a.np + i];
+    const Coef ci = load_coef(q0, q1, q2, q3);
     float g[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
-    const float4* const planes[2] = {a.posh, a.velV};
-    sweep_loop<CH4, 2, false>(a, planes, leaf, lane, xi, yi, zi, hi2, tile, queue, [&](int cnt) {
-        const int maxc = __reduce_max_sync(0xffffffffu, cnt);
-        for (int s = 0; s < maxc; ++s) {
-            if (s < cnt) {
-                const int qe = queue[s * 32 + lane];
-                const int jj = qe & 0x7f;
-                const float4 pj = tile[jj];
-                const float4 vj = tile[CH4 + jj];
-                float dx, dy, dz, r2;
-                sep3(a, (qe & 0x80) != 0, xi, yi, zi, pj, dx, dy, dz, r2);
-                const float r = r2 * rsqrtf(fmaxf(r2, R2_TINY));
-                float W, D, gx, gy, gz;
-                wendland_dim(r, ih, k3, W, D);
-                rk_grad(ci, dx, dy, dz, W, D, gx, gy, gz);
-                const float Vj = vj.w;
-                const float ux = Vj * (vi.x - vj.x), uy = Vj * (vi.y - vj.y), uz = Vj * (vi.z - vj.z);
-                g[0] = fmaf(-ux, gx, g[0]); g[1] = fmaf(-ux, gy, g[1]); g[2] = fmaf(-ux, gz, g[2]);
-                g[3] = fmaf(-uy, gx, g[3]); g[4] = fmaf(-uy, gy, g[4]); g[5] = fmaf(-uy, gz, g[5]);
-                g[6] = fmaf(-uz, gx, g[6]); g[7] = fmaf(-uz, gy, g[7]); g[8] = fmaf(-uz, gz, g[8]);
-            }
-        }
+    const float4* const planes[2] = {a.posV, a.velV};
+    leaf_sweep<W4_WPL, 2, false>(a, planes, leaf, lg, wl, lane, tile, [&](int c, bool wrapped) {
+        const float4 pj = tile[c];
+        const float4 vj = tile[CRK_CCAP + c];
+        float dx, dy, dz, r2;
+        sep3(a, wrapped, xi, yi, zi, pj, dx, dy, dz, r2);
+        const float r = r2 * rsqrtf(fmaxf(r2, R2_TINY));
+        float W, D, gx, gy, gz;
+        wendland_dim(r, ih, k3, k5, W, D);
+        rk_grad(ci, dx, dy, dz, W, D, gx, gy, gz);
+        const float Vj = pj.w;
+        const float ux = Vj * (vi.x - vj.x), uy = Vj * (vi.y - vj.y), uz = Vj * (vi.z - vj.z);
+        g[0] = fmaf(-ux, gx, g[0]); g[1] = fmaf(-ux, gy, g[1]); g[2] = fmaf(-ux, gz, g[2]);
+        g[3] = fmaf(-uy, gx, g[3]); g[4] = fmaf(-uy, gy, g[4]); g[5] = fmaf(-uy, gz, g[5]);
+        g[6] = fmaf(-uz, gx, g[6]); g[7] = fmaf(-uz, gy, g[7]); g[8] = fmaf(-uz, gz, g[8]);
     });
-    const float hhat = hi / a.n_h;
-    a.gv[i] = make_float4(g[0], g[1], g[2], g[3]);
-    a.gv[a.np + i] = make_float4(g[4], g[5], g[6], g[7]);
-    a.gv[2 * a.np + i] = make_float4(g[8], k3, hhat, hhat * hhat * a.eps2);
+    group_reduce<W4_WPL, 9>(g, lg, wl, lane, (float*)tile);
+    if (wl != 0) return;
+    // force-sweep state: (x,y,z,1/h) (v,V) | (P,rho,cs,A) (B,cx) (cy,cz,M0,M1) (M2..M5) (M6,M7,M8,g0) (g1..g4) (g5..g8)
+    const float u = u_s[i], rho = a.rho_s[i], gm = a.gamma;
+    const float P = (gm - 1.0f) * rho * u;
+    const float cs = sqrtf(gm * (gm - 1.0f) * fmaxf(u, 0.0f));
+    float4* f = a.fst + i;
+    const int64_t np = a.np;
+    f[2 * np] = make_float4(P, rho, cs, q0.x);
+    f[3 * np] = make_float4(q0.y, q0.z, q0.w, q1.x);
+    f[4 * np] = make_float4(q1.y, q1.z, q1.w, q2.x);
+    f[5 * np] = make_float4(q2.y, q2.z, q2.w, q3.x);
+    f[6 * np] = make_float4(q3.y, q3.z, q3.w, g[0]);
+    f[7 * np] = make_float4(g[1], g[2], g[3], g[4]);
+    f[8 * np] = make_float4(g[5], g[6], g[7], g[8]);
 }
 
 // ============================================================================================ a5: momentum and energy
 // Eq. 17:  m_i dv_i/dt = sum_j (1/2) V_i V_j (P_i+Q_i+P_j+Q_j) (grad WR_ji - grad WR_ij)
 // Eq. 18:  m_i du_i/dt = sum_j (1/2) V_i V_j (P_j+Q_j) (v_j - v_i).(grad WR_ji - grad WR_ij)       (S6)
 // Q from Eqs. 24-25 with the limited midpoint projection of Eqs. 27-32 (S7: division-free van Leer form).
-// Sums over all j != i with r2 < max(h_i^2, h_j^2); each ordered pair is evaluated by the lane that owns i.
-constexpr int CH5 = 64;
-constexpr int PL5 = 10;
-__global__ void __launch_bounds__(WPC * 32) k_forces(SweepArgs a) {
+// Sums over all j != i with r2 < max(h_i^2, h_j^2); each ordered pair is evaluated on a lane that holds i in registers.
+// One CTA = one leaf: W5_WPL warps share the tile of the leaf's candidates and split each lane's entries by rows.
+constexpr int W5_WPL = 8;
+struct PState {           // one particle's force-sweep state in registers
+    float x, y, z, ih, vx, vy, vz, V, P, rho, cs;
+    Coef c;
+    float g[9];
+};
+__device__ __forceinline__ PState load_pstate(const float4* __restrict__ f, int64_t stride) {
+    const float4 a0 = f[0], a1 = f[stride], a2 = f[2 * stride], a3 = f[3 * stride], a4 = f[4 * stride], a5 = f[5 * stride],
+                 a6 = f[6 * stride], a7 = f[7 * stride], a8 = f[8 * stride];
+    PState s;
+    s.x = a0.x; s.y = a0.y; s.z = a0.z; s.ih = a0.w;
+    s.vx = a1.x; s.vy = a1.y; s.vz = a1.z; s.V = a1.w;
+    s.P = a2.x; s.rho = a2.y; s.cs = a2.z; s.c.A = a2.w;
+    s.c.Bx = a3.x; s.c.By = a3.y; s.c.Bz = a3.z; s.c.cx = a3.w;
+    s.c.cy = a4.x; s.c.cz = a4.y; s.c.M[0] = a4.z; s.c.M[1] = a4.w;
+    s.c.M[2] = a5.x; s.c.M[3] = a5.y; s.c.M[4] = a5.z; s.c.M[5] = a5.w;
+    s.c.M[6] = a6.x; s.c.M[7] = a6.y; s.c.M[8] = a6.z; s.g[0] = a6.w;
+    s.g[1] = a7.x; s.g[2] = a7.y; s.g[3] = a7.z; s.g[4] = a7.w;
+    s.g[5] = a8.x; s.g[6] = a8.y; s.g[7] = a8.z; s.g[8] = a8.w;
+    return s;
+}
+__global__ void __launch_bounds__(W5_WPL * 32) k_forces(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    using S = Smem<CH5, PL5>;
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int64_t leaf = (int64_t)blockIdx.x * WPC + w;
-    if (leaf >= a.nl) return;
-    float4* tile = (float4*)(smem_raw + (size_t)w * S::PER_WARP);
-    uint8_t* queue = (uint8_t*)(tile + S::TILE_F4);
+    const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
+    const int64_t leaf = blockIdx.x;
+    float4* tile = (float4*)smem_raw;
     const int64_t i = leaf * CRK_LEAF + lane;
     const bool valid = i < a.n;
-    const float4 ph = a.posh[i];
-    const float xi = ph.x, yi = ph.y, zi = ph.z, hi = ph.w;
-    const float hi2 = __fmul_rn(hi, hi);
-    const float4 vi = a.velV[i];        // vx,vy,vz,V
-    const float4 ti = a.thermo[i];      // P,rho,cs,1/h
-    const Coef ci = load_coef(a.coef[i], a.coef[a.np + i], a.coef[2 * a.np + i], a.coef[3 * a.np + i]);
-    const float4 g0 = a.gv[i], g1 = a.gv[a.np + i], g2 = a.gv[2 * a.np + i];
-    const float gi[9] = {g0.x, g0.y, g0.z, g0.w, g1.x, g1.y, g1.z, g1.w, g2.x};
-    const float k3i = g2.y, hhi = g2.z, he2i = g2.w;
+    const PState I = load_pstate(a.fst + i, a.np);
+    const float k3i = SIGMA_C4 * I.ih * I.ih * I.ih, k5i = k3i * I.ih * I.ih;
+    const float qhi = a.n_h * I.ih;                      // 1 / hhat_i
+    const float qhi2 = qhi * qhi;
     const float eta_crit = 1.0f / a.n_h, inv_fold = a.n_h / 0.2f;
-    float Fx = 0.f, Fy = 0.f, Fz = 0.f, dE = 0.f;
-    uint32_t count = 0;
-    const float4* const planes[PL5] = {a.posh, a.velV, a.thermo, a.coef, a.coef + a.np, a.coef + 2 * a.np,
-                                       a.coef + 3 * a.np, a.gv, a.gv + a.np, a.gv + 2 * a.np};
-    constexpr int PS = CH5;        // plane stride in the tile
-    sweep_loop<CH5, PL5, true>(a, planes, leaf, lane, xi, yi, zi, hi2, tile, queue, [&](int cnt) {
-        const int maxc = __reduce_max_sync(0xffffffffu, cnt);
-        for (int s = 0; s < maxc; ++s) {
-            if (s < cnt) {
-                const int qe = queue[s * 32 + lane];
-                const int jj = qe & 0x7f;
-                const float4 pj = tile[jj];
-                const float4 vj = tile[PS + jj];
-                const float4 tj = tile[2 * PS + jj];
-                const Coef cj = load_coef(tile[3 * PS + jj], tile[4 * PS + jj], tile[5 * PS + jj], tile[6 * PS + jj]);
-                const float4 h0 = tile[7 * PS + jj], h1 = tile[8 * PS + jj], h2 = tile[9 * PS + jj];
-                float dx, dy, dz, r2;
-                sep3(a, (qe & 0x80) != 0, xi, yi, zi, pj, dx, dy, dz, r2);
-                const float r = __fmul_rn(r2, rsqrtf(fmaxf(r2, R2_TINY)));
-                float Wi, Di, Wj, Dj;
-                wendland_dim(r, ti.w, k3i, Wi, Di);
-                wendland_dim(r, tj.w, h2.y, Wj, Dj);
-                float aix, aiy, aiz, ajx, ajy, ajz;
-                rk_grad(ci, dx, dy, dz, Wi, Di, aix, aiy, aiz);            // grad WR_ij
-                rk_grad(cj, -dx, -dy, -dz, Wj, Dj, ajx, ajy, ajz);         // grad WR_ji  (x_ji = -x_ij)
-                const float Gx = __fsub_rn(ajx, aix), Gy = __fsub_rn(ajy, aiy), Gz = __fsub_rn(ajz, aiz);
-                // (grad v . x_ij) for both particles, written so that the mirrored lane forms the same numbers
-                const float wix = __fmaf_rn(gi[2], dz, __fmaf_rn(gi[1], dy, __fmul_rn(gi[0], dx)));
-                const float wiy = __fmaf_rn(gi[5], dz, __fmaf_rn(gi[4], dy, __fmul_rn(gi[3], dx)));
-                const float wiz = __fmaf_rn(gi[8], dz, __fmaf_rn(gi[7], dy, __fmul_rn(gi[6], dx)));
-                const float wjx = __fmaf_rn(h0.z, dz, __fmaf_rn(h0.y, dy, __fmul_rn(h0.x, dx)));
-                const float wjy = __fmaf_rn(h1.y, dz, __fmaf_rn(h1.x, dy, __fmul_rn(h0.w, dx)));
-                const float wjz = __fmaf_rn(h2.x, dz, __fmaf_rn(h1.w, dy, __fmul_rn(h1.z, dx)));
-                const float Nn = __fmaf_rn(dz, wiz, __fmaf_rn(dy, wiy, __fmul_rn(dx, wix)));   // Eq. 30 numerator
-                const float Dn = __fmaf_rn(dz, wjz, __fmaf_rn(dy, wjy, __fmul_rn(dx, wjx)));   // Eq. 30 denominator
-                // Eq. 29 with r_ij = N/Dn:  phi_VL = 4 N Dn / (N + Dn)^2 if N Dn > 0 else 0  (S7)
-                const float nd = __fmul_rn(Nn, Dn);
-                const float sm = __fadd_rn(Nn, Dn);
-                float phi = 0.0f;
-                if (nd > 0.0f) phi = __fdividef(4.0f * nd, __fmul_rn(sm, sm));
-                phi = fminf(phi, 1.0f);
-                // Eqs. 31-32
-                const float eta = __fmul_rn(r, fminf(ti.w, tj.w));
-                if (eta < eta_crit) {
-                    const float q = (eta - eta_crit) * inv_fold;
-                    phi *= __expf(-q * q);
-                }
-                // Eq. 27 (adot = 0): uhat_ij = v_ij - (1/2) phi (grad v_i + grad v_j).x_ij ; then uhat_ij . x_ij
-                const float hp = 0.5f * phi;
-                const float ux = __fsub_rn(__fsub_rn(vi.x, vj.x), __fmul_rn(hp, __fadd_rn(wix, wjx)));
-                const float uy = __fsub_rn(__fsub_rn(vi.y, vj.y), __fmul_rn(hp, __fadd_rn(wiy, wjy)));
-                const float uz = __fsub_rn(__fsub_rn(vi.z, vj.z), __fmul_rn(hp, __fadd_rn(wiz, wjz)));
-                const float udx = __fmaf_rn(uz, dz, __fmaf_rn(uy, dy, __fmul_rn(ux, dx)));
-                // Eq. 25: mu_k = min(0, hhat_k (uhat.x) / (r^2 + hhat_k^2 eps^2));  Eq. 24: Q_k = rho_k (-C_l c_k mu_k + C_q mu_k^2)
-                const float mui = fminf(0.0f, __fdividef(__fmul_rn(hhi, udx), __fadd_rn(r2, he2i)));
-                const float muj = fminf(0.0f, __fdividef(__fmul_rn(h2.z, udx), __fadd_rn(r2, h2.w)));
-                const float Qi = visc_Q(ti.y, ti.z, mui, a.C_l, a.C_q);
-                const float Qj = visc_Q(tj.y, tj.z, muj, a.C_l, a.C_q);
-                const float PQi = __fadd_rn(ti.x, Qi), PQj = __fadd_rn(tj.x, Qj);
-                const float hvv = 0.5f * __fmul_rn(vi.w, vj.w);
-                const float pf = __fmul_rn(hvv, __fadd_rn(PQi, PQj));
-                Fx = fmaf(pf, Gx, Fx); Fy = fmaf(pf, Gy, Fy); Fz = fmaf(pf, Gz, Fz);
-                const float vG = (vj.x - vi.x) * Gx + (vj.y - vi.y) * Gy + (vj.z - vi.z) * Gz;
-                dE = fmaf(hvv * PQj, vG, dE);
-            }
+    const float eps2 = a.eps2;
+    float acc[4] = {0.f, 0.f, 0.f, 0.f};                 // Fx, Fy, Fz, dE
+    const float4* planes[FPL];
+#pragma unroll
+    for (int p = 0; p < FPL; ++p) planes[p] = a.fst + (int64_t)p * a.np;
+    const uint32_t count = leaf_sweep<W5_WPL, FPL, true>(a, planes, leaf, 0, wl, lane, tile, [&](int c, bool wrapped) {
+        const PState J = load_pstate(tile + c, CRK_CCAP);
+        float dx, dy, dz, r2;
+        sep3(a, wrapped, I.x, I.y, I.z, make_float4(J.x, J.y, J.z, 0.f), dx, dy, dz, r2);
+        const float r = __fmul_rn(r2, rsqrtf(fmaxf(r2, R2_TINY)));
+        const float k3j = __fmul_rn(__fmul_rn(__fmul_rn(SIGMA_C4, J.ih), J.ih), J.ih);
+        const float k5j = __fmul_rn(__fmul_rn(k3j, J.ih), J.ih);
+        float Wi, Di, Wj, Dj;
+        wendland_dim(r, I.ih, k3i, k5i, Wi, Di);
+        wendland_dim(r, J.ih, k3j, k5j, Wj, Dj);
+        float aix, aiy, aiz, ajx, ajy, ajz;
+        rk_grad(I.c, dx, dy, dz, Wi, Di, aix, aiy, aiz);            // grad WR_ij
+        rk_grad(J.c, -dx, -dy, -dz, Wj, Dj, ajx, ajy, ajz);         // grad WR_ji  (x_ji = -x_ij)
+        const float Gx = __fsub_rn(ajx, aix), Gy = __fsub_rn(ajy, aiy), Gz = __fsub_rn(ajz, aiz);
+        // (grad v . x_ij) for both particles, written so that the mirrored lane forms the same numbers
+        const float wix = __fmaf_rn(I.g[2], dz, __fmaf_rn(I.g[1], dy, __fmul_rn(I.g[0], dx)));
+        const float wiy = __fmaf_rn(I.g[5], dz, __fmaf_rn(I.g[4], dy, __fmul_rn(I.g[3], dx)));
+        const float wiz = __fmaf_rn(I.g[8], dz, __fmaf_rn(I.g[7], dy, __fmul_rn(I.g[6], dx)));
+        const float wjx = __fmaf_rn(J.g[2], dz, __fmaf_rn(J.g[1], dy, __fmul_rn(J.g[0], dx)));
+        const float wjy = __fmaf_rn(J.g[5], dz, __fmaf_rn(J.g[4], dy, __fmul_rn(J.g[3], dx)));
+        const float wjz = __fmaf_rn(J.g[8], dz, __fmaf_rn(J.g[7], dy, __fmul_rn(J.g[6], dx)));
+        const float Nn = __fmaf_rn(dz, wiz, __fmaf_rn(dy, wiy, __fmul_rn(dx, wix)));   // Eq. 30 numerator
+        const float Dn = __fmaf_rn(dz, wjz, __fmaf_rn(dy, wjy, __fmul_rn(dx, wjx)));   // Eq. 30 denominator
+        // Eq. 29 with r_ij = N/Dn:  phi_VL = 4 N Dn / (N + Dn)^2 if N Dn > 0 else 0  (S7)
+        const float nd = __fmul_rn(Nn, Dn);
+        const float sm = __fadd_rn(Nn, Dn);
+        float phi = 0.0f;
+        if (nd > 0.0f) phi = __fdividef(4.0f * nd, __fmul_rn(sm, sm));
+        phi = fminf(phi, 1.0f);
+        // Eqs. 31-32
+        const float eta = __fmul_rn(r, fminf(I.ih, J.ih));
+        if (eta < eta_crit) {
+            const float q = (eta - eta_crit) * inv_fold;
+            phi *= __expf(-q * q);
         }
-        count += cnt;
+        // Eq. 27 (adot = 0): uhat_ij = v_ij - (1/2) phi (grad v_i + grad v_j).x_ij ; then uhat_ij . x_ij
+        const float hp = 0.5f * phi;
+        const float ux = __fsub_rn(__fsub_rn(I.vx, J.vx), __fmul_rn(hp, __fadd_rn(wix, wjx)));
+        const float uy = __fsub_rn(__fsub_rn(I.vy, J.vy), __fmul_rn(hp, __fadd_rn(wiy, wjy)));
+        const float uz = __fsub_rn(__fsub_rn(I.vz, J.vz), __fmul_rn(hp, __fadd_rn(wiz, wjz)));
+        const float udx = __fmaf_rn(uz, dz, __fmaf_rn(uy, dy, __fmul_rn(ux, dx)));
+        // Eq. 25 with hhat = h/n_h, q = 1/hhat:  mu_k = min(0, hhat_k (uhat.x) / (r^2 + hhat_k^2 eps^2))
+        //                                             = min(0, q_k (uhat.x) / (q_k^2 r^2 + eps^2));  Eq. 24: Q_k
+        const float qhj = __fmul_rn(a.n_h, J.ih);
+        const float mui = fminf(0.0f, __fdividef(__fmul_rn(qhi, udx), __fmaf_rn(qhi2, r2, eps2)));
+        const float muj = fminf(0.0f, __fdividef(__fmul_rn(qhj, udx), __fmaf_rn(__fmul_rn(qhj, qhj), r2, eps2)));
+        const float Qi = visc_Q(I.rho, I.cs, mui, a.C_l, a.C_q);
+        const float Qj = visc_Q(J.rho, J.cs, muj, a.C_l, a.C_q);
+        const float PQi = __fadd_rn(I.P, Qi), PQj = __fadd_rn(J.P, Qj);
+        const float hvv = 0.5f * __fmul_rn(I.V, J.V);
+        const float pf = __fmul_rn(hvv, __fadd_rn(PQi, PQj));
+        acc[0] = fmaf(pf, Gx, acc[0]); acc[1] = fmaf(pf, Gy, acc[1]); acc[2] = fmaf(pf, Gz, acc[2]);
+        const float vG = (J.vx - I.vx) * Gx + (J.vy - I.vy) * Gy + (J.vz - I.vz) * Gz;
+        acc[3] = fmaf(hvv * PQj, vG, acc[3]);
     });
-    if (valid) {
+    group_reduce<W5_WPL, 4>(acc, 0, wl, lane, (float*)tile);
+    if (wl == 0 && valid) {
         const float im = 1.0f / a.m_s[i];
         const int32_t p = a.perm[i];
-        a.o0[p] = Fx * im;
-        a.o1[p] = Fy * im;
-        a.o2[p] = Fz * im;
-        a.o3[p] = dE * im;
+        a.o0[p] = acc[0] * im;
+        a.o1[p] = acc[1] * im;
+        a.o2[p] = acc[2] * im;
+        a.o3[p] = acc[3] * im;
         if (a.ocnt) a.ocnt[p] = count;
     }
 }
@@ -637,11 +605,10 @@ SweepArgs make_args(crk_ctx* c) {
     memset(&a, 0, sizeof(a));
     a.n = c->n; a.nl = c->nl; a.np = c->nl * CRK_LEAF;
     a.L = c->prm.box; a.half = 0.5f * c->prm.box;
-    a.off = (const uint32_t*)c->nbr_off.p; a.list = (const uint32_t*)c->nbr_list.p;
+    a.arena = (const uint4*)c->arena.p; a.seg_first = (const uint32_t*)c->seg_first.p;
     a.perm = c->perm;
-    a.leaf_lo = (const float4*)c->leaf_lo.p; a.leaf_hi = (const float4*)c->leaf_hi.p;
-    a.posh = (const float4*)c->posh.p; a.posV = (float4*)c->posV.p; a.velV = (float4*)c->velV.p;
-    a.thermo = (float4*)c->thermo.p; a.coef = (float4*)c->coef.p; a.gv = (float4*)c->gv.p;
+    a.posh = (const float4*)c->posh.p; a.posV = (float4*)c->posV.p; a.velV = nullptr;
+    a.coef = (float4*)c->coef.p; a.fst = (float4*)c->fst.p;
     a.rho_s = (float*)c->rho_s.p; a.m_s = (const float*)c->m_s.p;
     a.gamma = c->prm.gamma; a.n_h = c->prm.n_h; a.C_l = c->prm.C_l; a.C_q = c->prm.C_q;
     a.eps2 = c->prm.eps * c->prm.eps;
@@ -665,9 +632,9 @@ int crk_launch_volumes(crk_ctx* c, const float* m, float* V, float* rho, uint32_
     CRK_TRY(crk_check_launch(c, "k_gather_f32"));
     SweepArgs a = make_args(c);
     a.o0 = V; a.o1 = rho; a.ocnt = nbr_count;
-    const int smem = WPC * Smem<CH1, 1>::PER_WARP;
+    const int smem = W1_WPC * CRK_CCAP * (int)sizeof(float4);
     CRK_TRY(set_smem(c, k_volumes, smem));
-    k_volumes<<<(unsigned)((c->nl + WPC - 1) / WPC), WPC * 32, smem, c->stream>>>(a);
+    k_volumes<<<(unsigned)((c->nl + W1_WPC - 1) / W1_WPC), W1_WPC * 32, smem, c->stream>>>(a);
     return crk_check_launch(c, "k_volumes");
 }
 
@@ -676,9 +643,9 @@ int crk_launch_moments(crk_ctx* c, float* A, float* B, float* gradA, float* grad
     CRK_TRY(crk_ensure(c, c->coef, (size_t)np * 4 * sizeof(float4)));
     SweepArgs a = make_args(c);
     a.o0 = A; a.o1 = B; a.o2 = gradA; a.o3 = gradB;
-    const int smem = WPC * Smem<CH2, 1>::PER_WARP;
+    const int smem = W2_WPC * CRK_CCAP * (int)sizeof(float4);
     CRK_TRY(set_smem(c, k_moments, smem));
-    k_moments<<<(unsigned)((c->nl + WPC - 1) / WPC), WPC * 32, smem, c->stream>>>(a);
+    k_moments<<<(unsigned)((c->nl + W2_WPC - 1) / W2_WPC), W2_WPC * 32, smem, c->stream>>>(a);
     return crk_check_launch(c, "k_moments");
 }
 
@@ -686,27 +653,27 @@ int crk_launch_hydro(crk_ctx* c, const float* vx, const float* vy, const float* 
                      float* ay, float* az, float* dudt, uint32_t* pair_count) {
     const int64_t np = c->nl * CRK_LEAF;
     CRK_TRY(crk_ensure(c, c->vel_orig, (size_t)c->n * sizeof(float4)));
-    CRK_TRY(crk_ensure(c, c->velV, (size_t)np * sizeof(float4)));
-    CRK_TRY(crk_ensure(c, c->thermo, (size_t)np * sizeof(float4)));
-    CRK_TRY(crk_ensure(c, c->gv, (size_t)np * 3 * sizeof(float4)));
+    CRK_TRY(crk_ensure(c, c->u_s, (size_t)np * sizeof(float)));
+    CRK_TRY(crk_ensure(c, c->fst, (size_t)np * FPL * sizeof(float4)));
     k_pack_vel<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>(vx, vy, vz, u, c->n, (float4*)c->vel_orig.p);
     CRK_TRY(crk_check_launch(c, "k_pack_vel"));
     SweepArgs a = make_args(c);
-    k_hydro_prep<<<(unsigned)((np + 255) / 256), 256, 0, c->stream>>>(a, (const float4*)c->vel_orig.p);
+    a.velV = (float4*)c->fst.p + np;                     // plane 1 of the force-sweep state is (vx,vy,vz,V)
+    k_hydro_prep<<<(unsigned)((np + 255) / 256), 256, 0, c->stream>>>(a, (const float4*)c->vel_orig.p, (float*)c->u_s.p);
     CRK_TRY(crk_check_launch(c, "k_hydro_prep"));
     crk_rec(c, EV_GV0);
     {
-        const int smem = WPC * Smem<CH4, 2>::PER_WARP;
+        const int smem = W4_LPC * 2 * CRK_CCAP * (int)sizeof(float4);
         CRK_TRY(set_smem(c, k_gradv, smem));
-        k_gradv<<<(unsigned)((c->nl + WPC - 1) / WPC), WPC * 32, smem, c->stream>>>(a);
+        k_gradv<<<(unsigned)((c->nl + W4_LPC - 1) / W4_LPC), W4_WPL * W4_LPC * 32, smem, c->stream>>>(a, (const float*)c->u_s.p);
         CRK_TRY(crk_check_launch(c, "k_gradv"));
     }
     crk_rec(c, EV_GV1);
     a.o0 = ax; a.o1 = ay; a.o2 = az; a.o3 = dudt; a.ocnt = pair_count;
     {
-        const int smem = WPC * Smem<CH5, PL5>::PER_WARP;
+        const int smem = FPL * CRK_CCAP * (int)sizeof(float4);
         CRK_TRY(set_smem(c, k_forces, smem));
-        k_forces<<<(unsigned)((c->nl + WPC - 1) / WPC), WPC * 32, smem, c->stream>>>(a);
+        k_forces<<<(unsigned)c->nl, W5_WPL * 32, smem, c->stream>>>(a);
         CRK_TRY(crk_check_launch(c, "k_forces"));
     }
     crk_rec(c, EV_F1);
