@@ -37,6 +37,28 @@ FLOPS_PER_PAIR = {"volumes": 16.0, "moments": 100.0, "gradv": 90.0, "forces": 25
 FP32_PEAK_THEORETICAL = 148 * 128 * 2 * 1.965e9     # SMs x FP32 lanes x 2 (FMA) x max SM clock
 
 
+BASE_SEEDS = {"tiny_uniform": 1001, "blast_wave": 1002, "clustered": 1003, "cosmo": 1004, "cosmo_large": 1005}
+
+
+def rank_seed(config: str, rank: int) -> int:
+    """N > 1 shards by independent boxes: rank r evaluates its own seeded box of the same recipe (rank 0 = the
+    BASELINE seed), so there is no data-path collective."""
+    return BASE_SEEDS[config] + 7919 * rank
+
+
+def aggregate_over_ranks(ms, e2e_ms, pairs, particles, world, device):
+    """whole-job numbers: times are the MAX over ranks, work is the SUM over ranks (one all-reduce each; the only
+    collectives of the run, outside the timed region).  Works with nccl (cuda device) and gloo (cpu device)."""
+    import torch
+    import torch.distributed as dist
+    tot = torch.tensor([ms, e2e_ms], device=device, dtype=torch.float64)
+    work = torch.tensor([pairs, particles], device=device, dtype=torch.float64)
+    if world > 1:
+        dist.all_reduce(tot, op=dist.ReduceOp.MAX)
+        dist.all_reduce(work, op=dist.ReduceOp.SUM)
+    return float(tot[0]), float(tot[1]), float(work[0]), float(work[1])
+
+
 def load_peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -149,8 +171,7 @@ def run_ours(args, rank, world, local_rank):
         dist.init_process_group("nccl", device_id=dev)
 
     # each rank owns an independent seeded box of the same recipe (weak scaling; the path has no exchange step on one box)
-    base_seed = {"tiny_uniform": 1001, "blast_wave": 1002, "clustered": 1003, "cosmo": 1004, "cosmo_large": 1005}[args.config]
-    ps = wl.make_config(args.config, args.n_side, seed=base_seed + 7919 * rank)
+    ps = wl.make_config(args.config, args.n_side, seed=rank_seed(args.config, rank))
     names = ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")
     host = [torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).pin_memory() for k in names]
     t = [h.to(dev, non_blocking=True) for h in host]
@@ -204,13 +225,7 @@ def run_ours(args, rank, world, local_rank):
     torch.cuda.synchronize()
     e2e_ms = 1e3 * (time.perf_counter() - t0) / k2
 
-    tot = torch.tensor([ms, e2e_ms], device=dev, dtype=torch.float64)
-    work = torch.tensor([pairs_per_step, float(ps.n)], device=dev, dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(tot, op=dist.ReduceOp.MAX)
-        dist.all_reduce(work, op=dist.ReduceOp.SUM)
-    ms_all, e2e_all = float(tot[0]), float(tot[1])
-    pairs_all, n_all = float(work[0]), float(work[1])
+    ms_all, e2e_all, pairs_all, n_all = aggregate_over_ranks(ms, e2e_ms, pairs_per_step, float(ps.n), world, dev)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
