@@ -245,7 +245,7 @@ def run_ours(args, rank, world, local_rank):
                                f"{fp32_meas / 1e12:.1f} TFLOP/s in this run",
                 "flops_per_pair": FLOPS_PER_PAIR["forces"], "pairs_per_launch": sym_pairs, "kernel_ms": forces_ms,
                 "traffic": None}
-    passes = {k: st[k] for k in ("ms_sort", "ms_tree", "ms_volumes", "ms_rk", "ms_gradv", "ms_forces")}
+    passes = {k: st[k] for k in ("ms_sort", "ms_tree", "ms_lists", "ms_volumes", "ms_rk", "ms_gradv", "ms_forces")}
     alg_flops = (FLOPS_PER_PAIR["volumes"] + FLOPS_PER_PAIR["moments"] + FLOPS_PER_PAIR["gradv"]) * gather_pairs + forces_flops
     sweeps_ms = st["ms_volumes"] + st["ms_rk"] + st["ms_gradv"] + st["ms_forces"]
     sort_bytes = ps.n * (6 * 32.0 + 16 + 12 + 32 + 16)    # radix passes + pack + gather

@@ -184,25 +184,11 @@ int crk_get_perm(crk_ctx* c, int32_t* perm) {
     return CRK_OK;
 }
 
-// grad v sits in planes 6 (w), 7 and 8 of the force-sweep state
-__global__ void k_scatter_gradv(const float4* __restrict__ fst, const int32_t* __restrict__ perm, int64_t n, int64_t np,
-                                float* __restrict__ out) {
-    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= n) return;
-    const float4 a = fst[6 * np + k], b = fst[7 * np + k], cc = fst[8 * np + k];
-    const int32_t p = perm[k];
-    const float g[9] = {a.w, b.x, b.y, b.z, b.w, cc.x, cc.y, cc.z, cc.w};
-#pragma unroll
-    for (int q = 0; q < 9; ++q) out[q * n + p] = g[q];
-}
-
 int crk_get_gradv(crk_ctx* c, float* gradv) {
     if (!c || !gradv) return CRK_EINVAL;
     if (c->stage < 4) return CRK_ESTATE;
     if (c->n == 0) return CRK_OK;
-    k_scatter_gradv<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>((const float4*)c->fst.p, c->perm, c->n,
-                                                                           c->nl * CRK_LEAF, gradv);
-    return crk_check_launch(c, "k_scatter_gradv");
+    return crk_launch_gradv_full(c, gradv);   // the force-sweep state keeps only the symmetric part: re-run the sweep
 }
 
 int crk_set_timing(crk_ctx* c, int on) {

@@ -22,7 +22,7 @@ enum { EV_BUILD0 = 0, EV_SORTED, EV_TREE1, EV_BUILD1, EV_VOL0, EV_VOL1, EV_RK0, 
 //   cand[c]   = sorted-order index of candidate c (only candidates accepted by at least one lane of the leaf)
 //   ell[k][l] = k-th entry of lane l: candidate index | bit 15 (pair crosses the periodic boundary); lane l owns
 //               cnt_g[l] gather entries (r2 < h_i^2) followed by cnt[l] - cnt_g[l] entries that are symmetric-only
-#define CRK_CCAP 640             // candidates per segment (tile capacity of the sweeps)
+#define CRK_CCAP 384             // candidates per segment (tile capacity of the sweeps)
 #define CRK_QCAP 160             // entries per lane per segment
 #define CRK_TCULL 64             // cull tile of the list builder
 #define CRK_SEG_HDR_UNITS 9
@@ -141,3 +141,4 @@ int crk_launch_volumes(crk_ctx* c, const float* m, float* V, float* rho, uint32_
 int crk_launch_moments(crk_ctx* c, float* A, float* B, float* gradA, float* gradB);                   // pairs.cu
 int crk_launch_hydro(crk_ctx* c, const float* vx, const float* vy, const float* vz, const float* u,
                      float* ax, float* ay, float* az, float* dudt, uint32_t* pair_count);             // pairs.cu
+int crk_launch_gradv_full(crk_ctx* c, float* gradv);                                                  // pairs.cu

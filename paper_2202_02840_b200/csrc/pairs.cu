@@ -59,6 +59,10 @@ __device__ __forceinline__ Seg load_seg(const uint4* __restrict__ arena, uint32_
     return s;
 }
 
+__device__ __forceinline__ void cp_async16(uint32_t dst_shared, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst_shared), "l"(src) : "memory");
+}
+
 template <int WPL>
 __device__ __forceinline__ void group_sync(int lg) {
     if (WPL == 1) __syncwarp();
@@ -71,33 +75,27 @@ __device__ __forceinline__ void group_sync(int lg) {
 template <int WPL, int PLANES, bool SYM, typename Pair>
 __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4* const* planes, int64_t leaf, int lg, int wl,
                                                int lane, float4* tile, Pair pair) {
-    constexpr int NQ = (PLANES >= 4) ? 1 : 4;                  // candidates per thread in flight while staging
     uint32_t count = 0;
     const int tg = wl * 32 + lane;
+    const uint32_t tile_s = (uint32_t)__cvta_generic_to_shared(tile);
     for (uint32_t unit = __ldg(a.seg_first + leaf); unit != 0u;) {
         const Seg s = load_seg(a.arena, unit, lane);
         group_sync<WPL>(lg);                                   // the previous segment's drain is finished
-        for (int c0 = 0; c0 < s.C; c0 += WPL * 32 * NQ) {
-            uint32_t j[NQ];
+        // stage: 16-byte asynchronous copies global -> shared (LDGSTS), no register round trip
+        for (int c0 = 0; c0 < s.C; c0 += WPL * 32 * 2) {
+            const int ca = c0 + tg, cb = ca + WPL * 32;
+            const uint32_t ja = (ca < s.C) ? __ldg(s.cand + ca) : 0u;
+            const uint32_t jb = (cb < s.C) ? __ldg(s.cand + cb) : 0u;
+            if (ca < s.C) {
 #pragma unroll
-            for (int q = 0; q < NQ; ++q) {
-                const int c = c0 + q * WPL * 32 + tg;
-                j[q] = (c < s.C) ? __ldg(s.cand + c) : 0u;
+                for (int p = 0; p < PLANES; ++p) cp_async16(tile_s + (uint32_t)(p * CRK_CCAP + ca) * 16u, planes[p] + ja);
             }
-            float4 v[NQ][PLANES];
+            if (cb < s.C) {
 #pragma unroll
-            for (int q = 0; q < NQ; ++q)
-#pragma unroll
-                for (int p = 0; p < PLANES; ++p) v[q][p] = __ldg(planes[p] + j[q]);
-#pragma unroll
-            for (int q = 0; q < NQ; ++q) {
-                const int c = c0 + q * WPL * 32 + tg;
-                if (c < s.C) {
-#pragma unroll
-                    for (int p = 0; p < PLANES; ++p) tile[p * CRK_CCAP + c] = v[q][p];
-                }
+                for (int p = 0; p < PLANES; ++p) cp_async16(tile_s + (uint32_t)(p * CRK_CCAP + cb) * 16u, planes[p] + jb);
             }
         }
+        asm volatile("cp.async.wait_all;" ::: "memory");
         group_sync<WPL>(lg);
         const int rows = SYM ? s.K : s.Kg;
         const int mine = SYM ? s.ct : s.cg;
@@ -432,7 +430,7 @@ __device__ __forceinline__ void wendland_dim(float r, float ih, float k3, float 
 // The epilogue also forms P = (gamma-1) rho u (Eq. 4, unclamped) and c_s = sqrt(gamma (gamma-1) max(u,0)) (S12) and writes
 // the packed force-sweep state of the particle.
 constexpr int W4_WPL = 2, W4_LPC = 2;
-__global__ void __launch_bounds__(W4_WPL * W4_LPC * 32) k_gradv(SweepArgs a, const float* __restrict__ u_s) {
+__global__ void __launch_bounds__(W4_WPL * W4_LPC * 32) k_gradv(SweepArgs a, const float* __restrict__ u_s, float* __restrict__ gv_full) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int lg = w / W4_WPL, wl = w % W4_WPL;
@@ -468,19 +466,26 @@ __global__ void __launch_bounds__(W4_WPL * W4_LPC * 32) k_gradv(SweepArgs a, con
     });
     group_reduce<W4_WPL, 9>(g, lg, wl, lane, (float*)tile);
     if (wl != 0) return;
-    // force-sweep state: (x,y,z,1/h) (v,V) | (P,rho,cs,A) (B,cx) (cy,cz,M0,M1) (M2..M5) (M6,M7,M8,g0) (g1..g4) (g5..g8)
+    // force-sweep state planes: (x,y,z,1/h) (v,V) | (P,rho,cs,k3) (A,B) (c,M0) (M1..M4) (M5..M8) (gxx,gyy,gzz,k5)
+    // (gxy+gyx, gxz+gzx, gyz+gzy, n_h/h).  Only x.(grad v x) enters Eqs. 27-30 and Eq. 25 (uhat_ij.x_ij), so the
+    // symmetric part of grad v is all the force sweep needs; k3 = sigma/h^3, k5 = sigma/h^5.
     const float u = u_s[i], rho = a.rho_s[i], gm = a.gamma;
     const float P = (gm - 1.0f) * rho * u;
     const float cs = sqrtf(gm * (gm - 1.0f) * fmaxf(u, 0.0f));
     float4* f = a.fst + i;
     const int64_t np = a.np;
-    f[2 * np] = make_float4(P, rho, cs, q0.x);
-    f[3 * np] = make_float4(q0.y, q0.z, q0.w, q1.x);
-    f[4 * np] = make_float4(q1.y, q1.z, q1.w, q2.x);
-    f[5 * np] = make_float4(q2.y, q2.z, q2.w, q3.x);
-    f[6 * np] = make_float4(q3.y, q3.z, q3.w, g[0]);
-    f[7 * np] = make_float4(g[1], g[2], g[3], g[4]);
-    f[8 * np] = make_float4(g[5], g[6], g[7], g[8]);
+    f[2 * np] = make_float4(P, rho, cs, k3);
+    f[3 * np] = q0;
+    f[4 * np] = q1;
+    f[5 * np] = q2;
+    f[6 * np] = q3;
+    f[7 * np] = make_float4(g[0], g[4], g[8], k5);
+    f[8 * np] = make_float4(g[1] + g[3], g[2] + g[6], g[5] + g[7], a.n_h * ih);
+    if (gv_full && valid) {                              // diagnostics (crk_get_gradv): all nine components, caller order
+        const int32_t p = a.perm[i];
+#pragma unroll
+        for (int q = 0; q < 9; ++q) gv_full[q * a.n + p] = g[q];
+    }
 }
 
 // ============================================================================================ a5: momentum and energy
@@ -489,11 +494,11 @@ __global__ void __launch_bounds__(W4_WPL * W4_LPC * 32) k_gradv(SweepArgs a, con
 // Q from Eqs. 24-25 with the limited midpoint projection of Eqs. 27-32 (S7: division-free van Leer form).
 // Sums over all j != i with r2 < max(h_i^2, h_j^2); each ordered pair is evaluated on a lane that holds i in registers.
 // One CTA = one leaf: W5_WPL warps share the tile of the leaf's candidates and split each lane's entries by rows.
-constexpr int W5_WPL = 8;
+constexpr int W5_WPL = 4;
 struct PState {           // one particle's force-sweep state in registers
-    float x, y, z, ih, vx, vy, vz, V, P, rho, cs;
+    float x, y, z, ih, vx, vy, vz, V, P, rho, cs, k3, k5, qh;
     Coef c;
-    float g[9];
+    float gxx, gyy, gzz, gxy, gxz, gyz;                  // symmetric part of grad v, off-diagonals summed
 };
 __device__ __forceinline__ PState load_pstate(const float4* __restrict__ f, int64_t stride) {
     const float4 a0 = f[0], a1 = f[stride], a2 = f[2 * stride], a3 = f[3 * stride], a4 = f[4 * stride], a5 = f[5 * stride],
@@ -501,16 +506,22 @@ __device__ __forceinline__ PState load_pstate(const float4* __restrict__ f, int6
     PState s;
     s.x = a0.x; s.y = a0.y; s.z = a0.z; s.ih = a0.w;
     s.vx = a1.x; s.vy = a1.y; s.vz = a1.z; s.V = a1.w;
-    s.P = a2.x; s.rho = a2.y; s.cs = a2.z; s.c.A = a2.w;
-    s.c.Bx = a3.x; s.c.By = a3.y; s.c.Bz = a3.z; s.c.cx = a3.w;
-    s.c.cy = a4.x; s.c.cz = a4.y; s.c.M[0] = a4.z; s.c.M[1] = a4.w;
-    s.c.M[2] = a5.x; s.c.M[3] = a5.y; s.c.M[4] = a5.z; s.c.M[5] = a5.w;
-    s.c.M[6] = a6.x; s.c.M[7] = a6.y; s.c.M[8] = a6.z; s.g[0] = a6.w;
-    s.g[1] = a7.x; s.g[2] = a7.y; s.g[3] = a7.z; s.g[4] = a7.w;
-    s.g[5] = a8.x; s.g[6] = a8.y; s.g[7] = a8.z; s.g[8] = a8.w;
+    s.P = a2.x; s.rho = a2.y; s.cs = a2.z; s.k3 = a2.w;
+    s.c = load_coef(a3, a4, a5, a6);
+    s.gxx = a7.x; s.gyy = a7.y; s.gzz = a7.z; s.k5 = a7.w;
+    s.gxy = a8.x; s.gxz = a8.y; s.gyz = a8.z; s.qh = a8.w;
     return s;
 }
-__global__ void __launch_bounds__(W5_WPL * 32) k_forces(SweepArgs a) {
+// x.(grad v x) with the symmetric part (Eq. 30 numerator / denominator)
+__device__ __forceinline__ float quad_form(const PState& s, float dxx, float dyy, float dzz, float dxy, float dxz, float dyz) {
+    return __fmaf_rn(s.gyz, dyz, __fmaf_rn(s.gxz, dxz, __fmaf_rn(s.gxy, dxy,
+           __fmaf_rn(s.gzz, dzz, __fmaf_rn(s.gyy, dyy, __fmul_rn(s.gxx, dxx))))));
+}
+// Eq. 25 with hhat = h/n_h, q = 1/hhat:  mu = min(0, hhat (uhat.x) / (r^2 + hhat^2 eps^2)) = min(0, q (uhat.x) / (q^2 r^2 + eps^2))
+__device__ __forceinline__ float visc_mu(float qh, float udx, float r2, float eps2) {
+    return fminf(0.0f, __fdividef(__fmul_rn(qh, udx), __fmaf_rn(__fmul_rn(qh, qh), r2, eps2)));
+}
+__global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
     const int64_t leaf = blockIdx.x;
@@ -518,11 +529,9 @@ __global__ void __launch_bounds__(W5_WPL * 32) k_forces(SweepArgs a) {
     const int64_t i = leaf * CRK_LEAF + lane;
     const bool valid = i < a.n;
     const PState I = load_pstate(a.fst + i, a.np);
-    const float k3i = SIGMA_C4 * I.ih * I.ih * I.ih, k5i = k3i * I.ih * I.ih;
-    const float qhi = a.n_h * I.ih;                      // 1 / hhat_i
-    const float qhi2 = qhi * qhi;
     const float eta_crit = 1.0f / a.n_h, inv_fold = a.n_h / 0.2f;
     const float eps2 = a.eps2;
+    const float Cl = a.C_l, Cq = a.C_q;
     float acc[4] = {0.f, 0.f, 0.f, 0.f};                 // Fx, Fy, Fz, dE
     const float4* planes[FPL];
 #pragma unroll
@@ -532,55 +541,41 @@ __global__ void __launch_bounds__(W5_WPL * 32) k_forces(SweepArgs a) {
         float dx, dy, dz, r2;
         sep3(a, wrapped, I.x, I.y, I.z, make_float4(J.x, J.y, J.z, 0.f), dx, dy, dz, r2);
         const float r = __fmul_rn(r2, rsqrtf(fmaxf(r2, R2_TINY)));
-        const float k3j = __fmul_rn(__fmul_rn(__fmul_rn(SIGMA_C4, J.ih), J.ih), J.ih);
-        const float k5j = __fmul_rn(__fmul_rn(k3j, J.ih), J.ih);
         float Wi, Di, Wj, Dj;
-        wendland_dim(r, I.ih, k3i, k5i, Wi, Di);
-        wendland_dim(r, J.ih, k3j, k5j, Wj, Dj);
+        wendland_dim(r, I.ih, I.k3, I.k5, Wi, Di);
+        wendland_dim(r, J.ih, J.k3, J.k5, Wj, Dj);
         float aix, aiy, aiz, ajx, ajy, ajz;
         rk_grad(I.c, dx, dy, dz, Wi, Di, aix, aiy, aiz);            // grad WR_ij
         rk_grad(J.c, -dx, -dy, -dz, Wj, Dj, ajx, ajy, ajz);         // grad WR_ji  (x_ji = -x_ij)
         const float Gx = __fsub_rn(ajx, aix), Gy = __fsub_rn(ajy, aiy), Gz = __fsub_rn(ajz, aiz);
-        // (grad v . x_ij) for both particles, written so that the mirrored lane forms the same numbers
-        const float wix = __fmaf_rn(I.g[2], dz, __fmaf_rn(I.g[1], dy, __fmul_rn(I.g[0], dx)));
-        const float wiy = __fmaf_rn(I.g[5], dz, __fmaf_rn(I.g[4], dy, __fmul_rn(I.g[3], dx)));
-        const float wiz = __fmaf_rn(I.g[8], dz, __fmaf_rn(I.g[7], dy, __fmul_rn(I.g[6], dx)));
-        const float wjx = __fmaf_rn(J.g[2], dz, __fmaf_rn(J.g[1], dy, __fmul_rn(J.g[0], dx)));
-        const float wjy = __fmaf_rn(J.g[5], dz, __fmaf_rn(J.g[4], dy, __fmul_rn(J.g[3], dx)));
-        const float wjz = __fmaf_rn(J.g[8], dz, __fmaf_rn(J.g[7], dy, __fmul_rn(J.g[6], dx)));
-        const float Nn = __fmaf_rn(dz, wiz, __fmaf_rn(dy, wiy, __fmul_rn(dx, wix)));   // Eq. 30 numerator
-        const float Dn = __fmaf_rn(dz, wjz, __fmaf_rn(dy, wjy, __fmul_rn(dx, wjx)));   // Eq. 30 denominator
+        // Eq. 30: N = x.(grad v_i x), Dn = x.(grad v_j x); every product is even in x, so the mirrored lane forms the same bits
+        const float dxx = __fmul_rn(dx, dx), dyy = __fmul_rn(dy, dy), dzz = __fmul_rn(dz, dz);
+        const float dxy = __fmul_rn(dx, dy), dxz = __fmul_rn(dx, dz), dyz = __fmul_rn(dy, dz);
+        const float Nn = quad_form(I, dxx, dyy, dzz, dxy, dxz, dyz);
+        const float Dn = quad_form(J, dxx, dyy, dzz, dxy, dxz, dyz);
         // Eq. 29 with r_ij = N/Dn:  phi_VL = 4 N Dn / (N + Dn)^2 if N Dn > 0 else 0  (S7)
         const float nd = __fmul_rn(Nn, Dn);
         const float sm = __fadd_rn(Nn, Dn);
-        float phi = 0.0f;
-        if (nd > 0.0f) phi = __fdividef(4.0f * nd, __fmul_rn(sm, sm));
-        phi = fminf(phi, 1.0f);
+        float phi = (nd > 0.0f) ? fminf(__fdividef(4.0f * nd, __fmul_rn(sm, sm)), 1.0f) : 0.0f;
         // Eqs. 31-32
         const float eta = __fmul_rn(r, fminf(I.ih, J.ih));
         if (eta < eta_crit) {
             const float q = (eta - eta_crit) * inv_fold;
             phi *= __expf(-q * q);
         }
-        // Eq. 27 (adot = 0): uhat_ij = v_ij - (1/2) phi (grad v_i + grad v_j).x_ij ; then uhat_ij . x_ij
-        const float hp = 0.5f * phi;
-        const float ux = __fsub_rn(__fsub_rn(I.vx, J.vx), __fmul_rn(hp, __fadd_rn(wix, wjx)));
-        const float uy = __fsub_rn(__fsub_rn(I.vy, J.vy), __fmul_rn(hp, __fadd_rn(wiy, wjy)));
-        const float uz = __fsub_rn(__fsub_rn(I.vz, J.vz), __fmul_rn(hp, __fadd_rn(wiz, wjz)));
-        const float udx = __fmaf_rn(uz, dz, __fmaf_rn(uy, dy, __fmul_rn(ux, dx)));
-        // Eq. 25 with hhat = h/n_h, q = 1/hhat:  mu_k = min(0, hhat_k (uhat.x) / (r^2 + hhat_k^2 eps^2))
-        //                                             = min(0, q_k (uhat.x) / (q_k^2 r^2 + eps^2));  Eq. 24: Q_k
-        const float qhj = __fmul_rn(a.n_h, J.ih);
-        const float mui = fminf(0.0f, __fdividef(__fmul_rn(qhi, udx), __fmaf_rn(qhi2, r2, eps2)));
-        const float muj = fminf(0.0f, __fdividef(__fmul_rn(qhj, udx), __fmaf_rn(__fmul_rn(qhj, qhj), r2, eps2)));
-        const float Qi = visc_Q(I.rho, I.cs, mui, a.C_l, a.C_q);
-        const float Qj = visc_Q(J.rho, J.cs, muj, a.C_l, a.C_q);
+        // Eq. 27 (adot = 0): uhat_ij.x_ij = v_ij.x_ij - (1/2) phi x_ij.(grad v_i + grad v_j).x_ij = v_ij.x_ij - (1/2) phi (N + Dn)
+        const float vx = __fsub_rn(I.vx, J.vx), vy = __fsub_rn(I.vy, J.vy), vz = __fsub_rn(I.vz, J.vz);
+        const float vdx = __fmaf_rn(vz, dz, __fmaf_rn(vy, dy, __fmul_rn(vx, dx)));
+        const float udx = __fmaf_rn(__fmul_rn(-0.5f, phi), sm, vdx);
+        // Eqs. 24-25
+        const float Qi = visc_Q(I.rho, I.cs, visc_mu(I.qh, udx, r2, eps2), Cl, Cq);
+        const float Qj = visc_Q(J.rho, J.cs, visc_mu(J.qh, udx, r2, eps2), Cl, Cq);
         const float PQi = __fadd_rn(I.P, Qi), PQj = __fadd_rn(J.P, Qj);
         const float hvv = 0.5f * __fmul_rn(I.V, J.V);
         const float pf = __fmul_rn(hvv, __fadd_rn(PQi, PQj));
         acc[0] = fmaf(pf, Gx, acc[0]); acc[1] = fmaf(pf, Gy, acc[1]); acc[2] = fmaf(pf, Gz, acc[2]);
-        const float vG = (J.vx - I.vx) * Gx + (J.vy - I.vy) * Gy + (J.vz - I.vz) * Gz;
-        acc[3] = fmaf(hvv * PQj, vG, acc[3]);
+        const float vG = fmaf(vz, Gz, fmaf(vy, Gy, vx * Gx));       // (v_i - v_j).G = -(v_j - v_i).G
+        acc[3] = fmaf(-hvv * PQj, vG, acc[3]);
     });
     group_reduce<W5_WPL, 4>(acc, 0, wl, lane, (float*)tile);
     if (wl == 0 && valid) {
@@ -665,7 +660,7 @@ int crk_launch_hydro(crk_ctx* c, const float* vx, const float* vy, const float* 
     {
         const int smem = W4_LPC * 2 * CRK_CCAP * (int)sizeof(float4);
         CRK_TRY(set_smem(c, k_gradv, smem));
-        k_gradv<<<(unsigned)((c->nl + W4_LPC - 1) / W4_LPC), W4_WPL * W4_LPC * 32, smem, c->stream>>>(a, (const float*)c->u_s.p);
+        k_gradv<<<(unsigned)((c->nl + W4_LPC - 1) / W4_LPC), W4_WPL * W4_LPC * 32, smem, c->stream>>>(a, (const float*)c->u_s.p, nullptr);
         CRK_TRY(crk_check_launch(c, "k_gradv"));
     }
     crk_rec(c, EV_GV1);
@@ -678,4 +673,15 @@ int crk_launch_hydro(crk_ctx* c, const float* vx, const float* vy, const float* 
     }
     crk_rec(c, EV_F1);
     return CRK_OK;
+}
+
+// diagnostics: re-run the Eq. 26 sweep on the resident state and write all nine components of grad v in caller order
+int crk_launch_gradv_full(crk_ctx* c, float* gradv) {
+    const int64_t np = c->nl * CRK_LEAF;
+    SweepArgs a = make_args(c);
+    a.velV = (float4*)c->fst.p + np;
+    const int smem = W4_LPC * 2 * CRK_CCAP * (int)sizeof(float4);
+    CRK_TRY(set_smem(c, k_gradv, smem));
+    k_gradv<<<(unsigned)((c->nl + W4_LPC - 1) / W4_LPC), W4_WPL * W4_LPC * 32, smem, c->stream>>>(a, (const float*)c->u_s.p, gradv);
+    return crk_check_launch(c, "k_gradv");
 }
