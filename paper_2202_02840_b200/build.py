@@ -30,7 +30,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_dep():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    flags = list(NVCC_FLAGS) + (["-Xptxas", "-v"] if verbose else [])
+    flags = list(NVCC_FLAGS) + (["-Xptxas", "-v"] if verbose else []) + os.environ.get("CRK_NVCC_EXTRA", "").split()
     objs = []
 
     def compile_one(src):
