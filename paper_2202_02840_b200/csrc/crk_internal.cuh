@@ -19,6 +19,8 @@ enum { EV_BUILD0 = 0, EV_SORTED, EV_TREE1, EV_BUILD1, EV_VOL0, EV_VOL1, EV_RK0, 
 // ---- neighbour lists (lists.cu): per leaf a chain of segments in one arena of 16-byte units --------------------------
 //   segment = header (9 units) | cand[C] u32, padded to 4 | ell[K][32] u16
 //   header unit 0: {next segment (arena unit, 0 = none), C | Kg << 16, K, 0}; units 1-4: cnt_g[32] u16; units 5-8: cnt[32] u16
+//   the first segment's header is mirrored in dense per-leaf arrays: seg_first[leaf] = {next, C | Kg << 16, K, own arena unit
+//   (0 = leaf has no segment)} and leaf_cnt[leaf][64] = cnt_g | cnt
 //   cand[c]   = sorted-order index of candidate c (only candidates accepted by at least one lane of the leaf)
 //   ell[k][l] = k-th entry of lane l: candidate index | bit 15 (pair crosses the periodic boundary); lane l owns
 //               cnt_g[l] gather entries (r2 < h_i^2) followed by cnt[l] - cnt_g[l] entries that are symmetric-only
@@ -66,7 +68,8 @@ struct crk_ctx {
     int64_t level_cnt[CRK_MAX_LEVELS + 1];
     DevBuf nbr_cnt, nbr_off, nbr_list, nbr_gcnt;
     int64_t n_pairs = 0, n_pairs_gather = 0;
-    DevBuf arena, seg_first;       // neighbour-list arena (16-byte units) and first-segment unit per leaf
+    DevBuf arena, seg_first;       // neighbour-list arena (16-byte units); per leaf a uint4 copy of its first segment's header
+    DevBuf leaf_cnt;               // u16[nl][64]: per-lane cnt_g | cnt of the first segment (dense, so the sweeps need no pointer chase)
     int64_t arena_units = 0;       // units used by the last build
     // per-particle state in sorted order
     DevBuf posV;                   // float4 (x,y,z,V)

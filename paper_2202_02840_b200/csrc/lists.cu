@@ -26,12 +26,13 @@ struct ListArgs {
     uint4* arena;
     unsigned long long arena_cap;          // units
     unsigned long long* counter;           // next free unit (unit 0 is reserved as "none")
-    uint32_t* __restrict__ seg_first;
+    uint4* __restrict__ seg_first;         // dense copy of each leaf's first header (.w = its arena unit)
+    uint16_t* __restrict__ leaf_cnt;       // [nl][64]
 };
 
 struct WarpSmem {
-    float4 tile[CRK_TCULL];
-    uint32_t tidx[CRK_TCULL];
+    float4 tile[CRK_TCULL + 4];
+    __align__(16) uint32_t tidx[CRK_TCULL + 4];
     uint32_t cand[CRK_CCAP];
     uint16_t queue[CRK_QCAP][32];
 };
@@ -51,31 +52,46 @@ __device__ __forceinline__ float gap1_wrap(float lo, float hi, float x, float L)
     return fminf(g0, fminf(gp, gm));
 }
 
-// test every staged candidate against the lane's particle; returns the new candidate count of the segment
-template <bool WRAP>
+// test every staged candidate against the lane's particle; returns the new candidate count of the segment.
+// Branch-free, four candidates per trip (the tile is padded to a multiple of 4 with far-away sentinels): about 4 of 5
+// culled candidates are accepted by some lane, so predicated appends beat a vote-and-branch per candidate.
+// tile[t] = (x, y, z, h_j^2).  SELF: the tile holds the query leaf itself, so j = i has to be excluded.
+template <bool WRAP, bool SELF>
 __device__ __forceinline__ int test_tile(WarpSmem& S, int fill, int C, int& g, int& s, int lane, uint32_t self, float xi,
                                          float yi, float zi, float hi2, float L, float half) {
-#pragma unroll 2
-    for (int t = 0; t < fill; ++t) {
-        const float4 pj = S.tile[t];
-        const uint32_t jidx = S.tidx[t];
-        float dx = __fsub_rn(xi, pj.x), dy = __fsub_rn(yi, pj.y), dz = __fsub_rn(zi, pj.z);
-        bool wrapped = false;
-        if (WRAP) {
-            const float wx = wrap1(dx, L, half), wy = wrap1(dy, L, half), wz = wrap1(dz, L, half);
-            wrapped = (wx != dx) || (wy != dy) || (wz != dz);
-            dx = wx; dy = wy; dz = wz;
+    for (int t0 = 0; t0 < fill; t0 += 4) {
+        bool ag[4], as[4], wrapped[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const float4 pj = S.tile[t0 + u];
+            float dx = __fsub_rn(xi, pj.x), dy = __fsub_rn(yi, pj.y), dz = __fsub_rn(zi, pj.z);
+            wrapped[u] = false;
+            if (WRAP) {
+                const float wx = wrap1(dx, L, half), wy = wrap1(dy, L, half), wz = wrap1(dz, L, half);
+                wrapped[u] = (wx != dx) || (wy != dy) || (wz != dz);
+                dx = wx; dy = wy; dz = wz;
+            }
+            const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+            ag[u] = r2 < hi2;                                              // gather: Eqs. 13-14
+            as[u] = r2 < fmaxf(hi2, pj.w);                                 // symmetric: Eqs. 17-18
+            if (SELF) {
+                const bool notself = S.tidx[t0 + u] != self;
+                ag[u] = ag[u] && notself;
+                as[u] = as[u] && notself;
+            }
         }
-        const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-        const bool notself = jidx != self;
-        const bool ag = (r2 < hi2) && notself;                                       // gather: Eqs. 13-14
-        const bool as = (r2 < fmaxf(hi2, __fmul_rn(pj.w, pj.w))) && notself;         // symmetric: Eqs. 17-18
-        if (__any_sync(0xffffffffu, as)) {
-            if (lane == 0) S.cand[C] = jidx;
-            const uint16_t e = (uint16_t)(C | (wrapped ? CRK_ELL_WRAP : 0u));
-            if (ag) S.queue[g++][lane] = e;
-            else if (as) S.queue[CRK_QCAP - 1 - (s++)][lane] = e;
-            ++C;
+        const uint4 ji = *(const uint4*)&S.tidx[t0];
+        const uint32_t jv[4] = {ji.x, ji.y, ji.z, ji.w};
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const bool any = __any_sync(0xffffffffu, as[u]);
+            const uint16_t e = (uint16_t)(C | (wrapped[u] ? CRK_ELL_WRAP : 0u));
+            if (ag[u]) S.queue[g][lane] = e;
+            else if (as[u]) S.queue[CRK_QCAP - 1 - s][lane] = e;
+            g += ag[u] ? 1 : 0;
+            s += (as[u] && !ag[u]) ? 1 : 0;
+            if (any && lane == 0) S.cand[C] = jv[u];
+            C += any ? 1 : 0;
         }
     }
     return C;
@@ -96,7 +112,7 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
     const uint32_t lt = (1u << lane) - 1u;
     int C = 0, g = 0, s = 0, fill = 0;
     bool cwrap = false;
-    uint32_t prev = 0;   // arena unit of the previous segment header of this leaf
+    uint32_t prev = 0, first = 0;   // arena units of the previous / first segment header of this leaf
 
     auto emit = [&]() {
         const int Kg = __reduce_max_sync(0xffffffffu, g);
@@ -120,21 +136,28 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
                 else if (k < g + s) v = S.queue[CRK_QCAP - 1 - (k - g)][lane];
                 el[k * 32 + lane] = v;
             }
-            if (lane == 0) {
-                if (prev == 0) a.seg_first[leaf] = (uint32_t)base;
-                else ((uint32_t*)(a.arena + prev))[0] = (uint32_t)base;
+            if (prev == 0) {
+                if (lane == 0) a.seg_first[leaf] = make_uint4(0u, (uint32_t)C | ((uint32_t)Kg << 16), (uint32_t)K, (uint32_t)base);
+                a.leaf_cnt[leaf * 64 + lane] = (uint16_t)g;
+                a.leaf_cnt[leaf * 64 + 32 + lane] = (uint16_t)(g + s);
+                first = (uint32_t)base;
+            } else if (lane == 0) {
+                ((uint32_t*)(a.arena + prev))[0] = (uint32_t)base;
+                if (prev == first) ((uint32_t*)(a.seg_first + leaf))[0] = (uint32_t)base;
             }
             prev = (uint32_t)base;
         }
         C = 0; g = 0; s = 0;
         __syncwarp();
     };
-    auto flush = [&]() {
+    auto flush = [&](bool selftile) {
         const int maxlen = __reduce_max_sync(0xffffffffu, g + s);
         if (C + fill > CRK_CCAP || maxlen + fill > CRK_QCAP) emit();
+        if (lane < ((4 - fill) & 3)) S.tile[fill + lane] = make_float4(3.0e30f, 3.0e30f, 3.0e30f, 0.0f);
         __syncwarp();
-        if (cwrap) C = test_tile<true>(S, fill, C, g, s, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
-        else C = test_tile<false>(S, fill, C, g, s, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
+        if (selftile) C = test_tile<true, true>(S, fill, C, g, s, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
+        else if (cwrap) C = test_tile<true, false>(S, fill, C, g, s, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
+        else C = test_tile<false, false>(S, fill, C, g, s, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
         fill = 0;
         cwrap = false;
         __syncwarp();
@@ -159,22 +182,25 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
             gx = gap1_wrap(blo.x, bhi.x, pc.x, a.L); gy = gap1_wrap(blo.y, bhi.y, pc.y, a.L); gz = gap1_wrap(blo.z, bhi.z, pc.z, a.L);
         }
         const float g2 = __fmaf_rn(gz, gz, __fmaf_rn(gy, gy, __fmul_rn(gx, gx)));
-        const bool surv = g2 < fmaxf(hq2, __fmul_rn(pc.w, pc.w));
+        const float hj2 = __fmul_rn(pc.w, pc.w);
+        const bool surv = g2 < fmaxf(hq2, hj2);
         const uint32_t m = __ballot_sync(0xffffffffu, surv);
         const int cnt = __popc(m);
         if (cnt == 0) continue;
-        if (fill + cnt > CRK_TCULL) flush();
+        const bool own = b == leaf;
+        if (fill > 0 && (own || fill + cnt > CRK_TCULL)) flush(false);   // the query leaf gets a tile of its own (self test)
         const int slot = fill + __popc(m & lt);
         if (surv) {
-            S.tile[slot] = pc;
+            S.tile[slot] = make_float4(pc.x, pc.y, pc.z, hj2);
             S.tidx[slot] = (uint32_t)(b * CRK_LEAF + lane);
         }
         cwrap = cwrap || wrap;
         fill += cnt;
+        if (own) flush(true);
     }
-    if (fill > 0) flush();
+    if (fill > 0) flush(false);
     if (C > 0) emit();
-    if (prev == 0 && lane == 0) a.seg_first[leaf] = 0u;
+    if (prev == 0 && lane == 0) a.seg_first[leaf] = make_uint4(0u, 0u, 0u, 0u);
 }
 
 __global__ void k_set_u64(unsigned long long* p, unsigned long long v) { *p = v; }
@@ -183,7 +209,8 @@ __global__ void k_set_u64(unsigned long long* p, unsigned long long v) { *p = v;
 
 int crk_build_nbr_lists(crk_ctx* c) {
     const int64_t nl = c->nl;
-    CRK_TRY(crk_ensure(c, c->seg_first, (size_t)(nl + 1) * sizeof(uint32_t)));
+    CRK_TRY(crk_ensure(c, c->seg_first, (size_t)(nl + 1) * sizeof(uint4)));
+    CRK_TRY(crk_ensure(c, c->leaf_cnt, (size_t)(nl + 1) * 64 * sizeof(uint16_t)));
     // first guess: ~7 KB per leaf at ~60 neighbours; grown to the exact need if the builder reports more
     if (!c->arena.p) CRK_TRY(crk_ensure(c, c->arena, (size_t)nl * 9216 + 65536));
     unsigned long long* d_counter = (unsigned long long*)((char*)c->flag.p + 32);
@@ -197,7 +224,8 @@ int crk_build_nbr_lists(crk_ctx* c) {
         a.arena_cap = (unsigned long long)(c->arena.cap / 16);
         if (a.arena_cap > 0xffffffffull) a.arena_cap = 0xffffffffull;      // segment links are 32-bit unit indices (64 GB)
         a.counter = d_counter;
-        a.seg_first = (uint32_t*)c->seg_first.p;
+        a.seg_first = (uint4*)c->seg_first.p;
+        a.leaf_cnt = (uint16_t*)c->leaf_cnt.p;
         k_set_u64<<<1, 1, 0, c->stream>>>(d_counter, 1ull);
         CRK_TRY(crk_check_launch(c, "k_set_u64"));
         k_nbr_lists<<<(unsigned)((nl + LW - 1) / LW), LW * 32, 0, c->stream>>>(a);

@@ -22,7 +22,8 @@ struct SweepArgs {
     int64_t n, nl;
     float L, half;
     const uint4* __restrict__ arena;      // neighbour-list segments
-    const uint32_t* __restrict__ seg_first;
+    const uint4* __restrict__ seg_first;  // dense copy of each leaf's first segment header (.w = its arena unit, 0 = none)
+    const uint16_t* __restrict__ leaf_cnt;  // [nl][64] per-lane cnt_g | cnt of the first segment
     const int32_t* __restrict__ perm;     // sorted slot -> caller index
     const float4* __restrict__ posh;      // (x,y,z,h)
     float4* __restrict__ posV;            // (x,y,z,V)
@@ -44,19 +45,31 @@ struct Seg {
     int C, Kg, K, cg, ct;
     uint32_t next;
 };
-__device__ __forceinline__ Seg load_seg(const uint4* __restrict__ arena, uint32_t unit, int lane) {
+__device__ __forceinline__ Seg make_seg(const uint4* __restrict__ arena, uint32_t unit, const uint4& h0, int cg, int ct) {
     const uint4* hdr = arena + unit;
-    const uint4 h0 = __ldg(hdr);
     Seg s;
     s.next = h0.x;
     s.C = (int)(h0.y & 0xffffu);
     s.Kg = (int)(h0.y >> 16);
     s.K = (int)h0.z;
-    s.cg = (int)__ldg((const uint16_t*)(hdr + 1) + lane);
-    s.ct = (int)__ldg((const uint16_t*)(hdr + 5) + lane);
+    s.cg = cg;
+    s.ct = ct;
     s.cand = (const uint32_t*)(hdr + CRK_SEG_HDR_UNITS);
     s.ell = (const uint16_t*)(hdr + CRK_SEG_HDR_UNITS + ((s.C + 3) >> 2));
     return s;
+}
+// first segment: header and per-lane counts come from the dense per-leaf arrays (no dependent load before the payload)
+__device__ __forceinline__ Seg first_seg(const uint4* __restrict__ arena, const uint4* __restrict__ seg_first,
+                                         const uint16_t* __restrict__ leaf_cnt, int64_t leaf, int lane, uint32_t& unit) {
+    const uint4 h0 = __ldg(seg_first + leaf);
+    const int cg = (int)__ldg(leaf_cnt + leaf * 64 + lane), ct = (int)__ldg(leaf_cnt + leaf * 64 + 32 + lane);
+    unit = h0.w;
+    return make_seg(arena, unit, h0, cg, ct);
+}
+__device__ __forceinline__ Seg load_seg(const uint4* __restrict__ arena, uint32_t unit, int lane) {
+    const uint4* hdr = arena + unit;
+    const uint4 h0 = __ldg(hdr);
+    return make_seg(arena, unit, h0, (int)__ldg((const uint16_t*)(hdr + 1) + lane), (int)__ldg((const uint16_t*)(hdr + 5) + lane));
 }
 
 __device__ __forceinline__ void cp_async16(uint32_t dst_shared, const void* src) {
@@ -96,8 +109,19 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
     uint32_t count = 0;
     const int tg = wl * 32 + lane;
     const uint32_t tile_s = (uint32_t)__cvta_generic_to_shared(tile);
-    for (uint32_t unit = __ldg(a.seg_first + leaf); unit != 0u;) {
-        const Seg s = load_seg(a.arena, unit, lane);
+    uint32_t unit;
+    Seg s = first_seg(a.arena, a.seg_first, a.leaf_cnt, leaf, lane, unit);
+    while (unit != 0u) {
+        const int rows = SYM ? s.K : s.Kg;
+        const int mine = SYM ? s.ct : s.cg;
+        const uint16_t* ep = s.ell + lane;
+        // the first rows of the ELL block travel together with the candidate indices
+        uint32_t e[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int k = wl + q * WPL;
+            e[q] = (k < rows) ? (uint32_t)__ldg(ep + k * 32) : 0u;
+        }
         group_sync<WPL>(lg);                                   // the previous segment's drain is finished
         // stage: 16-byte asynchronous copies global -> shared (LDGSTS), no register round trip
         for (int c0 = 0; c0 < s.C; c0 += WPL * 32 * 2) {
@@ -115,15 +139,6 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
         }
         asm volatile("cp.async.wait_all;" ::: "memory");
         group_sync<WPL>(lg);
-        const int rows = SYM ? s.K : s.Kg;
-        const int mine = SYM ? s.ct : s.cg;
-        const uint16_t* ep = s.ell + lane;
-        uint32_t e[4];
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const int k = wl + q * WPL;
-            e[q] = (k < rows) ? (uint32_t)__ldg(ep + k * 32) : 0u;
-        }
         for (int k0 = wl; k0 < rows; k0 += 4 * WPL) {
             uint32_t nx[4];
 #pragma unroll
@@ -141,6 +156,7 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
         }
         count += (uint32_t)mine;
         unit = s.next;
+        if (unit != 0u) s = load_seg(a.arena, unit, lane);
     }
     return count;
 }
@@ -618,7 +634,7 @@ SweepArgs make_args(crk_ctx* c) {
     memset(&a, 0, sizeof(a));
     a.n = c->n; a.nl = c->nl; a.np = c->nl * CRK_LEAF;
     a.L = c->prm.box; a.half = 0.5f * c->prm.box;
-    a.arena = (const uint4*)c->arena.p; a.seg_first = (const uint32_t*)c->seg_first.p;
+    a.arena = (const uint4*)c->arena.p; a.seg_first = (const uint4*)c->seg_first.p; a.leaf_cnt = (const uint16_t*)c->leaf_cnt.p;
     a.perm = c->perm;
     a.posh = (const float4*)c->posh.p; a.posV = (float4*)c->posV.p; a.velV = nullptr;
     a.coef = (float4*)c->coef.p; a.fst = (float4*)c->fst.p;
