@@ -52,6 +52,14 @@ __device__ __forceinline__ float gap1_wrap(float lo, float hi, float x, float L)
     return fminf(g0, fminf(gp, gm));
 }
 
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void sts_u16_if(uint32_t addr, uint32_t v, bool pred) {
+    asm volatile("{ .reg .pred p; setp.ne.b32 p, %2, 0; @p st.shared.u16 [%0], %1; }" ::"r"(addr), "h"((uint16_t)v), "r"((int)pred) : "memory");
+}
+__device__ __forceinline__ void sts_u32_if(uint32_t addr, uint32_t v, bool pred) {
+    asm volatile("{ .reg .pred p; setp.ne.b32 p, %2, 0; @p st.shared.u32 [%0], %1; }" ::"r"(addr), "r"(v), "r"((int)pred) : "memory");
+}
+
 // test every staged candidate against the lane's particle; returns the new candidate count of the segment.
 // Branch-free, four candidates per trip (the tile is padded to a multiple of 4 with far-away sentinels): about 4 of 5
 // culled candidates are accepted by some lane, so predicated appends beat a vote-and-branch per candidate.
@@ -59,6 +67,9 @@ __device__ __forceinline__ float gap1_wrap(float lo, float hi, float x, float L)
 template <bool WRAP, bool SELF>
 __device__ __forceinline__ int test_tile(WarpSmem& S, int fill, int C, int& g, int& s, int lane, uint32_t self, float xi,
                                          float yi, float zi, float hi2, float L, float half) {
+    uint32_t gp = smem_u32(&S.queue[g][lane]);                  // next gather entry of this lane (row stride 64 bytes)
+    uint32_t sp = smem_u32(&S.queue[CRK_QCAP - 1 - s][lane]);   // next symmetric-only entry (stack from the top)
+    uint32_t cp = smem_u32(&S.cand[C]);
     for (int t0 = 0; t0 < fill; t0 += 4) {
         bool ag[4], as[4], wrapped[4];
 #pragma unroll
@@ -85,15 +96,17 @@ __device__ __forceinline__ int test_tile(WarpSmem& S, int fill, int C, int& g, i
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
             const bool any = __any_sync(0xffffffffu, as[u]);
-            const uint16_t e = (uint16_t)(C | (wrapped[u] ? CRK_ELL_WRAP : 0u));
-            if (ag[u]) S.queue[g][lane] = e;
-            else if (as[u]) S.queue[CRK_QCAP - 1 - s][lane] = e;
-            g += ag[u] ? 1 : 0;
-            s += (as[u] && !ag[u]) ? 1 : 0;
-            if (any && lane == 0) S.cand[C] = jv[u];
+            const uint32_t e = (uint32_t)C | (wrapped[u] ? CRK_ELL_WRAP : 0u);
+            sts_u16_if(ag[u] ? gp : sp, e, as[u]);                         // one predicated store, no branch
+            gp += ag[u] ? 64u : 0u;
+            sp -= (as[u] && !ag[u]) ? 64u : 0u;
+            sts_u32_if(cp, jv[u], any && lane == 0);
+            cp += any ? 4u : 0u;
             C += any ? 1 : 0;
         }
     }
+    g = (int)((gp - smem_u32(&S.queue[0][lane])) >> 6);
+    s = (int)((smem_u32(&S.queue[CRK_QCAP - 1][lane]) - sp) >> 6);
     return C;
 }
 
