@@ -99,6 +99,9 @@ int  crk_step_derivs_host(crk_ctx* c, int64_t n, const float* x, const float* y,
 const char* crk_last_error(const crk_ctx* c);
 int  crk_get_perm(crk_ctx* c, int32_t* perm);        /* device int32[n]: perm[k] = caller index of sorted slot k   */
 int  crk_get_gradv(crk_ctx* c, float* gradv);         /* device float[9][n], index 3*a+b = d_b v^a (Eq. 26), caller order */
+/* device uint32[n_leaves][4]: first neighbour-list segment of every leaf = {next segment, C | Kg << 16, K, arena unit};
+ * C = candidate slots, Kg / K = rows of the gather / symmetric entry block (layout: csrc/crk_internal.cuh)     */
+int  crk_get_leaf_segments(crk_ctx* c, uint32_t* seg);
 int  crk_get_stats(crk_ctx* c, crk_stats* out);       /* host struct                                                */
 int  crk_reset_stats(crk_ctx* c);
 int  crk_set_timing(crk_ctx* c, int on);              /* record CUDA events around each pass (adds stream syncs when read) */

@@ -11,7 +11,7 @@ _LIB_PATH = os.path.join(_HERE, "libcrk.so")
 
 EXPORTED_SYMBOLS = (
     "crk_create", "crk_destroy", "crk_build_cells", "crk_volumes", "crk_rk_coefficients", "crk_hydro_derivs",
-    "crk_step_derivs", "crk_step_derivs_host", "crk_last_error", "crk_get_perm", "crk_get_gradv", "crk_get_stats",
+    "crk_step_derivs", "crk_step_derivs_host", "crk_last_error", "crk_get_perm", "crk_get_gradv", "crk_get_leaf_segments", "crk_get_stats",
     "crk_reset_stats", "crk_set_timing", "crk_get_leaf_list", "crk_measure_fp32_peak",
 )
 
@@ -72,6 +72,7 @@ def _load():
     L.crk_last_error.restype = C.c_char_p
     L.crk_get_perm.argtypes = [vp, vp]
     L.crk_get_gradv.argtypes = [vp, vp]
+    L.crk_get_leaf_segments.argtypes = [vp, vp]
     L.crk_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.crk_reset_stats.argtypes = [vp]
     L.crk_set_timing.argtypes = [vp, C.c_int]
@@ -185,6 +186,13 @@ class Crk:
         p = torch.empty(self.n, device=self._dev, dtype=torch.int32)
         self._chk(self._L.crk_get_perm(self._h, _dev(p, torch.int32)))
         return p
+
+    def leaf_segments(self):
+        """uint32 [n_leaves, 4]: {next, C | Kg << 16, K, arena unit} of every leaf's first neighbour-list segment"""
+        nl = (self.n + 31) // 32
+        t = torch.empty((nl, 4), device=self._dev, dtype=torch.int32)
+        self._chk(self._L.crk_get_leaf_segments(self._h, _dev(t, torch.int32)))
+        return t
 
     def gradv(self):
         g = torch.empty((9, self.n), device=self._dev)

@@ -184,6 +184,14 @@ int crk_get_perm(crk_ctx* c, int32_t* perm) {
     return CRK_OK;
 }
 
+int crk_get_leaf_segments(crk_ctx* c, uint32_t* seg) {
+    if (!c || !seg) return CRK_EINVAL;
+    if (c->stage < 1) return CRK_ESTATE;
+    if (c->n == 0) return CRK_OK;
+    CRK_CUDA(c, cudaMemcpyAsync(seg, c->seg_first.p, (size_t)c->nl * sizeof(uint4), cudaMemcpyDeviceToDevice, c->stream));
+    return CRK_OK;
+}
+
 int crk_get_gradv(crk_ctx* c, float* gradv) {
     if (!c || !gradv) return CRK_EINVAL;
     if (c->stage < 4) return CRK_ESTATE;

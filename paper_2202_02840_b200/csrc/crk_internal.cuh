@@ -21,12 +21,13 @@ enum { EV_BUILD0 = 0, EV_SORTED, EV_TREE1, EV_BUILD1, EV_VOL0, EV_VOL1, EV_RK0, 
 //   header unit 0: {next segment (arena unit, 0 = none), C | Kg << 16, K, 0}; units 1-4: cnt_g[32] u16; units 5-8: cnt[32] u16
 //   the first segment's header is mirrored in dense per-leaf arrays: seg_first[leaf] = {next, C | Kg << 16, K, own arena unit
 //   (0 = leaf has no segment)} and leaf_cnt[leaf][64] = cnt_g | cnt
-//   cand[c]   = sorted-order index of candidate c (only candidates accepted by at least one lane of the leaf)
+//   cand[c]   = sorted-order index of candidate c (only candidates accepted by at least one lane of the leaf); in a
+//               leaf's first segment cand[0..31] are the leaf's own 32 particles in lane order (always kept)
 //   ell[k][l] = k-th entry of lane l: candidate index | bit 15 (pair crosses the periodic boundary); lane l owns
 //               cnt_g[l] gather entries (r2 < h_i^2) followed by cnt[l] - cnt_g[l] entries that are symmetric-only
-#define CRK_CCAP 384             // candidates per segment (tile capacity of the sweeps)
-#define CRK_QCAP 160             // entries per lane per segment
-#define CRK_TCULL 64             // cull tile of the list builder
+#define CRK_CCAP 352             // candidates per segment (tile capacity of the sweeps)
+#define CRK_QCAP 176             // entries per lane per segment
+#define CRK_TCULL 48             // cull tile of the list builder
 #define CRK_SEG_HDR_UNITS 9
 #define CRK_ELL_WRAP 0x8000u
 #define CRK_ELL_MASK 0x7fffu

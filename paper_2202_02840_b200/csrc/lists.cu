@@ -95,7 +95,7 @@ __device__ __forceinline__ int test_tile(WarpSmem& S, int fill, int C, int& g, i
         const uint32_t jv[4] = {ji.x, ji.y, ji.z, ji.w};
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
-            const bool any = __any_sync(0xffffffffu, as[u]);
+            const bool any = SELF || __any_sync(0xffffffffu, as[u]);      // the leaf's own particles always get a slot
             const uint32_t e = (uint32_t)C | (wrapped[u] ? CRK_ELL_WRAP : 0u);
             sts_u16_if(ag[u] ? gp : sp, e, as[u]);                         // one predicated store, no branch
             gp += ag[u] ? 64u : 0u;
@@ -144,7 +144,7 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
             for (int c = lane; c < C; c += 32) cd[c] = S.cand[c];
             uint16_t* el = (uint16_t*)(hdr + CRK_SEG_HDR_UNITS + ((C + 3) >> 2));
             for (int k = 0; k < K; ++k) {
-                uint16_t v = 0xffffu;
+                uint16_t v = 0u;   // padding of shorter lanes: slot 0 (the sweeps prefetch it, never evaluate it)
                 if (k < g) v = S.queue[k][lane];
                 else if (k < g + s) v = S.queue[CRK_QCAP - 1 - (k - g)][lane];
                 el[k * 32 + lane] = v;
@@ -179,6 +179,12 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
     const uint32_t e0 = a.off[leaf], e1 = a.off[leaf + 1];
     uint32_t ent = (e0 < e1) ? a.list[e0] : 0u;
     float4 pj = (e0 < e1) ? a.posh[(int64_t)(ent & CRK_LEAF_MASK) * CRK_LEAF + lane] : make_float4(0, 0, 0, 0);
+    // the query leaf itself goes first and keeps all 32 particles: slots 0..31 of the first segment are the leaf's own
+    // particles in lane order, so a sweep finds the i-state of its lanes in the tile it stages anyway
+    S.tile[lane] = make_float4(xi, yi, zi, hi2);
+    S.tidx[lane] = (uint32_t)i;
+    fill = 32;
+    flush(true);
     for (uint32_t e = e0; e < e1; ++e) {
         const uint32_t cur = ent;
         const float4 pc = pj;
@@ -200,8 +206,8 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
         const uint32_t m = __ballot_sync(0xffffffffu, surv);
         const int cnt = __popc(m);
         if (cnt == 0) continue;
-        const bool own = b == leaf;
-        if (fill > 0 && (own || fill + cnt > CRK_TCULL)) flush(false);   // the query leaf gets a tile of its own (self test)
+        if (b == leaf) continue;                                         // done first
+        if (fill + cnt > CRK_TCULL) flush(false);
         const int slot = fill + __popc(m & lt);
         if (surv) {
             S.tile[slot] = make_float4(pc.x, pc.y, pc.z, hj2);
@@ -209,7 +215,6 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
         }
         cwrap = cwrap || wrap;
         fill += cnt;
-        if (own) flush(true);
     }
     if (fill > 0) flush(false);
     if (C > 0) emit();

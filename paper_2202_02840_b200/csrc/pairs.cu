@@ -76,6 +76,14 @@ __device__ __forceinline__ void cp_async16(uint32_t dst_shared, const void* src)
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst_shared), "l"(src) : "memory");
 }
 
+__device__ __forceinline__ uint32_t smem_u32addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+// 128-bit shared-memory load from a 32-bit shared address (no generic-address window arithmetic in the inner loops)
+__device__ __forceinline__ float4 lds128(uint32_t addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(addr));
+    return v;
+}
+
 // MUFU approximations with flush-to-zero: one instruction each (the default rsqrtf / __fdividef / __expf wrap the MUFU in
 // denormal rescaling, 3-4 extra instructions per call); relative error 2^-22, far below the 1e-4 parity bar
 __device__ __forceinline__ float rsqrt_fast(float x) {
@@ -102,7 +110,8 @@ __device__ __forceinline__ void group_sync(int lg) {
 
 // ---- the sweep over one leaf's segment chain -------------------------------------------------------------------------
 // SYM = false: rows [0, Kg), lane active while k < cnt_g (gather set, Eqs. 13-14);  SYM = true: rows [0, K), k < cnt.
-// pair(slot, crosses_boundary) evaluates one accepted pair; returns the number of entries the lane owns (= its count).
+// pair(slot_addr, crosses_boundary, plane0) evaluates one accepted pair (slot_addr = shared address of the candidate's
+// plane-0 entry; plane p sits CRK_CCAP * 16 * p bytes further); returns the number of entries the lane owns (= its count).
 template <int WPL, int PLANES, bool SYM, typename Pair>
 __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4* const* planes, int64_t leaf, int lg, int wl,
                                                int lane, float4* tile, Pair pair) {
@@ -139,6 +148,9 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
         }
         asm volatile("cp.async.wait_all;" ::: "memory");
         group_sync<WPL>(lg);
+        // plane 0 of the next pair's candidate is fetched one pair ahead: the pair math starts without waiting for shared
+        // memory, and the loads of the remaining planes are covered by the arithmetic that needs plane 0 only
+        float4 cur0 = lds128(tile_s + (e[0] & CRK_ELL_MASK) * 16u);
         for (int k0 = wl; k0 < rows; k0 += 4 * WPL) {
             uint32_t nx[4];
 #pragma unroll
@@ -149,7 +161,10 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const int k = k0 + q * WPL;
-                if (k < mine) pair((int)(e[q] & CRK_ELL_MASK), (e[q] & CRK_ELL_WRAP) != 0u);
+                const uint32_t en = (q < 3) ? e[(q + 1) & 3] : nx[0];
+                const float4 nxt0 = lds128(tile_s + (en & CRK_ELL_MASK) * 16u);
+                if (k < mine) pair(tile_s + (e[q] & CRK_ELL_MASK) * 16u, (e[q] & CRK_ELL_WRAP) != 0u, cur0);
+                cur0 = nxt0;
             }
 #pragma unroll
             for (int q = 0; q < 4; ++q) e[q] = nx[q];
@@ -233,8 +248,7 @@ __global__ void __launch_bounds__(W1_WPC * 32) k_volumes(SweepArgs a) {
     const float inv_h = valid ? 1.0f / hi : 0.0f;
     float acc = 0.0f;
     const float4* const planes[1] = {a.posh};
-    const uint32_t count = leaf_sweep<1, 1, false>(a, planes, leaf, w, 0, lane, tile, [&](int c, bool wrapped) {
-        const float4 pj = tile[c];
+    const uint32_t count = leaf_sweep<1, 1, false>(a, planes, leaf, w, 0, lane, tile, [&](uint32_t, bool wrapped, const float4& pj) {
         float dx, dy, dz, r2;
         sep3(a, wrapped, xi, yi, zi, pj, dx, dy, dz, r2);
         const float r = r2 * rsqrt_fast(fmaxf(r2, R2_TINY));
@@ -284,8 +298,7 @@ __global__ void __launch_bounds__(W2_WPC * 32) k_moments(SweepArgs a) {
     float txx = 0.f, txy = 0.f, txz = 0.f, tyy = 0.f, tyz = 0.f, tzz = 0.f;
     float c0 = 0.f, c1 = 0.f, c2 = 0.f, c3 = 0.f, c4 = 0.f, c5 = 0.f, c6 = 0.f, c7 = 0.f, c8 = 0.f, c9 = 0.f;
     const float4* const planes[1] = {a.posV};
-    leaf_sweep<1, 1, false>(a, planes, leaf, w, 0, lane, tile, [&](int c, bool wrapped) {
-        const float4 pj = tile[c];
+    leaf_sweep<1, 1, false>(a, planes, leaf, w, 0, lane, tile, [&](uint32_t, bool wrapped, const float4& pj) {
         float dx, dy, dz, r2;
         sep3(a, wrapped, xi, yi, zi, pj, dx, dy, dz, r2);
         const float r = r2 * rsqrt_fast(fmaxf(r2, R2_TINY));
@@ -483,9 +496,8 @@ __global__ void __launch_bounds__(W4_WPL * W4_LPC * 32) k_gradv(SweepArgs a, con
     const Coef ci = load_coef(q0, q1, q2, q3);
     float g[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
     const float4* const planes[2] = {a.posV, a.velV};
-    leaf_sweep<W4_WPL, 2, false>(a, planes, leaf, lg, wl, lane, tile, [&](int c, bool wrapped) {
-        const float4 pj = tile[c];
-        const float4 vj = tile[CRK_CCAP + c];
+    leaf_sweep<W4_WPL, 2, false>(a, planes, leaf, lg, wl, lane, tile, [&](uint32_t sa, bool wrapped, const float4& pj) {
+        const float4 vj = lds128(sa + CRK_CCAP * 16u);
         float dx, dy, dz, r2;
         sep3(a, wrapped, xi, yi, zi, pj, dx, dy, dz, r2);
         const float r = r2 * rsqrt_fast(fmaxf(r2, R2_TINY));
@@ -528,7 +540,6 @@ __global__ void __launch_bounds__(W4_WPL * W4_LPC * 32) k_gradv(SweepArgs a, con
 // Q from Eqs. 24-25 with the limited midpoint projection of Eqs. 27-32 (S7: division-free van Leer form).
 // Sums over all j != i with r2 < max(h_i^2, h_j^2); each ordered pair is evaluated on a lane that holds i in registers.
 // One CTA = one leaf: W5_WPL warps share the tile of the leaf's candidates and split each lane's entries by rows.
-constexpr int W5_WPL = 4;
 struct PState {           // one particle's force-sweep state in registers
     float x, y, z, ih, vx, vy, vz, V, P, rho, cs, k3, k5, qh;
     Coef c;
@@ -537,6 +548,19 @@ struct PState {           // one particle's force-sweep state in registers
 __device__ __forceinline__ PState load_pstate(const float4* __restrict__ f, int64_t stride) {
     const float4 a0 = f[0], a1 = f[stride], a2 = f[2 * stride], a3 = f[3 * stride], a4 = f[4 * stride], a5 = f[5 * stride],
                  a6 = f[6 * stride], a7 = f[7 * stride], a8 = f[8 * stride];
+    PState s;
+    s.x = a0.x; s.y = a0.y; s.z = a0.z; s.ih = a0.w;
+    s.vx = a1.x; s.vy = a1.y; s.vz = a1.z; s.V = a1.w;
+    s.P = a2.x; s.rho = a2.y; s.cs = a2.z; s.k3 = a2.w;
+    s.c = load_coef(a3, a4, a5, a6);
+    s.gxx = a7.x; s.gyy = a7.y; s.gzz = a7.z; s.k5 = a7.w;
+    s.gxy = a8.x; s.gxz = a8.y; s.gyz = a8.z; s.qh = a8.w;
+    return s;
+}
+__device__ __forceinline__ PState load_pstate_shared(uint32_t sa, const float4& a0) {
+    constexpr uint32_t ST = CRK_CCAP * 16u;
+    const float4 a1 = lds128(sa + ST), a2 = lds128(sa + 2 * ST), a3 = lds128(sa + 3 * ST), a4 = lds128(sa + 4 * ST),
+                 a5 = lds128(sa + 5 * ST), a6 = lds128(sa + 6 * ST), a7 = lds128(sa + 7 * ST), a8 = lds128(sa + 8 * ST);
     PState s;
     s.x = a0.x; s.y = a0.y; s.z = a0.z; s.ih = a0.w;
     s.vx = a1.x; s.vy = a1.y; s.vz = a1.z; s.V = a1.w;
@@ -555,6 +579,65 @@ __device__ __forceinline__ float quad_form(const PState& s, float dxx, float dyy
 __device__ __forceinline__ float visc_mu(float qh, float udx, float r2, float eps2) {
     return fminf(0.0f, __fmul_rn(__fmul_rn(qh, udx), rcp_fast(__fmaf_rn(__fmul_rn(qh, qh), r2, eps2))));
 }
+struct ForceConst {
+    float L, half, eta_crit, inv_fold, eps2, Cl, Cq;
+};
+// one ordered pair (i, j): accumulates m_i dv_i/dt (acc[0..2]) and m_i du_i/dt (acc[3])
+__device__ __forceinline__ void force_pair(const ForceConst& k, const PState& I, const PState& J, bool wrapped, float (&acc)[4]) {
+    float dx, dy, dz;
+    if (!wrapped) {
+        dx = __fsub_rn(I.x, J.x);
+        dy = __fsub_rn(I.y, J.y);
+        dz = __fsub_rn(I.z, J.z);
+    } else {
+        dx = sep1_wrapped(I.x, J.x, k.L, k.half);
+        dy = sep1_wrapped(I.y, J.y, k.L, k.half);
+        dz = sep1_wrapped(I.z, J.z, k.L, k.half);
+    }
+    const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
+    const float r = __fmul_rn(r2, rsqrt_fast(fmaxf(r2, R2_TINY)));
+    float Wi, Di, Wj, Dj;
+    wendland_dim(r, I.ih, I.k3, I.k5, Wi, Di);
+    wendland_dim(r, J.ih, J.k3, J.k5, Wj, Dj);
+    float aix, aiy, aiz, ajx, ajy, ajz;
+    rk_grad(I.c, dx, dy, dz, Wi, Di, aix, aiy, aiz);            // grad WR_ij
+    rk_grad(J.c, -dx, -dy, -dz, Wj, Dj, ajx, ajy, ajz);         // grad WR_ji  (x_ji = -x_ij)
+    const float Gx = __fsub_rn(ajx, aix), Gy = __fsub_rn(ajy, aiy), Gz = __fsub_rn(ajz, aiz);
+    // Eq. 30: N = x.(grad v_i x), Dn = x.(grad v_j x); every product is even in x, so the mirrored lane forms the same bits
+    const float dxx = __fmul_rn(dx, dx), dyy = __fmul_rn(dy, dy), dzz = __fmul_rn(dz, dz);
+    const float dxy = __fmul_rn(dx, dy), dxz = __fmul_rn(dx, dz), dyz = __fmul_rn(dy, dz);
+    const float Nn = quad_form(I, dxx, dyy, dzz, dxy, dxz, dyz);
+    const float Dn = quad_form(J, dxx, dyy, dzz, dxy, dxz, dyz);
+    // Eq. 29 with r_ij = N/Dn:  phi_VL = 4 N Dn / (N + Dn)^2 if N Dn > 0 else 0  (S7)
+    const float nd = __fmul_rn(Nn, Dn);
+    const float sm = __fadd_rn(Nn, Dn);
+    float phi = (nd > 0.0f) ? fminf(__fmul_rn(4.0f * nd, rcp_fast(__fmul_rn(sm, sm))), 1.0f) : 0.0f;
+    // Eqs. 31-32
+    const float eta = __fmul_rn(r, fminf(I.ih, J.ih));
+    if (eta < k.eta_crit) {
+        const float q = (eta - k.eta_crit) * k.inv_fold;
+        phi *= ex2_fast(-1.4426950408889634f * q * q);
+    }
+    // Eq. 27 (adot = 0): uhat_ij.x_ij = v_ij.x_ij - (1/2) phi x_ij.(grad v_i + grad v_j).x_ij = v_ij.x_ij - (1/2) phi (N + Dn)
+    const float vx = __fsub_rn(I.vx, J.vx), vy = __fsub_rn(I.vy, J.vy), vz = __fsub_rn(I.vz, J.vz);
+    const float vdx = __fmaf_rn(vz, dz, __fmaf_rn(vy, dy, __fmul_rn(vx, dx)));
+    const float udx = __fmaf_rn(__fmul_rn(-0.5f, phi), sm, vdx);
+    // Eqs. 24-25
+    const float Qi = visc_Q(I.rho, I.cs, visc_mu(I.qh, udx, r2, k.eps2), k.Cl, k.Cq);
+    const float Qj = visc_Q(J.rho, J.cs, visc_mu(J.qh, udx, r2, k.eps2), k.Cl, k.Cq);
+    const float PQi = __fadd_rn(I.P, Qi), PQj = __fadd_rn(J.P, Qj);
+    const float hvv = 0.5f * __fmul_rn(I.V, J.V);
+    const float pf = __fmul_rn(hvv, __fadd_rn(PQi, PQj));
+    acc[0] = fmaf(pf, Gx, acc[0]); acc[1] = fmaf(pf, Gy, acc[1]); acc[2] = fmaf(pf, Gz, acc[2]);
+    const float vG = fmaf(vz, Gz, fmaf(vy, Gy, vx * Gx));       // (v_i - v_j).G = -(v_j - v_i).G
+    acc[3] = fmaf(-hvv * PQj, vG, acc[3]);
+}
+
+// One CTA = one leaf: W5_WPL warps share the tile of the leaf's candidates and split each lane's entries by rows; four
+// CTAs are resident per SM, so one CTA's staging (header -> candidates -> state, three dependent global loads) overlaps the
+// other three's pair math.  (A persistent, double-buffered variant with 2 x 8 warps per SM was measured slower: 13.1 vs
+// 11.7 ms -- its per-leaf barrier couples all warps of the SM half; profiles/r01_forces_notes.md.)
+constexpr int W5_WPL = 4;
 __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
@@ -563,53 +646,14 @@ __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
     const int64_t i = leaf * CRK_LEAF + lane;
     const bool valid = i < a.n;
     const PState I = load_pstate(a.fst + i, a.np);
-    const float eta_crit = 1.0f / a.n_h, inv_fold = a.n_h / 0.2f;
-    const float eps2 = a.eps2;
-    const float Cl = a.C_l, Cq = a.C_q;
+    const ForceConst fc = {a.L, a.half, 1.0f / a.n_h, a.n_h / 0.2f, a.eps2, a.C_l, a.C_q};
     float acc[4] = {0.f, 0.f, 0.f, 0.f};                 // Fx, Fy, Fz, dE
     const float4* planes[FPL];
 #pragma unroll
     for (int p = 0; p < FPL; ++p) planes[p] = a.fst + (int64_t)p * a.np;
-    const uint32_t count = leaf_sweep<W5_WPL, FPL, true>(a, planes, leaf, 0, wl, lane, tile, [&](int c, bool wrapped) {
-        const PState J = load_pstate(tile + c, CRK_CCAP);
-        float dx, dy, dz, r2;
-        sep3(a, wrapped, I.x, I.y, I.z, make_float4(J.x, J.y, J.z, 0.f), dx, dy, dz, r2);
-        const float r = __fmul_rn(r2, rsqrt_fast(fmaxf(r2, R2_TINY)));
-        float Wi, Di, Wj, Dj;
-        wendland_dim(r, I.ih, I.k3, I.k5, Wi, Di);
-        wendland_dim(r, J.ih, J.k3, J.k5, Wj, Dj);
-        float aix, aiy, aiz, ajx, ajy, ajz;
-        rk_grad(I.c, dx, dy, dz, Wi, Di, aix, aiy, aiz);            // grad WR_ij
-        rk_grad(J.c, -dx, -dy, -dz, Wj, Dj, ajx, ajy, ajz);         // grad WR_ji  (x_ji = -x_ij)
-        const float Gx = __fsub_rn(ajx, aix), Gy = __fsub_rn(ajy, aiy), Gz = __fsub_rn(ajz, aiz);
-        // Eq. 30: N = x.(grad v_i x), Dn = x.(grad v_j x); every product is even in x, so the mirrored lane forms the same bits
-        const float dxx = __fmul_rn(dx, dx), dyy = __fmul_rn(dy, dy), dzz = __fmul_rn(dz, dz);
-        const float dxy = __fmul_rn(dx, dy), dxz = __fmul_rn(dx, dz), dyz = __fmul_rn(dy, dz);
-        const float Nn = quad_form(I, dxx, dyy, dzz, dxy, dxz, dyz);
-        const float Dn = quad_form(J, dxx, dyy, dzz, dxy, dxz, dyz);
-        // Eq. 29 with r_ij = N/Dn:  phi_VL = 4 N Dn / (N + Dn)^2 if N Dn > 0 else 0  (S7)
-        const float nd = __fmul_rn(Nn, Dn);
-        const float sm = __fadd_rn(Nn, Dn);
-        float phi = (nd > 0.0f) ? fminf(__fmul_rn(4.0f * nd, rcp_fast(__fmul_rn(sm, sm))), 1.0f) : 0.0f;
-        // Eqs. 31-32
-        const float eta = __fmul_rn(r, fminf(I.ih, J.ih));
-        if (eta < eta_crit) {
-            const float q = (eta - eta_crit) * inv_fold;
-            phi *= ex2_fast(-1.4426950408889634f * q * q);
-        }
-        // Eq. 27 (adot = 0): uhat_ij.x_ij = v_ij.x_ij - (1/2) phi x_ij.(grad v_i + grad v_j).x_ij = v_ij.x_ij - (1/2) phi (N + Dn)
-        const float vx = __fsub_rn(I.vx, J.vx), vy = __fsub_rn(I.vy, J.vy), vz = __fsub_rn(I.vz, J.vz);
-        const float vdx = __fmaf_rn(vz, dz, __fmaf_rn(vy, dy, __fmul_rn(vx, dx)));
-        const float udx = __fmaf_rn(__fmul_rn(-0.5f, phi), sm, vdx);
-        // Eqs. 24-25
-        const float Qi = visc_Q(I.rho, I.cs, visc_mu(I.qh, udx, r2, eps2), Cl, Cq);
-        const float Qj = visc_Q(J.rho, J.cs, visc_mu(J.qh, udx, r2, eps2), Cl, Cq);
-        const float PQi = __fadd_rn(I.P, Qi), PQj = __fadd_rn(J.P, Qj);
-        const float hvv = 0.5f * __fmul_rn(I.V, J.V);
-        const float pf = __fmul_rn(hvv, __fadd_rn(PQi, PQj));
-        acc[0] = fmaf(pf, Gx, acc[0]); acc[1] = fmaf(pf, Gy, acc[1]); acc[2] = fmaf(pf, Gz, acc[2]);
-        const float vG = fmaf(vz, Gz, fmaf(vy, Gy, vx * Gx));       // (v_i - v_j).G = -(v_j - v_i).G
-        acc[3] = fmaf(-hvv * PQj, vG, acc[3]);
+    const uint32_t count = leaf_sweep<W5_WPL, FPL, true>(a, planes, leaf, 0, wl, lane, tile, [&](uint32_t sa, bool wrapped, const float4& p0) {
+        const PState J = load_pstate_shared(sa, p0);
+        force_pair(fc, I, J, wrapped, acc);
     });
     group_reduce<W5_WPL, 4>(acc, 0, wl, lane, (float*)tile);
     if (wl == 0 && valid) {
