@@ -35,6 +35,9 @@ UNIT = "pair-interactions/s"
 # canonical algorithmic FP32 flops per accepted ordered pair (restated in DESIGN.md)
 FLOPS_PER_PAIR = {"volumes": 16.0, "moments": 100.0, "gradv": 90.0, "forces": 250.0}
 FP32_PEAK_THEORETICAL = 148 * 128 * 2 * 1.965e9     # SMs x FP32 lanes x 2 (FMA) x max SM clock
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_forces launch on the default workload (cosmo 256^3), from the
+# ncu --set full capture summarised in profiles/r01_sweeps_v5_ncu_full.md; other workloads report null
+FORCES_DRAM_BYTES_COSMO256 = 6.10e9 + 0.27e9
 
 
 BASE_SEEDS = {"tiny_uniform": 1001, "blast_wave": 1002, "clustered": 1003, "cosmo": 1004, "cosmo_large": 1005}
@@ -244,7 +247,8 @@ def run_ours(args, rank, world, local_rank):
                 "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md); FFMA micro-benchmark measured "
                                f"{fp32_meas / 1e12:.1f} TFLOP/s in this run",
                 "flops_per_pair": FLOPS_PER_PAIR["forces"], "pairs_per_launch": sym_pairs, "kernel_ms": forces_ms,
-                "traffic": None}
+                "traffic": FORCES_DRAM_BYTES_COSMO256 if (ps.name == "cosmo" and ps.meta["n_side"] == 256) else None,
+                "traffic_unit": "bytes per launch (ncu dram read + write; algorithmic minimum = 160 B/particle = 2.7e9)"}
     passes = {k: st[k] for k in ("ms_sort", "ms_tree", "ms_lists", "ms_volumes", "ms_rk", "ms_gradv", "ms_forces")}
     alg_flops = (FLOPS_PER_PAIR["volumes"] + FLOPS_PER_PAIR["moments"] + FLOPS_PER_PAIR["gradv"]) * gather_pairs + forces_flops
     sweeps_ms = st["ms_volumes"] + st["ms_rk"] + st["ms_gradv"] + st["ms_forces"]
@@ -286,7 +290,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", default="cosmo", choices=list(wl.CONFIG_NAMES))
     ap.add_argument("--n-side", type=int, default=None)
-    ap.add_argument("--oracle-particles", type=int, default=80000)
+    ap.add_argument("--oracle-particles", type=int, default=262144,
+                    help="size of the bounded sample handed to the O(n^2) oracle (262144 particles ~ 10-20 s of CPU work)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))

@@ -284,3 +284,60 @@ def test_parity_config4_cosmo_full(oracle_mod):
     g = _window_check(ps, oracle_mod, centres, half_in_h=3.0, label="cosmo256")
     st = g["stats"]
     print(f"[stats] cosmo256 leaves={st['n_leaves']} leaf_pairs={st['n_leaf_pairs']} launches={st['launches']}")
+
+
+def test_parity_config5_cosmo_large_full(oracle_mod):
+    """BASELINE configs[4]: 512^3 = 134 M particles, rms displacement 1.5 spacings (shell-crossed, wide h range).  The
+    full outputs stay on the GPU (invariants are reduced there in FP64); only the padded oracle windows come back."""
+    torch = _torch()
+    from paper_2202_02840_b200 import Crk
+    ps = wl.make_config("cosmo_large")
+    dev = torch.device("cuda:0")
+    t = {k: torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).to(dev) for k in
+         ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")}
+    ctx = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h)
+    ctx.set_timing(True)
+    ctx.build_cells(t["x"], t["y"], t["z"], t["h"])
+    V, rho, cnt = ctx.volumes(t["m"])
+    A, B, gA, gB = ctx.rk_coefficients()
+    ax, ay, az, du, pc = ctx.hydro_derivs(t["vx"], t["vy"], t["vz"], t["u"])
+    gv = ctx.gradv()
+    torch.cuda.synchronize()
+    st = ctx.stats()
+    print(f"[stats] cosmo512 n={ps.n} leaves={st['n_leaves']} leaf_pairs={st['n_leaf_pairs']} ms: sort {st['ms_sort']:.1f} "
+          f"tree {st['ms_tree']:.1f} lists {st['ms_lists']:.1f} volumes {st['ms_volumes']:.1f} rk {st['ms_rk']:.1f} "
+          f"gradv {st['ms_gradv']:.1f} forces {st['ms_forces']:.1f}; mean gather neighbours "
+          f"{float(cnt.to(torch.float64).mean()):.1f}, h max/min {float(ps.h.max() / ps.h.min()):.1f}")
+    # conservation invariants on the full output, FP64 on the device
+    m = t["m"].double()
+    a3 = [q.double() for q in (ax, ay, az)]
+    v3 = [t[k].double() for k in ("vx", "vy", "vz")]
+    amag = torch.sqrt(a3[0] ** 2 + a3[1] ** 2 + a3[2] ** 2)
+    mom = max(abs(float((m * a3[q]).sum())) for q in range(3)) / float((m * amag).sum())
+    work = m * (v3[0] * a3[0] + v3[1] * a3[1] + v3[2] * a3[2])
+    en = abs(float((work + m * du.double()).sum())) / (float((m * du.double().abs()).sum()) + float(work.abs().sum()))
+    assert mom < TOL_INV and en < TOL_INV, (mom, en)
+    del m, a3, v3, amag, work
+    full = dict(V=V, rho=rho, nbr_count=cnt, A=A, B=B, gradA=gA, gradB=gB, ax=ax, ay=ay, az=az, dudt=du, pair_count=pc, gradv=gv)
+    done = 0
+    dens = int(np.argmin(ps.h))
+    centres = [(0.5, 0.5, 0.5), (0.0005, 0.9995, 0.5), (float(ps.x[dens]), float(ps.y[dens]), float(ps.z[dens]))]
+    for c in centres:
+        idx0, _ = wl.select_window(ps, c, 0.01, 0.0)
+        if len(idx0) == 0:
+            continue
+        win = _pick_window(ps, c, 2.5 * float(np.median(ps.h[idx0])))
+        if win is None:
+            print(f"[parity] cosmo512 window@{np.round(c, 4)} skipped (too many particles in the padded window)")
+            continue
+        idxp, corep = win
+        sub = ps.subset(idxp)
+        o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+        od = o.step_derivs(sub)
+        sel = torch.from_numpy(idxp).to(dev)
+        gs = {k: (v[sel] if v.ndim == 1 else v[:, sel]).cpu().numpy() for k, v in full.items()}
+        e_a, e_u = check_parity(sub, gs, od, oracle_gv=o.gradv(), mask=corep, label=f"cosmo512 window@{np.round(c, 4)}")
+        print(f"[parity] cosmo512 window n={len(idxp)} core={int(corep.sum())}: dv/dt {e_a:.2e} du/dt {e_u:.2e} "
+              f"momentum {mom:.2e} energy {en:.2e}")
+        done += 1
+    assert done >= 1
