@@ -56,6 +56,14 @@ __global__ void __launch_bounds__(256) k_keys_pack(const float* __restrict__ x, 
                                                    uint32_t* __restrict__ vals, float4* __restrict__ posh_orig,
                                                    int* __restrict__ flag) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    // smallest support radius of the set -> flag[1] (encoded so that a zero-initialised atomicMax finds the minimum);
+    // it decides how many key bits are worth sorting (crk_sort_particles)
+    {
+        const float hv = (i < n) ? h[i] : 3.0e38f;
+        uint32_t enc = (hv > 0.f && hv < 3.0e38f) ? 0x7f800000u - __float_as_uint(hv) : 0u;
+        enc = __reduce_max_sync(0xffffffffu, enc);
+        if ((threadIdx.x & 31) == 0 && enc != 0u) atomicMax((unsigned int*)flag + 1, enc);
+    }
     if (i >= n) return;
     const float xi = x[i], yi = y[i], zi = z[i], hi = h[i];
     const bool ok = (xi >= 0.f) && (xi < L) && (yi >= 0.f) && (yi < L) && (zi >= 0.f) && (zi < L) && (hi > 0.f) &&
@@ -100,21 +108,32 @@ __global__ void __launch_bounds__(SORT_THREADS) k_radix_scatter(const uint64_t* 
     const int64_t wbase = (int64_t)blockIdx.x * SORT_TILE + (int64_t)w * (32 * SORT_ROUNDS);
     uint64_t k[SORT_ROUNDS];
     uint32_t v[SORT_ROUNDS];
-    uint32_t rk[SORT_ROUNDS];
+    uint32_t rk[SORT_ROUNDS];     // first: digit | rank among equal digits of the round << 9 | group size << 15 ; then: final rank
     const uint32_t lt = (1u << lane) - 1u;
+    // phase 1 (independent per round, so the loads and the match instructions overlap): digit, rank within the round
 #pragma unroll
     for (int r = 0; r < SORT_ROUNDS; ++r) {
         const int64_t idx = wbase + r * 32 + lane;
         const bool valid = idx < n;
         k[r] = valid ? keys_in[idx] : 0ull;
         v[r] = valid ? vals_in[idx] : 0u;
+    }
+#pragma unroll
+    for (int r = 0; r < SORT_ROUNDS; ++r) {
+        const bool valid = (wbase + r * 32 + lane) < n;
         const uint32_t d = valid ? ((uint32_t)(k[r] >> shift) & (RADIX - 1)) : (uint32_t)RADIX;
         const uint32_t peers = __match_any_sync(0xffffffffu, d);
-        const uint32_t rank = __popc(peers & lt);
+        rk[r] = d | ((uint32_t)__popc(peers & lt) << 9) | ((uint32_t)__popc(peers) << 15);
+    }
+    // phase 2 (serial over rounds: stable counts per warp and digit)
+#pragma unroll
+    for (int r = 0; r < SORT_ROUNDS; ++r) {
+        const uint32_t d = rk[r] & 0x1ffu, rank = (rk[r] >> 9) & 0x3fu, gsz = rk[r] >> 15;
+        const bool valid = d < (uint32_t)RADIX;
         uint32_t prev = 0;
         if (valid) prev = wcnt[w][d];
         __syncwarp();
-        if (valid && rank == 0) wcnt[w][d] = prev + __popc(peers);
+        if (valid && rank == 0) wcnt[w][d] = prev + gsz;
         __syncwarp();
         rk[r] = prev + rank;
     }
@@ -275,8 +294,28 @@ int crk_sort_particles(crk_ctx* c, const float* x, const float* y, const float* 
                                                                     (uint32_t*)c->vals[0].p, (float4*)c->posh_orig.p,
                                                                     (int*)c->flag.p);
     CRK_TRY(crk_check_launch(c, "k_keys_pack"));
+    // Key bits worth sorting: cells of half the smallest support radius order everything the leaves need (a finer
+    // order inside such a cell does not make a 32-particle leaf more compact than its h).  The top 3 b bits of a Hilbert
+    // key are the key of the b-bit grid, so the low passes are simply skipped.  One 4-byte read-back (h_min).
+    CRK_CUDA(c, cudaMemcpyAsync(c->h_flag + 12, (int*)c->flag.p + 1, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CRK_CUDA(c, cudaStreamSynchronize(c->stream));
+    int bits = CRK_KEY_BITS;
+    {
+        const uint32_t enc = (uint32_t)c->h_flag[12];
+        if (enc != 0u) {
+            const uint32_t hb = 0x7f800000u - enc;
+            float hmin;
+            memcpy(&hmin, &hb, sizeof(hmin));
+            if (hmin > 0.f) {
+                const double cells = 2.0 * (double)c->prm.box / (double)hmin;
+                bits = 1;
+                while (bits < CRK_KEY_BITS && (double)(1u << bits) < cells) ++bits;
+            }
+        }
+        if (bits < 6) bits = 6;
+    }
     int cur = 0;
-    for (int shift = 0; shift < 3 * CRK_KEY_BITS; shift += RADIX_BITS) {
+    for (int shift = 3 * (CRK_KEY_BITS - bits); shift < 3 * CRK_KEY_BITS; shift += RADIX_BITS) {
         k_radix_hist<<<nblk, SORT_THREADS, 0, c->stream>>>((const uint64_t*)c->keys[cur].p, n, shift, hist, nblk);
         CRK_TRY(crk_check_launch(c, "k_radix_hist"));
         CRK_TRY(crk_exclusive_scan_u32(c, hist, offs, (int64_t)RADIX * nblk, c->scan_tmp));
