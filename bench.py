@@ -252,7 +252,7 @@ def run_ours(args, rank, world, local_rank):
     passes = {k: st[k] for k in ("ms_sort", "ms_tree", "ms_lists", "ms_volumes", "ms_rk", "ms_gradv", "ms_forces")}
     alg_flops = (FLOPS_PER_PAIR["volumes"] + FLOPS_PER_PAIR["moments"] + FLOPS_PER_PAIR["gradv"]) * gather_pairs + forces_flops
     sweeps_ms = st["ms_volumes"] + st["ms_rk"] + st["ms_gradv"] + st["ms_forces"]
-    sort_bytes = ps.n * (6 * 32.0 + 16 + 12 + 32 + 16)    # radix passes + pack + gather
+    sort_bytes = ps.n * (st["sort_passes"] * 32.0 + 16 + 12 + 32 + 16)    # radix passes + pack + gather
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",

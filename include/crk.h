@@ -68,6 +68,7 @@ typedef struct {
     float    ms_sort, ms_tree, ms_gradv, ms_forces;   /* finer split: sort+pack | leaves+leaf list | Eq.26 | Eqs.17-18 */
     float    ms_lists;        /* per-particle neighbour lists (third part of crk_build_cells)                  */
     int32_t  timed_steps;     /* number of completed steps the ms_* fields average over (event ring of 64)    */
+    int32_t  sort_passes;     /* 8-bit radix passes of the last build (key bits follow the smallest h)         */
 } crk_stats;
 
 /* stream: a cudaStream_t (0 = default stream).  Returns CRK_OK and *out, or an error.                       */

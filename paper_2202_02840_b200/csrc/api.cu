@@ -223,6 +223,7 @@ int crk_get_stats(crk_ctx* c, crk_stats* out) {
     out->launches = c->launches;
     out->scratch_bytes = (int64_t)c->scratch_bytes;
     out->list_bytes = c->arena_units * 16;
+    out->sort_passes = c->st.sort_passes;
     if (c->timing && c->n > 0) {
         // mean over the completed steps still held in the event ring (all steps since crk_reset_stats if <= 64)
         CRK_CUDA(c, cudaStreamSynchronize(c->stream));

@@ -315,6 +315,7 @@ int crk_sort_particles(crk_ctx* c, const float* x, const float* y, const float* 
         if (bits < 6) bits = 6;
     }
     int cur = 0;
+    c->st.sort_passes = (3 * bits + RADIX_BITS - 1) / RADIX_BITS;
     for (int shift = 3 * (CRK_KEY_BITS - bits); shift < 3 * CRK_KEY_BITS; shift += RADIX_BITS) {
         k_radix_hist<<<nblk, SORT_THREADS, 0, c->stream>>>((const uint64_t*)c->keys[cur].p, n, shift, hist, nblk);
         CRK_TRY(crk_check_launch(c, "k_radix_hist"));
