@@ -74,6 +74,7 @@ struct crk_oracle_ctx {
     std::vector<Coef> coef;
     std::vector<Moments> mom;
     std::vector<double> vx, vy, vz, u, P, cs;
+    std::vector<double> ax, ay, az;              // dv/dt of the last crk_oracle_hydro_derivs (Eq. 17), for Eqs. 19-23
     std::vector<double> gradv;                   // [i][alpha][beta] = d_beta v^alpha  (Eq. 26, reading S9)
     int stage = 0;                               // 0 none, 1 built, 2 volumes, 3 coefficients, 4 hydro
 };
@@ -390,6 +391,7 @@ int crk_oracle_hydro_derivs(crk_oracle_ctx* c, const float* vx, const float* vy,
     const int64_t n = c->n;
     c->vx.assign(vx, vx + n); c->vy.assign(vy, vy + n); c->vz.assign(vz, vz + n); c->u.assign(u, u + n);
     c->P.resize(n); c->cs.resize(n); c->gradv.assign((size_t)9 * n, 0.0);
+    c->ax.resize(n); c->ay.resize(n); c->az.resize(n);
     const double g = c->p.gamma;
     for (int64_t i = 0; i < n; ++i) {
         c->P[i] = (g - 1.0) * c->rho[i] * c->u[i];                        // Eq. 4 (unclamped, reading S12)
@@ -426,6 +428,7 @@ int crk_oracle_hydro_derivs(crk_oracle_ctx* c, const float* vx, const float* vy,
             ++cnt;
         }
         const double im = 1.0 / c->m[i];
+        c->ax[i] = F[0] * im; c->ay[i] = F[1] * im; c->az[i] = F[2] * im;
         if (ax) ax[i] = F[0] * im;
         if (ay) ay[i] = F[1] * im;
         if (az) az[i] = F[2] * im;
@@ -433,6 +436,64 @@ int crk_oracle_hydro_derivs(crk_oracle_ctx* c, const float* vx, const float* vy,
         if (pair_count) pair_count[i] = cnt;
     }
     c->stage = 4;
+    return 0;
+}
+
+// ---- NEXT row 1: compatible energy update, Eqs. 19-23, a = 1, adot = 0, p = v ----------------------
+// Eq. 22: v'_i = v_i + (dv_i/dt) dt.   Eq. 20: du_ij = (f_ij / 2) (v_j + v'_j - v_i - v'_i) . a_ij with a_ij the pairwise
+// acceleration of Eq. 17 (P -> P + Q).   Eq. 21: dE_ij = m_i du_ij + m_j du_ji; because m_i a_ij = -m_j a_ji
+// and f_ij + f_ji = 1 this is (1/2) m_i a_ij . (v_j + v'_j - v_i - v'_i) whatever f is, which is how its sign is taken.
+// Eq. 23 as printed is garbled; reading G1: f_ij = min(s_i,s_j)/(s_i+s_j) if (dE_ij >= 0 and s_i >= s_j) or
+// (dE_ij < 0 and s_i < s_j), else max(s_i,s_j)/(s_i+s_j), s = P / rho^gamma  ("cooler nodes are heated or hotter nodes
+// are cooled", f_ij + f_ji = 1).  Reading S16: if either entropy is not positive (u <= 0, config 2's unstable steps),
+// f_ij = 1/2.   Eq. 19: Delta u_i = sum_j du_ij dt.
+struct CompatOut { double du, dE, f; };
+inline void pair_compat(const crk_oracle_ctx* c, int64_t i, int64_t j, double dt, CompatOut& o) {
+    PairOut po;
+    pair_term(c, i, j, po);                                   // po.F = m_i a_ij
+    const double im = 1.0 / c->m[i];
+    const double aij[3] = {po.F[0] * im, po.F[1] * im, po.F[2] * im};
+    const double vi[3] = {c->vx[i], c->vy[i], c->vz[i]}, vj[3] = {c->vx[j], c->vy[j], c->vz[j]};
+    const double ai[3] = {c->ax[i], c->ay[i], c->az[i]}, aj[3] = {c->ax[j], c->ay[j], c->az[j]};
+    double w = 0.0;
+    for (int q = 0; q < 3; ++q) {
+        const double vpi = vi[q] + ai[q] * dt, vpj = vj[q] + aj[q] * dt;          // Eq. 22
+        w += (vj[q] + vpj - vi[q] - vpi) * aij[q];
+    }
+    o.dE = 0.5 * c->m[i] * w;                                                     // Eq. 21
+    const double g = c->p.gamma;
+    const double si = c->P[i] / std::pow(c->rho[i], g), sj = c->P[j] / std::pow(c->rho[j], g);
+    double f = 0.5;
+    if (si > 0.0 && sj > 0.0) {
+        const bool small = (o.dE >= 0.0 && si >= sj) || (o.dE < 0.0 && si < sj);
+        f = (small ? std::min(si, sj) : std::max(si, sj)) / (si + sj);            // Eq. 23 (reading G1)
+    }
+    o.f = f;
+    o.du = 0.5 * f * w;                                                           // Eq. 20
+}
+
+int crk_oracle_compatible_energy(crk_oracle_ctx* c, double dt, double* delta_u) {
+    if (!c || c->stage < 4 || !delta_u) return -1;
+    set_threads();
+    const int64_t n = c->n;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < n; ++i) {
+        double s = 0.0;
+        for (int64_t k = c->off[i]; k < c->off[i + 1]; ++k) {
+            CompatOut o;
+            pair_compat(c, i, (int64_t)(c->nbr[k] & IDX_MASK), dt, o);
+            s += o.du;
+        }
+        delta_u[i] = s * dt;                                                      // Eq. 19 with adot = 0
+    }
+    return 0;
+}
+
+int crk_oracle_pair_compat(crk_oracle_ctx* c, int64_t i, int64_t j, double dt, double out[3]) {
+    if (!c || c->stage < 4 || i < 0 || j < 0 || i >= c->n || j >= c->n || i == j) return -1;
+    CompatOut o;
+    pair_compat(c, i, j, dt, o);
+    out[0] = o.du; out[1] = o.dE; out[2] = o.f;
     return 0;
 }
 

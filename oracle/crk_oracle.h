@@ -53,6 +53,14 @@ int crk_oracle_step_derivs(crk_oracle_ctx* c, int64_t n, const float* x, const f
                            const float* h, const float* vx, const float* vy, const float* vz, const float* m,
                            const float* u, double* ax, double* ay, double* az, double* dudt);
 
+/* NEXT row 1 -- compatible energy update, Eqs. 19-23 with a = 1, adot = 0, after
+ * crk_oracle_hydro_derivs: delta_u[i] = dt * sum_j (f_ij/2) (v_j + v'_j - v_i - v'_i) . a_ij, v' = v + (dv/dt) dt.
+ * Pinned: sum_i m_i delta_u_i + Delta KE = 0 to roundoff, f_ij + f_ji = 1, the heating/cooling rule of PAPER.md:141.
+ * PARITY UNPINNED: the exact form of the garbled Eq. 23 (reading G1) and f = 1/2 for s <= 0 (S16).      */
+int crk_oracle_compatible_energy(crk_oracle_ctx* c, double dt, double* delta_u);
+/* one pair of the above: out = { du_ij (Eq. 20), dE_ij (Eq. 21), f_ij (Eq. 23) }                                 */
+int crk_oracle_pair_compat(crk_oracle_ctx* c, int64_t i, int64_t j, double dt, double out[3]);
+
 /* ---- diagnostics used by the pins (tests only) ---- */
 double crk_oracle_W(double r, double h);        /* Eq. 12                                   */
 double crk_oracle_dWdr(double r, double h);     /* its radial derivative                    */

@@ -49,6 +49,8 @@ def lib():
         L.crk_oracle_eval_AB_at.argtypes = [C.c_void_p, dp, C.c_double, dp, dp]
         L.crk_oracle_pair_term.argtypes = [C.c_void_p, C.c_int64, C.c_int64, dp]
         L.crk_oracle_pair_visc.argtypes = [C.c_void_p, C.c_int64, C.c_int64, dp]
+        L.crk_oracle_compatible_energy.argtypes = [C.c_void_p, C.c_double, dp]
+        L.crk_oracle_pair_compat.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_double, dp]
         L.crk_oracle_neighbors.restype = C.c_int64
         L.crk_oracle_neighbors.argtypes = [C.c_void_p, C.c_int64, up, C.c_int64]
         _lib = L
@@ -137,6 +139,17 @@ class Oracle:
         ax, ay, az, du, pc = self.hydro_derivs(ps.vx, ps.vy, ps.vz, ps.u)
         return dict(V=V, rho=rho, nbr_count=nbr, A=A, B=B, gradA=gA, gradB=gB,
                     ax=ax, ay=ay, az=az, dudt=du, pair_count=pc)
+
+    def compatible_energy(self, dt):
+        """Eqs. 19-23: Delta u over dt from the pairwise accelerations of the last hydro_derivs"""
+        du = np.empty(self.n)
+        assert lib().crk_oracle_compatible_energy(self._c, float(dt), _d(du)) == 0
+        return du
+
+    def pair_compat(self, i, j, dt):
+        out = np.empty(3)
+        assert lib().crk_oracle_pair_compat(self._c, int(i), int(j), float(dt), _d(out)) == 0
+        return out   # du_ij, dE_ij, f_ij
 
     # ---- diagnostics for the pins
     def moments(self):

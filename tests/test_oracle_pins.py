@@ -345,3 +345,77 @@ def test_euler_steps_update_rule(oracle_mod):
     assert np.allclose(st1.vx, st0.vx + d0["ax"] * dt, rtol=1e-6, atol=1e-9)
     assert np.allclose(st1.u, st0.u + d0["dudt"] * dt, rtol=1e-6, atol=1e-12)
     assert np.array_equal(st1.h, st0.h)
+
+
+# ---------------------------------------------------------------------------------------- NEXT row 1: Eqs. 19-23
+@pytest.mark.parametrize("which", ["tiny", "clustered"])
+def test_compatible_energy_conserves_total_energy_exactly(which, tiny, clustered):
+    """'Any definition of f_ij will uphold energy conservation as long as f_ij + f_ji = 1': the thermal
+    energy gained over dt equals the kinetic energy lost by v -> v' = v + a dt (Eq. 22), to roundoff, for ANY dt."""
+    ps, o, d = tiny if which == "tiny" else clustered
+    m = ps.m.astype(np.float64)
+    v = np.stack([ps.vx, ps.vy, ps.vz]).astype(np.float64)
+    a = np.stack([d["ax"], d["ay"], d["az"]])
+    for dt in (1e-4, 1e-2, 0.3):
+        du = o.compatible_energy(dt)
+        vp = v + a * dt
+        dke = 0.5 * (m * ((vp ** 2).sum(0) - (v ** 2).sum(0))).sum()
+        dth = (m * du).sum()
+        scale = (m * np.abs(du)).sum() + 1e-300
+        assert abs(dke + dth) / scale < 1e-11, (dt, dke, dth)
+
+
+def test_compatible_energy_pair_partition_rules(clustered):
+    """Eq. 21 (dE_ij = m_i du_ij + m_j du_ji), f_ij + f_ji = 1, and the rule of PAPER.md:141: when the pair's work heats
+    (dE > 0) the lower-entropy particle takes the larger share, when it cools (dE < 0) the higher-entropy one does."""
+    ps, o, d = clustered
+    m = ps.m.astype(np.float64)
+    rho = d["rho"]
+    s = (ps.gamma - 1.0) * ps.u.astype(np.float64) * rho ** (1.0 - ps.gamma)       # s = P / rho^gamma
+    rng = np.random.default_rng(5)
+    dt = 1e-3
+    seen = {"heat": 0, "cool": 0}
+    for i in rng.integers(0, ps.n, 60):
+        js, _, _ = o.neighbors(i)
+        for j in js[:6]:
+            du_ij, dE_ij, f_ij = o.pair_compat(i, j, dt)
+            du_ji, dE_ji, f_ji = o.pair_compat(j, i, dt)
+            assert abs(f_ij + f_ji - 1.0) < 1e-14
+            assert abs(dE_ij - dE_ji) <= 1e-12 * max(abs(dE_ij), 1e-300)
+            assert abs(m[i] * du_ij + m[j] * du_ji - dE_ij) <= 1e-12 * abs(dE_ij) + 1e-300
+            assert 0.0 <= f_ij <= 1.0
+            if s[i] == s[j] or dE_ij == 0.0:
+                continue
+            cooler_is_i = s[i] < s[j]
+            if dE_ij > 0:
+                assert (f_ij > 0.5) == cooler_is_i
+                seen["heat"] += 1
+            else:
+                assert (f_ij < 0.5) == cooler_is_i
+                seen["cool"] += 1
+    assert seen["heat"] > 10 and seen["cool"] > 10
+
+
+def test_compatible_energy_small_dt_limit_and_uniform_entropy(oracle_mod):
+    """(i) Uniform entropy => f = 1/2, so Delta u_i / dt -> (1/2) sum_j (v_j - v_i) . a_ij as dt -> 0: rebuilt here from
+    the pair diagnostic of Eq. 17 (a different code path).  (ii) The total heating rate equals that of Eq. 18."""
+    ps = wl.tiny_uniform(n_side=8)
+    # uniform entropy: u = s rho^(gamma-1) / (gamma-1); rho is only known after the volume pass, so iterate once
+    o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+    d0 = o.step_derivs(ps)
+    ps.u[:] = (1.3 * d0["rho"] ** (ps.gamma - 1.0) / (ps.gamma - 1.0)).astype(np.float32)
+    d = o.step_derivs(ps)
+    m = ps.m.astype(np.float64)
+    v = np.stack([ps.vx, ps.vy, ps.vz]).astype(np.float64)
+    dt = 1e-9
+    du = o.compatible_energy(dt) / dt
+    for i in (0, 17, 300):
+        js, _, _ = o.neighbors(i)
+        ref = 0.0
+        for j in js:
+            F = o.pair_term(i, j)[:3]                  # m_i a_ij
+            _, _, f = o.pair_compat(i, j, dt)
+            assert abs(f - 0.5) < 2e-7                 # float32 u => entropies equal to rounding only
+            ref += 0.5 * np.dot(v[:, j] - v[:, i], F / m[i])
+        assert abs(du[i] - ref) <= 1e-6 * abs(ref) + 1e-12
+    assert abs((m * du).sum() - (m * d["dudt"]).sum()) <= 1e-7 * (m * np.abs(d["dudt"])).sum()
