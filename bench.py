@@ -216,6 +216,19 @@ def run_ours(args, rank, world, local_rank):
     clocks = sampler.stop() if rank == 0 else None
     launches = st["launches"]
 
+    # NEXT row 1 (compatible energy sweep, Eqs. 19-23) on the resident state: reported beside the step, not part of it
+    du = torch.empty(ps.n, device=dev)
+    ctx.compatible_energy(1e-3, out=du)
+    torch.cuda.synchronize()
+    c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    c0.record()
+    for _ in range(3):
+        ctx.compatible_energy(1e-3, out=du)
+    c1.record()
+    torch.cuda.synchronize()
+    compat_ms = c0.elapsed_time(c1) / 3
+    del du
+
     # end to end through the host-pointer C ABI entry (pinned host inputs -> device -> compute -> host outputs)
     oh = [torch.empty(ps.n).pin_memory() for _ in range(4)]
     ctx.set_timing(False)
@@ -269,6 +282,8 @@ def run_ours(args, rank, world, local_rank):
         "e2e": {"value": pairs_all / (e2e_all * 1e-3), "unit": UNIT, "ms_per_step": e2e_all,
                 "h2d_bytes_per_step": int(9 * 4 * n_all), "d2h_bytes_per_step": int(4 * 4 * n_all)},
         "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
+        "next_rows": {"compatible_energy_ms": compat_ms,
+                      "compatible_energy_fp32_frac": (FLOPS_PER_PAIR["forces"] + 20.0) * sym_pairs / (compat_ms * 1e-3) / FP32_PEAK_THEORETICAL},
     }
     if world == 1 and not args.no_cpu_baseline:
         sub, half = oracle_sample(ps, args.oracle_particles)

@@ -96,6 +96,14 @@ int  crk_step_derivs_host(crk_ctx* c, int64_t n, const float* x, const float* y,
                           const float* vx, const float* vy, const float* vz, const float* m, const float* u,
                           float* ax, float* ay, float* az, float* dudt);
 
+/* ---- NEXT row 1: compatible energy update, Eqs. 19-23, PAPER.md:126-141 -------------
+ * After crk_hydro_derivs (else CRK_ESTATE).  With a = 1, adot = 0, p = v:
+ *   delta_u[i] = dt * sum_j (f_ij / 2) (v_j + v'_j - v_i - v'_i) . a_ij,   v' = v + (dv/dt) dt  (Eq. 22),
+ * a_ij = the pairwise acceleration of Eq. 17 (with Q), f_ij the entropy-weighted partition of Eq. 23 (DESIGN.md reading
+ * G1; 1/2 when an entropy P / rho^gamma is not positive).  sum_i m_i delta_u_i = -(kinetic energy change of v -> v').
+ * delta_u: device float[n], caller order, written.  One more symmetric pair sweep on the resident state.          */
+int  crk_compatible_energy(crk_ctx* c, float dt, float* delta_u);
+
 /* ---- diagnostics ---- */
 const char* crk_last_error(const crk_ctx* c);
 int  crk_get_perm(crk_ctx* c, int32_t* perm);        /* device int32[n]: perm[k] = caller index of sorted slot k   */

@@ -11,7 +11,7 @@ _LIB_PATH = os.path.join(_HERE, "libcrk.so")
 
 EXPORTED_SYMBOLS = (
     "crk_create", "crk_destroy", "crk_build_cells", "crk_volumes", "crk_rk_coefficients", "crk_hydro_derivs",
-    "crk_step_derivs", "crk_step_derivs_host", "crk_last_error", "crk_get_perm", "crk_get_gradv", "crk_get_leaf_segments", "crk_get_stats",
+    "crk_step_derivs", "crk_step_derivs_host", "crk_compatible_energy", "crk_last_error", "crk_get_perm", "crk_get_gradv", "crk_get_leaf_segments", "crk_get_stats",
     "crk_reset_stats", "crk_set_timing", "crk_get_leaf_list", "crk_measure_fp32_peak",
 )
 
@@ -72,6 +72,7 @@ def _load():
     L.crk_last_error.restype = C.c_char_p
     L.crk_get_perm.argtypes = [vp, vp]
     L.crk_get_gradv.argtypes = [vp, vp]
+    L.crk_compatible_energy.argtypes = [vp, C.c_float, vp]
     L.crk_get_leaf_segments.argtypes = [vp, vp]
     L.crk_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.crk_reset_stats.argtypes = [vp]
@@ -180,6 +181,12 @@ class Crk:
         self._chk(self._L.crk_step_derivs_host(self._h, n, *[C.c_void_p(t.data_ptr()) for t in (x, y, z, h, vx, vy, vz, m, u)],
                                                *[C.c_void_p(t.data_ptr()) for t in out]))
         return out
+
+    def compatible_energy(self, dt: float, out=None):
+        """Eqs. 19-23 after hydro_derivs: Delta u over dt, caller order"""
+        du = out if out is not None else torch.empty(self.n, device=self._dev)
+        self._chk(self._L.crk_compatible_energy(self._h, C.c_float(dt), _dev(du)))
+        return du
 
     # ---- diagnostics
     def perm(self):

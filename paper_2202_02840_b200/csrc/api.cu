@@ -184,6 +184,16 @@ int crk_get_perm(crk_ctx* c, int32_t* perm) {
     return CRK_OK;
 }
 
+int crk_compatible_energy(crk_ctx* c, float dt, float* delta_u) {
+    if (!c || !delta_u || !(dt == dt)) return CRK_EINVAL;
+    if (c->stage < 4) {
+        snprintf(c->err, sizeof(c->err), "crk_compatible_energy needs crk_hydro_derivs first");
+        return CRK_ESTATE;
+    }
+    if (c->n == 0) return CRK_OK;
+    return crk_launch_compat(c, dt, delta_u);
+}
+
 int crk_get_leaf_segments(crk_ctx* c, uint32_t* seg) {
     if (!c || !seg) return CRK_EINVAL;
     if (c->stage < 1) return CRK_ESTATE;

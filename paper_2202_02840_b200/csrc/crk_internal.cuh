@@ -76,7 +76,7 @@ struct crk_ctx {
     DevBuf posV;                   // float4 (x,y,z,V)
     DevBuf rho_s;                  // float
     DevBuf coef;                   // 4 planes float4[n]: (A,Bx,By,Bz) (cx,cy,cz,M00) (M01,M02,M10,M11) (M12,M20,M21,M22)
-    DevBuf fst;                    // force-sweep state, 9 planes float4[np] (layout at k_forces in pairs.cu)
+    DevBuf fst;                    // force-sweep state, 9 planes float4[np] (layout at k_gradv in pairs.cu) + plane 9 = (dv/dt, s)
     DevBuf u_s;                    // float, specific internal energy in sorted order
     DevBuf vel_orig;               // float4 (vx,vy,vz,u) caller order (packed for a 16-byte gather)
     DevBuf m_s;                    // float, sorted
@@ -145,4 +145,5 @@ int crk_launch_volumes(crk_ctx* c, const float* m, float* V, float* rho, uint32_
 int crk_launch_moments(crk_ctx* c, float* A, float* B, float* gradA, float* gradB);                   // pairs.cu
 int crk_launch_hydro(crk_ctx* c, const float* vx, const float* vy, const float* vz, const float* u,
                      float* ax, float* ay, float* az, float* dudt, uint32_t* pair_count);             // pairs.cu
-int crk_launch_gradv_full(crk_ctx* c, float* gradv);                                                  // pairs.cu
+int crk_launch_gradv_full(crk_ctx* c, float* gradv);
+int crk_launch_compat(crk_ctx* c, float dt, float* delta_u);                                          // pairs.cu                                                  // pairs.cu

@@ -17,6 +17,7 @@ constexpr float C35_3 = 35.0f / 3.0f;
 constexpr float C56_3 = 56.0f / 3.0f;
 constexpr float R2_TINY = 1.0e-37f;
 constexpr int FPL = 9;                             // j-state planes of the force sweep
+constexpr int CPL = FPL + 1;                       // + (dv/dt, s = P / rho^gamma) for the compatible-energy sweep
 
 struct SweepArgs {
     int64_t n, nl;
@@ -582,8 +583,10 @@ __device__ __forceinline__ float visc_mu(float qh, float udx, float r2, float ep
 struct ForceConst {
     float L, half, eta_crit, inv_fold, eps2, Cl, Cq;
 };
-// one ordered pair (i, j): accumulates m_i dv_i/dt (acc[0..2]) and m_i du_i/dt (acc[3])
-__device__ __forceinline__ void force_pair(const ForceConst& k, const PState& I, const PState& J, bool wrapped, float (&acc)[4]) {
+// one ordered pair (i, j): F = m_i a_ij (Eq. 17 with P -> P + Q) and e = its term of m_i du_i/dt (Eq. 18);
+// vji = v_j - v_i
+struct PairF { float Fx, Fy, Fz, e, vjix, vjiy, vjiz; };
+__device__ __forceinline__ PairF force_pair(const ForceConst& k, const PState& I, const PState& J, bool wrapped) {
     float dx, dy, dz;
     if (!wrapped) {
         dx = __fsub_rn(I.x, J.x);
@@ -628,9 +631,12 @@ __device__ __forceinline__ void force_pair(const ForceConst& k, const PState& I,
     const float PQi = __fadd_rn(I.P, Qi), PQj = __fadd_rn(J.P, Qj);
     const float hvv = 0.5f * __fmul_rn(I.V, J.V);
     const float pf = __fmul_rn(hvv, __fadd_rn(PQi, PQj));
-    acc[0] = fmaf(pf, Gx, acc[0]); acc[1] = fmaf(pf, Gy, acc[1]); acc[2] = fmaf(pf, Gz, acc[2]);
     const float vG = fmaf(vz, Gz, fmaf(vy, Gy, vx * Gx));       // (v_i - v_j).G = -(v_j - v_i).G
-    acc[3] = fmaf(-hvv * PQj, vG, acc[3]);
+    PairF o;
+    o.Fx = __fmul_rn(pf, Gx); o.Fy = __fmul_rn(pf, Gy); o.Fz = __fmul_rn(pf, Gz);
+    o.e = -hvv * PQj * vG;
+    o.vjix = -vx; o.vjiy = -vy; o.vjiz = -vz;
+    return o;
 }
 
 // One CTA = one leaf: W5_WPL warps share the tile of the leaf's candidates and split each lane's entries by rows; four
@@ -653,18 +659,64 @@ __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
     for (int p = 0; p < FPL; ++p) planes[p] = a.fst + (int64_t)p * a.np;
     const uint32_t count = leaf_sweep<W5_WPL, FPL, true>(a, planes, leaf, 0, wl, lane, tile, [&](uint32_t sa, bool wrapped, const float4& p0) {
         const PState J = load_pstate_shared(sa, p0);
-        force_pair(fc, I, J, wrapped, acc);
+        const PairF f = force_pair(fc, I, J, wrapped);
+        acc[0] += f.Fx; acc[1] += f.Fy; acc[2] += f.Fz; acc[3] += f.e;
     });
     group_reduce<W5_WPL, 4>(acc, 0, wl, lane, (float*)tile);
-    if (wl == 0 && valid) {
+    if (wl != 0) return;
+    float4 as = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (valid) {
         const float im = 1.0f / a.m_s[i];
         const int32_t p = a.perm[i];
-        a.o0[p] = acc[0] * im;
-        a.o1[p] = acc[1] * im;
-        a.o2[p] = acc[2] * im;
+        as = make_float4(acc[0] * im, acc[1] * im, acc[2] * im, I.P * __powf(I.rho, -a.gamma));
+        a.o0[p] = as.x;
+        a.o1[p] = as.y;
+        a.o2[p] = as.z;
         a.o3[p] = acc[3] * im;
         if (a.ocnt) a.ocnt[p] = count;
     }
+    a.fst[(int64_t)FPL * a.np + i] = as;                 // plane 9: (dv/dt, s = P / rho^gamma) for crk_compatible_energy
+}
+
+// ================================================================================ NEXT row 1: compatible energy update
+// Eqs. 19-23 with a = 1, adot = 0, p = v:  Delta u_i = dt sum_j (f_ij / 2) (v_j + v'_j - v_i - v'_i) . a_ij,
+// v' = v + (dv/dt) dt (Eq. 22), a_ij the pairwise acceleration of Eq. 17 (recomputed: storing it per pair would cost 12 GB).
+// sign(dE_ij) = sign(m_i a_ij . (v_j + v'_j - v_i - v'_i)) (Eq. 21, independent of f); Eq. 23 per DESIGN.md reading G1;
+// f = 1/2 if an entropy is not positive (S16).  Both lanes of a pair form bit-identical F and velocity sums, so they take
+// the same branch of Eq. 23 and f_ij + f_ji = 1 up to the rounding of the reciprocal.
+__global__ void __launch_bounds__(W5_WPL * 32, 4) k_compat(SweepArgs a, float dt) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
+    const int64_t leaf = blockIdx.x;
+    float4* tile = (float4*)smem_raw;
+    const int64_t i = leaf * CRK_LEAF + lane;
+    const bool valid = i < a.n;
+    const PState I = load_pstate(a.fst + i, a.np);
+    const float4 qi = a.fst[(int64_t)FPL * a.np + i];
+    const ForceConst fc = {a.L, a.half, 1.0f / a.n_h, a.n_h / 0.2f, a.eps2, a.C_l, a.C_q};
+    float acc[1] = {0.f};
+    const float4* planes[CPL];
+#pragma unroll
+    for (int p = 0; p < CPL; ++p) planes[p] = a.fst + (int64_t)p * a.np;
+    leaf_sweep<W5_WPL, CPL, true>(a, planes, leaf, 0, wl, lane, tile, [&](uint32_t sa, bool wrapped, const float4& p0) {
+        const PState J = load_pstate_shared(sa, p0);
+        const float4 qj = lds128(sa + (uint32_t)FPL * CRK_CCAP * 16u);
+        const PairF f = force_pair(fc, I, J, wrapped);
+        // (v_j + v'_j - v_i - v'_i) = 2 (v_j - v_i) + (a_j - a_i) dt
+        const float wx = __fmaf_rn(dt, __fsub_rn(qj.x, qi.x), __fmul_rn(2.0f, f.vjix));
+        const float wy = __fmaf_rn(dt, __fsub_rn(qj.y, qi.y), __fmul_rn(2.0f, f.vjiy));
+        const float wz = __fmaf_rn(dt, __fsub_rn(qj.z, qi.z), __fmul_rn(2.0f, f.vjiz));
+        const float w = __fmaf_rn(f.Fz, wz, __fmaf_rn(f.Fy, wy, __fmul_rn(f.Fx, wx)));       // = 2 dE_ij
+        const float si = qi.w, sj = qj.w;
+        float part = 0.5f;
+        if (si > 0.0f && sj > 0.0f) {
+            const bool small = (w >= 0.0f) ? (si >= sj) : (si < sj);
+            part = (small ? fminf(si, sj) : fmaxf(si, sj)) * rcp_fast(__fadd_rn(si, sj));
+        }
+        acc[0] = fmaf(0.5f * part, w, acc[0]);
+    });
+    group_reduce<W5_WPL, 1>(acc, 0, wl, lane, (float*)tile);
+    if (wl == 0 && valid) a.o0[a.perm[i]] = acc[0] * dt / a.m_s[i];
 }
 
 __global__ void __launch_bounds__(256) k_gather_f32(const float* __restrict__ in, const int32_t* __restrict__ perm,
@@ -727,7 +779,7 @@ int crk_launch_hydro(crk_ctx* c, const float* vx, const float* vy, const float* 
     const int64_t np = c->nl * CRK_LEAF;
     CRK_TRY(crk_ensure(c, c->vel_orig, (size_t)c->n * sizeof(float4)));
     CRK_TRY(crk_ensure(c, c->u_s, (size_t)np * sizeof(float)));
-    CRK_TRY(crk_ensure(c, c->fst, (size_t)np * FPL * sizeof(float4)));
+    CRK_TRY(crk_ensure(c, c->fst, (size_t)np * CPL * sizeof(float4)));
     k_pack_vel<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>(vx, vy, vz, u, c->n, (float4*)c->vel_orig.p);
     CRK_TRY(crk_check_launch(c, "k_pack_vel"));
     SweepArgs a = make_args(c);
@@ -762,4 +814,14 @@ int crk_launch_gradv_full(crk_ctx* c, float* gradv) {
     CRK_TRY(set_smem(c, k_gradv, smem));
     k_gradv<<<(unsigned)((c->nl + W4_LPC - 1) / W4_LPC), W4_WPL * W4_LPC * 32, smem, c->stream>>>(a, (const float*)c->u_s.p, gradv);
     return crk_check_launch(c, "k_gradv");
+}
+
+// NEXT row 1: Eqs. 19-23 on the state left by crk_hydro_derivs
+int crk_launch_compat(crk_ctx* c, float dt, float* delta_u) {
+    SweepArgs a = make_args(c);
+    a.o0 = delta_u;
+    const int smem = CPL * CRK_CCAP * (int)sizeof(float4);
+    CRK_TRY(set_smem(c, k_compat, smem));
+    k_compat<<<(unsigned)c->nl, W5_WPL * 32, smem, c->stream>>>(a, dt);
+    return crk_check_launch(c, "k_compat");
 }

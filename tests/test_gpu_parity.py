@@ -284,6 +284,19 @@ def test_parity_config4_cosmo_full(oracle_mod):
     g = _window_check(ps, oracle_mod, centres, half_in_h=3.0, label="cosmo256")
     st = g["stats"]
     print(f"[stats] cosmo256 leaves={st['n_leaves']} leaf_pairs={st['n_leaf_pairs']} launches={st['launches']}")
+    # NEXT row 1 at the full size: the exactness property of PAPER.md:141 holds at any size
+    torch = _torch()
+    dt = 1e-2
+    du = g["ctx"].compatible_energy(dt)
+    torch.cuda.synchronize()
+    du = du.cpu().numpy().astype(np.float64)
+    m = ps.m.astype(np.float64)
+    v = np.stack([ps.vx, ps.vy, ps.vz]).astype(np.float64)
+    a = np.stack([g["ax"], g["ay"], g["az"]]).astype(np.float64)
+    dke = 0.5 * (m * (((v + a * dt) ** 2).sum(0) - (v ** 2).sum(0))).sum()
+    res = abs(dke + (m * du).sum()) / (m * np.abs(du)).sum()
+    assert res < TOL_INV, f"cosmo256 compatible energy residual {res:.3e}"
+    print(f"[parity] cosmo256 compatible energy residual {res:.2e}")
 
 
 def test_parity_config5_cosmo_large_full(oracle_mod):
@@ -341,3 +354,41 @@ def test_parity_config5_cosmo_large_full(oracle_mod):
               f"momentum {mom:.2e} energy {en:.2e}")
         done += 1
     assert done >= 1
+
+
+# ------------------------------------------------------------------------------- NEXT row 1: compatible energy update
+@pytest.mark.parametrize("name,n_side,dt", [("tiny_uniform", 16, 1e-3), ("blast_wave", 24, 1e-5), ("clustered", 24, 1e-3),
+                                            ("cosmo", 32, 1e-2)])
+def test_compatible_energy_parity(name, n_side, dt, oracle_mod):
+    """Eqs. 19-23: GPU sweep vs the FP64 oracle, and the exactness property of PAPER.md:141
+    (thermal gain = kinetic loss of v -> v + a dt) on the GPU's own accelerations."""
+    torch = _torch()
+    ps = wl.make_config(name, n_side)
+    o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+    o.step_derivs(ps)
+    du_o = o.compatible_energy(dt)
+    g = gpu_eval(ps)
+    du_g = g["ctx"].compatible_energy(dt)
+    torch.cuda.synchronize()
+    du_g = du_g.cpu().numpy().astype(np.float64)
+    e = rel_l2(du_g, du_o)
+    assert e < TOL_DERIV, f"{name} compatible Delta u rel L2 {e:.3e}"
+    m = ps.m.astype(np.float64)
+    v = np.stack([ps.vx, ps.vy, ps.vz]).astype(np.float64)
+    a = np.stack([g["ax"], g["ay"], g["az"]]).astype(np.float64)
+    dke = 0.5 * (m * (((v + a * dt) ** 2).sum(0) - (v ** 2).sum(0))).sum()
+    res = abs(dke + (m * du_g).sum()) / ((m * np.abs(du_g)).sum() + 1e-300)
+    assert res < TOL_INV, f"{name} compatible energy residual {res:.3e}"
+    print(f"[parity] {name} n={ps.n} dt={dt}: compatible Delta u {e:.2e}, energy residual {res:.2e}")
+
+
+def test_compatible_energy_needs_hydro_first():
+    torch = _torch()
+    from paper_2202_02840_b200 import Crk, CrkError
+    ps = wl.tiny_uniform(n_side=8)
+    dev = torch.device("cuda:0")
+    t = [torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).to(dev) for k in ("x", "y", "z", "h")]
+    ctx = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h)
+    ctx.build_cells(*t)
+    with pytest.raises(CrkError):
+        ctx.compatible_energy(1e-3)
