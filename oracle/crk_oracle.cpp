@@ -439,6 +439,25 @@ int crk_oracle_hydro_derivs(crk_oracle_ctx* c, const float* vx, const float* vy,
     return 0;
 }
 
+// ---- NEXT row 3: evolved smoothing length, Eqs. 51-53 ---------------------------------------------
+// Eq. 51: N_i = (4/3) pi h_i^3 n_i with n_i the SPH number density of Eq. 14.  Target N_res = (4/3) pi n_h^3 (PAPER.md:336,
+// reading S1: h is the support radius).  Delta_N = (N_res / N_i)^(1/3).  Eq. 53: lambda = 0.2 (1 + Delta_N^2) if Delta_N < 1,
+// 0.2 (1 + 1/Delta_N^3) otherwise.  Eq. 52: h~ = h (1 - lambda + lambda Delta_N).
+double crk_oracle_h_update(double h, double n_i, double n_h) {
+    const double four_thirds_pi = 4.0 / 3.0 * 3.14159265358979323846;
+    const double N_i = four_thirds_pi * h * h * h * n_i;
+    const double N_res = four_thirds_pi * n_h * n_h * n_h;
+    const double dN = std::cbrt(N_res / N_i);
+    const double lambda = dN < 1.0 ? 0.2 * (1.0 + dN * dN) : 0.2 * (1.0 + 1.0 / (dN * dN * dN));
+    return h * (1.0 - lambda + lambda * dN);
+}
+
+int crk_oracle_evolve_h(crk_oracle_ctx* c, double* h_new) {
+    if (!c || c->stage < 2 || !h_new) return -1;
+    for (int64_t i = 0; i < c->n; ++i) h_new[i] = crk_oracle_h_update((double)c->h[i], 1.0 / c->V[i], c->p.n_h);
+    return 0;
+}
+
 // ---- NEXT row 1: compatible energy update, Eqs. 19-23, a = 1, adot = 0, p = v ----------------------
 // Eq. 22: v'_i = v_i + (dv_i/dt) dt.   Eq. 20: du_ij = (f_ij / 2) (v_j + v'_j - v_i - v'_i) . a_ij with a_ij the pairwise
 // acceleration of Eq. 17 (P -> P + Q).   Eq. 21: dE_ij = m_i du_ij + m_j du_ji; because m_i a_ij = -m_j a_ji

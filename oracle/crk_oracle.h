@@ -61,6 +61,12 @@ int crk_oracle_compatible_energy(crk_oracle_ctx* c, double dt, double* delta_u);
 /* one pair of the above: out = { du_ij (Eq. 20), dE_ij (Eq. 21), f_ij (Eq. 23) }                                 */
 int crk_oracle_pair_compat(crk_oracle_ctx* c, int64_t i, int64_t j, double dt, double out[3]);
 
+/* NEXT row 3 -- evolved smoothing length, Eqs. 51-53, after crk_oracle_volumes:
+ * h_new[i] = h_i (1 - lambda + lambda Delta_N), Delta_N^3 = N_res / N_i, N_i = (4/3) pi h_i^3 / V_i, N_res = (4/3) pi n_h^3.
+ * Pinned: hand-evaluated values of Eqs. 52-53 at Delta_N = 1/2, 1, 2; continuity of lambda at 1; iteration -> N_res.    */
+int    crk_oracle_evolve_h(crk_oracle_ctx* c, double* h_new);
+double crk_oracle_h_update(double h, double n_i, double n_h);   /* the per-particle rule on its own */
+
 /* ---- diagnostics used by the pins (tests only) ---- */
 double crk_oracle_W(double r, double h);        /* Eq. 12                                   */
 double crk_oracle_dWdr(double r, double h);     /* its radial derivative                    */

@@ -50,6 +50,9 @@ def lib():
         L.crk_oracle_pair_term.argtypes = [C.c_void_p, C.c_int64, C.c_int64, dp]
         L.crk_oracle_pair_visc.argtypes = [C.c_void_p, C.c_int64, C.c_int64, dp]
         L.crk_oracle_compatible_energy.argtypes = [C.c_void_p, C.c_double, dp]
+        L.crk_oracle_evolve_h.argtypes = [C.c_void_p, dp]
+        L.crk_oracle_h_update.argtypes = [C.c_double, C.c_double, C.c_double]
+        L.crk_oracle_h_update.restype = C.c_double
         L.crk_oracle_pair_compat.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_double, dp]
         L.crk_oracle_neighbors.restype = C.c_int64
         L.crk_oracle_neighbors.argtypes = [C.c_void_p, C.c_int64, up, C.c_int64]
@@ -140,6 +143,12 @@ class Oracle:
         return dict(V=V, rho=rho, nbr_count=nbr, A=A, B=B, gradA=gA, gradB=gB,
                     ax=ax, ay=ay, az=az, dudt=du, pair_count=pc)
 
+    def evolve_h(self):
+        """Eqs. 51-53 after volumes(): the adjusted support radii"""
+        h = np.empty(self.n)
+        assert lib().crk_oracle_evolve_h(self._c, _d(h)) == 0
+        return h
+
     def compatible_energy(self, dt):
         """Eqs. 19-23: Delta u over dt from the pairwise accelerations of the last hydro_derivs"""
         du = np.empty(self.n)
@@ -218,3 +227,8 @@ def euler_steps(ps, n_steps: int, dt: float, oracle: Oracle | None = None):
             st[k] = p - np.floor(p / L) * L          # re-wrap with floor (reading S12)
             st[v] = st[v] + d[a] * dt
         st["u"] = st["u"] + d["dudt"] * dt
+
+
+def h_update(h, n_i, n_h):
+    """Eqs. 51-53 for one particle (number density n_i)"""
+    return lib().crk_oracle_h_update(float(h), float(n_i), float(n_h))

@@ -419,3 +419,37 @@ def test_compatible_energy_small_dt_limit_and_uniform_entropy(oracle_mod):
             ref += 0.5 * np.dot(v[:, j] - v[:, i], F / m[i])
         assert abs(du[i] - ref) <= 1e-6 * abs(ref) + 1e-12
     assert abs((m * du).sum() - (m * d["dudt"]).sum()) <= 1e-7 * (m * np.abs(d["dudt"])).sum()
+
+
+# ---------------------------------------------------------------------------------------- NEXT row 3: Eqs. 51-53
+def test_evolved_h_rule_hand_values_and_continuity(oracle_mod):
+    """Eqs. 52-53 evaluated by hand: Delta_N = 1/2 -> lambda = 0.2 (1 + 1/4) = 0.25, h~/h = 1 - 0.25 + 0.125 = 0.875;
+    Delta_N = 1 -> h~ = h; Delta_N = 2 -> lambda = 0.2 (1 + 1/8) = 0.225, h~/h = 1 - 0.225 + 0.45 = 1.225.  N_res =
+    (4/3) pi n_h^3 = 268.08 at n_h = 4."""
+    n_h, h = 4.0, 0.37
+    N_res = 4.0 / 3.0 * math.pi * n_h ** 3
+    assert abs(N_res - 268.08) < 0.01
+    for dN, ratio in ((0.5, 0.875), (1.0, 1.0), (2.0, 1.225)):
+        n_i = (N_res / dN ** 3) / (4.0 / 3.0 * math.pi * h ** 3)       # Eq. 51 solved for the density that gives Delta_N
+        assert abs(oracle_mod.h_update(h, n_i, n_h) / h - ratio) < 1e-13
+    # lambda is continuous at Delta_N = 1 (0.4 from both branches), so h~ is continuous there
+    n1 = N_res / (4.0 / 3.0 * math.pi * h ** 3)
+    lo, hi = oracle_mod.h_update(h, n1 * (1 + 1e-9), n_h), oracle_mod.h_update(h, n1 * (1 - 1e-9), n_h)
+    assert abs(lo - h) < 1e-9 and abs(hi - h) < 1e-9 and lo < h < hi   # too many neighbours shrink h, too few grow it
+
+
+def test_evolved_h_iteration_reaches_target_neighbour_number(oracle_mod):
+    """evolving h with Eq. 52 drives N_i = (4/3) pi h^3 n_i (Eq. 51) to N_res"""
+    ps = wl.tiny_uniform(n_side=10)
+    N_res = 4.0 / 3.0 * math.pi * ps.n_h ** 3
+    h = (ps.h * np.where(np.arange(ps.n) % 2 == 0, 1.3, 0.75)).astype(np.float32)    # start 30 % / 25 % off
+    o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+    err = []
+    for _ in range(26):
+        o.build(ps.x, ps.y, ps.z, h)
+        V, _, _ = o.volumes(ps.m)
+        N = 4.0 / 3.0 * math.pi * h.astype(np.float64) ** 3 / V
+        err.append(np.abs(N / N_res - 1).max())
+        h = o.evolve_h().astype(np.float32)
+    # a contraction (lambda <= 0.4 damps the correction): the error shrinks every step and ends far below the start
+    assert err[0] > 0.5 and err[-1] < 1e-3 and all(b < 0.8 * a for a, b in zip(err[:15], err[1:16])), err
