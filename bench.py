@@ -227,6 +227,15 @@ def run_ours(args, rank, world, local_rank):
     c1.record()
     torch.cuda.synchronize()
     compat_ms = c0.elapsed_time(c1) / 3
+    # NEXT row 3 (evolved h, Eqs. 51-53): a 40 B/particle stream pass (posh 16 + posV 16 + perm 4 read, h 4 written)
+    ctx.evolve_h(out=du)
+    torch.cuda.synchronize()
+    c0.record()
+    for _ in range(5):
+        ctx.evolve_h(out=du)
+    c1.record()
+    torch.cuda.synchronize()
+    evolve_ms = c0.elapsed_time(c1) / 5
     del du
 
     # end to end through the host-pointer C ABI entry (pinned host inputs -> device -> compute -> host outputs)
@@ -282,7 +291,8 @@ def run_ours(args, rank, world, local_rank):
         "e2e": {"value": pairs_all / (e2e_all * 1e-3), "unit": UNIT, "ms_per_step": e2e_all,
                 "h2d_bytes_per_step": int(9 * 4 * n_all), "d2h_bytes_per_step": int(4 * 4 * n_all)},
         "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
-        "next_rows": {"compatible_energy_ms": compat_ms,
+        "next_rows": {"evolve_h_ms": evolve_ms, "evolve_h_gbs": 40.0 * ps.n / (evolve_ms * 1e-3) / 1e9,
+                      "compatible_energy_ms": compat_ms,
                       "compatible_energy_fp32_frac": (FLOPS_PER_PAIR["forces"] + 20.0) * sym_pairs / (compat_ms * 1e-3) / FP32_PEAK_THEORETICAL},
     }
     if world == 1 and not args.no_cpu_baseline:

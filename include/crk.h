@@ -104,6 +104,12 @@ int  crk_step_derivs_host(crk_ctx* c, int64_t n, const float* x, const float* y,
  * delta_u: device float[n], caller order, written.  One more symmetric pair sweep on the resident state.          */
 int  crk_compatible_energy(crk_ctx* c, float dt, float* delta_u);
 
+/* ---- NEXT row 3: evolved smoothing length, Eqs. 51-53, PAPER.md:340-354 -----------------------------------------
+ * After crk_volumes (else CRK_ESTATE): h_new[i] = h_i (1 - lambda + lambda Delta_N) with Delta_N^3 = N_res / N_i,
+ * N_i = (4/3) pi h_i^3 / V_i (Eq. 51), N_res = (4/3) pi n_h^3, lambda of Eq. 53.  h_new: device float[n], caller order,
+ * written (may alias nothing the library reads later: the build keeps its own copy of h).  One 40 B/particle stream pass. */
+int  crk_evolve_h(crk_ctx* c, float* h_new);
+
 /* ---- diagnostics ---- */
 const char* crk_last_error(const crk_ctx* c);
 int  crk_get_perm(crk_ctx* c, int32_t* perm);        /* device int32[n]: perm[k] = caller index of sorted slot k   */

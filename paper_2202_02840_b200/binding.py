@@ -11,7 +11,7 @@ _LIB_PATH = os.path.join(_HERE, "libcrk.so")
 
 EXPORTED_SYMBOLS = (
     "crk_create", "crk_destroy", "crk_build_cells", "crk_volumes", "crk_rk_coefficients", "crk_hydro_derivs",
-    "crk_step_derivs", "crk_step_derivs_host", "crk_compatible_energy", "crk_last_error", "crk_get_perm", "crk_get_gradv", "crk_get_leaf_segments", "crk_get_stats",
+    "crk_step_derivs", "crk_step_derivs_host", "crk_compatible_energy", "crk_evolve_h", "crk_last_error", "crk_get_perm", "crk_get_gradv", "crk_get_leaf_segments", "crk_get_stats",
     "crk_reset_stats", "crk_set_timing", "crk_get_leaf_list", "crk_measure_fp32_peak",
 )
 
@@ -73,6 +73,7 @@ def _load():
     L.crk_get_perm.argtypes = [vp, vp]
     L.crk_get_gradv.argtypes = [vp, vp]
     L.crk_compatible_energy.argtypes = [vp, C.c_float, vp]
+    L.crk_evolve_h.argtypes = [vp, vp]
     L.crk_get_leaf_segments.argtypes = [vp, vp]
     L.crk_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.crk_reset_stats.argtypes = [vp]
@@ -181,6 +182,12 @@ class Crk:
         self._chk(self._L.crk_step_derivs_host(self._h, n, *[C.c_void_p(t.data_ptr()) for t in (x, y, z, h, vx, vy, vz, m, u)],
                                                *[C.c_void_p(t.data_ptr()) for t in out]))
         return out
+
+    def evolve_h(self, out=None):
+        """Eqs. 51-53 after volumes(): adjusted support radii, caller order"""
+        h = out if out is not None else torch.empty(self.n, device=self._dev)
+        self._chk(self._L.crk_evolve_h(self._h, _dev(h)))
+        return h
 
     def compatible_energy(self, dt: float, out=None):
         """Eqs. 19-23 after hydro_derivs: Delta u over dt, caller order"""

@@ -184,6 +184,16 @@ int crk_get_perm(crk_ctx* c, int32_t* perm) {
     return CRK_OK;
 }
 
+int crk_evolve_h(crk_ctx* c, float* h_new) {
+    if (!c || !h_new) return CRK_EINVAL;
+    if (c->stage < 2) {
+        snprintf(c->err, sizeof(c->err), "crk_evolve_h needs crk_volumes first");
+        return CRK_ESTATE;
+    }
+    if (c->n == 0) return CRK_OK;
+    return crk_launch_evolve_h(c, h_new);
+}
+
 int crk_compatible_energy(crk_ctx* c, float dt, float* delta_u) {
     if (!c || !delta_u || !(dt == dt)) return CRK_EINVAL;
     if (c->stage < 4) {

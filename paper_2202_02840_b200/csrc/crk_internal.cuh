@@ -146,4 +146,5 @@ int crk_launch_moments(crk_ctx* c, float* A, float* B, float* gradA, float* grad
 int crk_launch_hydro(crk_ctx* c, const float* vx, const float* vy, const float* vz, const float* u,
                      float* ax, float* ay, float* az, float* dudt, uint32_t* pair_count);             // pairs.cu
 int crk_launch_gradv_full(crk_ctx* c, float* gradv);
+int crk_launch_evolve_h(crk_ctx* c, float* h_new);                                                    // pairs.cu
 int crk_launch_compat(crk_ctx* c, float dt, float* delta_u);                                          // pairs.cu                                                  // pairs.cu

@@ -825,3 +825,25 @@ int crk_launch_compat(crk_ctx* c, float dt, float* delta_u) {
     k_compat<<<(unsigned)c->nl, W5_WPL * 32, smem, c->stream>>>(a, dt);
     return crk_check_launch(c, "k_compat");
 }
+
+// NEXT row 3: evolved smoothing length, Eqs. 51-53, a stream pass over (h, V) of the last crk_volumes:
+// N_i = (4/3) pi h^3 / V (Eq. 51), N_res = (4/3) pi n_h^3, Delta_N = (N_res/N_i)^(1/3) = n_h V^(1/3) / h,
+// lambda = 0.2 (1 + Delta_N^2) if Delta_N < 1 else 0.2 (1 + 1/Delta_N^3) (Eq. 53), h~ = h (1 - lambda + lambda Delta_N) (Eq. 52)
+namespace {
+__global__ void __launch_bounds__(256) k_evolve_h(const float4* __restrict__ posh, const float4* __restrict__ posV,
+                                                  const int32_t* __restrict__ perm, int64_t n, float n_h,
+                                                  float* __restrict__ h_new) {
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const float h = posh[k].w, V = posV[k].w;
+    const float dN = n_h * cbrtf(V) / h;
+    const float lambda = dN < 1.0f ? 0.2f * (1.0f + dN * dN) : 0.2f * (1.0f + 1.0f / (dN * dN * dN));
+    h_new[perm[k]] = h * (1.0f - lambda + lambda * dN);
+}
+}  // namespace
+
+int crk_launch_evolve_h(crk_ctx* c, float* h_new) {
+    k_evolve_h<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>((const float4*)c->posh.p, (const float4*)c->posV.p,
+                                                                      c->perm, c->n, c->prm.n_h, h_new);
+    return crk_check_launch(c, "k_evolve_h");
+}

@@ -392,3 +392,29 @@ def test_compatible_energy_needs_hydro_first():
     ctx.build_cells(*t)
     with pytest.raises(CrkError):
         ctx.compatible_energy(1e-3)
+
+
+# ------------------------------------------------------------------------------- NEXT row 3: evolved smoothing length
+@pytest.mark.parametrize("name,n_side", [("tiny_uniform", 16), ("clustered", 24), ("cosmo", 32)])
+def test_evolved_h_parity(name, n_side, oracle_mod):
+    """Eqs. 51-53: the stream pass vs the FP64 oracle; h perturbed so that Delta_N covers both branches"""
+    torch = _torch()
+    from paper_2202_02840_b200 import Crk
+    ps = wl.make_config(name, n_side)
+    ps.h[:] = (ps.h * np.where(np.arange(ps.n) % 3 == 0, 1.25, np.where(np.arange(ps.n) % 3 == 1, 0.8, 1.0))).astype(np.float32)
+    o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+    o.build(ps.x, ps.y, ps.z, ps.h)
+    o.volumes(ps.m)
+    h_o = o.evolve_h()
+    dev = torch.device("cuda:0")
+    t = {k: torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).to(dev) for k in ("x", "y", "z", "h", "m")}
+    ctx = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h)
+    ctx.build_cells(t["x"], t["y"], t["z"], t["h"])
+    ctx.volumes(t["m"])
+    h_g = ctx.evolve_h()
+    torch.cuda.synchronize()
+    h_g = h_g.cpu().numpy().astype(np.float64)
+    e = np.max(np.abs(h_g / h_o - 1))
+    assert e < TOL_SCALAR, f"{name} evolved h max rel err {e:.3e}"
+    assert (h_o > ps.h).any() and (h_o < ps.h).any()
+    print(f"[parity] {name} n={ps.n}: evolved h max rel err {e:.2e}")
