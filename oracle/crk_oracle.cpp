@@ -10,6 +10,7 @@
 
 #include <algorithm>
 #include <cmath>
+#include <limits>
 #include <cstring>
 #include <vector>
 #include <omp.h>
@@ -436,6 +437,47 @@ int crk_oracle_hydro_derivs(crk_oracle_ctx* c, const float* vx, const float* vy,
         if (pair_count) pair_count[i] = cnt;
     }
     c->stage = 4;
+    return 0;
+}
+
+// ---- NEXT row 2a: time-step criteria, Eqs. 46-50, a = 1, adot = 0, dy/dt = 1, no gravity ----------
+// Eq. 50 (sign garbled as printed; reading S17: the approach speed): v_sig,ij = max(-(v_ij . x_ij) / |x_ij|, 0),
+//   v_sig,i = max_j v_sig,ij over the pairs of the momentum sweep (r < max(h_i, h_j)).
+// Eq. 46: v_max,i = max(v_sig,i, c_s,i, c_sq,i, hhat_i |Tr grad v_i|), c_sq = sqrt(zeta Q_i / rho_i), zeta = 4, with
+//   Q_i the largest viscous pressure of particle i over its pairs (reading S18: "maximum viscous sound speed").
+// Eq. 47: dt_hyd = C_CFL hhat_i / v_max,i.   Eq. 48 (r_soft = infinity without gravity): dt_acc = sqrt(hhat_i / |dv_i/dt|).
+// Eq. 49: dt_min = min(dt_hyd, dt_acc).
+int crk_oracle_timestep(crk_oracle_ctx* c, double C_cfl, double* dt_min, double* dt_hyd_out, double* dt_acc_out) {
+    if (!c || c->stage < 4 || !dt_min) return -1;
+    set_threads();
+    const int64_t n = c->n;
+    const double inf = std::numeric_limits<double>::infinity();
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < n; ++i) {
+        double vsig = 0.0, Qmax = 0.0;
+        for (int64_t k = c->off[i]; k < c->off[i + 1]; ++k) {
+            const int64_t j = c->nbr[k] & IDX_MASK;
+            double x[3];
+            sep(c, i, j, x);
+            const double r = std::sqrt(x[0] * x[0] + x[1] * x[1] + x[2] * x[2]);
+            const double vx = (c->vx[i] - c->vx[j]) * x[0] + (c->vy[i] - c->vy[j]) * x[1] + (c->vz[i] - c->vz[j]) * x[2];
+            if (r > 0.0) vsig = std::max(vsig, std::max(-vx / r, 0.0));                     // Eq. 50
+            PairOut o;
+            pair_term(c, i, j, o);
+            Qmax = std::max(Qmax, o.Qi);
+        }
+        const double hhat = (double)c->h[i] / c->p.n_h;
+        const double* gv = &c->gradv[9 * i];
+        const double div = std::fabs(gv[0] + gv[4] + gv[8]);
+        const double csq = std::sqrt(4.0 * Qmax / c->rho[i]);
+        const double vmax = std::max(std::max(vsig, c->cs[i]), std::max(csq, hhat * div));  // Eq. 46
+        const double th = vmax > 0.0 ? C_cfl * hhat / vmax : inf;                           // Eq. 47
+        const double amag = std::sqrt(c->ax[i] * c->ax[i] + c->ay[i] * c->ay[i] + c->az[i] * c->az[i]);
+        const double ta = amag > 0.0 ? std::sqrt(hhat / amag) : inf;                        // Eq. 48
+        dt_min[i] = std::min(th, ta);                                                       // Eq. 49
+        if (dt_hyd_out) dt_hyd_out[i] = th;
+        if (dt_acc_out) dt_acc_out[i] = ta;
+    }
     return 0;
 }
 

@@ -61,6 +61,13 @@ int crk_oracle_compatible_energy(crk_oracle_ctx* c, double dt, double* delta_u);
 /* one pair of the above: out = { du_ij (Eq. 20), dE_ij (Eq. 21), f_ij (Eq. 23) }                                 */
 int crk_oracle_pair_compat(crk_oracle_ctx* c, int64_t i, int64_t j, double dt, double out[3]);
 
+/* NEXT row 2a -- time-step criteria, Eqs. 46-50 with a = 1, adot = 0, no gravity, after
+ * crk_oracle_hydro_derivs: dt_min = min(C_cfl hhat / max(v_sig, c_s, sqrt(4 Q_max / rho), hhat |Tr grad v|), sqrt(hhat / |a|)).
+ * dt_hyd / dt_acc (nullable) return the two criteria separately.  Pinned: static gas closed form C hhat / c_s, linear
+ * compression closed form, acceleration criterion from the Eq. 17 pair diagnostic.  PARITY UNPINNED: the sign reading
+ * of the garbled Eq. 50 (S17) and "Q_i" = the maximum over pairs (S18).                                              */
+int crk_oracle_timestep(crk_oracle_ctx* c, double C_cfl, double* dt_min, double* dt_hyd, double* dt_acc);
+
 /* NEXT row 3 -- evolved smoothing length, Eqs. 51-53, after crk_oracle_volumes:
  * h_new[i] = h_i (1 - lambda + lambda Delta_N), Delta_N^3 = N_res / N_i, N_i = (4/3) pi h_i^3 / V_i, N_res = (4/3) pi n_h^3.
  * Pinned: hand-evaluated values of Eqs. 52-53 at Delta_N = 1/2, 1, 2; continuity of lambda at 1; iteration -> N_res.    */

@@ -51,6 +51,7 @@ def lib():
         L.crk_oracle_pair_visc.argtypes = [C.c_void_p, C.c_int64, C.c_int64, dp]
         L.crk_oracle_compatible_energy.argtypes = [C.c_void_p, C.c_double, dp]
         L.crk_oracle_evolve_h.argtypes = [C.c_void_p, dp]
+        L.crk_oracle_timestep.argtypes = [C.c_void_p, C.c_double, dp, dp, dp]
         L.crk_oracle_h_update.argtypes = [C.c_double, C.c_double, C.c_double]
         L.crk_oracle_h_update.restype = C.c_double
         L.crk_oracle_pair_compat.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_double, dp]
@@ -142,6 +143,12 @@ class Oracle:
         ax, ay, az, du, pc = self.hydro_derivs(ps.vx, ps.vy, ps.vz, ps.u)
         return dict(V=V, rho=rho, nbr_count=nbr, A=A, B=B, gradA=gA, gradB=gB,
                     ax=ax, ay=ay, az=az, dudt=du, pair_count=pc)
+
+    def timestep(self, C_cfl=0.25):
+        """Eqs. 46-50 after hydro_derivs: (dt_min, dt_hyd, dt_acc) per particle"""
+        a, b, c = np.empty(self.n), np.empty(self.n), np.empty(self.n)
+        assert lib().crk_oracle_timestep(self._c, float(C_cfl), _d(a), _d(b), _d(c)) == 0
+        return a, b, c
 
     def evolve_h(self):
         """Eqs. 51-53 after volumes(): the adjusted support radii"""

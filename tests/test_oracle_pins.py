@@ -453,3 +453,60 @@ def test_evolved_h_iteration_reaches_target_neighbour_number(oracle_mod):
         h = o.evolve_h().astype(np.float32)
     # a contraction (lambda <= 0.4 damps the correction): the error shrinks every step and ends far below the start
     assert err[0] > 0.5 and err[-1] < 1e-3 and all(b < 0.8 * a for a, b in zip(err[:15], err[1:16])), err
+
+
+# ---------------------------------------------------------------------------------------- NEXT row 2a: Eqs. 46-50
+def test_timestep_static_gas_is_the_sound_crossing_limit(oracle_mod):
+    """v = 0 on a perfect lattice with uniform u: v_sig = 0, Q = 0, Tr grad v = 0, a = 0 by symmetry (pin P8), so Eq. 46
+    leaves c_s and Eqs. 47-49 give dt = C_CFL hhat / c_s with c_s = sqrt(gamma (gamma - 1) u)."""
+    ns = 8
+    g = (np.arange(ns) + 0.5) / ns
+    X = np.stack(np.meshgrid(g, g, g, indexing="ij")).reshape(3, -1).astype(np.float32)
+    n = ns ** 3
+    ps = wl.ParticleSet(x=X[0].copy(), y=X[1].copy(), z=X[2].copy(), h=np.full(n, 2.4 / ns, np.float32),
+                        vx=np.zeros(n, np.float32), vy=np.zeros(n, np.float32), vz=np.zeros(n, np.float32),
+                        m=np.full(n, 1.0 / n, np.float32), u=np.full(n, 1.7, np.float32), box=1.0, gamma=5.0 / 3.0, n_h=2.4,
+                        name="lattice", seed=0, meta={})
+    o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+    o.step_derivs(ps)
+    dt, dth, dta = o.timestep(0.25)
+    cs = math.sqrt(ps.gamma * (ps.gamma - 1.0) * float(np.float32(1.7)))
+    expect = 0.25 * (float(np.float32(2.4 / ns)) / 2.4) / cs
+    assert np.allclose(dth, expect, rtol=1e-12)
+    assert np.all(dta > 1e3 * expect)                 # residual accelerations are roundoff
+    assert np.allclose(dt, expect, rtol=1e-12)
+
+
+def test_timestep_linear_compression_closed_form(oracle_mod):
+    """v = -k x (cold gas): viscosity is off for linear flows, Tr grad v = -3k exactly (pin P6), and the
+    approach speed of a pair is k |x_ij| (Eq. 50), so v_max = k max(r_max,i, 3 hhat_i) with r_max,i the largest pair
+    separation of particle i, found here by an independent numpy search."""
+    ps = wl.tiny_uniform(seed=5)
+    k = 0.8
+    X = np.stack([ps.x, ps.y, ps.z]).astype(np.float64)
+    for a, nm in enumerate(("vx", "vy", "vz")):
+        setattr(ps, nm, (-k * (X[a] - 0.5)).astype(np.float32))
+    ps.u[:] = 1e-12                                      # c_s ~ 1e-6: never the maximum
+    o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+    o.step_derivs(ps)
+    dt, dth, dta = o.timestep(0.25)
+    inner = np.nonzero(np.all((X > 0.35) & (X < 0.65), axis=0))[0]
+    h = ps.h.astype(np.float64)
+    for i in inner[:25]:
+        d = X - X[:, [i]]
+        r = np.sqrt((d ** 2).sum(0))
+        sel = (r < np.maximum(h[i], h)) & (r > 0)        # symmetric pair set, no box face within reach
+        hhat = h[i] / ps.n_h
+        vmax = k * max(r[sel].max(), 3.0 * hhat)
+        assert dth[i] == pytest.approx(0.25 * hhat / vmax, rel=2e-5)     # float32 velocities
+
+
+def test_timestep_acceleration_criterion_from_pair_terms(tiny):
+    """Eq. 48 without gravity: dt_acc^2 |dv/dt| = hhat, with dv/dt rebuilt from the Eq. 17 pair diagnostic"""
+    ps, o, d = tiny
+    dt, dth, dta = o.timestep(0.25)
+    assert np.all(dt == np.minimum(dth, dta))
+    for i in (3, 1000, 4000):
+        js, _, _ = o.neighbors(i)
+        F = sum(o.pair_term(i, j)[:3] for j in js) / float(ps.m[i])
+        assert dta[i] ** 2 * np.linalg.norm(F) == pytest.approx(float(ps.h[i]) / ps.n_h, rel=1e-10)
