@@ -236,7 +236,27 @@ def run_ours(args, rank, world, local_rank):
     c1.record()
     torch.cuda.synchronize()
     evolve_ms = c0.elapsed_time(c1) / 5
-    del du
+    # NEXT row 2a (time-step criteria, Eqs. 46-50): the momentum sweep with the two extra maxima, and the stream pass
+    ctx_ts = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h, timestep=True)
+    ctx_ts.set_timing(True)
+    for _ in range(2):
+        ctx_ts.step_derivs(*t, out=out)
+    torch.cuda.synchronize()
+    ctx_ts.reset_stats()
+    for _ in range(3):
+        ctx_ts.step_derivs(*t, out=out)
+    torch.cuda.synchronize()
+    forces_ts_ms = ctx_ts.stats()["ms_forces"]
+    ctx_ts.timestep(0.25, out=du)
+    torch.cuda.synchronize()
+    c0.record()
+    for _ in range(5):
+        ctx_ts.timestep(0.25, out=du)
+    c1.record()
+    torch.cuda.synchronize()
+    timestep_ms = c0.elapsed_time(c1) / 5
+    dt_global = float(du.min().item())
+    del du, ctx_ts
 
     # end to end through the host-pointer C ABI entry (pinned host inputs -> device -> compute -> host outputs)
     oh = [torch.empty(ps.n).pin_memory() for _ in range(4)]
@@ -291,7 +311,8 @@ def run_ours(args, rank, world, local_rank):
         "e2e": {"value": pairs_all / (e2e_all * 1e-3), "unit": UNIT, "ms_per_step": e2e_all,
                 "h2d_bytes_per_step": int(9 * 4 * n_all), "d2h_bytes_per_step": int(4 * 4 * n_all)},
         "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline,
-        "next_rows": {"evolve_h_ms": evolve_ms, "evolve_h_gbs": 40.0 * ps.n / (evolve_ms * 1e-3) / 1e9,
+        "next_rows": {"forces_with_timestep_maxima_ms": forces_ts_ms, "timestep_pass_ms": timestep_ms,
+                      "timestep_global_min": dt_global, "evolve_h_ms": evolve_ms, "evolve_h_gbs": 40.0 * ps.n / (evolve_ms * 1e-3) / 1e9,
                       "compatible_energy_ms": compat_ms,
                       "compatible_energy_fp32_frac": (FLOPS_PER_PAIR["forces"] + 20.0) * sym_pairs / (compat_ms * 1e-3) / FP32_PEAK_THEORETICAL},
     }

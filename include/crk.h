@@ -52,7 +52,7 @@ typedef struct {
     float C_l, C_q;   /* linear / quadratic viscosity coefficients, (2, 1) in the paper        */
     float eps;        /* 0.1; enters Eq. 25 as eps^2 * hhat^2                                                 */
     int   leaf_size;  /* particles per leaf bucket; must be 32 in this version (one warp lane per particle)   */
-    int   flags;      /* reserved, 0                                                                          */
+    int   flags;      /* 0, or CRK_FLAG_TIMESTEP: the momentum sweep also reduces what crk_timestep needs        */
 } crk_params;
 
 typedef struct {
@@ -103,6 +103,15 @@ int  crk_step_derivs_host(crk_ctx* c, int64_t n, const float* x, const float* y,
  * G1; 1/2 when an entropy P / rho^gamma is not positive).  sum_i m_i delta_u_i = -(kinetic energy change of v -> v').
  * delta_u: device float[n], caller order, written.  One more symmetric pair sweep on the resident state.          */
 int  crk_compatible_energy(crk_ctx* c, float dt, float* delta_u);
+
+/* ---- NEXT row 2a: time-step criteria, Eqs. 46-50, PAPER.md:262-276 (a = 1, adot = 0, no gravity) ----------------
+ * Needs a context created with CRK_FLAG_TIMESTEP in crk_params.flags and a completed crk_hydro_derivs (else CRK_ESTATE):
+ *   v_max = max(v_sig, c_s, sqrt(4 Q_max / rho), hhat |Tr grad v|),  v_sig = max_j max(-(v_ij.x_ij)/|x_ij|, 0)  (S17),
+ *   Q_max = max over the particle's pairs of its Q of Eq. 24 (S18),   dt_min = min(C_cfl hhat / v_max, sqrt(hhat / |dv/dt|)).
+ * dt_min: device float[n], caller order, written (inf where both criteria are unbounded).  One stream pass; the two
+ * maxima ride on the momentum sweep (two fmax per pair).                                                           */
+#define CRK_FLAG_TIMESTEP 1
+int  crk_timestep(crk_ctx* c, float C_cfl, float* dt_min);
 
 /* ---- NEXT row 3: evolved smoothing length, Eqs. 51-53, PAPER.md:340-354 -----------------------------------------
  * After crk_volumes (else CRK_ESTATE): h_new[i] = h_i (1 - lambda + lambda Delta_N) with Delta_N^3 = N_res / N_i,

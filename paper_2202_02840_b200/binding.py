@@ -11,7 +11,7 @@ _LIB_PATH = os.path.join(_HERE, "libcrk.so")
 
 EXPORTED_SYMBOLS = (
     "crk_create", "crk_destroy", "crk_build_cells", "crk_volumes", "crk_rk_coefficients", "crk_hydro_derivs",
-    "crk_step_derivs", "crk_step_derivs_host", "crk_compatible_energy", "crk_evolve_h", "crk_last_error", "crk_get_perm", "crk_get_gradv", "crk_get_leaf_segments", "crk_get_stats",
+    "crk_step_derivs", "crk_step_derivs_host", "crk_compatible_energy", "crk_evolve_h", "crk_timestep", "crk_last_error", "crk_get_perm", "crk_get_gradv", "crk_get_leaf_segments", "crk_get_stats",
     "crk_reset_stats", "crk_set_timing", "crk_get_leaf_list", "crk_measure_fp32_peak",
 )
 
@@ -74,6 +74,7 @@ def _load():
     L.crk_get_gradv.argtypes = [vp, vp]
     L.crk_compatible_energy.argtypes = [vp, C.c_float, vp]
     L.crk_evolve_h.argtypes = [vp, vp]
+    L.crk_timestep.argtypes = [vp, C.c_float, vp]
     L.crk_get_leaf_segments.argtypes = [vp, vp]
     L.crk_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.crk_reset_stats.argtypes = [vp]
@@ -99,12 +100,12 @@ def _opt(t, dtype=torch.float32):
 class Crk:
     """One library context (crk_ctx) bound to the current torch CUDA stream."""
 
-    def __init__(self, box=1.0, gamma=5.0 / 3.0, n_h=2.4, C_l=2.0, C_q=1.0, eps=0.1, stream=None):
+    def __init__(self, box=1.0, gamma=5.0 / 3.0, n_h=2.4, C_l=2.0, C_q=1.0, eps=0.1, stream=None, timestep=False):
         L = _load()
         if not torch.cuda.is_available():
             raise RuntimeError("libcrk needs a CUDA device; there is no CPU fallback")
         self._L = L
-        self._p = _Params(box, gamma, n_h, C_l, C_q, eps, 32, 0)
+        self._p = _Params(box, gamma, n_h, C_l, C_q, eps, 32, 1 if timestep else 0)   # CRK_FLAG_TIMESTEP
         self.stream = stream if stream is not None else torch.cuda.current_stream()
         h = C.c_void_p()
         rc = L.crk_create(C.byref(h), C.byref(self._p), C.c_void_p(self.stream.cuda_stream))
@@ -182,6 +183,12 @@ class Crk:
         self._chk(self._L.crk_step_derivs_host(self._h, n, *[C.c_void_p(t.data_ptr()) for t in (x, y, z, h, vx, vy, vz, m, u)],
                                                *[C.c_void_p(t.data_ptr()) for t in out]))
         return out
+
+    def timestep(self, C_cfl: float = 0.25, out=None):
+        """Eqs. 46-50 after hydro_derivs on a context created with timestep=True"""
+        dt = out if out is not None else torch.empty(self.n, device=self._dev)
+        self._chk(self._L.crk_timestep(self._h, C.c_float(C_cfl), _dev(dt)))
+        return dt
 
     def evolve_h(self, out=None):
         """Eqs. 51-53 after volumes(): adjusted support radii, caller order"""

@@ -54,7 +54,7 @@ void crk_destroy(crk_ctx* c) {
     DevBuf* bufs[] = {&c->keys[0], &c->keys[1], &c->vals[0], &c->vals[1], &c->hist, &c->scan_tmp, &c->posh_orig,
                       &c->posh, &c->leaf_lo, &c->leaf_hi, &c->nbr_cnt, &c->nbr_off, &c->nbr_list, &c->nbr_gcnt,
                       &c->posV, &c->rho_s, &c->coef, &c->fst, &c->u_s, &c->vel_orig, &c->m_s, &c->flag,
-                      &c->host_stage, &c->arena, &c->seg_first, &c->leaf_cnt};
+                      &c->host_stage, &c->arena, &c->seg_first, &c->leaf_cnt, &c->ts_s};
     for (DevBuf* b : bufs)
         if (b->p) cudaFree(b->p);
     if (c->h_flag) cudaFreeHost(c->h_flag);
@@ -182,6 +182,16 @@ int crk_get_perm(crk_ctx* c, int32_t* perm) {
     if (c->n == 0) return CRK_OK;
     CRK_CUDA(c, cudaMemcpyAsync(perm, c->perm, (size_t)c->n * sizeof(int32_t), cudaMemcpyDeviceToDevice, c->stream));
     return CRK_OK;
+}
+
+int crk_timestep(crk_ctx* c, float C_cfl, float* dt_min) {
+    if (!c || !dt_min || !(C_cfl > 0.f)) return CRK_EINVAL;
+    if (c->stage < 4 || !(c->prm.flags & CRK_FLAG_TIMESTEP) || !c->ts_s.p) {
+        snprintf(c->err, sizeof(c->err), "crk_timestep needs crk_hydro_derivs on a context created with CRK_FLAG_TIMESTEP");
+        return CRK_ESTATE;
+    }
+    if (c->n == 0) return CRK_OK;
+    return crk_launch_timestep(c, C_cfl, dt_min);
 }
 
 int crk_evolve_h(crk_ctx* c, float* h_new) {

@@ -77,6 +77,7 @@ struct crk_ctx {
     DevBuf rho_s;                  // float
     DevBuf coef;                   // 4 planes float4[n]: (A,Bx,By,Bz) (cx,cy,cz,M00) (M01,M02,M10,M11) (M12,M20,M21,M22)
     DevBuf fst;                    // force-sweep state, 9 planes float4[np] (layout at k_gradv in pairs.cu) + plane 9 = (dv/dt, s)
+    DevBuf ts_s;                   // float2 (max approach speed, max Q_i), sorted; only with CRK_FLAG_TIMESTEP
     DevBuf u_s;                    // float, specific internal energy in sorted order
     DevBuf vel_orig;               // float4 (vx,vy,vz,u) caller order (packed for a 16-byte gather)
     DevBuf m_s;                    // float, sorted
@@ -146,5 +147,6 @@ int crk_launch_moments(crk_ctx* c, float* A, float* B, float* gradA, float* grad
 int crk_launch_hydro(crk_ctx* c, const float* vx, const float* vy, const float* vz, const float* u,
                      float* ax, float* ay, float* az, float* dudt, uint32_t* pair_count);             // pairs.cu
 int crk_launch_gradv_full(crk_ctx* c, float* gradv);
+int crk_launch_timestep(crk_ctx* c, float C_cfl, float* dt_min);                                       // pairs.cu
 int crk_launch_evolve_h(crk_ctx* c, float* h_new);                                                    // pairs.cu
 int crk_launch_compat(crk_ctx* c, float dt, float* delta_u);                                          // pairs.cu                                                  // pairs.cu

@@ -38,6 +38,7 @@ struct SweepArgs {
     // outputs in caller order (may be null)
     float* __restrict__ o0; float* __restrict__ o1; float* __restrict__ o2; float* __restrict__ o3;
     uint32_t* __restrict__ ocnt;
+    float2* __restrict__ ts;              // (max approach speed, max Q_i) per particle, sorted (time-step criteria), or null
 };
 
 struct Seg {
@@ -178,7 +179,7 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
 }
 
 // add the WPL partial sums of each lane in warp order; the result lands in warp 0 of the group
-template <int WPL, int NACC>
+template <int WPL, int NACC, bool MAX = false>
 __device__ __forceinline__ void group_reduce(float (&acc)[NACC], int lg, int wl, int lane, float* red) {
     if (WPL == 1) return;
     group_sync<WPL>(lg);                                       // the tile is no longer read: reuse it
@@ -190,7 +191,10 @@ __device__ __forceinline__ void group_reduce(float (&acc)[NACC], int lg, int wl,
     if (wl == 0) {
         for (int w2 = 1; w2 < WPL; ++w2)
 #pragma unroll
-            for (int q = 0; q < NACC; ++q) acc[q] += red[((w2 - 1) * NACC + q) * 32 + lane];
+            for (int q = 0; q < NACC; ++q) {
+                const float v = red[((w2 - 1) * NACC + q) * 32 + lane];
+                acc[q] = MAX ? fmaxf(acc[q], v) : acc[q] + v;
+            }
     }
 }
 
@@ -585,7 +589,7 @@ struct ForceConst {
 };
 // one ordered pair (i, j): F = m_i a_ij (Eq. 17 with P -> P + Q) and e = its term of m_i du_i/dt (Eq. 18);
 // vji = v_j - v_i
-struct PairF { float Fx, Fy, Fz, e, vjix, vjiy, vjiz; };
+struct PairF { float Fx, Fy, Fz, e, vjix, vjiy, vjiz, app, Qi; };   // app = approach speed (Eq. 50), Qi (Eq. 24)
 __device__ __forceinline__ PairF force_pair(const ForceConst& k, const PState& I, const PState& J, bool wrapped) {
     float dx, dy, dz;
     if (!wrapped) {
@@ -598,7 +602,8 @@ __device__ __forceinline__ PairF force_pair(const ForceConst& k, const PState& I
         dz = sep1_wrapped(I.z, J.z, k.L, k.half);
     }
     const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-    const float r = __fmul_rn(r2, rsqrt_fast(fmaxf(r2, R2_TINY)));
+    const float rinv = rsqrt_fast(fmaxf(r2, R2_TINY));
+    const float r = __fmul_rn(r2, rinv);
     float Wi, Di, Wj, Dj;
     wendland_dim(r, I.ih, I.k3, I.k5, Wi, Di);
     wendland_dim(r, J.ih, J.k3, J.k5, Wj, Dj);
@@ -636,6 +641,8 @@ __device__ __forceinline__ PairF force_pair(const ForceConst& k, const PState& I
     o.Fx = __fmul_rn(pf, Gx); o.Fy = __fmul_rn(pf, Gy); o.Fz = __fmul_rn(pf, Gz);
     o.e = -hvv * PQj * vG;
     o.vjix = -vx; o.vjiy = -vy; o.vjiz = -vz;
+    o.app = fmaxf(-vdx * rinv, 0.0f);
+    o.Qi = Qi;
     return o;
 }
 
@@ -644,6 +651,7 @@ __device__ __forceinline__ PairF force_pair(const ForceConst& k, const PState& I
 // other three's pair math.  (A persistent, double-buffered variant with 2 x 8 warps per SM was measured slower: 13.1 vs
 // 11.7 ms -- its per-leaf barrier couples all warps of the SM half; profiles/r01_sweeps_v6_ncu_full.md.)
 constexpr int W5_WPL = 4;
+template <bool TS>   // TS: also reduce the per-particle maxima the time-step criteria need (Eqs. 46, 50)
 __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
@@ -654,6 +662,7 @@ __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
     const PState I = load_pstate(a.fst + i, a.np);
     const ForceConst fc = {a.L, a.half, 1.0f / a.n_h, a.n_h / 0.2f, a.eps2, a.C_l, a.C_q};
     float acc[4] = {0.f, 0.f, 0.f, 0.f};                 // Fx, Fy, Fz, dE
+    float mx[2] = {0.f, 0.f};                            // max approach speed, max Q_i
     const float4* planes[FPL];
 #pragma unroll
     for (int p = 0; p < FPL; ++p) planes[p] = a.fst + (int64_t)p * a.np;
@@ -661,9 +670,15 @@ __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
         const PState J = load_pstate_shared(sa, p0);
         const PairF f = force_pair(fc, I, J, wrapped);
         acc[0] += f.Fx; acc[1] += f.Fy; acc[2] += f.Fz; acc[3] += f.e;
+        if (TS) {
+            mx[0] = fmaxf(mx[0], f.app);
+            mx[1] = fmaxf(mx[1], f.Qi);
+        }
     });
     group_reduce<W5_WPL, 4>(acc, 0, wl, lane, (float*)tile);
+    if (TS) group_reduce<W5_WPL, 2, true>(mx, 0, wl, lane, (float*)tile);
     if (wl != 0) return;
+    if (TS) a.ts[i] = make_float2(mx[0], mx[1]);
     float4 as = make_float4(0.f, 0.f, 0.f, 0.f);
     if (valid) {
         const float im = 1.0f / a.m_s[i];
@@ -797,8 +812,15 @@ int crk_launch_hydro(crk_ctx* c, const float* vx, const float* vy, const float* 
     a.o0 = ax; a.o1 = ay; a.o2 = az; a.o3 = dudt; a.ocnt = pair_count;
     {
         const int smem = FPL * CRK_CCAP * (int)sizeof(float4);
-        CRK_TRY(set_smem(c, k_forces, smem));
-        k_forces<<<(unsigned)c->nl, W5_WPL * 32, smem, c->stream>>>(a);
+        if (c->prm.flags & CRK_FLAG_TIMESTEP) {
+            CRK_TRY(crk_ensure(c, c->ts_s, (size_t)np * sizeof(float2)));
+            a.ts = (float2*)c->ts_s.p;
+            CRK_TRY(set_smem(c, k_forces<true>, smem));
+            k_forces<true><<<(unsigned)c->nl, W5_WPL * 32, smem, c->stream>>>(a);
+        } else {
+            CRK_TRY(set_smem(c, k_forces<false>, smem));
+            k_forces<false><<<(unsigned)c->nl, W5_WPL * 32, smem, c->stream>>>(a);
+        }
         CRK_TRY(crk_check_launch(c, "k_forces"));
     }
     crk_rec(c, EV_F1);
@@ -846,4 +868,31 @@ int crk_launch_evolve_h(crk_ctx* c, float* h_new) {
     k_evolve_h<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>((const float4*)c->posh.p, (const float4*)c->posV.p,
                                                                       c->perm, c->n, c->prm.n_h, h_new);
     return crk_check_launch(c, "k_evolve_h");
+}
+
+// NEXT row 2a: time-step criteria, Eqs. 46-50 with a = 1, adot = 0, no gravity: a stream pass over the
+// force-sweep state and the two per-particle maxima reduced by k_forces<true>
+namespace {
+__global__ void __launch_bounds__(256) k_timestep(const float4* __restrict__ fst, const float2* __restrict__ ts,
+                                                  const int32_t* __restrict__ perm, int64_t n, int64_t np, float C_cfl,
+                                                  float* __restrict__ dt_min) {
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= n) return;
+    const float4 th = fst[2 * np + k];                   // P, rho, c_s, k3
+    const float4 g = fst[7 * np + k];                    // g_xx, g_yy, g_zz
+    const float hhat = 1.0f / fst[8 * np + k].w;         // h / n_h
+    const float4 acc = fst[(int64_t)FPL * np + k];       // dv/dt
+    const float2 mx = ts[k];
+    const float csq = sqrtf(4.0f * mx.y / th.y);                                             // sqrt(zeta Q / rho)
+    const float vmax = fmaxf(fmaxf(mx.x, th.z), fmaxf(csq, hhat * fabsf(g.x + g.y + g.z)));  // Eq. 46
+    const float dth = C_cfl * hhat / vmax;                                                   // Eq. 47
+    const float dta = sqrtf(hhat / sqrtf(acc.x * acc.x + acc.y * acc.y + acc.z * acc.z));    // Eq. 48, r_soft = inf
+    dt_min[perm[k]] = fminf(dth, dta);                                                       // Eq. 49
+}
+}  // namespace
+
+int crk_launch_timestep(crk_ctx* c, float C_cfl, float* dt_min) {
+    k_timestep<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>((const float4*)c->fst.p, (const float2*)c->ts_s.p,
+                                                                      c->perm, c->n, c->nl * CRK_LEAF, C_cfl, dt_min);
+    return crk_check_launch(c, "k_timestep");
 }

@@ -418,3 +418,38 @@ def test_evolved_h_parity(name, n_side, oracle_mod):
     assert e < TOL_SCALAR, f"{name} evolved h max rel err {e:.3e}"
     assert (h_o > ps.h).any() and (h_o < ps.h).any()
     print(f"[parity] {name} n={ps.n}: evolved h max rel err {e:.2e}")
+
+
+# ------------------------------------------------------------------------------- NEXT row 2a: time-step criteria
+@pytest.mark.parametrize("name,n_side", [("tiny_uniform", 16), ("blast_wave", 24), ("clustered", 24), ("cosmo", 32)])
+def test_timestep_parity(name, n_side, oracle_mod):
+    """Eqs. 46-50: maxima reduced inside the momentum sweep + the stream pass, vs the FP64 oracle"""
+    torch = _torch()
+    from paper_2202_02840_b200 import Crk, CrkError
+    ps = wl.make_config(name, n_side)
+    o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+    od = o.step_derivs(ps)
+    dt_o, _, _ = o.timestep(0.25)
+    dev = torch.device("cuda:0")
+    t = {k: torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).to(dev) for k in
+         ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")}
+    ctx = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h, timestep=True)
+    ctx.build_cells(t["x"], t["y"], t["z"], t["h"])
+    ctx.volumes(t["m"])
+    ctx.rk_coefficients(want=False)
+    ax, ay, az, du, pc = ctx.hydro_derivs(t["vx"], t["vy"], t["vz"], t["u"])
+    dt_g = ctx.timestep(0.25)
+    torch.cuda.synchronize()
+    # the TS variant of the sweep must give the same derivatives
+    e_a = rel_l2(np.stack([q.cpu().numpy() for q in (ax, ay, az)]), np.stack([od["ax"], od["ay"], od["az"]]))
+    assert e_a < TOL_DERIV
+    dt_g = dt_g.cpu().numpy().astype(np.float64)
+    fin = np.isfinite(dt_o)
+    assert np.array_equal(np.isfinite(dt_g), fin)
+    e = np.max(np.abs(dt_g[fin] / dt_o[fin] - 1))
+    assert e < TOL_DERIV, f"{name} dt_min max rel err {e:.3e}"
+    print(f"[parity] {name} n={ps.n}: dt_min max rel err {e:.2e}, global min {dt_g[fin].min():.3e} (oracle {dt_o[fin].min():.3e})")
+    plain = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h)
+    plain.build_cells(t["x"], t["y"], t["z"], t["h"])
+    with pytest.raises(CrkError):
+        plain.timestep(0.25)
