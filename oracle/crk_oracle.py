@@ -236,6 +236,48 @@ def euler_steps(ps, n_steps: int, dt: float, oracle: Oracle | None = None):
         st["u"] = st["u"] + d["dudt"] * dt
 
 
+def _f32_state(ps, st, L):
+    import copy
+    cur = copy.copy(ps)
+    for k in st:
+        setattr(cur, k, st[k].astype(np.float32))
+    for k in ("x", "y", "z"):           # the float32 cast may round up to L
+        a = getattr(cur, k)
+        a[a >= np.float32(L)] = np.float32(0.0)
+    return cur
+
+
+def kdk_steps(ps, n_steps: int, dt: float, oracle: Oracle | None = None):
+    """NEXT row 2b: the hydro-only velocity-Verlet operator U_V of Eq. 43 with a = 1, dt/dy = 1,
+    p = v, in FP64 on the oracle's derivatives (each evaluation sees the float32 cast of the state, like the library):
+        v^1/2 = v^0 + (1/2) a(x^0, v^0, u^0) dt          u^1/2 = u^0 + (1/2) udot(x^0, v^0, u^0) dt
+        x^1   = x^0 + v^1/2 dt  (wrapped into [0, L))
+        v_p   = v^1/2 + (1/2) a(x^0, v^0, u^0) dt        u_p   = u^1/2 + (1/2) udot(x^0, v^0, u^0) dt     (predictions)
+        v^1   = v^1/2 + (1/2) a(x^1, v_p, u_p) dt        u^1   = u^1/2 + (1/2) udot(x^1, v_p, u_p) dt
+    Reading S19: the "Delta u" of Eq. 43 is taken as (du/dt of Eq. 18) dt.  h and m stay fixed.
+    Returns the FP64 state dict after n_steps."""
+    o = oracle or Oracle(ps.box, ps.gamma, ps.n_h)
+    st = {k: np.asarray(getattr(ps, k), dtype=np.float64).copy() for k in ("x", "y", "z", "vx", "vy", "vz", "u")}
+    L = ps.box
+    ax = (("x", "vx", "ax"), ("y", "vy", "ay"), ("z", "vz", "az"))
+    for _ in range(n_steps):
+        d0 = o.step_derivs(_f32_state(ps, st, L))
+        half = {v: st[v] + 0.5 * d0[a] * dt for _, v, a in ax}
+        u_half = st["u"] + 0.5 * d0["dudt"] * dt
+        pred = dict(st)
+        for k, v, a in ax:
+            p = st[k] + half[v] * dt
+            pred[k] = p - np.floor(p / L) * L
+            pred[v] = half[v] + 0.5 * d0[a] * dt
+        pred["u"] = u_half + 0.5 * d0["dudt"] * dt
+        d1 = o.step_derivs(_f32_state(ps, pred, L))
+        for k, v, a in ax:
+            st[k] = pred[k]
+            st[v] = half[v] + 0.5 * d1[a] * dt
+        st["u"] = u_half + 0.5 * d1["dudt"] * dt
+    return st
+
+
 def h_update(h, n_i, n_h):
     """Eqs. 51-53 for one particle (number density n_i)"""
     return lib().crk_oracle_h_update(float(h), float(n_i), float(n_h))

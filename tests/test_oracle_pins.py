@@ -510,3 +510,36 @@ def test_timestep_acceleration_criterion_from_pair_terms(tiny):
         js, _, _ = o.neighbors(i)
         F = sum(o.pair_term(i, j)[:3] for j in js) / float(ps.m[i])
         assert dta[i] ** 2 * np.linalg.norm(F) == pytest.approx(float(ps.h[i]) / ps.n_h, rel=1e-10)
+
+
+# ---------------------------------------------------------------------------------------- NEXT row 2b: Eq. 43
+def test_kdk_free_streaming_and_wrap(oracle_mod):
+    """u = 0 and no viscosity: P = Q = 0, so a = 0 and Eq. 43 reduces to x^1 = x^0 + v^0 dt (wrapped), v^1 = v^0"""
+    ps = wl.tiny_uniform(n_side=6)
+    ps.u[:] = 0.0
+    o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h, C_l=0.0, C_q=0.0)
+    st = oracle_mod.kdk_steps(ps, 3, 0.4, o)                  # 0.4 * |v| ~ 0.04..0.15: many particles cross a face
+    for k, v in (("x", "vx"), ("y", "vy"), ("z", "vz")):
+        expect = (getattr(ps, k).astype(np.float64) + 3 * 0.4 * getattr(ps, v).astype(np.float64)) % 1.0
+        d = np.abs(st[k] - expect)
+        assert np.minimum(d, 1.0 - d).max() < 1e-6            # float32 cast of x at each evaluation
+        assert np.array_equal(st[v], getattr(ps, v).astype(np.float64))
+    assert ((st["x"] < 0.05) | (st["x"] > 0.95)).any()
+
+
+def test_kdk_conserves_momentum_and_converges_at_second_order(oracle_mod):
+    """Eq. 43 is 'the commonly used second-order velocity Verlet operator': halving dt divides the error
+    by ~4; pairwise antisymmetric forces keep sum m v fixed to roundoff over the steps."""
+    ps = wl.tiny_uniform(n_side=6)
+    o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+    T = 0.016
+    sol = {k: oracle_mod.kdk_steps(ps, k, T / k, o) for k in (1, 2, 4, 16)}
+    m = ps.m.astype(np.float64)
+    for q in ("vx", "vy", "vz"):
+        p0 = (m * getattr(ps, q).astype(np.float64)).sum()
+        assert abs((m * sol[4][q]).sum() - p0) < 1e-12 * (m * np.abs(sol[4][q])).sum()
+    def err(k, key):
+        return np.sqrt(((sol[k][key] - sol[16][key]) ** 2).mean())
+    for key in ("vx", "u"):
+        r1, r2 = err(1, key) / err(2, key), err(2, key) / err(4, key)
+        assert 3.0 < r1 < 5.5 and 3.0 < r2 < 5.5, (key, r1, r2)
