@@ -104,6 +104,16 @@ int  crk_step_derivs_host(crk_ctx* c, int64_t n, const float* x, const float* y,
  * delta_u: device float[n], caller order, written.  One more symmetric pair sweep on the resident state.          */
 int  crk_compatible_energy(crk_ctx* c, float dt, float* delta_u);
 
+/* ---- NEXT row 2b: hydro-only velocity-Verlet step U_V, Eq. 43, PAPER.md:232-241 (a = 1, dt/dy = 1, p = v) --------
+ * Advances the caller's device arrays IN PLACE by one step dt (x, y, z wrapped into [0, box); h, m untouched):
+ *   v^1/2 = v + a dt/2, u^1/2 = u + udot dt/2;  x^1 = x + v^1/2 dt;  predictions v_p = v^1/2 + a dt/2, u_p likewise;
+ *   v^1 = v^1/2 + a(x^1, v_p, u_p) dt/2,  u^1 = u^1/2 + udot(x^1, v_p, u_p) dt/2,
+ * a and udot from two full crk_step_derivs evaluations (udot = Eq. 18, reading S19).  Errors as
+ * crk_step_derivs (CRK_ERANGE if the state leaves the admissible range).  The context is left in the state of the
+ * second evaluation (predicted velocities), so crk_timestep / crk_compatible_energy afterwards refer to that state.   */
+int  crk_kdk_step(crk_ctx* c, int64_t n, float* x, float* y, float* z, const float* h, float* vx, float* vy, float* vz,
+                  const float* m, float* u, float dt);
+
 /* ---- NEXT row 2a: time-step criteria, Eqs. 46-50, PAPER.md:262-276 (a = 1, adot = 0, no gravity) ----------------
  * Needs a context created with CRK_FLAG_TIMESTEP in crk_params.flags and a completed crk_hydro_derivs (else CRK_ESTATE):
  *   v_max = max(v_sig, c_s, sqrt(4 Q_max / rho), hhat |Tr grad v|),  v_sig = max_j max(-(v_ij.x_ij)/|x_ij|, 0)  (S17),

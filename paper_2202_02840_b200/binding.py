@@ -11,7 +11,7 @@ _LIB_PATH = os.path.join(_HERE, "libcrk.so")
 
 EXPORTED_SYMBOLS = (
     "crk_create", "crk_destroy", "crk_build_cells", "crk_volumes", "crk_rk_coefficients", "crk_hydro_derivs",
-    "crk_step_derivs", "crk_step_derivs_host", "crk_compatible_energy", "crk_evolve_h", "crk_timestep", "crk_last_error", "crk_get_perm", "crk_get_gradv", "crk_get_leaf_segments", "crk_get_stats",
+    "crk_step_derivs", "crk_step_derivs_host", "crk_compatible_energy", "crk_evolve_h", "crk_timestep", "crk_kdk_step", "crk_last_error", "crk_get_perm", "crk_get_gradv", "crk_get_leaf_segments", "crk_get_stats",
     "crk_reset_stats", "crk_set_timing", "crk_get_leaf_list", "crk_measure_fp32_peak",
 )
 
@@ -75,6 +75,7 @@ def _load():
     L.crk_compatible_energy.argtypes = [vp, C.c_float, vp]
     L.crk_evolve_h.argtypes = [vp, vp]
     L.crk_timestep.argtypes = [vp, C.c_float, vp]
+    L.crk_kdk_step.argtypes = [vp, i64] + [vp] * 9 + [C.c_float]
     L.crk_get_leaf_segments.argtypes = [vp, vp]
     L.crk_get_stats.argtypes = [vp, C.POINTER(Stats)]
     L.crk_reset_stats.argtypes = [vp]
@@ -183,6 +184,12 @@ class Crk:
         self._chk(self._L.crk_step_derivs_host(self._h, n, *[C.c_void_p(t.data_ptr()) for t in (x, y, z, h, vx, vy, vz, m, u)],
                                                *[C.c_void_p(t.data_ptr()) for t in out]))
         return out
+
+    def kdk_step(self, x, y, z, h, vx, vy, vz, m, u, dt: float):
+        """Eq. 43: one velocity-Verlet step, x, y, z, vx, vy, vz, u advanced in place"""
+        n = x.numel()
+        self.n = n
+        self._chk(self._L.crk_kdk_step(self._h, n, *[_dev(t) for t in (x, y, z, h, vx, vy, vz, m, u)], C.c_float(dt)))
 
     def timestep(self, C_cfl: float = 0.25, out=None):
         """Eqs. 46-50 after hydro_derivs on a context created with timestep=True"""

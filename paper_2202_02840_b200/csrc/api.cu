@@ -54,7 +54,7 @@ void crk_destroy(crk_ctx* c) {
     DevBuf* bufs[] = {&c->keys[0], &c->keys[1], &c->vals[0], &c->vals[1], &c->hist, &c->scan_tmp, &c->posh_orig,
                       &c->posh, &c->leaf_lo, &c->leaf_hi, &c->nbr_cnt, &c->nbr_off, &c->nbr_list, &c->nbr_gcnt,
                       &c->posV, &c->rho_s, &c->coef, &c->fst, &c->u_s, &c->vel_orig, &c->m_s, &c->flag,
-                      &c->host_stage, &c->arena, &c->seg_first, &c->leaf_cnt, &c->ts_s};
+                      &c->host_stage, &c->arena, &c->seg_first, &c->leaf_cnt, &c->ts_s, &c->kdk};
     for (DevBuf* b : bufs)
         if (b->p) cudaFree(b->p);
     if (c->h_flag) cudaFreeHost(c->h_flag);
@@ -151,6 +151,66 @@ int crk_step_derivs(crk_ctx* c, int64_t n, const float* x, const float* y, const
     CRK_TRY(crk_volumes(c, m, nullptr, nullptr, nullptr));
     CRK_TRY(crk_rk_coefficients(c, nullptr, nullptr, nullptr, nullptr));
     return crk_hydro_derivs(c, vx, vy, vz, u, ax, ay, az, dudt, nullptr);
+}
+
+// ---- NEXT row 2b: hydro-only velocity-Verlet step, Eq. 43, a = 1, dt/dy = 1, p = v -----------------
+namespace {
+// v^1/2 = v + a dt/2, u^1/2 = u + udot dt/2 (kept); x <- wrap(x + v^1/2 dt); predictions v_p = v^1/2 + a dt/2, u_p likewise
+__global__ void __launch_bounds__(256) k_kdk_predict(int64_t n, float L, float dt, float* __restrict__ x, float* __restrict__ y,
+                                                     float* __restrict__ z, float* __restrict__ vx, float* __restrict__ vy,
+                                                     float* __restrict__ vz, float* __restrict__ u,
+                                                     const float* __restrict__ d /* [4][n]: a, udot */,
+                                                     float* __restrict__ half /* [4][n]: v^1/2, u^1/2 */) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float hd = 0.5f * dt;
+    float* pos[3] = {x, y, z};
+    float* vel[3] = {vx, vy, vz};
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        const float a = d[q * n + i];
+        const float vh = fmaf(a, hd, vel[q][i]);
+        half[q * n + i] = vh;
+        float p = fmaf(vh, dt, pos[q][i]);
+        p -= floorf(p / L) * L;                         // periodic wrap (reading S12)
+        if (!(p >= 0.f) || p >= L) p = 0.f;             // rounding can land on L
+        pos[q][i] = p;
+        vel[q][i] = fmaf(a, hd, vh);
+    }
+    const float ud = d[3 * n + i];
+    const float uh = fmaf(ud, hd, u[i]);
+    half[3 * n + i] = uh;
+    u[i] = fmaf(ud, hd, uh);
+}
+// v^1 = v^1/2 + a(x^1, v_p, u_p) dt/2, u^1 likewise
+__global__ void __launch_bounds__(256) k_kdk_correct(int64_t n, float dt, float* __restrict__ vx, float* __restrict__ vy,
+                                                     float* __restrict__ vz, float* __restrict__ u,
+                                                     const float* __restrict__ d, const float* __restrict__ half) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    const float hd = 0.5f * dt;
+    vx[i] = fmaf(d[i], hd, half[i]);
+    vy[i] = fmaf(d[n + i], hd, half[n + i]);
+    vz[i] = fmaf(d[2 * n + i], hd, half[2 * n + i]);
+    u[i] = fmaf(d[3 * n + i], hd, half[3 * n + i]);
+}
+}  // namespace
+
+int crk_kdk_step(crk_ctx* c, int64_t n, float* x, float* y, float* z, const float* h, float* vx, float* vy, float* vz,
+                 const float* m, float* u, float dt) {
+    if (!c || n < 0 || !(dt == dt)) return CRK_EINVAL;
+    if (n == 0) return CRK_OK;
+    if (!x || !y || !z || !h || !vx || !vy || !vz || !m || !u) return CRK_EINVAL;
+    CRK_TRY(crk_ensure(c, c->kdk, (size_t)8 * n * sizeof(float)));
+    float* d = (float*)c->kdk.p;
+    float* half = d + 4 * n;
+    const unsigned grid = (unsigned)((n + 255) / 256);
+    CRK_TRY(crk_step_derivs(c, n, x, y, z, h, vx, vy, vz, m, u, d, d + n, d + 2 * n, d + 3 * n));
+    k_kdk_predict<<<grid, 256, 0, c->stream>>>(n, c->prm.box, dt, x, y, z, vx, vy, vz, u, d, half);
+    CRK_TRY(crk_check_launch(c, "k_kdk_predict"));
+    CRK_TRY(crk_step_derivs(c, n, x, y, z, h, vx, vy, vz, m, u, d, d + n, d + 2 * n, d + 3 * n));
+    k_kdk_correct<<<grid, 256, 0, c->stream>>>(n, dt, vx, vy, vz, u, d, half);
+    return crk_check_launch(c, "k_kdk_correct");
 }
 
 int crk_step_derivs_host(crk_ctx* c, int64_t n, const float* x, const float* y, const float* z, const float* h,

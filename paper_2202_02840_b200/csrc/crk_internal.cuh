@@ -78,6 +78,7 @@ struct crk_ctx {
     DevBuf coef;                   // 4 planes float4[n]: (A,Bx,By,Bz) (cx,cy,cz,M00) (M01,M02,M10,M11) (M12,M20,M21,M22)
     DevBuf fst;                    // force-sweep state, 9 planes float4[np] (layout at k_gradv in pairs.cu) + plane 9 = (dv/dt, s)
     DevBuf ts_s;                   // float2 (max approach speed, max Q_i), sorted; only with CRK_FLAG_TIMESTEP
+    DevBuf kdk;                    // crk_kdk_step scratch: derivatives [4][n] and half-step state [4][n]
     DevBuf u_s;                    // float, specific internal energy in sorted order
     DevBuf vel_orig;               // float4 (vx,vy,vz,u) caller order (packed for a 16-byte gather)
     DevBuf m_s;                    // float, sorted

@@ -453,3 +453,37 @@ def test_timestep_parity(name, n_side, oracle_mod):
     plain.build_cells(t["x"], t["y"], t["z"], t["h"])
     with pytest.raises(CrkError):
         plain.timestep(0.25)
+
+
+# ------------------------------------------------------------------------------- NEXT row 2b: velocity-Verlet step
+@pytest.mark.parametrize("name,n_side,dt,steps", [("tiny_uniform", 16, 4e-3, 3), ("clustered", 20, 2e-5, 2), ("cosmo", 32, 2e-3, 2)])
+def test_kdk_step_parity(name, n_side, dt, steps, oracle_mod):
+    """Eq. 43: crk_kdk_step advances the FP32 state in place; compared with the oracle's FP64 KDK"""
+    torch = _torch()
+    from paper_2202_02840_b200 import Crk
+    ps = wl.make_config(name, n_side)
+    ref = oracle_mod.kdk_steps(ps, steps, dt)
+    dev = torch.device("cuda:0")
+    t = {k: torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).to(dev) for k in
+         ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")}
+    ctx = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h)
+    for _ in range(steps):
+        ctx.kdk_step(*[t[k] for k in ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")], dt)
+    torch.cuda.synchronize()
+    g = {k: v.cpu().numpy().astype(np.float64) for k, v in t.items()}
+    for k in ("x", "y", "z"):
+        d = np.abs(g[k] - ref[k])
+        d = np.minimum(d, ps.box - d)
+        assert d.max() < 5e-7 * ps.box, f"{name} {k} max abs err {d.max():.2e}"
+        assert (g[k] >= 0).all() and (g[k] < ps.box).all()
+    moved = max(np.abs(ref[k] - getattr(ps, k)).max() for k in ("x", "y", "z"))
+    e_v = rel_l2(np.stack([g["vx"], g["vy"], g["vz"]]), np.stack([ref["vx"], ref["vy"], ref["vz"]]))
+    e_u = rel_l2(g["u"], ref["u"])
+    assert e_v < TOL_DERIV and e_u < TOL_DERIV, (e_v, e_u)
+    # the step changed something: the velocity change itself must match to 1e-3 of its own size
+    dv_g = np.stack([g[q] - getattr(ps, q) for q in ("vx", "vy", "vz")])
+    dv_o = np.stack([ref[q] - getattr(ps, q) for q in ("vx", "vy", "vz")])
+    e_dv = rel_l2(dv_g, dv_o)
+    assert e_dv < 1e-3, e_dv
+    assert np.array_equal(g["h"], ps.h) and np.array_equal(g["m"], ps.m)
+    print(f"[parity] {name} n={ps.n} {steps} KDK steps dt={dt}: v {e_v:.2e} u {e_u:.2e} dv {e_dv:.2e}, max displacement {moved:.2e}")
