@@ -175,6 +175,9 @@ def run_ours(args, rank, world, local_rank):
 
     # each rank owns an independent seeded box of the same recipe (weak scaling; the path has no exchange step on one box)
     ps = wl.make_config(args.config, args.n_side, seed=rank_seed(args.config, rank))
+    if args.n_h is not None:
+        ps.h[:] = (ps.h * (args.n_h / ps.n_h)).astype(np.float32)
+        ps.n_h = float(args.n_h)
     names = ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")
     host = [torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).pin_memory() for k in names]
     t = [h.to(dev, non_blocking=True) for h in host]
@@ -309,7 +312,8 @@ def run_ours(args, rank, world, local_rank):
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
         "data": "synthetic",
-        "config": {"workload": f"{ps.name} n_side={ps.meta['n_side']} ({ps.n} particles per GPU, ~{gather_pairs / ps.n:.1f} neighbours)",
+        "config": {"workload": f"{ps.name} n_side={ps.meta['n_side']} ({ps.n} particles per GPU, ~{gather_pairs / ps.n:.1f} neighbours"
+                               + (f", n_h rescaled to {args.n_h}" if args.n_h is not None else "") + ")",
                    "particles": int(n_all), "pairs_per_step": pairs_all,
                    "l2": "inputs and per-step state exceed the 126 MB L2 (no flush needed)" if ps.n * 200 > 126e6
                          else "state fits in L2 (small config; not the headline)"},
@@ -349,6 +353,9 @@ def main():
     ap.add_argument("--oracle-particles", type=int, default=262144,
                     help="size of the bounded sample handed to the O(n^2) oracle (262144 particles ~ 10-20 s of CPU work)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--n-h", type=float, default=None,
+                    help="NEXT row 4: rescale every support radius to this many particle spacings (paper default 4 = 268 "
+                         "neighbours, PAPER.md:336); not the BASELINE workload")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

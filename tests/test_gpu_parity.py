@@ -487,3 +487,24 @@ def test_kdk_step_parity(name, n_side, dt, steps, oracle_mod):
     assert e_dv < 1e-3, e_dv
     assert np.array_equal(g["h"], ps.h) and np.array_equal(g["m"], ps.m)
     print(f"[parity] {name} n={ps.n} {steps} KDK steps dt={dt}: v {e_v:.2e} u {e_u:.2e} dv {e_dv:.2e}, max displacement {moved:.2e}")
+
+
+# ------------------------------------------------------------------------------- NEXT row 4: paper-default resolution n_h = 4
+@pytest.mark.parametrize("name,n_side", [("tiny_uniform", 16), ("cosmo", 24)])
+def test_parity_paper_default_resolution_nh4(name, n_side, oracle_mod):
+    """n_h = 4 (N_res = 268 neighbours): every leaf needs a chain of neighbour-list segments (~900
+    candidates against 352 slots), which exercises the multi-segment path of the builder and of all sweeps."""
+    ps = wl.make_config(name, n_side)
+    ps.h[:] = (ps.h * (4.0 / ps.n_h)).astype(np.float32)
+    ps.n_h = 4.0
+    assert float(ps.h.max()) < 0.5 * ps.box
+    o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+    od = o.step_derivs(ps)
+    g = gpu_eval(ps)
+    e_a, e_u = check_parity(ps, g, od, oracle_gv=o.gradv(), label=name + " n_h=4")
+    mom, en = check_invariants(ps, g, label=name + " n_h=4")
+    seg = g["ctx"].leaf_segments().cpu().numpy()
+    multi = float((seg[:, 0] != 0).mean())
+    assert multi > 0.9
+    print(f"[parity] {name} n_h=4 n={ps.n}: mean neighbours {od['nbr_count'].mean():.0f}, multi-segment leaves {multi:.2f}, "
+          f"dv/dt {e_a:.2e} du/dt {e_u:.2e} momentum {mom:.2e} energy {en:.2e}")
