@@ -58,6 +58,10 @@ void crk_destroy(crk_ctx* c) {
     for (DevBuf* b : bufs)
         if (b->p) cudaFree(b->p);
     if (c->h_flag) cudaFreeHost(c->h_flag);
+    if (c->copy_stream) {
+        cudaStreamDestroy(c->copy_stream);
+        cudaEventDestroy(c->ev_copy);
+    }
     if (c->ev_ok)
         for (int r = 0; r < CRK_EV_RING; ++r)
             for (int e = 0; e < CRK_EV_N; ++e) cudaEventDestroy(c->ev[r][e]);
@@ -223,12 +227,30 @@ int crk_step_derivs_host(crk_ctx* c, int64_t n, const float* x, const float* y, 
     CRK_TRY(crk_ensure(c, c->host_stage, 13 * stride * sizeof(float)));
     float* d = (float*)c->host_stage.p;
     const float* in[9] = {x, y, z, h, vx, vy, vz, m, u};
-    for (int q = 0; q < 9; ++q)
+    // x, y, z, h go first on the compute stream; the other five arrays travel on a copy stream while the build (sort, tree,
+    // neighbour lists: about a third of the step) already runs -- the volume pass waits for them with an event
+    if (!c->copy_stream) {
+        CRK_CUDA(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        CRK_CUDA(c, cudaEventCreateWithFlags(&c->ev_copy, cudaEventDisableTiming));
+    }
+    for (int q = 0; q < 4; ++q)
         CRK_CUDA(c, cudaMemcpyAsync(d + q * stride, in[q], (size_t)n * sizeof(float), cudaMemcpyHostToDevice, c->stream));
+    for (int q = 4; q < 9; ++q)
+        CRK_CUDA(c, cudaMemcpyAsync(d + q * stride, in[q], (size_t)n * sizeof(float), cudaMemcpyHostToDevice, c->copy_stream));
+    CRK_CUDA(c, cudaEventRecord(c->ev_copy, c->copy_stream));
     float* o = d + 9 * stride;
-    CRK_TRY(crk_step_derivs(c, n, d, d + stride, d + 2 * stride, d + 3 * stride, d + 4 * stride, d + 5 * stride,
-                            d + 6 * stride, d + 7 * stride, d + 8 * stride, o, o + stride, o + 2 * stride,
-                            o + 3 * stride));
+    {
+        const int rc = crk_build_cells(c, n, d, d + stride, d + 2 * stride, d + 3 * stride);
+        if (rc != CRK_OK) {
+            cudaStreamSynchronize(c->copy_stream);       // the caller may reuse its buffers as soon as we return
+            return rc;
+        }
+    }
+    CRK_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_copy, 0));
+    CRK_TRY(crk_volumes(c, d + 7 * stride, nullptr, nullptr, nullptr));
+    CRK_TRY(crk_rk_coefficients(c, nullptr, nullptr, nullptr, nullptr));
+    CRK_TRY(crk_hydro_derivs(c, d + 4 * stride, d + 5 * stride, d + 6 * stride, d + 8 * stride, o, o + stride, o + 2 * stride,
+                             o + 3 * stride, nullptr));
     float* out[4] = {ax, ay, az, dudt};
     for (int q = 0; q < 4; ++q)
         CRK_CUDA(c, cudaMemcpyAsync(out[q], o + q * stride, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, c->stream));

@@ -44,6 +44,8 @@ struct DevBuf {
 struct crk_ctx {
     crk_params prm;
     cudaStream_t stream = 0;
+    cudaStream_t copy_stream = nullptr;      // crk_step_derivs_host: second H2D stream (created on first use)
+    cudaEvent_t ev_copy = nullptr;
     int64_t n = 0, nl = 0;
     int stage = 0;                 // 0 none, 1 built, 2 volumes, 3 coefficients, 4 hydro
     char err[256];
