@@ -95,20 +95,32 @@ __global__ void __launch_bounds__(SORT_THREADS) k_radix_hist(const uint64_t* __r
     hist[(int64_t)threadIdx.x * nblk + blockIdx.x] = cnt[threadIdx.x];
 }
 
-// stable scatter: each warp owns 512 consecutive keys (16 rounds of 32), ranks them with match_any
+// stable scatter: each warp owns 512 consecutive keys (16 rounds of 32) and ranks them with match_any; the tile is then
+// put in digit order in shared memory and written out as contiguous runs (one run per digit and CTA: ~16 keys = 128 B
+// for uniform digits), so a warp store touches a handful of sectors instead of 32
+struct ScatterSmem {
+    uint64_t key[SORT_TILE];                 // tile in local digit order
+    uint32_t val[SORT_TILE];
+    uint32_t wcnt[SORT_WARPS][RADIX];        // per-warp digit counts -> per-warp base inside the digit run
+    uint32_t lbase[RADIX];                   // first local position of the digit run
+    uint32_t gbase[RADIX];                   // first global position of the digit run
+    uint32_t wsum[SORT_WARPS];
+};
 __global__ void __launch_bounds__(SORT_THREADS) k_radix_scatter(const uint64_t* __restrict__ keys_in,
                                                                 const uint32_t* __restrict__ vals_in,
                                                                 uint64_t* __restrict__ keys_out,
                                                                 uint32_t* __restrict__ vals_out, int64_t n, int shift,
                                                                 const uint32_t* __restrict__ offs, int nblk) {
-    __shared__ uint32_t wcnt[SORT_WARPS][RADIX];
+    extern __shared__ __align__(16) unsigned char scatter_raw[];
+    ScatterSmem& S = *(ScatterSmem*)scatter_raw;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    for (int q = threadIdx.x; q < SORT_WARPS * RADIX; q += SORT_THREADS) (&wcnt[0][0])[q] = 0;
+    for (int q = threadIdx.x; q < SORT_WARPS * RADIX; q += SORT_THREADS) (&S.wcnt[0][0])[q] = 0;
     __syncthreads();
-    const int64_t wbase = (int64_t)blockIdx.x * SORT_TILE + (int64_t)w * (32 * SORT_ROUNDS);
+    const int64_t tbase = (int64_t)blockIdx.x * SORT_TILE;
+    const int64_t wbase = tbase + (int64_t)w * (32 * SORT_ROUNDS);
     uint64_t k[SORT_ROUNDS];
     uint32_t v[SORT_ROUNDS];
-    uint32_t rk[SORT_ROUNDS];     // first: digit | rank among equal digits of the round << 9 | group size << 15 ; then: final rank
+    uint32_t rk[SORT_ROUNDS];     // first: digit | rank among equal digits of the round << 9 | group size << 15 ; then: rank in (warp, digit)
     const uint32_t lt = (1u << lane) - 1u;
     // phase 1 (independent per round, so the loads and the match instructions overlap): digit, rank within the round
 #pragma unroll
@@ -131,33 +143,59 @@ __global__ void __launch_bounds__(SORT_THREADS) k_radix_scatter(const uint64_t* 
         const uint32_t d = rk[r] & 0x1ffu, rank = (rk[r] >> 9) & 0x3fu, gsz = rk[r] >> 15;
         const bool valid = d < (uint32_t)RADIX;
         uint32_t prev = 0;
-        if (valid) prev = wcnt[w][d];
+        if (valid) prev = S.wcnt[w][d];
         __syncwarp();
-        if (valid && rank == 0) wcnt[w][d] = prev + gsz;
+        if (valid && rank == 0) S.wcnt[w][d] = prev + gsz;
         __syncwarp();
         rk[r] = prev + rank;
     }
     __syncthreads();
+    // phase 3: thread d owns digit d (256 threads <-> 256 digits): per-warp bases inside the run, run length, block scan
     {
-        const int d = threadIdx.x;   // 256 threads <-> 256 digits
-        uint32_t run = offs[(int64_t)d * nblk + blockIdx.x];
+        const int d = threadIdx.x;
+        uint32_t run = 0;
 #pragma unroll
         for (int ww = 0; ww < SORT_WARPS; ++ww) {
-            const uint32_t cc = wcnt[ww][d];
-            wcnt[ww][d] = run;
+            const uint32_t cc = S.wcnt[ww][d];
+            S.wcnt[ww][d] = run;
             run += cc;
         }
+        // exclusive scan of the 256 run lengths
+        uint32_t inc = run;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) S.wsum[w] = inc;
+        __syncthreads();
+        uint32_t wpre = 0;
+#pragma unroll
+        for (int ww = 0; ww < SORT_WARPS; ++ww) wpre += (ww < w) ? S.wsum[ww] : 0u;
+        S.lbase[d] = wpre + inc - run;
+        S.gbase[d] = offs[(int64_t)d * nblk + blockIdx.x];
     }
     __syncthreads();
+    // phase 4: tile -> shared memory in digit order
 #pragma unroll
     for (int r = 0; r < SORT_ROUNDS; ++r) {
         const int64_t idx = wbase + r * 32 + lane;
         if (idx < n) {
             const uint32_t d = (uint32_t)(k[r] >> shift) & (RADIX - 1);
-            const uint32_t pos = wcnt[w][d] + rk[r];
-            keys_out[pos] = k[r];
-            vals_out[pos] = v[r];
+            const uint32_t lp = S.lbase[d] + S.wcnt[w][d] + rk[r];
+            S.key[lp] = k[r];
+            S.val[lp] = v[r];
         }
+    }
+    __syncthreads();
+    // phase 5: contiguous runs out
+    const int cnt = (int)min((int64_t)SORT_TILE, n - tbase);
+    for (int p = threadIdx.x; p < cnt; p += SORT_THREADS) {
+        const uint64_t kk = S.key[p];
+        const uint32_t d = (uint32_t)(kk >> shift) & (RADIX - 1);
+        const uint32_t pos = S.gbase[d] + ((uint32_t)p - S.lbase[d]);
+        keys_out[pos] = kk;
+        vals_out[pos] = S.val[p];
     }
 }
 
@@ -314,13 +352,14 @@ int crk_sort_particles(crk_ctx* c, const float* x, const float* y, const float* 
         }
         if (bits < 6) bits = 6;
     }
+    CRK_CUDA(c, cudaFuncSetAttribute(k_radix_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ScatterSmem)));
     int cur = 0;
     c->st.sort_passes = (3 * bits + RADIX_BITS - 1) / RADIX_BITS;
     for (int shift = 3 * (CRK_KEY_BITS - bits); shift < 3 * CRK_KEY_BITS; shift += RADIX_BITS) {
         k_radix_hist<<<nblk, SORT_THREADS, 0, c->stream>>>((const uint64_t*)c->keys[cur].p, n, shift, hist, nblk);
         CRK_TRY(crk_check_launch(c, "k_radix_hist"));
         CRK_TRY(crk_exclusive_scan_u32(c, hist, offs, (int64_t)RADIX * nblk, c->scan_tmp));
-        k_radix_scatter<<<nblk, SORT_THREADS, 0, c->stream>>>((const uint64_t*)c->keys[cur].p,
+        k_radix_scatter<<<nblk, SORT_THREADS, sizeof(ScatterSmem), c->stream>>>((const uint64_t*)c->keys[cur].p,
                                                               (const uint32_t*)c->vals[cur].p,
                                                               (uint64_t*)c->keys[cur ^ 1].p,
                                                               (uint32_t*)c->vals[cur ^ 1].p, n, shift, offs, nblk);
