@@ -285,7 +285,7 @@ __global__ void __launch_bounds__(W1_WPC * 32) k_volumes(SweepArgs a) {
 //   d_c A = -A^2 (d_c m0 + 2 B.d_c m1 + B^T d_c m2 B),  d_c B = -m2^-1 (d_c m1 + d_c m2 B).
 // 29 FP32 sums per particle in eta-normalised units, then an FP64 3x3 solve per particle.
 constexpr int W2_WPC = 4;
-__global__ void __launch_bounds__(W2_WPC * 32) k_moments(SweepArgs a) {
+__global__ void __launch_bounds__(W2_WPC * 32, 6) k_moments(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int64_t leaf = (int64_t)blockIdx.x * W2_WPC + w;
