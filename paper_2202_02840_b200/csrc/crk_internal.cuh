@@ -26,8 +26,8 @@ enum { EV_BUILD0 = 0, EV_SORTED, EV_TREE1, EV_BUILD1, EV_VOL0, EV_VOL1, EV_RK0, 
 //   ell[k][l] = k-th entry of lane l: candidate index | bit 15 (pair crosses the periodic boundary); lane l owns
 //               cnt_g[l] gather entries (r2 < h_i^2) followed by cnt[l] - cnt_g[l] entries that are symmetric-only
 #define CRK_CCAP 352             // candidates per segment (tile capacity of the sweeps)
-#define CRK_QCAP 176             // entries per lane per segment
-#define CRK_TCULL 48             // cull tile of the list builder
+#define CRK_QCAP 128             // entries per lane per segment
+#define CRK_TCULL 32             // cull tile of the list builder
 #define CRK_SEG_HDR_UNITS 9
 #define CRK_ELL_WRAP 0x8000u
 #define CRK_ELL_MASK 0x7fffu
