@@ -239,7 +239,7 @@ __device__ __forceinline__ void sep3(const SweepArgs& a, bool wrapped, float xi,
 
 // =================================================================================================== a1: volumes
 // Eq. 14: V_i^-1 = n_i = sum_j W(|x_i - x_j|, h_i), self term included (S4); rho_i = m_i / V_i (S2).
-constexpr int W1_WPC = 4;
+constexpr int W1_WPC = 2;
 __global__ void __launch_bounds__(W1_WPC * 32) k_volumes(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -284,8 +284,8 @@ __global__ void __launch_bounds__(W1_WPC * 32) k_volumes(SweepArgs a) {
 //   (g = V_j W'_ij / r):   B = -m2^-1 m1,  A = 1/(m0 + B.m1),
 //   d_c A = -A^2 (d_c m0 + 2 B.d_c m1 + B^T d_c m2 B),  d_c B = -m2^-1 (d_c m1 + d_c m2 B).
 // 29 FP32 sums per particle in eta-normalised units, then an FP64 3x3 solve per particle.
-constexpr int W2_WPC = 4;
-__global__ void __launch_bounds__(W2_WPC * 32, 6) k_moments(SweepArgs a) {
+constexpr int W2_WPC = 2;
+__global__ void __launch_bounds__(W2_WPC * 32, 12) k_moments(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int64_t leaf = (int64_t)blockIdx.x * W2_WPC + w;
