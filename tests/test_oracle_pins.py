@@ -543,3 +543,31 @@ def test_kdk_conserves_momentum_and_converges_at_second_order(oracle_mod):
     for key in ("vx", "u"):
         r1, r2 = err(1, key) / err(2, key), err(2, key) / err(4, key)
         assert 3.0 < r1 < 5.5 and 3.0 < r2 < 5.5, (key, r1, r2)
+
+
+def test_next_row_constants_match_the_paper(oracle_mod):
+    """the constants of Eqs. 47, 46 (zeta) and 53 as printed (tests/golden/paper_constants.txt) are the ones in the oracle"""
+    G = golden()
+    h, n_h = 0.2, 2.4
+    N_res = 4.0 / 3.0 * math.pi * n_h ** 3
+    # Delta_N -> 0+ (far too many neighbours): lambda -> 0.2, h~/h -> 1 - 0.2
+    n_big = 1e9 * N_res / (4.0 / 3.0 * math.pi * h ** 3)
+    assert abs(oracle_mod.h_update(h, n_big, n_h) / h - (1.0 - G["evolved_h_lambda_coeff"])) < 2e-4
+    # static lattice: dt = C_CFL hhat / c_s scales linearly with the CFL coefficient; C = 0.25 is the paper's
+    ps = wl.tiny_uniform(n_side=6)
+    o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+    d = o.step_derivs(ps)
+    _, th1, _ = o.timestep(G["cfl_coefficient"])
+    _, th2, _ = o.timestep(1.0)
+    assert np.allclose(th1, G["cfl_coefficient"] * th2, rtol=1e-14)
+    # zeta: a particle whose v_max is set by the viscous sound speed obeys v_max^2 rho = zeta Q_max
+    rho = d["rho"]
+    hhat = ps.h.astype(np.float64) / ps.n_h
+    vmax = 1.0 * hhat / th2
+    found = 0
+    for i in range(ps.n):
+        js, _, _ = o.neighbors(i)
+        Q = max(o.pair_visc(i, j)[1] for j in js)
+        if Q > 0 and abs(vmax[i] ** 2 * rho[i] / Q - G["visc_sound_zeta"]) < 1e-9:
+            found += 1
+    assert found > 0
