@@ -508,3 +508,44 @@ def test_parity_paper_default_resolution_nh4(name, n_side, oracle_mod):
     assert multi > 0.9
     print(f"[parity] {name} n_h=4 n={ps.n}: mean neighbours {od['nbr_count'].mean():.0f}, multi-segment leaves {multi:.2f}, "
           f"dv/dt {e_a:.2e} du/dt {e_u:.2e} momentum {mom:.2e} energy {en:.2e}")
+
+
+def test_parity_non_default_parameters(oracle_mod):
+    """box != 1, gamma = 1.4, unequal masses (reading S2), other viscosity constants and n_h: every runtime parameter of
+    crk_params reaches the kernels"""
+    torch = _torch()
+    from paper_2202_02840_b200 import Crk
+    ps = wl.clustered_plummer(n_side=20)
+    L = 2.5
+    rng = np.random.default_rng(11)
+    for k in ("x", "y", "z", "h"):
+        setattr(ps, k, (getattr(ps, k).astype(np.float64) * L).astype(np.float32))
+    for k in ("x", "y", "z"):
+        a = getattr(ps, k)
+        a[a >= np.float32(L)] = np.float32(0.0)
+    ps.m = (ps.m * rng.uniform(0.7, 1.3, ps.n)).astype(np.float32)
+    ps.box, ps.gamma, ps.n_h = L, 1.4, 3.0       # n_h enters through hhat, eta_crit, eta_fold only: the 58 neighbours stay
+    kw = dict(C_l=1.0, C_q=2.5, eps=0.05)
+    o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h, **kw)
+    od = o.step_derivs(ps)
+    dev = torch.device("cuda:0")
+    t = {k: torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).to(dev) for k in
+         ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")}
+    ctx = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h, timestep=True, **kw)
+    ctx.build_cells(t["x"], t["y"], t["z"], t["h"])
+    V, rho, cnt = ctx.volumes(t["m"])
+    A, B, gA, gB = ctx.rk_coefficients()
+    ax, ay, az, du, pc = ctx.hydro_derivs(t["vx"], t["vy"], t["vz"], t["u"])
+    g = dict(V=V, rho=rho, nbr_count=cnt, A=A, B=B, gradA=gA, gradB=gB, ax=ax, ay=ay, az=az, dudt=du, pair_count=pc,
+             gradv=ctx.gradv())
+    dt_g = ctx.timestep(0.3)
+    du_c = ctx.compatible_energy(1e-4)
+    torch.cuda.synchronize()
+    g = {k: v.cpu().numpy() for k, v in g.items()}
+    e_a, e_u = check_parity(ps, g, od, oracle_gv=o.gradv(), label="non-default params")
+    mom, en = check_invariants(ps, g, label="non-default params")
+    dt_o, _, _ = o.timestep(0.3)
+    fin = np.isfinite(dt_o)
+    assert np.max(np.abs(dt_g.cpu().numpy()[fin] / dt_o[fin] - 1)) < TOL_DERIV
+    assert rel_l2(du_c.cpu().numpy().astype(np.float64), o.compatible_energy(1e-4)) < TOL_DERIV
+    print(f"[parity] non-default params n={ps.n}: dv/dt {e_a:.2e} du/dt {e_u:.2e} momentum {mom:.2e} energy {en:.2e}")
