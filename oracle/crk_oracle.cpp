@@ -440,6 +440,63 @@ int crk_oracle_hydro_derivs(crk_oracle_ctx* c, const float* vx, const float* vy,
     return 0;
 }
 
+// ---- oracle at scale: neighbour COUNTS of a full configuration (SURVEY.md section 8(c) "oracle at scale") -------------
+// The brute-force scan is O(N^2); for the 128^3 .. 512^3 configurations the counts of every particle come from this second
+// formulation: particles are binned in a uniform periodic grid of cells no smaller than the largest h, so every j with
+// r < max(h_i, h_j) sits in the 27 cells around i; the predicate is the same prescribed FP32 expression (r2_f32, S3).
+// It is pinned by bit-exact agreement with crk_oracle_build on small sets (tests/test_oracle_pins.py).
+int crk_oracle_grid_counts(double box, int64_t n, const float* x, const float* y, const float* z, const float* h,
+                           uint32_t* nbr_count, uint32_t* pair_count) {
+    if (n < 0 || (n > 0 && (!x || !y || !z || !h || !nbr_count || !pair_count))) return -1;
+    set_threads();
+    const float L = (float)box, half = 0.5f * L;
+    float hmax = 0.0f;
+    for (int64_t i = 0; i < n; ++i) {
+        if (!(h[i] > 0.0f) || !(h[i] < half)) return -1;
+        if (!(x[i] >= 0.0f && x[i] < L && y[i] >= 0.0f && y[i] < L && z[i] >= 0.0f && z[i] < L)) return -1;
+        hmax = std::max(hmax, h[i]);
+    }
+    if (n == 0) return 0;
+    // cells of side >= hmax (a little larger so that FP32 rounding of r cannot reach across two cells)
+    int nc = (int)std::floor((double)L / ((double)hmax * 1.0001));
+    nc = std::min(nc, 1024);
+    if (nc < 3) return -2;                      // the 27-cell stencil would visit a cell twice: use the brute-force build
+    const double inv = (double)nc / (double)L;
+    auto cell_of = [&](float p) { int q = (int)std::floor((double)p * inv); return q < 0 ? 0 : (q >= nc ? nc - 1 : q); };
+    const int64_t ncell = (int64_t)nc * nc * nc;
+    std::vector<int64_t> start((size_t)ncell + 1, 0);
+    std::vector<int64_t> cid((size_t)n);
+    for (int64_t i = 0; i < n; ++i) {
+        cid[i] = ((int64_t)cell_of(x[i]) * nc + cell_of(y[i])) * nc + cell_of(z[i]);
+        ++start[cid[i] + 1];
+    }
+    for (int64_t q = 0; q < ncell; ++q) start[q + 1] += start[q];
+    std::vector<int64_t> fill(start.begin(), start.end() - 1), order((size_t)n);
+    for (int64_t i = 0; i < n; ++i) order[fill[cid[i]]++] = i;
+#pragma omp parallel for schedule(dynamic, 256)
+    for (int64_t i = 0; i < n; ++i) {
+        const float xi = x[i], yi = y[i], zi = z[i], hi2 = h[i] * h[i];
+        const int cx = cell_of(xi), cy = cell_of(yi), cz = cell_of(zi);
+        uint32_t cg = 0, cs = 0;
+        for (int dx = -1; dx <= 1; ++dx)
+            for (int dy = -1; dy <= 1; ++dy)
+                for (int dz = -1; dz <= 1; ++dz) {
+                    const int64_t q = ((int64_t)((cx + dx + nc) % nc) * nc + (cy + dy + nc) % nc) * nc + (cz + dz + nc) % nc;
+                    for (int64_t k = start[q]; k < start[q + 1]; ++k) {
+                        const int64_t j = order[k];
+                        if (j == i) continue;
+                        const float r2 = r2_f32(xi, yi, zi, x[j], y[j], z[j], L, half);
+                        const float hj2 = h[j] * h[j];
+                        if (r2 < hi2) ++cg;
+                        if (r2 < std::max(hi2, hj2)) ++cs;
+                    }
+                }
+        nbr_count[i] = cg;
+        pair_count[i] = cs;
+    }
+    return 0;
+}
+
 // ---- NEXT row 2a: time-step criteria, Eqs. 46-50, a = 1, adot = 0, dy/dt = 1, no gravity ----------
 // Eq. 50 (sign garbled as printed; reading S17: the approach speed): v_sig,ij = max(-(v_ij . x_ij) / |x_ij|, 0),
 //   v_sig,i = max_j v_sig,ij over the pairs of the momentum sweep (r < max(h_i, h_j)).

@@ -61,6 +61,13 @@ int crk_oracle_compatible_energy(crk_oracle_ctx* c, double dt, double* delta_u);
 /* one pair of the above: out = { du_ij (Eq. 20), dE_ij (Eq. 21), f_ij (Eq. 23) }                                 */
 int crk_oracle_pair_compat(crk_oracle_ctx* c, int64_t i, int64_t j, double dt, double out[3]);
 
+/* Oracle at scale: nbr_count[i] = #{j != i : r_ij < h_i} and pair_count[i] = #{j != i : r_ij < max(h_i, h_j)} of a FULL
+ * configuration through a uniform periodic grid of cells >= h_max (27-cell stencil) with the same FP32 predicate (S3).
+ * Pinned by bit-exact agreement with crk_oracle_build / _volumes / _hydro_derivs counts on small sets.  Returns -2 if
+ * the box holds fewer than 3 cells per side (use the brute-force build then), -1 on bad input.                        */
+int crk_oracle_grid_counts(double box, int64_t n, const float* x, const float* y, const float* z, const float* h,
+                           uint32_t* nbr_count, uint32_t* pair_count);
+
 /* NEXT row 2a -- time-step criteria, Eqs. 46-50 with a = 1, adot = 0, no gravity, after
  * crk_oracle_hydro_derivs: dt_min = min(C_cfl hhat / max(v_sig, c_s, sqrt(4 Q_max / rho), hhat |Tr grad v|), sqrt(hhat / |a|)).
  * dt_hyd / dt_acc (nullable) return the two criteria separately.  Pinned: static gas closed form C hhat / c_s, linear

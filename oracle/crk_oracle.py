@@ -51,6 +51,7 @@ def lib():
         L.crk_oracle_pair_visc.argtypes = [C.c_void_p, C.c_int64, C.c_int64, dp]
         L.crk_oracle_compatible_energy.argtypes = [C.c_void_p, C.c_double, dp]
         L.crk_oracle_evolve_h.argtypes = [C.c_void_p, dp]
+        L.crk_oracle_grid_counts.argtypes = [C.c_double, C.c_int64, fp, fp, fp, fp, up, up]
         L.crk_oracle_timestep.argtypes = [C.c_void_p, C.c_double, dp, dp, dp]
         L.crk_oracle_h_update.argtypes = [C.c_double, C.c_double, C.c_double]
         L.crk_oracle_h_update.restype = C.c_double
@@ -276,6 +277,18 @@ def kdk_steps(ps, n_steps: int, dt: float, oracle: Oracle | None = None):
             st[v] = half[v] + 0.5 * d1[a] * dt
         st["u"] = u_half + 0.5 * d1["dudt"] * dt
     return st
+
+
+def grid_counts(ps):
+    """oracle at scale: (nbr_count, pair_count) of every particle of a full configuration (uniform grid of cells >= h_max,
+    same FP32 predicate as the brute-force build)"""
+    n = ps.n
+    a, b = np.empty(n, dtype=np.uint32), np.empty(n, dtype=np.uint32)
+    arrs = [np.ascontiguousarray(getattr(ps, k), dtype=np.float32) for k in ("x", "y", "z", "h")]
+    rc = lib().crk_oracle_grid_counts(float(ps.box), n, *[_f(q)[1] for q in arrs], _u(a), _u(b))
+    if rc != 0:
+        raise RuntimeError(f"crk_oracle_grid_counts failed ({rc})")
+    return a, b
 
 
 def h_update(h, n_i, n_h):

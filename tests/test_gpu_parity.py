@@ -264,10 +264,19 @@ def _window_check(ps, oracle_mod, centres, half_in_h=2.5, label=""):
     return g
 
 
+def _full_count_check(ps, g, oracle_mod, label):
+    """bit-exact neighbour / pair counts of EVERY particle against the oracle's grid formulation (oracle at scale)"""
+    cg, cs = oracle_mod.grid_counts(ps)
+    assert np.array_equal(np.asarray(g["nbr_count"]).astype(np.uint32), cg), label + " nbr_count (all particles)"
+    assert np.array_equal(np.asarray(g["pair_count"]).astype(np.uint32), cs), label + " pair_count (all particles)"
+    print(f"[parity] {label}: counts of all {ps.n} particles bit-exact (gather {int(cg.sum())}, symmetric {int(cs.sum())})")
+
+
 def test_parity_config2_blast_full(oracle_mod):
     ps = wl.make_config("blast_wave")
     c = [(0.5, 0.5, 0.5), (0.1, 0.9, 0.3)]
-    _window_check(ps, oracle_mod, c, half_in_h=3.0, label="blast64")
+    g = _window_check(ps, oracle_mod, c, half_in_h=3.0, label="blast64")
+    _full_count_check(ps, g, oracle_mod, "blast64")
 
 
 def test_parity_config3_clustered_full(oracle_mod):
@@ -282,6 +291,7 @@ def test_parity_config4_cosmo_full(oracle_mod):
     ps = wl.make_config("cosmo")
     centres = [(0.5, 0.5, 0.5), (0.001, 0.999, 0.5), (0.25, 0.75, 0.1)]
     g = _window_check(ps, oracle_mod, centres, half_in_h=3.0, label="cosmo256")
+    _full_count_check(ps, g, oracle_mod, "cosmo256")
     st = g["stats"]
     print(f"[stats] cosmo256 leaves={st['n_leaves']} leaf_pairs={st['n_leaf_pairs']} launches={st['launches']}")
     # NEXT row 1 at the full size: the exactness property of PAPER.md:141 holds at any size
@@ -332,6 +342,7 @@ def test_parity_config5_cosmo_large_full(oracle_mod):
     assert mom < TOL_INV and en < TOL_INV, (mom, en)
     del m, a3, v3, amag, work
     full = dict(V=V, rho=rho, nbr_count=cnt, A=A, B=B, gradA=gA, gradB=gB, ax=ax, ay=ay, az=az, dudt=du, pair_count=pc, gradv=gv)
+    _full_count_check(ps, dict(nbr_count=cnt.cpu().numpy(), pair_count=pc.cpu().numpy()), oracle_mod, "cosmo512")
     done = 0
     dens = int(np.argmin(ps.h))
     centres = [(0.5, 0.5, 0.5), (0.0005, 0.9995, 0.5), (float(ps.x[dens]), float(ps.y[dens]), float(ps.z[dens]))]

@@ -571,3 +571,24 @@ def test_next_row_constants_match_the_paper(oracle_mod):
         if Q > 0 and abs(vmax[i] ** 2 * rho[i] / Q - G["visc_sound_zeta"]) < 1e-9:
             found += 1
     assert found > 0
+
+
+# ---------------------------------------------------------------------------------------- oracle at scale: counts
+@pytest.mark.parametrize("name,n_side", [("tiny_uniform", 12), ("clustered", 16), ("cosmo", 16), ("blast_wave", 10)])
+def test_grid_counts_agree_bit_exactly_with_brute_force(name, n_side, oracle_mod):
+    """the grid formulation used for full-size count parity equals the O(N^2) scan on every particle"""
+    ps = wl.make_config(name, n_side)
+    if name == "clustered":
+        ps.h[:] = np.minimum(ps.h, 0.3)          # keep >= 3 cells per side
+    o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+    d = o.step_derivs(ps)
+    cg, cs = oracle_mod.grid_counts(ps)
+    assert np.array_equal(cg, d["nbr_count"]) and np.array_equal(cs, d["pair_count"])
+    assert cs.sum() >= cg.sum() > 0
+
+
+def test_grid_counts_refuses_boxes_with_too_few_cells(oracle_mod):
+    ps = wl.tiny_uniform(n_side=4)
+    ps.h[:] = 0.45
+    with pytest.raises(RuntimeError):
+        oracle_mod.grid_counts(ps)
