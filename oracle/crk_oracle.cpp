@@ -497,6 +497,71 @@ int crk_oracle_grid_counts(double box, int64_t n, const float* x, const float* y
     return 0;
 }
 
+// the same CSR neighbour structure as crk_oracle_build, found through the uniform grid of crk_oracle_grid_counts instead of
+// the O(N^2) scan (so that volumes .. hydro_derivs can run on a full 128^3 / 256^3 configuration).  Entries of a row are
+// sorted by j, which makes the structure identical to the brute-force one (pinned: tests/test_oracle_pins.py).
+int crk_oracle_build_grid(crk_oracle_ctx* c, int64_t n, const float* x, const float* y, const float* z, const float* h) {
+    if (!c || n < 0 || n >= (int64_t)IDX_MASK || (n > 0 && (!x || !y || !z || !h))) return -1;
+    set_threads();
+    const float L = (float)c->p.box, half = 0.5f * L;
+    float hmax = 0.0f;
+    for (int64_t i = 0; i < n; ++i) {
+        if (!(h[i] > 0.0f) || !(h[i] < half)) return -1;                                  // reading S13
+        if (!(x[i] >= 0.0f && x[i] < L && y[i] >= 0.0f && y[i] < L && z[i] >= 0.0f && z[i] < L)) return -1;
+        hmax = std::max(hmax, h[i]);
+    }
+    int nc = n > 0 ? (int)std::floor((double)L / ((double)hmax * 1.0001)) : 3;
+    nc = std::min(nc, 1024);
+    if (nc < 3) return -2;
+    c->n = n;
+    c->x.assign(x, x + n); c->y.assign(y, y + n); c->z.assign(z, z + n); c->h.assign(h, h + n);
+    const double inv = (double)nc / (double)L;
+    auto cell_of = [&](float p) { int q = (int)std::floor((double)p * inv); return q < 0 ? 0 : (q >= nc ? nc - 1 : q); };
+    const int64_t ncell = (int64_t)nc * nc * nc;
+    std::vector<int64_t> start((size_t)ncell + 1, 0), cid((size_t)n);
+    for (int64_t i = 0; i < n; ++i) {
+        cid[i] = ((int64_t)cell_of(x[i]) * nc + cell_of(y[i])) * nc + cell_of(z[i]);
+        ++start[cid[i] + 1];
+    }
+    for (int64_t q = 0; q < ncell; ++q) start[q + 1] += start[q];
+    std::vector<int64_t> fill(start.begin(), start.end() - 1), order((size_t)n);
+    for (int64_t i = 0; i < n; ++i) order[fill[cid[i]]++] = i;
+    c->off.assign((size_t)n + 1, 0);
+    for (int pass = 0; pass < 2; ++pass) {          // count, then fill
+        if (pass == 1) {
+            for (int64_t i = 0; i < n; ++i) c->off[i + 1] += c->off[i];
+            c->nbr.resize((size_t)c->off[n]);
+        }
+#pragma omp parallel for schedule(dynamic, 256)
+        for (int64_t i = 0; i < n; ++i) {
+            const float xi = x[i], yi = y[i], zi = z[i], hi2 = h[i] * h[i];
+            const int cx = cell_of(xi), cy = cell_of(yi), cz = cell_of(zi);
+            int64_t w = pass == 1 ? c->off[i] : 0;
+            for (int dx = -1; dx <= 1; ++dx)
+                for (int dy = -1; dy <= 1; ++dy)
+                    for (int dz = -1; dz <= 1; ++dz) {
+                        const int64_t q = ((int64_t)((cx + dx + nc) % nc) * nc + (cy + dy + nc) % nc) * nc + (cz + dz + nc) % nc;
+                        for (int64_t k = start[q]; k < start[q + 1]; ++k) {
+                            const int64_t j = order[k];
+                            if (j == i) continue;
+                            const float r2 = r2_f32(xi, yi, zi, x[j], y[j], z[j], L, half);
+                            uint32_t f = 0;
+                            if (r2 < hi2) f |= FLAG_I;
+                            if (r2 < h[j] * h[j]) f |= FLAG_J;
+                            if (!f) continue;
+                            if (pass == 0) ++w;
+                            else c->nbr[w++] = (uint32_t)j | f;
+                        }
+                    }
+            if (pass == 0) c->off[i + 1] = w;
+            else std::sort(c->nbr.begin() + c->off[i], c->nbr.begin() + w,
+                           [](uint32_t p, uint32_t q2) { return (p & IDX_MASK) < (q2 & IDX_MASK); });
+        }
+    }
+    c->stage = 1;
+    return 0;
+}
+
 // ---- NEXT row 2a: time-step criteria, Eqs. 46-50, a = 1, adot = 0, dy/dt = 1, no gravity ----------
 // Eq. 50 (sign garbled as printed; reading S17: the approach speed): v_sig,ij = max(-(v_ij . x_ij) / |x_ij|, 0),
 //   v_sig,i = max_j v_sig,ij over the pairs of the momentum sweep (r < max(h_i, h_j)).

@@ -68,6 +68,10 @@ int crk_oracle_pair_compat(crk_oracle_ctx* c, int64_t i, int64_t j, double dt, d
 int crk_oracle_grid_counts(double box, int64_t n, const float* x, const float* y, const float* z, const float* h,
                            uint32_t* nbr_count, uint32_t* pair_count);
 
+/* crk_oracle_build through the same uniform grid (identical neighbour structure, rows sorted by j): lets volumes ..
+ * hydro_derivs run on a full 128^3 / 256^3 configuration.  -2 if the box holds fewer than 3 cells per side.          */
+int crk_oracle_build_grid(crk_oracle_ctx* c, int64_t n, const float* x, const float* y, const float* z, const float* h);
+
 /* NEXT row 2a -- time-step criteria, Eqs. 46-50 with a = 1, adot = 0, no gravity, after
  * crk_oracle_hydro_derivs: dt_min = min(C_cfl hhat / max(v_sig, c_s, sqrt(4 Q_max / rho), hhat |Tr grad v|), sqrt(hhat / |a|)).
  * dt_hyd / dt_acc (nullable) return the two criteria separately.  Pinned: static gas closed form C hhat / c_s, linear

@@ -36,6 +36,7 @@ def lib():
         L.crk_oracle_set_threads.argtypes = [C.c_int]
         L.crk_oracle_get_threads.restype = C.c_int
         L.crk_oracle_build.argtypes = [C.c_void_p, C.c_int64, fp, fp, fp, fp]
+        L.crk_oracle_build_grid.argtypes = [C.c_void_p, C.c_int64, fp, fp, fp, fp]
         L.crk_oracle_volumes.argtypes = [C.c_void_p, fp, dp, dp, up]
         L.crk_oracle_rk_coefficients.argtypes = [C.c_void_p, dp, dp, dp, dp]
         L.crk_oracle_hydro_derivs.argtypes = [C.c_void_p, fp, fp, fp, fp, dp, dp, dp, dp, up]
@@ -105,10 +106,13 @@ class Oracle:
             lib().crk_oracle_destroy(self._c)
             self._c = None
 
-    def build(self, x, y, z, h):
+    def build(self, x, y, z, h, grid=False):
+        """grid=True: same neighbour structure through the uniform grid (oracle at scale) instead of the O(N^2) scan"""
         (x, px), (y, py), (z, pz), (h, ph) = _f(x), _f(y), _f(z), _f(h)
         self.n = x.shape[0]
-        rc = lib().crk_oracle_build(self._c, self.n, px, py, pz, ph)
+        rc = (lib().crk_oracle_build_grid if grid else lib().crk_oracle_build)(self._c, self.n, px, py, pz, ph)
+        if rc == -2:
+            raise RuntimeError("crk_oracle_build_grid: fewer than 3 cells per side (use the brute-force build)")
         if rc:
             raise ValueError("crk_oracle_build: bad input (h<=0, h>=L/2 or position outside [0,L))")
 
@@ -136,9 +140,9 @@ class Oracle:
         assert rc == 0
         return ax, ay, az, du, cnt
 
-    def step_derivs(self, ps):
+    def step_derivs(self, ps, grid=False):
         """ps: crk_workloads.ParticleSet (or anything with x,y,z,h,vx,vy,vz,m,u). Returns dict of all outputs."""
-        self.build(ps.x, ps.y, ps.z, ps.h)
+        self.build(ps.x, ps.y, ps.z, ps.h, grid=grid)
         V, rho, nbr = self.volumes(ps.m)
         A, B, gA, gB = self.rk_coefficients()
         ax, ay, az, du, pc = self.hydro_derivs(ps.vx, ps.vy, ps.vz, ps.u)

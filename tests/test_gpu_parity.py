@@ -560,3 +560,19 @@ def test_parity_non_default_parameters(oracle_mod):
     assert np.max(np.abs(dt_g.cpu().numpy()[fin] / dt_o[fin] - 1)) < TOL_DERIV
     assert rel_l2(du_c.cpu().numpy().astype(np.float64), o.compatible_energy(1e-4)) < TOL_DERIV
     print(f"[parity] non-default params n={ps.n}: dv/dt {e_a:.2e} du/dt {e_u:.2e} momentum {mom:.2e} energy {en:.2e}")
+
+
+def test_parity_config4_cosmo_every_particle(oracle_mod):
+    """BASELINE configs[3] (256^3, the bench workload): EVERY particle against the FP64 oracle run on the full
+    configuration through its grid neighbour search (bit-identical to the brute-force oracle, tests/test_oracle_pins.py)"""
+    ps = wl.make_config("cosmo")
+    o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+    od = o.step_derivs(ps, grid=True)
+    g = gpu_eval(ps)
+    e_a, e_u = check_parity(ps, g, od, oracle_gv=o.gradv(), label="cosmo256 all particles")
+    mom, en = check_invariants(ps, g, label="cosmo256 all particles")
+    a_o = np.stack([od["ax"], od["ay"], od["az"]]); a_g = np.stack([g["ax"], g["ay"], g["az"]]).astype(np.float64)
+    worst = np.sqrt(((a_g - a_o) ** 2).sum(0)).max() / np.sqrt((a_o ** 2).sum(0).mean())
+    print(f"[parity] cosmo256 all {ps.n} particles: dv/dt {e_a:.2e} du/dt {e_u:.2e} (worst particle {worst:.2e} of rms) "
+          f"momentum {mom:.2e} energy {en:.2e}")
+    assert worst < 1e-3

@@ -592,3 +592,13 @@ def test_grid_counts_refuses_boxes_with_too_few_cells(oracle_mod):
     ps.h[:] = 0.45
     with pytest.raises(RuntimeError):
         oracle_mod.grid_counts(ps)
+
+
+@pytest.mark.parametrize("name,n_side", [("tiny_uniform", 12), ("cosmo", 16)])
+def test_grid_build_gives_the_brute_force_results_bit_for_bit(name, n_side, oracle_mod):
+    """same neighbour rows in the same order => every output of the oracle is identical, not merely close"""
+    ps = wl.make_config(name, n_side)
+    a = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h).step_derivs(ps)
+    b = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h).step_derivs(ps, grid=True)
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k
