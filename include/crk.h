@@ -111,6 +111,11 @@ int  crk_compatible_energy(crk_ctx* c, float dt, float* delta_u);
  * a and udot from two full crk_step_derivs evaluations (udot = Eq. 18, reading S19).  Errors as
  * crk_step_derivs (CRK_ERANGE if the state leaves the admissible range).  The context is left in the state of the
  * second evaluation (predicted velocities), so crk_timestep / crk_compatible_energy afterwards refer to that state.   */
+/* CRK_FLAG_KDK_REUSE (crk_params.flags): consecutive crk_kdk_step calls on the same arrays reuse sort, tree, neighbour
+ * lists, volumes and RK coefficients of the previous step's second evaluation for their first one (same x, h, m).  Set it
+ * only if nothing but crk_kdk_step changes x, y, z, h, m between the calls; any crk_build_cells / crk_volumes /
+ * crk_rk_coefficients call in between drops the reuse.                                                              */
+#define CRK_FLAG_KDK_REUSE 2
 int  crk_kdk_step(crk_ctx* c, int64_t n, float* x, float* y, float* z, const float* h, float* vx, float* vy, float* vz,
                   const float* m, float* u, float dt);
 

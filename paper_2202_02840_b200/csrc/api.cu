@@ -73,6 +73,7 @@ const char* crk_last_error(const crk_ctx* c) { return c ? c->err : "null context
 int crk_build_cells(crk_ctx* c, int64_t n, const float* x, const float* y, const float* z, const float* h) {
     if (!c) return CRK_EINVAL;
     c->stage = 0;
+    c->kdk_valid = false;
     if (n < 0 || n >= (int64_t)1 << 31 || (n > 0 && (!x || !y || !z || !h))) {
         snprintf(c->err, sizeof(c->err), "crk_build_cells: null pointer or n out of range");
         return CRK_EINVAL;
@@ -101,6 +102,7 @@ int crk_build_cells(crk_ctx* c, int64_t n, const float* x, const float* y, const
 }
 
 int crk_volumes(crk_ctx* c, const float* m, float* V, float* rho, uint32_t* nbr_count) {
+    if (c) c->kdk_valid = false;   // crk_kdk_step sets it again at its end
     if (!c) return CRK_EINVAL;
     if (c->stage < 1) {
         snprintf(c->err, sizeof(c->err), "crk_volumes called before crk_build_cells");
@@ -117,6 +119,7 @@ int crk_volumes(crk_ctx* c, const float* m, float* V, float* rho, uint32_t* nbr_
 }
 
 int crk_rk_coefficients(crk_ctx* c, float* A, float* B, float* gradA, float* gradB) {
+    if (c) c->kdk_valid = false;   // crk_kdk_step sets it again at its end
     if (!c) return CRK_EINVAL;
     if (c->stage < 2) {
         snprintf(c->err, sizeof(c->err), "crk_rk_coefficients called before crk_volumes");
@@ -209,12 +212,22 @@ int crk_kdk_step(crk_ctx* c, int64_t n, float* x, float* y, float* z, const floa
     float* d = (float*)c->kdk.p;
     float* half = d + 4 * n;
     const unsigned grid = (unsigned)((n + 255) / 256);
-    CRK_TRY(crk_step_derivs(c, n, x, y, z, h, vx, vy, vz, m, u, d, d + n, d + 2 * n, d + 3 * n));
+    // The second evaluation of the previous step was made at the positions this step starts from (x^1 of step k = x^0 of step
+    // k+1), and sort, tree, neighbour lists, volumes and RK coefficients depend on x, h, m only: with CRK_FLAG_KDK_REUSE
+    // the first evaluation of a follow-up step is just the hydro sweeps on the corrected v, u (tree and
+    // interaction lists are built once and reused).
+    const bool reuse = (c->prm.flags & CRK_FLAG_KDK_REUSE) && c->kdk_valid && c->stage >= 3 && c->n == n && c->kdk_x == x &&
+                       c->kdk_y == y && c->kdk_z == z && c->kdk_h == h && c->kdk_m == m;
+    if (reuse) CRK_TRY(crk_hydro_derivs(c, vx, vy, vz, u, d, d + n, d + 2 * n, d + 3 * n, nullptr));
+    else CRK_TRY(crk_step_derivs(c, n, x, y, z, h, vx, vy, vz, m, u, d, d + n, d + 2 * n, d + 3 * n));
     k_kdk_predict<<<grid, 256, 0, c->stream>>>(n, c->prm.box, dt, x, y, z, vx, vy, vz, u, d, half);
     CRK_TRY(crk_check_launch(c, "k_kdk_predict"));
     CRK_TRY(crk_step_derivs(c, n, x, y, z, h, vx, vy, vz, m, u, d, d + n, d + 2 * n, d + 3 * n));
     k_kdk_correct<<<grid, 256, 0, c->stream>>>(n, dt, vx, vy, vz, u, d, half);
-    return crk_check_launch(c, "k_kdk_correct");
+    CRK_TRY(crk_check_launch(c, "k_kdk_correct"));
+    c->kdk_valid = true;
+    c->kdk_x = x; c->kdk_y = y; c->kdk_z = z; c->kdk_h = h; c->kdk_m = m;
+    return CRK_OK;
 }
 
 int crk_step_derivs_host(crk_ctx* c, int64_t n, const float* x, const float* y, const float* z, const float* h,

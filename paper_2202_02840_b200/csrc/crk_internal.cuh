@@ -46,6 +46,9 @@ struct crk_ctx {
     cudaStream_t stream = 0;
     cudaStream_t copy_stream = nullptr;      // crk_step_derivs_host: second H2D stream (created on first use)
     cudaEvent_t ev_copy = nullptr;
+    // crk_kdk_step with CRK_FLAG_KDK_REUSE: the arrays the last step's second evaluation was built for
+    bool kdk_valid = false;
+    const float *kdk_x = nullptr, *kdk_y = nullptr, *kdk_z = nullptr, *kdk_h = nullptr, *kdk_m = nullptr;
     int64_t n = 0, nl = 0;
     int stage = 0;                 // 0 none, 1 built, 2 volumes, 3 coefficients, 4 hydro
     char err[256];

@@ -478,9 +478,16 @@ def test_kdk_step_parity(name, n_side, dt, steps, oracle_mod):
     t = {k: torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).to(dev) for k in
          ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")}
     ctx = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h)
+    t2 = {k: v.clone() for k, v in t.items()}
     for _ in range(steps):
         ctx.kdk_step(*[t[k] for k in ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")], dt)
+    # CRK_FLAG_KDK_REUSE: follow-up steps reuse the build of the previous step's second evaluation: same bits
+    ctx2 = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h, kdk_reuse=True)
+    for _ in range(steps):
+        ctx2.kdk_step(*[t2[k] for k in ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")], dt)
     torch.cuda.synchronize()
+    for k in ("x", "y", "z", "vx", "vy", "vz", "u"):
+        assert torch.equal(t[k], t2[k]), f"{name} reuse changed {k}"
     g = {k: v.cpu().numpy().astype(np.float64) for k, v in t.items()}
     for k in ("x", "y", "z"):
         d = np.abs(g[k] - ref[k])
