@@ -382,14 +382,14 @@ int64_t crk_get_leaf_list(crk_ctx* c, int64_t leaf, uint32_t* host_buf, int64_t 
     if (!c || leaf < 0) return CRK_EINVAL;
     if (c->stage < 1) return CRK_ESTATE;
     if (leaf >= c->nl) return CRK_EINVAL;
-    uint32_t o[2];
-    if (cudaMemcpyAsync(o, (uint32_t*)c->nbr_off.p + leaf, 2 * sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
+    uint32_t o[1];
+    if (cudaMemcpyAsync(o, (uint32_t*)c->nbr_cnt.p + leaf, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
         return CRK_ECUDA;
     cudaStreamSynchronize(c->stream);
-    const int64_t cnt = (int64_t)o[1] - (int64_t)o[0];
+    const int64_t cnt = (int64_t)o[0];
     const int64_t ncopy = cnt < cap ? cnt : cap;
     if (ncopy > 0 && host_buf) {
-        if (cudaMemcpyAsync(host_buf, (uint32_t*)c->nbr_list.p + o[0], (size_t)ncopy * sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
+        if (cudaMemcpyAsync(host_buf, (uint32_t*)c->nbr_list.p + (size_t)leaf * (size_t)c->leaf_list_cap, (size_t)ncopy * sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
             return CRK_ECUDA;
         cudaStreamSynchronize(c->stream);
     }

@@ -72,7 +72,8 @@ struct crk_ctx {
     int n_levels = 0;
     int64_t level_off[CRK_MAX_LEVELS + 1];
     int64_t level_cnt[CRK_MAX_LEVELS + 1];
-    DevBuf nbr_cnt, nbr_off, nbr_list, nbr_gcnt;
+    DevBuf nbr_cnt, nbr_off, nbr_list, nbr_gcnt;   // leaf interaction list: leaf q owns nbr_list[q * leaf_list_cap ...], nbr_cnt[q] entries
+    int64_t leaf_list_cap = 0;
     int64_t n_pairs = 0, n_pairs_gather = 0;
     DevBuf arena, seg_first;       // neighbour-list arena (16-byte units); per leaf a uint4 copy of its first segment's header
     DevBuf leaf_cnt;               // u16[nl][64]: per-lane cnt_g | cnt of the first segment (dense, so the sweeps need no pointer chase)

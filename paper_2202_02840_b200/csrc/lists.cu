@@ -18,8 +18,9 @@ constexpr int LW = 2;   // warps (= leaves) per CTA
 struct ListArgs {
     int64_t n, nl;
     float L, half;
-    const uint32_t* __restrict__ off;
-    const uint32_t* __restrict__ list;
+    const uint32_t* __restrict__ cnt;      // entries of each leaf's interaction list
+    const uint32_t* __restrict__ list;     // leaf q owns list[q * cap ...]
+    uint32_t cap;
     const float4* __restrict__ posh;
     const float4* __restrict__ leaf_lo;
     const float4* __restrict__ leaf_hi;
@@ -176,7 +177,7 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
         __syncwarp();
     };
 
-    const uint32_t e0 = a.off[leaf], e1 = a.off[leaf + 1];
+    const uint64_t e0 = (uint64_t)leaf * a.cap, e1 = e0 + a.cnt[leaf];
     uint32_t ent = (e0 < e1) ? a.list[e0] : 0u;
     float4 pj = (e0 < e1) ? a.posh[(int64_t)(ent & CRK_LEAF_MASK) * CRK_LEAF + lane] : make_float4(0, 0, 0, 0);
     // the query leaf itself goes first and keeps all 32 particles: slots 0..31 of the first segment are the leaf's own
@@ -185,7 +186,7 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
     S.tidx[lane] = (uint32_t)i;
     fill = 32;
     flush(true);
-    for (uint32_t e = e0; e < e1; ++e) {
+    for (uint64_t e = e0; e < e1; ++e) {
         const uint32_t cur = ent;
         const float4 pc = pj;
         if (e + 1 < e1) {   // prefetch the next leaf's positions
@@ -236,7 +237,7 @@ int crk_build_nbr_lists(crk_ctx* c) {
     for (int attempt = 0; attempt < 3; ++attempt) {
         ListArgs a;
         a.n = c->n; a.nl = nl; a.L = c->prm.box; a.half = 0.5f * c->prm.box;
-        a.off = (const uint32_t*)c->nbr_off.p; a.list = (const uint32_t*)c->nbr_list.p;
+        a.cnt = (const uint32_t*)c->nbr_cnt.p; a.list = (const uint32_t*)c->nbr_list.p; a.cap = (uint32_t)c->leaf_list_cap;
         a.posh = (const float4*)c->posh.p; a.leaf_lo = (const float4*)c->leaf_lo.p; a.leaf_hi = (const float4*)c->leaf_hi.p;
         a.arena = (uint4*)c->arena.p;
         a.arena_cap = (unsigned long long)(c->arena.cap / 16);

@@ -60,12 +60,13 @@ __device__ __forceinline__ float axis_gap(float qlo, float qhi, float blo, float
 constexpr int NBR_WARPS = 8;
 constexpr int NBR_STACK = 32 * (CRK_MAX_LEVELS + 1);
 
-template <bool FILL>
+// One traversal per query leaf.  Leaf q owns slots [q * cap, (q + 1) * cap) of the list; entries beyond cap are counted but
+// not written, and the host re-runs the kernel with a larger cap if the largest count (atomicMax -> *max_cnt) exceeds it
+// (the capacity found is kept in the context, so later builds need one pass and no prefix sum).
 __global__ void __launch_bounds__(NBR_WARPS * 32) k_leaf_list(const float4* __restrict__ lo, const float4* __restrict__ hi,
-                                                              Levels lv, float L, uint32_t* __restrict__ cnt,
-                                                              uint32_t* __restrict__ gcnt,
-                                                              const uint32_t* __restrict__ off,
-                                                              uint32_t* __restrict__ list) {
+                                                              Levels lv, float L, uint32_t cap, uint32_t* __restrict__ cnt,
+                                                              uint32_t* __restrict__ gcnt, uint32_t* __restrict__ list,
+                                                              uint32_t* __restrict__ max_cnt) {
     __shared__ uint32_t stack[NBR_WARPS][NBR_STACK];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int64_t q = (int64_t)blockIdx.x * NBR_WARPS + w;
@@ -75,7 +76,7 @@ __global__ void __launch_bounds__(NBR_WARPS * 32) k_leaf_list(const float4* __re
     const float half = 0.5f * L;
     const uint32_t lt = (1u << lane) - 1u;
     uint32_t n_out = 0, n_gather = 0;
-    const uint32_t base = FILL ? off[q] : 0u;
+    const uint64_t base = (uint64_t)q * cap;
     int sp = 0;
     if (lane == 0) stack[w][0] = ((uint32_t)lv.n_levels << 28);   // pseudo-root: children = all nodes of the top level
     sp = 1;
@@ -100,9 +101,9 @@ __global__ void __launch_bounds__(NBR_WARPS * 32) k_leaf_list(const float4* __re
         const uint32_t m = __ballot_sync(0xffffffffu, pass);
         if (clev == 0) {
             const uint32_t mg = __ballot_sync(0xffffffffu, gather);
-            if (FILL && pass) {
-                const uint32_t pos = base + n_out + __popc(m & lt);
-                list[pos] = (uint32_t)child | (gather ? CRK_FLAG_GATHER : 0u) | (wrap ? CRK_FLAG_WRAP : 0u);
+            if (pass) {
+                const uint32_t pos = n_out + __popc(m & lt);
+                if (pos < cap) list[base + pos] = (uint32_t)child | (gather ? CRK_FLAG_GATHER : 0u) | (wrap ? CRK_FLAG_WRAP : 0u);
             }
             n_out += __popc(m);
             n_gather += __popc(mg);
@@ -113,9 +114,10 @@ __global__ void __launch_bounds__(NBR_WARPS * 32) k_leaf_list(const float4* __re
             __syncwarp();
         }
     }
-    if (!FILL && lane == 0) {
+    if (lane == 0) {
         cnt[q] = n_out;
         gcnt[q] = n_gather;
+        if (n_out > cap) atomicMax(max_cnt, n_out);
     }
 }
 
@@ -148,30 +150,41 @@ int crk_build_tree_and_list(crk_ctx* c) {
     const int64_t nl = c->nl;
     CRK_TRY(crk_ensure(c, c->nbr_cnt, (size_t)(nl + 1) * sizeof(uint32_t)));
     CRK_TRY(crk_ensure(c, c->nbr_gcnt, (size_t)(nl + 1) * sizeof(uint32_t)));
-    CRK_TRY(crk_ensure(c, c->nbr_off, (size_t)(nl + 2) * sizeof(uint32_t)));
     const unsigned grid = (unsigned)((nl + NBR_WARPS - 1) / NBR_WARPS);
-    k_leaf_list<false><<<grid, NBR_WARPS * 32, 0, c->stream>>>(lo, hi, lv, c->prm.box, (uint32_t*)c->nbr_cnt.p,
-                                                               (uint32_t*)c->nbr_gcnt.p, nullptr, nullptr);
-    CRK_TRY(crk_check_launch(c, "k_leaf_list<count>"));
-    CRK_TRY(crk_exclusive_scan_u32(c, (const uint32_t*)c->nbr_cnt.p, (uint32_t*)c->nbr_off.p, nl, c->scan_tmp));
-    // totals -> host (the one synchronisation of crk_build_cells): [1] = error flag, [2..3] = gather pair count
+    // totals -> host (one synchronisation): [0] = error flag of the sort, [1] = largest list, [2..3] = gather / all pair counts
+    uint32_t* d_max = (uint32_t*)c->flag.p + 1;
     unsigned long long* d_sum = (unsigned long long*)((int*)c->flag.p + 2);
-    k_sum_u32<<<148, 256, 0, c->stream>>>((const uint32_t*)c->nbr_gcnt.p, nl, d_sum);
-    CRK_TRY(crk_check_launch(c, "k_sum_u32"));
-    CRK_CUDA(c, cudaMemcpyAsync(c->h_flag, c->flag.p, 4 * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-    CRK_CUDA(c, cudaMemcpyAsync(c->h_flag + 4, (uint32_t*)c->nbr_off.p + nl, sizeof(uint32_t), cudaMemcpyDeviceToHost,
-                                c->stream));
-    CRK_CUDA(c, cudaStreamSynchronize(c->stream));
-    if (c->h_flag[0] & 1) {
-        snprintf(c->err, sizeof(c->err), "input out of range: need 0 <= x,y,z < box and 0 < h < box/2");
-        return CRK_ERANGE;
+    unsigned long long* d_sum2 = (unsigned long long*)((int*)c->flag.p + 4);
+    if (c->leaf_list_cap < 64) c->leaf_list_cap = 96;
+    for (int attempt = 0; attempt < 3; ++attempt) {
+        CRK_TRY(crk_ensure(c, c->nbr_list, ((size_t)nl * c->leaf_list_cap + 1) * sizeof(uint32_t)));
+        CRK_CUDA(c, cudaMemsetAsync(d_max, 0, 5 * sizeof(int), c->stream));
+        k_leaf_list<<<grid, NBR_WARPS * 32, 0, c->stream>>>(lo, hi, lv, c->prm.box, (uint32_t)c->leaf_list_cap,
+                                                            (uint32_t*)c->nbr_cnt.p, (uint32_t*)c->nbr_gcnt.p,
+                                                            (uint32_t*)c->nbr_list.p, d_max);
+        CRK_TRY(crk_check_launch(c, "k_leaf_list"));
+        k_sum_u32<<<148, 256, 0, c->stream>>>((const uint32_t*)c->nbr_gcnt.p, nl, d_sum);
+        CRK_TRY(crk_check_launch(c, "k_sum_u32"));
+        k_sum_u32<<<148, 256, 0, c->stream>>>((const uint32_t*)c->nbr_cnt.p, nl, d_sum2);
+        CRK_TRY(crk_check_launch(c, "k_sum_u32"));
+        CRK_CUDA(c, cudaMemcpyAsync(c->h_flag, c->flag.p, 6 * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        CRK_CUDA(c, cudaStreamSynchronize(c->stream));
+        if (c->h_flag[0] & 1) {
+            snprintf(c->err, sizeof(c->err), "input out of range: need 0 <= x,y,z < box and 0 < h < box/2");
+            return CRK_ERANGE;
+        }
+        const int64_t need = (int64_t)(uint32_t)c->h_flag[1];
+        if (need <= c->leaf_list_cap) break;
+        c->leaf_list_cap = (need + need / 8 + 31) & ~(int64_t)31;       // some head room for the next builds
+        if (attempt == 2) {
+            snprintf(c->err, sizeof(c->err), "leaf interaction list capacity did not converge");
+            return CRK_ECUDA;
+        }
     }
-    c->n_pairs = (int64_t)(uint32_t)c->h_flag[4];
-    unsigned long long g;
+    unsigned long long g, t;
     memcpy(&g, c->h_flag + 2, sizeof(g));
+    memcpy(&t, c->h_flag + 4, sizeof(t));
     c->n_pairs_gather = (int64_t)g;
-    CRK_TRY(crk_ensure(c, c->nbr_list, (size_t)(c->n_pairs + 1) * sizeof(uint32_t)));
-    k_leaf_list<true><<<grid, NBR_WARPS * 32, 0, c->stream>>>(lo, hi, lv, c->prm.box, nullptr, nullptr,
-                                                              (const uint32_t*)c->nbr_off.p, (uint32_t*)c->nbr_list.p);
-    return crk_check_launch(c, "k_leaf_list<fill>");
+    c->n_pairs = (int64_t)t;
+    return CRK_OK;
 }
