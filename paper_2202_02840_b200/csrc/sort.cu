@@ -4,6 +4,7 @@
 // locality is obtained by sorting on a 48-bit Hilbert key (16 bits per axis) and cutting the sorted sequence into
 // contiguous 32-particle leaves (tree.cu).  HBM-bound: every kernel here streams keys/payload once per pass.
 #include "crk_internal.cuh"
+#include <algorithm>
 
 namespace {
 
@@ -25,9 +26,9 @@ __device__ __forceinline__ uint64_t spread3(uint32_t v) {
     return x;
 }
 
-__device__ __forceinline__ uint64_t hilbert_key(uint32_t X0, uint32_t X1, uint32_t X2) {
-    const uint32_t M = 1u << (CRK_KEY_BITS - 1);
-#pragma unroll
+// b bits per axis -> 3 b-bit key (b <= 16)
+__device__ __forceinline__ uint64_t hilbert_key(uint32_t X0, uint32_t X1, uint32_t X2, int b) {
+    const uint32_t M = 1u << (b - 1);
     for (uint32_t Q = M; Q > 1; Q >>= 1) {
         const uint32_t P = Q - 1;
         // axis 0
@@ -42,39 +43,43 @@ __device__ __forceinline__ uint64_t hilbert_key(uint32_t X0, uint32_t X1, uint32
     X1 ^= X0;
     X2 ^= X1;
     uint32_t t = 0;
-#pragma unroll
     for (uint32_t Q = M; Q > 1; Q >>= 1)
         if (X2 & Q) t ^= Q - 1;
     X0 ^= t; X1 ^= t; X2 ^= t;
     return (spread3(X0) << 2) | (spread3(X1) << 1) | spread3(X2);
 }
 
-// validate (S13), key, and pack (x,y,z,h) so the later permutation gather moves 16-byte words
+// smallest support radius of the set -> flag[1] (encoded so that a zero-initialised atomicMax finds the minimum); it
+// decides how many key bits are worth computing and sorting (crk_sort_particles)
+__global__ void __launch_bounds__(256) k_h_min(const float* __restrict__ h, int64_t n, int* __restrict__ flag) {
+    uint32_t enc = 0u;
+    for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) {
+        const float hv = h[i];
+        if (hv > 0.f && hv < 3.0e38f) enc = max(enc, 0x7f800000u - __float_as_uint(hv));
+    }
+    enc = __reduce_max_sync(0xffffffffu, enc);
+    if ((threadIdx.x & 31) == 0 && enc != 0u) atomicMax((unsigned int*)flag + 1, enc);
+}
+
+// validate (S13), key (Hilbert index of the 2^bits grid), and pack (x,y,z,h) so the later permutation gather
+// moves 16-byte words
 __global__ void __launch_bounds__(256) k_keys_pack(const float* __restrict__ x, const float* __restrict__ y,
                                                    const float* __restrict__ z, const float* __restrict__ h,
-                                                   int64_t n, float L, uint64_t* __restrict__ keys,
+                                                   int64_t n, float L, int bits, uint64_t* __restrict__ keys,
                                                    uint32_t* __restrict__ vals, float4* __restrict__ posh_orig,
                                                    int* __restrict__ flag) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    // smallest support radius of the set -> flag[1] (encoded so that a zero-initialised atomicMax finds the minimum);
-    // it decides how many key bits are worth sorting (crk_sort_particles)
-    {
-        const float hv = (i < n) ? h[i] : 3.0e38f;
-        uint32_t enc = (hv > 0.f && hv < 3.0e38f) ? 0x7f800000u - __float_as_uint(hv) : 0u;
-        enc = __reduce_max_sync(0xffffffffu, enc);
-        if ((threadIdx.x & 31) == 0 && enc != 0u) atomicMax((unsigned int*)flag + 1, enc);
-    }
     if (i >= n) return;
     const float xi = x[i], yi = y[i], zi = z[i], hi = h[i];
     const bool ok = (xi >= 0.f) && (xi < L) && (yi >= 0.f) && (yi < L) && (zi >= 0.f) && (zi < L) && (hi > 0.f) &&
                     (hi < 0.5f * L);
     if (!ok) atomicOr(flag, 1);
-    const float s = (float)(1u << CRK_KEY_BITS) / L;
-    const uint32_t cmax = (1u << CRK_KEY_BITS) - 1u;
+    const float s = (float)(1u << bits) / L;
+    const uint32_t cmax = (1u << bits) - 1u;
     const uint32_t ix = min((uint32_t)fmaxf(xi * s, 0.f), cmax);
     const uint32_t iy = min((uint32_t)fmaxf(yi * s, 0.f), cmax);
     const uint32_t iz = min((uint32_t)fmaxf(zi * s, 0.f), cmax);
-    keys[i] = hilbert_key(ix, iy, iz);
+    keys[i] = hilbert_key(ix, iy, iz, bits);
     vals[i] = (uint32_t)i;
     posh_orig[i] = make_float4(xi, yi, zi, hi);
 }
@@ -328,13 +333,11 @@ int crk_sort_particles(crk_ctx* c, const float* x, const float* y, const float* 
     uint32_t* offs = hist + (size_t)RADIX * nblk + 1;
 
     CRK_CUDA(c, cudaMemsetAsync(c->flag.p, 0, 4 * sizeof(int), c->stream));
-    k_keys_pack<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(x, y, z, h, n, c->prm.box, (uint64_t*)c->keys[0].p,
-                                                                    (uint32_t*)c->vals[0].p, (float4*)c->posh_orig.p,
-                                                                    (int*)c->flag.p);
-    CRK_TRY(crk_check_launch(c, "k_keys_pack"));
+    k_h_min<<<(unsigned)std::min<int64_t>((n + 255) / 256, 1184), 256, 0, c->stream>>>(h, n, (int*)c->flag.p);
+    CRK_TRY(crk_check_launch(c, "k_h_min"));
     // Key bits worth sorting: cells of half the smallest support radius order everything the leaves need (a finer
     // order inside such a cell does not make a 32-particle leaf more compact than its h).  The top 3 b bits of a Hilbert
-    // key are the key of the b-bit grid, so the low passes are simply skipped.  One 4-byte read-back (h_min).
+    // key are the key of the b-bit grid, so only b levels of the curve are computed and sorted.  One 4-byte read-back (h_min).
     CRK_CUDA(c, cudaMemcpyAsync(c->h_flag + 12, (int*)c->flag.p + 1, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     CRK_CUDA(c, cudaStreamSynchronize(c->stream));
     int bits = CRK_KEY_BITS;
@@ -352,10 +355,14 @@ int crk_sort_particles(crk_ctx* c, const float* x, const float* y, const float* 
         }
         if (bits < 6) bits = 6;
     }
+    k_keys_pack<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(x, y, z, h, n, c->prm.box, bits, (uint64_t*)c->keys[0].p,
+                                                                    (uint32_t*)c->vals[0].p, (float4*)c->posh_orig.p,
+                                                                    (int*)c->flag.p);
+    CRK_TRY(crk_check_launch(c, "k_keys_pack"));
     CRK_CUDA(c, cudaFuncSetAttribute(k_radix_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ScatterSmem)));
     int cur = 0;
     c->st.sort_passes = (3 * bits + RADIX_BITS - 1) / RADIX_BITS;
-    for (int shift = 3 * (CRK_KEY_BITS - bits); shift < 3 * CRK_KEY_BITS; shift += RADIX_BITS) {
+    for (int shift = 0; shift < 3 * bits; shift += RADIX_BITS) {
         k_radix_hist<<<nblk, SORT_THREADS, 0, c->stream>>>((const uint64_t*)c->keys[cur].p, n, shift, hist, nblk);
         CRK_TRY(crk_check_launch(c, "k_radix_hist"));
         CRK_TRY(crk_exclusive_scan_u32(c, hist, offs, (int64_t)RADIX * nblk, c->scan_tmp));
