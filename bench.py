@@ -36,7 +36,7 @@ UNIT = "pair-interactions/s"
 FLOPS_PER_PAIR = {"volumes": 16.0, "moments": 100.0, "gradv": 90.0, "forces": 250.0}
 FP32_PEAK_THEORETICAL = 148 * 128 * 2 * 1.965e9     # SMs x FP32 lanes x 2 (FMA) x max SM clock
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_forces launch on the default workload (cosmo 256^3), from the
-# ncu --set full capture summarised in profiles/r01_sweeps_v8_ncu_full.md; other workloads report null
+# ncu --set full capture summarised in profiles/r01_sweeps_v9_ncu_full.md; other workloads report null
 FORCES_DRAM_BYTES_COSMO256 = 6.10e9 + 0.27e9
 
 

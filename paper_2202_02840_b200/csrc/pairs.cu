@@ -660,7 +660,7 @@ __device__ __forceinline__ PairF force_pair(const ForceConst& k, const PState& I
 // One CTA = one leaf: W5_WPL warps share the tile of the leaf's candidates and split each lane's entries by rows; four
 // CTAs are resident per SM, so one CTA's staging (header -> candidates -> state, three dependent global loads) overlaps the
 // other three's pair math.  (A persistent, double-buffered variant with 2 x 8 warps per SM was measured slower: 13.1 vs
-// 11.7 ms -- its per-leaf barrier couples all warps of the SM half; profiles/r01_sweeps_v8_ncu_full.md.)
+// 11.7 ms -- its per-leaf barrier couples all warps of the SM half; profiles/r01_sweeps_v9_ncu_full.md.)
 constexpr int W5_WPL = 4;
 template <bool TS>   // TS: also reduce the per-particle maxima the time-step criteria need (Eqs. 46, 50)
 __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
