@@ -631,16 +631,20 @@ int crk_oracle_evolve_h(crk_oracle_ctx* c, double* h_new) {
 // are cooled", f_ij + f_ji = 1).  Reading S16: if either entropy is not positive (u <= 0, config 2's unstable steps),
 // f_ij = 1/2.   Eq. 19: Delta u_i = sum_j du_ij dt.
 struct CompatOut { double du, dE, f; };
-inline void pair_compat(const crk_oracle_ctx* c, int64_t i, int64_t j, double dt, CompatOut& o) {
+// kick = optional [3][n] array: the velocity change of each particle over the kick, v' - v, with v the velocities of the last
+// crk_oracle_hydro_derivs.  nullptr: Eq. 22 as printed, v' - v = (dv/dt) dt.
+inline void pair_compat(const crk_oracle_ctx* c, int64_t i, int64_t j, double dt, CompatOut& o, const double* kick = nullptr) {
     PairOut po;
     pair_term(c, i, j, po);                                   // po.F = m_i a_ij
     const double im = 1.0 / c->m[i];
     const double aij[3] = {po.F[0] * im, po.F[1] * im, po.F[2] * im};
     const double vi[3] = {c->vx[i], c->vy[i], c->vz[i]}, vj[3] = {c->vx[j], c->vy[j], c->vz[j]};
     const double ai[3] = {c->ax[i], c->ay[i], c->az[i]}, aj[3] = {c->ax[j], c->ay[j], c->az[j]};
+    const int64_t n = c->n;
     double w = 0.0;
     for (int q = 0; q < 3; ++q) {
-        const double vpi = vi[q] + ai[q] * dt, vpj = vj[q] + aj[q] * dt;          // Eq. 22
+        const double vpi = vi[q] + (kick ? kick[q * n + i] : ai[q] * dt);         // Eq. 22
+        const double vpj = vj[q] + (kick ? kick[q * n + j] : aj[q] * dt);
         w += (vj[q] + vpj - vi[q] - vpi) * aij[q];
     }
     o.dE = 0.5 * c->m[i] * w;                                                     // Eq. 21
@@ -668,6 +672,27 @@ int crk_oracle_compatible_energy(crk_oracle_ctx* c, double dt, double* delta_u) 
             s += o.du;
         }
         delta_u[i] = s * dt;                                                      // Eq. 19 with adot = 0
+    }
+    return 0;
+}
+
+// Eqs. 19-21, 23 for a kick whose velocity change v' - v is given per particle (kick[3][n]) instead of Eq. 22's (dv/dt) dt:
+// what the velocity-Verlet step needs, where the second half kick starts from v^1/2 while the derivatives were taken at
+// the predicted velocities (crk_oracle.py:kdk_steps).  Reduces to crk_oracle_compatible_energy for kick = (dv/dt) dt.
+// (v and v' enter only through v + v' = 2 v + kick, so a kick that starts from v - delta is passed as kick - 2 delta.)
+int crk_oracle_compatible_energy_kick(crk_oracle_ctx* c, double dt, const double* kick, double* delta_u) {
+    if (!c || c->stage < 4 || !delta_u || !kick) return -1;
+    set_threads();
+    const int64_t n = c->n;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t i = 0; i < n; ++i) {
+        double s = 0.0;
+        for (int64_t k = c->off[i]; k < c->off[i + 1]; ++k) {
+            CompatOut o;
+            pair_compat(c, i, (int64_t)(c->nbr[k] & IDX_MASK), dt, o, kick);
+            s += o.du;
+        }
+        delta_u[i] = s * dt;
     }
     return 0;
 }

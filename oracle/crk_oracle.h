@@ -58,6 +58,10 @@ int crk_oracle_step_derivs(crk_oracle_ctx* c, int64_t n, const float* x, const f
  * Pinned: sum_i m_i delta_u_i + Delta KE = 0 to roundoff, f_ij + f_ji = 1, the heating/cooling rule of PAPER.md:141.
  * PARITY UNPINNED: the exact form of the garbled Eq. 23 (reading G1) and f = 1/2 for s <= 0 (S16).      */
 int crk_oracle_compatible_energy(crk_oracle_ctx* c, double dt, double* delta_u);
+/* the same for a kick with a given velocity change per particle, kick[3][n] = v' - v (v = velocities of the last
+ * hydro_derivs): delta_u[i] = dt * sum_j (f_ij/2) (2 (v_j - v_i) + kick_j - kick_i) . a_ij.  Pinned: equals the call above
+ * for kick = (dv/dt) dt; makes the Verlet step of crk_oracle.py:kdk_steps(compatible=True) conserve energy to roundoff.   */
+int crk_oracle_compatible_energy_kick(crk_oracle_ctx* c, double dt, const double* kick, double* delta_u);
 /* one pair of the above: out = { du_ij (Eq. 20), dE_ij (Eq. 21), f_ij (Eq. 23) }                                 */
 int crk_oracle_pair_compat(crk_oracle_ctx* c, int64_t i, int64_t j, double dt, double out[3]);
 

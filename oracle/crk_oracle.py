@@ -51,6 +51,7 @@ def lib():
         L.crk_oracle_pair_term.argtypes = [C.c_void_p, C.c_int64, C.c_int64, dp]
         L.crk_oracle_pair_visc.argtypes = [C.c_void_p, C.c_int64, C.c_int64, dp]
         L.crk_oracle_compatible_energy.argtypes = [C.c_void_p, C.c_double, dp]
+        L.crk_oracle_compatible_energy_kick.argtypes = [C.c_void_p, C.c_double, dp, dp]
         L.crk_oracle_evolve_h.argtypes = [C.c_void_p, dp]
         L.crk_oracle_grid_counts.argtypes = [C.c_double, C.c_int64, fp, fp, fp, fp, up, up]
         L.crk_oracle_timestep.argtypes = [C.c_void_p, C.c_double, dp, dp, dp]
@@ -167,6 +168,14 @@ class Oracle:
         assert lib().crk_oracle_compatible_energy(self._c, float(dt), _d(du)) == 0
         return du
 
+    def compatible_energy_kick(self, dt, kick):
+        """Eqs. 19-21, 23 for a kick with velocity change kick[3][n] = v' - v over dt (v = velocities of the last hydro_derivs)"""
+        kick = np.ascontiguousarray(kick, dtype=np.float64)
+        assert kick.shape == (3, self.n)
+        du = np.empty(self.n)
+        assert lib().crk_oracle_compatible_energy_kick(self._c, float(dt), _d(kick), _d(du)) == 0
+        return du
+
     def pair_compat(self, i, j, dt):
         out = np.empty(3)
         assert lib().crk_oracle_pair_compat(self._c, int(i), int(j), float(dt), _d(out)) == 0
@@ -252,7 +261,7 @@ def _f32_state(ps, st, L):
     return cur
 
 
-def kdk_steps(ps, n_steps: int, dt: float, oracle: Oracle | None = None):
+def kdk_steps(ps, n_steps: int, dt: float, oracle: Oracle | None = None, compatible: bool = False):
     """NEXT row 2b: the hydro-only velocity-Verlet operator U_V of Eq. 43 with a = 1, dt/dy = 1,
     p = v, in FP64 on the oracle's derivatives (each evaluation sees the float32 cast of the state, like the library):
         v^1/2 = v^0 + (1/2) a(x^0, v^0, u^0) dt          u^1/2 = u^0 + (1/2) udot(x^0, v^0, u^0) dt
@@ -260,6 +269,10 @@ def kdk_steps(ps, n_steps: int, dt: float, oracle: Oracle | None = None):
         v_p   = v^1/2 + (1/2) a(x^0, v^0, u^0) dt        u_p   = u^1/2 + (1/2) udot(x^0, v^0, u^0) dt     (predictions)
         v^1   = v^1/2 + (1/2) a(x^1, v_p, u_p) dt        u^1   = u^1/2 + (1/2) udot(x^1, v_p, u_p) dt
     Reading S19: the "Delta u" of Eq. 43 is taken as (du/dt of Eq. 18) dt.  h and m stay fixed.
+    compatible=True (reading S20): the two half kicks use the compatible energy of Eqs. 19-23 instead, each for its own
+    velocity change: Delta u_1 for v^0 -> v^1/2 with the pair accelerations of the first evaluation, Delta u_2 for
+    v^1/2 -> v^1 with those of the second (which was taken at v_p = v^1/2 + a^0 dt/2, so relative to that state the kick
+    v^1/2 + v^1 = 2 v_p + (a^1 dt/2 - a^0 dt)); u_p = u^1/2 + Delta u_1.  Total energy is then conserved to roundoff.
     Returns the FP64 state dict after n_steps."""
     o = oracle or Oracle(ps.box, ps.gamma, ps.n_h)
     st = {k: np.asarray(getattr(ps, k), dtype=np.float64).copy() for k in ("x", "y", "z", "vx", "vy", "vz", "u")}
@@ -268,18 +281,26 @@ def kdk_steps(ps, n_steps: int, dt: float, oracle: Oracle | None = None):
     for _ in range(n_steps):
         d0 = o.step_derivs(_f32_state(ps, st, L))
         half = {v: st[v] + 0.5 * d0[a] * dt for _, v, a in ax}
-        u_half = st["u"] + 0.5 * d0["dudt"] * dt
+        if compatible:
+            du1 = o.compatible_energy_kick(0.5 * dt, np.stack([0.5 * dt * d0[a] for _, _, a in ax]))
+        else:
+            du1 = 0.5 * d0["dudt"] * dt
+        u_half = st["u"] + du1
         pred = dict(st)
         for k, v, a in ax:
             p = st[k] + half[v] * dt
             pred[k] = p - np.floor(p / L) * L
             pred[v] = half[v] + 0.5 * d0[a] * dt
-        pred["u"] = u_half + 0.5 * d0["dudt"] * dt
+        pred["u"] = u_half + du1
         d1 = o.step_derivs(_f32_state(ps, pred, L))
         for k, v, a in ax:
             st[k] = pred[k]
             st[v] = half[v] + 0.5 * d1[a] * dt
-        st["u"] = u_half + 0.5 * d1["dudt"] * dt
+        if compatible:
+            du2 = o.compatible_energy_kick(0.5 * dt, np.stack([0.5 * dt * d1[a] - dt * d0[a] for _, _, a in ax]))
+        else:
+            du2 = 0.5 * d1["dudt"] * dt
+        st["u"] = u_half + du2
     return st
 
 

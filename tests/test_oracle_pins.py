@@ -602,3 +602,27 @@ def test_grid_build_gives_the_brute_force_results_bit_for_bit(name, n_side, orac
     b = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h).step_derivs(ps, grid=True)
     for k in a:
         assert np.array_equal(a[k], b[k]), k
+
+
+# ---------------------------------------------------------------------------------------- Verlet step with compatible energy
+def test_compatible_kick_reduces_to_eq22_and_kdk_conserves_energy(oracle_mod):
+    """(i) kick = (dv/dt) dt reproduces Eqs. 19-23 as printed.  (ii) The Verlet step with the compatible energy for each
+    half kick conserves sum m (u + v^2/2) to roundoff -- the point of the formalism -- while the same
+    steps with Eq. 18's rate drift at O(dt^2)."""
+    ps = wl.tiny_uniform(n_side=8)
+    o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+    d = o.step_derivs(ps)
+    dt = 3e-3
+    a = np.stack([d["ax"], d["ay"], d["az"]])
+    assert np.allclose(o.compatible_energy_kick(dt, a * dt), o.compatible_energy(dt), rtol=1e-13, atol=1e-300)
+    m = ps.m.astype(np.float64)
+
+    def energy(st):
+        return (m * (st["u"] + 0.5 * (st["vx"] ** 2 + st["vy"] ** 2 + st["vz"] ** 2))).sum()
+
+    e0 = energy({k: np.asarray(getattr(ps, k), dtype=np.float64) for k in ("u", "vx", "vy", "vz")})
+    ec = energy(oracle_mod.kdk_steps(ps, 4, 4e-3, o, compatible=True))
+    ep = energy(oracle_mod.kdk_steps(ps, 4, 4e-3, o, compatible=False))
+    # the derivative evaluations see the float32 cast of v, so "roundoff" is float32 roundoff of the velocities
+    assert abs(ec / e0 - 1) < 2e-8, ec / e0 - 1
+    assert abs(ep / e0 - 1) > 20 * abs(ec / e0 - 1)
