@@ -116,6 +116,10 @@ int  crk_compatible_energy(crk_ctx* c, float dt, float* delta_u);
  * only if nothing but crk_kdk_step changes x, y, z, h, m between the calls; any crk_build_cells / crk_volumes /
  * crk_rk_coefficients call in between drops the reuse.                                                              */
 #define CRK_FLAG_KDK_REUSE 2
+/* CRK_FLAG_KDK_COMPATIBLE: the two half kicks of crk_kdk_step advance u with the compatible energy of Eqs. 19-23 (each for
+ * its own velocity change and pair accelerations, reading S20) instead of Eq. 18's rate: total energy is then
+ * conserved to roundoff -- the paper's fiducial energy integration.  Two more pair sweeps per step.     */
+#define CRK_FLAG_KDK_COMPATIBLE 4
 int  crk_kdk_step(crk_ctx* c, int64_t n, float* x, float* y, float* z, const float* h, float* vx, float* vy, float* vz,
                   const float* m, float* u, float dt);
 

@@ -54,7 +54,7 @@ void crk_destroy(crk_ctx* c) {
     DevBuf* bufs[] = {&c->keys[0], &c->keys[1], &c->vals[0], &c->vals[1], &c->hist, &c->scan_tmp, &c->posh_orig,
                       &c->posh, &c->leaf_lo, &c->leaf_hi, &c->nbr_cnt, &c->nbr_off, &c->nbr_list, &c->nbr_gcnt,
                       &c->posV, &c->rho_s, &c->coef, &c->fst, &c->u_s, &c->vel_orig, &c->m_s, &c->flag,
-                      &c->host_stage, &c->arena, &c->seg_first, &c->leaf_cnt, &c->ts_s, &c->kdk};
+                      &c->host_stage, &c->arena, &c->seg_first, &c->leaf_cnt, &c->ts_s, &c->kdk, &c->kick};
     for (DevBuf* b : bufs)
         if (b->p) cudaFree(b->p);
     if (c->h_flag) cudaFreeHost(c->h_flag);
@@ -167,7 +167,8 @@ __global__ void __launch_bounds__(256) k_kdk_predict(int64_t n, float L, float d
                                                      float* __restrict__ z, float* __restrict__ vx, float* __restrict__ vy,
                                                      float* __restrict__ vz, float* __restrict__ u,
                                                      const float* __restrict__ d /* [4][n]: a, udot */,
-                                                     float* __restrict__ half /* [4][n]: v^1/2, u^1/2 */) {
+                                                     float* __restrict__ half /* [4][n]: v^1/2, u^1/2 */,
+                                                     const float* __restrict__ du_half /* compatible Delta u_1 or null */) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const float hd = 0.5f * dt;
@@ -184,22 +185,23 @@ __global__ void __launch_bounds__(256) k_kdk_predict(int64_t n, float L, float d
         pos[q][i] = p;
         vel[q][i] = fmaf(a, hd, vh);
     }
-    const float ud = d[3 * n + i];
-    const float uh = fmaf(ud, hd, u[i]);
+    const float inc = du_half ? du_half[i] : d[3 * n + i] * hd;
+    const float uh = u[i] + inc;
     half[3 * n + i] = uh;
-    u[i] = fmaf(ud, hd, uh);
+    u[i] = uh + inc;
 }
 // v^1 = v^1/2 + a(x^1, v_p, u_p) dt/2, u^1 likewise
 __global__ void __launch_bounds__(256) k_kdk_correct(int64_t n, float dt, float* __restrict__ vx, float* __restrict__ vy,
                                                      float* __restrict__ vz, float* __restrict__ u,
-                                                     const float* __restrict__ d, const float* __restrict__ half) {
+                                                     const float* __restrict__ d, const float* __restrict__ half,
+                                                     const float* __restrict__ du_half) {
     const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
     const float hd = 0.5f * dt;
     vx[i] = fmaf(d[i], hd, half[i]);
     vy[i] = fmaf(d[n + i], hd, half[n + i]);
     vz[i] = fmaf(d[2 * n + i], hd, half[2 * n + i]);
-    u[i] = fmaf(d[3 * n + i], hd, half[3 * n + i]);
+    u[i] = half[3 * n + i] + (du_half ? du_half[i] : d[3 * n + i] * hd);
 }
 }  // namespace
 
@@ -208,9 +210,12 @@ int crk_kdk_step(crk_ctx* c, int64_t n, float* x, float* y, float* z, const floa
     if (!c || n < 0 || !(dt == dt)) return CRK_EINVAL;
     if (n == 0) return CRK_OK;
     if (!x || !y || !z || !h || !vx || !vy || !vz || !m || !u) return CRK_EINVAL;
-    CRK_TRY(crk_ensure(c, c->kdk, (size_t)8 * n * sizeof(float)));
+    CRK_TRY(crk_ensure(c, c->kdk, (size_t)12 * n * sizeof(float)));
     float* d = (float*)c->kdk.p;
     float* half = d + 4 * n;
+    float* a0 = d + 8 * n;                 // [3][n] accelerations of the first evaluation, [n] compatible Delta u
+    float* duc = d + 11 * n;
+    const bool compat = (c->prm.flags & CRK_FLAG_KDK_COMPATIBLE) != 0;
     const unsigned grid = (unsigned)((n + 255) / 256);
     // The second evaluation of the previous step was made at the positions this step starts from (x^1 of step k = x^0 of step
     // k+1), and sort, tree, neighbour lists, volumes and RK coefficients depend on x, h, m only: with CRK_FLAG_KDK_REUSE
@@ -220,10 +225,16 @@ int crk_kdk_step(crk_ctx* c, int64_t n, float* x, float* y, float* z, const floa
                        c->kdk_y == y && c->kdk_z == z && c->kdk_h == h && c->kdk_m == m;
     if (reuse) CRK_TRY(crk_hydro_derivs(c, vx, vy, vz, u, d, d + n, d + 2 * n, d + 3 * n, nullptr));
     else CRK_TRY(crk_step_derivs(c, n, x, y, z, h, vx, vy, vz, m, u, d, d + n, d + 2 * n, d + 3 * n));
-    k_kdk_predict<<<grid, 256, 0, c->stream>>>(n, c->prm.box, dt, x, y, z, vx, vy, vz, u, d, half);
+    if (compat) {   // Delta u_1: the half kick v^0 -> v^1/2 with the pair accelerations of this evaluation (reading S20)
+        CRK_TRY(crk_launch_compat(c, 0.5f * dt, 0.5f * dt, 0.0f, nullptr, nullptr, nullptr, duc));
+        CRK_CUDA(c, cudaMemcpyAsync(a0, d, (size_t)3 * n * sizeof(float), cudaMemcpyDeviceToDevice, c->stream));
+    }
+    k_kdk_predict<<<grid, 256, 0, c->stream>>>(n, c->prm.box, dt, x, y, z, vx, vy, vz, u, d, half, compat ? duc : nullptr);
     CRK_TRY(crk_check_launch(c, "k_kdk_predict"));
     CRK_TRY(crk_step_derivs(c, n, x, y, z, h, vx, vy, vz, m, u, d, d + n, d + 2 * n, d + 3 * n));
-    k_kdk_correct<<<grid, 256, 0, c->stream>>>(n, dt, vx, vy, vz, u, d, half);
+    if (compat)     // Delta u_2: v^1/2 -> v^1; the state holds v_p = v^1/2 + a^0 dt/2, so v^1/2 + v^1 = 2 v_p + (a^1 dt/2 - a^0 dt)
+        CRK_TRY(crk_launch_compat(c, 0.5f * dt, 0.5f * dt, -dt, a0, a0 + n, a0 + 2 * n, duc));
+    k_kdk_correct<<<grid, 256, 0, c->stream>>>(n, dt, vx, vy, vz, u, d, half, compat ? duc : nullptr);
     CRK_TRY(crk_check_launch(c, "k_kdk_correct"));
     c->kdk_valid = true;
     c->kdk_x = x; c->kdk_y = y; c->kdk_z = z; c->kdk_h = h; c->kdk_m = m;
@@ -306,7 +317,7 @@ int crk_compatible_energy(crk_ctx* c, float dt, float* delta_u) {
         return CRK_ESTATE;
     }
     if (c->n == 0) return CRK_OK;
-    return crk_launch_compat(c, dt, delta_u);
+    return crk_launch_compat(c, dt, dt, 0.0f, nullptr, nullptr, nullptr, delta_u);
 }
 
 int crk_get_leaf_segments(crk_ctx* c, uint32_t* seg) {

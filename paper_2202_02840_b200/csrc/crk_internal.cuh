@@ -84,6 +84,7 @@ struct crk_ctx {
     DevBuf coef;                   // 4 planes float4[n]: (A,Bx,By,Bz) (cx,cy,cz,M00) (M01,M02,M10,M11) (M12,M20,M21,M22)
     DevBuf fst;                    // force-sweep state, 9 planes float4[np] (layout at k_gradv in pairs.cu) + plane 9 = (dv/dt, s)
     DevBuf ts_s;                   // float2 (max approach speed, max Q_i), sorted; only with CRK_FLAG_TIMESTEP
+    DevBuf kick;                   // compatible-energy sweep: (v' - v, s) per particle, sorted
     DevBuf kdk;                    // crk_kdk_step scratch: derivatives [4][n] and half-step state [4][n]
     DevBuf u_s;                    // float, specific internal energy in sorted order
     DevBuf vel_orig;               // float4 (vx,vy,vz,u) caller order (packed for a 16-byte gather)
@@ -156,4 +157,5 @@ int crk_launch_hydro(crk_ctx* c, const float* vx, const float* vy, const float* 
 int crk_launch_gradv_full(crk_ctx* c, float* gradv);
 int crk_launch_timestep(crk_ctx* c, float C_cfl, float* dt_min);                                       // pairs.cu
 int crk_launch_evolve_h(crk_ctx* c, float* h_new);                                                    // pairs.cu
-int crk_launch_compat(crk_ctx* c, float dt, float* delta_u);                                          // pairs.cu                                                  // pairs.cu
+int crk_launch_compat(crk_ctx* c, float dt, float c1, float c0, const float* bx, const float* by, const float* bz,
+                      float* delta_u);                                          // pairs.cu                                                  // pairs.cu

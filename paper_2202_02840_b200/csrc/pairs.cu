@@ -710,7 +710,25 @@ __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
 // sign(dE_ij) = sign(m_i a_ij . (v_j + v'_j - v_i - v'_i)) (Eq. 21, independent of f); Eq. 23 per DESIGN.md reading G1;
 // f = 1/2 if an entropy is not positive (S16).  Both lanes of a pair form bit-identical F and velocity sums, so they take
 // the same branch of Eq. 23 and f_ij + f_ji = 1 up to the rounding of the reciprocal.
-__global__ void __launch_bounds__(W5_WPL * 32, 4) k_compat(SweepArgs a, float dt) {
+// kick plane: (v' - v, s) per particle, sorted order.  Eq. 22 as printed: v' - v = (dv/dt) dt (c1 = dt, no b).  The Verlet step's
+// second half kick starts from v^1/2 while the sweep state holds the predicted velocities v_p = v^1/2 + a^0 dt/2, so there
+// v^1/2 + v^1 = 2 v_p + (a^1 dt/2 - a^0 dt): c1 = dt/2 on the resident dv/dt, c0 = -dt on b = a^0 (caller order).
+__global__ void __launch_bounds__(256) k_compat_prep(const float4* __restrict__ acc_s, const int32_t* __restrict__ perm, int64_t n,
+                                                     int64_t np, float c1, float c0, const float* __restrict__ bx,
+                                                     const float* __restrict__ by, const float* __restrict__ bz,
+                                                     float4* __restrict__ kick) {
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= np) return;
+    const float4 q = acc_s[k];
+    float4 w = make_float4(c1 * q.x, c1 * q.y, c1 * q.z, q.w);
+    if (bx && k < n) {
+        const int32_t p = perm[k];
+        w.x = fmaf(c0, bx[p], w.x); w.y = fmaf(c0, by[p], w.y); w.z = fmaf(c0, bz[p], w.z);
+    }
+    kick[k] = w;
+}
+
+__global__ void __launch_bounds__(W5_WPL * 32, 4) k_compat(SweepArgs a, float dt, const float4* __restrict__ kick) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
     const int64_t leaf = blockIdx.x;
@@ -718,20 +736,21 @@ __global__ void __launch_bounds__(W5_WPL * 32, 4) k_compat(SweepArgs a, float dt
     const int64_t i = leaf * CRK_LEAF + lane;
     const bool valid = i < a.n;
     const PState I = load_pstate(a.fst + i, a.np);
-    const float4 qi = a.fst[(int64_t)FPL * a.np + i];
+    const float4 qi = kick[i];
     const ForceConst fc = {a.L, a.half, 1.0f / a.n_h, a.n_h / 0.2f, a.eps2, a.C_l, a.C_q};
     float acc[1] = {0.f};
     const float4* planes[CPL];
 #pragma unroll
-    for (int p = 0; p < CPL; ++p) planes[p] = a.fst + (int64_t)p * a.np;
+    for (int p = 0; p < FPL; ++p) planes[p] = a.fst + (int64_t)p * a.np;
+    planes[FPL] = kick;
     leaf_sweep<W5_WPL, CPL, true, FPRE>(a, planes, leaf, 0, wl, lane, tile, [&](uint32_t sa, bool wrapped, const float4* pre) {
         const PState J = load_pstate_shared(sa, pre);
         const float4 qj = lds128(sa + (uint32_t)FPL * CRK_CCAP * 16u);
         const PairF f = force_pair(fc, I, J, wrapped);
-        // (v_j + v'_j - v_i - v'_i) = 2 (v_j - v_i) + (a_j - a_i) dt
-        const float wx = __fmaf_rn(dt, __fsub_rn(qj.x, qi.x), __fmul_rn(2.0f, f.vjix));
-        const float wy = __fmaf_rn(dt, __fsub_rn(qj.y, qi.y), __fmul_rn(2.0f, f.vjiy));
-        const float wz = __fmaf_rn(dt, __fsub_rn(qj.z, qi.z), __fmul_rn(2.0f, f.vjiz));
+        // (v_j + v'_j - v_i - v'_i) = 2 (v_j - v_i) + (kick_j - kick_i)
+        const float wx = __fmaf_rn(2.0f, f.vjix, __fsub_rn(qj.x, qi.x));
+        const float wy = __fmaf_rn(2.0f, f.vjiy, __fsub_rn(qj.y, qi.y));
+        const float wz = __fmaf_rn(2.0f, f.vjiz, __fsub_rn(qj.z, qi.z));
         const float w = __fmaf_rn(f.Fz, wz, __fmaf_rn(f.Fy, wy, __fmul_rn(f.Fx, wx)));       // = 2 dE_ij
         const float si = qi.w, sj = qj.w;
         float part = 0.5f;
@@ -850,12 +869,18 @@ int crk_launch_gradv_full(crk_ctx* c, float* gradv) {
 }
 
 // NEXT row 1: Eqs. 19-23 on the state left by crk_hydro_derivs
-int crk_launch_compat(crk_ctx* c, float dt, float* delta_u) {
+int crk_launch_compat(crk_ctx* c, float dt, float c1, float c0, const float* bx, const float* by, const float* bz,
+                      float* delta_u) {
+    const int64_t np = c->nl * CRK_LEAF;
+    CRK_TRY(crk_ensure(c, c->kick, (size_t)np * sizeof(float4)));
     SweepArgs a = make_args(c);
+    k_compat_prep<<<(unsigned)((np + 255) / 256), 256, 0, c->stream>>>((const float4*)c->fst.p + (int64_t)FPL * np, c->perm, c->n,
+                                                                       np, c1, c0, bx, by, bz, (float4*)c->kick.p);
+    CRK_TRY(crk_check_launch(c, "k_compat_prep"));
     a.o0 = delta_u;
     const int smem = CPL * CRK_CCAP * (int)sizeof(float4);
     CRK_TRY(set_smem(c, k_compat, smem));
-    k_compat<<<(unsigned)c->nl, W5_WPL * 32, smem, c->stream>>>(a, dt);
+    k_compat<<<(unsigned)c->nl, W5_WPL * 32, smem, c->stream>>>(a, dt, (const float4*)c->kick.p);
     return crk_check_launch(c, "k_compat");
 }
 

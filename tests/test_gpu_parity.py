@@ -620,7 +620,8 @@ def _sod_exact(x_over_t, gamma, rl, pl, rr, pr):
     return rho, u, S, us
 
 
-def test_sod_shock_tube_with_kdk_timestep_and_evolved_h():
+@pytest.mark.parametrize("compatible", [False, True])
+def test_sod_shock_tube_with_kdk_timestep_and_evolved_h(compatible):
     """The next rows working together (Eq. 43 steps, Eqs. 46-50 time steps, Eqs. 51-53 smoothing lengths) on the paper's Sod
     set-up (rho_h = P_h = 1, rho_l = P_l = 1/8, gamma = 5/3, two interfaces in a periodic domain, step
     function IC, here at half scale: unit box, interfaces at 0.25 / 0.75, t = 0.075), against the exact Riemann solution.
@@ -641,7 +642,7 @@ def test_sod_shock_tube_with_kdk_timestep_and_evolved_h():
     u = f32(P0 / ((gamma - 1) * rho0))
     vx, vy, vz = (torch.zeros(n, device=dev) for _ in range(3))
     h = torch.full((n,), n_h / ns, device=dev)
-    ctx = Crk(box=1.0, gamma=gamma, n_h=n_h, timestep=True)
+    ctx = Crk(box=1.0, gamma=gamma, n_h=n_h, timestep=True, kdk_compatible=compatible)
     ctx.step_derivs(x, y, z, h, vx, vy, vz, m, u)
     t, t_end, steps = 0.0, 0.075, 0
     e0 = float((m.double() * (u.double() + 0.5 * (vx.double() ** 2 + vy.double() ** 2 + vz.double() ** 2))).sum())
@@ -665,9 +666,39 @@ def test_sod_shock_tube_with_kdk_timestep_and_evolved_h():
     # motion stays a small fraction of the flow speed
     vt = float(torch.sqrt((vy.double() ** 2 + vz.double() ** 2).mean()))
     nb = float(cnt.float().mean())
-    print(f"[sod] n={n} steps={steps}: L1(rho) {l1_rho:.3f} L1(u)/u* {l1_u:.3f}, shock speed {S:.3f}, u* {ustar:.3f}, "
+    print(f"[sod] compatible={compatible} n={n} steps={steps}: L1(rho) {l1_rho:.3f} L1(u)/u* {l1_u:.3f}, shock speed {S:.3f}, u* {ustar:.3f}, "
           f"rms transverse speed {vt:.1e}, energy drift {abs(e1 / e0 - 1):.1e}, mean neighbours {nb:.1f}")
     assert l1_rho < 0.08 and l1_u < 0.15
     assert vt < 0.05 * ustar
-    assert abs(e1 / e0 - 1) < 2e-3
+    assert abs(e1 / e0 - 1) < (2e-6 if compatible else 2e-3)     # Eqs. 19-23 conserve to roundoff, Eq. 18 to O(dt^2)
     assert 50 < nb < 66
+
+
+@pytest.mark.parametrize("name,n_side,dt,steps", [("tiny_uniform", 16, 4e-3, 3), ("cosmo", 32, 2e-3, 2)])
+def test_kdk_step_with_compatible_energy(name, n_side, dt, steps, oracle_mod):
+    """CRK_FLAG_KDK_COMPATIBLE (reading S20): Verlet step whose half kicks use Eqs. 19-23; against the oracle's FP64
+    version, and total energy conserved to FP32 roundoff on the GPU"""
+    torch = _torch()
+    from paper_2202_02840_b200 import Crk
+    ps = wl.make_config(name, n_side)
+    ref = oracle_mod.kdk_steps(ps, steps, dt, compatible=True)
+    dev = torch.device("cuda:0")
+    t = {k: torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).to(dev) for k in
+         ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")}
+    ctx = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h, kdk_compatible=True, kdk_reuse=True)
+    m = t["m"].double()
+    energy = lambda: float((m * (t["u"].double() + 0.5 * (t["vx"].double() ** 2 + t["vy"].double() ** 2 + t["vz"].double() ** 2))).sum())
+    e0 = energy()
+    for _ in range(steps):
+        ctx.kdk_step(*[t[k] for k in ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")], dt)
+    torch.cuda.synchronize()
+    e1 = energy()
+    g = {k: v.cpu().numpy().astype(np.float64) for k, v in t.items()}
+    e_v = rel_l2(np.stack([g["vx"], g["vy"], g["vz"]]), np.stack([ref["vx"], ref["vy"], ref["vz"]]))
+    e_u = rel_l2(g["u"], ref["u"])
+    du_g, du_o = g["u"] - ps.u, ref["u"] - ps.u
+    e_du = rel_l2(du_g, du_o)
+    assert e_v < TOL_DERIV and e_u < TOL_DERIV and e_du < 1e-3, (e_v, e_u, e_du)
+    drift = abs(e1 / e0 - 1)
+    assert drift < 2e-6, drift
+    print(f"[parity] {name} n={ps.n} {steps} compatible KDK steps: v {e_v:.2e} u {e_u:.2e} du {e_du:.2e}, energy drift {drift:.1e}")
