@@ -702,3 +702,47 @@ def test_kdk_step_with_compatible_energy(name, n_side, dt, steps, oracle_mod):
     drift = abs(e1 / e0 - 1)
     assert drift < 2e-6, drift
     print(f"[parity] {name} n={ps.n} {steps} compatible KDK steps: v {e_v:.2e} u {e_u:.2e} du {e_du:.2e}, energy drift {drift:.1e}")
+
+
+def test_sedov_blast_wave_shock_radius():
+    """BASELINE config 2 evolved for real: 64^3 blast wave with the Verlet step, the compatible energy,
+    the time-step criteria and the evolved smoothing length; the shock radius follows the Sedov-Taylor similarity
+    solution R = xi0 (E t^2 / rho)^(1/5), xi0 = 1.152 for gamma = 5/3.  A physics check."""
+    torch = _torch()
+    from paper_2202_02840_b200 import Crk
+    ps = wl.make_config("blast_wave")
+    dev = torch.device("cuda:0")
+    t = {k: torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).to(dev) for k in
+         ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")}
+    arg = lambda: [t[k] for k in ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")]
+    ctx = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h, timestep=True, kdk_compatible=True)
+    ctx.step_derivs(*arg())
+    m = t["m"].double()
+    energy = lambda: float((m * (t["u"].double() + 0.5 * (t["vx"].double() ** 2 + t["vy"].double() ** 2 + t["vz"].double() ** 2))).sum())
+    e0 = energy()
+    time, t_end, steps = 0.0, 0.04, 0
+    while time < t_end - 1e-12:
+        dt = min(float(ctx.timestep(0.25).min()), t_end - time)
+        ctx.kdk_step(*arg(), dt)
+        t["h"].copy_(ctx.evolve_h())
+        time += dt
+        steps += 1
+        assert steps < 5000
+    ctx.build_cells(t["x"], t["y"], t["z"], t["h"])
+    V, rho, cnt = ctx.volumes(t["m"])
+    torch.cuda.synchronize()
+    e1 = energy()
+    X = np.stack([t[k].cpu().numpy().astype(np.float64) for k in ("x", "y", "z")]) - 0.5
+    r = np.sqrt((X ** 2).sum(0))
+    rh = rho.cpu().numpy().astype(np.float64)
+    bins = np.linspace(0.05, 0.48, 44)
+    idx = np.digitize(r, bins)
+    prof = np.array([np.median(rh[idx == b]) if (idx == b).sum() > 20 else 0.0 for b in range(1, len(bins))])
+    r_peak = 0.5 * (bins[:-1] + bins[1:])[np.argmax(prof)]
+    r_exact = 1.152 * (1.0 * t_end ** 2 / 1.0) ** 0.2
+    umin = float(t["u"].min())
+    print(f"[sedov] steps={steps} shock radius {r_peak:.3f} (similarity solution {r_exact:.3f}), peak density {prof.max():.2f}, "
+          f"energy drift {abs(e1 / e0 - 1):.1e}, min u {umin:.2e}")
+    assert abs(r_peak / r_exact - 1) < 0.06
+    assert 1.8 < prof.max() < 4.0            # strong-shock limit (gamma + 1)/(gamma - 1) = 4, smeared at this resolution
+    assert abs(e1 / e0 - 1) < 1e-5
