@@ -1,4 +1,5 @@
-// pairs.cu -- steps a1..a5: the four pair sweeps of one CRKSPH derivative evaluation (FP32 pair math on the FMA pipes).
+// pairs.cu -- steps a1..a5: the four pair sweeps of one CRKSPH derivative evaluation (FP32 pair math on the FMA pipes),
+// and the next rows that ride on them: compatible energy sweep, time-step criteria, evolved smoothing length.
 //
 // All sweeps walk the neighbour lists built once per crk_build_cells (lists.cu).  A leaf (32 particles) is served by WPL
 // warps; lane l of each of them holds particle i = 32*leaf + l in registers.  Per segment of the leaf's chain:

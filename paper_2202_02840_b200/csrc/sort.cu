@@ -1,8 +1,8 @@
 // sort.cu -- step a0 (first half): space-filling-curve keys, LSD radix sort, packed sorted state.
 //
 // PAPER.md:292 sorts particles into chaining-mesh bins and cuts RCB leaves of N_ppl particles; here the same
-// locality is obtained by sorting on a 48-bit Hilbert key (16 bits per axis) and cutting the sorted sequence into
-// contiguous 32-particle leaves (tree.cu).  HBM-bound: every kernel here streams keys/payload once per pass.
+// locality is obtained by sorting on a 3b-bit Hilbert key (b <= 16 bits per axis, chosen from the smallest h) and cutting
+// the sorted sequence into contiguous 32-particle leaves (tree.cu).  Every kernel here streams keys/payload once per pass.
 #include "crk_internal.cuh"
 #include <algorithm>
 
