@@ -181,7 +181,7 @@ __global__ void __launch_bounds__(256) k_kdk_predict(int64_t n, float L, float d
         half[q * n + i] = vh;
         float p = fmaf(vh, dt, pos[q][i]);
         p -= floorf(p / L) * L;                         // periodic wrap (reading S12)
-        if (!(p >= 0.f) || p >= L) p = 0.f;             // rounding can land on L
+        if (p >= L || p < 0.f) p = 0.f;                 // rounding can land on L; a NaN stays and is rejected by the next build
         pos[q][i] = p;
         vel[q][i] = fmaf(a, hd, vh);
     }

@@ -190,6 +190,22 @@ def test_errors_and_empty_input():
     with pytest.raises(CrkError) as ei:
         ctx2.hydro_derivs(one, one, one, one)
     assert ei.value.code == -5
+    # next rows: wrong call order / missing flag -> CRK_ESTATE; empty input is fine; a step that leaves the box is caught
+    for call in (lambda: ctx2.evolve_h(), lambda: ctx2.compatible_energy(1e-3), lambda: ctx2.timestep(0.25)):
+        with pytest.raises(CrkError) as ei:
+            call()
+        assert ei.value.code == -5
+    ctx3 = Crk(timestep=True, kdk_compatible=True, kdk_reuse=True)
+    ctx3.kdk_step(e, e, e, e, e, e, e, e, e, 1e-3)
+    r = lambda: torch.rand(64, device=dev)
+    st = [r(), r(), r(), torch.full((64,), 0.2, device=dev), r(), r(), r(), torch.full((64,), 1.0 / 64, device=dev), r() + 1.0]
+    ctx3.kdk_step(*st, 1e-3)
+    assert all(torch.isfinite(q).all() for q in st)
+    st[4].fill_(float("nan"))                                                  # v = NaN -> positions leave [0, L)
+    with pytest.raises(CrkError) as ei:
+        ctx3.kdk_step(*st, 1e-3)
+        ctx3.kdk_step(*st, 1e-3)
+    assert ei.value.code == -2
 
 
 # ------------------------------------------------------------------------------------------------ config 2 multi-step
