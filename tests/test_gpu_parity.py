@@ -762,3 +762,20 @@ def test_sedov_blast_wave_shock_radius():
     assert abs(r_peak / r_exact - 1) < 0.06
     assert 1.8 < prof.max() < 4.0            # strong-shock limit (gamma + 1)/(gamma - 1) = 4, smeared at this resolution
     assert abs(e1 / e0 - 1) < 1e-5
+
+
+def test_results_are_bit_reproducible():
+    """no atomics in any sum, fixed-order reductions: two evaluations (fresh contexts) give identical bits"""
+    torch = _torch()
+    from paper_2202_02840_b200 import Crk
+    ps = wl.make_config("clustered", 24)
+    dev = torch.device("cuda:0")
+    t = [torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).to(dev) for k in ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")]
+    runs = []
+    for _ in range(2):
+        ctx = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h, timestep=True)
+        out = ctx.step_derivs(*t)
+        runs.append([o.clone() for o in out] + [ctx.compatible_energy(1e-3).clone(), ctx.timestep(0.25).clone()])
+    torch.cuda.synchronize()
+    for a, b in zip(*runs):
+        assert torch.equal(a, b)
