@@ -115,10 +115,16 @@ __device__ __forceinline__ void group_sync(int lg) {
 // SYM = false: rows [0, Kg), lane active while k < cnt_g (gather set, Eqs. 13-14);  SYM = true: rows [0, K), k < cnt.
 // pair(slot_addr, crosses_boundary, plane0) evaluates one accepted pair (slot_addr = shared address of the candidate's
 // plane-0 entry; plane p sits CRK_CCAP * 16 * p bytes further); returns the number of entries the lane owns (= its count).
-template <int WPL, int PLANES, bool SYM, int NPRE = 1, typename Pair>
+struct NoInit {
+    __device__ __forceinline__ void operator()(uint32_t) const {}
+};
+// init(tile_s) runs once, after the first segment is staged: slots 0..31 of that tile are the leaf's own particles in lane
+// order (lists.cu), so a sweep can take its i-state from there instead of loading it from global memory
+template <int WPL, int PLANES, bool SYM, int NPRE = 1, typename Pair, typename Init = NoInit>
 __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4* const* planes, int64_t leaf, int lg, int wl,
-                                               int lane, float4* tile, Pair pair) {
+                                               int lane, float4* tile, Pair pair, Init init = Init()) {
     uint32_t count = 0;
+    bool first = true;
     const int tg = wl * 32 + lane;
     const uint32_t tile_s = (uint32_t)__cvta_generic_to_shared(tile);
     uint32_t unit;
@@ -151,6 +157,10 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
         }
         asm volatile("cp.async.wait_all;" ::: "memory");
         group_sync<WPL>(lg);
+        if (first) {
+            init(tile_s);
+            first = false;
+        }
         // plane 0 of the next pair's candidate is fetched one pair ahead: the pair math starts without waiting for shared
         // memory, and the loads of the remaining planes are covered by the arithmetic that needs plane 0 only
         float4 cur[NPRE];
@@ -671,7 +681,7 @@ __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
     float4* tile = (float4*)smem_raw;
     const int64_t i = leaf * CRK_LEAF + lane;
     const bool valid = i < a.n;
-    const PState I = load_pstate(a.fst + i, a.np);
+    PState I;                                            // taken from the tile (slots 0..31 = the leaf's own particles)
     const ForceConst fc = {a.L, a.half, 1.0f / a.n_h, a.n_h / 0.2f, a.eps2, a.C_l, a.C_q};
     float acc[4] = {0.f, 0.f, 0.f, 0.f};                 // Fx, Fy, Fz, dE
     float mx[2] = {0.f, 0.f};                            // max approach speed, max Q_i
@@ -686,6 +696,11 @@ __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
             mx[0] = fmaxf(mx[0], f.app);
             mx[1] = fmaxf(mx[1], f.Qi);
         }
+    }, [&](uint32_t ts) {
+        float4 pre[FPRE];
+#pragma unroll
+        for (int p = 0; p < FPRE; ++p) pre[p] = lds128(ts + (uint32_t)(p * CRK_CCAP + lane) * 16u);
+        I = load_pstate_shared(ts + (uint32_t)lane * 16u, pre);
     });
     group_reduce<W5_WPL, 4>(acc, 0, wl, lane, (float*)tile);
     if (TS) group_reduce<W5_WPL, 2, true>(mx, 0, wl, lane, (float*)tile);
