@@ -38,6 +38,8 @@ FP32_PEAK_THEORETICAL = 148 * 128 * 2 * 1.965e9     # SMs x FP32 lanes x 2 (FMA)
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_forces launch on the default workload (cosmo 256^3), from the
 # ncu --set full capture summarised in profiles/r01_sweeps_v9_ncu_full.md; other workloads report null
 FORCES_DRAM_BYTES_COSMO256 = 6.10e9 + 0.27e9
+# sm__inst_executed_pipe_fma.avg.pct_of_peak_sustained_active of the four sweeps in the same capture (forces, moments, grad v, volumes)
+NCU_FMA_PIPE_PCT_COSMO256 = {"k_forces": 39.6, "k_moments": 56.9, "k_gradv": 49.0, "k_volumes": 40.9}
 
 
 BASE_SEEDS = {"tiny_uniform": 1001, "blast_wave": 1002, "clustered": 1003, "cosmo": 1004, "cosmo_large": 1005}
@@ -322,6 +324,7 @@ def run_ours(args, rank, world, local_rank):
                                f"{fp32_meas / 1e12:.1f} TFLOP/s in this run",
                 "flops_per_pair": FLOPS_PER_PAIR["forces"], "pairs_per_launch": sym_pairs, "kernel_ms": forces_ms,
                 "traffic": FORCES_DRAM_BYTES_COSMO256 if (ps.name == "cosmo" and ps.meta["n_side"] == 256) else None,
+                "ncu_fma_pipe_pct": NCU_FMA_PIPE_PCT_COSMO256 if (ps.name == "cosmo" and ps.meta["n_side"] == 256) else None,
                 "traffic_unit": "bytes per launch (ncu dram read + write; algorithmic minimum = 160 B/particle = 2.7e9)"}
     passes = {k: st[k] for k in ("ms_sort", "ms_tree", "ms_lists", "ms_volumes", "ms_rk", "ms_gradv", "ms_forces")}
     alg_flops = (FLOPS_PER_PAIR["volumes"] + FLOPS_PER_PAIR["moments"] + FLOPS_PER_PAIR["gradv"]) * gather_pairs + forces_flops
