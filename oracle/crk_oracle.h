@@ -13,7 +13,10 @@
  * (reading S3) so that neighbour sets are a bit-exact contract rather than a rounding accident.
  *
  * Pin status (tests/test_oracle_pins.py): kernel, volumes, moments, A, B, gradA, gradB, RK gradient,
- * grad v, limiter, viscosity switch-off, momentum/energy pair antisymmetry are pinned.  PARITY UNPINNED
+ * grad v, momentum/energy pair antisymmetry are pinned by invariants; the limiter (phi_VL off r = 1, phi_ad), mu, Q and
+ * the pair terms of Eqs. 17-18 are pinned against the paper's PRINTED forms rebuilt in numpy with the golden constants
+ * (C_l, C_q, eps, eta_fold/eta_crit), incl. closed-form pairs (head-on approach, close approach in a linear flow).
+ * PARITY UNPINNED
  * (fixed by DESIGN.md readings only): Eq. 18 P_j-vs-P_i choice (S6), rho = m/V for unequal masses (S2),
  * c_s clamp max(u,0) (S12).
  */

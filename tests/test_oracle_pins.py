@@ -626,3 +626,235 @@ def test_compatible_kick_reduces_to_eq22_and_kdk_conserves_energy(oracle_mod):
     # the derivative evaluations see the float32 cast of v, so "roundoff" is float32 roundoff of the velocities
     assert abs(ec / e0 - 1) < 2e-8, ec / e0 - 1
     assert abs(ep / e0 - 1) > 20 * abs(ec / e0 - 1)
+
+
+# =====================================================================================================================
+# Limiter and viscosity against the PRINTED forms (Eqs. 24-25, 28-32) -- the oracle's limiter() and pair_term() compute
+# phi_VL division-free and mu with q = 1/hhat; these pins rebuild every factor in numpy from the paper's text, from the
+# golden constants and from quantities that other pins fix (grad v: P6; V, rho: P2/P10; grad WR: P3/P4).
+# =====================================================================================================================
+def _minimg(d, L=1.0):
+    return d - L * np.round(d / L)
+
+
+def _pair_geometry(ps, i, j):
+    X = np.stack([ps.x, ps.y, ps.z], 0).astype(np.float64)
+    x = _minimg(X[:, i] - X[:, j], ps.box)
+    return x, float(np.linalg.norm(x))
+
+
+def _phi_printed(N, Dn, eta_ij, n_h, g):
+    """Eqs. 28-32 exactly as printed: phi = phi_VL phi_ad, phi_VL = max[0, min[1, 4 r/(1+r)^2]],
+    r = N/Dn; phi_ad = exp{-((eta_ij - eta_crit)/eta_fold)^2} below eta_crit, else 1."""
+    r = N / Dn
+    phi_vl = max(0.0, min(1.0, 4.0 * r / (1.0 + r) ** 2))
+    eta_crit = 1.0 / n_h
+    eta_fold = g["eta_fold_over_eta_crit"] * eta_crit
+    phi_ad = math.exp(-((eta_ij - eta_crit) / eta_fold) ** 2) if eta_ij < eta_crit else 1.0
+    return phi_vl, phi_ad
+
+
+def _visc_printed(ps, o, d, gv, i, j, n_h, g, C_l=None, C_q=None, eps=None):
+    """(phi, Q_i, Q_j, mu_i, mu_j) of the pair from the printed Eqs. 24-32; None if Dn = 0 (r_ij undefined as printed)."""
+    C_l = g["visc_C_l"] if C_l is None else C_l
+    C_q = g["visc_C_q"] if C_q is None else C_q
+    eps = g["visc_eps"] if eps is None else eps
+    x, r = _pair_geometry(ps, i, j)
+    Gi, Gj = gv[:, i].reshape(3, 3), gv[:, j].reshape(3, 3)             # index [a][b] = d_b v^a (reading S9, pin P6)
+    N, Dn = x @ (Gi @ x), x @ (Gj @ x)                                   # Eq. 30
+    if Dn == 0.0:
+        return None
+    hi, hj = float(ps.h[i]), float(ps.h[j])
+    phi_vl, phi_ad = _phi_printed(N, Dn, min(r / hi, r / hj), n_h, g)    # Eq. 32: eta_ij = min(eta_i, eta_j)
+    phi = phi_vl * phi_ad
+    V = np.array([ps.vx, ps.vy, ps.vz], dtype=np.float64)
+    vij = V[:, i] - V[:, j]
+    # Eq. 27 with adot = 0: vhat_i = v_i - (phi/2) grad v_i . x_ij, vhat_j = v_j - (phi/2) grad v_j . x_ji
+    uhat = (V[:, i] - 0.5 * phi * (Gi @ x)) - (V[:, j] - 0.5 * phi * (Gj @ (-x)))
+    ux = uhat @ x
+    out = [phi]
+    mus, Qs = [], []
+    for k, hk in ((i, hi), (j, hj)):
+        hhat = hk / n_h                                                  # PAPER.md:147 "hhat = h / n_h"
+        mu = min(0.0, hhat * ux / (r * r + hhat * hhat * eps * eps))     # Eq. 25
+        cs = math.sqrt(ps.gamma * (ps.gamma - 1.0) * max(float(ps.u[k]), 0.0))
+        Qs.append(d["rho"][k] * (-C_l * cs * mu + C_q * mu * mu))        # Eq. 24
+        mus.append(mu)
+    return np.array(out + Qs + mus), (N, Dn, phi_vl, phi_ad, vij @ x)
+
+
+@pytest.mark.parametrize("which", ["tiny", "clustered"])
+def test_limiter_and_viscosity_equal_the_printed_forms_on_general_flows(which, tiny, clustered):
+    """phi (Eqs. 28-32), mu (Eq. 25), Q (Eq. 24) of sampled pairs of a random-velocity
+    gas, rebuilt in numpy from the printed forms, the golden constants and grad v (pinned by P6)."""
+    ps, o, d = tiny if which == "tiny" else clustered
+    g = golden()
+    gv = o.gradv()
+    rng = np.random.default_rng(11)
+    seen = dict(neg=0, far=0, near1=0, ad=0, visc=0, pairs=0)
+    for i in rng.integers(0, ps.n, 400):
+        js, fi, fj = o.neighbors(i)
+        for j in js[rng.permutation(len(js))[:8]]:
+            exp = _visc_printed(ps, o, d, gv, int(i), int(j), ps.n_h, g)
+            if exp is None:
+                continue
+            want, (N, Dn, phi_vl, phi_ad, _) = exp
+            got = o.pair_visc(int(i), int(j))
+            assert got[0] == pytest.approx(want[0], rel=1e-10, abs=1e-14)
+            scale = abs(want[1]) + abs(want[2]) + 1e-300
+            assert np.allclose(got[1:3], want[1:3], rtol=1e-9, atol=1e-12 * scale)
+            assert np.allclose(got[3:5], want[3:5], rtol=1e-9, atol=1e-14)
+            r = N / Dn
+            seen["pairs"] += 1
+            seen["neg"] += r < 0
+            seen["far"] += (r > 3.0) or (0 < r < 1 / 3.0)
+            seen["near1"] += 0.8 < r < 1.25
+            seen["ad"] += phi_ad < 1.0
+            seen["visc"] += want[3] < 0
+    # the sample must exercise every branch: r < 0 (phi = 0), r far from 1, r ~ 1, the close-approach factor, mu < 0
+    assert seen["pairs"] > 2000 and seen["neg"] > 200 and seen["far"] > 200 and seen["near1"] > 50 and seen["visc"] > 500
+    if which == "tiny":
+        assert seen["ad"] > 3        # jittered lattice: closest pairs at ~0.8 spacing = 0.33 h < h / n_h
+
+
+def _with_extra_particles(ps, extra):
+    """ps plus hand-placed particles; extra = list of dicts with x, y, z, vx, vy, vz, h, u (masses as the rest)"""
+    import copy
+    q = copy.copy(ps)
+    for k in ("x", "y", "z", "vx", "vy", "vz", "h", "u"):
+        setattr(q, k, np.concatenate([getattr(ps, k), np.array([e[k] for e in extra], dtype=np.float32)]))
+    q.m = np.concatenate([ps.m, np.full(len(extra), ps.m[0], dtype=np.float32)])
+    return q
+
+
+@pytest.mark.parametrize("n_h", [2.4, 4.0])
+def test_phi_ad_close_approach_factor_in_a_linear_flow(n_h, oracle_mod):
+    """Eqs. 31-32.  In a linear flow grad v = M for every particle (P6), so r_ij = 1 and phi_VL = 1:
+    phi IS phi_ad.  Two particles are placed closer than h/n_h to a lattice particle, with supports that differ from its
+    own, so eta_ij = min(eta_i, eta_j), eta_crit = 1/n_h and eta_fold = 0.2/n_h (golden) all enter."""
+    g = golden()
+    base = wl.tiny_uniform(n_side=12, seed=5)
+    base.n_h = n_h
+    base.h[:] = np.float32(n_h / 12.0)                                 # h = n_h spacings (n_h = 4: 0.333 < L/2)
+    X = np.stack([base.x, base.y, base.z], 0).astype(np.float64)
+    c = int(np.argmin(((X - 0.5) ** 2).sum(0)))
+    h0 = float(base.h[c])
+    sep = [0.30 * h0 / n_h, 0.85 * h0 / n_h]                          # both inside eta_crit of the LARGER support
+    hs = [0.8 * h0, 1.3 * h0]
+    M = np.array([[0.3, -1.1, 0.4], [0.7, 0.2, -0.5], [-0.9, 0.6, -0.8]])
+    extra = []
+    for s, hx in zip(sep, hs):
+        dirn = np.array([0.6, -0.64, 0.48])
+        p = X[:, c] + s * dirn
+        extra.append(dict(x=p[0], y=p[1], z=p[2], vx=0, vy=0, vz=0, h=hx, u=1.0))
+    ps = _with_extra_particles(base, extra)
+    Xa = np.stack([ps.x, ps.y, ps.z], 0).astype(np.float64)
+    v = M @ Xa + np.array([[0.1], [-0.2], [0.3]])
+    ps.vx, ps.vy, ps.vz = (v[a].astype(np.float32) for a in range(3))
+    o = oracle_mod.Oracle(ps.box, ps.gamma, n_h)
+    o.step_derivs(ps)
+    for q, hx in enumerate(hs):
+        j = base.n + q
+        x, r = _pair_geometry(ps, c, j)
+        eta_ij = min(r / h0, r / hx)                                   # Eq. 32
+        eta_crit = 1.0 / n_h
+        eta_fold = g["eta_fold_over_eta_crit"] * eta_crit              # PAPER.md:179: (1/n_h, 0.2/n_h)
+        assert eta_ij < eta_crit
+        want = math.exp(-((eta_ij - eta_crit) / eta_fold) ** 2)        # Eq. 31
+        for a, b in ((c, j), (j, c)):
+            phi = o.pair_visc(a, b)[0]
+            assert phi == pytest.approx(want, rel=2e-4)                # phi_VL = 1 up to the float32 velocities
+        assert 1e-9 < want < 0.999
+
+
+@pytest.mark.parametrize("n_h,C_l,C_q,eps", [(2.4, None, None, None), (4.0, None, None, None), (2.4, 1.5, 0.7, 0.2)])
+def test_viscosity_head_on_pair_closed_form(n_h, C_l, C_q, eps, oracle_mod):
+    """Eqs. 24-25 on a pair whose uhat_ij . x_ij is known in closed form: two particles approach
+    head-on at a separation far below eta_crit, where phi <= exp(-25 (1 - eta/eta_crit)^2) ~ 1e-11 removes the projection
+    of Eq. 27, so uhat_ij . x_ij = v_ij . x_ij = -2 k d.  Then mu_k = hhat_k (-2kd)/(d^2 + hhat_k^2 eps^2) with
+    hhat_k = h_k/n_h, and Q_k = rho_k (-C_l c_k mu_k + C_q mu_k^2); constants from the golden file (or non-default ones,
+    to see each enter where the paper puts it)."""
+    g = golden()
+    base = wl.tiny_uniform(n_side=12, seed=6)
+    base.n_h = n_h
+    base.h[:] = np.float32(n_h / 12.0)
+    base.vx[:] = 0; base.vy[:] = 0; base.vz[:] = 0
+    h0 = float(base.h[0])
+    k, d = 0.37, 2.0e-3 * h0
+    hi, hj = 0.9 * h0, 1.2 * h0
+    pi = np.array([0.52, 0.49, 0.51])
+    extra = [dict(x=pi[0], y=pi[1], z=pi[2], vx=+k, vy=0, vz=0, h=hi, u=1.3),
+             dict(x=pi[0] + d, y=pi[1], z=pi[2], vx=-k, vy=0, vz=0, h=hj, u=2.1)]
+    ps = _with_extra_particles(base, extra)
+    kw = {}
+    if C_l is not None:
+        kw = dict(C_l=C_l, C_q=C_q, eps=eps)
+    o = oracle_mod.Oracle(ps.box, ps.gamma, n_h, **kw)
+    dd = o.step_derivs(ps)
+    Cl = g["visc_C_l"] if C_l is None else C_l
+    Cq = g["visc_C_q"] if C_q is None else C_q
+    ep = g["visc_eps"] if eps is None else eps
+    if C_l is None:                                                    # the library defaults ARE the paper's constants
+        assert (o.params.C_l, o.params.C_q, o.params.eps) == (g["visc_C_l"], g["visc_C_q"], g["visc_eps"])
+    i, j = base.n, base.n + 1
+    x, r = _pair_geometry(ps, i, j)
+    vx = (np.float64(ps.vx[i]) - np.float64(ps.vx[j])) * x[0]         # = -2 k d (approaching)
+    assert vx < 0
+    phi, Qi, Qj, mui, muj = o.pair_visc(i, j)
+    assert phi < 1e-9
+    for (hk, uk, rho, mu_got, Q_got) in ((hi, 1.3, dd["rho"][i], mui, Qi), (hj, 2.1, dd["rho"][j], muj, Qj)):
+        hhat = float(np.float32(hk)) / n_h
+        mu = hhat * vx / (r * r + hhat * hhat * ep * ep)
+        assert mu_got == pytest.approx(mu, rel=1e-8)
+        cs = math.sqrt(ps.gamma * (ps.gamma - 1.0) * float(np.float32(uk)))
+        assert Q_got == pytest.approx(rho * (-Cl * cs * mu + Cq * mu * mu), rel=1e-8)
+        assert Q_got > 0
+    # receding pair: mu = min(0, .) = 0 and Q = 0
+    ps.vx[i], ps.vx[j] = np.float32(-k), np.float32(+k)
+    o.step_derivs(ps)
+    out = o.pair_visc(i, j)
+    assert out[1] == 0.0 and out[2] == 0.0 and out[3] == 0.0 and out[4] == 0.0
+
+
+def test_pair_terms_equal_printed_eqs_17_18_with_P_plus_Q(clustered):
+    """Eqs. 17-18 with P -> P + Q for sampled pairs: m_i a_ij = (1/2) V_i V_j (P_i+Q_i+P_j+Q_j) G_ij
+    and m_i du_ij = (1/2) V_i V_j (P_j+Q_j) v_ji . G_ij, with G_ij = grad WR_ji - grad WR_ij rebuilt in numpy from Eq. 16 as
+    printed out of the oracle's A, B, grad A, grad B (pinned by P2-P5) and Q from the printed Eqs. 24-25."""
+    ps, o, d = clustered
+    g = golden()
+    gv = o.gradv()
+    V = np.array([ps.vx, ps.vy, ps.vz], dtype=np.float64)
+    P = (ps.gamma - 1.0) * d["rho"] * ps.u.astype(np.float64)          # Eq. 4
+
+    def grad_WR(a, x, r):                                              # Eq. 16 for particle a, separation x = x_a - x_b
+        h = float(ps.h[a])
+        W = oracle_W(r, h)
+        dW = oracle_dW(r, h)
+        A, B = d["A"][a], d["B"][:, a]
+        gA, gB = d["gradA"][:, a], d["gradB"][:, a].reshape(3, 3)      # gB[c][b] = d_c B^b
+        s = 1.0 + B @ x
+        gradW = dW * x / r if r > 0 else np.zeros(3)
+        return A * s * gradW + A * (gB @ x + B) * W + gA * s * W
+
+    import crk_oracle
+    oracle_W, oracle_dW = crk_oracle.kernel_W, crk_oracle.kernel_dWdr
+    rng = np.random.default_rng(21)
+    n_visc = 0
+    for i in rng.integers(0, ps.n, 60):
+        js, fi, fj = o.neighbors(i)
+        for j in js[rng.permutation(len(js))[:6]]:
+            i, j = int(i), int(j)
+            exp = _visc_printed(ps, o, d, gv, i, j, ps.n_h, g)
+            if exp is None:
+                continue
+            (phi, Qi, Qj, _, _), _ = exp
+            x, r = _pair_geometry(ps, i, j)
+            G = grad_WR(j, -x, r) - grad_WR(i, x, r)
+            hvv = 0.5 * d["V"][i] * d["V"][j]
+            F = hvv * (P[i] + Qi + P[j] + Qj) * G
+            dE = hvv * (P[j] + Qj) * ((V[:, j] - V[:, i]) @ G)
+            got = o.pair_term(i, j)
+            assert np.allclose(got[:3], F, rtol=1e-8, atol=1e-10 * np.abs(F).max())
+            assert got[3] == pytest.approx(dE, rel=1e-8, abs=1e-10 * abs(hvv * P[j] * np.linalg.norm(G)))
+            n_visc += Qi > 0
+    assert n_visc > 50
