@@ -127,7 +127,10 @@ inline bool inv3(const double m[3][3], double inv[3][3]) {
     const double c01 = m[1][2] * m[2][0] - m[1][0] * m[2][2];
     const double c02 = m[1][0] * m[2][1] - m[1][1] * m[2][0];
     const double det = m[0][0] * c00 + m[0][1] * c01 + m[0][2] * c02;
-    if (!(std::fabs(det) > 0.0) || !std::isfinite(det)) return false;
+    // reading S14: m2 counts as singular when det m2 <= 1e-4 (tr m2 / 3)^3, i.e. when the neighbours span less
+    // than three dimensions up to rounding (fewer than 3 non-collinear, or coplanar, neighbours); an isotropic m2 has ratio 1
+    const double tr3 = (m[0][0] + m[1][1] + m[2][2]) / 3.0;
+    if (!(det > 1.0e-4 * tr3 * tr3 * tr3) || !std::isfinite(det)) return false;
     const double id = 1.0 / det;
     inv[0][0] = c00 * id;
     inv[0][1] = (m[0][2] * m[2][1] - m[0][1] * m[2][2]) * id;

@@ -224,10 +224,11 @@ class Oracle:
         return buf & np.uint32(0x3fffffff), (buf >> np.uint32(31)).astype(bool), ((buf >> np.uint32(30)) & 1).astype(bool)
 
 
-def euler_steps(ps, n_steps: int, dt: float, oracle: Oracle | None = None):
+def euler_steps(ps, n_steps: int, dt: float, oracle: Oracle | None = None, grid: bool = False):
     """Step 12 of DESIGN.md (BASELINE config 2): forward Euler in FP64 on the oracle's derivatives.
     Yields (step, state_f32 ParticleSet-like dict, derivs dict) BEFORE each update, so a caller can
-    teacher-force another implementation on the same FP32 state.  h and m stay fixed."""
+    teacher-force another implementation on the same FP32 state.  h and m stay fixed.
+    grid=True: neighbours through crk_oracle_build_grid (bit-identical structure, pinned) so that 64^3 takes seconds."""
     import copy
     o = oracle or Oracle(ps.box, ps.gamma, ps.n_h)
     st = {k: np.asarray(getattr(ps, k), dtype=np.float64).copy() for k in ("x", "y", "z", "vx", "vy", "vz", "u")}
@@ -239,7 +240,7 @@ def euler_steps(ps, n_steps: int, dt: float, oracle: Oracle | None = None):
         for k in ("x", "y", "z"):           # the float32 cast may round up to L
             a = getattr(cur, k)
             a[a >= np.float32(L)] = np.float32(0.0)
-        d = o.step_derivs(cur)
+        d = o.step_derivs(cur, grid=grid)
         yield step, cur, d
         if step == n_steps:
             break

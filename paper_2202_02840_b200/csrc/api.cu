@@ -54,7 +54,7 @@ void crk_destroy(crk_ctx* c) {
     DevBuf* bufs[] = {&c->keys[0], &c->keys[1], &c->vals[0], &c->vals[1], &c->hist, &c->scan_tmp, &c->posh_orig,
                       &c->posh, &c->leaf_lo, &c->leaf_hi, &c->nbr_cnt, &c->nbr_off, &c->nbr_list, &c->nbr_gcnt,
                       &c->posV, &c->rho_s, &c->coef, &c->fst, &c->u_s, &c->vel_orig, &c->m_s, &c->flag,
-                      &c->host_stage, &c->arena, &c->seg_first, &c->leaf_cnt, &c->ts_s, &c->kdk, &c->kick};
+                      &c->host_stage, &c->arena, &c->seg_first, &c->leaf_cnt, &c->cand_first, &c->ts_s, &c->kdk, &c->kick};
     for (DevBuf* b : bufs)
         if (b->p) cudaFree(b->p);
     if (c->h_flag) cudaFreeHost(c->h_flag);
@@ -127,7 +127,7 @@ int crk_rk_coefficients(crk_ctx* c, float* A, float* B, float* gradA, float* gra
     }
     if (c->n > 0) {
         rec(c, EV_RK0);
-        CRK_TRY(crk_launch_moments(c, A, B, gradA, gradB));
+        CRK_TRY(crk_launch_rk(c, true, false, A, B, gradA, gradB, nullptr));
         rec(c, EV_RK1);
     }
     c->stage = 3;
@@ -144,7 +144,13 @@ int crk_hydro_derivs(crk_ctx* c, const float* vx, const float* vy, const float* 
     if (c->n > 0 && (!vx || !vy || !vz || !u || !ax || !ay || !az || !dudt)) return CRK_EINVAL;
     if (c->n > 0) {
         rec(c, EV_HY0);
-        CRK_TRY(crk_launch_hydro(c, vx, vy, vz, u, ax, ay, az, dudt, pair_count));
+        CRK_TRY(crk_launch_hydro_prep(c, vx, vy, vz, u));
+        rec(c, EV_PREP1);
+        rec(c, EV_GV0);
+        CRK_TRY(crk_launch_rk(c, false, true, nullptr, nullptr, nullptr, nullptr, nullptr));
+        rec(c, EV_GV1);
+        CRK_TRY(crk_launch_forces(c, ax, ay, az, dudt, pair_count));
+        rec(c, EV_F1);
         if (c->timing) c->ev_done[c->ev_slot] = true;
     }
     c->stage = 4;
@@ -156,8 +162,25 @@ int crk_step_derivs(crk_ctx* c, int64_t n, const float* x, const float* y, const
                     float* ay, float* az, float* dudt) {
     CRK_TRY(crk_build_cells(c, n, x, y, z, h));
     CRK_TRY(crk_volumes(c, m, nullptr, nullptr, nullptr));
-    CRK_TRY(crk_rk_coefficients(c, nullptr, nullptr, nullptr, nullptr));
-    return crk_hydro_derivs(c, vx, vy, vz, u, ax, ay, az, dudt, nullptr);
+    if (n == 0) {
+        c->stage = 4;
+        return CRK_OK;
+    }
+    if (!vx || !vy || !vz || !u || !ax || !ay || !az || !dudt) return CRK_EINVAL;
+    // moments + 3x3 solve and the velocity-gradient sums in ONE sweep over the lists (same bits as the two staged calls)
+    rec(c, EV_HY0);
+    CRK_TRY(crk_launch_hydro_prep(c, vx, vy, vz, u));
+    rec(c, EV_PREP1);
+    rec(c, EV_RK0);
+    CRK_TRY(crk_launch_rk(c, true, true, nullptr, nullptr, nullptr, nullptr, nullptr));
+    rec(c, EV_RK1);
+    rec(c, EV_GV0);
+    rec(c, EV_GV1);
+    CRK_TRY(crk_launch_forces(c, ax, ay, az, dudt, nullptr));
+    rec(c, EV_F1);
+    if (c->timing) c->ev_done[c->ev_slot] = true;
+    c->stage = 4;
+    return CRK_OK;
 }
 
 // ---- NEXT row 2b: hydro-only velocity-Verlet step, Eq. 43, a = 1, dt/dy = 1, p = v -----------------
@@ -332,7 +355,7 @@ int crk_get_gradv(crk_ctx* c, float* gradv) {
     if (!c || !gradv) return CRK_EINVAL;
     if (c->stage < 4) return CRK_ESTATE;
     if (c->n == 0) return CRK_OK;
-    return crk_launch_gradv_full(c, gradv);   // the force-sweep state keeps only the symmetric part: re-run the sweep
+    return crk_launch_rk(c, false, true, nullptr, nullptr, nullptr, nullptr, gradv);   // the force-sweep state keeps only the symmetric part: re-run the sweep
 }
 
 int crk_set_timing(crk_ctx* c, int on) {
@@ -374,7 +397,7 @@ int crk_get_stats(crk_ctx* c, crk_stats* out) {
             };
             acc[0] += el(EV_BUILD0, EV_SORTED); acc[1] += el(EV_SORTED, EV_TREE1); acc[2] += el(EV_BUILD0, EV_BUILD1);
             acc[8] += el(EV_TREE1, EV_BUILD1);
-            acc[3] += el(EV_VOL0, EV_VOL1); acc[4] += el(EV_RK0, EV_RK1); acc[5] += el(EV_HY0, EV_F1);
+            acc[3] += el(EV_VOL0, EV_VOL1); acc[4] += el(EV_RK0, EV_RK1); acc[5] += el(EV_HY0, EV_PREP1) + el(EV_GV0, EV_F1);
             acc[6] += el(EV_GV0, EV_GV1); acc[7] += el(EV_GV1, EV_F1);
             ++cnt;
         }

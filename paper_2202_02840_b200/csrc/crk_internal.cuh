@@ -14,23 +14,29 @@
 
 #define CRK_EV_RING 64
 #define CRK_EV_N 13
-enum { EV_BUILD0 = 0, EV_SORTED, EV_TREE1, EV_BUILD1, EV_VOL0, EV_VOL1, EV_RK0, EV_GV0, EV_GV1, EV_F1, EV_RK1, EV_HY0 };
+enum { EV_BUILD0 = 0, EV_SORTED, EV_TREE1, EV_BUILD1, EV_VOL0, EV_VOL1, EV_RK0, EV_GV0, EV_GV1, EV_F1, EV_RK1, EV_HY0, EV_PREP1 };
 
 // ---- neighbour lists (lists.cu): per leaf a chain of segments in one arena of 16-byte units --------------------------
-//   segment = header (9 units) | cand[C] u32, padded to 4 | ell[K][32] u16
-//   header unit 0: {next segment (arena unit, 0 = none), C | Kg << 16, K, 0}; units 1-4: cnt_g[32] u16; units 5-8: cnt[32] u16
-//   the first segment's header is mirrored in dense per-leaf arrays: seg_first[leaf] = {next, C | Kg << 16, K, own arena unit
-//   (0 = leaf has no segment)} and leaf_cnt[leaf][64] = cnt_g | cnt
+//   segment = header (9 units) | cand[C] u32, padded to 4 (not in a leaf's first segment) | ell[K][32] u16
+//   header unit 0: {next segment (arena unit, 0 = none), C | CRK_SEG_WRAP | K << 16, 0, 0}; units 1-4: cnt_g[32] u16;
+//   units 5-8: cnt[32] u16
+//   the first segment's header is mirrored in dense per-leaf arrays, so that a sweep reaches the payload without a
+//   pointer chase: seg_first[leaf] = {next, C | CRK_SEG_WRAP | K << 16, 0, own arena unit (0 = leaf has no segment)},
+//   leaf_cnt[leaf][64] = cnt_g | cnt, and cand_first[leaf][CRK_CAND_STRIDE] = the first segment's candidate indices
 //   cand[c]   = sorted-order index of candidate c (only candidates accepted by at least one lane of the leaf); in a
 //               leaf's first segment cand[0..31] are the leaf's own 32 particles in lane order (always kept)
-//   ell[k][l] = k-th entry of lane l: candidate index | bit 15 (pair crosses the periodic boundary); lane l owns
-//               cnt_g[l] gather entries (r2 < h_i^2) followed by cnt[l] - cnt_g[l] entries that are symmetric-only
+//   ell[k][l] = k-th entry of lane l: candidate index | CRK_ELL_SYM (h_i^2 <= r2 < h_j^2: a pair of the symmetric set that
+//               is not in the lane's gather set) | CRK_ELL_WRAP (pair crosses the periodic boundary); lane l owns cnt[l]
+//               entries, cnt_g[l] of them gather entries; CRK_SEG_WRAP: some entry of the segment may carry CRK_ELL_WRAP
 #define CRK_CCAP 352             // candidates per segment (tile capacity of the sweeps)
+#define CRK_CAND_STRIDE 384      // u32 per leaf in cand_first (the sweeps read it in 16-byte groups)
 #define CRK_QCAP 128             // entries per lane per segment
 #define CRK_TCULL 32             // cull tile of the list builder
 #define CRK_SEG_HDR_UNITS 9
 #define CRK_ELL_WRAP 0x8000u
-#define CRK_ELL_MASK 0x7fffu
+#define CRK_ELL_SYM  0x4000u
+#define CRK_ELL_MASK 0x3fffu
+#define CRK_SEG_WRAP 0x8000u
 
 #define CRK_FLAG_GATHER 0x80000000u   // leaf-list entry: gap(a,b) < hmax(a)   (one-sided passes use it)
 #define CRK_FLAG_WRAP   0x40000000u   // leaf pair may straddle the periodic boundary
@@ -77,12 +83,13 @@ struct crk_ctx {
     int64_t n_pairs = 0, n_pairs_gather = 0;
     DevBuf arena, seg_first;       // neighbour-list arena (16-byte units); per leaf a uint4 copy of its first segment's header
     DevBuf leaf_cnt;               // u16[nl][64]: per-lane cnt_g | cnt of the first segment (dense, so the sweeps need no pointer chase)
+    DevBuf cand_first;             // u32[nl][CRK_CAND_STRIDE]: candidate indices of the first segment (dense)
     int64_t arena_units = 0;       // units used by the last build
     // per-particle state in sorted order
     DevBuf posV;                   // float4 (x,y,z,V)
     DevBuf rho_s;                  // float
     DevBuf coef;                   // 4 planes float4[n]: (A,Bx,By,Bz) (cx,cy,cz,M00) (M01,M02,M10,M11) (M12,M20,M21,M22)
-    DevBuf fst;                    // force-sweep state, 9 planes float4[np] (layout at k_gradv in pairs.cu) + plane 9 = (dv/dt, s)
+    DevBuf fst;                    // force-sweep state, 9 planes float4[np] (layout at k_rk in pairs.cu) + plane 9 = (dv/dt, s)
     DevBuf ts_s;                   // float2 (max approach speed, max Q_i), sorted; only with CRK_FLAG_TIMESTEP
     DevBuf kick;                   // compatible-energy sweep: (v' - v, s) per particle, sorted
     DevBuf kdk;                    // crk_kdk_step scratch: derivatives [4][n] and half-step state [4][n]
@@ -151,10 +158,9 @@ int crk_exclusive_scan_u32(crk_ctx* c, const uint32_t* in, uint32_t* out, int64_
 int crk_build_tree_and_list(crk_ctx* c);                                                               // tree.cu
 int crk_build_nbr_lists(crk_ctx* c);                                                                   // lists.cu
 int crk_launch_volumes(crk_ctx* c, const float* m, float* V, float* rho, uint32_t* nbr_count);        // pairs.cu
-int crk_launch_moments(crk_ctx* c, float* A, float* B, float* gradA, float* gradB);                   // pairs.cu
-int crk_launch_hydro(crk_ctx* c, const float* vx, const float* vy, const float* vz, const float* u,
-                     float* ax, float* ay, float* az, float* dudt, uint32_t* pair_count);             // pairs.cu
-int crk_launch_gradv_full(crk_ctx* c, float* gradv);
+int crk_launch_hydro_prep(crk_ctx* c, const float* vx, const float* vy, const float* vz, const float* u);   // pairs.cu
+int crk_launch_rk(crk_ctx* c, bool mom, bool gv, float* A, float* B, float* gradA, float* gradB, float* gradv_full);   // pairs.cu
+int crk_launch_forces(crk_ctx* c, float* ax, float* ay, float* az, float* dudt, uint32_t* pair_count);   // pairs.cu
 int crk_launch_timestep(crk_ctx* c, float C_cfl, float* dt_min);                                       // pairs.cu
 int crk_launch_evolve_h(crk_ctx* c, float* h_new);                                                    // pairs.cu
 int crk_launch_compat(crk_ctx* c, float dt, float c1, float c0, const float* bx, const float* by, const float* bz,

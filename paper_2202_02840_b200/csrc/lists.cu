@@ -1,13 +1,15 @@
-// lists.cu -- step a0 (third part): per-particle neighbour lists, built once per crk_build_cells and reused by all four
+// lists.cu -- step a0 (third part): per-particle neighbour lists, built once per crk_build_cells and reused by all
 // pair sweeps ("all hydro operators utilize the same interaction list, which need only be assembled once per hydro
 // subcycle, and reused for each kernel", PAPER.md:302 -- here taken down to particle pairs).
 //
 // One warp = one 32-particle leaf, one lane = one particle i.  For every neighbour leaf of the leaf interaction list
 // (tree.cu) lane l takes particle l of that leaf and culls it against the query leaf's box; survivors go to a small tile;
-// every staged j is then tested against every lane's i with the prescribed FP32 predicate (S3).  A candidate
-// accepted by at least one lane receives the next candidate index c of the current segment; lane i appends c to its
-// gather entries (r2 < h_i^2) or to its symmetric-only entries (h_i^2 <= r2 < h_j^2).  A segment is written to the arena
-// as  header | cand[C] | ell[K][32]  (layout in crk_internal.cuh); it is cut when the candidate or entry capacity would
+// every staged j is then tested against every lane's i with the prescribed FP32 predicate (S3), two candidates
+// per instruction stream with the packed FP32 forms of sm_100 (add/mul/fma.rn.f32x2: each half is rounded to nearest, so
+// the bits are those of the scalar sequence).  A candidate accepted by at least one lane receives the next candidate
+// index c of the current segment; lane i appends c to its entries, flagged "symmetric only" when h_i^2 <= r2 < h_j^2
+// (a pair of Eqs. 17-18 that is not in the gather set of Eqs. 13-14).  A segment is written to the arena as
+// header | cand[C] | ell[K][32]  (layout in crk_internal.cuh); it is cut when the candidate or entry capacity would
 // overflow, so leaves in strongly clustered regions own a chain of segments.
 #include "crk_internal.cuh"
 
@@ -29,18 +31,17 @@ struct ListArgs {
     unsigned long long* counter;           // next free unit (unit 0 is reserved as "none")
     uint4* __restrict__ seg_first;         // dense copy of each leaf's first header (.w = its arena unit)
     uint16_t* __restrict__ leaf_cnt;       // [nl][64]
+    uint32_t* __restrict__ cand_first;     // [nl][CRK_CAND_STRIDE] candidates of each leaf's first segment
 };
 
 struct WarpSmem {
-    float4 tile[CRK_TCULL + 4];
-    __align__(16) uint32_t tidx[CRK_TCULL + 4];
+    float4 ta[(CRK_TCULL + 2) / 2];   // candidates 2t, 2t+1: (-x_a, -x_b, -y_a, -y_b)
+    float4 tb[(CRK_TCULL + 2) / 2];   //                      (-z_a, -z_b, h_a^2, h_b^2)
+    __align__(8) uint32_t tidx[CRK_TCULL + 2];
     uint32_t cand[CRK_CCAP];
     uint16_t queue[CRK_QCAP][32];
 };
 
-__device__ __forceinline__ float wrap1(float d, float L, float half) {
-    return d > half ? __fsub_rn(d, L) : (d < -half ? __fadd_rn(d, L) : d);
-}
 // lower bound of |wrap(x_i - x_j)| on one axis for x_i in [lo,hi] (monotone float ops, so nothing is lost)
 __device__ __forceinline__ float gap1(float lo, float hi, float x) {
     return fmaxf(0.f, fmaxf(__fsub_rn(lo, x), __fsub_rn(x, hi)));
@@ -61,53 +62,61 @@ __device__ __forceinline__ void sts_u32_if(uint32_t addr, uint32_t v, bool pred)
     asm volatile("{ .reg .pred p; setp.ne.b32 p, %2, 0; @p st.shared.u32 [%0], %1; }" ::"r"(addr), "r"(v), "r"((int)pred) : "memory");
 }
 
+// minimum-image wrap of both halves (S3: d > L/2 -> d - L, d < -L/2 -> d + L); adding 0 leaves the other values untouched
+__device__ __forceinline__ float2 wrap2(float2 d, float L, float half, bool& wa, bool& wb) {
+    const float sa = d.x > half ? -L : (d.x < -half ? L : 0.f);
+    const float sb = d.y > half ? -L : (d.y < -half ? L : 0.f);
+    wa = wa || (sa != 0.f);
+    wb = wb || (sb != 0.f);
+    return __fadd2_rn(d, make_float2(sa, sb));
+}
+
 // test every staged candidate against the lane's particle; returns the new candidate count of the segment.
-// Branch-free, four candidates per trip (the tile is padded to a multiple of 4 with far-away sentinels): about 4 of 5
+// Branch-free, two candidates per trip (the tile is padded to an even count with a far-away sentinel): about 9 of 10
 // culled candidates are accepted by some lane, so predicated appends beat a vote-and-branch per candidate.
-// tile[t] = (x, y, z, h_j^2).  SELF: the tile holds the query leaf itself, so j = i has to be excluded.
+// SELF: the tile holds the query leaf itself, so j = i has to be excluded (and every candidate keeps its slot).
 template <bool WRAP, bool SELF>
-__device__ __forceinline__ int test_tile(WarpSmem& S, int fill, int C, int& g, int& s, int lane, uint32_t self, float xi,
-                                         float yi, float zi, float hi2, float L, float half) {
-    uint32_t gp = smem_u32(&S.queue[g][lane]);                  // next gather entry of this lane (row stride 64 bytes)
-    uint32_t sp = smem_u32(&S.queue[CRK_QCAP - 1 - s][lane]);   // next symmetric-only entry (stack from the top)
+__device__ __forceinline__ int test_tile(WarpSmem& S, int fill, int C, int& g, int& ng, bool& wflag, int lane, uint32_t self,
+                                         float xi, float yi, float zi, float hi2, float L, float half) {
+    uint32_t gp = smem_u32(&S.queue[g][lane]);                  // next entry of this lane (row stride 64 bytes)
     uint32_t cp = smem_u32(&S.cand[C]);
-    for (int t0 = 0; t0 < fill; t0 += 4) {
-        bool ag[4], as[4], wrapped[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const float4 pj = S.tile[t0 + u];
-            float dx = __fsub_rn(xi, pj.x), dy = __fsub_rn(yi, pj.y), dz = __fsub_rn(zi, pj.z);
-            wrapped[u] = false;
-            if (WRAP) {
-                const float wx = wrap1(dx, L, half), wy = wrap1(dy, L, half), wz = wrap1(dz, L, half);
-                wrapped[u] = (wx != dx) || (wy != dy) || (wz != dz);
-                dx = wx; dy = wy; dz = wz;
-            }
-            const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
-            ag[u] = r2 < hi2;                                              // gather: Eqs. 13-14
-            as[u] = r2 < fmaxf(hi2, pj.w);                                 // symmetric: Eqs. 17-18
-            if (SELF) {
-                const bool notself = S.tidx[t0 + u] != self;
-                ag[u] = ag[u] && notself;
-                as[u] = as[u] && notself;
-            }
+    const float2 xi2 = make_float2(xi, xi), yi2 = make_float2(yi, yi), zi2 = make_float2(zi, zi);
+    for (int t0 = 0; t0 < fill; t0 += 2) {
+        const float4 pa = S.ta[t0 >> 1], pb = S.tb[t0 >> 1];
+        const uint2 ji = *(const uint2*)&S.tidx[t0];
+        float2 dx = __fadd2_rn(xi2, make_float2(pa.x, pa.y));    // x_i - x_j (the tile holds -x_j)
+        float2 dy = __fadd2_rn(yi2, make_float2(pa.z, pa.w));
+        float2 dz = __fadd2_rn(zi2, make_float2(pb.x, pb.y));
+        bool wr[2] = {false, false};
+        if (WRAP) {
+            dx = wrap2(dx, L, half, wr[0], wr[1]);
+            dy = wrap2(dy, L, half, wr[0], wr[1]);
+            dz = wrap2(dz, L, half, wr[0], wr[1]);
         }
-        const uint4 ji = *(const uint4*)&S.tidx[t0];
-        const uint32_t jv[4] = {ji.x, ji.y, ji.z, ji.w};
+        const float2 r2v = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+        const float r2[2] = {r2v.x, r2v.y}, hj2[2] = {pb.z, pb.w};
+        const uint32_t jv[2] = {ji.x, ji.y};
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-            const bool any = SELF || __any_sync(0xffffffffu, as[u]);      // the leaf's own particles always get a slot
-            const uint32_t e = (uint32_t)C | (wrapped[u] ? CRK_ELL_WRAP : 0u);
-            sts_u16_if(ag[u] ? gp : sp, e, as[u]);                         // one predicated store, no branch
-            gp += ag[u] ? 64u : 0u;
-            sp -= (as[u] && !ag[u]) ? 64u : 0u;
+        for (int u = 0; u < 2; ++u) {
+            bool ag = r2[u] < hi2;                                         // gather: Eqs. 13-14
+            bool as = r2[u] < fmaxf(hi2, hj2[u]);                          // symmetric: Eqs. 17-18
+            if (SELF) {
+                const bool notself = jv[u] != self;
+                ag = ag && notself;
+                as = as && notself;
+            }
+            const bool any = SELF || __any_sync(0xffffffffu, as);         // the leaf's own particles always get a slot
+            const uint32_t e = (uint32_t)C | (wr[u] ? CRK_ELL_WRAP : 0u) | (ag ? 0u : CRK_ELL_SYM);
+            sts_u16_if(gp, e, as);                                         // one predicated store, no branch
+            gp += as ? 64u : 0u;
+            ng += ag ? 1 : 0;
+            if (WRAP) wflag = wflag || (wr[u] && as);
             sts_u32_if(cp, jv[u], any && lane == 0);
             cp += any ? 4u : 0u;
             C += any ? 1 : 0;
         }
     }
     g = (int)((gp - smem_u32(&S.queue[0][lane])) >> 6);
-    s = (int)((smem_u32(&S.queue[CRK_QCAP - 1][lane]) - sp) >> 6);
     return C;
 }
 
@@ -124,54 +133,58 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
     const float4 blo = a.leaf_lo[leaf], bhi = a.leaf_hi[leaf];
     const float hq2 = __fmul_rn(blo.w, blo.w);
     const uint32_t lt = (1u << lane) - 1u;
-    int C = 0, g = 0, s = 0, fill = 0;
-    bool cwrap = false;
+    int C = 0, g = 0, ng = 0, fill = 0;   // candidates of the segment, entries / gather entries of this lane, staged candidates
+    bool cwrap = false, wflag = false;   // wflag: this lane owns an entry of the segment that crosses the periodic boundary
     uint32_t prev = 0, first = 0;   // arena units of the previous / first segment header of this leaf
 
+    auto put = [&](int slot, float x, float y, float z, float h2, uint32_t idx) {
+        float* fa = (float*)&S.ta[slot >> 1] + (slot & 1);
+        float* fb = (float*)&S.tb[slot >> 1] + (slot & 1);
+        fa[0] = -x; fa[2] = -y; fb[0] = -z; fb[2] = h2;
+        S.tidx[slot] = idx;
+    };
     auto emit = [&]() {
-        const int Kg = __reduce_max_sync(0xffffffffu, g);
-        const int K = __reduce_max_sync(0xffffffffu, g + s);
-        const unsigned long long units = CRK_SEG_HDR_UNITS + (unsigned long long)((C + 3) >> 2) + 4ull * K;
+        const int K = __reduce_max_sync(0xffffffffu, g);
+        const bool segwrap = __any_sync(0xffffffffu, wflag);
+        const bool head = (prev == 0);   // a leaf's first segment keeps its candidates in the dense per-leaf array
+        const unsigned long long units = CRK_SEG_HDR_UNITS + (head ? 0ull : (unsigned long long)((C + 3) >> 2)) + 4ull * K;
         unsigned long long base = 0;
         if (lane == 0) base = atomicAdd(a.counter, units);
         base = __shfl_sync(0xffffffffu, base, 0);
         __syncwarp();
         if (base + units <= a.arena_cap) {
             uint4* hdr = a.arena + base;
-            if (lane == 0) hdr[0] = make_uint4(0u, (uint32_t)C | ((uint32_t)Kg << 16), (uint32_t)K, 0u);
-            ((uint16_t*)(hdr + 1))[lane] = (uint16_t)g;
-            ((uint16_t*)(hdr + 5))[lane] = (uint16_t)(g + s);
-            uint32_t* cd = (uint32_t*)(hdr + CRK_SEG_HDR_UNITS);
+            const uint32_t h1 = (uint32_t)C | (segwrap ? CRK_SEG_WRAP : 0u) | ((uint32_t)K << 16);
+            if (lane == 0) hdr[0] = make_uint4(0u, h1, 0u, 0u);
+            ((uint16_t*)(hdr + 1))[lane] = (uint16_t)ng;
+            ((uint16_t*)(hdr + 5))[lane] = (uint16_t)g;
+            uint32_t* cd = head ? a.cand_first + leaf * CRK_CAND_STRIDE : (uint32_t*)(hdr + CRK_SEG_HDR_UNITS);
             for (int c = lane; c < C; c += 32) cd[c] = S.cand[c];
-            uint16_t* el = (uint16_t*)(hdr + CRK_SEG_HDR_UNITS + ((C + 3) >> 2));
-            for (int k = 0; k < K; ++k) {
-                uint16_t v = 0u;   // padding of shorter lanes: slot 0 (the sweeps prefetch it, never evaluate it)
-                if (k < g) v = S.queue[k][lane];
-                else if (k < g + s) v = S.queue[CRK_QCAP - 1 - (k - g)][lane];
-                el[k * 32 + lane] = v;
-            }
-            if (prev == 0) {
-                if (lane == 0) a.seg_first[leaf] = make_uint4(0u, (uint32_t)C | ((uint32_t)Kg << 16), (uint32_t)K, (uint32_t)base);
-                a.leaf_cnt[leaf * 64 + lane] = (uint16_t)g;
-                a.leaf_cnt[leaf * 64 + 32 + lane] = (uint16_t)(g + s);
+            uint16_t* el = (uint16_t*)(hdr + CRK_SEG_HDR_UNITS + (head ? 0 : ((C + 3) >> 2)));
+            for (int k = 0; k < K; ++k)   // padding of shorter lanes: slot 0 (the sweeps prefetch it, never evaluate it)
+                el[k * 32 + lane] = (k < g) ? S.queue[k][lane] : (uint16_t)0u;
+            if (head) {
+                if (lane == 0) a.seg_first[leaf] = make_uint4(0u, h1, 0u, (uint32_t)base);
+                a.leaf_cnt[leaf * 64 + lane] = (uint16_t)ng;
+                a.leaf_cnt[leaf * 64 + 32 + lane] = (uint16_t)g;
                 first = (uint32_t)base;
             } else if (lane == 0) {
                 ((uint32_t*)(a.arena + prev))[0] = (uint32_t)base;
                 if (prev == first) ((uint32_t*)(a.seg_first + leaf))[0] = (uint32_t)base;
             }
             prev = (uint32_t)base;
-        }
-        C = 0; g = 0; s = 0;
+        }   // else: arena overflow -- the host re-runs the kernel with a larger arena; the counter keeps the total need
+        C = 0; g = 0; ng = 0; wflag = false;
         __syncwarp();
     };
     auto flush = [&](bool selftile) {
-        const int maxlen = __reduce_max_sync(0xffffffffu, g + s);
+        const int maxlen = __reduce_max_sync(0xffffffffu, g);
         if (C + fill > CRK_CCAP || maxlen + fill > CRK_QCAP) emit();
-        if (lane < ((4 - fill) & 3)) S.tile[fill + lane] = make_float4(3.0e30f, 3.0e30f, 3.0e30f, 0.0f);
+        if ((fill & 1) && lane == 0) put(fill, 3.0e30f, 3.0e30f, 3.0e30f, 0.0f, 0u);
         __syncwarp();
-        if (selftile) C = test_tile<true, true>(S, fill, C, g, s, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
-        else if (cwrap) C = test_tile<true, false>(S, fill, C, g, s, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
-        else C = test_tile<false, false>(S, fill, C, g, s, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
+        if (selftile) C = test_tile<true, true>(S, fill, C, g, ng, wflag, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
+        else if (cwrap) C = test_tile<true, false>(S, fill, C, g, ng, wflag, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
+        else C = test_tile<false, false>(S, fill, C, g, ng, wflag, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
         fill = 0;
         cwrap = false;
         __syncwarp();
@@ -182,8 +195,7 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
     float4 pj = (e0 < e1) ? a.posh[(int64_t)(ent & CRK_LEAF_MASK) * CRK_LEAF + lane] : make_float4(0, 0, 0, 0);
     // the query leaf itself goes first and keeps all 32 particles: slots 0..31 of the first segment are the leaf's own
     // particles in lane order, so a sweep finds the i-state of its lanes in the tile it stages anyway
-    S.tile[lane] = make_float4(xi, yi, zi, hi2);
-    S.tidx[lane] = (uint32_t)i;
+    put(lane, xi, yi, zi, hi2, (uint32_t)i);
     fill = 32;
     flush(true);
     for (uint64_t e = e0; e < e1; ++e) {
@@ -209,11 +221,7 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
         if (cnt == 0) continue;
         if (b == leaf) continue;                                         // done first
         if (fill + cnt > CRK_TCULL) flush(false);
-        const int slot = fill + __popc(m & lt);
-        if (surv) {
-            S.tile[slot] = make_float4(pc.x, pc.y, pc.z, hj2);
-            S.tidx[slot] = (uint32_t)(b * CRK_LEAF + lane);
-        }
+        if (surv) put(fill + __popc(m & lt), pc.x, pc.y, pc.z, hj2, (uint32_t)(b * CRK_LEAF + lane));
         cwrap = cwrap || wrap;
         fill += cnt;
     }
@@ -230,8 +238,9 @@ int crk_build_nbr_lists(crk_ctx* c) {
     const int64_t nl = c->nl;
     CRK_TRY(crk_ensure(c, c->seg_first, (size_t)(nl + 1) * sizeof(uint4)));
     CRK_TRY(crk_ensure(c, c->leaf_cnt, (size_t)(nl + 1) * 64 * sizeof(uint16_t)));
-    // first guess: ~7 KB per leaf at ~60 neighbours; grown to the exact need if the builder reports more
-    if (!c->arena.p) CRK_TRY(crk_ensure(c, c->arena, (size_t)nl * 9216 + 65536));
+    CRK_TRY(crk_ensure(c, c->cand_first, (size_t)(nl + 1) * CRK_CAND_STRIDE * sizeof(uint32_t)));
+    // first guess: ~6 KB per leaf at ~60 neighbours; grown to the exact need if the builder reports more
+    if (!c->arena.p) CRK_TRY(crk_ensure(c, c->arena, (size_t)nl * 7168 + 65536));
     unsigned long long* d_counter = (unsigned long long*)((char*)c->flag.p + 32);
     unsigned long long* h_counter = (unsigned long long*)((char*)c->h_flag + 32);
     for (int attempt = 0; attempt < 3; ++attempt) {
@@ -240,11 +249,14 @@ int crk_build_nbr_lists(crk_ctx* c) {
         a.cnt = (const uint32_t*)c->nbr_cnt.p; a.list = (const uint32_t*)c->nbr_list.p; a.cap = (uint32_t)c->leaf_list_cap;
         a.posh = (const float4*)c->posh.p; a.leaf_lo = (const float4*)c->leaf_lo.p; a.leaf_hi = (const float4*)c->leaf_hi.p;
         a.arena = (uint4*)c->arena.p;
+        // the sweeps read whole 16-byte groups of candidate indices and prefetch entry rows: keep a tail margin
         a.arena_cap = (unsigned long long)(c->arena.cap / 16);
+        a.arena_cap = a.arena_cap > 256 ? a.arena_cap - 256 : 0;
         if (a.arena_cap > 0xffffffffull) a.arena_cap = 0xffffffffull;      // segment links are 32-bit unit indices (64 GB)
         a.counter = d_counter;
         a.seg_first = (uint4*)c->seg_first.p;
         a.leaf_cnt = (uint16_t*)c->leaf_cnt.p;
+        a.cand_first = (uint32_t*)c->cand_first.p;
         k_set_u64<<<1, 1, 0, c->stream>>>(d_counter, 1ull);
         CRK_TRY(crk_check_launch(c, "k_set_u64"));
         k_nbr_lists<<<(unsigned)((nl + LW - 1) / LW), LW * 32, 0, c->stream>>>(a);

@@ -26,6 +26,7 @@ struct SweepArgs {
     const uint4* __restrict__ arena;      // neighbour-list segments
     const uint4* __restrict__ seg_first;  // dense copy of each leaf's first segment header (.w = its arena unit, 0 = none)
     const uint16_t* __restrict__ leaf_cnt;  // [nl][64] per-lane cnt_g | cnt of the first segment
+    const uint32_t* __restrict__ cand_first; // [nl][CRK_CAND_STRIDE] candidate indices of the first segment
     const int32_t* __restrict__ perm;     // sorted slot -> caller index
     const float4* __restrict__ posh;      // (x,y,z,h)
     float4* __restrict__ posV;            // (x,y,z,V)
@@ -45,34 +46,36 @@ struct SweepArgs {
 struct Seg {
     const uint32_t* cand;
     const uint16_t* ell;
-    int C, Kg, K, cg, ct;
+    int C, K, cg, ct;
+    bool wrap;               // some entry of the segment may cross the periodic boundary
     uint32_t next;
 };
-__device__ __forceinline__ Seg make_seg(const uint4* __restrict__ arena, uint32_t unit, const uint4& h0, int cg, int ct) {
+// dense: candidate array of a leaf's first segment (cand_first), else the candidates follow the header in the arena
+__device__ __forceinline__ Seg make_seg(const uint4* __restrict__ arena, uint32_t unit, const uint4& h0, int cg, int ct,
+                                        const uint32_t* dense) {
     const uint4* hdr = arena + unit;
     Seg s;
     s.next = h0.x;
-    s.C = (int)(h0.y & 0xffffu);
-    s.Kg = (int)(h0.y >> 16);
-    s.K = (int)h0.z;
+    s.C = (int)(h0.y & 0x7fffu);
+    s.wrap = (h0.y & CRK_SEG_WRAP) != 0u;
+    s.K = (int)(h0.y >> 16);
     s.cg = cg;
     s.ct = ct;
-    s.cand = (const uint32_t*)(hdr + CRK_SEG_HDR_UNITS);
-    s.ell = (const uint16_t*)(hdr + CRK_SEG_HDR_UNITS + ((s.C + 3) >> 2));
+    s.cand = dense ? dense : (const uint32_t*)(hdr + CRK_SEG_HDR_UNITS);
+    s.ell = (const uint16_t*)(hdr + CRK_SEG_HDR_UNITS + (dense ? 0 : ((s.C + 3) >> 2)));
     return s;
 }
-// first segment: header and per-lane counts come from the dense per-leaf arrays (no dependent load before the payload)
-__device__ __forceinline__ Seg first_seg(const uint4* __restrict__ arena, const uint4* __restrict__ seg_first,
-                                         const uint16_t* __restrict__ leaf_cnt, int64_t leaf, int lane, uint32_t& unit) {
-    const uint4 h0 = __ldg(seg_first + leaf);
-    const int cg = (int)__ldg(leaf_cnt + leaf * 64 + lane), ct = (int)__ldg(leaf_cnt + leaf * 64 + 32 + lane);
+// first segment: header, per-lane counts and candidates come from the dense per-leaf arrays (no dependent load before the payload)
+__device__ __forceinline__ Seg first_seg(const SweepArgs& a, int64_t leaf, int lane, uint32_t& unit) {
+    const uint4 h0 = __ldg(a.seg_first + leaf);
+    const int cg = (int)__ldg(a.leaf_cnt + leaf * 64 + lane), ct = (int)__ldg(a.leaf_cnt + leaf * 64 + 32 + lane);
     unit = h0.w;
-    return make_seg(arena, unit, h0, cg, ct);
+    return make_seg(a.arena, unit, h0, cg, ct, a.cand_first + leaf * CRK_CAND_STRIDE);
 }
 __device__ __forceinline__ Seg load_seg(const uint4* __restrict__ arena, uint32_t unit, int lane) {
     const uint4* hdr = arena + unit;
     const uint4 h0 = __ldg(hdr);
-    return make_seg(arena, unit, h0, (int)__ldg((const uint16_t*)(hdr + 1) + lane), (int)__ldg((const uint16_t*)(hdr + 5) + lane));
+    return make_seg(arena, unit, h0, (int)__ldg((const uint16_t*)(hdr + 1) + lane), (int)__ldg((const uint16_t*)(hdr + 5) + lane), nullptr);
 }
 
 __device__ __forceinline__ void cp_async16(uint32_t dst_shared, const void* src) {
@@ -112,28 +115,34 @@ __device__ __forceinline__ void group_sync(int lg) {
 }
 
 // ---- the sweep over one leaf's segment chain -------------------------------------------------------------------------
-// SYM = false: rows [0, Kg), lane active while k < cnt_g (gather set, Eqs. 13-14);  SYM = true: rows [0, K), k < cnt.
+// Rows [0, K) of a segment's entry block; lane l is active while k < cnt[l].  SYM = false (gather set, Eqs. 13-14): entries
+// flagged CRK_ELL_SYM are skipped;  SYM = true (Eqs. 17-18): every entry is a pair.
 // pair(slot_addr, crosses_boundary, plane0) evaluates one accepted pair (slot_addr = shared address of the candidate's
-// plane-0 entry; plane p sits CRK_CCAP * 16 * p bytes further); returns the number of entries the lane owns (= its count).
+// plane-0 entry; plane p sits CRK_CCAP * 16 * p bytes further); returns the number of pairs the lane owns.
 struct NoInit {
     __device__ __forceinline__ void operator()(uint32_t) const {}
 };
 // init(tile_s) runs once, after the first segment is staged: slots 0..31 of that tile are the leaf's own particles in lane
-// order (lists.cu), so a sweep can take its i-state from there instead of loading it from global memory
+// order (lists.cu), so a sweep can take its i-state from there instead of loading it from global memory.
+// (Measured and not kept, profiles/r02_notes.md: a second, branch-free instantiation of the row loop for segments without
+// boundary-crossing entries -- 172 instead of 190 instructions per pair of k_forces, but ptxas then sinks the shared loads
+// next to their uses and the sweep loses 1.6 ms to short-scoreboard stalls; candidate indices fetched as 16-byte groups
+// ahead of the header -- +0.5 ms.)
 template <int WPL, int PLANES, bool SYM, int NPRE = 1, typename Pair, typename Init = NoInit>
 __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4* const* planes, int64_t leaf, int lg, int wl,
                                                int lane, float4* tile, Pair pair, Init init = Init()) {
+    constexpr int NT = WPL * 32;                                  // threads that serve the leaf
     uint32_t count = 0;
     bool first = true;
     const int tg = wl * 32 + lane;
     const uint32_t tile_s = (uint32_t)__cvta_generic_to_shared(tile);
     uint32_t unit;
-    Seg s = first_seg(a.arena, a.seg_first, a.leaf_cnt, leaf, lane, unit);
+    Seg s = first_seg(a, leaf, lane, unit);
     while (unit != 0u) {
-        const int rows = SYM ? s.K : s.Kg;
-        const int mine = SYM ? s.ct : s.cg;
+        const int rows = s.K;
+        const int mine = s.ct;
         const uint16_t* ep = s.ell + lane;
-        // the first rows of the ELL block travel together with the candidate indices
+        // the first rows of the entry block travel together with the candidate indices
         uint32_t e[4];
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
@@ -142,8 +151,8 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
         }
         group_sync<WPL>(lg);                                   // the previous segment's drain is finished
         // stage: 16-byte asynchronous copies global -> shared (LDGSTS), no register round trip
-        for (int c0 = 0; c0 < s.C; c0 += WPL * 32 * 2) {
-            const int ca = c0 + tg, cb = ca + WPL * 32;
+        for (int c0 = 0; c0 < s.C; c0 += NT * 2) {
+            const int ca = c0 + tg, cb = ca + NT;
             const uint32_t ja = (ca < s.C) ? __ldg(s.cand + ca) : 0u;
             const uint32_t jb = (cb < s.C) ? __ldg(s.cand + cb) : 0u;
             if (ca < s.C) {
@@ -180,14 +189,15 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
                 float4 nxt[NPRE];
 #pragma unroll
                 for (int p = 0; p < NPRE; ++p) nxt[p] = lds128(tile_s + (uint32_t)(p * CRK_CCAP) * 16u + (en & CRK_ELL_MASK) * 16u);
-                if (k < mine) pair(tile_s + (e[q] & CRK_ELL_MASK) * 16u, (e[q] & CRK_ELL_WRAP) != 0u, cur);
+                if (k < mine && (SYM || !(e[q] & CRK_ELL_SYM)))
+                    pair(tile_s + (e[q] & CRK_ELL_MASK) * 16u, (e[q] & CRK_ELL_WRAP) != 0u, cur);
 #pragma unroll
                 for (int p = 0; p < NPRE; ++p) cur[p] = nxt[p];
             }
 #pragma unroll
             for (int q = 0; q < 4; ++q) e[q] = nx[q];
         }
-        count += (uint32_t)mine;
+        count += (uint32_t)(SYM ? s.ct : s.cg);
         unit = s.next;
         if (unit != 0u) s = load_seg(a.arena, unit, lane);
     }
@@ -294,146 +304,6 @@ __global__ void __launch_bounds__(W1_WPC * 32) k_volumes(SweepArgs a) {
     }
 }
 
-// ========================================================================================== a2 + a3: RK coefficients
-// PAPER.md:116: A, B from  sum_j V_j WR_ij = 1,  sum_j V_j x_ij WR_ij = 0.  With moments over the gather set
-//   m0 = sum w, m1 = sum w x, m2 = sum w x x  (w = V_j W_ij, self term in m0 only) and their gradients
-//   d_c m0 = sum g x_c, d_c m1_a = sum g x_a x_c + delta_ac m0, d_c m2_ab = sum g x_a x_b x_c + delta_ac m1_b + delta_bc m1_a
-//   (g = V_j W'_ij / r):   B = -m2^-1 m1,  A = 1/(m0 + B.m1),
-//   d_c A = -A^2 (d_c m0 + 2 B.d_c m1 + B^T d_c m2 B),  d_c B = -m2^-1 (d_c m1 + d_c m2 B).
-// 29 FP32 sums per particle in eta-normalised units, then an FP64 3x3 solve per particle.
-constexpr int W2_WPC = 2;
-__global__ void __launch_bounds__(W2_WPC * 32, 12) k_moments(SweepArgs a) {
-    extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int64_t leaf = (int64_t)blockIdx.x * W2_WPC + w;
-    if (leaf >= a.nl) return;
-    float4* tile = (float4*)smem_raw + (size_t)w * CRK_CCAP;
-    const int64_t i = leaf * CRK_LEAF + lane;
-    const bool valid = i < a.n;
-    const float4 ph = a.posh[i];
-    const float xi = ph.x, yi = ph.y, zi = ph.z, hi = ph.w;
-    const float inv_h = valid ? 1.0f / hi : 0.0f;
-    // accumulators: s0; s1[3]; s2[6] (xx,xy,xz,yy,yz,zz); t0[3]; t1[6]; t2[10] (xxx,xxy,xxz,xyy,xyz,xzz,yyy,yyz,yzz,zzz)
-    float s0 = 0.f, s1x = 0.f, s1y = 0.f, s1z = 0.f;
-    float sxx = 0.f, sxy = 0.f, sxz = 0.f, syy = 0.f, syz = 0.f, szz = 0.f;
-    float t0x = 0.f, t0y = 0.f, t0z = 0.f;
-    float txx = 0.f, txy = 0.f, txz = 0.f, tyy = 0.f, tyz = 0.f, tzz = 0.f;
-    float c0 = 0.f, c1 = 0.f, c2 = 0.f, c3 = 0.f, c4 = 0.f, c5 = 0.f, c6 = 0.f, c7 = 0.f, c8 = 0.f, c9 = 0.f;
-    const float4* const planes[1] = {a.posV};
-    leaf_sweep<1, 1, false>(a, planes, leaf, w, 0, lane, tile, [&](uint32_t, bool wrapped, const float4* pre) {
-        const float4 pj = pre[0];
-        float dx, dy, dz, r2;
-        sep3(a, wrapped, xi, yi, zi, pj, dx, dy, dz, r2);
-        const float r = r2 * rsqrt_fast(fmaxf(r2, R2_TINY));
-        float Wt, Dt;
-        wendland(r * inv_h, Wt, Dt);
-        const float wv = pj.w * Wt, gv = pj.w * Dt;
-        const float x = dx * inv_h, y = dy * inv_h, z = dz * inv_h;
-        const float xx = x * x, xy = x * y, xz = x * z, yy = y * y, yz = y * z, zz = z * z;
-        s0 += wv;
-        s1x = fmaf(wv, x, s1x); s1y = fmaf(wv, y, s1y); s1z = fmaf(wv, z, s1z);
-        sxx = fmaf(wv, xx, sxx); sxy = fmaf(wv, xy, sxy); sxz = fmaf(wv, xz, sxz);
-        syy = fmaf(wv, yy, syy); syz = fmaf(wv, yz, syz); szz = fmaf(wv, zz, szz);
-        t0x = fmaf(gv, x, t0x); t0y = fmaf(gv, y, t0y); t0z = fmaf(gv, z, t0z);
-        txx = fmaf(gv, xx, txx); txy = fmaf(gv, xy, txy); txz = fmaf(gv, xz, txz);
-        tyy = fmaf(gv, yy, tyy); tyz = fmaf(gv, yz, tyz); tzz = fmaf(gv, zz, tzz);
-        c0 = fmaf(gv, xx * x, c0); c1 = fmaf(gv, xx * y, c1); c2 = fmaf(gv, xx * z, c2);
-        c3 = fmaf(gv, xy * y, c3); c4 = fmaf(gv, xy * z, c4); c5 = fmaf(gv, xz * z, c5);
-        c6 = fmaf(gv, yy * y, c6); c7 = fmaf(gv, yy * z, c7); c8 = fmaf(gv, yz * z, c8);
-        c9 = fmaf(gv, zz * z, c9);
-    });
-    float4 o0 = make_float4(0, 0, 0, 0), o1 = o0, o2 = o0, o3 = o0;
-    if (valid) {
-        // ---- a3: FP64 solve (dimensional quantities; k3 = sigma/h^3)
-        const double h = (double)hi, ih = 1.0 / h;
-        const double k3 = (double)SIGMA_C4 * ih * ih * ih;
-        const double Vi = (double)a.posV[i].w;
-        const double m0 = k3 * ((double)s0 + Vi);
-        const double m1[3] = {k3 * h * s1x, k3 * h * s1y, k3 * h * s1z};
-        const double k3h2 = k3 * h * h;
-        const double m2[3][3] = {{k3h2 * sxx, k3h2 * sxy, k3h2 * sxz},
-                                 {k3h2 * sxy, k3h2 * syy, k3h2 * syz},
-                                 {k3h2 * sxz, k3h2 * syz, k3h2 * szz}};
-        const double dm0[3] = {k3 * ih * t0x, k3 * ih * t0y, k3 * ih * t0z};
-        // sum g x_a x_c (symmetric)
-        const double q1[3][3] = {{k3 * txx, k3 * txy, k3 * txz}, {k3 * txy, k3 * tyy, k3 * tyz}, {k3 * txz, k3 * tyz, k3 * tzz}};
-        const double k3h = k3 * h;
-        const double cc[10] = {k3h * c0, k3h * c1, k3h * c2, k3h * c3, k3h * c4, k3h * c5, k3h * c6, k3h * c7, k3h * c8, k3h * c9};
-        // inverse of m2 (adjugate)
-        const double a00 = m2[1][1] * m2[2][2] - m2[1][2] * m2[1][2];
-        const double a01 = m2[0][2] * m2[1][2] - m2[0][1] * m2[2][2];
-        const double a02 = m2[0][1] * m2[1][2] - m2[0][2] * m2[1][1];
-        const double a11 = m2[0][0] * m2[2][2] - m2[0][2] * m2[0][2];
-        const double a12 = m2[0][1] * m2[0][2] - m2[0][0] * m2[1][2];
-        const double a22 = m2[0][0] * m2[1][1] - m2[0][1] * m2[0][1];
-        const double det = m2[0][0] * a00 + m2[0][1] * a01 + m2[0][2] * a02;
-        double A, B[3], dA[3], dB[3][3];   // dB[c][a] = d_c B^a
-        if (fabs(det) > 0.0 && isfinite(det)) {
-            const double id = 1.0 / det;
-            const double inv[3][3] = {{a00 * id, a01 * id, a02 * id}, {a01 * id, a11 * id, a12 * id}, {a02 * id, a12 * id, a22 * id}};
-#pragma unroll
-            for (int p = 0; p < 3; ++p) B[p] = -(inv[p][0] * m1[0] + inv[p][1] * m1[1] + inv[p][2] * m1[2]);
-            A = 1.0 / (m0 + B[0] * m1[0] + B[1] * m1[1] + B[2] * m1[2]);
-            // index of the symmetric cubic monomial x_a x_b x_c in cc[]
-            const int cub[3][3][3] = {{{0, 1, 2}, {1, 3, 4}, {2, 4, 5}}, {{1, 3, 4}, {3, 6, 7}, {4, 7, 8}}, {{2, 4, 5}, {4, 7, 8}, {5, 8, 9}}};
-#pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                double Bdm1 = 0.0, BdmB = 0.0, rhs[3];
-#pragma unroll
-                for (int p = 0; p < 3; ++p) {
-                    const double dm1_pc = q1[p][c] + (p == c ? m0 : 0.0);
-                    Bdm1 += B[p] * dm1_pc;
-                    double t = 0.0;
-#pragma unroll
-                    for (int q = 0; q < 3; ++q) {
-                        const double dm2_pqc = cc[cub[p][q][c]] + (p == c ? m1[q] : 0.0) + (q == c ? m1[p] : 0.0);
-                        t += dm2_pqc * B[q];
-                    }
-                    BdmB += B[p] * t;
-                    rhs[p] = dm1_pc + t;
-                }
-                dA[c] = -A * A * (dm0[c] + 2.0 * Bdm1 + BdmB);
-#pragma unroll
-                for (int p = 0; p < 3; ++p) dB[c][p] = -(inv[p][0] * rhs[0] + inv[p][1] * rhs[1] + inv[p][2] * rhs[2]);
-            }
-        } else {   // S14: degenerate neighbourhood -> zeroth-order correction only
-            A = 1.0 / m0;
-#pragma unroll
-            for (int c = 0; c < 3; ++c) {
-                B[c] = 0.0;
-                dA[c] = -A * A * dm0[c];
-                dB[c][0] = dB[c][1] = dB[c][2] = 0.0;
-            }
-        }
-        // pre-combined form used by the later sweeps:  (grad WR_ij)_c = W (cvec_c + M_ca x_a) + A s D x_c, s = 1 + B.x
-        //   cvec_c = d_c A + A B_c,   M_ca = d_c A B_a + A d_c B_a
-        o0 = make_float4((float)A, (float)B[0], (float)B[1], (float)B[2]);
-        float Mf[9];
-#pragma unroll
-        for (int c = 0; c < 3; ++c)
-#pragma unroll
-            for (int p = 0; p < 3; ++p) Mf[3 * c + p] = (float)(dA[c] * B[p] + A * dB[c][p]);
-        o1 = make_float4((float)(dA[0] + A * B[0]), (float)(dA[1] + A * B[1]), (float)(dA[2] + A * B[2]), Mf[0]);
-        o2 = make_float4(Mf[1], Mf[2], Mf[3], Mf[4]);
-        o3 = make_float4(Mf[5], Mf[6], Mf[7], Mf[8]);
-        const int32_t p = a.perm[i];
-        const int64_t n = a.n;
-        if (a.o0) a.o0[p] = (float)A;
-        if (a.o1) { a.o1[p] = (float)B[0]; a.o1[n + p] = (float)B[1]; a.o1[2 * n + p] = (float)B[2]; }
-        if (a.o2) { a.o2[p] = (float)dA[0]; a.o2[n + p] = (float)dA[1]; a.o2[2 * n + p] = (float)dA[2]; }
-        if (a.o3) {
-#pragma unroll
-            for (int c = 0; c < 3; ++c)
-#pragma unroll
-                for (int q = 0; q < 3; ++q) a.o3[(3 * c + q) * n + p] = (float)dB[c][q];
-        }
-    }
-    a.coef[i] = o0;
-    a.coef[a.np + i] = o1;
-    a.coef[2 * a.np + i] = o2;
-    a.coef[3 * a.np + i] = o3;
-}
-
 // ---- hydro preparation: sorted (vx,vy,vz,V), and force-sweep plane 0 = (x,y,z,1/h) -----------------------------------
 __global__ void __launch_bounds__(256) k_pack_vel(const float* __restrict__ vx, const float* __restrict__ vy,
                                                   const float* __restrict__ vz, const float* __restrict__ u, int64_t n,
@@ -495,62 +365,242 @@ __device__ __forceinline__ void wendland_dim(float r, float ih, float k3, float 
     D = __fmul_rn(k5, Dt);
 }
 
-// =============================================================================================== a4: velocity gradient
-// Eq. 26: grad v_i = - sum_j V_j (v_i - v_j) (x) grad WR_ij   over the gather set; index [3a+b] = d_b v^a.
-// The epilogue also forms P = (gamma-1) rho u (Eq. 4, unclamped) and c_s = sqrt(gamma (gamma-1) max(u,0)) (S12) and writes
-// the packed force-sweep state of the particle.
-constexpr int W4_WPL = 1, W4_LPC = 4;
-__global__ void __launch_bounds__(W4_WPL * W4_LPC * 32) k_gradv(SweepArgs a, const float* __restrict__ u_s, float* __restrict__ gv_full) {
+// ================================================================== a2 + a3 + a4: RK coefficients and velocity gradient
+// PAPER.md:116: A, B from  sum_j V_j WR_ij = 1,  sum_j V_j x_ij WR_ij = 0.  With moments over the gather set
+//   m0 = sum w, m1 = sum w x, m2 = sum w x x  (w = V_j W_ij, self term in m0 only) and their gradients
+//   d_c m0 = sum g x_c, d_c m1_a = sum g x_a x_c + delta_ac m0, d_c m2_ab = sum g x_a x_b x_c + delta_ac m1_b + delta_bc m1_a
+//   (g = V_j W'_ij / r):   B = -m2^-1 m1,  A = 1/(m0 + B.m1),
+//   d_c A = -A^2 (d_c m0 + 2 B.d_c m1 + B^T d_c m2 B),  d_c B = -m2^-1 (d_c m1 + d_c m2 B).
+// 29 FP32 sums per particle in eta-normalised units, then an FP64 3x3 solve per particle (a3).
+//
+// Eq. 26: grad v_i = - sum_j V_j (v_i - v_j) (x) grad WR_ij over the same gather set; index [3a+b] = d_b v^a.
+// grad WR_ij = W (cvec + M x) + A (1 + B.x) D x is linear in the coefficients of particle i, so the sweep accumulates 39
+// velocity-weighted sums that do not need them (u = v_i - v_j, w = V_j W, g = V_j D):
+//   S0^a = sum u^a w (3),  S1^ac = sum u^a w x^c (9),  T1^ab = sum u^a g x^b (9),  T2^a(cb) = sum u^a g x^c x^b (3 x 6)
+// and the epilogue contracts  (grad v)^ab = -(cvec_b S0^a + M_bc S1^ac + A T1^ab + A B_c T2^acb)  with the stored FP32
+// coefficients.  MOM && GV (crk_step_derivs): one sweep does both, so the lists and the tile are read once.  The
+// accumulation code of each sum is the same in all three instantiations (explicit round-to-nearest intrinsics, nothing for
+// the compiler to contract differently), so the staged calls and crk_step_derivs produce identical bits.
+// The epilogue with GV also forms P = (gamma-1) rho u (Eq. 4, unclamped) and c_s = sqrt(gamma (gamma-1) max(u,0)) (S12) and
+// writes the packed force-sweep state of the particle.
+#ifndef CRK_RK_MINB
+#define CRK_RK_MINB 8
+#endif
+constexpr int W2_WPC = 2;
+template <bool MOM, bool GV>
+__global__ void __launch_bounds__(W2_WPC * 32, (MOM && GV) ? CRK_RK_MINB : (GV ? 8 : 10))
+k_rk(SweepArgs a, const float* __restrict__ u_s, float* __restrict__ gv_full) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int PL = GV ? 2 : 1;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int lg = w / W4_WPL, wl = w % W4_WPL;
-    const int64_t leaf = (int64_t)blockIdx.x * W4_LPC + lg;
+    const int64_t leaf = (int64_t)blockIdx.x * W2_WPC + w;
     if (leaf >= a.nl) return;
-    float4* tile = (float4*)smem_raw + (size_t)lg * 2 * CRK_CCAP;
+    float4* tile = (float4*)smem_raw + (size_t)w * PL * CRK_CCAP;
     const int64_t i = leaf * CRK_LEAF + lane;
     const bool valid = i < a.n;
     const float4 ph = a.posh[i];
     const float xi = ph.x, yi = ph.y, zi = ph.z, hi = ph.w;
-    const float ih = valid ? 1.0f / hi : 0.0f;
-    const float k3 = SIGMA_C4 * ih * ih * ih;
-    const float k5 = k3 * ih * ih;
-    const float4 vi = a.velV[i];
-    const float4 q0 = a.coef[i], q1 = a.coef[a.np + i], q2 = a.coef[2 * a.np + i], q3 = a.coef[3 * a.np + i];
-    const Coef ci = load_coef(q0, q1, q2, q3);
-    float g[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0};
-    const float4* const planes[2] = {a.posV, a.velV};
-    leaf_sweep<W4_WPL, 2, false>(a, planes, leaf, lg, wl, lane, tile, [&](uint32_t sa, bool wrapped, const float4* pre) {
+    const float inv_h = valid ? 1.0f / hi : 0.0f;
+    float4 vi = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (GV) vi = a.velV[i];
+    // moment accumulators: s0; s1[3]; s2[6] (xx,xy,xz,yy,yz,zz); t0[3]; t1[6]; t2[10] (xxx,xxy,xxz,xyy,xyz,xzz,yyy,yyz,yzz,zzz)
+    float s0 = 0.f, s1[3] = {0.f, 0.f, 0.f}, s2[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    float t0[3] = {0.f, 0.f, 0.f}, t1[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, t2[10] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+    // velocity sums, [a][..]
+    float S0[3], S1[3][3], T1[3][3], T2[3][6];
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+        S0[q] = 0.f;
+#pragma unroll
+        for (int r = 0; r < 3; ++r) { S1[q][r] = 0.f; T1[q][r] = 0.f; }
+#pragma unroll
+        for (int r = 0; r < 6; ++r) T2[q][r] = 0.f;
+    }
+    const float4* planes[2] = {a.posV, GV ? a.velV : a.posV};
+    leaf_sweep<1, PL, false>(a, planes, leaf, w, 0, lane, tile, [&](uint32_t sa, bool wrapped, const float4* pre) {
         const float4 pj = pre[0];
-        const float4 vj = lds128(sa + CRK_CCAP * 16u);
         float dx, dy, dz, r2;
         sep3(a, wrapped, xi, yi, zi, pj, dx, dy, dz, r2);
-        const float r = r2 * rsqrt_fast(fmaxf(r2, R2_TINY));
-        float W, D, gx, gy, gz;
-        wendland_dim(r, ih, k3, k5, W, D);
-        rk_grad(ci, dx, dy, dz, W, D, gx, gy, gz);
-        const float Vj = pj.w;
-        const float ux = Vj * (vi.x - vj.x), uy = Vj * (vi.y - vj.y), uz = Vj * (vi.z - vj.z);
-        g[0] = fmaf(-ux, gx, g[0]); g[1] = fmaf(-ux, gy, g[1]); g[2] = fmaf(-ux, gz, g[2]);
-        g[3] = fmaf(-uy, gx, g[3]); g[4] = fmaf(-uy, gy, g[4]); g[5] = fmaf(-uy, gz, g[5]);
-        g[6] = fmaf(-uz, gx, g[6]); g[7] = fmaf(-uz, gy, g[7]); g[8] = fmaf(-uz, gz, g[8]);
+        const float r = __fmul_rn(r2, rsqrt_fast(fmaxf(r2, R2_TINY)));
+        float Wt, Dt;
+        wendland(__fmul_rn(r, inv_h), Wt, Dt);
+        const float wv = __fmul_rn(pj.w, Wt), gv = __fmul_rn(pj.w, Dt);
+        const float x[3] = {__fmul_rn(dx, inv_h), __fmul_rn(dy, inv_h), __fmul_rn(dz, inv_h)};
+        const float m2[6] = {__fmul_rn(x[0], x[0]), __fmul_rn(x[0], x[1]), __fmul_rn(x[0], x[2]),
+                             __fmul_rn(x[1], x[1]), __fmul_rn(x[1], x[2]), __fmul_rn(x[2], x[2])};
+        if (MOM) {
+            s0 = __fadd_rn(s0, wv);
+#pragma unroll
+            for (int q = 0; q < 3; ++q) {
+                s1[q] = __fmaf_rn(wv, x[q], s1[q]);
+                t0[q] = __fmaf_rn(gv, x[q], t0[q]);
+            }
+            float g2[6];
+#pragma unroll
+            for (int q = 0; q < 6; ++q) {
+                s2[q] = __fmaf_rn(wv, m2[q], s2[q]);
+                g2[q] = __fmul_rn(gv, m2[q]);
+                t1[q] = __fadd_rn(t1[q], g2[q]);
+            }
+            t2[0] = __fmaf_rn(g2[0], x[0], t2[0]); t2[1] = __fmaf_rn(g2[0], x[1], t2[1]); t2[2] = __fmaf_rn(g2[0], x[2], t2[2]);
+            t2[3] = __fmaf_rn(g2[1], x[1], t2[3]); t2[4] = __fmaf_rn(g2[1], x[2], t2[4]); t2[5] = __fmaf_rn(g2[2], x[2], t2[5]);
+            t2[6] = __fmaf_rn(g2[3], x[1], t2[6]); t2[7] = __fmaf_rn(g2[3], x[2], t2[7]); t2[8] = __fmaf_rn(g2[4], x[2], t2[8]);
+            t2[9] = __fmaf_rn(g2[5], x[2], t2[9]);
+        }
+        if (GV) {
+            const float4 vj = lds128(sa + CRK_CCAP * 16u);
+            const float u[3] = {__fsub_rn(vi.x, vj.x), __fsub_rn(vi.y, vj.y), __fsub_rn(vi.z, vj.z)};
+#pragma unroll
+            for (int q = 0; q < 3; ++q) {
+                const float uw = __fmul_rn(u[q], wv), ug = __fmul_rn(u[q], gv);
+                S0[q] = __fadd_rn(S0[q], uw);
+#pragma unroll
+                for (int r = 0; r < 3; ++r) {
+                    S1[q][r] = __fmaf_rn(uw, x[r], S1[q][r]);
+                    T1[q][r] = __fmaf_rn(ug, x[r], T1[q][r]);
+                }
+#pragma unroll
+                for (int r = 0; r < 6; ++r) T2[q][r] = __fmaf_rn(ug, m2[r], T2[q][r]);
+            }
+        }
     });
-    group_reduce<W4_WPL, 9>(g, lg, wl, lane, (float*)tile);
-    if (wl != 0) return;
+    float4 o0 = make_float4(0, 0, 0, 0), o1 = o0, o2 = o0, o3 = o0;
+    const double h = (double)hi, ih = valid ? 1.0 / h : 0.0;
+    const double k3 = (double)SIGMA_C4 * ih * ih * ih;
+    if (MOM) {
+        if (valid) {
+            // ---- a3: FP64 solve (dimensional quantities; k3 = sigma/h^3)
+            const double Vi = (double)a.posV[i].w;
+            const double m0 = k3 * ((double)s0 + Vi);
+            const double m1[3] = {k3 * h * s1[0], k3 * h * s1[1], k3 * h * s1[2]};
+            const double k3h2 = k3 * h * h;
+            const double mm[3][3] = {{k3h2 * s2[0], k3h2 * s2[1], k3h2 * s2[2]},
+                                     {k3h2 * s2[1], k3h2 * s2[3], k3h2 * s2[4]},
+                                     {k3h2 * s2[2], k3h2 * s2[4], k3h2 * s2[5]}};
+            const double dm0[3] = {k3 * ih * t0[0], k3 * ih * t0[1], k3 * ih * t0[2]};
+            // sum g x_a x_c (symmetric)
+            const double q1[3][3] = {{k3 * t1[0], k3 * t1[1], k3 * t1[2]}, {k3 * t1[1], k3 * t1[3], k3 * t1[4]}, {k3 * t1[2], k3 * t1[4], k3 * t1[5]}};
+            const double k3h = k3 * h;
+            double cc[10];
+#pragma unroll
+            for (int q = 0; q < 10; ++q) cc[q] = k3h * t2[q];
+            // inverse of m2 (adjugate)
+            const double a00 = mm[1][1] * mm[2][2] - mm[1][2] * mm[1][2];
+            const double a01 = mm[0][2] * mm[1][2] - mm[0][1] * mm[2][2];
+            const double a02 = mm[0][1] * mm[1][2] - mm[0][2] * mm[1][1];
+            const double a11 = mm[0][0] * mm[2][2] - mm[0][2] * mm[0][2];
+            const double a12 = mm[0][1] * mm[0][2] - mm[0][0] * mm[1][2];
+            const double a22 = mm[0][0] * mm[1][1] - mm[0][1] * mm[0][1];
+            const double det = mm[0][0] * a00 + mm[0][1] * a01 + mm[0][2] * a02;
+            double A, B[3], dA[3], dB[3][3];   // dB[c][a] = d_c B^a
+            // S14: m2 counts as singular when det m2 <= 1e-4 (tr m2 / 3)^3 (neighbours span less than three dimensions)
+            const double tr3 = (mm[0][0] + mm[1][1] + mm[2][2]) * (1.0 / 3.0);
+            if (det > 1.0e-4 * tr3 * tr3 * tr3 && isfinite(det)) {
+                const double id = 1.0 / det;
+                const double inv[3][3] = {{a00 * id, a01 * id, a02 * id}, {a01 * id, a11 * id, a12 * id}, {a02 * id, a12 * id, a22 * id}};
+#pragma unroll
+                for (int p = 0; p < 3; ++p) B[p] = -(inv[p][0] * m1[0] + inv[p][1] * m1[1] + inv[p][2] * m1[2]);
+                A = 1.0 / (m0 + B[0] * m1[0] + B[1] * m1[1] + B[2] * m1[2]);
+                // index of the symmetric cubic monomial x_a x_b x_c in cc[]
+                const int cub[3][3][3] = {{{0, 1, 2}, {1, 3, 4}, {2, 4, 5}}, {{1, 3, 4}, {3, 6, 7}, {4, 7, 8}}, {{2, 4, 5}, {4, 7, 8}, {5, 8, 9}}};
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    double Bdm1 = 0.0, BdmB = 0.0, rhs[3];
+#pragma unroll
+                    for (int p = 0; p < 3; ++p) {
+                        const double dm1_pc = q1[p][c] + (p == c ? m0 : 0.0);
+                        Bdm1 += B[p] * dm1_pc;
+                        double t = 0.0;
+#pragma unroll
+                        for (int q = 0; q < 3; ++q) {
+                            const double dm2_pqc = cc[cub[p][q][c]] + (p == c ? m1[q] : 0.0) + (q == c ? m1[p] : 0.0);
+                            t += dm2_pqc * B[q];
+                        }
+                        BdmB += B[p] * t;
+                        rhs[p] = dm1_pc + t;
+                    }
+                    dA[c] = -A * A * (dm0[c] + 2.0 * Bdm1 + BdmB);
+#pragma unroll
+                    for (int p = 0; p < 3; ++p) dB[c][p] = -(inv[p][0] * rhs[0] + inv[p][1] * rhs[1] + inv[p][2] * rhs[2]);
+                }
+            } else {   // S14: degenerate neighbourhood -> zeroth-order correction only
+                A = 1.0 / m0;
+#pragma unroll
+                for (int c = 0; c < 3; ++c) {
+                    B[c] = 0.0;
+                    dA[c] = -A * A * dm0[c];
+                    dB[c][0] = dB[c][1] = dB[c][2] = 0.0;
+                }
+            }
+            // pre-combined form used by the later sweeps:  (grad WR_ij)_c = W (cvec_c + M_ca x_a) + A s D x_c, s = 1 + B.x
+            //   cvec_c = d_c A + A B_c,   M_ca = d_c A B_a + A d_c B_a
+            o0 = make_float4((float)A, (float)B[0], (float)B[1], (float)B[2]);
+            float Mf[9];
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int p = 0; p < 3; ++p) Mf[3 * c + p] = (float)(dA[c] * B[p] + A * dB[c][p]);
+            o1 = make_float4((float)(dA[0] + A * B[0]), (float)(dA[1] + A * B[1]), (float)(dA[2] + A * B[2]), Mf[0]);
+            o2 = make_float4(Mf[1], Mf[2], Mf[3], Mf[4]);
+            o3 = make_float4(Mf[5], Mf[6], Mf[7], Mf[8]);
+            const int32_t p = a.perm[i];
+            const int64_t n = a.n;
+            if (a.o0) a.o0[p] = (float)A;
+            if (a.o1) { a.o1[p] = (float)B[0]; a.o1[n + p] = (float)B[1]; a.o1[2 * n + p] = (float)B[2]; }
+            if (a.o2) { a.o2[p] = (float)dA[0]; a.o2[n + p] = (float)dA[1]; a.o2[2 * n + p] = (float)dA[2]; }
+            if (a.o3) {
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+#pragma unroll
+                    for (int q = 0; q < 3; ++q) a.o3[(3 * c + q) * n + p] = (float)dB[c][q];
+            }
+        }
+        a.coef[i] = o0;
+        a.coef[a.np + i] = o1;
+        a.coef[2 * a.np + i] = o2;
+        a.coef[3 * a.np + i] = o3;
+    } else {
+        o0 = a.coef[i]; o1 = a.coef[a.np + i]; o2 = a.coef[2 * a.np + i]; o3 = a.coef[3 * a.np + i];
+    }
+    if (!GV) return;
+    // ---- a4: contraction of the velocity sums with the stored FP32 coefficients (FP64 arithmetic)
+    float g[9];
+    {
+        const Coef k = load_coef(o0, o1, o2, o3);
+        const double cv[3] = {(double)k.cx, (double)k.cy, (double)k.cz};
+        const double Bv[3] = {(double)k.Bx, (double)k.By, (double)k.Bz};
+        const double A = (double)k.A;
+        const double k3h = k3 * h, k3ih = k3 * ih;
+        const int sym[3][3] = {{0, 1, 2}, {1, 3, 4}, {2, 4, 5}};
+#pragma unroll
+        for (int al = 0; al < 3; ++al)
+#pragma unroll
+            for (int be = 0; be < 3; ++be) {
+                double t = cv[be] * (k3 * (double)S0[al]) + A * (k3ih * (double)T1[al][be]);
+#pragma unroll
+                for (int c = 0; c < 3; ++c)
+                    t += (double)k.M[3 * be + c] * (k3h * (double)S1[al][c]) + A * Bv[c] * (k3 * (double)T2[al][sym[c][be]]);
+                g[3 * al + be] = (float)(-t);
+            }
+    }
     // force-sweep state planes: (x,y,z,1/h) (v,V) | (P,rho,cs,k3) (A,B) (c,M0) (M1..M4) (M5..M8) (gxx,gyy,gzz,k5)
     // (gxy+gyx, gxz+gzx, gyz+gzy, n_h/h).  Only x.(grad v x) enters Eqs. 27-30 and Eq. 25 (uhat_ij.x_ij), so the
     // symmetric part of grad v is all the force sweep needs; k3 = sigma/h^3, k5 = sigma/h^5.
+    const float ihf = valid ? 1.0f / hi : 0.0f;
+    const float k3f = SIGMA_C4 * ihf * ihf * ihf;
+    const float k5f = k3f * ihf * ihf;
     const float u = u_s[i], rho = a.rho_s[i], gm = a.gamma;
     const float P = (gm - 1.0f) * rho * u;
     const float cs = sqrtf(gm * (gm - 1.0f) * fmaxf(u, 0.0f));
     float4* f = a.fst + i;
     const int64_t np = a.np;
-    f[2 * np] = make_float4(P, rho, cs, k3);
-    f[3 * np] = q0;
-    f[4 * np] = q1;
-    f[5 * np] = q2;
-    f[6 * np] = q3;
-    f[7 * np] = make_float4(g[0], g[4], g[8], k5);
-    f[8 * np] = make_float4(g[1] + g[3], g[2] + g[6], g[5] + g[7], a.n_h * ih);
+    f[2 * np] = make_float4(P, rho, cs, k3f);
+    f[3 * np] = o0;
+    f[4 * np] = o1;
+    f[5 * np] = o2;
+    f[6 * np] = o3;
+    f[7 * np] = make_float4(g[0], g[4], g[8], k5f);
+    f[8 * np] = make_float4(g[1] + g[3], g[2] + g[6], g[5] + g[7], a.n_h * ihf);
     if (gv_full && valid) {                              // diagnostics (crk_get_gradv): all nine components, caller order
         const int32_t p = a.perm[i];
 #pragma unroll
@@ -792,6 +842,7 @@ SweepArgs make_args(crk_ctx* c) {
     a.n = c->n; a.nl = c->nl; a.np = c->nl * CRK_LEAF;
     a.L = c->prm.box; a.half = 0.5f * c->prm.box;
     a.arena = (const uint4*)c->arena.p; a.seg_first = (const uint4*)c->seg_first.p; a.leaf_cnt = (const uint16_t*)c->leaf_cnt.p;
+    a.cand_first = (const uint32_t*)c->cand_first.p;
     a.perm = c->perm;
     a.posh = (const float4*)c->posh.p; a.posV = (float4*)c->posV.p; a.velV = nullptr;
     a.coef = (float4*)c->coef.p; a.fst = (float4*)c->fst.p;
@@ -824,19 +875,8 @@ int crk_launch_volumes(crk_ctx* c, const float* m, float* V, float* rho, uint32_
     return crk_check_launch(c, "k_volumes");
 }
 
-int crk_launch_moments(crk_ctx* c, float* A, float* B, float* gradA, float* gradB) {
-    const int64_t np = c->nl * CRK_LEAF;
-    CRK_TRY(crk_ensure(c, c->coef, (size_t)np * 4 * sizeof(float4)));
-    SweepArgs a = make_args(c);
-    a.o0 = A; a.o1 = B; a.o2 = gradA; a.o3 = gradB;
-    const int smem = W2_WPC * CRK_CCAP * (int)sizeof(float4);
-    CRK_TRY(set_smem(c, k_moments, smem));
-    k_moments<<<(unsigned)((c->nl + W2_WPC - 1) / W2_WPC), W2_WPC * 32, smem, c->stream>>>(a);
-    return crk_check_launch(c, "k_moments");
-}
-
-int crk_launch_hydro(crk_ctx* c, const float* vx, const float* vy, const float* vz, const float* u, float* ax,
-                     float* ay, float* az, float* dudt, uint32_t* pair_count) {
+// hydro preparation: velocities / energies in sorted order (force-sweep state planes 0 and 1); needs the volumes
+int crk_launch_hydro_prep(crk_ctx* c, const float* vx, const float* vy, const float* vz, const float* u) {
     const int64_t np = c->nl * CRK_LEAF;
     CRK_TRY(crk_ensure(c, c->vel_orig, (size_t)c->n * sizeof(float4)));
     CRK_TRY(crk_ensure(c, c->u_s, (size_t)np * sizeof(float)));
@@ -846,42 +886,49 @@ int crk_launch_hydro(crk_ctx* c, const float* vx, const float* vy, const float* 
     SweepArgs a = make_args(c);
     a.velV = (float4*)c->fst.p + np;                     // plane 1 of the force-sweep state is (vx,vy,vz,V)
     k_hydro_prep<<<(unsigned)((np + 255) / 256), 256, 0, c->stream>>>(a, (const float4*)c->vel_orig.p, (float*)c->u_s.p);
-    CRK_TRY(crk_check_launch(c, "k_hydro_prep"));
-    crk_rec(c, EV_GV0);
-    {
-        const int smem = W4_LPC * 2 * CRK_CCAP * (int)sizeof(float4);
-        CRK_TRY(set_smem(c, k_gradv, smem));
-        k_gradv<<<(unsigned)((c->nl + W4_LPC - 1) / W4_LPC), W4_WPL * W4_LPC * 32, smem, c->stream>>>(a, (const float*)c->u_s.p, nullptr);
-        CRK_TRY(crk_check_launch(c, "k_gradv"));
-    }
-    crk_rec(c, EV_GV1);
-    a.o0 = ax; a.o1 = ay; a.o2 = az; a.o3 = dudt; a.ocnt = pair_count;
-    {
-        const int smem = FPL * CRK_CCAP * (int)sizeof(float4);
-        if (c->prm.flags & CRK_FLAG_TIMESTEP) {
-            CRK_TRY(crk_ensure(c, c->ts_s, (size_t)np * sizeof(float2)));
-            a.ts = (float2*)c->ts_s.p;
-            CRK_TRY(set_smem(c, k_forces<true>, smem));
-            k_forces<true><<<(unsigned)c->nl, W5_WPL * 32, smem, c->stream>>>(a);
-        } else {
-            CRK_TRY(set_smem(c, k_forces<false>, smem));
-            k_forces<false><<<(unsigned)c->nl, W5_WPL * 32, smem, c->stream>>>(a);
-        }
-        CRK_TRY(crk_check_launch(c, "k_forces"));
-    }
-    crk_rec(c, EV_F1);
-    return CRK_OK;
+    return crk_check_launch(c, "k_hydro_prep");
 }
 
-// diagnostics: re-run the Eq. 26 sweep on the resident state and write all nine components of grad v in caller order
-int crk_launch_gradv_full(crk_ctx* c, float* gradv) {
+// a2 + a3 (mom), a4 (gv) or both in one sweep; gv needs crk_launch_hydro_prep first; gradv_full: diagnostics (all 9 components)
+int crk_launch_rk(crk_ctx* c, bool mom, bool gv, float* A, float* B, float* gradA, float* gradB, float* gradv_full) {
+    const int64_t np = c->nl * CRK_LEAF;
+    CRK_TRY(crk_ensure(c, c->coef, (size_t)np * 4 * sizeof(float4)));
+    SweepArgs a = make_args(c);
+    a.o0 = A; a.o1 = B; a.o2 = gradA; a.o3 = gradB;
+    a.velV = gv ? (float4*)c->fst.p + np : nullptr;
+    const unsigned grid = (unsigned)((c->nl + W2_WPC - 1) / W2_WPC);
+    const int smem = W2_WPC * (gv ? 2 : 1) * CRK_CCAP * (int)sizeof(float4);
+    const float* us = (const float*)c->u_s.p;
+    if (mom && gv) {
+        CRK_TRY(set_smem(c, k_rk<true, true>, smem));
+        k_rk<true, true><<<grid, W2_WPC * 32, smem, c->stream>>>(a, us, gradv_full);
+    } else if (mom) {
+        CRK_TRY(set_smem(c, k_rk<true, false>, smem));
+        k_rk<true, false><<<grid, W2_WPC * 32, smem, c->stream>>>(a, nullptr, nullptr);
+    } else {
+        CRK_TRY(set_smem(c, k_rk<false, true>, smem));
+        k_rk<false, true><<<grid, W2_WPC * 32, smem, c->stream>>>(a, us, gradv_full);
+    }
+    return crk_check_launch(c, "k_rk");
+}
+
+// a5 on the state written by crk_launch_hydro_prep and the grad v sweep
+int crk_launch_forces(crk_ctx* c, float* ax, float* ay, float* az, float* dudt, uint32_t* pair_count) {
     const int64_t np = c->nl * CRK_LEAF;
     SweepArgs a = make_args(c);
     a.velV = (float4*)c->fst.p + np;
-    const int smem = W4_LPC * 2 * CRK_CCAP * (int)sizeof(float4);
-    CRK_TRY(set_smem(c, k_gradv, smem));
-    k_gradv<<<(unsigned)((c->nl + W4_LPC - 1) / W4_LPC), W4_WPL * W4_LPC * 32, smem, c->stream>>>(a, (const float*)c->u_s.p, gradv);
-    return crk_check_launch(c, "k_gradv");
+    a.o0 = ax; a.o1 = ay; a.o2 = az; a.o3 = dudt; a.ocnt = pair_count;
+    const int smem = FPL * CRK_CCAP * (int)sizeof(float4);
+    if (c->prm.flags & CRK_FLAG_TIMESTEP) {
+        CRK_TRY(crk_ensure(c, c->ts_s, (size_t)np * sizeof(float2)));
+        a.ts = (float2*)c->ts_s.p;
+        CRK_TRY(set_smem(c, k_forces<true>, smem));
+        k_forces<true><<<(unsigned)c->nl, W5_WPL * 32, smem, c->stream>>>(a);
+    } else {
+        CRK_TRY(set_smem(c, k_forces<false>, smem));
+        k_forces<false><<<(unsigned)c->nl, W5_WPL * 32, smem, c->stream>>>(a);
+    }
+    return crk_check_launch(c, "k_forces");
 }
 
 // NEXT row 1: Eqs. 19-23 on the state left by crk_hydro_derivs

@@ -210,8 +210,9 @@ def test_errors_and_empty_input():
 
 # ------------------------------------------------------------------------------------------------ config 2 multi-step
 def test_blast_wave_teacher_forced_euler_steps(oracle_mod):
-    """BASELINE config 2 protocol at reduced size (S12): at each Euler step the GPU evaluates derivatives on the
-    oracle's FP32 state and must meet the bar; states come from oracle/crk_oracle.py:euler_steps (FP64 update)."""
+    """Config 2's protocol at reduced size and step, against the O(N^2) brute-force build (the full-size, full-dt protocol
+    is test_config2_protocol_as_written): at each Euler step the GPU evaluates derivatives on the oracle's FP32 state
+    and must meet the bar; states come from oracle/crk_oracle.py:euler_steps (FP64 update)."""
     ps = wl.blast_wave(n_side=24)
     worst = 0.0
     for step, cur, od in oracle_mod.euler_steps(ps, 6, 1e-4 * (64 / 24) ** 0 * 0.25):
@@ -219,6 +220,92 @@ def test_blast_wave_teacher_forced_euler_steps(oracle_mod):
         e_a, e_u = check_parity(cur, g, od, label=f"blast step {step}")
         worst = max(worst, e_a, e_u)
     print(f"[parity] blast teacher-forced worst rel L2 {worst:.2e}")
+
+
+def _gpu_euler_free_run(ps, n_steps, dt):
+    """forward Euler on the GPU's own FP32 state: three AXPYs on the caller's tensors around crk_step_derivs (the update
+    rule of DESIGN.md step 12 / S12; kept in the test, the library only evaluates derivatives).  Yields (step, state, derivs)."""
+    torch = _torch()
+    from paper_2202_02840_b200 import Crk
+    dev = torch.device("cuda:0")
+    t = {k: torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).to(dev) for k in
+         ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")}
+    ctx = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h)
+    L = float(ps.box)
+    for step in range(n_steps + 1):
+        out = ctx.step_derivs(*[t[k] for k in ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")])
+        torch.cuda.synchronize()
+        yield step, {k: v.cpu().numpy() for k, v in t.items()}, [o.cpu().numpy() for o in out]
+        if step == n_steps:
+            break
+        for xk, vk, a in (("x", "vx", out[0]), ("y", "vy", out[1]), ("z", "vz", out[2])):
+            p = t[xk] + t[vk] * dt
+            p = p - torch.floor(p / L) * L
+            p[(p >= L) | (p < 0)] = 0.0
+            t[xk] = p
+            t[vk] = t[vk] + a * dt
+        t["u"] = t["u"] + out[3] * dt
+
+
+def test_config2_protocol_as_written(oracle_mod):
+    """BASELINE.json configs[1] at its stated size and step: 64^3 blast wave, one derivative evaluation plus 10 forward-Euler
+    steps at fixed dt = 1e-4 (4.9x the CFL step of the hot centre: the trajectory explodes from step ~6, reading S12).
+    (ii) teacher-forced: at every state of the oracle's FP64 trajectory the GPU evaluates the derivatives of the FP32 cast of
+         that state and must meet the bars (counts bit-exact, 1e-4 rel L2), as long as the oracle's values fit FP32;
+    (iii) free-running GPU trajectory against the oracle's, reported per step with the step at which it leaves 1e-4."""
+    ps = wl.blast_wave()
+    dt = 1e-4
+    assert ps.n == 64 ** 3
+    fp32_ok = 1e30        # beyond this the derivatives leave the range in which FP32 products are safe (3.4e38)
+    oracle_states = []
+    worst, asserted = 0.0, 0
+    for step, cur, od in oracle_mod.euler_steps(ps, 10, dt, grid=True):
+        big = max(np.abs(od["dudt"]).max(), np.abs(od["ax"]).max(), np.abs(od["ay"]).max(), np.abs(od["az"]).max())
+        oracle_states.append((cur, od))
+        g = gpu_eval(cur)
+        if big < fp32_ok:
+            e_a, e_u = check_parity(cur, g, od, label=f"config2 teacher-forced state {step}")
+            worst = max(worst, e_a, e_u)
+            asserted += 1
+            print(f"[config2 dt=1e-4] teacher-forced state {step}: dv/dt {e_a:.2e} du/dt {e_u:.2e} (max |deriv| {big:.1e}, u<0: {(cur.u < 0).sum()})")
+        else:
+            fin = all(np.isfinite(g[k]).all() for k in ("ax", "ay", "az", "dudt"))
+            assert np.array_equal(g["nbr_count"].astype(np.int64), od["nbr_count"].astype(np.int64))
+            assert np.array_equal(g["pair_count"].astype(np.int64), od["pair_count"].astype(np.int64))
+            print(f"[config2 dt=1e-4] teacher-forced state {step}: oracle max |deriv| {big:.1e} is outside the FP32-safe range; "
+                  f"GPU output finite: {fin}; counts bit-exact (reported, not asserted: S12)")
+    assert asserted >= 9 and worst < TOL_DERIV
+    left = None
+    for (step, st, d), (cur, od) in zip(_gpu_euler_free_run(ps, 10, dt), oracle_states):
+        with np.errstate(all="ignore"):
+            e_v = rel_l2(np.stack([st["vx"], st["vy"], st["vz"]]), np.stack([cur.vx, cur.vy, cur.vz])) if step else 0.0
+            e_a = rel_l2(np.stack(d[:3]), np.stack([od["ax"], od["ay"], od["az"]]))
+            e_u = rel_l2(d[3], od["dudt"])
+        if left is None and not (max(e_a, e_u) < TOL_DERIV):
+            left = step
+        print(f"[config2 dt=1e-4] free-running step {step}: state v {e_v:.2e}, dv/dt {e_a:.2e}, du/dt {e_u:.2e}")
+    print(f"[config2 dt=1e-4] free-running GPU trajectory leaves the 1e-4 bar at step {left} (reported, not asserted)")
+
+
+def test_config2_stable_variant_free_running(oracle_mod):
+    """Labelled NON-BASELINE variant of config 2 (S12 iv): the same 64^3 blast wave at dt = 2e-5 (1x the CFL step), where a
+    free-running comparison is meaningful: 10 forward-Euler steps on the GPU's own FP32 state against the oracle's FP64
+    trajectory; derivatives at every step within 1e-4 rel L2, velocities and energies of the state within 1e-5."""
+    ps = wl.blast_wave()
+    dt = 2e-5
+    worst_d, worst_s = 0.0, 0.0
+    for (step, st, d), (_, cur, od) in zip(_gpu_euler_free_run(ps, 10, dt), oracle_mod.euler_steps(ps, 10, dt, grid=True)):
+        e_a = rel_l2(np.stack(d[:3]), np.stack([od["ax"], od["ay"], od["az"]]))
+        e_u = rel_l2(d[3], od["dudt"])
+        e_v = rel_l2(np.stack([st["vx"], st["vy"], st["vz"]]), np.stack([cur.vx, cur.vy, cur.vz])) if step else 0.0
+        e_e = rel_l2(st["u"], cur.u)
+        dx = np.abs(st["x"].astype(np.float64) - cur.x.astype(np.float64))
+        dx = np.minimum(dx, ps.box - dx).max()
+        print(f"[config2 dt=2e-5] free-running step {step}: dv/dt {e_a:.2e} du/dt {e_u:.2e} | state v {e_v:.2e} u {e_e:.2e} x {dx:.1e}")
+        worst_d = max(worst_d, e_a, e_u)
+        worst_s = max(worst_s, e_v, e_e)
+        assert dx < 1e-6
+    assert worst_d < TOL_DERIV and worst_s < 1e-5
 
 
 # ------------------------------------------------------------------------------------------------ BASELINE sizes
