@@ -443,6 +443,26 @@ int crk_oracle_hydro_derivs(crk_oracle_ctx* c, const float* vx, const float* vy,
     return 0;
 }
 
+// NEXT row 4b -- active / passive particles ("all ('active') gas leaves that require force updates will
+// evaluate the necessary derivatives ... while the remaining ('passive') leaves are simply streamed").  The same sums as
+// crk_oracle_hydro_derivs, restricted to the particles i with active[i] != 0; j ranges over everyone, and grad v (Eq. 26) is
+// evaluated for every particle because a passive neighbour's grad v_j enters Eqs. 27-30 of an active i.  Outputs of passive
+// particles are set to NaN (they are never evaluated).
+int crk_oracle_hydro_derivs_active(crk_oracle_ctx* c, const uint8_t* active, const float* vx, const float* vy, const float* vz,
+                                   const float* u, double* ax, double* ay, double* az, double* dudt) {
+    if (!c || !active || !ax || !ay || !az || !dudt) return -1;
+    const int64_t n = c->n;
+    std::vector<double> fx((size_t)n), fy((size_t)n), fz((size_t)n), fe((size_t)n);
+    const int rc = crk_oracle_hydro_derivs(c, vx, vy, vz, u, fx.data(), fy.data(), fz.data(), fe.data(), nullptr);
+    if (rc) return rc;
+    const double nan = std::numeric_limits<double>::quiet_NaN();
+    for (int64_t i = 0; i < n; ++i) {
+        const bool on = active[i] != 0;
+        ax[i] = on ? fx[i] : nan; ay[i] = on ? fy[i] : nan; az[i] = on ? fz[i] : nan; dudt[i] = on ? fe[i] : nan;
+    }
+    return 0;
+}
+
 // ---- oracle at scale: neighbour COUNTS of a full configuration (SURVEY.md section 8(c) "oracle at scale") -------------
 // The brute-force scan is O(N^2); for the 128^3 .. 512^3 configurations the counts of every particle come from this second
 // formulation: particles are binned in a uniform periodic grid of cells no smaller than the largest h, so every j with

@@ -68,6 +68,13 @@ int crk_oracle_compatible_energy_kick(crk_oracle_ctx* c, double dt, const double
 /* one pair of the above: out = { du_ij (Eq. 20), dE_ij (Eq. 21), f_ij (Eq. 23) }                                 */
 int crk_oracle_pair_compat(crk_oracle_ctx* c, int64_t i, int64_t j, double dt, double out[3]);
 
+/* NEXT row 4b -- active / passive particles: crk_oracle_hydro_derivs restricted to the particles with
+ * active[i] != 0 (j ranges over everyone; grad v is evaluated for all, a passive neighbour's grad v_j enters Eqs. 27-30 of an
+ * active i).  Outputs of passive particles are NaN.  Pinned: mask = all gives the bits of crk_oracle_hydro_derivs; the
+ * results of an active particle do not depend on which other particles are active.                                      */
+int crk_oracle_hydro_derivs_active(crk_oracle_ctx* c, const uint8_t* active, const float* vx, const float* vy,
+                                   const float* vz, const float* u, double* ax, double* ay, double* az, double* dudt);
+
 /* Oracle at scale: nbr_count[i] = #{j != i : r_ij < h_i} and pair_count[i] = #{j != i : r_ij < max(h_i, h_j)} of a FULL
  * configuration through a uniform periodic grid of cells >= h_max (27-cell stencil) with the same FP32 predicate (S3).
  * Pinned by bit-exact agreement with crk_oracle_build / _volumes / _hydro_derivs counts on small sets.  Returns -2 if

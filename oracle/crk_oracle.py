@@ -40,6 +40,7 @@ def lib():
         L.crk_oracle_volumes.argtypes = [C.c_void_p, fp, dp, dp, up]
         L.crk_oracle_rk_coefficients.argtypes = [C.c_void_p, dp, dp, dp, dp]
         L.crk_oracle_hydro_derivs.argtypes = [C.c_void_p, fp, fp, fp, fp, dp, dp, dp, dp, up]
+        L.crk_oracle_hydro_derivs_active.argtypes = [C.c_void_p, C.POINTER(C.c_uint8), fp, fp, fp, fp, dp, dp, dp, dp]
         L.crk_oracle_W.restype = C.c_double
         L.crk_oracle_W.argtypes = [C.c_double, C.c_double]
         L.crk_oracle_dWdr.restype = C.c_double
@@ -140,6 +141,17 @@ class Oracle:
         rc = lib().crk_oracle_hydro_derivs(self._c, p1, p2, p3, p4, _d(ax), _d(ay), _d(az), _d(du), _u(cnt))
         assert rc == 0
         return ax, ay, az, du, cnt
+
+    def hydro_derivs_active(self, active, vx, vy, vz, u):
+        """Eqs. 17-18 for the particles with active[i] != 0 only (NaN elsewhere)"""
+        (vx, p1), (vy, p2), (vz, p3), (u, p4) = _f(vx), _f(vy), _f(vz), _f(u)
+        act = np.ascontiguousarray(active, dtype=np.uint8)
+        n = self.n
+        ax, ay, az, du = np.empty(n), np.empty(n), np.empty(n), np.empty(n)
+        rc = lib().crk_oracle_hydro_derivs_active(self._c, act.ctypes.data_as(C.POINTER(C.c_uint8)), p1, p2, p3, p4,
+                                                  _d(ax), _d(ay), _d(az), _d(du))
+        assert rc == 0
+        return ax, ay, az, du
 
     def step_derivs(self, ps, grid=False):
         """ps: crk_workloads.ParticleSet (or anything with x,y,z,h,vx,vy,vz,m,u). Returns dict of all outputs."""

@@ -858,3 +858,26 @@ def test_pair_terms_equal_printed_eqs_17_18_with_P_plus_Q(clustered):
             assert got[3] == pytest.approx(dE, rel=1e-8, abs=1e-10 * abs(hvv * P[j] * np.linalg.norm(G)))
             n_visc += Qi > 0
     assert n_visc > 50
+
+
+# ------------------------------------------------------------------------------------------------ active / passive
+def test_active_mask_restricts_the_sums_and_nothing_else(clustered):
+    """PAPER.md:282 (active leaves evaluate derivatives, passive ones are streamed): mask = all reproduces the bits of the
+    full evaluation; an active particle's result does not depend on which other particles are active; passive outputs are
+    never evaluated (NaN)."""
+    ps, o, d = clustered
+    full = o.hydro_derivs(ps.vx, ps.vy, ps.vz, ps.u)[:4]
+    ones = np.ones(ps.n, dtype=np.uint8)
+    allm = o.hydro_derivs_active(ones, ps.vx, ps.vy, ps.vz, ps.u)
+    for a, b in zip(full, allm):
+        assert np.array_equal(a, b)
+    rng = np.random.default_rng(8)
+    m1 = (rng.random(ps.n) < 0.1).astype(np.uint8)
+    m2 = m1.copy(); m2[rng.random(ps.n) < 0.3] = 1          # superset of m1
+    r1 = o.hydro_derivs_active(m1, ps.vx, ps.vy, ps.vz, ps.u)
+    r2 = o.hydro_derivs_active(m2, ps.vx, ps.vy, ps.vz, ps.u)
+    on = m1 != 0
+    assert on.sum() > 100
+    for a, b, f in zip(r1, r2, full):
+        assert np.array_equal(a[on], b[on]) and np.array_equal(a[on], f[on])
+        assert np.isnan(a[~on]).all()
