@@ -69,6 +69,7 @@ typedef struct {
     float    ms_lists;        /* per-particle neighbour lists (third part of crk_build_cells)                  */
     int32_t  timed_steps;     /* number of completed steps the ms_* fields average over (event ring of 64)    */
     int32_t  sort_passes;     /* 8-bit radix passes of the last build (key bits follow the smallest h)         */
+    int64_t  n_active_leaves, n_halo_leaves;   /* of the last crk_hydro_derivs_active                                 */
 } crk_stats;
 
 /* stream: a cudaStream_t (0 = default stream).  Returns CRK_OK and *out, or an error.                       */
@@ -137,6 +138,18 @@ int  crk_timestep(crk_ctx* c, float C_cfl, float* dt_min);
  * N_i = (4/3) pi h_i^3 / V_i (Eq. 51), N_res = (4/3) pi n_h^3, lambda of Eq. 53.  h_new: device float[n], caller order,
  * written (may alias nothing the library reads later: the build keeps its own copy of h).  One 40 B/particle stream pass. */
 int  crk_evolve_h(crk_ctx* c, float* h_new);
+
+/* ---- NEXT row 4b: active / passive particles, PAPER.md:282 ("all ('active') gas leaves that require force updates will
+ * evaluate the necessary derivatives ... while the remaining ('passive') leaves are simply streamed") -----------------
+ * After crk_rk_coefficients (else CRK_ESTATE).  active: device uint8[n], caller order.  Evaluates Eqs. 17-18 (with the
+ * limited viscosity, as crk_hydro_derivs) for the particles with active[i] != 0 only and writes ax, ay, az, dudt THERE;
+ * entries of passive particles are left untouched.  j ranges over all particles.  Internally a 32-particle leaf is active
+ * when one of its particles is; the force sweep runs over the active leaves, the Eq. 26 sweep over the leaves of their
+ * interaction lists (a passive neighbour's grad v_j enters Eqs. 27-30 of an active particle).  Synchronises once (leaf
+ * counts).  The context is left at the stage of crk_rk_coefficients: crk_compatible_energy / crk_timestep need a full
+ * crk_hydro_derivs.                                                                                                  */
+int  crk_hydro_derivs_active(crk_ctx* c, const uint8_t* active, const float* vx, const float* vy, const float* vz,
+                             const float* u, float* ax, float* ay, float* az, float* dudt);
 
 /* ---- diagnostics ---- */
 const char* crk_last_error(const crk_ctx* c);

@@ -11,7 +11,7 @@ _LIB_PATH = os.path.join(_HERE, "libcrk.so")
 
 EXPORTED_SYMBOLS = (
     "crk_create", "crk_destroy", "crk_build_cells", "crk_volumes", "crk_rk_coefficients", "crk_hydro_derivs",
-    "crk_step_derivs", "crk_step_derivs_host", "crk_compatible_energy", "crk_evolve_h", "crk_timestep", "crk_kdk_step", "crk_last_error", "crk_get_perm", "crk_get_gradv", "crk_get_leaf_segments", "crk_get_stats",
+    "crk_step_derivs", "crk_step_derivs_host", "crk_hydro_derivs_active", "crk_compatible_energy", "crk_evolve_h", "crk_timestep", "crk_kdk_step", "crk_last_error", "crk_get_perm", "crk_get_gradv", "crk_get_leaf_segments", "crk_get_stats",
     "crk_reset_stats", "crk_set_timing", "crk_get_leaf_list", "crk_measure_fp32_peak",
 )
 
@@ -34,7 +34,8 @@ class Stats(C.Structure):
                 ("n_leaf_pairs_gather", C.c_int64), ("launches", C.c_int64), ("scratch_bytes", C.c_int64), ("list_bytes", C.c_int64),
                 ("ms_build", C.c_float), ("ms_volumes", C.c_float), ("ms_rk", C.c_float), ("ms_hydro", C.c_float),
                 ("ms_sort", C.c_float), ("ms_tree", C.c_float), ("ms_gradv", C.c_float), ("ms_forces", C.c_float),
-                ("ms_lists", C.c_float), ("timed_steps", C.c_int32), ("sort_passes", C.c_int32)]
+                ("ms_lists", C.c_float), ("timed_steps", C.c_int32), ("sort_passes", C.c_int32),
+                ("n_active_leaves", C.c_int64), ("n_halo_leaves", C.c_int64)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -67,6 +68,7 @@ def _load():
     L.crk_rk_coefficients.argtypes = [vp, vp, vp, vp, vp]
     L.crk_hydro_derivs.argtypes = [vp] + [vp] * 9
     L.crk_step_derivs.argtypes = [vp, i64] + [vp] * 13
+    L.crk_hydro_derivs_active.argtypes = [vp] + [vp] * 9
     L.crk_step_derivs_host.argtypes = [vp, i64] + [vp] * 13
     L.crk_last_error.argtypes = [vp]
     L.crk_last_error.restype = C.c_char_p
@@ -135,14 +137,14 @@ class Crk:
     def build_cells(self, x, y, z, h):
         self.n = int(x.numel())
         self._dev = x.device
-        self._chk(self._L.crk_build_cells(self._h, self.n, _dev(x), _dev(y), _dev(z), _dev(h)))
+        self._chk(self._L.crk_build_cells(self._h, self.n, *[self._len(t) for t in (x, y, z, h)]))
 
     def volumes(self, m, want_count=True):
         n, d = self.n, self._dev
         V = torch.empty(n, device=d)
         rho = torch.empty(n, device=d)
         cnt = torch.empty(n, device=d, dtype=torch.int32) if want_count else None
-        self._chk(self._L.crk_volumes(self._h, _dev(m), _dev(V), _dev(rho), _opt(cnt, torch.int32)))
+        self._chk(self._L.crk_volumes(self._h, self._len(m), _dev(V), _dev(rho), _opt(cnt, torch.int32)))
         return V, rho, cnt
 
     def rk_coefficients(self, want=True):
@@ -161,17 +163,33 @@ class Crk:
         n, d = self.n, self._dev
         out = [torch.empty(n, device=d) for _ in range(4)]
         cnt = torch.empty(n, device=d, dtype=torch.int32) if want_count else None
-        self._chk(self._L.crk_hydro_derivs(self._h, _dev(vx), _dev(vy), _dev(vz), _dev(u), *[_dev(o) for o in out],
+        self._chk(self._L.crk_hydro_derivs(self._h, *[self._len(t) for t in (vx, vy, vz, u)], *[_dev(o) for o in out],
                                            _opt(cnt, torch.int32)))
         return out[0], out[1], out[2], out[3], cnt
+
+    def hydro_derivs_active(self, active, vx, vy, vz, u, out=None):
+        """Eqs. 17-18 for the particles with active[i] != 0 (uint8 tensor); other entries of `out` are left as
+        they are (NaN in freshly made outputs)"""
+        n, d = self.n, self._dev
+        if out is None:
+            out = [torch.full((n,), float("nan"), device=d) for _ in range(4)]
+        self._chk(self._L.crk_hydro_derivs_active(self._h, self._len(active, torch.uint8), *[self._len(t) for t in (vx, vy, vz, u)],
+                                                  *[self._len(o) for o in out]))
+        return out
+
+    def _len(self, t, dtype=torch.float32):
+        """device pointer of a per-particle tensor; its length must be the particle count of the last build"""
+        if int(t.numel()) != self.n:
+            raise ValueError(f"per-particle tensor has {int(t.numel())} elements, the context holds {self.n} particles")
+        return _dev(t, dtype)
 
     def step_derivs(self, x, y, z, h, vx, vy, vz, m, u, out=None):
         n = int(x.numel())
         self.n, self._dev = n, x.device
         if out is None:
             out = [torch.empty(n, device=x.device) for _ in range(4)]
-        self._chk(self._L.crk_step_derivs(self._h, n, *[_dev(t) for t in (x, y, z, h, vx, vy, vz, m, u)],
-                                          *[_dev(o) for o in out]))
+        self._chk(self._L.crk_step_derivs(self._h, n, *[self._len(t) for t in (x, y, z, h, vx, vy, vz, m, u)],
+                                          *[self._len(o) for o in out]))
         return out
 
     def step_derivs_host(self, x, y, z, h, vx, vy, vz, m, u, out):
@@ -179,17 +197,17 @@ class Crk:
         n = int(x.numel())
         self.n = n
         for t in (x, y, z, h, vx, vy, vz, m, u, *out):
-            if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
-                raise TypeError("expected contiguous host float32 tensors")
+            if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous() or int(t.numel()) != n:
+                raise TypeError("expected contiguous host float32 tensors of one length")
         self._chk(self._L.crk_step_derivs_host(self._h, n, *[C.c_void_p(t.data_ptr()) for t in (x, y, z, h, vx, vy, vz, m, u)],
                                                *[C.c_void_p(t.data_ptr()) for t in out]))
         return out
 
     def kdk_step(self, x, y, z, h, vx, vy, vz, m, u, dt: float):
         """Eq. 43: one velocity-Verlet step, x, y, z, vx, vy, vz, u advanced in place"""
-        n = x.numel()
+        n = int(x.numel())
         self.n = n
-        self._chk(self._L.crk_kdk_step(self._h, n, *[_dev(t) for t in (x, y, z, h, vx, vy, vz, m, u)], C.c_float(dt)))
+        self._chk(self._L.crk_kdk_step(self._h, n, *[self._len(t) for t in (x, y, z, h, vx, vy, vz, m, u)], C.c_float(dt)))
 
     def timestep(self, C_cfl: float = 0.25, out=None):
         """Eqs. 46-50 after hydro_derivs on a context created with timestep=True"""

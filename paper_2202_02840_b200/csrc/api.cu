@@ -54,7 +54,7 @@ void crk_destroy(crk_ctx* c) {
     DevBuf* bufs[] = {&c->keys[0], &c->keys[1], &c->vals[0], &c->vals[1], &c->hist, &c->scan_tmp, &c->posh_orig,
                       &c->posh, &c->leaf_lo, &c->leaf_hi, &c->nbr_cnt, &c->nbr_off, &c->nbr_list, &c->nbr_gcnt,
                       &c->posV, &c->rho_s, &c->coef, &c->fst, &c->u_s, &c->vel_orig, &c->m_s, &c->flag,
-                      &c->host_stage, &c->arena, &c->seg_first, &c->leaf_cnt, &c->cand_first, &c->ts_s, &c->kdk, &c->kick};
+                      &c->host_stage, &c->arena, &c->seg_first, &c->leaf_cnt, &c->cand_first, &c->act_flags, &c->act_offs, &c->act_ids, &c->ts_s, &c->kdk, &c->kick};
     for (DevBuf* b : bufs)
         if (b->p) cudaFree(b->p);
     if (c->h_flag) cudaFreeHost(c->h_flag);
@@ -157,17 +157,34 @@ int crk_hydro_derivs(crk_ctx* c, const float* vx, const float* vy, const float* 
     return CRK_OK;
 }
 
-int crk_step_derivs(crk_ctx* c, int64_t n, const float* x, const float* y, const float* z, const float* h,
-                    const float* vx, const float* vy, const float* vz, const float* m, const float* u, float* ax,
-                    float* ay, float* az, float* dudt) {
-    CRK_TRY(crk_build_cells(c, n, x, y, z, h));
+// NEXT row 4b: active / passive particles
+int crk_hydro_derivs_active(crk_ctx* c, const uint8_t* active, const float* vx, const float* vy, const float* vz, const float* u,
+                            float* ax, float* ay, float* az, float* dudt) {
+    if (!c) return CRK_EINVAL;
+    if (c->stage < 3) {
+        snprintf(c->err, sizeof(c->err), "crk_hydro_derivs_active called before crk_rk_coefficients");
+        return CRK_ESTATE;
+    }
+    if (c->n == 0) return CRK_OK;
+    if (!active || !vx || !vy || !vz || !u || !ax || !ay || !az || !dudt) return CRK_EINVAL;
+    c->stage = 3;                                        // the force-sweep state is about to be partial
+    CRK_TRY(crk_launch_hydro_prep(c, vx, vy, vz, u));
+    CRK_TRY(crk_select_active(c, active, &c->n_active_leaves, &c->n_halo_leaves));
+    const int32_t* ids = (const int32_t*)c->act_ids.p;
+    CRK_TRY(crk_launch_rk(c, false, true, nullptr, nullptr, nullptr, nullptr, nullptr, ids + c->n_active_leaves, c->n_halo_leaves));
+    return crk_launch_forces(c, ax, ay, az, dudt, nullptr, ids, c->n_active_leaves, active);
+}
+
+// volumes, then moments + 3x3 solve and the velocity-gradient sums in ONE sweep over the lists (same bits as the staged
+// calls), then the momentum / energy sweep; crk_build_cells must have run
+static int crk_step_derivs_built(crk_ctx* c, const float* vx, const float* vy, const float* vz, const float* m, const float* u,
+                                 float* ax, float* ay, float* az, float* dudt) {
     CRK_TRY(crk_volumes(c, m, nullptr, nullptr, nullptr));
-    if (n == 0) {
+    if (c->n == 0) {
         c->stage = 4;
         return CRK_OK;
     }
     if (!vx || !vy || !vz || !u || !ax || !ay || !az || !dudt) return CRK_EINVAL;
-    // moments + 3x3 solve and the velocity-gradient sums in ONE sweep over the lists (same bits as the two staged calls)
     rec(c, EV_HY0);
     CRK_TRY(crk_launch_hydro_prep(c, vx, vy, vz, u));
     rec(c, EV_PREP1);
@@ -181,6 +198,13 @@ int crk_step_derivs(crk_ctx* c, int64_t n, const float* x, const float* y, const
     if (c->timing) c->ev_done[c->ev_slot] = true;
     c->stage = 4;
     return CRK_OK;
+}
+
+int crk_step_derivs(crk_ctx* c, int64_t n, const float* x, const float* y, const float* z, const float* h,
+                    const float* vx, const float* vy, const float* vz, const float* m, const float* u, float* ax,
+                    float* ay, float* az, float* dudt) {
+    CRK_TRY(crk_build_cells(c, n, x, y, z, h));
+    return crk_step_derivs_built(c, vx, vy, vz, m, u, ax, ay, az, dudt);
 }
 
 // ---- NEXT row 2b: hydro-only velocity-Verlet step, Eq. 43, a = 1, dt/dy = 1, p = v -----------------
@@ -286,21 +310,22 @@ int crk_step_derivs_host(crk_ctx* c, int64_t n, const float* x, const float* y, 
         CRK_CUDA(c, cudaMemcpyAsync(d + q * stride, in[q], (size_t)n * sizeof(float), cudaMemcpyHostToDevice, c->copy_stream));
     CRK_CUDA(c, cudaEventRecord(c->ev_copy, c->copy_stream));
     float* o = d + 9 * stride;
-    {
-        const int rc = crk_build_cells(c, n, d, d + stride, d + 2 * stride, d + 3 * stride);
-        if (rc != CRK_OK) {
-            cudaStreamSynchronize(c->copy_stream);       // the caller may reuse its buffers as soon as we return
-            return rc;
-        }
-    }
-    CRK_CUDA(c, cudaStreamWaitEvent(c->stream, c->ev_copy, 0));
-    CRK_TRY(crk_volumes(c, d + 7 * stride, nullptr, nullptr, nullptr));
-    CRK_TRY(crk_rk_coefficients(c, nullptr, nullptr, nullptr, nullptr));
-    CRK_TRY(crk_hydro_derivs(c, d + 4 * stride, d + 5 * stride, d + 6 * stride, d + 8 * stride, o, o + stride, o + 2 * stride,
-                             o + 3 * stride, nullptr));
+    // on any failure both streams are drained before returning: the caller may reuse its host buffers right away
+    auto fail = [&](int rc) {
+        cudaStreamSynchronize(c->copy_stream);
+        cudaStreamSynchronize(c->stream);
+        return rc;
+    };
+    int rc = crk_build_cells(c, n, d, d + stride, d + 2 * stride, d + 3 * stride);
+    if (rc != CRK_OK) return fail(rc);
+    if (cudaStreamWaitEvent(c->stream, c->ev_copy, 0) != cudaSuccess) return fail(CRK_ECUDA);
+    rc = crk_step_derivs_built(c, d + 4 * stride, d + 5 * stride, d + 6 * stride, d + 7 * stride, d + 8 * stride, o, o + stride,
+                               o + 2 * stride, o + 3 * stride);
+    if (rc != CRK_OK) return fail(rc);
     float* out[4] = {ax, ay, az, dudt};
     for (int q = 0; q < 4; ++q)
-        CRK_CUDA(c, cudaMemcpyAsync(out[q], o + q * stride, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, c->stream));
+        if (cudaMemcpyAsync(out[q], o + q * stride, (size_t)n * sizeof(float), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
+            return fail(CRK_ECUDA);
     CRK_CUDA(c, cudaStreamSynchronize(c->stream));
     return CRK_OK;
 }
@@ -330,6 +355,7 @@ int crk_evolve_h(crk_ctx* c, float* h_new) {
         return CRK_ESTATE;
     }
     if (c->n == 0) return CRK_OK;
+    c->kdk_valid = false;   // the caller is about to change h (possibly in place): lists, volumes, coefficients of this build go stale
     return crk_launch_evolve_h(c, h_new);
 }
 
@@ -383,6 +409,8 @@ int crk_get_stats(crk_ctx* c, crk_stats* out) {
     out->scratch_bytes = (int64_t)c->scratch_bytes;
     out->list_bytes = c->arena_units * 16;
     out->sort_passes = c->st.sort_passes;
+    out->n_active_leaves = c->n_active_leaves;
+    out->n_halo_leaves = c->n_halo_leaves;
     if (c->timing && c->n > 0) {
         // mean over the completed steps still held in the event ring (all steps since crk_reset_stats if <= 64)
         CRK_CUDA(c, cudaStreamSynchronize(c->stream));

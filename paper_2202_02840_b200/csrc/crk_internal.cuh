@@ -84,6 +84,8 @@ struct crk_ctx {
     DevBuf arena, seg_first;       // neighbour-list arena (16-byte units); per leaf a uint4 copy of its first segment's header
     DevBuf leaf_cnt;               // u16[nl][64]: per-lane cnt_g | cnt of the first segment (dense, so the sweeps need no pointer chase)
     DevBuf cand_first;             // u32[nl][CRK_CAND_STRIDE]: candidate indices of the first segment (dense)
+    DevBuf act_flags, act_offs, act_ids;   // crk_hydro_derivs_active: leaf flags (active | halo), their scan, compacted leaf ids
+    int64_t n_active_leaves = 0, n_halo_leaves = 0;
     int64_t arena_units = 0;       // units used by the last build
     // per-particle state in sorted order
     DevBuf posV;                   // float4 (x,y,z,V)
@@ -159,8 +161,11 @@ int crk_build_tree_and_list(crk_ctx* c);                                        
 int crk_build_nbr_lists(crk_ctx* c);                                                                   // lists.cu
 int crk_launch_volumes(crk_ctx* c, const float* m, float* V, float* rho, uint32_t* nbr_count);        // pairs.cu
 int crk_launch_hydro_prep(crk_ctx* c, const float* vx, const float* vy, const float* vz, const float* u);   // pairs.cu
-int crk_launch_rk(crk_ctx* c, bool mom, bool gv, float* A, float* B, float* gradA, float* gradB, float* gradv_full);   // pairs.cu
-int crk_launch_forces(crk_ctx* c, float* ax, float* ay, float* az, float* dudt, uint32_t* pair_count);   // pairs.cu
+int crk_launch_rk(crk_ctx* c, bool mom, bool gv, float* A, float* B, float* gradA, float* gradB, float* gradv_full,
+                  const int32_t* ids = nullptr, int64_t n_ids = 0);   // pairs.cu
+int crk_launch_forces(crk_ctx* c, float* ax, float* ay, float* az, float* dudt, uint32_t* pair_count, const int32_t* ids = nullptr,
+                      int64_t n_ids = 0, const uint8_t* active = nullptr);   // pairs.cu
+int crk_select_active(crk_ctx* c, const uint8_t* active, int64_t* n_active, int64_t* n_halo);   // pairs.cu
 int crk_launch_timestep(crk_ctx* c, float C_cfl, float* dt_min);                                       // pairs.cu
 int crk_launch_evolve_h(crk_ctx* c, float* h_new);                                                    // pairs.cu
 int crk_launch_compat(crk_ctx* c, float dt, float c1, float c0, const float* bx, const float* by, const float* bz,

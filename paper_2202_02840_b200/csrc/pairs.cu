@@ -41,6 +41,9 @@ struct SweepArgs {
     float* __restrict__ o0; float* __restrict__ o1; float* __restrict__ o2; float* __restrict__ o3;
     uint32_t* __restrict__ ocnt;
     float2* __restrict__ ts;              // (max approach speed, max Q_i) per particle, sorted (time-step criteria), or null
+    const int32_t* __restrict__ ids;      // compacted list of leaves to sweep (crk_hydro_derivs_active), or null = all nl leaves
+    int64_t n_ids;
+    const uint8_t* __restrict__ active;   // per particle, caller order: outputs are written where active[p] != 0 (null = everywhere)
 };
 
 struct Seg {
@@ -393,8 +396,9 @@ k_rk(SweepArgs a, const float* __restrict__ u_s, float* __restrict__ gv_full) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int PL = GV ? 2 : 1;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int64_t leaf = (int64_t)blockIdx.x * W2_WPC + w;
-    if (leaf >= a.nl) return;
+    const int64_t slot = (int64_t)blockIdx.x * W2_WPC + w;
+    if (slot >= (a.ids ? a.n_ids : a.nl)) return;
+    const int64_t leaf = a.ids ? (int64_t)a.ids[slot] : slot;
     float4* tile = (float4*)smem_raw + (size_t)w * PL * CRK_CCAP;
     const int64_t i = leaf * CRK_LEAF + lane;
     const bool valid = i < a.n;
@@ -727,7 +731,7 @@ template <bool TS>   // TS: also reduce the per-particle maxima the time-step cr
 __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
-    const int64_t leaf = blockIdx.x;
+    const int64_t leaf = a.ids ? (int64_t)a.ids[blockIdx.x] : (int64_t)blockIdx.x;
     float4* tile = (float4*)smem_raw;
     const int64_t i = leaf * CRK_LEAF + lane;
     const bool valid = i < a.n;
@@ -761,11 +765,13 @@ __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
         const float im = 1.0f / a.m_s[i];
         const int32_t p = a.perm[i];
         as = make_float4(acc[0] * im, acc[1] * im, acc[2] * im, I.P * __powf(I.rho, -a.gamma));
-        a.o0[p] = as.x;
-        a.o1[p] = as.y;
-        a.o2[p] = as.z;
-        a.o3[p] = acc[3] * im;
-        if (a.ocnt) a.ocnt[p] = count;
+        if (!a.active || a.active[p]) {
+            a.o0[p] = as.x;
+            a.o1[p] = as.y;
+            a.o2[p] = as.z;
+            a.o3[p] = acc[3] * im;
+            if (a.ocnt) a.ocnt[p] = count;
+        }
     }
     a.fst[(int64_t)FPL * a.np + i] = as;                 // plane 9: (dv/dt, s = P / rho^gamma) for crk_compatible_energy
 }
@@ -890,13 +896,16 @@ int crk_launch_hydro_prep(crk_ctx* c, const float* vx, const float* vy, const fl
 }
 
 // a2 + a3 (mom), a4 (gv) or both in one sweep; gv needs crk_launch_hydro_prep first; gradv_full: diagnostics (all 9 components)
-int crk_launch_rk(crk_ctx* c, bool mom, bool gv, float* A, float* B, float* gradA, float* gradB, float* gradv_full) {
+int crk_launch_rk(crk_ctx* c, bool mom, bool gv, float* A, float* B, float* gradA, float* gradB, float* gradv_full,
+                  const int32_t* ids, int64_t n_ids) {
     const int64_t np = c->nl * CRK_LEAF;
     CRK_TRY(crk_ensure(c, c->coef, (size_t)np * 4 * sizeof(float4)));
     SweepArgs a = make_args(c);
     a.o0 = A; a.o1 = B; a.o2 = gradA; a.o3 = gradB;
     a.velV = gv ? (float4*)c->fst.p + np : nullptr;
-    const unsigned grid = (unsigned)((c->nl + W2_WPC - 1) / W2_WPC);
+    a.ids = ids; a.n_ids = n_ids;
+    const unsigned grid = (unsigned)(((ids ? n_ids : c->nl) + W2_WPC - 1) / W2_WPC);
+    if (grid == 0) return CRK_OK;
     const int smem = W2_WPC * (gv ? 2 : 1) * CRK_CCAP * (int)sizeof(float4);
     const float* us = (const float*)c->u_s.p;
     if (mom && gv) {
@@ -913,9 +922,13 @@ int crk_launch_rk(crk_ctx* c, bool mom, bool gv, float* A, float* B, float* grad
 }
 
 // a5 on the state written by crk_launch_hydro_prep and the grad v sweep
-int crk_launch_forces(crk_ctx* c, float* ax, float* ay, float* az, float* dudt, uint32_t* pair_count) {
+int crk_launch_forces(crk_ctx* c, float* ax, float* ay, float* az, float* dudt, uint32_t* pair_count, const int32_t* ids,
+                      int64_t n_ids, const uint8_t* active) {
     const int64_t np = c->nl * CRK_LEAF;
     SweepArgs a = make_args(c);
+    a.ids = ids; a.n_ids = n_ids; a.active = active;
+    const unsigned grid = (unsigned)(ids ? n_ids : c->nl);
+    if (grid == 0) return CRK_OK;
     a.velV = (float4*)c->fst.p + np;
     a.o0 = ax; a.o1 = ay; a.o2 = az; a.o3 = dudt; a.ocnt = pair_count;
     const int smem = FPL * CRK_CCAP * (int)sizeof(float4);
@@ -923,12 +936,61 @@ int crk_launch_forces(crk_ctx* c, float* ax, float* ay, float* az, float* dudt, 
         CRK_TRY(crk_ensure(c, c->ts_s, (size_t)np * sizeof(float2)));
         a.ts = (float2*)c->ts_s.p;
         CRK_TRY(set_smem(c, k_forces<true>, smem));
-        k_forces<true><<<(unsigned)c->nl, W5_WPL * 32, smem, c->stream>>>(a);
+        k_forces<true><<<grid, W5_WPL * 32, smem, c->stream>>>(a);
     } else {
         CRK_TRY(set_smem(c, k_forces<false>, smem));
-        k_forces<false><<<(unsigned)c->nl, W5_WPL * 32, smem, c->stream>>>(a);
+        k_forces<false><<<grid, W5_WPL * 32, smem, c->stream>>>(a);
     }
     return crk_check_launch(c, "k_forces");
+}
+
+// NEXT row 4b: active / passive leaves.  A leaf is active when one of its particles is; the force sweep runs
+// over the active leaves only, the grad v sweep over their "halo" (every leaf of an active leaf's interaction list, itself
+// included: a passive neighbour's grad v_j enters Eqs. 27-30 of an active particle).  flags: [0, nl) active, [nl, 2 nl) halo.
+namespace {
+__global__ void __launch_bounds__(256) k_mark_active(const uint8_t* __restrict__ active, const int32_t* __restrict__ perm, int64_t n,
+                                                     int64_t nl, const uint32_t* __restrict__ cnt, const uint32_t* __restrict__ list,
+                                                     uint32_t cap, uint32_t* __restrict__ flags) {
+    const int lane = threadIdx.x & 31;
+    const int64_t leaf = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (leaf >= nl) return;
+    const int64_t i = leaf * CRK_LEAF + lane;
+    const bool on = (i < n) && active[perm[i]] != 0;
+    if (!__any_sync(0xffffffffu, on)) return;
+    if (lane == 0) flags[leaf] = 1u;
+    const uint32_t m = cnt[leaf];
+    for (uint32_t e = lane; e < m; e += 32) flags[nl + (list[(uint64_t)leaf * cap + e] & CRK_LEAF_MASK)] = 1u;
+}
+// ids[offs[q]] = q - base for every set flag (offs = exclusive scan of flags)
+__global__ void __launch_bounds__(256) k_compact_ids(const uint32_t* __restrict__ flags, const uint32_t* __restrict__ offs, int64_t m,
+                                                     int64_t nl, int32_t* __restrict__ ids) {
+    const int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q < m && flags[q]) ids[offs[q]] = (int32_t)(q < nl ? q : q - nl);
+}
+}  // namespace
+
+// fills c->act_ids with the active leaves followed by the halo leaves; counts on the host (one synchronisation)
+int crk_select_active(crk_ctx* c, const uint8_t* active, int64_t* n_active, int64_t* n_halo) {
+    const int64_t nl = c->nl;
+    CRK_TRY(crk_ensure(c, c->act_flags, (size_t)2 * nl * sizeof(uint32_t)));
+    CRK_TRY(crk_ensure(c, c->act_offs, ((size_t)2 * nl + 1) * sizeof(uint32_t)));
+    CRK_TRY(crk_ensure(c, c->act_ids, (size_t)2 * nl * sizeof(int32_t)));
+    uint32_t* flags = (uint32_t*)c->act_flags.p;
+    uint32_t* offs = (uint32_t*)c->act_offs.p;
+    CRK_CUDA(c, cudaMemsetAsync(flags, 0, (size_t)2 * nl * sizeof(uint32_t), c->stream));
+    k_mark_active<<<(unsigned)((nl + 7) / 8), 256, 0, c->stream>>>(active, c->perm, c->n, nl, (const uint32_t*)c->nbr_cnt.p,
+                                                                   (const uint32_t*)c->nbr_list.p, (uint32_t)c->leaf_list_cap, flags);
+    CRK_TRY(crk_check_launch(c, "k_mark_active"));
+    CRK_TRY(crk_exclusive_scan_u32(c, flags, offs, 2 * nl, c->scan_tmp));
+    k_compact_ids<<<(unsigned)((2 * nl + 255) / 256), 256, 0, c->stream>>>(flags, offs, 2 * nl, nl, (int32_t*)c->act_ids.p);
+    CRK_TRY(crk_check_launch(c, "k_compact_ids"));
+    uint32_t* h = (uint32_t*)((char*)c->h_flag + 48);
+    CRK_CUDA(c, cudaMemcpyAsync(h, offs + nl, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
+    CRK_CUDA(c, cudaMemcpyAsync(h + 1, offs + 2 * nl, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
+    CRK_CUDA(c, cudaStreamSynchronize(c->stream));
+    *n_active = (int64_t)h[0];
+    *n_halo = (int64_t)h[1] - (int64_t)h[0];
+    return CRK_OK;
 }
 
 // NEXT row 1: Eqs. 19-23 on the state left by crk_hydro_derivs

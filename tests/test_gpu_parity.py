@@ -212,6 +212,67 @@ def test_parity_negative_internal_energy(oracle_mod):
     print(f"[parity] u<0 on {len(neg)} particles: dv/dt {e_a:.2e} du/dt {e_u:.2e} compatible du {e_c:.2e}")
 
 
+@pytest.mark.parametrize("name,n_side,frac", [("clustered", 24, 0.10), ("cosmo", 32, 0.25), ("tiny_uniform", 16, 1.0)])
+def test_active_particles_parity(name, n_side, frac, oracle_mod):
+    """NEXT row 4b: derivatives of the active particles only.  Active = the `frac` of the particles with the
+    smallest h (the ones a hierarchical time-step scheme would put in the deepest bins); compared with the oracle's
+    restricted sums, with the library's own full evaluation (same kernels, so identical bits), and passive entries stay
+    untouched."""
+    torch = _torch()
+    ps = wl.make_config(name, n_side)
+    order = np.argsort(ps.h, kind="stable")
+    active = np.zeros(ps.n, dtype=np.uint8)
+    active[order[:max(1, int(frac * ps.n))]] = 1
+    o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
+    o.step_derivs(ps)
+    oa = o.hydro_derivs_active(active, ps.vx, ps.vy, ps.vz, ps.u)
+    g = gpu_eval(ps)
+    ctx = g["ctx"]
+    dev = torch.device("cuda:0")
+    t = {k: torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).to(dev) for k in ("vx", "vy", "vz", "u")}
+    # velocities changed since the last full evaluation: the active call must redo grad v of the halo leaves
+    ctx.hydro_derivs(t["vx"] * 0.5, t["vy"] * 0.5, t["vz"] * 0.5, t["u"])
+    out = ctx.hydro_derivs_active(torch.from_numpy(active).to(dev), t["vx"], t["vy"], t["vz"], t["u"])
+    torch.cuda.synchronize()
+    st = ctx.stats()
+    on = active != 0
+    got = [q.cpu().numpy() for q in out]
+    for q, k in zip(got, ("ax", "ay", "az", "dudt")):
+        assert np.isnan(q[~on]).all(), "a passive entry was written"
+        assert np.array_equal(q[on], g[k][on]), "active results differ from the full evaluation"
+    e_a = rel_l2(np.stack([q[on] for q in got[:3]]), np.stack([q[on] for q in oa[:3]]))
+    e_u = rel_l2(got[3][on], oa[3][on])
+    assert e_a < TOL_DERIV and e_u < TOL_DERIV
+    assert 0 < st["n_active_leaves"] <= st["n_leaves"] and st["n_active_leaves"] <= st["n_halo_leaves"] <= st["n_leaves"]
+    if frac == 1.0:
+        assert st["n_active_leaves"] == st["n_leaves"]
+    print(f"[active] {name}: {on.sum()} of {ps.n} particles active, leaves active {st['n_active_leaves']} halo {st['n_halo_leaves']} "
+          f"of {st['n_leaves']}; dv/dt {e_a:.2e} du/dt {e_u:.2e}")
+
+
+def test_kdk_reuse_is_dropped_when_h_evolves():
+    """CRK_FLAG_KDK_REUSE keeps lists, volumes and coefficients between consecutive crk_kdk_step calls on the same arrays;
+    crk_evolve_h followed by an in-place change of h (the integration loop of the Sod / Sedov tests) must drop that reuse."""
+    torch = _torch()
+    from paper_2202_02840_b200 import Crk
+    ps = wl.tiny_uniform()
+    dev = torch.device("cuda:0")
+    names = ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")
+
+    def run(reuse):
+        t = [torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).to(dev) for k in names]
+        ctx = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h, kdk_reuse=reuse)
+        for _ in range(3):
+            ctx.kdk_step(*t, 2e-3)
+            t[3].copy_(ctx.evolve_h() * 1.05)          # same address, new values
+        torch.cuda.synchronize()
+        return [q.cpu().numpy() for q in t]
+
+    a, b = run(False), run(True)
+    for qa, qb, k in zip(a, b, names):
+        assert np.array_equal(qa, qb), k
+
+
 def test_step_derivs_and_host_entry_match_staged_calls():
     torch = _torch()
     from paper_2202_02840_b200 import Crk
