@@ -11,7 +11,7 @@ N_H = 2.4          # particles per support radius: (4/3) pi n_h^3 = 57.9 (PAPER.
 GAMMA = 5.0 / 3.0
 BOX = 1.0
 
-CONFIG_NAMES = ("tiny_uniform", "blast_wave", "clustered", "cosmo", "cosmo_large")
+CONFIG_NAMES = ("tiny_uniform", "blast_wave", "clustered", "cosmo", "cosmo_large", "clustered_large")
 
 
 @dataclass
@@ -117,7 +117,7 @@ def _knn_support(pos32: np.ndarray, k: int) -> np.ndarray:
 
 
 def clustered_plummer(n_side: int = 128, seed: int = 1003, frac_clustered: float = 0.7,
-                      n_spheres: int | None = None, k_nbr: int = 58) -> ParticleSet:
+                      n_spheres: int | None = None, k_nbr: int = 58, name: str = "clustered") -> ParticleSet:
     """BASELINE config 3: 70% of particles in Plummer spheres (centres uniform, scale radii log-uniform in
     [0.002, 0.02]), 30% uniform background; v ~ N(0, 0.05^2); u log-uniform in [0.1, 10]; adaptive h with
     exactly k_nbr neighbours inside the support (k-th-neighbour rule; >10x range in h)."""
@@ -143,7 +143,8 @@ def clustered_plummer(n_side: int = 128, seed: int = 1003, frac_clustered: float
     pos = pos[order]
     vel = _rng(seed, 7).normal(0.0, 0.05, size=(n, 3))
     u = np.exp(_rng(seed, 8).uniform(np.log(0.1), np.log(10.0), size=n))
-    ps = _pack("clustered", seed, pos, vel, u, np.ones(n), {"n_side": n_side, "n_spheres": n_spheres})
+    ps = _pack(name, seed, pos, vel, u, np.ones(n), {"n_side": n_side, "n_spheres": n_spheres})
+    del pos, vel, u
     p32 = np.stack([ps.x, ps.y, ps.z], axis=1)
     h = _knn_support(p32, k_nbr)
     ps.h = np.minimum(h, 0.49 * BOX).astype(np.float32)
@@ -218,6 +219,10 @@ def make_config(name: str, n_side: int | None = None, seed: int | None = None) -
         return zeldovich(n_side or 256, seed or 1004, rms_disp=0.3, name="cosmo")
     if name == "cosmo_large":
         return zeldovich(n_side or 512, seed or 1005, rms_disp=1.5, name="cosmo_large")
+    if name == "clustered_large":
+        # BASELINE configs[4] read literally ("generated as in config 3"): the Plummer generator of config 3 at 512^3
+        # (the same sphere number density: 512 * 64 spheres), k-th-neighbour h
+        return clustered_plummer(n_side or 512, seed or 1006, name="clustered_large")
     raise ValueError(f"unknown config {name!r}; choose from {CONFIG_NAMES}")
 
 
