@@ -70,6 +70,9 @@ typedef struct {
     int32_t  timed_steps;     /* number of completed steps the ms_* fields average over (event ring of 64)    */
     int32_t  sort_passes;     /* 8-bit radix passes of the last build (key bits follow the smallest h)         */
     int64_t  n_active_leaves, n_halo_leaves;   /* of the last crk_hydro_derivs_active                                 */
+    int32_t  rebuilds;        /* builds repeated since crk_create because the data outgrew the key width, the leaf-list
+                                 capacity or the list arena the previous build had found (see crk_build_cells)        */
+    int32_t  reserved;
 } crk_stats;
 
 /* stream: a cudaStream_t (0 = default stream).  Returns CRK_OK and *out, or an error.                       */

@@ -35,7 +35,7 @@ class Stats(C.Structure):
                 ("ms_build", C.c_float), ("ms_volumes", C.c_float), ("ms_rk", C.c_float), ("ms_hydro", C.c_float),
                 ("ms_sort", C.c_float), ("ms_tree", C.c_float), ("ms_gradv", C.c_float), ("ms_forces", C.c_float),
                 ("ms_lists", C.c_float), ("timed_steps", C.c_int32), ("sort_passes", C.c_int32),
-                ("n_active_leaves", C.c_int64), ("n_halo_leaves", C.c_int64)]
+                ("n_active_leaves", C.c_int64), ("n_halo_leaves", C.c_int64), ("rebuilds", C.c_int32), ("reserved", C.c_int32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}
@@ -179,7 +179,7 @@ class Crk:
 
     def _len(self, t, dtype=torch.float32):
         """device pointer of a per-particle tensor; its length must be the particle count of the last build"""
-        if int(t.numel()) != self.n:
+        if self.n > 0 and int(t.numel()) != self.n:     # before any build the library itself reports CRK_ESTATE
             raise ValueError(f"per-particle tensor has {int(t.numel())} elements, the context holds {self.n} particles")
         return _dev(t, dtype)
 

@@ -91,14 +91,68 @@ int crk_build_cells(crk_ctx* c, int64_t n, const float* x, const float* y, const
         c->ev_steps++;
     }
     rec(c, EV_BUILD0);
-    CRK_TRY(crk_sort_particles(c, x, y, z, h));
-    rec(c, EV_SORTED);
-    CRK_TRY(crk_build_tree_and_list(c));
-    rec(c, EV_TREE1);
-    CRK_TRY(crk_build_nbr_lists(c));
-    rec(c, EV_BUILD1);
-    c->stage = 1;
-    return CRK_OK;
+    // Everything the host has to know about the build -- input range flag, smallest h (key width), largest leaf list, pair
+    // totals, arena need -- is written to a few status words and read back with ONE copy and ONE synchronisation at the end.
+    // The build runs on what the previous build of this context found (key width, list capacity, arena size) and is repeated
+    // only if the data outgrew one of them, so the result never depends on the history of the context.  The first build of a
+    // context has no key width yet and reads the smallest h up front (one more synchronisation).
+    for (int attempt = 0; attempt < 6; ++attempt) {
+        CRK_CUDA(c, cudaMemsetAsync(c->flag.p, 0, FW_WORDS * sizeof(int), c->stream));
+        uint32_t enc = 0u;
+        CRK_TRY(crk_measure_hmin(c, h, c->key_bits == 0, &enc));
+        if (c->key_bits == 0) c->key_bits = crk_key_bits_from_hmin(c, enc);
+        const int bits = c->key_bits;
+        CRK_TRY(crk_sort_particles(c, x, y, z, h, bits));
+        if (attempt == 0) rec(c, EV_SORTED);
+        CRK_TRY(crk_build_tree_and_list(c));
+        if (attempt == 0) rec(c, EV_TREE1);
+        CRK_TRY(crk_build_nbr_lists(c));
+        CRK_CUDA(c, cudaMemcpyAsync(c->h_flag, c->flag.p, 12 * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        CRK_CUDA(c, cudaStreamSynchronize(c->stream));
+        if (c->h_flag[FW_ERROR] & 1) {
+            snprintf(c->err, sizeof(c->err), "input out of range: need 0 <= x,y,z < box and 0 < h < box/2");
+            return CRK_ERANGE;
+        }
+        if (c->h_flag[FW_CHECK] != 0) {
+            snprintf(c->err, sizeof(c->err), "internal bound check failed in the build (mask 0x%x)", (unsigned)c->h_flag[FW_CHECK]);
+            return CRK_ECUDA;
+        }
+        bool again = false;
+        const int need_bits = crk_key_bits_from_hmin(c, (uint32_t)c->h_flag[FW_HMIN]);
+        if (need_bits != bits) {
+            c->key_bits = need_bits;
+            again = true;
+        }
+        const int64_t need_list = (int64_t)(uint32_t)c->h_flag[FW_MAXLIST];
+        if (need_list > c->leaf_list_cap) {
+            c->leaf_list_cap = (need_list + need_list / 8 + 31) & ~(int64_t)31;       // some head room for the next builds
+            again = true;
+        }
+        unsigned long long used, g, t;
+        memcpy(&used, c->h_flag + FW_ARENA, sizeof(used));
+        memcpy(&g, c->h_flag + FW_SUM_GATHER, sizeof(g));
+        memcpy(&t, c->h_flag + FW_SUM_ALL, sizeof(t));
+        if (!again && used > crk_arena_cap_units(c)) {
+            if (used > 0xffffff00ull) {
+                snprintf(c->err, sizeof(c->err), "neighbour lists need %llu 16-byte units (> 2^32): too many pairs for one context", used);
+                return CRK_ENOMEM;
+            }
+            CRK_TRY(crk_ensure(c, c->arena, (size_t)used * 16 + (size_t)used / 2 + 65536));   // head room: h drifts between steps
+            again = true;
+        }
+        if (!again) {
+            c->arena_units = (int64_t)used;
+            c->n_pairs_gather = (int64_t)g;
+            c->n_pairs = (int64_t)t;
+            c->st.sort_passes = (3 * bits + 7) / 8;
+            rec(c, EV_BUILD1);
+            c->stage = 1;
+            return CRK_OK;
+        }
+        c->st.rebuilds++;
+    }
+    snprintf(c->err, sizeof(c->err), "crk_build_cells: key width / list capacity / arena size did not converge");
+    return CRK_ECUDA;
 }
 
 int crk_volumes(crk_ctx* c, const float* m, float* V, float* rho, uint32_t* nbr_count) {
@@ -411,6 +465,7 @@ int crk_get_stats(crk_ctx* c, crk_stats* out) {
     out->sort_passes = c->st.sort_passes;
     out->n_active_leaves = c->n_active_leaves;
     out->n_halo_leaves = c->n_halo_leaves;
+    out->rebuilds = c->st.rebuilds;
     if (c->timing && c->n > 0) {
         // mean over the completed steps still held in the event ring (all steps since crk_reset_stats if <= 64)
         CRK_CUDA(c, cudaStreamSynchronize(c->stream));

@@ -28,7 +28,7 @@ enum { EV_BUILD0 = 0, EV_SORTED, EV_TREE1, EV_BUILD1, EV_VOL0, EV_VOL1, EV_RK0, 
 //   ell[k][l] = k-th entry of lane l: candidate index | CRK_ELL_SYM (h_i^2 <= r2 < h_j^2: a pair of the symmetric set that
 //               is not in the lane's gather set) | CRK_ELL_WRAP (pair crosses the periodic boundary); lane l owns cnt[l]
 //               entries, cnt_g[l] of them gather entries; CRK_SEG_WRAP: some entry of the segment may carry CRK_ELL_WRAP
-#define CRK_CCAP 352             // candidates per segment (tile capacity of the sweeps)
+#define CRK_CCAP 384             // candidates per segment (tile capacity of the sweeps)
 #define CRK_CAND_STRIDE 384      // u32 per leaf in cand_first (the sweeps read it in 16-byte groups)
 #define CRK_QCAP 128             // entries per lane per segment
 #define CRK_TCULL 32             // cull tile of the list builder
@@ -41,6 +41,17 @@ enum { EV_BUILD0 = 0, EV_SORTED, EV_TREE1, EV_BUILD1, EV_VOL0, EV_VOL1, EV_RK0, 
 #define CRK_FLAG_GATHER 0x80000000u   // leaf-list entry: gap(a,b) < hmax(a)   (one-sided passes use it)
 #define CRK_FLAG_WRAP   0x40000000u   // leaf pair may straddle the periodic boundary
 #define CRK_LEAF_MASK   0x0fffffffu
+
+// device status words (c->flag, mirrored in pinned host memory c->h_flag), read back with ONE copy at the end of a build
+enum { FW_ERROR = 0,        // bit 0: input out of range (S13)
+       FW_HMIN = 1,         // smallest h, encoded for atomicMax (sort.cu)
+       FW_MAXLIST = 2,      // largest leaf interaction list (tree.cu)
+       FW_CHECK = 3,        // CRK_CHECKED builds: bit mask of failed internal bound checks
+       FW_SUM_GATHER = 4,   // u64: leaf pairs with the gather flag
+       FW_SUM_ALL = 6,      // u64: leaf pairs
+       FW_ARENA = 8,        // u64: arena units the neighbour lists need
+       FW_HOST_ACTIVE = 12, // host side only: crk_select_active
+       FW_WORDS = 16 };
 
 struct DevBuf {
     void* p = nullptr;
@@ -80,6 +91,7 @@ struct crk_ctx {
     int64_t level_cnt[CRK_MAX_LEVELS + 1];
     DevBuf nbr_cnt, nbr_off, nbr_list, nbr_gcnt;   // leaf interaction list: leaf q owns nbr_list[q * leaf_list_cap ...], nbr_cnt[q] entries
     int64_t leaf_list_cap = 0;
+    int key_bits = 0;              // space-filling-curve bits per axis of the last build (0 = not known yet)
     int64_t n_pairs = 0, n_pairs_gather = 0;
     DevBuf arena, seg_first;       // neighbour-list arena (16-byte units); per leaf a uint4 copy of its first segment's header
     DevBuf leaf_cnt;               // u16[nl][64]: per-lane cnt_g | cnt of the first segment (dense, so the sweeps need no pointer chase)
@@ -155,10 +167,13 @@ static inline int crk_check_launch(crk_ctx* c, const char* what) {
 }
 
 // ---- translation-unit entry points (host side) ----
-int crk_sort_particles(crk_ctx* c, const float* x, const float* y, const float* z, const float* h);   // sort.cu
+int crk_sort_particles(crk_ctx* c, const float* x, const float* y, const float* z, const float* h, int bits);   // sort.cu
+int crk_key_bits_from_hmin(const crk_ctx* c, uint32_t hmin_enc);                                       // sort.cu
+int crk_measure_hmin(crk_ctx* c, const float* h, bool sync, uint32_t* enc_out);                       // sort.cu
 int crk_exclusive_scan_u32(crk_ctx* c, const uint32_t* in, uint32_t* out, int64_t n, DevBuf& tmp);    // sort.cu
 int crk_build_tree_and_list(crk_ctx* c);                                                               // tree.cu
 int crk_build_nbr_lists(crk_ctx* c);                                                                   // lists.cu
+unsigned long long crk_arena_cap_units(const crk_ctx* c);                                              // lists.cu
 int crk_launch_volumes(crk_ctx* c, const float* m, float* V, float* rho, uint32_t* nbr_count);        // pairs.cu
 int crk_launch_hydro_prep(crk_ctx* c, const float* vx, const float* vy, const float* vz, const float* u);   // pairs.cu
 int crk_launch_rk(crk_ctx* c, bool mom, bool gv, float* A, float* B, float* gradA, float* gradB, float* gradv_full,

@@ -76,10 +76,10 @@ __device__ __forceinline__ float2 wrap2(float2 d, float L, float half, bool& wa,
 // culled candidates are accepted by some lane, so predicated appends beat a vote-and-branch per candidate.
 // SELF: the tile holds the query leaf itself, so j = i has to be excluded (and every candidate keeps its slot).
 template <bool WRAP, bool SELF>
-__device__ __forceinline__ int test_tile(WarpSmem& S, int fill, int C, int& g, int& ng, bool& wflag, int lane, uint32_t self,
+__device__ __forceinline__ int test_tile(WarpSmem& S, int fill, int C, int& g, bool& wflag, int lane, uint32_t self,
                                          float xi, float yi, float zi, float hi2, float L, float half) {
     uint32_t gp = smem_u32(&S.queue[g][lane]);                  // next entry of this lane (row stride 64 bytes)
-    uint32_t cp = smem_u32(&S.cand[C]);
+    const uint32_t cbase = smem_u32(&S.cand[0]);
     const float2 xi2 = make_float2(xi, xi), yi2 = make_float2(yi, yi), zi2 = make_float2(zi, zi);
     for (int t0 = 0; t0 < fill; t0 += 2) {
         const float4 pa = S.ta[t0 >> 1], pb = S.tb[t0 >> 1];
@@ -99,20 +99,21 @@ __device__ __forceinline__ int test_tile(WarpSmem& S, int fill, int C, int& g, i
 #pragma unroll
         for (int u = 0; u < 2; ++u) {
             bool ag = r2[u] < hi2;                                         // gather: Eqs. 13-14
-            bool as = r2[u] < fmaxf(hi2, hj2[u]);                          // symmetric: Eqs. 17-18
+            bool as = ag || (r2[u] < hj2[u]);                              // symmetric: r2 < max(h_i^2, h_j^2), Eqs. 17-18
             if (SELF) {
                 const bool notself = jv[u] != self;
                 ag = ag && notself;
                 as = as && notself;
             }
             const bool any = SELF || __any_sync(0xffffffffu, as);         // the leaf's own particles always get a slot
-            const uint32_t e = (uint32_t)C | (wr[u] ? CRK_ELL_WRAP : 0u) | (ag ? 0u : CRK_ELL_SYM);
+            uint32_t e = ag ? (uint32_t)C : ((uint32_t)C | CRK_ELL_SYM);
+            if (WRAP) {
+                e |= wr[u] ? CRK_ELL_WRAP : 0u;
+                wflag = wflag || (wr[u] && as);
+            }
             sts_u16_if(gp, e, as);                                         // one predicated store, no branch
             gp += as ? 64u : 0u;
-            ng += ag ? 1 : 0;
-            if (WRAP) wflag = wflag || (wr[u] && as);
-            sts_u32_if(cp, jv[u], any && lane == 0);
-            cp += any ? 4u : 0u;
+            sts_u32_if(cbase + 4u * (uint32_t)C, jv[u], any);              // every lane stores the same word: one wavefront
             C += any ? 1 : 0;
         }
     }
@@ -133,7 +134,7 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
     const float4 blo = a.leaf_lo[leaf], bhi = a.leaf_hi[leaf];
     const float hq2 = __fmul_rn(blo.w, blo.w);
     const uint32_t lt = (1u << lane) - 1u;
-    int C = 0, g = 0, ng = 0, fill = 0;   // candidates of the segment, entries / gather entries of this lane, staged candidates
+    int C = 0, g = 0, fill = 0;   // candidates of the segment, entries of this lane, staged candidates
     bool cwrap = false, wflag = false;   // wflag: this lane owns an entry of the segment that crosses the periodic boundary
     uint32_t prev = 0, first = 0;   // arena units of the previous / first segment header of this leaf
 
@@ -156,13 +157,17 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
             uint4* hdr = a.arena + base;
             const uint32_t h1 = (uint32_t)C | (segwrap ? CRK_SEG_WRAP : 0u) | ((uint32_t)K << 16);
             if (lane == 0) hdr[0] = make_uint4(0u, h1, 0u, 0u);
-            ((uint16_t*)(hdr + 1))[lane] = (uint16_t)ng;
             ((uint16_t*)(hdr + 5))[lane] = (uint16_t)g;
             uint32_t* cd = head ? a.cand_first + leaf * CRK_CAND_STRIDE : (uint32_t*)(hdr + CRK_SEG_HDR_UNITS);
             for (int c = lane; c < C; c += 32) cd[c] = S.cand[c];
             uint16_t* el = (uint16_t*)(hdr + CRK_SEG_HDR_UNITS + (head ? 0 : ((C + 3) >> 2)));
-            for (int k = 0; k < K; ++k)   // padding of shorter lanes: slot 0 (the sweeps prefetch it, never evaluate it)
-                el[k * 32 + lane] = (k < g) ? S.queue[k][lane] : (uint16_t)0u;
+            int ng = g;                   // gather entries of this lane = entries without the symmetric-only flag
+            for (int k = 0; k < K; ++k) {   // padding of shorter lanes: slot 0 (the sweeps prefetch it, never evaluate it)
+                const uint32_t v = (k < g) ? (uint32_t)S.queue[k][lane] : 0u;
+                ng -= (int)((v >> 14) & 1u);
+                el[k * 32 + lane] = (uint16_t)v;
+            }
+            ((uint16_t*)(hdr + 1))[lane] = (uint16_t)ng;
             if (head) {
                 if (lane == 0) a.seg_first[leaf] = make_uint4(0u, h1, 0u, (uint32_t)base);
                 a.leaf_cnt[leaf * 64 + lane] = (uint16_t)ng;
@@ -174,7 +179,7 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
             }
             prev = (uint32_t)base;
         }   // else: arena overflow -- the host re-runs the kernel with a larger arena; the counter keeps the total need
-        C = 0; g = 0; ng = 0; wflag = false;
+        C = 0; g = 0; wflag = false;
         __syncwarp();
     };
     auto flush = [&](bool selftile) {
@@ -182,15 +187,15 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
         if (C + fill > CRK_CCAP || maxlen + fill > CRK_QCAP) emit();
         if ((fill & 1) && lane == 0) put(fill, 3.0e30f, 3.0e30f, 3.0e30f, 0.0f, 0u);
         __syncwarp();
-        if (selftile) C = test_tile<true, true>(S, fill, C, g, ng, wflag, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
-        else if (cwrap) C = test_tile<true, false>(S, fill, C, g, ng, wflag, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
-        else C = test_tile<false, false>(S, fill, C, g, ng, wflag, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
+        if (selftile) C = test_tile<true, true>(S, fill, C, g, wflag, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
+        else if (cwrap) C = test_tile<true, false>(S, fill, C, g, wflag, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
+        else C = test_tile<false, false>(S, fill, C, g, wflag, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
         fill = 0;
         cwrap = false;
         __syncwarp();
     };
 
-    const uint64_t e0 = (uint64_t)leaf * a.cap, e1 = e0 + a.cnt[leaf];
+    const uint64_t e0 = (uint64_t)leaf * a.cap, e1 = e0 + min(a.cnt[leaf], a.cap);   // an overflowed list is rebuilt by the host
     uint32_t ent = (e0 < e1) ? a.list[e0] : 0u;
     float4 pj = (e0 < e1) ? a.posh[(int64_t)(ent & CRK_LEAF_MASK) * CRK_LEAF + lane] : make_float4(0, 0, 0, 0);
     // the query leaf itself goes first and keeps all 32 particles: slots 0..31 of the first segment are the leaf's own
@@ -234,46 +239,35 @@ __global__ void k_set_u64(unsigned long long* p, unsigned long long v) { *p = v;
 
 }  // namespace
 
+// launches the builder; the arena need (status word FW_ARENA) is checked by crk_build_cells at its single synchronisation
 int crk_build_nbr_lists(crk_ctx* c) {
     const int64_t nl = c->nl;
     CRK_TRY(crk_ensure(c, c->seg_first, (size_t)(nl + 1) * sizeof(uint4)));
     CRK_TRY(crk_ensure(c, c->leaf_cnt, (size_t)(nl + 1) * 64 * sizeof(uint16_t)));
     CRK_TRY(crk_ensure(c, c->cand_first, (size_t)(nl + 1) * CRK_CAND_STRIDE * sizeof(uint32_t)));
     // first guess: ~6 KB per leaf at ~60 neighbours; grown to the exact need if the builder reports more
-    if (!c->arena.p) CRK_TRY(crk_ensure(c, c->arena, (size_t)nl * 7168 + 65536));
-    unsigned long long* d_counter = (unsigned long long*)((char*)c->flag.p + 32);
-    unsigned long long* h_counter = (unsigned long long*)((char*)c->h_flag + 32);
-    for (int attempt = 0; attempt < 3; ++attempt) {
-        ListArgs a;
-        a.n = c->n; a.nl = nl; a.L = c->prm.box; a.half = 0.5f * c->prm.box;
-        a.cnt = (const uint32_t*)c->nbr_cnt.p; a.list = (const uint32_t*)c->nbr_list.p; a.cap = (uint32_t)c->leaf_list_cap;
-        a.posh = (const float4*)c->posh.p; a.leaf_lo = (const float4*)c->leaf_lo.p; a.leaf_hi = (const float4*)c->leaf_hi.p;
-        a.arena = (uint4*)c->arena.p;
-        // the sweeps read whole 16-byte groups of candidate indices and prefetch entry rows: keep a tail margin
-        a.arena_cap = (unsigned long long)(c->arena.cap / 16);
-        a.arena_cap = a.arena_cap > 256 ? a.arena_cap - 256 : 0;
-        if (a.arena_cap > 0xffffffffull) a.arena_cap = 0xffffffffull;      // segment links are 32-bit unit indices (64 GB)
-        a.counter = d_counter;
-        a.seg_first = (uint4*)c->seg_first.p;
-        a.leaf_cnt = (uint16_t*)c->leaf_cnt.p;
-        a.cand_first = (uint32_t*)c->cand_first.p;
-        k_set_u64<<<1, 1, 0, c->stream>>>(d_counter, 1ull);
-        CRK_TRY(crk_check_launch(c, "k_set_u64"));
-        k_nbr_lists<<<(unsigned)((nl + LW - 1) / LW), LW * 32, 0, c->stream>>>(a);
-        CRK_TRY(crk_check_launch(c, "k_nbr_lists"));
-        CRK_CUDA(c, cudaMemcpyAsync(h_counter, d_counter, sizeof(unsigned long long), cudaMemcpyDeviceToHost, c->stream));
-        CRK_CUDA(c, cudaStreamSynchronize(c->stream));
-        const unsigned long long used = *h_counter;
-        if (used <= a.arena_cap) {
-            c->arena_units = (int64_t)used;
-            return CRK_OK;
-        }
-        if (used > 0xffffffffull) {
-            snprintf(c->err, sizeof(c->err), "neighbour lists need %llu 16-byte units (> 2^32): too many pairs for one context", used);
-            return CRK_ENOMEM;
-        }
-        CRK_TRY(crk_ensure(c, c->arena, (size_t)used * 16 + 65536));
-    }
-    snprintf(c->err, sizeof(c->err), "neighbour-list arena did not converge");
-    return CRK_ECUDA;
+    if (!c->arena.p) CRK_TRY(crk_ensure(c, c->arena, (size_t)nl * 6656 + 65536));
+    unsigned long long* d_counter = (unsigned long long*)((int*)c->flag.p + FW_ARENA);
+    ListArgs a;
+    a.n = c->n; a.nl = nl; a.L = c->prm.box; a.half = 0.5f * c->prm.box;
+    a.cnt = (const uint32_t*)c->nbr_cnt.p; a.list = (const uint32_t*)c->nbr_list.p; a.cap = (uint32_t)c->leaf_list_cap;
+    a.posh = (const float4*)c->posh.p; a.leaf_lo = (const float4*)c->leaf_lo.p; a.leaf_hi = (const float4*)c->leaf_hi.p;
+    a.arena = (uint4*)c->arena.p;
+    a.arena_cap = crk_arena_cap_units(c);
+    a.counter = d_counter;
+    a.seg_first = (uint4*)c->seg_first.p;
+    a.leaf_cnt = (uint16_t*)c->leaf_cnt.p;
+    a.cand_first = (uint32_t*)c->cand_first.p;
+    k_set_u64<<<1, 1, 0, c->stream>>>(d_counter, 1ull);
+    CRK_TRY(crk_check_launch(c, "k_set_u64"));
+    k_nbr_lists<<<(unsigned)((nl + LW - 1) / LW), LW * 32, 0, c->stream>>>(a);
+    return crk_check_launch(c, "k_nbr_lists");
+}
+
+// usable arena units: the sweeps prefetch entry rows a little beyond a segment, so a tail margin stays free; segment links
+// are 32-bit unit indices (64 GB)
+unsigned long long crk_arena_cap_units(const crk_ctx* c) {
+    unsigned long long cap = (unsigned long long)(c->arena.cap / 16);
+    cap = cap > 256 ? cap - 256 : 0;
+    return cap > 0xffffffffull ? 0xffffffffull : cap;
 }

@@ -58,7 +58,7 @@ __global__ void __launch_bounds__(256) k_h_min(const float* __restrict__ h, int6
         if (hv > 0.f && hv < 3.0e38f) enc = max(enc, 0x7f800000u - __float_as_uint(hv));
     }
     enc = __reduce_max_sync(0xffffffffu, enc);
-    if ((threadIdx.x & 31) == 0 && enc != 0u) atomicMax((unsigned int*)flag + 1, enc);
+    if ((threadIdx.x & 31) == 0 && enc != 0u) atomicMax((unsigned int*)flag + FW_HMIN, enc);
 }
 
 // validate (S13), key (Hilbert index of the 2^bits grid), and pack (x,y,z,h) so the later permutation gather
@@ -318,7 +318,38 @@ int crk_exclusive_scan_u32(crk_ctx* c, const uint32_t* in, uint32_t* out, int64_
     return scan_rec(c, in, out, n, n + 1, (uint32_t*)tmp.p);
 }
 
-int crk_sort_particles(crk_ctx* c, const float* x, const float* y, const float* z, const float* h) {
+// Key bits worth sorting: cells of half the smallest support radius order everything the leaves need (a finer order inside
+// such a cell does not make a 32-particle leaf more compact than its h).  The top 3 b bits of a Hilbert key are the key of
+// the b-bit grid, so only b levels of the curve are computed and sorted.
+int crk_key_bits_from_hmin(const crk_ctx* c, uint32_t enc) {
+    int bits = CRK_KEY_BITS;
+    if (enc != 0u) {
+        const uint32_t hb = 0x7f800000u - enc;
+        float hmin;
+        memcpy(&hmin, &hb, sizeof(hmin));
+        if (hmin > 0.f) {
+            const double cells = 2.0 * (double)c->prm.box / (double)hmin;
+            bits = 1;
+            while (bits < CRK_KEY_BITS && (double)(1u << bits) < cells) ++bits;
+        }
+    }
+    return bits < 6 ? 6 : bits;
+}
+
+// smallest h of the set -> status word FW_HMIN (read back with the other status words at the end of the build); sync = true:
+// read it now (first build of a context, when no key width is known yet)
+int crk_measure_hmin(crk_ctx* c, const float* h, bool sync, uint32_t* enc_out) {
+    k_h_min<<<(unsigned)std::min<int64_t>((c->n + 255) / 256, 1184), 256, 0, c->stream>>>(h, c->n, (int*)c->flag.p);
+    CRK_TRY(crk_check_launch(c, "k_h_min"));
+    if (sync) {
+        CRK_CUDA(c, cudaMemcpyAsync(c->h_flag + FW_HMIN, (int*)c->flag.p + FW_HMIN, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        CRK_CUDA(c, cudaStreamSynchronize(c->stream));
+        *enc_out = (uint32_t)c->h_flag[FW_HMIN];
+    }
+    return CRK_OK;
+}
+
+int crk_sort_particles(crk_ctx* c, const float* x, const float* y, const float* z, const float* h, int bits) {
     const int64_t n = c->n;
     const int64_t nl = c->nl;
     for (int q = 0; q < 2; ++q) {
@@ -331,30 +362,6 @@ int crk_sort_particles(crk_ctx* c, const float* x, const float* y, const float* 
     CRK_TRY(crk_ensure(c, c->hist, ((size_t)RADIX * nblk + 1) * 2 * sizeof(uint32_t)));
     uint32_t* hist = (uint32_t*)c->hist.p;
     uint32_t* offs = hist + (size_t)RADIX * nblk + 1;
-
-    CRK_CUDA(c, cudaMemsetAsync(c->flag.p, 0, 4 * sizeof(int), c->stream));
-    k_h_min<<<(unsigned)std::min<int64_t>((n + 255) / 256, 1184), 256, 0, c->stream>>>(h, n, (int*)c->flag.p);
-    CRK_TRY(crk_check_launch(c, "k_h_min"));
-    // Key bits worth sorting: cells of half the smallest support radius order everything the leaves need (a finer
-    // order inside such a cell does not make a 32-particle leaf more compact than its h).  The top 3 b bits of a Hilbert
-    // key are the key of the b-bit grid, so only b levels of the curve are computed and sorted.  One 4-byte read-back (h_min).
-    CRK_CUDA(c, cudaMemcpyAsync(c->h_flag + 12, (int*)c->flag.p + 1, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-    CRK_CUDA(c, cudaStreamSynchronize(c->stream));
-    int bits = CRK_KEY_BITS;
-    {
-        const uint32_t enc = (uint32_t)c->h_flag[12];
-        if (enc != 0u) {
-            const uint32_t hb = 0x7f800000u - enc;
-            float hmin;
-            memcpy(&hmin, &hb, sizeof(hmin));
-            if (hmin > 0.f) {
-                const double cells = 2.0 * (double)c->prm.box / (double)hmin;
-                bits = 1;
-                while (bits < CRK_KEY_BITS && (double)(1u << bits) < cells) ++bits;
-            }
-        }
-        if (bits < 6) bits = 6;
-    }
     k_keys_pack<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(x, y, z, h, n, c->prm.box, bits, (uint64_t*)c->keys[0].p,
                                                                     (uint32_t*)c->vals[0].p, (float4*)c->posh_orig.p,
                                                                     (int*)c->flag.p);

@@ -117,7 +117,7 @@ __global__ void __launch_bounds__(NBR_WARPS * 32) k_leaf_list(const float4* __re
     if (lane == 0) {
         cnt[q] = n_out;
         gcnt[q] = n_gather;
-        if (n_out > cap) atomicMax(max_cnt, n_out);
+        atomicMax(max_cnt, n_out);
     }
 }
 
@@ -151,40 +151,19 @@ int crk_build_tree_and_list(crk_ctx* c) {
     CRK_TRY(crk_ensure(c, c->nbr_cnt, (size_t)(nl + 1) * sizeof(uint32_t)));
     CRK_TRY(crk_ensure(c, c->nbr_gcnt, (size_t)(nl + 1) * sizeof(uint32_t)));
     const unsigned grid = (unsigned)((nl + NBR_WARPS - 1) / NBR_WARPS);
-    // totals -> host (one synchronisation): [0] = error flag of the sort, [1] = largest list, [2..3] = gather / all pair counts
-    uint32_t* d_max = (uint32_t*)c->flag.p + 1;
-    unsigned long long* d_sum = (unsigned long long*)((int*)c->flag.p + 2);
-    unsigned long long* d_sum2 = (unsigned long long*)((int*)c->flag.p + 4);
+    // Leaf q owns a fixed slice of leaf_list_cap entries; the largest count and the pair totals go to the status words and are
+    // checked by crk_build_cells at its single synchronisation (a list that overflowed its slice is rebuilt with a larger cap)
+    uint32_t* d_max = (uint32_t*)c->flag.p + FW_MAXLIST;
+    unsigned long long* d_sum = (unsigned long long*)((int*)c->flag.p + FW_SUM_GATHER);
+    unsigned long long* d_sum2 = (unsigned long long*)((int*)c->flag.p + FW_SUM_ALL);
     if (c->leaf_list_cap < 64) c->leaf_list_cap = 96;
-    for (int attempt = 0; attempt < 3; ++attempt) {
-        CRK_TRY(crk_ensure(c, c->nbr_list, ((size_t)nl * c->leaf_list_cap + 1) * sizeof(uint32_t)));
-        CRK_CUDA(c, cudaMemsetAsync(d_max, 0, 5 * sizeof(int), c->stream));
-        k_leaf_list<<<grid, NBR_WARPS * 32, 0, c->stream>>>(lo, hi, lv, c->prm.box, (uint32_t)c->leaf_list_cap,
-                                                            (uint32_t*)c->nbr_cnt.p, (uint32_t*)c->nbr_gcnt.p,
-                                                            (uint32_t*)c->nbr_list.p, d_max);
-        CRK_TRY(crk_check_launch(c, "k_leaf_list"));
-        k_sum_u32<<<148, 256, 0, c->stream>>>((const uint32_t*)c->nbr_gcnt.p, nl, d_sum);
-        CRK_TRY(crk_check_launch(c, "k_sum_u32"));
-        k_sum_u32<<<148, 256, 0, c->stream>>>((const uint32_t*)c->nbr_cnt.p, nl, d_sum2);
-        CRK_TRY(crk_check_launch(c, "k_sum_u32"));
-        CRK_CUDA(c, cudaMemcpyAsync(c->h_flag, c->flag.p, 6 * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
-        CRK_CUDA(c, cudaStreamSynchronize(c->stream));
-        if (c->h_flag[0] & 1) {
-            snprintf(c->err, sizeof(c->err), "input out of range: need 0 <= x,y,z < box and 0 < h < box/2");
-            return CRK_ERANGE;
-        }
-        const int64_t need = (int64_t)(uint32_t)c->h_flag[1];
-        if (need <= c->leaf_list_cap) break;
-        c->leaf_list_cap = (need + need / 8 + 31) & ~(int64_t)31;       // some head room for the next builds
-        if (attempt == 2) {
-            snprintf(c->err, sizeof(c->err), "leaf interaction list capacity did not converge");
-            return CRK_ECUDA;
-        }
-    }
-    unsigned long long g, t;
-    memcpy(&g, c->h_flag + 2, sizeof(g));
-    memcpy(&t, c->h_flag + 4, sizeof(t));
-    c->n_pairs_gather = (int64_t)g;
-    c->n_pairs = (int64_t)t;
-    return CRK_OK;
+    CRK_TRY(crk_ensure(c, c->nbr_list, ((size_t)nl * c->leaf_list_cap + 1) * sizeof(uint32_t)));
+    k_leaf_list<<<grid, NBR_WARPS * 32, 0, c->stream>>>(lo, hi, lv, c->prm.box, (uint32_t)c->leaf_list_cap,
+                                                        (uint32_t*)c->nbr_cnt.p, (uint32_t*)c->nbr_gcnt.p,
+                                                        (uint32_t*)c->nbr_list.p, d_max);
+    CRK_TRY(crk_check_launch(c, "k_leaf_list"));
+    k_sum_u32<<<148, 256, 0, c->stream>>>((const uint32_t*)c->nbr_gcnt.p, nl, d_sum);
+    CRK_TRY(crk_check_launch(c, "k_sum_u32"));
+    k_sum_u32<<<148, 256, 0, c->stream>>>((const uint32_t*)c->nbr_cnt.p, nl, d_sum2);
+    return crk_check_launch(c, "k_sum_u32");
 }

@@ -1,7 +1,7 @@
 """GPU parity: the CUDA library (through its C ABI / thin binding) against the FP64 CPU oracle, element by element,
 on identical seeded inputs.  Bars (BASELINE.json north_star):
   * neighbour counts / pair counts: bit-exact
-  * V, rho, A: <= 3e-5 relative (max norm);  B, grad A, grad B: <= 1e-4 relative L2 (normalised by rms)
+  * V, rho, A: <= 4e-6 relative (max norm, 2x the measured worst);  B, grad A, grad B: <= 1e-4 relative L2 (normalised by rms)
   * dv/dt, du/dt: <= 1e-4 relative L2 (normalised by rms); conservation invariants <= 1e-5
 Run with `pytest -m gpu` on a B200.
 """
@@ -14,7 +14,9 @@ pytestmark = pytest.mark.gpu
 
 TOL_DERIV = 1e-4
 TOL_INV = 1e-5
-TOL_SCALAR = 3e-5      # max-norm on V, rho, A: FP32 sums of ~60 terms with (1-eta)^6 weights
+TOL_SCALAR = 4e-6      # max-norm on V, rho, A.  Measured maxima over every case of this file (printed as [scalars]): V 1.3e-6,
+                       # rho 1.3e-6 (n_h = 4, 268-term FP32 sums), A 1.8e-6 (non-default parameters); the bar is 2x the worst.
+                       # Source: FP32 accumulation of 60-268 kernel terms, each through rsqrt.approx (2^-22) -- DESIGN.md 5.3
 
 
 def _torch():
@@ -271,6 +273,33 @@ def test_kdk_reuse_is_dropped_when_h_evolves():
     a, b = run(False), run(True)
     for qa, qb, k in zip(a, b, names):
         assert np.array_equal(qa, qb), k
+
+
+def test_build_does_not_depend_on_the_history_of_the_context():
+    """crk_build_cells runs on the key width, leaf-list capacity and arena size the previous build found and synchronises once;
+    if the new data outgrew one of them the build is repeated.  A context that has seen other data must give the bits of a
+    fresh one (different smallest h -> different key width; denser lists -> larger capacity / arena)."""
+    torch = _torch()
+    from paper_2202_02840_b200 import Crk
+    dev = torch.device("cuda:0")
+    names = ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")
+    sets = [wl.tiny_uniform(), wl.clustered_plummer(n_side=20), wl.zeldovich(n_side=24), wl.tiny_uniform(n_side=10)]
+    sets[3].h = (sets[3].h * np.float32(1.6)).astype(np.float32)          # 4x the neighbours, lists outgrow the first guess
+
+    def evaluate(ctx, ps):
+        t = [torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).to(dev) for k in names]
+        out = ctx.step_derivs(*t)
+        torch.cuda.synchronize()
+        return [o.cpu().numpy() for o in out]
+
+    fresh = [evaluate(Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h), ps) for ps in sets]
+    used = Crk(box=sets[0].box, gamma=sets[0].gamma, n_h=sets[0].n_h)
+    for order in ((0, 1, 2, 3), (3, 2, 1, 0), (1, 1, 3, 0)):
+        for k in order:
+            got = evaluate(used, sets[k])
+            for a, b in zip(got, fresh[k]):
+                assert np.array_equal(a, b), f"set {k} after other data differs from a fresh context"
+    assert used.stats()["rebuilds"] >= 1
 
 
 def test_step_derivs_and_host_entry_match_staged_calls():
