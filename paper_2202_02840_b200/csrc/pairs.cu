@@ -141,6 +141,18 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
     const uint32_t tile_s = (uint32_t)__cvta_generic_to_shared(tile);
     uint32_t unit;
     Seg s = first_seg(a, leaf, lane, unit);
+    // the dense per-leaf arrays of a leaf that a later wave of CTAs will sweep (two waves ahead: 148 SMs x leaves in flight per
+    // SM x 2): into L2 now, so that its prologue finds header, counts and candidate indices there instead of in DRAM
+    if (wl == 0) {
+        const int64_t lf = leaf + (WPL == 1 ? 4736 : 1184);
+        if (lf < a.nl) {
+            const char* pa = nullptr;
+            if (lane < 12) pa = (const char*)(a.cand_first + lf * CRK_CAND_STRIDE) + lane * 128;
+            else if (lane == 12) pa = (const char*)(a.leaf_cnt + lf * 64);
+            else if (lane == 13) pa = (const char*)(a.seg_first + lf);
+            if (pa) asm volatile("prefetch.global.L2 [%0];" ::"l"(pa));
+        }
+    }
     while (unit != 0u) {
         const int rows = s.K;
         const int mine = s.ct;
@@ -635,7 +647,7 @@ __device__ __forceinline__ PState load_pstate(const float4* __restrict__ f, int6
     s.gxy = a8.x; s.gxz = a8.y; s.gyz = a8.z; s.qh = a8.w;
     return s;
 }
-constexpr int FPRE = 1;   // planes of the next pair's j-state fetched one pair ahead (3 measured slower: 11.6 vs 11.4 ms)
+constexpr int FPRE = 1;   // planes of the next pair's j-state fetched one pair ahead (3, 5, 9 measured slower: 11.3, 11.5, 13.5 vs 11.1 ms)
 __device__ __forceinline__ PState load_pstate_shared(uint32_t sa, const float4* pre) {
     constexpr uint32_t ST = CRK_CCAP * 16u;
     float4 q[FPL];
