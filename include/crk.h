@@ -19,7 +19,12 @@
  *   - Every array pointer is a DEVICE pointer owned by the caller (except in crk_step_derivs_host), SoA, length n,
  *     float32 / uint32.  Inputs are never modified.  Outputs are written in the caller's particle order.
  *   - Calls are asynchronous on the stream given to crk_create and ordered on it, except that crk_build_cells
- *     synchronises once (it must learn the interaction-list size before allocating it).
+ *     synchronises ONCE at its end: one 48-byte read-back carries the input-range flag, the smallest h (which fixes the
+ *     width of the sort key), the largest leaf list, the pair totals and the size of the neighbour lists.  The build runs
+ *     on what the previous build of the context found for these and is repeated if the data outgrew one of them, so the
+ *     result never depends on the history of the context (crk_stats.rebuilds counts the repeats).  The first build of
+ *     a context synchronises once more, up front, to learn the smallest h.  crk_hydro_derivs_active synchronises once
+ *     (leaf counts); crk_step_derivs_host synchronises at its end; nothing else does.
  *   - State flows build -> volumes -> rk_coefficients -> hydro_derivs inside the context; calling out of order
  *     returns CRK_ESTATE.  The context owns all scratch memory (cudaMalloc, grown on demand, freed by crk_destroy).
  *   - Errors: every call returns CRK_OK (0) or a negative code; nothing aborts or throws across the boundary; there
@@ -52,7 +57,8 @@ typedef struct {
     float C_l, C_q;   /* linear / quadratic viscosity coefficients, (2, 1) in the paper        */
     float eps;        /* 0.1; enters Eq. 25 as eps^2 * hhat^2                                                 */
     int   leaf_size;  /* particles per leaf bucket; must be 32 in this version (one warp lane per particle)   */
-    int   flags;      /* 0, or CRK_FLAG_TIMESTEP: the momentum sweep also reduces what crk_timestep needs        */
+    int   flags;      /* 0 or an OR of CRK_FLAG_TIMESTEP (the momentum sweep also reduces what crk_timestep needs),
+                         CRK_FLAG_KDK_REUSE and CRK_FLAG_KDK_COMPATIBLE (both about crk_kdk_step), defined below       */
 } crk_params;
 
 typedef struct {
@@ -114,11 +120,15 @@ int  crk_compatible_energy(crk_ctx* c, float dt, float* delta_u);
  *   v^1 = v^1/2 + a(x^1, v_p, u_p) dt/2,  u^1 = u^1/2 + udot(x^1, v_p, u_p) dt/2,
  * a and udot from two full crk_step_derivs evaluations (udot = Eq. 18, reading S19).  Errors as
  * crk_step_derivs (CRK_ERANGE if the state leaves the admissible range).  The context is left in the state of the
- * second evaluation (predicted velocities), so crk_timestep / crk_compatible_energy afterwards refer to that state.   */
+ * second evaluation (predicted velocities), so crk_timestep / crk_compatible_energy afterwards refer to that state.
+ * On failure of the SECOND evaluation (e.g. CRK_ERANGE: a predicted position left the admissible range) the arrays are
+ * left at the predicted state x^1, v_p, u_p -- the step is not rolled back; keep a copy if a retry with a smaller dt is
+ * wanted.                                                                                                            */
 /* CRK_FLAG_KDK_REUSE (crk_params.flags): consecutive crk_kdk_step calls on the same arrays reuse sort, tree, neighbour
  * lists, volumes and RK coefficients of the previous step's second evaluation for their first one (same x, h, m).  Set it
- * only if nothing but crk_kdk_step changes x, y, z, h, m between the calls; any crk_build_cells / crk_volumes /
- * crk_rk_coefficients call in between drops the reuse.                                                              */
+ * only if nothing but crk_kdk_step changes x, y, z, h, m between the calls (the check is by array address): any
+ * crk_build_cells / crk_volumes / crk_rk_coefficients call in between drops the reuse, and so does crk_evolve_h (its
+ * caller is about to change h, possibly in place).                                                                  */
 #define CRK_FLAG_KDK_REUSE 2
 /* CRK_FLAG_KDK_COMPATIBLE: the two half kicks of crk_kdk_step advance u with the compatible energy of Eqs. 19-23 (each for
  * its own velocity change and pair accelerations, reading S20) instead of Eq. 18's rate: total energy is then
@@ -139,7 +149,8 @@ int  crk_timestep(crk_ctx* c, float C_cfl, float* dt_min);
 /* ---- NEXT row 3: evolved smoothing length, Eqs. 51-53, PAPER.md:340-354 -----------------------------------------
  * After crk_volumes (else CRK_ESTATE): h_new[i] = h_i (1 - lambda + lambda Delta_N) with Delta_N^3 = N_res / N_i,
  * N_i = (4/3) pi h_i^3 / V_i (Eq. 51), N_res = (4/3) pi n_h^3, lambda of Eq. 53.  h_new: device float[n], caller order,
- * written (may alias nothing the library reads later: the build keeps its own copy of h).  One 40 B/particle stream pass. */
+ * written (may alias nothing the library reads later: the build keeps its own copy of h).  One stream pass that moves 40 B
+ * per particle (two 16-byte packed records, the permutation, the result).                                            */
 int  crk_evolve_h(crk_ctx* c, float* h_new);
 
 /* ---- NEXT row 4b: active / passive particles, PAPER.md:282 ("all ('active') gas leaves that require force updates will
@@ -158,8 +169,9 @@ int  crk_hydro_derivs_active(crk_ctx* c, const uint8_t* active, const float* vx,
 const char* crk_last_error(const crk_ctx* c);
 int  crk_get_perm(crk_ctx* c, int32_t* perm);        /* device int32[n]: perm[k] = caller index of sorted slot k   */
 int  crk_get_gradv(crk_ctx* c, float* gradv);         /* device float[9][n], index 3*a+b = d_b v^a (Eq. 26), caller order */
-/* device uint32[n_leaves][4]: first neighbour-list segment of every leaf = {next segment, C | Kg << 16, K, arena unit};
- * C = candidate slots, Kg / K = rows of the gather / symmetric entry block (layout: csrc/crk_internal.cuh)     */
+/* device uint32[n_leaves][4]: first neighbour-list segment of every leaf = {next segment (0 = none), C | 0x8000 if some entry
+ * crosses the periodic boundary | K << 16, 0, arena unit}; C = candidate slots, K = rows of the entry block (layout:
+ * csrc/crk_internal.cuh)                                                                                       */
 int  crk_get_leaf_segments(crk_ctx* c, uint32_t* seg);
 int  crk_get_stats(crk_ctx* c, crk_stats* out);       /* host struct                                                */
 int  crk_reset_stats(crk_ctx* c);

@@ -17,13 +17,18 @@ LIB = os.path.join(HERE, "libcrk_oracle.so")
 
 
 def build(force: bool = False) -> str:
-    if (not force and os.path.exists(LIB)
-            and os.path.getmtime(LIB) >= max(os.path.getmtime(SRC), os.path.getmtime(HDR))):
-        return LIB
-    cmd = ["g++", "-O2", "-ftree-vectorize", "-std=c++17", "-fopenmp", "-ffp-contract=off", "-mavx2", "-mfma",
-           "-fPIC", "-shared", "-Wall", "-Wextra", "-o", LIB, SRC]
+    """CRK_ORACLE_SANITIZE=1 builds libcrk_oracle_san.so with AddressSanitizer + UndefinedBehaviorSanitizer instead (run the
+    CPU tests with LD_PRELOAD=$(g++ -print-file-name=libasan.so); summary in profiles/r02_sanitizers.md)."""
+    san = os.environ.get("CRK_ORACLE_SANITIZE", "0") == "1"
+    lib = os.path.join(HERE, "libcrk_oracle_san.so") if san else LIB
+    if (not force and os.path.exists(lib)
+            and os.path.getmtime(lib) >= max(os.path.getmtime(SRC), os.path.getmtime(HDR))):
+        return lib
+    opt = ["-O1", "-g", "-fsanitize=address,undefined", "-fno-omit-frame-pointer"] if san else ["-O2", "-ftree-vectorize"]
+    cmd = ["g++"] + opt + ["-std=c++17", "-fopenmp", "-ffp-contract=off", "-mavx2", "-mfma",
+                           "-fPIC", "-shared", "-Wall", "-Wextra", "-o", lib, SRC]
     subprocess.run(cmd, check=True, cwd=HERE)
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":

@@ -7,7 +7,7 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libcrk.so")
+_LIB_PATH = os.environ.get("CRK_LIB") or os.path.join(_HERE, "libcrk.so")   # CRK_LIB: e.g. the range-checked build libcrk_checked.so
 
 EXPORTED_SYMBOLS = (
     "crk_create", "crk_destroy", "crk_build_cells", "crk_volumes", "crk_rk_coefficients", "crk_hydro_derivs",

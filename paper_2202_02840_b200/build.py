@@ -26,15 +26,18 @@ def _newest_dep() -> float:
     return max(os.path.getmtime(p) for p in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
-    if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_dep():
-        return LIB
+def build(force: bool = False, verbose: bool = False, checked: bool = False) -> str:
+    """checked=True: libcrk_checked.so with -DCRK_CHECKED (device-side range checks of every list / tile / arena index; the
+    binding loads it when CRK_LIB points at it)."""
+    lib = os.path.join(HERE, "libcrk_checked.so") if checked else LIB
+    if not force and os.path.exists(lib) and os.path.getmtime(lib) >= _newest_dep():
+        return lib
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    flags = list(NVCC_FLAGS) + (["-Xptxas", "-v"] if verbose else []) + os.environ.get("CRK_NVCC_EXTRA", "").split()
+    flags = list(NVCC_FLAGS) + (["-Xptxas", "-v"] if verbose else []) + (["-DCRK_CHECKED"] if checked else []) + os.environ.get("CRK_NVCC_EXTRA", "").split()
     objs = []
 
     def compile_one(src):
-        obj = os.path.join(CSRC, src.replace(".cu", ".o"))
+        obj = os.path.join(CSRC, src.replace(".cu", ".chk.o" if checked else ".o"))
         cmd = [nvcc] + flags + ["-c", os.path.join(CSRC, src), "-o", obj]
         r = subprocess.run(cmd, capture_output=True, text=True)
         return src, obj, r
@@ -47,10 +50,10 @@ def build(force: bool = False, verbose: bool = False) -> str:
         if r.returncode != 0:
             raise RuntimeError(f"nvcc failed on {src}")
         objs.append(obj)
-    cmd = [nvcc, "-shared", "-o", LIB] + objs + ["-lcudart"]
+    cmd = [nvcc, "-shared", "-o", lib] + objs + ["-lcudart"]
     subprocess.run(cmd, check=True)
-    return LIB
+    return lib
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, checked="--checked" in sys.argv))

@@ -5,6 +5,21 @@ namespace {
 
 void rec(crk_ctx* c, int e) { crk_rec(c, e); }
 
+// CRK_CHECKED builds: synchronise and report a failed device-side bound check of the sweeps just launched
+int check_sweeps(crk_ctx* c, const char* what) {
+#ifdef CRK_CHECKED
+    CRK_CUDA(c, cudaMemcpyAsync(c->h_flag + FW_CHECK, (int*)c->flag.p + FW_CHECK, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    CRK_CUDA(c, cudaStreamSynchronize(c->stream));
+    if (c->h_flag[FW_CHECK] != 0) {
+        snprintf(c->err, sizeof(c->err), "internal bound check failed in %s (mask 0x%x)", what, (unsigned)c->h_flag[FW_CHECK]);
+        return CRK_ECUDA;
+    }
+#else
+    (void)c; (void)what;
+#endif
+    return CRK_OK;
+}
+
 __global__ void k_fp32_peak(float* out, int iters, float b, float cc) {
     float a0 = threadIdx.x * 1e-3f, a1 = a0 + 1.f, a2 = a0 + 2.f, a3 = a0 + 3.f, a4 = a0 + 4.f, a5 = a0 + 5.f,
           a6 = a0 + 6.f, a7 = a0 + 7.f;
@@ -167,6 +182,7 @@ int crk_volumes(crk_ctx* c, const float* m, float* V, float* rho, uint32_t* nbr_
         rec(c, EV_VOL0);
         CRK_TRY(crk_launch_volumes(c, m, V, rho, nbr_count));
         rec(c, EV_VOL1);
+        CRK_TRY(check_sweeps(c, "crk_volumes"));
     }
     c->stage = 2;
     return CRK_OK;
@@ -183,6 +199,7 @@ int crk_rk_coefficients(crk_ctx* c, float* A, float* B, float* gradA, float* gra
         rec(c, EV_RK0);
         CRK_TRY(crk_launch_rk(c, true, false, A, B, gradA, gradB, nullptr));
         rec(c, EV_RK1);
+        CRK_TRY(check_sweeps(c, "crk_rk_coefficients"));
     }
     c->stage = 3;
     return CRK_OK;
@@ -205,6 +222,7 @@ int crk_hydro_derivs(crk_ctx* c, const float* vx, const float* vy, const float* 
         rec(c, EV_GV1);
         CRK_TRY(crk_launch_forces(c, ax, ay, az, dudt, pair_count));
         rec(c, EV_F1);
+        CRK_TRY(check_sweeps(c, "crk_hydro_derivs"));
         if (c->timing) c->ev_done[c->ev_slot] = true;
     }
     c->stage = 4;
@@ -226,7 +244,8 @@ int crk_hydro_derivs_active(crk_ctx* c, const uint8_t* active, const float* vx, 
     CRK_TRY(crk_select_active(c, active, &c->n_active_leaves, &c->n_halo_leaves));
     const int32_t* ids = (const int32_t*)c->act_ids.p;
     CRK_TRY(crk_launch_rk(c, false, true, nullptr, nullptr, nullptr, nullptr, nullptr, ids + c->n_active_leaves, c->n_halo_leaves));
-    return crk_launch_forces(c, ax, ay, az, dudt, nullptr, ids, c->n_active_leaves, active);
+    CRK_TRY(crk_launch_forces(c, ax, ay, az, dudt, nullptr, ids, c->n_active_leaves, active));
+    return check_sweeps(c, "crk_hydro_derivs_active");
 }
 
 // volumes, then moments + 3x3 solve and the velocity-gradient sums in ONE sweep over the lists (same bits as the staged
@@ -249,6 +268,7 @@ static int crk_step_derivs_built(crk_ctx* c, const float* vx, const float* vy, c
     rec(c, EV_GV1);
     CRK_TRY(crk_launch_forces(c, ax, ay, az, dudt, nullptr));
     rec(c, EV_F1);
+    CRK_TRY(check_sweeps(c, "crk_step_derivs"));
     if (c->timing) c->ev_done[c->ev_slot] = true;
     c->stage = 4;
     return CRK_OK;
@@ -420,7 +440,8 @@ int crk_compatible_energy(crk_ctx* c, float dt, float* delta_u) {
         return CRK_ESTATE;
     }
     if (c->n == 0) return CRK_OK;
-    return crk_launch_compat(c, dt, dt, 0.0f, nullptr, nullptr, nullptr, delta_u);
+    CRK_TRY(crk_launch_compat(c, dt, dt, 0.0f, nullptr, nullptr, nullptr, delta_u));
+    return check_sweeps(c, "crk_compatible_energy");
 }
 
 int crk_get_leaf_segments(crk_ctx* c, uint32_t* seg) {

@@ -53,6 +53,16 @@ enum { FW_ERROR = 0,        // bit 0: input out of range (S13)
        FW_HOST_ACTIVE = 12, // host side only: crk_select_active
        FW_WORDS = 16 };
 
+// CRK_CHECKED builds (python -m paper_2202_02840_b200.build --checked -> libcrk_checked.so): every index the list builder and the
+// sweeps form into shared memory, the arena and the particle arrays is range-checked on the device; a failed check sets a
+// bit of the status word FW_CHECK (and the access is skipped or clamped), which the next entry point reports as CRK_ECUDA.
+// compute-sanitizer is not available on the GPU pool this was developed on; this is the stand-in (profiles/r02_sanitizers.md).
+#ifdef CRK_CHECKED
+#define CRK_CHECK(flagp, cond, bit) do { if (!(cond)) atomicOr((int*)(flagp) + FW_CHECK, 1 << (bit)); } while (0)
+#else
+#define CRK_CHECK(flagp, cond, bit) do { } while (0)
+#endif
+
 struct DevBuf {
     void* p = nullptr;
     size_t cap = 0;

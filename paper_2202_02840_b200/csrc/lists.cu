@@ -32,6 +32,7 @@ struct ListArgs {
     uint4* __restrict__ seg_first;         // dense copy of each leaf's first header (.w = its arena unit)
     uint16_t* __restrict__ leaf_cnt;       // [nl][64]
     uint32_t* __restrict__ cand_first;     // [nl][CRK_CAND_STRIDE] candidates of each leaf's first segment
+    int* flag;                             // status words (CRK_CHECKED builds write FW_CHECK)
 };
 
 struct WarpSmem {
@@ -76,7 +77,7 @@ __device__ __forceinline__ float2 wrap2(float2 d, float L, float half, bool& wa,
 // culled candidates are accepted by some lane, so predicated appends beat a vote-and-branch per candidate.
 // SELF: the tile holds the query leaf itself, so j = i has to be excluded (and every candidate keeps its slot).
 template <bool WRAP, bool SELF>
-__device__ __forceinline__ int test_tile(WarpSmem& S, int fill, int C, int& g, bool& wflag, int lane, uint32_t self,
+__device__ __forceinline__ int test_tile(WarpSmem& S, int* flag, int fill, int C, int& g, bool& wflag, int lane, uint32_t self,
                                          float xi, float yi, float zi, float hi2, float L, float half) {
     uint32_t gp = smem_u32(&S.queue[g][lane]);                  // next entry of this lane (row stride 64 bytes)
     const uint32_t cbase = smem_u32(&S.cand[0]);
@@ -111,6 +112,8 @@ __device__ __forceinline__ int test_tile(WarpSmem& S, int fill, int C, int& g, b
                 e |= wr[u] ? CRK_ELL_WRAP : 0u;
                 wflag = wflag || (wr[u] && as);
             }
+            CRK_CHECK(flag, !as || gp < smem_u32(&S.queue[CRK_QCAP - 1][31]) + 2u, 0);   // entry queue row < CRK_QCAP
+            CRK_CHECK(flag, !any || C < CRK_CCAP, 1);                                      // candidate slot < CRK_CCAP
             sts_u16_if(gp, e, as);                                         // one predicated store, no branch
             gp += as ? 64u : 0u;
             sts_u32_if(cbase + 4u * (uint32_t)C, jv[u], any);              // every lane stores the same word: one wavefront
@@ -139,6 +142,7 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
     uint32_t prev = 0, first = 0;   // arena units of the previous / first segment header of this leaf
 
     auto put = [&](int slot, float x, float y, float z, float h2, uint32_t idx) {
+        CRK_CHECK(a.flag, slot >= 0 && slot < CRK_TCULL + 2, 2);                           // cull tile slot
         float* fa = (float*)&S.ta[slot >> 1] + (slot & 1);
         float* fb = (float*)&S.tb[slot >> 1] + (slot & 1);
         fa[0] = -x; fa[2] = -y; fb[0] = -z; fb[2] = h2;
@@ -154,6 +158,7 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
         base = __shfl_sync(0xffffffffu, base, 0);
         __syncwarp();
         if (base + units <= a.arena_cap) {
+            CRK_CHECK(a.flag, K <= CRK_QCAP && C <= CRK_CCAP && base >= 1, 3);                 // segment sizes
             uint4* hdr = a.arena + base;
             const uint32_t h1 = (uint32_t)C | (segwrap ? CRK_SEG_WRAP : 0u) | ((uint32_t)K << 16);
             if (lane == 0) hdr[0] = make_uint4(0u, h1, 0u, 0u);
@@ -187,9 +192,9 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
         if (C + fill > CRK_CCAP || maxlen + fill > CRK_QCAP) emit();
         if ((fill & 1) && lane == 0) put(fill, 3.0e30f, 3.0e30f, 3.0e30f, 0.0f, 0u);
         __syncwarp();
-        if (selftile) C = test_tile<true, true>(S, fill, C, g, wflag, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
-        else if (cwrap) C = test_tile<true, false>(S, fill, C, g, wflag, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
-        else C = test_tile<false, false>(S, fill, C, g, wflag, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
+        if (selftile) C = test_tile<true, true>(S, a.flag, fill, C, g, wflag, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
+        else if (cwrap) C = test_tile<true, false>(S, a.flag, fill, C, g, wflag, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
+        else C = test_tile<false, false>(S, a.flag, fill, C, g, wflag, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
         fill = 0;
         cwrap = false;
         __syncwarp();
@@ -211,6 +216,7 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
             pj = a.posh[(int64_t)(ent & CRK_LEAF_MASK) * CRK_LEAF + lane];
         }
         const int64_t b = (int64_t)(cur & CRK_LEAF_MASK);
+        CRK_CHECK(a.flag, b < a.nl, 4);                                                        // leaf-list entry
         const bool wrap = (cur & CRK_FLAG_WRAP) != 0;
         float gx, gy, gz;
         if (!wrap) {
@@ -258,6 +264,7 @@ int crk_build_nbr_lists(crk_ctx* c) {
     a.seg_first = (uint4*)c->seg_first.p;
     a.leaf_cnt = (uint16_t*)c->leaf_cnt.p;
     a.cand_first = (uint32_t*)c->cand_first.p;
+    a.flag = (int*)c->flag.p;
     k_set_u64<<<1, 1, 0, c->stream>>>(d_counter, 1ull);
     CRK_TRY(crk_check_launch(c, "k_set_u64"));
     k_nbr_lists<<<(unsigned)((nl + LW - 1) / LW), LW * 32, 0, c->stream>>>(a);

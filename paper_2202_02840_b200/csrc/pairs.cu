@@ -44,6 +44,7 @@ struct SweepArgs {
     const int32_t* __restrict__ ids;      // compacted list of leaves to sweep (crk_hydro_derivs_active), or null = all nl leaves
     int64_t n_ids;
     const uint8_t* __restrict__ active;   // per particle, caller order: outputs are written where active[p] != 0 (null = everywhere)
+    int* flag;                            // status words (CRK_CHECKED builds write FW_CHECK)
 };
 
 struct Seg {
@@ -164,12 +165,14 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
             const int k = wl + q * WPL;
             e[q] = (k < rows) ? (uint32_t)__ldg(ep + k * 32) : 0u;
         }
+        CRK_CHECK(a.flag, s.C >= 0 && s.C <= CRK_CCAP && rows >= 0 && rows <= CRK_QCAP && mine <= rows, 8);   // segment header
         group_sync<WPL>(lg);                                   // the previous segment's drain is finished
         // stage: 16-byte asynchronous copies global -> shared (LDGSTS), no register round trip
         for (int c0 = 0; c0 < s.C; c0 += NT * 2) {
             const int ca = c0 + tg, cb = ca + NT;
             const uint32_t ja = (ca < s.C) ? __ldg(s.cand + ca) : 0u;
             const uint32_t jb = (cb < s.C) ? __ldg(s.cand + cb) : 0u;
+            CRK_CHECK(a.flag, (int64_t)ja < a.np && (int64_t)jb < a.np, 9);                 // candidate index
             if (ca < s.C) {
 #pragma unroll
                 for (int p = 0; p < PLANES; ++p) cp_async16(tile_s + (uint32_t)(p * CRK_CCAP + ca) * 16u, planes[p] + ja);
@@ -204,6 +207,7 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
                 float4 nxt[NPRE];
 #pragma unroll
                 for (int p = 0; p < NPRE; ++p) nxt[p] = lds128(tile_s + (uint32_t)(p * CRK_CCAP) * 16u + (en & CRK_ELL_MASK) * 16u);
+                CRK_CHECK(a.flag, k >= mine || (int)(e[q] & CRK_ELL_MASK) < s.C, 10);       // entry -> staged slot
                 if (k < mine && (SYM || !(e[q] & CRK_ELL_SYM)))
                     pair(tile_s + (e[q] & CRK_ELL_MASK) * 16u, (e[q] & CRK_ELL_WRAP) != 0u, cur);
 #pragma unroll
@@ -867,6 +871,7 @@ SweepArgs make_args(crk_ctx* c) {
     a.rho_s = (float*)c->rho_s.p; a.m_s = (const float*)c->m_s.p;
     a.gamma = c->prm.gamma; a.n_h = c->prm.n_h; a.C_l = c->prm.C_l; a.C_q = c->prm.C_q;
     a.eps2 = c->prm.eps * c->prm.eps;
+    a.flag = (int*)c->flag.p;
     return a;
 }
 
