@@ -121,6 +121,7 @@ struct crk_ctx {
     DevBuf vel_orig;               // float4 (vx,vy,vz,u) caller order (packed for a 16-byte gather)
     DevBuf m_s;                    // float, sorted
     DevBuf flag;                   // int[4] device error / status flags
+    DevBuf sched;                  // work counter of the persistent sweeps (pairs.cu)
     DevBuf host_stage;             // device staging for crk_step_derivs_host (13 float arrays)
     int* h_flag = nullptr;         // pinned host mirror
 };

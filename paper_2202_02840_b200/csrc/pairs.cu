@@ -11,6 +11,18 @@
 // Equation numbers refer to /root/reference/PAPER.md; the closed forms of A, B, grad A, grad B are derived in DESIGN.md.
 #include "crk_internal.cuh"
 
+#ifdef CRK_PROBE
+// development probe (never in the product build): per sweep (index = planes in the tile) the summed cycles a group spends
+// staging, the summed cycles of its whole leaf sweep, and the number of leaves
+__device__ unsigned long long crk_probe[48];
+extern "C" int crk_probe_read(unsigned long long* out, int reset) {
+    cudaDeviceSynchronize();
+    cudaMemcpyFromSymbol(out, crk_probe, sizeof(crk_probe));
+    if (reset) { unsigned long long z[48] = {0}; cudaMemcpyToSymbol(crk_probe, z, sizeof(z)); }
+    return 0;
+}
+#endif
+
 namespace {
 
 constexpr float SIGMA_C4 = 4.923856051905513f;     // 495 / (32 pi), Eq. 12
@@ -45,48 +57,35 @@ struct SweepArgs {
     int64_t n_ids;
     const uint8_t* __restrict__ active;   // per particle, caller order: outputs are written where active[p] != 0 (null = everywhere)
     int* flag;                            // status words (CRK_CHECKED builds write FW_CHECK)
+    unsigned int* sched;                  // work counter of the persistent groups (zeroed before every launch)
 };
 
 struct Seg {
-    const uint32_t* cand;
     const uint16_t* ell;
     int C, K, cg, ct;
     bool wrap;               // some entry of the segment may cross the periodic boundary
     uint32_t next;
 };
-// dense: candidate array of a leaf's first segment (cand_first), else the candidates follow the header in the arena
-__device__ __forceinline__ Seg make_seg(const uint4* __restrict__ arena, uint32_t unit, const uint4& h0, int cg, int ct,
-                                        const uint32_t* dense) {
-    const uint4* hdr = arena + unit;
-    Seg s;
-    s.next = h0.x;
-    s.C = (int)(h0.y & 0x7fffu);
-    s.wrap = (h0.y & CRK_SEG_WRAP) != 0u;
-    s.K = (int)(h0.y >> 16);
-    s.cg = cg;
-    s.ct = ct;
-    s.cand = dense ? dense : (const uint32_t*)(hdr + CRK_SEG_HDR_UNITS);
-    s.ell = (const uint16_t*)(hdr + CRK_SEG_HDR_UNITS + (dense ? 0 : ((s.C + 3) >> 2)));
-    return s;
-}
-// first segment: header, per-lane counts and candidates come from the dense per-leaf arrays (no dependent load before the payload)
-__device__ __forceinline__ Seg first_seg(const SweepArgs& a, int64_t leaf, int lane, uint32_t& unit) {
-    const uint4 h0 = __ldg(a.seg_first + leaf);
-    const int cg = (int)__ldg(a.leaf_cnt + leaf * 64 + lane), ct = (int)__ldg(a.leaf_cnt + leaf * 64 + 32 + lane);
-    unit = h0.w;
-    return make_seg(a.arena, unit, h0, cg, ct, a.cand_first + leaf * CRK_CAND_STRIDE);
-}
-__device__ __forceinline__ Seg load_seg(const uint4* __restrict__ arena, uint32_t unit, int lane) {
-    const uint4* hdr = arena + unit;
-    const uint4 h0 = __ldg(hdr);
-    return make_seg(arena, unit, h0, (int)__ldg((const uint16_t*)(hdr + 1) + lane), (int)__ldg((const uint16_t*)(hdr + 5) + lane), nullptr);
-}
+
+// Metadata of the segment a group stages next, in shared memory: the same 105 16-byte chunks a segment carries in the arena
+// (header | cnt_g[32] cnt[32] u16 | cand[CRK_CCAP] u32; a leaf's first segment keeps them in the dense per-leaf arrays).
+// It is fetched with cp.async while the group is still evaluating the rows of the previous segment, so the three dependent
+// loads (header -> candidate indices -> state) that used to open every leaf shrink to the last one.
+struct __align__(16) Meta {
+    uint4 hdr;                    // {next segment unit, C | CRK_SEG_WRAP | K << 16, 0, own unit (first segments only)}
+    uint16_t cnt[64];
+    uint32_t cand[CRK_CCAP];
+    long long next_leaf;          // the group's next work item (-1 = none), written by thread 0 of the group
+    long long pad;
+};
+constexpr int META_CHUNKS = 1 + 8 + CRK_CCAP / 4;
+static_assert(sizeof(Meta) == META_CHUNKS * 16 + 16, "Meta layout");
 
 __device__ __forceinline__ void cp_async16(uint32_t dst_shared, const void* src) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst_shared), "l"(src) : "memory");
 }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 
-__device__ __forceinline__ uint32_t smem_u32addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 // 128-bit shared-memory load from a 32-bit shared address (no generic-address window arithmetic in the inner loops)
 __device__ __forceinline__ float4 lds128(uint32_t addr) {
     float4 v;
@@ -118,11 +117,49 @@ __device__ __forceinline__ void group_sync(int lg) {
     else asm volatile("bar.sync %0, %1;" ::"r"(lg + 1), "r"(WPL * 32) : "memory");
 }
 
+// ---- persistent groups: work distribution and metadata prefetch --------------------------------------------------------
+// A group (WPL warps) serves one leaf at a time and keeps taking leaves from a global counter until none is left; the
+// kernels are launched with as many CTAs as are resident at once.  (One CTA per leaf cost the force sweep 19 % of its time
+// in CTA turnover and 27 % in the dependent loads of the prologue -- measured with clock64 probes, profiles/r02_notes.md.)
+__device__ __forceinline__ long long grab_leaf(const SweepArgs& a) {
+    const long long total = a.ids ? a.n_ids : a.nl;
+    const long long slot = (long long)atomicAdd(a.sched, 1u);
+    if (slot >= total) return -1;
+    return a.ids ? (long long)a.ids[slot] : slot;
+}
+// copies the metadata of a leaf's first segment (unit == 0) or of the arena segment `unit` into m; the caller commits
+template <int NT>
+__device__ __forceinline__ void issue_meta(Meta* m, const SweepArgs& a, long long leaf, uint32_t unit, int tg) {
+    const uint32_t ms = (uint32_t)__cvta_generic_to_shared(m);
+    for (int ch = tg; ch < META_CHUNKS; ch += NT) {
+        const char* src;
+        if (unit != 0u) src = (const char*)(a.arena + unit + ch);
+        else if (ch == 0) src = (const char*)(a.seg_first + leaf);
+        else if (ch < 9) src = (const char*)(a.leaf_cnt + leaf * 64) + (ch - 1) * 16;
+        else src = (const char*)(a.cand_first + leaf * CRK_CAND_STRIDE) + (ch - 9) * 16;
+        cp_async16(ms + (uint32_t)ch * 16u, src);
+    }
+}
+// first work item of a group: returns the leaf (or -1) with the copy of its metadata in flight (committed)
+template <int WPL>
+__device__ __forceinline__ long long sweep_begin(const SweepArgs& a, Meta* m, int lg, int wl, int lane) {
+    const int tg = wl * 32 + lane;
+    if (tg == 0) m->next_leaf = grab_leaf(a);
+    group_sync<WPL>(lg);
+    const long long leaf = m->next_leaf;
+    if (leaf >= 0) issue_meta<WPL * 32>(m, a, leaf, 0u, tg);
+    cp_async_commit();
+    return leaf;
+}
+
 // ---- the sweep over one leaf's segment chain -------------------------------------------------------------------------
 // Rows [0, K) of a segment's entry block; lane l is active while k < cnt[l].  SYM = false (gather set, Eqs. 13-14): entries
 // flagged CRK_ELL_SYM are skipped;  SYM = true (Eqs. 17-18): every entry is a pair.
 // pair(slot_addr, crosses_boundary, plane0) evaluates one accepted pair (slot_addr = shared address of the candidate's
 // plane-0 entry; plane p sits CRK_CCAP * 16 * p bytes further); returns the number of pairs the lane owns.
+// On entry the copy of the leaf's metadata into m is in flight; on exit the group's next leaf is in `next_leaf` and the copy
+// of ITS metadata is in flight.  Barriers per segment: B1 metadata landed and the previous rows are done (tile free);
+// B2 everybody has read the metadata (m may be overwritten) and the next work item is known; B3 the state has landed.
 struct NoInit {
     __device__ __forceinline__ void operator()(uint32_t) const {}
 };
@@ -130,48 +167,53 @@ struct NoInit {
 // order (lists.cu), so a sweep can take its i-state from there instead of loading it from global memory.
 // (Measured and not kept, profiles/r02_notes.md: a second, branch-free instantiation of the row loop for segments without
 // boundary-crossing entries -- 172 instead of 190 instructions per pair of k_forces, but ptxas then sinks the shared loads
-// next to their uses and the sweep loses 1.6 ms to short-scoreboard stalls; candidate indices fetched as 16-byte groups
-// ahead of the header -- +0.5 ms.)
+// next to their uses and the sweep loses 1.6 ms to short-scoreboard stalls.)
 template <int WPL, int PLANES, bool SYM, int NPRE = 1, typename Pair, typename Init = NoInit>
-__device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4* const* planes, int64_t leaf, int lg, int wl,
-                                               int lane, float4* tile, Pair pair, Init init = Init()) {
+__device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4* const* planes, long long leaf, long long& next_leaf,
+                                               int lg, int wl, int lane, float4* tile, Meta* m, Pair pair, Init init = Init()) {
     constexpr int NT = WPL * 32;                                  // threads that serve the leaf
     uint32_t count = 0;
     bool first = true;
     const int tg = wl * 32 + lane;
     const uint32_t tile_s = (uint32_t)__cvta_generic_to_shared(tile);
-    uint32_t unit;
-    Seg s = first_seg(a, leaf, lane, unit);
-    // the dense per-leaf arrays of a leaf that a later wave of CTAs will sweep (two waves ahead: 148 SMs x leaves in flight per
-    // SM x 2): into L2 now, so that its prologue finds header, counts and candidate indices there instead of in DRAM
-    if (wl == 0) {
-        const int64_t lf = leaf + (WPL == 1 ? 4736 : 1184);
-        if (lf < a.nl) {
-            const char* pa = nullptr;
-            if (lane < 12) pa = (const char*)(a.cand_first + lf * CRK_CAND_STRIDE) + lane * 128;
-            else if (lane == 12) pa = (const char*)(a.leaf_cnt + lf * 64);
-            else if (lane == 13) pa = (const char*)(a.seg_first + lf);
-            if (pa) asm volatile("prefetch.global.L2 [%0];" ::"l"(pa));
+    uint32_t unit = 0;                                            // arena unit of the segment being staged (0: not known yet)
+    next_leaf = -1;
+#ifdef CRK_PROBE
+    long long pr_stage = 0, pr_t0 = clock64();
+#endif
+    for (;;) {
+        asm volatile("cp.async.wait_all;" ::: "memory");
+        group_sync<WPL>(lg);                                   // B1
+#ifdef CRK_PROBE
+        const long long pr_s0 = clock64();
+#endif
+        const uint4 h0 = m->hdr;
+        if (first) unit = h0.w;
+        if (unit == 0u) {                                      // a leaf without a segment (cannot happen for a built leaf)
+            if (tg == 0) m->next_leaf = grab_leaf(a);
+            group_sync<WPL>(lg);
+            next_leaf = m->next_leaf;
+            if (next_leaf >= 0) issue_meta<NT>(m, a, next_leaf, 0u, tg);
+            cp_async_commit();
+            break;
         }
-    }
-    while (unit != 0u) {
+        Seg s;
+        s.next = h0.x;
+        s.C = (int)(h0.y & 0x7fffu);
+        s.wrap = (h0.y & CRK_SEG_WRAP) != 0u;
+        s.K = (int)(h0.y >> 16);
+        s.cg = (int)m->cnt[lane];
+        s.ct = (int)m->cnt[32 + lane];
+        s.ell = (const uint16_t*)(a.arena + unit + CRK_SEG_HDR_UNITS + (first ? 0 : ((s.C + 3) >> 2)));
         const int rows = s.K;
         const int mine = s.ct;
         const uint16_t* ep = s.ell + lane;
-        // the first rows of the entry block travel together with the candidate indices
-        uint32_t e[4];
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const int k = wl + q * WPL;
-            e[q] = (k < rows) ? (uint32_t)__ldg(ep + k * 32) : 0u;
-        }
         CRK_CHECK(a.flag, s.C >= 0 && s.C <= CRK_CCAP && rows >= 0 && rows <= CRK_QCAP && mine <= rows, 8);   // segment header
-        group_sync<WPL>(lg);                                   // the previous segment's drain is finished
         // stage: 16-byte asynchronous copies global -> shared (LDGSTS), no register round trip
         for (int c0 = 0; c0 < s.C; c0 += NT * 2) {
             const int ca = c0 + tg, cb = ca + NT;
-            const uint32_t ja = (ca < s.C) ? __ldg(s.cand + ca) : 0u;
-            const uint32_t jb = (cb < s.C) ? __ldg(s.cand + cb) : 0u;
+            const uint32_t ja = (ca < s.C) ? m->cand[ca] : 0u;
+            const uint32_t jb = (cb < s.C) ? m->cand[cb] : 0u;
             CRK_CHECK(a.flag, (int64_t)ja < a.np && (int64_t)jb < a.np, 9);                 // candidate index
             if (ca < s.C) {
 #pragma unroll
@@ -182,8 +224,29 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
                 for (int p = 0; p < PLANES; ++p) cp_async16(tile_s + (uint32_t)(p * CRK_CCAP + cb) * 16u, planes[p] + jb);
             }
         }
-        asm volatile("cp.async.wait_all;" ::: "memory");
-        group_sync<WPL>(lg);
+        cp_async_commit();
+        // the first rows of the entry block travel together with the state
+        uint32_t e[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int k = wl + q * WPL;
+            e[q] = (k < rows) ? (uint32_t)__ldg(ep + k * 32) : 0u;
+        }
+        const bool last = (s.next == 0u);
+        if (last && tg == 0) m->next_leaf = grab_leaf(a);
+        group_sync<WPL>(lg);                                   // B2
+        if (last) {
+            next_leaf = m->next_leaf;
+            if (next_leaf >= 0) issue_meta<NT>(m, a, next_leaf, 0u, tg);
+        } else {
+            issue_meta<NT>(m, a, 0, s.next, tg);
+        }
+        cp_async_commit();
+        asm volatile("cp.async.wait_group 1;" ::: "memory");   // the state copies (the metadata copy may still be in flight)
+        group_sync<WPL>(lg);                                   // B3
+#ifdef CRK_PROBE
+        pr_stage += clock64() - pr_s0;
+#endif
         if (first) {
             init(tile_s);
             first = false;
@@ -217,9 +280,16 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
             for (int q = 0; q < 4; ++q) e[q] = nx[q];
         }
         count += (uint32_t)(SYM ? s.ct : s.cg);
+        if (last) break;
         unit = s.next;
-        if (unit != 0u) s = load_seg(a.arena, unit, lane);
     }
+#ifdef CRK_PROBE
+    if (tg == 0) {
+        atomicAdd(&crk_probe[PLANES * 4 + 0], (unsigned long long)pr_stage);
+        atomicAdd(&crk_probe[PLANES * 4 + 1], (unsigned long long)(clock64() - pr_t0));
+        atomicAdd(&crk_probe[PLANES * 4 + 2], 1ull);
+    }
+#endif
     return count;
 }
 
@@ -285,41 +355,46 @@ __device__ __forceinline__ void sep3(const SweepArgs& a, bool wrapped, float xi,
 // =================================================================================================== a1: volumes
 // Eq. 14: V_i^-1 = n_i = sum_j W(|x_i - x_j|, h_i), self term included (S4); rho_i = m_i / V_i (S2).
 constexpr int W1_WPC = 2;
+constexpr int W1_SMEM = CRK_CCAP * (int)sizeof(float4) + (int)sizeof(Meta);     // per warp
 __global__ void __launch_bounds__(W1_WPC * 32) k_volumes(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int64_t leaf = (int64_t)blockIdx.x * W1_WPC + w;
-    if (leaf >= a.nl) return;
-    float4* tile = (float4*)smem_raw + (size_t)w * CRK_CCAP;
-    const int64_t i = leaf * CRK_LEAF + lane;
-    const bool valid = i < a.n;
-    const float4 pi = a.posh[i];
-    const float xi = pi.x, yi = pi.y, zi = pi.z, hi = pi.w;
-    const float inv_h = valid ? 1.0f / hi : 0.0f;
-    float acc = 0.0f;
+    float4* tile = (float4*)(smem_raw + (size_t)w * W1_SMEM);
+    Meta* meta = (Meta*)(tile + CRK_CCAP);
     const float4* const planes[1] = {a.posh};
-    const uint32_t count = leaf_sweep<1, 1, false>(a, planes, leaf, w, 0, lane, tile, [&](uint32_t, bool wrapped, const float4* pre) {
-        const float4 pj = pre[0];
-        float dx, dy, dz, r2;
-        sep3(a, wrapped, xi, yi, zi, pj, dx, dy, dz, r2);
-        const float r = r2 * rsqrt_fast(fmaxf(r2, R2_TINY));
-        acc += wendland_w(r * inv_h);
-    });
-    if (valid) {
-        const float k3 = SIGMA_C4 * inv_h * inv_h * inv_h;
-        const float ni = k3 * (acc + 1.0f);              // self term W~(0) = 1
-        const float V = 1.0f / ni;
-        const float mi = a.m_s[i];
-        const float rho = mi * ni;
-        a.posV[i] = make_float4(xi, yi, zi, V);
-        a.rho_s[i] = rho;
-        const int32_t p = a.perm[i];
-        if (a.o0) a.o0[p] = V;
-        if (a.o1) a.o1[p] = rho;
-        if (a.ocnt) a.ocnt[p] = count;
-    } else {
-        a.posV[i] = make_float4(pi.x, pi.y, pi.z, 0.0f);
-        a.rho_s[i] = 0.0f;
+    long long leaf = sweep_begin<1>(a, meta, w, 0, lane);
+    while (leaf >= 0) {
+        const int64_t i = leaf * CRK_LEAF + lane;
+        const bool valid = i < a.n;
+        const float4 pi = a.posh[i];
+        const float xi = pi.x, yi = pi.y, zi = pi.z, hi = pi.w;
+        const float inv_h = valid ? 1.0f / hi : 0.0f;
+        float acc = 0.0f;
+        long long next;
+        const uint32_t count = leaf_sweep<1, 1, false>(a, planes, leaf, next, w, 0, lane, tile, meta, [&](uint32_t, bool wrapped, const float4* pre) {
+            const float4 pj = pre[0];
+            float dx, dy, dz, r2;
+            sep3(a, wrapped, xi, yi, zi, pj, dx, dy, dz, r2);
+            const float r = r2 * rsqrt_fast(fmaxf(r2, R2_TINY));
+            acc += wendland_w(r * inv_h);
+        });
+        if (valid) {
+            const float k3 = SIGMA_C4 * inv_h * inv_h * inv_h;
+            const float ni = k3 * (acc + 1.0f);              // self term W~(0) = 1
+            const float V = 1.0f / ni;
+            const float mi = a.m_s[i];
+            const float rho = mi * ni;
+            a.posV[i] = make_float4(xi, yi, zi, V);
+            a.rho_s[i] = rho;
+            const int32_t p = a.perm[i];
+            if (a.o0) a.o0[p] = V;
+            if (a.o1) a.o1[p] = rho;
+            if (a.ocnt) a.ocnt[p] = count;
+        } else {
+            a.posV[i] = make_float4(pi.x, pi.y, pi.z, 0.0f);
+            a.rho_s[i] = 0.0f;
+        }
+        leaf = next;
     }
 }
 
@@ -412,219 +487,226 @@ k_rk(SweepArgs a, const float* __restrict__ u_s, float* __restrict__ gv_full) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     constexpr int PL = GV ? 2 : 1;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int64_t slot = (int64_t)blockIdx.x * W2_WPC + w;
-    if (slot >= (a.ids ? a.n_ids : a.nl)) return;
-    const int64_t leaf = a.ids ? (int64_t)a.ids[slot] : slot;
-    float4* tile = (float4*)smem_raw + (size_t)w * PL * CRK_CCAP;
-    const int64_t i = leaf * CRK_LEAF + lane;
-    const bool valid = i < a.n;
-    const float4 ph = a.posh[i];
-    const float xi = ph.x, yi = ph.y, zi = ph.z, hi = ph.w;
-    const float inv_h = valid ? 1.0f / hi : 0.0f;
-    float4 vi = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (GV) vi = a.velV[i];
-    // moment accumulators: s0; s1[3]; s2[6] (xx,xy,xz,yy,yz,zz); t0[3]; t1[6]; t2[10] (xxx,xxy,xxz,xyy,xyz,xzz,yyy,yyz,yzz,zzz)
-    float s0 = 0.f, s1[3] = {0.f, 0.f, 0.f}, s2[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    float t0[3] = {0.f, 0.f, 0.f}, t1[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, t2[10] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
-    // velocity sums, [a][..]
-    float S0[3], S1[3][3], T1[3][3], T2[3][6];
-#pragma unroll
-    for (int q = 0; q < 3; ++q) {
-        S0[q] = 0.f;
-#pragma unroll
-        for (int r = 0; r < 3; ++r) { S1[q][r] = 0.f; T1[q][r] = 0.f; }
-#pragma unroll
-        for (int r = 0; r < 6; ++r) T2[q][r] = 0.f;
-    }
+    constexpr int WSMEM = PL * CRK_CCAP * (int)sizeof(float4) + (int)sizeof(Meta);     // per warp
+    float4* tile = (float4*)(smem_raw + (size_t)w * WSMEM);
+    Meta* meta = (Meta*)(tile + PL * CRK_CCAP);
     const float4* planes[2] = {a.posV, GV ? a.velV : a.posV};
-    leaf_sweep<1, PL, false>(a, planes, leaf, w, 0, lane, tile, [&](uint32_t sa, bool wrapped, const float4* pre) {
-        const float4 pj = pre[0];
-        float dx, dy, dz, r2;
-        sep3(a, wrapped, xi, yi, zi, pj, dx, dy, dz, r2);
-        const float r = __fmul_rn(r2, rsqrt_fast(fmaxf(r2, R2_TINY)));
-        float Wt, Dt;
-        wendland(__fmul_rn(r, inv_h), Wt, Dt);
-        const float wv = __fmul_rn(pj.w, Wt), gv = __fmul_rn(pj.w, Dt);
-        const float x[3] = {__fmul_rn(dx, inv_h), __fmul_rn(dy, inv_h), __fmul_rn(dz, inv_h)};
-        const float m2[6] = {__fmul_rn(x[0], x[0]), __fmul_rn(x[0], x[1]), __fmul_rn(x[0], x[2]),
-                             __fmul_rn(x[1], x[1]), __fmul_rn(x[1], x[2]), __fmul_rn(x[2], x[2])};
-        if (MOM) {
-            s0 = __fadd_rn(s0, wv);
+    long long leaf = sweep_begin<1>(a, meta, w, 0, lane);
+    while (leaf >= 0) {
+        long long next;
+        const int64_t i = leaf * CRK_LEAF + lane;
+        const bool valid = i < a.n;
+        const float4 ph = a.posh[i];
+        const float xi = ph.x, yi = ph.y, zi = ph.z, hi = ph.w;
+        const float inv_h = valid ? 1.0f / hi : 0.0f;
+        float4 vi = make_float4(0.f, 0.f, 0.f, 0.f);
+        if (GV) vi = a.velV[i];
+        // moment accumulators: s0; s1[3]; s2[6] (xx,xy,xz,yy,yz,zz); t0[3]; t1[6]; t2[10] (xxx,xxy,xxz,xyy,xyz,xzz,yyy,yyz,yzz,zzz)
+        float s0 = 0.f, s1[3] = {0.f, 0.f, 0.f}, s2[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        float t0[3] = {0.f, 0.f, 0.f}, t1[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, t2[10] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
+        // velocity sums, [a][..]
+        float S0[3], S1[3][3], T1[3][3], T2[3][6];
 #pragma unroll
-            for (int q = 0; q < 3; ++q) {
-                s1[q] = __fmaf_rn(wv, x[q], s1[q]);
-                t0[q] = __fmaf_rn(gv, x[q], t0[q]);
-            }
-            float g2[6];
+        for (int q = 0; q < 3; ++q) {
+            S0[q] = 0.f;
 #pragma unroll
-            for (int q = 0; q < 6; ++q) {
-                s2[q] = __fmaf_rn(wv, m2[q], s2[q]);
-                g2[q] = __fmul_rn(gv, m2[q]);
-                t1[q] = __fadd_rn(t1[q], g2[q]);
-            }
-            t2[0] = __fmaf_rn(g2[0], x[0], t2[0]); t2[1] = __fmaf_rn(g2[0], x[1], t2[1]); t2[2] = __fmaf_rn(g2[0], x[2], t2[2]);
-            t2[3] = __fmaf_rn(g2[1], x[1], t2[3]); t2[4] = __fmaf_rn(g2[1], x[2], t2[4]); t2[5] = __fmaf_rn(g2[2], x[2], t2[5]);
-            t2[6] = __fmaf_rn(g2[3], x[1], t2[6]); t2[7] = __fmaf_rn(g2[3], x[2], t2[7]); t2[8] = __fmaf_rn(g2[4], x[2], t2[8]);
-            t2[9] = __fmaf_rn(g2[5], x[2], t2[9]);
+            for (int r = 0; r < 3; ++r) { S1[q][r] = 0.f; T1[q][r] = 0.f; }
+#pragma unroll
+            for (int r = 0; r < 6; ++r) T2[q][r] = 0.f;
         }
-        if (GV) {
-            const float4 vj = lds128(sa + CRK_CCAP * 16u);
-            const float u[3] = {__fsub_rn(vi.x, vj.x), __fsub_rn(vi.y, vj.y), __fsub_rn(vi.z, vj.z)};
+        leaf_sweep<1, PL, false>(a, planes, leaf, next, w, 0, lane, tile, meta, [&](uint32_t sa, bool wrapped, const float4* pre) {
+            const float4 pj = pre[0];
+            float dx, dy, dz, r2;
+            sep3(a, wrapped, xi, yi, zi, pj, dx, dy, dz, r2);
+            const float r = __fmul_rn(r2, rsqrt_fast(fmaxf(r2, R2_TINY)));
+            float Wt, Dt;
+            wendland(__fmul_rn(r, inv_h), Wt, Dt);
+            const float wv = __fmul_rn(pj.w, Wt), gv = __fmul_rn(pj.w, Dt);
+            const float x[3] = {__fmul_rn(dx, inv_h), __fmul_rn(dy, inv_h), __fmul_rn(dz, inv_h)};
+            const float m2[6] = {__fmul_rn(x[0], x[0]), __fmul_rn(x[0], x[1]), __fmul_rn(x[0], x[2]),
+                                 __fmul_rn(x[1], x[1]), __fmul_rn(x[1], x[2]), __fmul_rn(x[2], x[2])};
+            if (MOM) {
+                s0 = __fadd_rn(s0, wv);
 #pragma unroll
-            for (int q = 0; q < 3; ++q) {
-                const float uw = __fmul_rn(u[q], wv), ug = __fmul_rn(u[q], gv);
-                S0[q] = __fadd_rn(S0[q], uw);
-#pragma unroll
-                for (int r = 0; r < 3; ++r) {
-                    S1[q][r] = __fmaf_rn(uw, x[r], S1[q][r]);
-                    T1[q][r] = __fmaf_rn(ug, x[r], T1[q][r]);
+                for (int q = 0; q < 3; ++q) {
+                    s1[q] = __fmaf_rn(wv, x[q], s1[q]);
+                    t0[q] = __fmaf_rn(gv, x[q], t0[q]);
                 }
+                float g2[6];
 #pragma unroll
-                for (int r = 0; r < 6; ++r) T2[q][r] = __fmaf_rn(ug, m2[r], T2[q][r]);
+                for (int q = 0; q < 6; ++q) {
+                    s2[q] = __fmaf_rn(wv, m2[q], s2[q]);
+                    g2[q] = __fmul_rn(gv, m2[q]);
+                    t1[q] = __fadd_rn(t1[q], g2[q]);
+                }
+                t2[0] = __fmaf_rn(g2[0], x[0], t2[0]); t2[1] = __fmaf_rn(g2[0], x[1], t2[1]); t2[2] = __fmaf_rn(g2[0], x[2], t2[2]);
+                t2[3] = __fmaf_rn(g2[1], x[1], t2[3]); t2[4] = __fmaf_rn(g2[1], x[2], t2[4]); t2[5] = __fmaf_rn(g2[2], x[2], t2[5]);
+                t2[6] = __fmaf_rn(g2[3], x[1], t2[6]); t2[7] = __fmaf_rn(g2[3], x[2], t2[7]); t2[8] = __fmaf_rn(g2[4], x[2], t2[8]);
+                t2[9] = __fmaf_rn(g2[5], x[2], t2[9]);
             }
-        }
-    });
-    float4 o0 = make_float4(0, 0, 0, 0), o1 = o0, o2 = o0, o3 = o0;
-    const double h = (double)hi, ih = valid ? 1.0 / h : 0.0;
-    const double k3 = (double)SIGMA_C4 * ih * ih * ih;
-    if (MOM) {
-        if (valid) {
-            // ---- a3: FP64 solve (dimensional quantities; k3 = sigma/h^3)
-            const double Vi = (double)a.posV[i].w;
-            const double m0 = k3 * ((double)s0 + Vi);
-            const double m1[3] = {k3 * h * s1[0], k3 * h * s1[1], k3 * h * s1[2]};
-            const double k3h2 = k3 * h * h;
-            const double mm[3][3] = {{k3h2 * s2[0], k3h2 * s2[1], k3h2 * s2[2]},
-                                     {k3h2 * s2[1], k3h2 * s2[3], k3h2 * s2[4]},
-                                     {k3h2 * s2[2], k3h2 * s2[4], k3h2 * s2[5]}};
-            const double dm0[3] = {k3 * ih * t0[0], k3 * ih * t0[1], k3 * ih * t0[2]};
-            // sum g x_a x_c (symmetric)
-            const double q1[3][3] = {{k3 * t1[0], k3 * t1[1], k3 * t1[2]}, {k3 * t1[1], k3 * t1[3], k3 * t1[4]}, {k3 * t1[2], k3 * t1[4], k3 * t1[5]}};
-            const double k3h = k3 * h;
-            double cc[10];
+            if (GV) {
+                const float4 vj = lds128(sa + CRK_CCAP * 16u);
+                const float u[3] = {__fsub_rn(vi.x, vj.x), __fsub_rn(vi.y, vj.y), __fsub_rn(vi.z, vj.z)};
 #pragma unroll
-            for (int q = 0; q < 10; ++q) cc[q] = k3h * t2[q];
-            // inverse of m2 (adjugate)
-            const double a00 = mm[1][1] * mm[2][2] - mm[1][2] * mm[1][2];
-            const double a01 = mm[0][2] * mm[1][2] - mm[0][1] * mm[2][2];
-            const double a02 = mm[0][1] * mm[1][2] - mm[0][2] * mm[1][1];
-            const double a11 = mm[0][0] * mm[2][2] - mm[0][2] * mm[0][2];
-            const double a12 = mm[0][1] * mm[0][2] - mm[0][0] * mm[1][2];
-            const double a22 = mm[0][0] * mm[1][1] - mm[0][1] * mm[0][1];
-            const double det = mm[0][0] * a00 + mm[0][1] * a01 + mm[0][2] * a02;
-            double A, B[3], dA[3], dB[3][3];   // dB[c][a] = d_c B^a
-            // S14: m2 counts as singular when det m2 <= 1e-4 (tr m2 / 3)^3 (neighbours span less than three dimensions)
-            const double tr3 = (mm[0][0] + mm[1][1] + mm[2][2]) * (1.0 / 3.0);
-            if (det > 1.0e-4 * tr3 * tr3 * tr3 && isfinite(det)) {
-                const double id = 1.0 / det;
-                const double inv[3][3] = {{a00 * id, a01 * id, a02 * id}, {a01 * id, a11 * id, a12 * id}, {a02 * id, a12 * id, a22 * id}};
+                for (int q = 0; q < 3; ++q) {
+                    const float uw = __fmul_rn(u[q], wv), ug = __fmul_rn(u[q], gv);
+                    S0[q] = __fadd_rn(S0[q], uw);
 #pragma unroll
-                for (int p = 0; p < 3; ++p) B[p] = -(inv[p][0] * m1[0] + inv[p][1] * m1[1] + inv[p][2] * m1[2]);
-                A = 1.0 / (m0 + B[0] * m1[0] + B[1] * m1[1] + B[2] * m1[2]);
-                // index of the symmetric cubic monomial x_a x_b x_c in cc[]
-                const int cub[3][3][3] = {{{0, 1, 2}, {1, 3, 4}, {2, 4, 5}}, {{1, 3, 4}, {3, 6, 7}, {4, 7, 8}}, {{2, 4, 5}, {4, 7, 8}, {5, 8, 9}}};
-#pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    double Bdm1 = 0.0, BdmB = 0.0, rhs[3];
-#pragma unroll
-                    for (int p = 0; p < 3; ++p) {
-                        const double dm1_pc = q1[p][c] + (p == c ? m0 : 0.0);
-                        Bdm1 += B[p] * dm1_pc;
-                        double t = 0.0;
-#pragma unroll
-                        for (int q = 0; q < 3; ++q) {
-                            const double dm2_pqc = cc[cub[p][q][c]] + (p == c ? m1[q] : 0.0) + (q == c ? m1[p] : 0.0);
-                            t += dm2_pqc * B[q];
-                        }
-                        BdmB += B[p] * t;
-                        rhs[p] = dm1_pc + t;
+                    for (int r = 0; r < 3; ++r) {
+                        S1[q][r] = __fmaf_rn(uw, x[r], S1[q][r]);
+                        T1[q][r] = __fmaf_rn(ug, x[r], T1[q][r]);
                     }
-                    dA[c] = -A * A * (dm0[c] + 2.0 * Bdm1 + BdmB);
 #pragma unroll
-                    for (int p = 0; p < 3; ++p) dB[c][p] = -(inv[p][0] * rhs[0] + inv[p][1] * rhs[1] + inv[p][2] * rhs[2]);
-                }
-            } else {   // S14: degenerate neighbourhood -> zeroth-order correction only
-                A = 1.0 / m0;
-#pragma unroll
-                for (int c = 0; c < 3; ++c) {
-                    B[c] = 0.0;
-                    dA[c] = -A * A * dm0[c];
-                    dB[c][0] = dB[c][1] = dB[c][2] = 0.0;
+                    for (int r = 0; r < 6; ++r) T2[q][r] = __fmaf_rn(ug, m2[r], T2[q][r]);
                 }
             }
-            // pre-combined form used by the later sweeps:  (grad WR_ij)_c = W (cvec_c + M_ca x_a) + A s D x_c, s = 1 + B.x
-            //   cvec_c = d_c A + A B_c,   M_ca = d_c A B_a + A d_c B_a
-            o0 = make_float4((float)A, (float)B[0], (float)B[1], (float)B[2]);
-            float Mf[9];
+        });
+        float4 o0 = make_float4(0, 0, 0, 0), o1 = o0, o2 = o0, o3 = o0;
+        const double h = (double)hi, ih = valid ? 1.0 / h : 0.0;
+        const double k3 = (double)SIGMA_C4 * ih * ih * ih;
+        if (MOM) {
+            if (valid) {
+                // ---- a3: FP64 solve (dimensional quantities; k3 = sigma/h^3)
+                const double Vi = (double)a.posV[i].w;
+                const double m0 = k3 * ((double)s0 + Vi);
+                const double m1[3] = {k3 * h * s1[0], k3 * h * s1[1], k3 * h * s1[2]};
+                const double k3h2 = k3 * h * h;
+                const double mm[3][3] = {{k3h2 * s2[0], k3h2 * s2[1], k3h2 * s2[2]},
+                                         {k3h2 * s2[1], k3h2 * s2[3], k3h2 * s2[4]},
+                                         {k3h2 * s2[2], k3h2 * s2[4], k3h2 * s2[5]}};
+                const double dm0[3] = {k3 * ih * t0[0], k3 * ih * t0[1], k3 * ih * t0[2]};
+                // sum g x_a x_c (symmetric)
+                const double q1[3][3] = {{k3 * t1[0], k3 * t1[1], k3 * t1[2]}, {k3 * t1[1], k3 * t1[3], k3 * t1[4]}, {k3 * t1[2], k3 * t1[4], k3 * t1[5]}};
+                const double k3h = k3 * h;
+                double cc[10];
 #pragma unroll
-            for (int c = 0; c < 3; ++c)
+                for (int q = 0; q < 10; ++q) cc[q] = k3h * t2[q];
+                // inverse of m2 (adjugate)
+                const double a00 = mm[1][1] * mm[2][2] - mm[1][2] * mm[1][2];
+                const double a01 = mm[0][2] * mm[1][2] - mm[0][1] * mm[2][2];
+                const double a02 = mm[0][1] * mm[1][2] - mm[0][2] * mm[1][1];
+                const double a11 = mm[0][0] * mm[2][2] - mm[0][2] * mm[0][2];
+                const double a12 = mm[0][1] * mm[0][2] - mm[0][0] * mm[1][2];
+                const double a22 = mm[0][0] * mm[1][1] - mm[0][1] * mm[0][1];
+                const double det = mm[0][0] * a00 + mm[0][1] * a01 + mm[0][2] * a02;
+                double A, B[3], dA[3], dB[3][3];   // dB[c][a] = d_c B^a
+                // S14: m2 counts as singular when det m2 <= 1e-4 (tr m2 / 3)^3 (neighbours span less than three dimensions)
+                const double tr3 = (mm[0][0] + mm[1][1] + mm[2][2]) * (1.0 / 3.0);
+                if (det > 1.0e-4 * tr3 * tr3 * tr3 && isfinite(det)) {
+                    const double id = 1.0 / det;
+                    const double inv[3][3] = {{a00 * id, a01 * id, a02 * id}, {a01 * id, a11 * id, a12 * id}, {a02 * id, a12 * id, a22 * id}};
 #pragma unroll
-                for (int p = 0; p < 3; ++p) Mf[3 * c + p] = (float)(dA[c] * B[p] + A * dB[c][p]);
-            o1 = make_float4((float)(dA[0] + A * B[0]), (float)(dA[1] + A * B[1]), (float)(dA[2] + A * B[2]), Mf[0]);
-            o2 = make_float4(Mf[1], Mf[2], Mf[3], Mf[4]);
-            o3 = make_float4(Mf[5], Mf[6], Mf[7], Mf[8]);
-            const int32_t p = a.perm[i];
-            const int64_t n = a.n;
-            if (a.o0) a.o0[p] = (float)A;
-            if (a.o1) { a.o1[p] = (float)B[0]; a.o1[n + p] = (float)B[1]; a.o1[2 * n + p] = (float)B[2]; }
-            if (a.o2) { a.o2[p] = (float)dA[0]; a.o2[n + p] = (float)dA[1]; a.o2[2 * n + p] = (float)dA[2]; }
-            if (a.o3) {
+                    for (int p = 0; p < 3; ++p) B[p] = -(inv[p][0] * m1[0] + inv[p][1] * m1[1] + inv[p][2] * m1[2]);
+                    A = 1.0 / (m0 + B[0] * m1[0] + B[1] * m1[1] + B[2] * m1[2]);
+                    // index of the symmetric cubic monomial x_a x_b x_c in cc[]
+                    const int cub[3][3][3] = {{{0, 1, 2}, {1, 3, 4}, {2, 4, 5}}, {{1, 3, 4}, {3, 6, 7}, {4, 7, 8}}, {{2, 4, 5}, {4, 7, 8}, {5, 8, 9}}};
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        double Bdm1 = 0.0, BdmB = 0.0, rhs[3];
+#pragma unroll
+                        for (int p = 0; p < 3; ++p) {
+                            const double dm1_pc = q1[p][c] + (p == c ? m0 : 0.0);
+                            Bdm1 += B[p] * dm1_pc;
+                            double t = 0.0;
+#pragma unroll
+                            for (int q = 0; q < 3; ++q) {
+                                const double dm2_pqc = cc[cub[p][q][c]] + (p == c ? m1[q] : 0.0) + (q == c ? m1[p] : 0.0);
+                                t += dm2_pqc * B[q];
+                            }
+                            BdmB += B[p] * t;
+                            rhs[p] = dm1_pc + t;
+                        }
+                        dA[c] = -A * A * (dm0[c] + 2.0 * Bdm1 + BdmB);
+#pragma unroll
+                        for (int p = 0; p < 3; ++p) dB[c][p] = -(inv[p][0] * rhs[0] + inv[p][1] * rhs[1] + inv[p][2] * rhs[2]);
+                    }
+                } else {   // S14: degenerate neighbourhood -> zeroth-order correction only
+                    A = 1.0 / m0;
+#pragma unroll
+                    for (int c = 0; c < 3; ++c) {
+                        B[c] = 0.0;
+                        dA[c] = -A * A * dm0[c];
+                        dB[c][0] = dB[c][1] = dB[c][2] = 0.0;
+                    }
+                }
+                // pre-combined form used by the later sweeps:  (grad WR_ij)_c = W (cvec_c + M_ca x_a) + A s D x_c, s = 1 + B.x
+                //   cvec_c = d_c A + A B_c,   M_ca = d_c A B_a + A d_c B_a
+                o0 = make_float4((float)A, (float)B[0], (float)B[1], (float)B[2]);
+                float Mf[9];
 #pragma unroll
                 for (int c = 0; c < 3; ++c)
 #pragma unroll
-                    for (int q = 0; q < 3; ++q) a.o3[(3 * c + q) * n + p] = (float)dB[c][q];
+                    for (int p = 0; p < 3; ++p) Mf[3 * c + p] = (float)(dA[c] * B[p] + A * dB[c][p]);
+                o1 = make_float4((float)(dA[0] + A * B[0]), (float)(dA[1] + A * B[1]), (float)(dA[2] + A * B[2]), Mf[0]);
+                o2 = make_float4(Mf[1], Mf[2], Mf[3], Mf[4]);
+                o3 = make_float4(Mf[5], Mf[6], Mf[7], Mf[8]);
+                const int32_t p = a.perm[i];
+                const int64_t n = a.n;
+                if (a.o0) a.o0[p] = (float)A;
+                if (a.o1) { a.o1[p] = (float)B[0]; a.o1[n + p] = (float)B[1]; a.o1[2 * n + p] = (float)B[2]; }
+                if (a.o2) { a.o2[p] = (float)dA[0]; a.o2[n + p] = (float)dA[1]; a.o2[2 * n + p] = (float)dA[2]; }
+                if (a.o3) {
+#pragma unroll
+                    for (int c = 0; c < 3; ++c)
+#pragma unroll
+                        for (int q = 0; q < 3; ++q) a.o3[(3 * c + q) * n + p] = (float)dB[c][q];
+                }
             }
+            a.coef[i] = o0;
+            a.coef[a.np + i] = o1;
+            a.coef[2 * a.np + i] = o2;
+            a.coef[3 * a.np + i] = o3;
+        } else {
+            o0 = a.coef[i]; o1 = a.coef[a.np + i]; o2 = a.coef[2 * a.np + i]; o3 = a.coef[3 * a.np + i];
         }
-        a.coef[i] = o0;
-        a.coef[a.np + i] = o1;
-        a.coef[2 * a.np + i] = o2;
-        a.coef[3 * a.np + i] = o3;
-    } else {
-        o0 = a.coef[i]; o1 = a.coef[a.np + i]; o2 = a.coef[2 * a.np + i]; o3 = a.coef[3 * a.np + i];
-    }
-    if (!GV) return;
-    // ---- a4: contraction of the velocity sums with the stored FP32 coefficients (FP64 arithmetic)
-    float g[9];
-    {
-        const Coef k = load_coef(o0, o1, o2, o3);
-        const double cv[3] = {(double)k.cx, (double)k.cy, (double)k.cz};
-        const double Bv[3] = {(double)k.Bx, (double)k.By, (double)k.Bz};
-        const double A = (double)k.A;
-        const double k3h = k3 * h, k3ih = k3 * ih;
-        const int sym[3][3] = {{0, 1, 2}, {1, 3, 4}, {2, 4, 5}};
+        if (!GV) {
+            leaf = next;
+            continue;
+        }
+        // ---- a4: contraction of the velocity sums with the stored FP32 coefficients (FP64 arithmetic)
+        float g[9];
+        {
+            const Coef k = load_coef(o0, o1, o2, o3);
+            const double cv[3] = {(double)k.cx, (double)k.cy, (double)k.cz};
+            const double Bv[3] = {(double)k.Bx, (double)k.By, (double)k.Bz};
+            const double A = (double)k.A;
+            const double k3h = k3 * h, k3ih = k3 * ih;
+            const int sym[3][3] = {{0, 1, 2}, {1, 3, 4}, {2, 4, 5}};
 #pragma unroll
-        for (int al = 0; al < 3; ++al)
+            for (int al = 0; al < 3; ++al)
 #pragma unroll
-            for (int be = 0; be < 3; ++be) {
-                double t = cv[be] * (k3 * (double)S0[al]) + A * (k3ih * (double)T1[al][be]);
+                for (int be = 0; be < 3; ++be) {
+                    double t = cv[be] * (k3 * (double)S0[al]) + A * (k3ih * (double)T1[al][be]);
 #pragma unroll
-                for (int c = 0; c < 3; ++c)
-                    t += (double)k.M[3 * be + c] * (k3h * (double)S1[al][c]) + A * Bv[c] * (k3 * (double)T2[al][sym[c][be]]);
-                g[3 * al + be] = (float)(-t);
-            }
-    }
-    // force-sweep state planes: (x,y,z,1/h) (v,V) | (P,rho,cs,k3) (A,B) (c,M0) (M1..M4) (M5..M8) (gxx,gyy,gzz,k5)
-    // (gxy+gyx, gxz+gzx, gyz+gzy, n_h/h).  Only x.(grad v x) enters Eqs. 27-30 and Eq. 25 (uhat_ij.x_ij), so the
-    // symmetric part of grad v is all the force sweep needs; k3 = sigma/h^3, k5 = sigma/h^5.
-    const float ihf = valid ? 1.0f / hi : 0.0f;
-    const float k3f = SIGMA_C4 * ihf * ihf * ihf;
-    const float k5f = k3f * ihf * ihf;
-    const float u = u_s[i], rho = a.rho_s[i], gm = a.gamma;
-    const float P = (gm - 1.0f) * rho * u;
-    const float cs = sqrtf(gm * (gm - 1.0f) * fmaxf(u, 0.0f));
-    float4* f = a.fst + i;
-    const int64_t np = a.np;
-    f[2 * np] = make_float4(P, rho, cs, k3f);
-    f[3 * np] = o0;
-    f[4 * np] = o1;
-    f[5 * np] = o2;
-    f[6 * np] = o3;
-    f[7 * np] = make_float4(g[0], g[4], g[8], k5f);
-    f[8 * np] = make_float4(g[1] + g[3], g[2] + g[6], g[5] + g[7], a.n_h * ihf);
-    if (gv_full && valid) {                              // diagnostics (crk_get_gradv): all nine components, caller order
-        const int32_t p = a.perm[i];
+                    for (int c = 0; c < 3; ++c)
+                        t += (double)k.M[3 * be + c] * (k3h * (double)S1[al][c]) + A * Bv[c] * (k3 * (double)T2[al][sym[c][be]]);
+                    g[3 * al + be] = (float)(-t);
+                }
+        }
+        // force-sweep state planes: (x,y,z,1/h) (v,V) | (P,rho,cs,k3) (A,B) (c,M0) (M1..M4) (M5..M8) (gxx,gyy,gzz,k5)
+        // (gxy+gyx, gxz+gzx, gyz+gzy, n_h/h).  Only x.(grad v x) enters Eqs. 27-30 and Eq. 25 (uhat_ij.x_ij), so the
+        // symmetric part of grad v is all the force sweep needs; k3 = sigma/h^3, k5 = sigma/h^5.
+        const float ihf = valid ? 1.0f / hi : 0.0f;
+        const float k3f = SIGMA_C4 * ihf * ihf * ihf;
+        const float k5f = k3f * ihf * ihf;
+        const float u = u_s[i], rho = a.rho_s[i], gm = a.gamma;
+        const float P = (gm - 1.0f) * rho * u;
+        const float cs = sqrtf(gm * (gm - 1.0f) * fmaxf(u, 0.0f));
+        float4* f = a.fst + i;
+        const int64_t np = a.np;
+        f[2 * np] = make_float4(P, rho, cs, k3f);
+        f[3 * np] = o0;
+        f[4 * np] = o1;
+        f[5 * np] = o2;
+        f[6 * np] = o3;
+        f[7 * np] = make_float4(g[0], g[4], g[8], k5f);
+        f[8 * np] = make_float4(g[1] + g[3], g[2] + g[6], g[5] + g[7], a.n_h * ihf);
+        if (gv_full && valid) {                              // diagnostics (crk_get_gradv): all nine components, caller order
+            const int32_t p = a.perm[i];
 #pragma unroll
-        for (int q = 0; q < 9; ++q) gv_full[q * a.n + p] = g[q];
+            for (int q = 0; q < 9; ++q) gv_full[q * a.n + p] = g[q];
+        }
+        leaf = next;
     }
 }
 
@@ -747,49 +829,55 @@ template <bool TS>   // TS: also reduce the per-particle maxima the time-step cr
 __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
-    const int64_t leaf = a.ids ? (int64_t)a.ids[blockIdx.x] : (int64_t)blockIdx.x;
     float4* tile = (float4*)smem_raw;
-    const int64_t i = leaf * CRK_LEAF + lane;
-    const bool valid = i < a.n;
-    PState I;                                            // taken from the tile (slots 0..31 = the leaf's own particles)
+    Meta* meta = (Meta*)(tile + FPL * CRK_CCAP);
     const ForceConst fc = {a.L, a.half, 1.0f / a.n_h, a.n_h / 0.2f, a.eps2, a.C_l, a.C_q};
-    float acc[4] = {0.f, 0.f, 0.f, 0.f};                 // Fx, Fy, Fz, dE
-    float mx[2] = {0.f, 0.f};                            // max approach speed, max Q_i
     const float4* planes[FPL];
 #pragma unroll
     for (int p = 0; p < FPL; ++p) planes[p] = a.fst + (int64_t)p * a.np;
-    const uint32_t count = leaf_sweep<W5_WPL, FPL, true, FPRE>(a, planes, leaf, 0, wl, lane, tile, [&](uint32_t sa, bool wrapped, const float4* pre) {
-        const PState J = load_pstate_shared(sa, pre);
-        const PairF f = force_pair(fc, I, J, wrapped);
-        acc[0] += f.Fx; acc[1] += f.Fy; acc[2] += f.Fz; acc[3] += f.e;
-        if (TS) {
-            mx[0] = fmaxf(mx[0], f.app);
-            mx[1] = fmaxf(mx[1], f.Qi);
-        }
-    }, [&](uint32_t ts) {
-        float4 pre[FPRE];
+    long long leaf = sweep_begin<W5_WPL>(a, meta, 0, wl, lane);
+    while (leaf >= 0) {
+        const int64_t i = leaf * CRK_LEAF + lane;
+        const bool valid = i < a.n;
+        PState I;                                            // taken from the tile (slots 0..31 = the leaf's own particles)
+        float acc[4] = {0.f, 0.f, 0.f, 0.f};                 // Fx, Fy, Fz, dE
+        float mx[2] = {0.f, 0.f};                            // max approach speed, max Q_i
+        long long next;
+        const uint32_t count = leaf_sweep<W5_WPL, FPL, true, FPRE>(a, planes, leaf, next, 0, wl, lane, tile, meta, [&](uint32_t sa, bool wrapped, const float4* pre) {
+            const PState J = load_pstate_shared(sa, pre);
+            const PairF f = force_pair(fc, I, J, wrapped);
+            acc[0] += f.Fx; acc[1] += f.Fy; acc[2] += f.Fz; acc[3] += f.e;
+            if (TS) {
+                mx[0] = fmaxf(mx[0], f.app);
+                mx[1] = fmaxf(mx[1], f.Qi);
+            }
+        }, [&](uint32_t ts) {
+            float4 pre[FPRE];
 #pragma unroll
-        for (int p = 0; p < FPRE; ++p) pre[p] = lds128(ts + (uint32_t)(p * CRK_CCAP + lane) * 16u);
-        I = load_pstate_shared(ts + (uint32_t)lane * 16u, pre);
-    });
-    group_reduce<W5_WPL, 4>(acc, 0, wl, lane, (float*)tile);
-    if (TS) group_reduce<W5_WPL, 2, true>(mx, 0, wl, lane, (float*)tile);
-    if (wl != 0) return;
-    if (TS) a.ts[i] = make_float2(mx[0], mx[1]);
-    float4 as = make_float4(0.f, 0.f, 0.f, 0.f);
-    if (valid) {
-        const float im = 1.0f / a.m_s[i];
-        const int32_t p = a.perm[i];
-        as = make_float4(acc[0] * im, acc[1] * im, acc[2] * im, I.P * __powf(I.rho, -a.gamma));
-        if (!a.active || a.active[p]) {
-            a.o0[p] = as.x;
-            a.o1[p] = as.y;
-            a.o2[p] = as.z;
-            a.o3[p] = acc[3] * im;
-            if (a.ocnt) a.ocnt[p] = count;
+            for (int p = 0; p < FPRE; ++p) pre[p] = lds128(ts + (uint32_t)(p * CRK_CCAP + lane) * 16u);
+            I = load_pstate_shared(ts + (uint32_t)lane * 16u, pre);
+        });
+        group_reduce<W5_WPL, 4>(acc, 0, wl, lane, (float*)tile);
+        if (TS) group_reduce<W5_WPL, 2, true>(mx, 0, wl, lane, (float*)tile);
+        if (wl == 0) {
+            if (TS) a.ts[i] = make_float2(mx[0], mx[1]);
+            float4 as = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (valid) {
+                const float im = 1.0f / a.m_s[i];
+                const int32_t p = a.perm[i];
+                as = make_float4(acc[0] * im, acc[1] * im, acc[2] * im, I.P * __powf(I.rho, -a.gamma));
+                if (!a.active || a.active[p]) {
+                    a.o0[p] = as.x;
+                    a.o1[p] = as.y;
+                    a.o2[p] = as.z;
+                    a.o3[p] = acc[3] * im;
+                    if (a.ocnt) a.ocnt[p] = count;
+                }
+            }
+            a.fst[(int64_t)FPL * a.np + i] = as;             // plane 9: (dv/dt, s = P / rho^gamma) for crk_compatible_energy
         }
+        leaf = next;
     }
-    a.fst[(int64_t)FPL * a.np + i] = as;                 // plane 9: (dv/dt, s = P / rho^gamma) for crk_compatible_energy
 }
 
 // ================================================================================ NEXT row 1: compatible energy update
@@ -816,40 +904,45 @@ __global__ void __launch_bounds__(256) k_compat_prep(const float4* __restrict__ 
     kick[k] = w;
 }
 
-__global__ void __launch_bounds__(W5_WPL * 32, 4) k_compat(SweepArgs a, float dt, const float4* __restrict__ kick) {
+__global__ void __launch_bounds__(W5_WPL * 32, 3) k_compat(SweepArgs a, float dt, const float4* __restrict__ kick) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
-    const int64_t leaf = blockIdx.x;
     float4* tile = (float4*)smem_raw;
-    const int64_t i = leaf * CRK_LEAF + lane;
-    const bool valid = i < a.n;
-    const PState I = load_pstate(a.fst + i, a.np);
-    const float4 qi = kick[i];
+    Meta* meta = (Meta*)(tile + CPL * CRK_CCAP);
     const ForceConst fc = {a.L, a.half, 1.0f / a.n_h, a.n_h / 0.2f, a.eps2, a.C_l, a.C_q};
-    float acc[1] = {0.f};
     const float4* planes[CPL];
 #pragma unroll
     for (int p = 0; p < FPL; ++p) planes[p] = a.fst + (int64_t)p * a.np;
     planes[FPL] = kick;
-    leaf_sweep<W5_WPL, CPL, true, FPRE>(a, planes, leaf, 0, wl, lane, tile, [&](uint32_t sa, bool wrapped, const float4* pre) {
-        const PState J = load_pstate_shared(sa, pre);
-        const float4 qj = lds128(sa + (uint32_t)FPL * CRK_CCAP * 16u);
-        const PairF f = force_pair(fc, I, J, wrapped);
-        // (v_j + v'_j - v_i - v'_i) = 2 (v_j - v_i) + (kick_j - kick_i)
-        const float wx = __fmaf_rn(2.0f, f.vjix, __fsub_rn(qj.x, qi.x));
-        const float wy = __fmaf_rn(2.0f, f.vjiy, __fsub_rn(qj.y, qi.y));
-        const float wz = __fmaf_rn(2.0f, f.vjiz, __fsub_rn(qj.z, qi.z));
-        const float w = __fmaf_rn(f.Fz, wz, __fmaf_rn(f.Fy, wy, __fmul_rn(f.Fx, wx)));       // = 2 dE_ij
-        const float si = qi.w, sj = qj.w;
-        float part = 0.5f;
-        if (si > 0.0f && sj > 0.0f) {
-            const bool small = (w >= 0.0f) ? (si >= sj) : (si < sj);
-            part = (small ? fminf(si, sj) : fmaxf(si, sj)) * rcp_fast(__fadd_rn(si, sj));
-        }
-        acc[0] = fmaf(0.5f * part, w, acc[0]);
-    });
-    group_reduce<W5_WPL, 1>(acc, 0, wl, lane, (float*)tile);
-    if (wl == 0 && valid) a.o0[a.perm[i]] = acc[0] * dt / a.m_s[i];
+    long long leaf = sweep_begin<W5_WPL>(a, meta, 0, wl, lane);
+    while (leaf >= 0) {
+        const int64_t i = leaf * CRK_LEAF + lane;
+        const bool valid = i < a.n;
+        const PState I = load_pstate(a.fst + i, a.np);
+        const float4 qi = kick[i];
+        float acc[1] = {0.f};
+        long long next;
+        leaf_sweep<W5_WPL, CPL, true, FPRE>(a, planes, leaf, next, 0, wl, lane, tile, meta, [&](uint32_t sa, bool wrapped, const float4* pre) {
+            const PState J = load_pstate_shared(sa, pre);
+            const float4 qj = lds128(sa + (uint32_t)FPL * CRK_CCAP * 16u);
+            const PairF f = force_pair(fc, I, J, wrapped);
+            // (v_j + v'_j - v_i - v'_i) = 2 (v_j - v_i) + (kick_j - kick_i)
+            const float wx = __fmaf_rn(2.0f, f.vjix, __fsub_rn(qj.x, qi.x));
+            const float wy = __fmaf_rn(2.0f, f.vjiy, __fsub_rn(qj.y, qi.y));
+            const float wz = __fmaf_rn(2.0f, f.vjiz, __fsub_rn(qj.z, qi.z));
+            const float w = __fmaf_rn(f.Fz, wz, __fmaf_rn(f.Fy, wy, __fmul_rn(f.Fx, wx)));       // = 2 dE_ij
+            const float si = qi.w, sj = qj.w;
+            float part = 0.5f;
+            if (si > 0.0f && sj > 0.0f) {
+                const bool small = (w >= 0.0f) ? (si >= sj) : (si < sj);
+                part = (small ? fminf(si, sj) : fmaxf(si, sj)) * rcp_fast(__fadd_rn(si, sj));
+            }
+            acc[0] = fmaf(0.5f * part, w, acc[0]);
+        });
+        group_reduce<W5_WPL, 1>(acc, 0, wl, lane, (float*)tile);
+        if (wl == 0 && valid) a.o0[a.perm[i]] = acc[0] * dt / a.m_s[i];
+        leaf = next;
+    }
 }
 
 __global__ void __launch_bounds__(256) k_gather_f32(const float* __restrict__ in, const int32_t* __restrict__ perm,
@@ -872,12 +965,28 @@ SweepArgs make_args(crk_ctx* c) {
     a.gamma = c->prm.gamma; a.n_h = c->prm.n_h; a.C_l = c->prm.C_l; a.C_q = c->prm.C_q;
     a.eps2 = c->prm.eps * c->prm.eps;
     a.flag = (int*)c->flag.p;
+    a.sched = (unsigned int*)c->sched.p;
     return a;
 }
 
+// Launch geometry of a persistent sweep: as many CTAs as are resident at once (occupancy x SMs), never more than there are
+// work items; the work counter is zeroed on the stream first.  groups_per_cta = leaves a CTA serves concurrently.
 template <typename K>
-int set_smem(crk_ctx* c, K kernel, int bytes) {
-    if (bytes > 48 * 1024) CRK_CUDA(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+int persistent_grid(crk_ctx* c, K kernel, int threads, int smem, int groups_per_cta, int64_t items, unsigned* grid) {
+    if (smem > 48 * 1024) CRK_CUDA(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    int per_sm = 0, dev = 0, sms = 0;
+    CRK_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, (size_t)smem));
+    CRK_CUDA(c, cudaGetDevice(&dev));
+    CRK_CUDA(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if (per_sm < 1) {
+        snprintf(c->err, sizeof(c->err), "a sweep kernel does not fit on an SM (%d bytes of shared memory)", smem);
+        return CRK_ECUDA;
+    }
+    const int64_t need = (items + groups_per_cta - 1) / groups_per_cta;
+    const int64_t res = (int64_t)per_sm * sms;
+    *grid = (unsigned)(need < res ? need : res);
+    CRK_TRY(crk_ensure(c, c->sched, 64));
+    CRK_CUDA(c, cudaMemsetAsync(c->sched.p, 0, sizeof(unsigned int), c->stream));
     return CRK_OK;
 }
 
@@ -892,9 +1001,11 @@ int crk_launch_volumes(crk_ctx* c, const float* m, float* V, float* rho, uint32_
     CRK_TRY(crk_check_launch(c, "k_gather_f32"));
     SweepArgs a = make_args(c);
     a.o0 = V; a.o1 = rho; a.ocnt = nbr_count;
-    const int smem = W1_WPC * CRK_CCAP * (int)sizeof(float4);
-    CRK_TRY(set_smem(c, k_volumes, smem));
-    k_volumes<<<(unsigned)((c->nl + W1_WPC - 1) / W1_WPC), W1_WPC * 32, smem, c->stream>>>(a);
+    const int smem = W1_WPC * W1_SMEM;
+    unsigned grid = 0;
+    CRK_TRY(persistent_grid(c, k_volumes, W1_WPC * 32, smem, W1_WPC, c->nl, &grid));
+    a.sched = (unsigned int*)c->sched.p;
+    k_volumes<<<grid, W1_WPC * 32, smem, c->stream>>>(a);
     return crk_check_launch(c, "k_volumes");
 }
 
@@ -921,18 +1032,22 @@ int crk_launch_rk(crk_ctx* c, bool mom, bool gv, float* A, float* B, float* grad
     a.o0 = A; a.o1 = B; a.o2 = gradA; a.o3 = gradB;
     a.velV = gv ? (float4*)c->fst.p + np : nullptr;
     a.ids = ids; a.n_ids = n_ids;
-    const unsigned grid = (unsigned)(((ids ? n_ids : c->nl) + W2_WPC - 1) / W2_WPC);
-    if (grid == 0) return CRK_OK;
-    const int smem = W2_WPC * (gv ? 2 : 1) * CRK_CCAP * (int)sizeof(float4);
+    const int64_t items = ids ? n_ids : c->nl;
+    if (items == 0) return CRK_OK;
+    const int smem = W2_WPC * ((gv ? 2 : 1) * CRK_CCAP * (int)sizeof(float4) + (int)sizeof(Meta));
     const float* us = (const float*)c->u_s.p;
+    unsigned grid = 0;
     if (mom && gv) {
-        CRK_TRY(set_smem(c, k_rk<true, true>, smem));
+        CRK_TRY(persistent_grid(c, k_rk<true, true>, W2_WPC * 32, smem, W2_WPC, items, &grid));
+        a.sched = (unsigned int*)c->sched.p;
         k_rk<true, true><<<grid, W2_WPC * 32, smem, c->stream>>>(a, us, gradv_full);
     } else if (mom) {
-        CRK_TRY(set_smem(c, k_rk<true, false>, smem));
+        CRK_TRY(persistent_grid(c, k_rk<true, false>, W2_WPC * 32, smem, W2_WPC, items, &grid));
+        a.sched = (unsigned int*)c->sched.p;
         k_rk<true, false><<<grid, W2_WPC * 32, smem, c->stream>>>(a, nullptr, nullptr);
     } else {
-        CRK_TRY(set_smem(c, k_rk<false, true>, smem));
+        CRK_TRY(persistent_grid(c, k_rk<false, true>, W2_WPC * 32, smem, W2_WPC, items, &grid));
+        a.sched = (unsigned int*)c->sched.p;
         k_rk<false, true><<<grid, W2_WPC * 32, smem, c->stream>>>(a, us, gradv_full);
     }
     return crk_check_launch(c, "k_rk");
@@ -944,18 +1059,21 @@ int crk_launch_forces(crk_ctx* c, float* ax, float* ay, float* az, float* dudt, 
     const int64_t np = c->nl * CRK_LEAF;
     SweepArgs a = make_args(c);
     a.ids = ids; a.n_ids = n_ids; a.active = active;
-    const unsigned grid = (unsigned)(ids ? n_ids : c->nl);
-    if (grid == 0) return CRK_OK;
+    const int64_t items = ids ? n_ids : c->nl;
+    if (items == 0) return CRK_OK;
     a.velV = (float4*)c->fst.p + np;
     a.o0 = ax; a.o1 = ay; a.o2 = az; a.o3 = dudt; a.ocnt = pair_count;
-    const int smem = FPL * CRK_CCAP * (int)sizeof(float4);
+    const int smem = FPL * CRK_CCAP * (int)sizeof(float4) + (int)sizeof(Meta);
+    unsigned grid = 0;
     if (c->prm.flags & CRK_FLAG_TIMESTEP) {
         CRK_TRY(crk_ensure(c, c->ts_s, (size_t)np * sizeof(float2)));
         a.ts = (float2*)c->ts_s.p;
-        CRK_TRY(set_smem(c, k_forces<true>, smem));
+        CRK_TRY(persistent_grid(c, k_forces<true>, W5_WPL * 32, smem, 1, items, &grid));
+        a.sched = (unsigned int*)c->sched.p;
         k_forces<true><<<grid, W5_WPL * 32, smem, c->stream>>>(a);
     } else {
-        CRK_TRY(set_smem(c, k_forces<false>, smem));
+        CRK_TRY(persistent_grid(c, k_forces<false>, W5_WPL * 32, smem, 1, items, &grid));
+        a.sched = (unsigned int*)c->sched.p;
         k_forces<false><<<grid, W5_WPL * 32, smem, c->stream>>>(a);
     }
     return crk_check_launch(c, "k_forces");
@@ -1020,9 +1138,11 @@ int crk_launch_compat(crk_ctx* c, float dt, float c1, float c0, const float* bx,
                                                                        np, c1, c0, bx, by, bz, (float4*)c->kick.p);
     CRK_TRY(crk_check_launch(c, "k_compat_prep"));
     a.o0 = delta_u;
-    const int smem = CPL * CRK_CCAP * (int)sizeof(float4);
-    CRK_TRY(set_smem(c, k_compat, smem));
-    k_compat<<<(unsigned)c->nl, W5_WPL * 32, smem, c->stream>>>(a, dt, (const float4*)c->kick.p);
+    const int smem = CPL * CRK_CCAP * (int)sizeof(float4) + (int)sizeof(Meta);
+    unsigned grid = 0;
+    CRK_TRY(persistent_grid(c, k_compat, W5_WPL * 32, smem, 1, c->nl, &grid));
+    a.sched = (unsigned int*)c->sched.p;
+    k_compat<<<grid, W5_WPL * 32, smem, c->stream>>>(a, dt, (const float4*)c->kick.p);
     return crk_check_launch(c, "k_compat");
 }
 
