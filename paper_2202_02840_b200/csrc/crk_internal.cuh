@@ -113,7 +113,8 @@ struct crk_ctx {
     DevBuf posV;                   // float4 (x,y,z,V)
     DevBuf rho_s;                  // float
     DevBuf coef;                   // 4 planes float4[n]: (A,Bx,By,Bz) (cx,cy,cz,M00) (M01,M02,M10,M11) (M12,M20,M21,M22)
-    DevBuf fst;                    // force-sweep state, 9 planes float4[np] (layout at k_rk in pairs.cu) + plane 9 = (dv/dt, s)
+    DevBuf fst;                    // force-sweep state, one 128-byte row per particle (layout at k_rk in pairs.cu)
+    DevBuf facc;                   // float4 (dv/dt, s = P / rho^gamma) per particle, sorted, written by k_forces
     DevBuf ts_s;                   // float2 (max approach speed, max Q_i), sorted; only with CRK_FLAG_TIMESTEP
     DevBuf kick;                   // compatible-energy sweep: (v' - v, s) per particle, sorted
     DevBuf kdk;                    // crk_kdk_step scratch: derivatives [4][n] and half-step state [4][n]

@@ -29,8 +29,11 @@ constexpr float SIGMA_C4 = 4.923856051905513f;     // 495 / (32 pi), Eq. 12
 constexpr float C35_3 = 35.0f / 3.0f;
 constexpr float C56_3 = 56.0f / 3.0f;
 constexpr float R2_TINY = 1.0e-37f;
-constexpr int FPL = 9;                             // j-state planes of the force sweep
-constexpr int CPL = FPL + 1;                       // + (dv/dt, s = P / rho^gamma) for the compatible-energy sweep
+constexpr int FROW = 8;                            // float4 per force-sweep state row: one 128-byte line per particle
+constexpr int CPL = FROW + 1;                      // + the kick plane (v' - v, s = P / rho^gamma) of the compatible-energy sweep
+// shared-memory tile: plane-major, plane p of candidate slot c at p * PSTRIDE + c * 16 bytes.  The 16 bytes of padding per
+// plane put the FROW pieces of one candidate row (written by eight neighbouring lanes of one LDGSTS) into different banks.
+constexpr uint32_t PSTRIDE = CRK_CCAP * 16u + 16u;
 
 struct SweepArgs {
     int64_t n, nl;
@@ -42,9 +45,9 @@ struct SweepArgs {
     const int32_t* __restrict__ perm;     // sorted slot -> caller index
     const float4* __restrict__ posh;      // (x,y,z,h)
     float4* __restrict__ posV;            // (x,y,z,V)
-    float4* __restrict__ velV;            // (vx,vy,vz,V)
     float4* __restrict__ coef;            // 4 planes, stride np: (A,B) (c,M0) (M1..M4) (M5..M8)
-    float4* __restrict__ fst;             // FPL planes, stride np: force-sweep state (layout at k_forces)
+    float4* __restrict__ fst;             // force-sweep state, one row of FROW float4 per particle (layout at k_rk)
+    float4* __restrict__ facc;            // (dv/dt, s = P / rho^gamma) per particle, written by k_forces
     float* __restrict__ rho_s;
     const float* __restrict__ m_s;
     int64_t np;                           // padded particle count nl*32 (plane stride)
@@ -156,7 +159,10 @@ __device__ __forceinline__ long long sweep_begin(const SweepArgs& a, Meta* m, in
 // Rows [0, K) of a segment's entry block; lane l is active while k < cnt[l].  SYM = false (gather set, Eqs. 13-14): entries
 // flagged CRK_ELL_SYM are skipped;  SYM = true (Eqs. 17-18): every entry is a pair.
 // pair(slot_addr, crosses_boundary, plane0) evaluates one accepted pair (slot_addr = shared address of the candidate's
-// plane-0 entry; plane p sits CRK_CCAP * 16 * p bytes further); returns the number of pairs the lane owns.
+// plane-0 entry; plane p sits p * PSTRIDE bytes further); returns the number of pairs the lane owns.
+// The tile's planes 0 .. ROWP-1 are the first ROWP float4 of the candidates' force-state rows (`rows_src`, FROW float4 per
+// particle: consecutive lanes copy consecutive pieces of one row, so a warp-wide LDGSTS touches 32 / ROWP full lines or
+// sectors instead of 32 scattered ones), planes ROWP .. ROWP+PLANES-1 come from the SoA arrays `planes`.
 // On entry the copy of the leaf's metadata into m is in flight; on exit the group's next leaf is in `next_leaf` and the copy
 // of ITS metadata is in flight.  Barriers per segment: B1 metadata landed and the previous rows are done (tile free);
 // B2 everybody has read the metadata (m may be overwritten) and the next work item is known; B3 the state has landed.
@@ -168,9 +174,11 @@ struct NoInit {
 // (Measured and not kept, profiles/r02_notes.md: a second, branch-free instantiation of the row loop for segments without
 // boundary-crossing entries -- 172 instead of 190 instructions per pair of k_forces, but ptxas then sinks the shared loads
 // next to their uses and the sweep loses 1.6 ms to short-scoreboard stalls.)
-template <int WPL, int PLANES, bool SYM, int NPRE = 1, typename Pair, typename Init = NoInit>
-__device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4* const* planes, long long leaf, long long& next_leaf,
-                                               int lg, int wl, int lane, float4* tile, Meta* m, Pair pair, Init init = Init()) {
+template <int WPL, int ROWP, int PLANES, bool SYM, int NPRE = 1, typename Pair, typename Init = NoInit>
+__device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4* __restrict__ rows_src, const float4* const* planes,
+                                               long long leaf, long long& next_leaf, int lg, int wl, int lane, float4* tile, Meta* m,
+                                               Pair pair, Init init = Init()) {
+    static_assert(ROWP == 0 || ROWP == 2 || ROWP == 8, "row pieces per candidate");
     constexpr int NT = WPL * 32;                                  // threads that serve the leaf
     uint32_t count = 0;
     bool first = true;
@@ -210,18 +218,34 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
         const uint16_t* ep = s.ell + lane;
         CRK_CHECK(a.flag, s.C >= 0 && s.C <= CRK_CCAP && rows >= 0 && rows <= CRK_QCAP && mine <= rows, 8);   // segment header
         // stage: 16-byte asynchronous copies global -> shared (LDGSTS), no register round trip
-        for (int c0 = 0; c0 < s.C; c0 += NT * 2) {
-            const int ca = c0 + tg, cb = ca + NT;
-            const uint32_t ja = (ca < s.C) ? m->cand[ca] : 0u;
-            const uint32_t jb = (cb < s.C) ? m->cand[cb] : 0u;
-            CRK_CHECK(a.flag, (int64_t)ja < a.np && (int64_t)jb < a.np, 9);                 // candidate index
-            if (ca < s.C) {
-#pragma unroll
-                for (int p = 0; p < PLANES; ++p) cp_async16(tile_s + (uint32_t)(p * CRK_CCAP + ca) * 16u, planes[p] + ja);
+        if (ROWP > 0) {
+            constexpr int RS = (ROWP == 8) ? 3 : 1;                // log2(ROWP)
+            const int total = s.C << RS;
+            const uint32_t pc = (uint32_t)(tg & (ROWP - 1));       // NT is a multiple of ROWP: a thread always copies the same piece
+            const uint32_t dst0 = tile_s + pc * PSTRIDE;
+            const float4* src0 = rows_src + pc;
+#pragma unroll 4
+            for (int f = tg; f < total; f += NT) {
+                const int c = f >> RS;
+                const uint32_t j = m->cand[c];
+                CRK_CHECK(a.flag, (int64_t)j < a.np, 9);                                    // candidate index
+                cp_async16(dst0 + (uint32_t)c * 16u, src0 + (int64_t)j * FROW);
             }
-            if (cb < s.C) {
+        }
+        if (PLANES > 0) {
+            for (int c0 = 0; c0 < s.C; c0 += NT * 2) {
+                const int ca = c0 + tg, cb = ca + NT;
+                const uint32_t ja = (ca < s.C) ? m->cand[ca] : 0u;
+                const uint32_t jb = (cb < s.C) ? m->cand[cb] : 0u;
+                CRK_CHECK(a.flag, (int64_t)ja < a.np && (int64_t)jb < a.np, 9);             // candidate index
+                if (ca < s.C) {
 #pragma unroll
-                for (int p = 0; p < PLANES; ++p) cp_async16(tile_s + (uint32_t)(p * CRK_CCAP + cb) * 16u, planes[p] + jb);
+                    for (int p = 0; p < PLANES; ++p) cp_async16(tile_s + (uint32_t)(ROWP + p) * PSTRIDE + (uint32_t)ca * 16u, planes[p] + ja);
+                }
+                if (cb < s.C) {
+#pragma unroll
+                    for (int p = 0; p < PLANES; ++p) cp_async16(tile_s + (uint32_t)(ROWP + p) * PSTRIDE + (uint32_t)cb * 16u, planes[p] + jb);
+                }
             }
         }
         cp_async_commit();
@@ -255,7 +279,7 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
         // memory, and the loads of the remaining planes are covered by the arithmetic that needs plane 0 only
         float4 cur[NPRE];
 #pragma unroll
-        for (int p = 0; p < NPRE; ++p) cur[p] = lds128(tile_s + (uint32_t)(p * CRK_CCAP) * 16u + (e[0] & CRK_ELL_MASK) * 16u);
+        for (int p = 0; p < NPRE; ++p) cur[p] = lds128(tile_s + (uint32_t)p * PSTRIDE + (e[0] & CRK_ELL_MASK) * 16u);
         for (int k0 = wl; k0 < rows; k0 += 4 * WPL) {
             uint32_t nx[4];
 #pragma unroll
@@ -269,7 +293,7 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
                 const uint32_t en = (q < 3) ? e[(q + 1) & 3] : nx[0];
                 float4 nxt[NPRE];
 #pragma unroll
-                for (int p = 0; p < NPRE; ++p) nxt[p] = lds128(tile_s + (uint32_t)(p * CRK_CCAP) * 16u + (en & CRK_ELL_MASK) * 16u);
+                for (int p = 0; p < NPRE; ++p) nxt[p] = lds128(tile_s + (uint32_t)p * PSTRIDE + (en & CRK_ELL_MASK) * 16u);
                 CRK_CHECK(a.flag, k >= mine || (int)(e[q] & CRK_ELL_MASK) < s.C, 10);       // entry -> staged slot
                 if (k < mine && (SYM || !(e[q] & CRK_ELL_SYM)))
                     pair(tile_s + (e[q] & CRK_ELL_MASK) * 16u, (e[q] & CRK_ELL_WRAP) != 0u, cur);
@@ -285,9 +309,9 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
     }
 #ifdef CRK_PROBE
     if (tg == 0) {
-        atomicAdd(&crk_probe[PLANES * 4 + 0], (unsigned long long)pr_stage);
-        atomicAdd(&crk_probe[PLANES * 4 + 1], (unsigned long long)(clock64() - pr_t0));
-        atomicAdd(&crk_probe[PLANES * 4 + 2], 1ull);
+        atomicAdd(&crk_probe[(ROWP + PLANES) * 4 + 0], (unsigned long long)pr_stage);
+        atomicAdd(&crk_probe[(ROWP + PLANES) * 4 + 1], (unsigned long long)(clock64() - pr_t0));
+        atomicAdd(&crk_probe[(ROWP + PLANES) * 4 + 2], 1ull);
     }
 #endif
     return count;
@@ -355,12 +379,12 @@ __device__ __forceinline__ void sep3(const SweepArgs& a, bool wrapped, float xi,
 // =================================================================================================== a1: volumes
 // Eq. 14: V_i^-1 = n_i = sum_j W(|x_i - x_j|, h_i), self term included (S4); rho_i = m_i / V_i (S2).
 constexpr int W1_WPC = 2;
-constexpr int W1_SMEM = CRK_CCAP * (int)sizeof(float4) + (int)sizeof(Meta);     // per warp
+constexpr int W1_SMEM = (int)PSTRIDE + (int)sizeof(Meta);     // per warp
 __global__ void __launch_bounds__(W1_WPC * 32) k_volumes(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     float4* tile = (float4*)(smem_raw + (size_t)w * W1_SMEM);
-    Meta* meta = (Meta*)(tile + CRK_CCAP);
+    Meta* meta = (Meta*)((unsigned char*)tile + PSTRIDE);
     const float4* const planes[1] = {a.posh};
     long long leaf = sweep_begin<1>(a, meta, w, 0, lane);
     while (leaf >= 0) {
@@ -371,7 +395,7 @@ __global__ void __launch_bounds__(W1_WPC * 32) k_volumes(SweepArgs a) {
         const float inv_h = valid ? 1.0f / hi : 0.0f;
         float acc = 0.0f;
         long long next;
-        const uint32_t count = leaf_sweep<1, 1, false>(a, planes, leaf, next, w, 0, lane, tile, meta, [&](uint32_t, bool wrapped, const float4* pre) {
+        const uint32_t count = leaf_sweep<1, 0, 1, false>(a, nullptr, planes, leaf, next, w, 0, lane, tile, meta, [&](uint32_t, bool wrapped, const float4* pre) {
             const float4 pj = pre[0];
             float dx, dy, dz, r2;
             sep3(a, wrapped, xi, yi, zi, pj, dx, dy, dz, r2);
@@ -411,13 +435,13 @@ __global__ void __launch_bounds__(256) k_hydro_prep(SweepArgs a, const float4* _
     const float4 ph = a.posh[k];
     if (k < a.n) {
         const float4 v = vel_orig[a.perm[k]];
-        a.velV[k] = make_float4(v.x, v.y, v.z, a.posV[k].w);
+        a.fst[k * FROW] = make_float4(ph.x, ph.y, ph.z, 1.0f / ph.w);
+        a.fst[k * FROW + 1] = make_float4(v.x, v.y, v.z, a.posV[k].w);
         u_s[k] = v.w;
-        a.fst[k] = make_float4(ph.x, ph.y, ph.z, 1.0f / ph.w);
     } else {
-        a.velV[k] = make_float4(0, 0, 0, 0);
+        a.fst[k * FROW] = make_float4(ph.x, ph.y, ph.z, 0.0f);
+        a.fst[k * FROW + 1] = make_float4(0, 0, 0, 0);
         u_s[k] = 0.0f;
-        a.fst[k] = make_float4(ph.x, ph.y, ph.z, 0.0f);
     }
 }
 
@@ -451,12 +475,14 @@ __device__ __forceinline__ void rk_grad(const Coef& k, float x, float y, float z
 __device__ __forceinline__ float visc_Q(float rho, float cs, float mu, float Cl, float Cq) {
     return __fmul_rn(__fmul_rn(rho, mu), __fmaf_rn(Cq, mu, -__fmul_rn(Cl, cs)));
 }
-// dimensional W and D = W'/r for support h:  k3 = sigma/h^3, k5 = sigma/h^5, ih = 1/h
-__device__ __forceinline__ void wendland_dim(float r, float ih, float k3, float k5, float& W, float& D) {
-    float Wt, Dt;
-    wendland(__fmul_rn(r, ih), Wt, Dt);
-    W = __fmul_rn(k3, Wt);
-    D = __fmul_rn(k5, Dt);
+// W~ = (1-eta)^6 (1 + 6 eta + 35/3 eta^2) and D~ = (1-eta)^5 (1 + 5 eta): Eq. 12 and W'/r without sigma/h^3 and
+// -(56/3) sigma/h^5, which the force sweep keeps folded into c', M' and A' (explicit intrinsics: identical bits on both lanes)
+__device__ __forceinline__ void wendland_folded(float eta, float& Wt, float& Dt) {
+    const float t = fmaxf(__fsub_rn(1.0f, eta), 0.0f);
+    const float t2 = __fmul_rn(t, t);
+    const float t5 = __fmul_rn(__fmul_rn(t2, t2), t);
+    Wt = __fmul_rn(__fmul_rn(t5, t), __fmaf_rn(eta, __fmaf_rn(eta, C35_3, 6.0f), 1.0f));
+    Dt = __fmul_rn(t5, __fmaf_rn(5.0f, eta, 1.0f));
 }
 
 // ================================================================== a2 + a3 + a4: RK coefficients and velocity gradient
@@ -485,12 +511,14 @@ template <bool MOM, bool GV>
 __global__ void __launch_bounds__(W2_WPC * 32, (MOM && GV) ? CRK_RK_MINB : (GV ? 8 : 10))
 k_rk(SweepArgs a, const float* __restrict__ u_s, float* __restrict__ gv_full) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    // tile: GV -> the first two pieces of the candidates' force-state rows, (x,y,z,1/h) and (vx,vy,vz,V): one 32-byte sector
+    // each; moments only (crk_rk_coefficients, before the hydro preparation) -> the SoA plane (x,y,z,V)
     constexpr int PL = GV ? 2 : 1;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    constexpr int WSMEM = PL * CRK_CCAP * (int)sizeof(float4) + (int)sizeof(Meta);     // per warp
+    constexpr int WSMEM = PL * (int)PSTRIDE + (int)sizeof(Meta);     // per warp
     float4* tile = (float4*)(smem_raw + (size_t)w * WSMEM);
-    Meta* meta = (Meta*)(tile + PL * CRK_CCAP);
-    const float4* planes[2] = {a.posV, GV ? a.velV : a.posV};
+    Meta* meta = (Meta*)((unsigned char*)tile + PL * PSTRIDE);
+    const float4* planes[1] = {a.posV};
     long long leaf = sweep_begin<1>(a, meta, w, 0, lane);
     while (leaf >= 0) {
         long long next;
@@ -500,7 +528,7 @@ k_rk(SweepArgs a, const float* __restrict__ u_s, float* __restrict__ gv_full) {
         const float xi = ph.x, yi = ph.y, zi = ph.z, hi = ph.w;
         const float inv_h = valid ? 1.0f / hi : 0.0f;
         float4 vi = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (GV) vi = a.velV[i];
+        if (GV) vi = a.fst[i * FROW + 1];
         // moment accumulators: s0; s1[3]; s2[6] (xx,xy,xz,yy,yz,zz); t0[3]; t1[6]; t2[10] (xxx,xxy,xxz,xyy,xyz,xzz,yyy,yyz,yzz,zzz)
         float s0 = 0.f, s1[3] = {0.f, 0.f, 0.f}, s2[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         float t0[3] = {0.f, 0.f, 0.f}, t1[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, t2[10] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
@@ -514,14 +542,17 @@ k_rk(SweepArgs a, const float* __restrict__ u_s, float* __restrict__ gv_full) {
 #pragma unroll
             for (int r = 0; r < 6; ++r) T2[q][r] = 0.f;
         }
-        leaf_sweep<1, PL, false>(a, planes, leaf, next, w, 0, lane, tile, meta, [&](uint32_t sa, bool wrapped, const float4* pre) {
+        leaf_sweep<1, GV ? 2 : 0, GV ? 0 : 1, false>(a, a.fst, planes, leaf, next, w, 0, lane, tile, meta, [&](uint32_t sa, bool wrapped, const float4* pre) {
             const float4 pj = pre[0];
+            float4 vj = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (GV) vj = lds128(sa + PSTRIDE);
+            const float Vj = GV ? vj.w : pj.w;
             float dx, dy, dz, r2;
             sep3(a, wrapped, xi, yi, zi, pj, dx, dy, dz, r2);
             const float r = __fmul_rn(r2, rsqrt_fast(fmaxf(r2, R2_TINY)));
             float Wt, Dt;
             wendland(__fmul_rn(r, inv_h), Wt, Dt);
-            const float wv = __fmul_rn(pj.w, Wt), gv = __fmul_rn(pj.w, Dt);
+            const float wv = __fmul_rn(Vj, Wt), gv = __fmul_rn(Vj, Dt);
             const float x[3] = {__fmul_rn(dx, inv_h), __fmul_rn(dy, inv_h), __fmul_rn(dz, inv_h)};
             const float m2[6] = {__fmul_rn(x[0], x[0]), __fmul_rn(x[0], x[1]), __fmul_rn(x[0], x[2]),
                                  __fmul_rn(x[1], x[1]), __fmul_rn(x[1], x[2]), __fmul_rn(x[2], x[2])};
@@ -545,7 +576,6 @@ k_rk(SweepArgs a, const float* __restrict__ u_s, float* __restrict__ gv_full) {
                 t2[9] = __fmaf_rn(g2[5], x[2], t2[9]);
             }
             if (GV) {
-                const float4 vj = lds128(sa + CRK_CCAP * 16u);
                 const float u[3] = {__fsub_rn(vi.x, vj.x), __fsub_rn(vi.y, vj.y), __fsub_rn(vi.z, vj.z)};
 #pragma unroll
                 for (int q = 0; q < 3; ++q) {
@@ -683,24 +713,24 @@ k_rk(SweepArgs a, const float* __restrict__ u_s, float* __restrict__ gv_full) {
                     g[3 * al + be] = (float)(-t);
                 }
         }
-        // force-sweep state planes: (x,y,z,1/h) (v,V) | (P,rho,cs,k3) (A,B) (c,M0) (M1..M4) (M5..M8) (gxx,gyy,gzz,k5)
-        // (gxy+gyx, gxz+gzx, gyz+gzy, n_h/h).  Only x.(grad v x) enters Eqs. 27-30 and Eq. 25 (uhat_ij.x_ij), so the
-        // symmetric part of grad v is all the force sweep needs; k3 = sigma/h^3, k5 = sigma/h^5.
+        // force-sweep state row (FROW float4 = one 128-byte line per particle; pieces 0 and 1 are written by k_hydro_prep):
+        //   (x,y,z,1/h) (vx,vy,vz,V) | (A',B) (c',M'0) (M'1..M'4) (M'5..M'8) (gxx,gyy,gzz,P) (gxy+gyx, gxz+gzx, gyz+gzy, rho)
+        // with the kernel normalisation folded into the coefficients, A' = -(56/3) sigma/h^5 A, c' = sigma/h^3 c,
+        // M' = sigma/h^3 M, so that grad WR_ij = W~ (c' + M' x) + A' s D~ x with the dimensionless W~ = (1-eta)^6 (1+6 eta+35/3 eta^2),
+        // D~ = (1-eta)^5 (1+5 eta).  Only x.(grad v x) enters Eqs. 27-30 and Eq. 25 (uhat_ij.x_ij), so the symmetric part of
+        // grad v is all the force sweep needs; c_s = sqrt(gamma P / rho) is re-derived there (S12: P <= 0 -> c_s = 0).
         const float ihf = valid ? 1.0f / hi : 0.0f;
         const float k3f = SIGMA_C4 * ihf * ihf * ihf;
-        const float k5f = k3f * ihf * ihf;
+        const float k5f = -C56_3 * (k3f * ihf * ihf);
         const float u = u_s[i], rho = a.rho_s[i], gm = a.gamma;
         const float P = (gm - 1.0f) * rho * u;
-        const float cs = sqrtf(gm * (gm - 1.0f) * fmaxf(u, 0.0f));
-        float4* f = a.fst + i;
-        const int64_t np = a.np;
-        f[2 * np] = make_float4(P, rho, cs, k3f);
-        f[3 * np] = o0;
-        f[4 * np] = o1;
-        f[5 * np] = o2;
-        f[6 * np] = o3;
-        f[7 * np] = make_float4(g[0], g[4], g[8], k5f);
-        f[8 * np] = make_float4(g[1] + g[3], g[2] + g[6], g[5] + g[7], a.n_h * ihf);
+        float4* f = a.fst + i * FROW;
+        f[2] = make_float4(k5f * o0.x, o0.y, o0.z, o0.w);
+        f[3] = make_float4(k3f * o1.x, k3f * o1.y, k3f * o1.z, k3f * o1.w);
+        f[4] = make_float4(k3f * o2.x, k3f * o2.y, k3f * o2.z, k3f * o2.w);
+        f[5] = make_float4(k3f * o3.x, k3f * o3.y, k3f * o3.z, k3f * o3.w);
+        f[6] = make_float4(g[0], g[4], g[8], P);
+        f[7] = make_float4(g[1] + g[3], g[2] + g[6], g[5] + g[7], rho);
         if (gv_full && valid) {                              // diagnostics (crk_get_gradv): all nine components, caller order
             const int32_t p = a.perm[i];
 #pragma unroll
@@ -716,37 +746,30 @@ k_rk(SweepArgs a, const float* __restrict__ u_s, float* __restrict__ gv_full) {
 // Q from Eqs. 24-25 with the limited midpoint projection of Eqs. 27-32 (S7: division-free van Leer form).
 // Sums over all j != i with r2 < max(h_i^2, h_j^2); each ordered pair is evaluated on a lane that holds i in registers.
 // One CTA = one leaf: W5_WPL warps share the tile of the leaf's candidates and split each lane's entries by rows.
+struct ForceConst {
+    float L, half, eta_crit, inv_fold, eps2, Cl, Cq, gamma, n_h;
+};
 struct PState {           // one particle's force-sweep state in registers
-    float x, y, z, ih, vx, vy, vz, V, P, rho, cs, k3, k5, qh;
-    Coef c;
+    float x, y, z, ih, vx, vy, vz, V, P, rho, cs, qh;
+    Coef c;                                              // A', B, c', M' (kernel normalisation folded in, see k_rk)
     float gxx, gyy, gzz, gxy, gxz, gyz;                  // symmetric part of grad v, off-diagonals summed
 };
-__device__ __forceinline__ PState load_pstate(const float4* __restrict__ f, int64_t stride) {
-    const float4 a0 = f[0], a1 = f[stride], a2 = f[2 * stride], a3 = f[3 * stride], a4 = f[4 * stride], a5 = f[5 * stride],
-                 a6 = f[6 * stride], a7 = f[7 * stride], a8 = f[8 * stride];
-    PState s;
-    s.x = a0.x; s.y = a0.y; s.z = a0.z; s.ih = a0.w;
-    s.vx = a1.x; s.vy = a1.y; s.vz = a1.z; s.V = a1.w;
-    s.P = a2.x; s.rho = a2.y; s.cs = a2.z; s.k3 = a2.w;
-    s.c = load_coef(a3, a4, a5, a6);
-    s.gxx = a7.x; s.gyy = a7.y; s.gzz = a7.z; s.k5 = a7.w;
-    s.gxy = a8.x; s.gxz = a8.y; s.gyz = a8.z; s.qh = a8.w;
-    return s;
-}
 constexpr int FPRE = 1;   // planes of the next pair's j-state fetched one pair ahead (3, 5, 9 measured slower: 11.3, 11.5, 13.5 vs 11.1 ms)
-__device__ __forceinline__ PState load_pstate_shared(uint32_t sa, const float4* pre) {
-    constexpr uint32_t ST = CRK_CCAP * 16u;
-    float4 q[FPL];
+// the row of candidate slot `sa` from the tile.  c_s = sqrt(gamma max(P,0) / rho) (Eq. 4 + PAPER.md:149, S12) and q = n_h / h are
+// re-derived here with a fixed instruction sequence, so both lanes of a pair hold identical bits for either particle.
+__device__ __forceinline__ PState load_pstate_shared(const ForceConst& k, uint32_t sa, const float4* pre) {
+    float4 q[FROW];
 #pragma unroll
-    for (int p = 0; p < FPL; ++p) q[p] = (p < FPRE) ? pre[p] : lds128(sa + (uint32_t)p * ST);
-    const float4 a0 = q[0], a1 = q[1], a2 = q[2], a3 = q[3], a4 = q[4], a5 = q[5], a6 = q[6], a7 = q[7], a8 = q[8];
+    for (int p = 0; p < FROW; ++p) q[p] = (p < FPRE) ? pre[p] : lds128(sa + (uint32_t)p * PSTRIDE);
     PState s;
-    s.x = a0.x; s.y = a0.y; s.z = a0.z; s.ih = a0.w;
-    s.vx = a1.x; s.vy = a1.y; s.vz = a1.z; s.V = a1.w;
-    s.P = a2.x; s.rho = a2.y; s.cs = a2.z; s.k3 = a2.w;
-    s.c = load_coef(a3, a4, a5, a6);
-    s.gxx = a7.x; s.gyy = a7.y; s.gzz = a7.z; s.k5 = a7.w;
-    s.gxy = a8.x; s.gxz = a8.y; s.gyz = a8.z; s.qh = a8.w;
+    s.x = q[0].x; s.y = q[0].y; s.z = q[0].z; s.ih = q[0].w;
+    s.vx = q[1].x; s.vy = q[1].y; s.vz = q[1].z; s.V = q[1].w;
+    s.c = load_coef(q[2], q[3], q[4], q[5]);
+    s.gxx = q[6].x; s.gyy = q[6].y; s.gzz = q[6].z; s.P = q[6].w;
+    s.gxy = q[7].x; s.gxz = q[7].y; s.gyz = q[7].z; s.rho = q[7].w;
+    s.qh = __fmul_rn(k.n_h, s.ih);
+    const float gp = __fmul_rn(k.gamma, fmaxf(s.P, 0.0f));
+    s.cs = __fmul_rn(gp, rsqrt_fast(fmaxf(__fmul_rn(gp, s.rho), R2_TINY)));
     return s;
 }
 // x.(grad v x) with the symmetric part (Eq. 30 numerator / denominator)
@@ -758,9 +781,6 @@ __device__ __forceinline__ float quad_form(const PState& s, float dxx, float dyy
 __device__ __forceinline__ float visc_mu(float qh, float udx, float r2, float eps2) {
     return fminf(0.0f, __fmul_rn(__fmul_rn(qh, udx), rcp_fast(__fmaf_rn(__fmul_rn(qh, qh), r2, eps2))));
 }
-struct ForceConst {
-    float L, half, eta_crit, inv_fold, eps2, Cl, Cq;
-};
 // one ordered pair (i, j): F = m_i a_ij (Eq. 17 with P -> P + Q) and e = its term of m_i du_i/dt (Eq. 18);
 // vji = v_j - v_i
 struct PairF { float Fx, Fy, Fz, e, vjix, vjiy, vjiz, app, Qi; };   // app = approach speed (Eq. 50), Qi (Eq. 24)
@@ -778,9 +798,9 @@ __device__ __forceinline__ PairF force_pair(const ForceConst& k, const PState& I
     const float r2 = __fmaf_rn(dz, dz, __fmaf_rn(dy, dy, __fmul_rn(dx, dx)));
     const float rinv = rsqrt_fast(fmaxf(r2, R2_TINY));
     const float r = __fmul_rn(r2, rinv);
-    float Wi, Di, Wj, Dj;
-    wendland_dim(r, I.ih, I.k3, I.k5, Wi, Di);
-    wendland_dim(r, J.ih, J.k3, J.k5, Wj, Dj);
+    float Wi, Di, Wj, Dj;                                       // W~, D~ (the normalisation sits in A', c', M')
+    wendland_folded(__fmul_rn(r, I.ih), Wi, Di);
+    wendland_folded(__fmul_rn(r, J.ih), Wj, Dj);
     float aix, aiy, aiz, ajx, ajy, ajz;
     rk_grad(I.c, dx, dy, dz, Wi, Di, aix, aiy, aiz);            // grad WR_ij
     rk_grad(J.c, -dx, -dy, -dz, Wj, Dj, ajx, ajy, ajz);         // grad WR_ji  (x_ji = -x_ij)
@@ -830,11 +850,8 @@ __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
     float4* tile = (float4*)smem_raw;
-    Meta* meta = (Meta*)(tile + FPL * CRK_CCAP);
-    const ForceConst fc = {a.L, a.half, 1.0f / a.n_h, a.n_h / 0.2f, a.eps2, a.C_l, a.C_q};
-    const float4* planes[FPL];
-#pragma unroll
-    for (int p = 0; p < FPL; ++p) planes[p] = a.fst + (int64_t)p * a.np;
+    Meta* meta = (Meta*)(smem_raw + FROW * PSTRIDE);
+    const ForceConst fc = {a.L, a.half, 1.0f / a.n_h, a.n_h / 0.2f, a.eps2, a.C_l, a.C_q, a.gamma, a.n_h};
     long long leaf = sweep_begin<W5_WPL>(a, meta, 0, wl, lane);
     while (leaf >= 0) {
         const int64_t i = leaf * CRK_LEAF + lane;
@@ -843,8 +860,8 @@ __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
         float acc[4] = {0.f, 0.f, 0.f, 0.f};                 // Fx, Fy, Fz, dE
         float mx[2] = {0.f, 0.f};                            // max approach speed, max Q_i
         long long next;
-        const uint32_t count = leaf_sweep<W5_WPL, FPL, true, FPRE>(a, planes, leaf, next, 0, wl, lane, tile, meta, [&](uint32_t sa, bool wrapped, const float4* pre) {
-            const PState J = load_pstate_shared(sa, pre);
+        const uint32_t count = leaf_sweep<W5_WPL, FROW, 0, true, FPRE>(a, a.fst, nullptr, leaf, next, 0, wl, lane, tile, meta, [&](uint32_t sa, bool wrapped, const float4* pre) {
+            const PState J = load_pstate_shared(fc, sa, pre);
             const PairF f = force_pair(fc, I, J, wrapped);
             acc[0] += f.Fx; acc[1] += f.Fy; acc[2] += f.Fz; acc[3] += f.e;
             if (TS) {
@@ -854,8 +871,8 @@ __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
         }, [&](uint32_t ts) {
             float4 pre[FPRE];
 #pragma unroll
-            for (int p = 0; p < FPRE; ++p) pre[p] = lds128(ts + (uint32_t)(p * CRK_CCAP + lane) * 16u);
-            I = load_pstate_shared(ts + (uint32_t)lane * 16u, pre);
+            for (int p = 0; p < FPRE; ++p) pre[p] = lds128(ts + (uint32_t)p * PSTRIDE + (uint32_t)lane * 16u);
+            I = load_pstate_shared(fc, ts + (uint32_t)lane * 16u, pre);
         });
         group_reduce<W5_WPL, 4>(acc, 0, wl, lane, (float*)tile);
         if (TS) group_reduce<W5_WPL, 2, true>(mx, 0, wl, lane, (float*)tile);
@@ -874,7 +891,7 @@ __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
                     if (a.ocnt) a.ocnt[p] = count;
                 }
             }
-            a.fst[(int64_t)FPL * a.np + i] = as;             // plane 9: (dv/dt, s = P / rho^gamma) for crk_compatible_energy
+            a.facc[i] = as;                                  // (dv/dt, s = P / rho^gamma) for crk_compatible_energy, crk_timestep
         }
         leaf = next;
     }
@@ -904,27 +921,24 @@ __global__ void __launch_bounds__(256) k_compat_prep(const float4* __restrict__ 
     kick[k] = w;
 }
 
-__global__ void __launch_bounds__(W5_WPL * 32, 3) k_compat(SweepArgs a, float dt, const float4* __restrict__ kick) {
+__global__ void __launch_bounds__(W5_WPL * 32, 4) k_compat(SweepArgs a, float dt, const float4* __restrict__ kick) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
     float4* tile = (float4*)smem_raw;
-    Meta* meta = (Meta*)(tile + CPL * CRK_CCAP);
-    const ForceConst fc = {a.L, a.half, 1.0f / a.n_h, a.n_h / 0.2f, a.eps2, a.C_l, a.C_q};
-    const float4* planes[CPL];
-#pragma unroll
-    for (int p = 0; p < FPL; ++p) planes[p] = a.fst + (int64_t)p * a.np;
-    planes[FPL] = kick;
+    Meta* meta = (Meta*)(smem_raw + CPL * PSTRIDE);
+    const ForceConst fc = {a.L, a.half, 1.0f / a.n_h, a.n_h / 0.2f, a.eps2, a.C_l, a.C_q, a.gamma, a.n_h};
+    const float4* planes[1] = {kick};                       // tile plane FROW
     long long leaf = sweep_begin<W5_WPL>(a, meta, 0, wl, lane);
     while (leaf >= 0) {
         const int64_t i = leaf * CRK_LEAF + lane;
         const bool valid = i < a.n;
-        const PState I = load_pstate(a.fst + i, a.np);
+        PState I;                                            // from the tile, as in k_forces
         const float4 qi = kick[i];
         float acc[1] = {0.f};
         long long next;
-        leaf_sweep<W5_WPL, CPL, true, FPRE>(a, planes, leaf, next, 0, wl, lane, tile, meta, [&](uint32_t sa, bool wrapped, const float4* pre) {
-            const PState J = load_pstate_shared(sa, pre);
-            const float4 qj = lds128(sa + (uint32_t)FPL * CRK_CCAP * 16u);
+        leaf_sweep<W5_WPL, FROW, 1, true, FPRE>(a, a.fst, planes, leaf, next, 0, wl, lane, tile, meta, [&](uint32_t sa, bool wrapped, const float4* pre) {
+            const PState J = load_pstate_shared(fc, sa, pre);
+            const float4 qj = lds128(sa + (uint32_t)FROW * PSTRIDE);
             const PairF f = force_pair(fc, I, J, wrapped);
             // (v_j + v'_j - v_i - v'_i) = 2 (v_j - v_i) + (kick_j - kick_i)
             const float wx = __fmaf_rn(2.0f, f.vjix, __fsub_rn(qj.x, qi.x));
@@ -938,6 +952,11 @@ __global__ void __launch_bounds__(W5_WPL * 32, 3) k_compat(SweepArgs a, float dt
                 part = (small ? fminf(si, sj) : fmaxf(si, sj)) * rcp_fast(__fadd_rn(si, sj));
             }
             acc[0] = fmaf(0.5f * part, w, acc[0]);
+        }, [&](uint32_t ts) {
+            float4 pre[FPRE];
+#pragma unroll
+            for (int p = 0; p < FPRE; ++p) pre[p] = lds128(ts + (uint32_t)p * PSTRIDE + (uint32_t)lane * 16u);
+            I = load_pstate_shared(fc, ts + (uint32_t)lane * 16u, pre);
         });
         group_reduce<W5_WPL, 1>(acc, 0, wl, lane, (float*)tile);
         if (wl == 0 && valid) a.o0[a.perm[i]] = acc[0] * dt / a.m_s[i];
@@ -959,8 +978,8 @@ SweepArgs make_args(crk_ctx* c) {
     a.arena = (const uint4*)c->arena.p; a.seg_first = (const uint4*)c->seg_first.p; a.leaf_cnt = (const uint16_t*)c->leaf_cnt.p;
     a.cand_first = (const uint32_t*)c->cand_first.p;
     a.perm = c->perm;
-    a.posh = (const float4*)c->posh.p; a.posV = (float4*)c->posV.p; a.velV = nullptr;
-    a.coef = (float4*)c->coef.p; a.fst = (float4*)c->fst.p;
+    a.posh = (const float4*)c->posh.p; a.posV = (float4*)c->posV.p;
+    a.coef = (float4*)c->coef.p; a.fst = (float4*)c->fst.p; a.facc = (float4*)c->facc.p;
     a.rho_s = (float*)c->rho_s.p; a.m_s = (const float*)c->m_s.p;
     a.gamma = c->prm.gamma; a.n_h = c->prm.n_h; a.C_l = c->prm.C_l; a.C_q = c->prm.C_q;
     a.eps2 = c->prm.eps * c->prm.eps;
@@ -1014,11 +1033,11 @@ int crk_launch_hydro_prep(crk_ctx* c, const float* vx, const float* vy, const fl
     const int64_t np = c->nl * CRK_LEAF;
     CRK_TRY(crk_ensure(c, c->vel_orig, (size_t)c->n * sizeof(float4)));
     CRK_TRY(crk_ensure(c, c->u_s, (size_t)np * sizeof(float)));
-    CRK_TRY(crk_ensure(c, c->fst, (size_t)np * CPL * sizeof(float4)));
+    CRK_TRY(crk_ensure(c, c->fst, (size_t)np * FROW * sizeof(float4)));
+    CRK_TRY(crk_ensure(c, c->facc, (size_t)np * sizeof(float4)));
     k_pack_vel<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>(vx, vy, vz, u, c->n, (float4*)c->vel_orig.p);
     CRK_TRY(crk_check_launch(c, "k_pack_vel"));
     SweepArgs a = make_args(c);
-    a.velV = (float4*)c->fst.p + np;                     // plane 1 of the force-sweep state is (vx,vy,vz,V)
     k_hydro_prep<<<(unsigned)((np + 255) / 256), 256, 0, c->stream>>>(a, (const float4*)c->vel_orig.p, (float*)c->u_s.p);
     return crk_check_launch(c, "k_hydro_prep");
 }
@@ -1030,11 +1049,10 @@ int crk_launch_rk(crk_ctx* c, bool mom, bool gv, float* A, float* B, float* grad
     CRK_TRY(crk_ensure(c, c->coef, (size_t)np * 4 * sizeof(float4)));
     SweepArgs a = make_args(c);
     a.o0 = A; a.o1 = B; a.o2 = gradA; a.o3 = gradB;
-    a.velV = gv ? (float4*)c->fst.p + np : nullptr;
     a.ids = ids; a.n_ids = n_ids;
     const int64_t items = ids ? n_ids : c->nl;
     if (items == 0) return CRK_OK;
-    const int smem = W2_WPC * ((gv ? 2 : 1) * CRK_CCAP * (int)sizeof(float4) + (int)sizeof(Meta));
+    const int smem = W2_WPC * ((gv ? 2 : 1) * (int)PSTRIDE + (int)sizeof(Meta));
     const float* us = (const float*)c->u_s.p;
     unsigned grid = 0;
     if (mom && gv) {
@@ -1061,9 +1079,8 @@ int crk_launch_forces(crk_ctx* c, float* ax, float* ay, float* az, float* dudt, 
     a.ids = ids; a.n_ids = n_ids; a.active = active;
     const int64_t items = ids ? n_ids : c->nl;
     if (items == 0) return CRK_OK;
-    a.velV = (float4*)c->fst.p + np;
     a.o0 = ax; a.o1 = ay; a.o2 = az; a.o3 = dudt; a.ocnt = pair_count;
-    const int smem = FPL * CRK_CCAP * (int)sizeof(float4) + (int)sizeof(Meta);
+    const int smem = FROW * (int)PSTRIDE + (int)sizeof(Meta);
     unsigned grid = 0;
     if (c->prm.flags & CRK_FLAG_TIMESTEP) {
         CRK_TRY(crk_ensure(c, c->ts_s, (size_t)np * sizeof(float2)));
@@ -1134,11 +1151,11 @@ int crk_launch_compat(crk_ctx* c, float dt, float c1, float c0, const float* bx,
     const int64_t np = c->nl * CRK_LEAF;
     CRK_TRY(crk_ensure(c, c->kick, (size_t)np * sizeof(float4)));
     SweepArgs a = make_args(c);
-    k_compat_prep<<<(unsigned)((np + 255) / 256), 256, 0, c->stream>>>((const float4*)c->fst.p + (int64_t)FPL * np, c->perm, c->n,
+    k_compat_prep<<<(unsigned)((np + 255) / 256), 256, 0, c->stream>>>((const float4*)c->facc.p, c->perm, c->n,
                                                                        np, c1, c0, bx, by, bz, (float4*)c->kick.p);
     CRK_TRY(crk_check_launch(c, "k_compat_prep"));
     a.o0 = delta_u;
-    const int smem = CPL * CRK_CCAP * (int)sizeof(float4) + (int)sizeof(Meta);
+    const int smem = CPL * (int)PSTRIDE + (int)sizeof(Meta);
     unsigned grid = 0;
     CRK_TRY(persistent_grid(c, k_compat, W5_WPL * 32, smem, 1, c->nl, &grid));
     a.sched = (unsigned int*)c->sched.p;
@@ -1171,18 +1188,19 @@ int crk_launch_evolve_h(crk_ctx* c, float* h_new) {
 // NEXT row 2a: time-step criteria, Eqs. 46-50 with a = 1, adot = 0, no gravity: a stream pass over the
 // force-sweep state and the two per-particle maxima reduced by k_forces<true>
 namespace {
-__global__ void __launch_bounds__(256) k_timestep(const float4* __restrict__ fst, const float2* __restrict__ ts,
-                                                  const int32_t* __restrict__ perm, int64_t n, int64_t np, float C_cfl,
-                                                  float* __restrict__ dt_min) {
+__global__ void __launch_bounds__(256) k_timestep(const float4* __restrict__ fst, const float4* __restrict__ facc,
+                                                  const float2* __restrict__ ts, const int32_t* __restrict__ perm, int64_t n,
+                                                  float gamma, float n_h, float C_cfl, float* __restrict__ dt_min) {
     const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= n) return;
-    const float4 th = fst[2 * np + k];                   // P, rho, c_s, k3
-    const float4 g = fst[7 * np + k];                    // g_xx, g_yy, g_zz
-    const float hhat = 1.0f / fst[8 * np + k].w;         // h / n_h
-    const float4 acc = fst[(int64_t)FPL * np + k];       // dv/dt
+    const float4 g = fst[k * FROW + 6];                  // g_xx, g_yy, g_zz, P
+    const float rho = fst[k * FROW + 7].w;
+    const float cs = sqrtf(gamma * fmaxf(g.w, 0.0f) / rho);
+    const float hhat = 1.0f / (n_h * fst[k * FROW].w);   // h / n_h
+    const float4 acc = facc[k];                          // dv/dt
     const float2 mx = ts[k];
-    const float csq = sqrtf(4.0f * mx.y / th.y);                                             // sqrt(zeta Q / rho)
-    const float vmax = fmaxf(fmaxf(mx.x, th.z), fmaxf(csq, hhat * fabsf(g.x + g.y + g.z)));  // Eq. 46
+    const float csq = sqrtf(4.0f * mx.y / rho);                                              // sqrt(zeta Q / rho)
+    const float vmax = fmaxf(fmaxf(mx.x, cs), fmaxf(csq, hhat * fabsf(g.x + g.y + g.z)));    // Eq. 46
     const float dth = C_cfl * hhat / vmax;                                                   // Eq. 47
     const float dta = sqrtf(hhat / sqrtf(acc.x * acc.x + acc.y * acc.y + acc.z * acc.z));    // Eq. 48, r_soft = inf
     dt_min[perm[k]] = fminf(dth, dta);                                                       // Eq. 49
@@ -1190,7 +1208,8 @@ __global__ void __launch_bounds__(256) k_timestep(const float4* __restrict__ fst
 }  // namespace
 
 int crk_launch_timestep(crk_ctx* c, float C_cfl, float* dt_min) {
-    k_timestep<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>((const float4*)c->fst.p, (const float2*)c->ts_s.p,
-                                                                      c->perm, c->n, c->nl * CRK_LEAF, C_cfl, dt_min);
+    k_timestep<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>((const float4*)c->fst.p, (const float4*)c->facc.p,
+                                                                      (const float2*)c->ts_s.p, c->perm, c->n, c->prm.gamma,
+                                                                      c->prm.n_h, C_cfl, dt_min);
     return crk_check_launch(c, "k_timestep");
 }
