@@ -17,22 +17,21 @@
 enum { EV_BUILD0 = 0, EV_SORTED, EV_TREE1, EV_BUILD1, EV_VOL0, EV_VOL1, EV_RK0, EV_GV0, EV_GV1, EV_F1, EV_RK1, EV_HY0, EV_PREP1 };
 
 // ---- neighbour lists (lists.cu): per leaf a chain of segments in one arena of 16-byte units --------------------------
-//   segment = header (9 units) | cand[C] u32, padded to 4 (not in a leaf's first segment) | ell[K][32] u16
-//   header unit 0: {next segment (arena unit, 0 = none), C | CRK_SEG_WRAP | K << 16, 0, 0}; units 1-4: cnt_g[32] u16;
-//   units 5-8: cnt[32] u16
+//   segment = header (5 units) | cand[C] u32, padded to 4 (not in a leaf's first segment) | ell[K][32] u16
+//   header unit 0: {next segment (arena unit, 0 = none), C | CRK_SEG_WRAP | K << 16, 0, 0}; units 1-4: cnt[32] u16
 //   the first segment's header is mirrored in dense per-leaf arrays, so that a sweep reaches the payload without a
 //   pointer chase: seg_first[leaf] = {next, C | CRK_SEG_WRAP | K << 16, 0, own arena unit (0 = leaf has no segment)},
-//   leaf_cnt[leaf][64] = cnt_g | cnt, and cand_first[leaf][CRK_CAND_STRIDE] = the first segment's candidate indices
+//   leaf_cnt[leaf][32] = cnt, and cand_first[leaf][CRK_CAND_STRIDE] = the first segment's candidate indices
 //   cand[c]   = sorted-order index of candidate c (only candidates accepted by at least one lane of the leaf); in a
 //               leaf's first segment cand[0..31] are the leaf's own 32 particles in lane order (always kept)
 //   ell[k][l] = k-th entry of lane l: candidate index | CRK_ELL_SYM (h_i^2 <= r2 < h_j^2: a pair of the symmetric set that
 //               is not in the lane's gather set) | CRK_ELL_WRAP (pair crosses the periodic boundary); lane l owns cnt[l]
-//               entries, cnt_g[l] of them gather entries; CRK_SEG_WRAP: some entry of the segment may carry CRK_ELL_WRAP
+//               entries; CRK_SEG_WRAP: some entry of the segment may carry CRK_ELL_WRAP
 #define CRK_CCAP 384             // candidates per segment (tile capacity of the sweeps)
 #define CRK_CAND_STRIDE 384      // u32 per leaf in cand_first (the sweeps read it in 16-byte groups)
 #define CRK_QCAP 128             // entries per lane per segment
 #define CRK_TCULL 32             // cull tile of the list builder
-#define CRK_SEG_HDR_UNITS 9
+#define CRK_SEG_HDR_UNITS 5
 #define CRK_ELL_WRAP 0x8000u
 #define CRK_ELL_SYM  0x4000u
 #define CRK_ELL_MASK 0x3fffu
@@ -104,7 +103,7 @@ struct crk_ctx {
     int key_bits = 0;              // space-filling-curve bits per axis of the last build (0 = not known yet)
     int64_t n_pairs = 0, n_pairs_gather = 0;
     DevBuf arena, seg_first;       // neighbour-list arena (16-byte units); per leaf a uint4 copy of its first segment's header
-    DevBuf leaf_cnt;               // u16[nl][64]: per-lane cnt_g | cnt of the first segment (dense, so the sweeps need no pointer chase)
+    DevBuf leaf_cnt;               // u16[nl][32]: per-lane entry counts of the first segment (dense, like cand_first)
     DevBuf cand_first;             // u32[nl][CRK_CAND_STRIDE]: candidate indices of the first segment (dense)
     DevBuf act_flags, act_offs, act_ids;   // crk_hydro_derivs_active: leaf flags (active | halo), their scan, compacted leaf ids
     int64_t n_active_leaves = 0, n_halo_leaves = 0;

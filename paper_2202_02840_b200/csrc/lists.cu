@@ -30,7 +30,7 @@ struct ListArgs {
     unsigned long long arena_cap;          // units
     unsigned long long* counter;           // next free unit (unit 0 is reserved as "none")
     uint4* __restrict__ seg_first;         // dense copy of each leaf's first header (.w = its arena unit)
-    uint16_t* __restrict__ leaf_cnt;       // [nl][64]
+    uint16_t* __restrict__ leaf_cnt;       // [nl][32]
     uint32_t* __restrict__ cand_first;     // [nl][CRK_CAND_STRIDE] candidates of each leaf's first segment
     int* flag;                             // status words (CRK_CHECKED builds write FW_CHECK)
 };
@@ -40,7 +40,7 @@ struct WarpSmem {
     float4 tb[(CRK_TCULL + 2) / 2];   //                      (-z_a, -z_b, h_a^2, h_b^2)
     __align__(8) uint32_t tidx[CRK_TCULL + 2];
     uint32_t cand[CRK_CCAP];
-    uint16_t queue[CRK_QCAP][32];
+    __align__(16) uint16_t queue[CRK_QCAP][32];   // same layout as a segment's entry block: emit copies it in 16-byte units
 };
 
 // lower bound of |wrap(x_i - x_j)| on one axis for x_i in [lo,hi] (monotone float ops, so nothing is lost)
@@ -59,10 +59,6 @@ __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)_
 __device__ __forceinline__ void sts_u16_if(uint32_t addr, uint32_t v, bool pred) {
     asm volatile("{ .reg .pred p; setp.ne.b32 p, %2, 0; @p st.shared.u16 [%0], %1; }" ::"r"(addr), "h"((uint16_t)v), "r"((int)pred) : "memory");
 }
-__device__ __forceinline__ void sts_u32_if(uint32_t addr, uint32_t v, bool pred) {
-    asm volatile("{ .reg .pred p; setp.ne.b32 p, %2, 0; @p st.shared.u32 [%0], %1; }" ::"r"(addr), "r"(v), "r"((int)pred) : "memory");
-}
-
 // minimum-image wrap of both halves (S3: d > L/2 -> d - L, d < -L/2 -> d + L); adding 0 leaves the other values untouched
 __device__ __forceinline__ float2 wrap2(float2 d, float L, float half, bool& wa, bool& wb) {
     const float sa = d.x > half ? -L : (d.x < -half ? L : 0.f);
@@ -73,18 +69,22 @@ __device__ __forceinline__ float2 wrap2(float2 d, float L, float half, bool& wa,
 }
 
 // test every staged candidate against the lane's particle; returns the new candidate count of the segment.
-// Branch-free, two candidates per trip (the tile is padded to an even count with a far-away sentinel): about 9 of 10
-// culled candidates are accepted by some lane, so predicated appends beat a vote-and-branch per candidate.
-// SELF: the tile holds the query leaf itself, so j = i has to be excluded (and every candidate keeps its slot).
+// Branch-free, two candidates per trip (the tile is padded to an even count with a far-away sentinel): about 3 of 4
+// culled candidates are accepted by some lane, so predicated appends beat a vote-and-branch per candidate.  A candidate
+// accepted by at least one lane receives the next slot of the segment (kept = bit mask of those candidates; their indices
+// are compacted into S.cand after the loop); keeping every culled candidate instead was measured: a third more slots, half of
+// the leaves spill into a second segment and every sweep stages and pays for them (forces 11.0 -> 12.8 ms).
+// SELF: the tile holds the query leaf itself in lane order (C = 0), so j = i is the candidate t = lane, and every candidate
+// keeps its slot.
 template <bool WRAP, bool SELF>
-__device__ __forceinline__ int test_tile(WarpSmem& S, int* flag, int fill, int C, int& g, bool& wflag, int lane, uint32_t self,
+__device__ __forceinline__ int test_tile(WarpSmem& S, int* flag, int fill, int C, int& g, bool& wflag, int lane,
                                          float xi, float yi, float zi, float hi2, float L, float half) {
     uint32_t gp = smem_u32(&S.queue[g][lane]);                  // next entry of this lane (row stride 64 bytes)
-    const uint32_t cbase = smem_u32(&S.cand[0]);
     const float2 xi2 = make_float2(xi, xi), yi2 = make_float2(yi, yi), zi2 = make_float2(zi, zi);
+    const int C0 = C;
+    uint32_t kept = 0u;
     for (int t0 = 0; t0 < fill; t0 += 2) {
         const float4 pa = S.ta[t0 >> 1], pb = S.tb[t0 >> 1];
-        const uint2 ji = *(const uint2*)&S.tidx[t0];
         float2 dx = __fadd2_rn(xi2, make_float2(pa.x, pa.y));    // x_i - x_j (the tile holds -x_j)
         float2 dy = __fadd2_rn(yi2, make_float2(pa.z, pa.w));
         float2 dz = __fadd2_rn(zi2, make_float2(pb.x, pb.y));
@@ -96,13 +96,12 @@ __device__ __forceinline__ int test_tile(WarpSmem& S, int* flag, int fill, int C
         }
         const float2 r2v = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
         const float r2[2] = {r2v.x, r2v.y}, hj2[2] = {pb.z, pb.w};
-        const uint32_t jv[2] = {ji.x, ji.y};
 #pragma unroll
         for (int u = 0; u < 2; ++u) {
             bool ag = r2[u] < hi2;                                         // gather: Eqs. 13-14
             bool as = ag || (r2[u] < hj2[u]);                              // symmetric: r2 < max(h_i^2, h_j^2), Eqs. 17-18
             if (SELF) {
-                const bool notself = jv[u] != self;
+                const bool notself = (t0 + u) != lane;
                 ag = ag && notself;
                 as = as && notself;
             }
@@ -116,10 +115,11 @@ __device__ __forceinline__ int test_tile(WarpSmem& S, int* flag, int fill, int C
             CRK_CHECK(flag, !any || C < CRK_CCAP, 1);                                      // candidate slot < CRK_CCAP
             sts_u16_if(gp, e, as);                                         // one predicated store, no branch
             gp += as ? 64u : 0u;
-            sts_u32_if(cbase + 4u * (uint32_t)C, jv[u], any);              // every lane stores the same word: one wavefront
+            kept |= any ? (1u << (t0 + u)) : 0u;
             C += any ? 1 : 0;
         }
     }
+    if (lane < fill && ((kept >> lane) & 1u)) S.cand[C0 + __popc(kept & ((1u << lane) - 1u))] = S.tidx[lane];
     g = (int)((gp - smem_u32(&S.queue[0][lane])) >> 6);
     return C;
 }
@@ -152,31 +152,29 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
         const int K = __reduce_max_sync(0xffffffffu, g);
         const bool segwrap = __any_sync(0xffffffffu, wflag);
         const bool head = (prev == 0);   // a leaf's first segment keeps its candidates in the dense per-leaf array
-        const unsigned long long units = CRK_SEG_HDR_UNITS + (head ? 0ull : (unsigned long long)((C + 3) >> 2)) + 4ull * K;
+        const unsigned long long cunits = head ? 0ull : (unsigned long long)((C + 3) >> 2);
+        const unsigned long long units = CRK_SEG_HDR_UNITS + cunits + 4ull * K;
         unsigned long long base = 0;
         if (lane == 0) base = atomicAdd(a.counter, units);
         base = __shfl_sync(0xffffffffu, base, 0);
+        // padding of shorter lanes: slot 0 (the sweeps prefetch it, never evaluate it)
+        for (int k = g; k < K; ++k) S.queue[k][lane] = (uint16_t)0;
         __syncwarp();
         if (base + units <= a.arena_cap) {
             CRK_CHECK(a.flag, K <= CRK_QCAP && C <= CRK_CCAP && base >= 1, 3);                 // segment sizes
             uint4* hdr = a.arena + base;
             const uint32_t h1 = (uint32_t)C | (segwrap ? CRK_SEG_WRAP : 0u) | ((uint32_t)K << 16);
             if (lane == 0) hdr[0] = make_uint4(0u, h1, 0u, 0u);
-            ((uint16_t*)(hdr + 5))[lane] = (uint16_t)g;
+            ((uint16_t*)(hdr + 1))[lane] = (uint16_t)g;
             uint32_t* cd = head ? a.cand_first + leaf * CRK_CAND_STRIDE : (uint32_t*)(hdr + CRK_SEG_HDR_UNITS);
             for (int c = lane; c < C; c += 32) cd[c] = S.cand[c];
-            uint16_t* el = (uint16_t*)(hdr + CRK_SEG_HDR_UNITS + (head ? 0 : ((C + 3) >> 2)));
-            int ng = g;                   // gather entries of this lane = entries without the symmetric-only flag
-            for (int k = 0; k < K; ++k) {   // padding of shorter lanes: slot 0 (the sweeps prefetch it, never evaluate it)
-                const uint32_t v = (k < g) ? (uint32_t)S.queue[k][lane] : 0u;
-                ng -= (int)((v >> 14) & 1u);
-                el[k * 32 + lane] = (uint16_t)v;
-            }
-            ((uint16_t*)(hdr + 1))[lane] = (uint16_t)ng;
+            // the entry block is the queue as it stands: K rows of 32 u16 = 4 K units
+            uint4* el = hdr + CRK_SEG_HDR_UNITS + cunits;
+            const uint4* qs = (const uint4*)&S.queue[0][0];
+            for (int q = lane; q < 4 * K; q += 32) el[q] = qs[q];
             if (head) {
                 if (lane == 0) a.seg_first[leaf] = make_uint4(0u, h1, 0u, (uint32_t)base);
-                a.leaf_cnt[leaf * 64 + lane] = (uint16_t)ng;
-                a.leaf_cnt[leaf * 64 + 32 + lane] = (uint16_t)g;
+                a.leaf_cnt[leaf * 32 + lane] = (uint16_t)g;
                 first = (uint32_t)base;
             } else if (lane == 0) {
                 ((uint32_t*)(a.arena + prev))[0] = (uint32_t)base;
@@ -187,14 +185,17 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
         C = 0; g = 0; wflag = false;
         __syncwarp();
     };
+    // a leaf that straddles the periodic boundary needs the wrap in its own tile too
+    const bool selfwrap = (bhi.x - blo.x > a.half) || (bhi.y - blo.y > a.half) || (bhi.z - blo.z > a.half);
     auto flush = [&](bool selftile) {
         const int maxlen = __reduce_max_sync(0xffffffffu, g);
         if (C + fill > CRK_CCAP || maxlen + fill > CRK_QCAP) emit();
         if ((fill & 1) && lane == 0) put(fill, 3.0e30f, 3.0e30f, 3.0e30f, 0.0f, 0u);
         __syncwarp();
-        if (selftile) C = test_tile<true, true>(S, a.flag, fill, C, g, wflag, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
-        else if (cwrap) C = test_tile<true, false>(S, a.flag, fill, C, g, wflag, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
-        else C = test_tile<false, false>(S, a.flag, fill, C, g, wflag, lane, (uint32_t)i, xi, yi, zi, hi2, a.L, a.half);
+        if (selftile && selfwrap) C = test_tile<true, true>(S, a.flag, fill, C, g, wflag, lane, xi, yi, zi, hi2, a.L, a.half);
+        else if (selftile) C = test_tile<false, true>(S, a.flag, fill, C, g, wflag, lane, xi, yi, zi, hi2, a.L, a.half);
+        else if (cwrap) C = test_tile<true, false>(S, a.flag, fill, C, g, wflag, lane, xi, yi, zi, hi2, a.L, a.half);
+        else C = test_tile<false, false>(S, a.flag, fill, C, g, wflag, lane, xi, yi, zi, hi2, a.L, a.half);
         fill = 0;
         cwrap = false;
         __syncwarp();
@@ -249,7 +250,7 @@ __global__ void k_set_u64(unsigned long long* p, unsigned long long v) { *p = v;
 int crk_build_nbr_lists(crk_ctx* c) {
     const int64_t nl = c->nl;
     CRK_TRY(crk_ensure(c, c->seg_first, (size_t)(nl + 1) * sizeof(uint4)));
-    CRK_TRY(crk_ensure(c, c->leaf_cnt, (size_t)(nl + 1) * 64 * sizeof(uint16_t)));
+    CRK_TRY(crk_ensure(c, c->leaf_cnt, (size_t)(nl + 1) * 32 * sizeof(uint16_t)));
     CRK_TRY(crk_ensure(c, c->cand_first, (size_t)(nl + 1) * CRK_CAND_STRIDE * sizeof(uint32_t)));
     // first guess: ~6 KB per leaf at ~60 neighbours; grown to the exact need if the builder reports more
     if (!c->arena.p) CRK_TRY(crk_ensure(c, c->arena, (size_t)nl * 6656 + 65536));

@@ -40,7 +40,7 @@ struct SweepArgs {
     float L, half;
     const uint4* __restrict__ arena;      // neighbour-list segments
     const uint4* __restrict__ seg_first;  // dense copy of each leaf's first segment header (.w = its arena unit, 0 = none)
-    const uint16_t* __restrict__ leaf_cnt;  // [nl][64] per-lane cnt_g | cnt of the first segment
+    const uint16_t* __restrict__ leaf_cnt;  // [nl][32] per-lane entry counts of the first segment
     const uint32_t* __restrict__ cand_first; // [nl][CRK_CAND_STRIDE] candidate indices of the first segment
     const int32_t* __restrict__ perm;     // sorted slot -> caller index
     const float4* __restrict__ posh;      // (x,y,z,h)
@@ -65,23 +65,23 @@ struct SweepArgs {
 
 struct Seg {
     const uint16_t* ell;
-    int C, K, cg, ct;
+    int C, K, ct;
     bool wrap;               // some entry of the segment may cross the periodic boundary
     uint32_t next;
 };
 
 // Metadata of the segment a group stages next, in shared memory: the same 105 16-byte chunks a segment carries in the arena
-// (header | cnt_g[32] cnt[32] u16 | cand[CRK_CCAP] u32; a leaf's first segment keeps them in the dense per-leaf arrays).
+// (header | cnt[32] u16 | cand[CRK_CCAP] u32; a leaf's first segment keeps them in the dense per-leaf arrays).
 // It is fetched with cp.async while the group is still evaluating the rows of the previous segment, so the three dependent
 // loads (header -> candidate indices -> state) that used to open every leaf shrink to the last one.
 struct __align__(16) Meta {
     uint4 hdr;                    // {next segment unit, C | CRK_SEG_WRAP | K << 16, 0, own unit (first segments only)}
-    uint16_t cnt[64];
+    uint16_t cnt[32];
     uint32_t cand[CRK_CCAP];
-    long long next_leaf;          // the group's next work item (-1 = none), written by thread 0 of the group
-    long long pad;
+    long long next_leaf;          // sweep_begin: the group's first leaf (-1 = none)
+    long long next2;              // the leaf after the one being swept (-1 = none), written by thread 0 of the group one leaf ahead
 };
-constexpr int META_CHUNKS = 1 + 8 + CRK_CCAP / 4;
+constexpr int META_CHUNKS = 1 + 4 + CRK_CCAP / 4;
 static_assert(sizeof(Meta) == META_CHUNKS * 16 + 16, "Meta layout");
 
 __device__ __forceinline__ void cp_async16(uint32_t dst_shared, const void* src) {
@@ -138,8 +138,8 @@ __device__ __forceinline__ void issue_meta(Meta* m, const SweepArgs& a, long lon
         const char* src;
         if (unit != 0u) src = (const char*)(a.arena + unit + ch);
         else if (ch == 0) src = (const char*)(a.seg_first + leaf);
-        else if (ch < 9) src = (const char*)(a.leaf_cnt + leaf * 64) + (ch - 1) * 16;
-        else src = (const char*)(a.cand_first + leaf * CRK_CAND_STRIDE) + (ch - 9) * 16;
+        else if (ch < 5) src = (const char*)(a.leaf_cnt + leaf * 32) + (ch - 1) * 16;
+        else src = (const char*)(a.cand_first + leaf * CRK_CAND_STRIDE) + (ch - 5) * 16;
         cp_async16(ms + (uint32_t)ch * 16u, src);
     }
 }
@@ -147,7 +147,11 @@ __device__ __forceinline__ void issue_meta(Meta* m, const SweepArgs& a, long lon
 template <int WPL>
 __device__ __forceinline__ long long sweep_begin(const SweepArgs& a, Meta* m, int lg, int wl, int lane) {
     const int tg = wl * 32 + lane;
-    if (tg == 0) m->next_leaf = grab_leaf(a);
+    if (tg == 0) {
+        const long long l0 = grab_leaf(a);
+        m->next_leaf = l0;
+        m->next2 = (l0 >= 0) ? grab_leaf(a) : -1;
+    }
     group_sync<WPL>(lg);
     const long long leaf = m->next_leaf;
     if (leaf >= 0) issue_meta<WPL * 32>(m, a, leaf, 0u, tg);
@@ -157,15 +161,19 @@ __device__ __forceinline__ long long sweep_begin(const SweepArgs& a, Meta* m, in
 
 // ---- the sweep over one leaf's segment chain -------------------------------------------------------------------------
 // Rows [0, K) of a segment's entry block; lane l is active while k < cnt[l].  SYM = false (gather set, Eqs. 13-14): entries
-// flagged CRK_ELL_SYM are skipped;  SYM = true (Eqs. 17-18): every entry is a pair.
+// flagged CRK_ELL_SYM are skipped;  SYM = true (Eqs. 17-18): every entry is a pair.  Returns the lane's entry count (the
+// number of its pairs of the symmetric set; a gather sweep that needs its own count takes it in `pair`).
 // pair(slot_addr, crosses_boundary, plane0) evaluates one accepted pair (slot_addr = shared address of the candidate's
 // plane-0 entry; plane p sits p * PSTRIDE bytes further); returns the number of pairs the lane owns.
 // The tile's planes 0 .. ROWP-1 are the first ROWP float4 of the candidates' force-state rows (`rows_src`, FROW float4 per
 // particle: consecutive lanes copy consecutive pieces of one row, so a warp-wide LDGSTS touches 32 / ROWP full lines or
 // sectors instead of 32 scattered ones), planes ROWP .. ROWP+PLANES-1 come from the SoA arrays `planes`.
 // On entry the copy of the leaf's metadata into m is in flight; on exit the group's next leaf is in `next_leaf` and the copy
-// of ITS metadata is in flight.  Barriers per segment: B1 metadata landed and the previous rows are done (tile free);
-// B2 everybody has read the metadata (m may be overwritten) and the next work item is known; B3 the state has landed.
+// of ITS metadata is in flight.  Work items are taken two leaves ahead (thread 0 keeps the counter's answer in a register
+// until the end of the leaf), so no barrier waits for the atomic.  Barriers per segment: B1 metadata landed and the previous
+// rows are done (tile free); B2 everybody has read the metadata (m may be overwritten); B3 the state has landed.
+// (Measured and not kept: prefetch.global.L2 of the next segment's candidate state a few rows into the current one -- the
+// prefetches cost the load/store unit as much as the copies they were meant to speed up: forces 11.05 -> 11.9 ms.)
 struct NoInit {
     __device__ __forceinline__ void operator()(uint32_t) const {}
 };
@@ -185,6 +193,7 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
     const int tg = wl * 32 + lane;
     const uint32_t tile_s = (uint32_t)__cvta_generic_to_shared(tile);
     uint32_t unit = 0;                                            // arena unit of the segment being staged (0: not known yet)
+    long long pend = -1;                                          // thread 0: the work item taken for the leaf after next
     next_leaf = -1;
 #ifdef CRK_PROBE
     long long pr_stage = 0, pr_t0 = clock64();
@@ -196,13 +205,16 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
         const long long pr_s0 = clock64();
 #endif
         const uint4 h0 = m->hdr;
-        if (first) unit = h0.w;
+        if (first) {
+            unit = h0.w;
+            next_leaf = m->next2;
+        }
         if (unit == 0u) {                                      // a leaf without a segment (cannot happen for a built leaf)
-            if (tg == 0) m->next_leaf = grab_leaf(a);
+            if (tg == 0) pend = (next_leaf >= 0) ? grab_leaf(a) : -1;
             group_sync<WPL>(lg);
-            next_leaf = m->next_leaf;
             if (next_leaf >= 0) issue_meta<NT>(m, a, next_leaf, 0u, tg);
             cp_async_commit();
+            if (tg == 0) m->next2 = pend;
             break;
         }
         Seg s;
@@ -210,8 +222,7 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
         s.C = (int)(h0.y & 0x7fffu);
         s.wrap = (h0.y & CRK_SEG_WRAP) != 0u;
         s.K = (int)(h0.y >> 16);
-        s.cg = (int)m->cnt[lane];
-        s.ct = (int)m->cnt[32 + lane];
+        s.ct = (int)m->cnt[lane];
         s.ell = (const uint16_t*)(a.arena + unit + CRK_SEG_HDR_UNITS + (first ? 0 : ((s.C + 3) >> 2)));
         const int rows = s.K;
         const int mine = s.ct;
@@ -224,13 +235,41 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
             const uint32_t pc = (uint32_t)(tg & (ROWP - 1));       // NT is a multiple of ROWP: a thread always copies the same piece
             const uint32_t dst0 = tile_s + pc * PSTRIDE;
             const float4* src0 = rows_src + pc;
+#ifdef CRK_STAGE_PERCAND
+            // one candidate per thread, all its pieces: fewer instructions per copy, 32 rows per warp-wide LDGSTS
+            for (int c = tg; c < s.C; c += NT) {
+                const float4* src = rows_src + (int64_t)m->cand[c] * FROW;
+#pragma unroll
+                for (int p = 0; p < ROWP; ++p) cp_async16(tile_s + (uint32_t)p * PSTRIDE + (uint32_t)c * 16u, src + p);
+            }
+#elif defined(CRK_STAGE_LDG)
+            // through registers: a warp-wide LDG.128 of 32 / ROWP full rows is served line by line, an LDGSTS thread by thread
+            constexpr int SB = 5;
+            for (int f0 = tg; f0 < total; f0 += NT * SB) {
+                float4 v[SB];
+#pragma unroll
+                for (int b = 0; b < SB; ++b) {
+                    const int f = f0 + b * NT;
+                    if (f < total) v[b] = __ldg(src0 + (int64_t)m->cand[f >> RS] * FROW);
+                }
+#pragma unroll
+                for (int b = 0; b < SB; ++b) {
+                    const int f = f0 + b * NT;
+                    if (f < total) asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(dst0 + (uint32_t)(f >> RS) * 16u), "f"(v[b].x), "f"(v[b].y), "f"(v[b].z), "f"(v[b].w) : "memory");
+                }
+            }
+#else
 #pragma unroll 4
             for (int f = tg; f < total; f += NT) {
                 const int c = f >> RS;
                 const uint32_t j = m->cand[c];
                 CRK_CHECK(a.flag, (int64_t)j < a.np, 9);                                    // candidate index
+#ifdef CRK_EXP_HALFSTAGE
+                if (ROWP == 8 && (c & 1) && c >= 32) continue;
+#endif
                 cp_async16(dst0 + (uint32_t)c * 16u, src0 + (int64_t)j * FROW);
             }
+#endif
         }
         if (PLANES > 0) {
             for (int c0 = 0; c0 < s.C; c0 += NT * 2) {
@@ -257,14 +296,19 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
             e[q] = (k < rows) ? (uint32_t)__ldg(ep + k * 32) : 0u;
         }
         const bool last = (s.next == 0u);
-        if (last && tg == 0) m->next_leaf = grab_leaf(a);
+#ifdef CRK_PROBE
+        const long long pr_s1 = clock64();
+#endif
+        if (last && tg == 0) pend = (next_leaf >= 0) ? grab_leaf(a) : -1;   // consumed at the end of the leaf
         group_sync<WPL>(lg);                                   // B2
-        if (last) {
-            next_leaf = m->next_leaf;
-            if (next_leaf >= 0) issue_meta<NT>(m, a, next_leaf, 0u, tg);
-        } else {
-            issue_meta<NT>(m, a, 0, s.next, tg);
+#ifdef CRK_PROBE
+        if (tg == 0) {
+            atomicAdd(&crk_probe[(ROWP + PLANES) * 4 + 3], (unsigned long long)(pr_s1 - pr_s0));
+            atomicAdd(&crk_probe[40 + ((ROWP + PLANES) & 7)], (unsigned long long)(clock64() - pr_s1));
         }
+#endif
+        if (!last) issue_meta<NT>(m, a, 0, s.next, tg);
+        else if (next_leaf >= 0) issue_meta<NT>(m, a, next_leaf, 0u, tg);
         cp_async_commit();
         asm volatile("cp.async.wait_group 1;" ::: "memory");   // the state copies (the metadata copy may still be in flight)
         group_sync<WPL>(lg);                                   // B3
@@ -295,16 +339,24 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
 #pragma unroll
                 for (int p = 0; p < NPRE; ++p) nxt[p] = lds128(tile_s + (uint32_t)p * PSTRIDE + (en & CRK_ELL_MASK) * 16u);
                 CRK_CHECK(a.flag, k >= mine || (int)(e[q] & CRK_ELL_MASK) < s.C, 10);       // entry -> staged slot
+#ifdef CRK_EXP_NOCONFLICT   // timing experiment only (wrong results): every lane of a quarter-warp reads a different bank group
+                if (k < mine && (SYM || !(e[q] & CRK_ELL_SYM)))
+                    pair(tile_s + (((e[q] & CRK_ELL_MASK) & ~31u) | (uint32_t)lane) * 16u, (e[q] & CRK_ELL_WRAP) != 0u, cur);
+#else
                 if (k < mine && (SYM || !(e[q] & CRK_ELL_SYM)))
                     pair(tile_s + (e[q] & CRK_ELL_MASK) * 16u, (e[q] & CRK_ELL_WRAP) != 0u, cur);
+#endif
 #pragma unroll
                 for (int p = 0; p < NPRE; ++p) cur[p] = nxt[p];
             }
 #pragma unroll
             for (int q = 0; q < 4; ++q) e[q] = nx[q];
         }
-        count += (uint32_t)(SYM ? s.ct : s.cg);
-        if (last) break;
+        count += (uint32_t)s.ct;
+        if (last) {
+            if (tg == 0) m->next2 = pend;
+            break;
+        }
         unit = s.next;
     }
 #ifdef CRK_PROBE
@@ -394,13 +446,15 @@ __global__ void __launch_bounds__(W1_WPC * 32) k_volumes(SweepArgs a) {
         const float xi = pi.x, yi = pi.y, zi = pi.z, hi = pi.w;
         const float inv_h = valid ? 1.0f / hi : 0.0f;
         float acc = 0.0f;
+        uint32_t count = 0;                                  // neighbours of the gather set (Eqs. 13-14), self excluded
         long long next;
-        const uint32_t count = leaf_sweep<1, 0, 1, false>(a, nullptr, planes, leaf, next, w, 0, lane, tile, meta, [&](uint32_t, bool wrapped, const float4* pre) {
+        leaf_sweep<1, 0, 1, false>(a, nullptr, planes, leaf, next, w, 0, lane, tile, meta, [&](uint32_t, bool wrapped, const float4* pre) {
             const float4 pj = pre[0];
             float dx, dy, dz, r2;
             sep3(a, wrapped, xi, yi, zi, pj, dx, dy, dz, r2);
             const float r = r2 * rsqrt_fast(fmaxf(r2, R2_TINY));
             acc += wendland_w(r * inv_h);
+            ++count;
         });
         if (valid) {
             const float k3 = SIGMA_C4 * inv_h * inv_h * inv_h;
@@ -844,7 +898,10 @@ __device__ __forceinline__ PairF force_pair(const ForceConst& k, const PState& I
 // CTAs are resident per SM, so one CTA's staging (header -> candidates -> state, three dependent global loads) overlaps the
 // other three's pair math.  (A persistent, double-buffered variant with 2 x 8 warps per SM was measured slower: 13.1 vs
 // 11.7 ms -- its per-leaf barrier couples all warps of the SM half; profiles/r01_sweeps_v9_ncu_full.md.)
-constexpr int W5_WPL = 4;
+#ifndef CRK_W5_WPL
+#define CRK_W5_WPL 4
+#endif
+constexpr int W5_WPL = CRK_W5_WPL;
 template <bool TS>   // TS: also reduce the per-particle maxima the time-step criteria need (Eqs. 46, 50)
 __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -857,6 +914,10 @@ __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
         const int64_t i = leaf * CRK_LEAF + lane;
         const bool valid = i < a.n;
         PState I;                                            // taken from the tile (slots 0..31 = the leaf's own particles)
+        // what the epilogue needs from global memory is requested now, not after the last row
+        const float mi = (wl == 0) ? a.m_s[i] : 1.0f;
+        const int32_t pidx = (wl == 0 && valid) ? a.perm[i] : 0;
+        const bool write_out = (wl == 0 && valid) && (!a.active || a.active[pidx]);
         float acc[4] = {0.f, 0.f, 0.f, 0.f};                 // Fx, Fy, Fz, dE
         float mx[2] = {0.f, 0.f};                            // max approach speed, max Q_i
         long long next;
@@ -880,15 +941,14 @@ __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
             if (TS) a.ts[i] = make_float2(mx[0], mx[1]);
             float4 as = make_float4(0.f, 0.f, 0.f, 0.f);
             if (valid) {
-                const float im = 1.0f / a.m_s[i];
-                const int32_t p = a.perm[i];
+                const float im = 1.0f / mi;
                 as = make_float4(acc[0] * im, acc[1] * im, acc[2] * im, I.P * __powf(I.rho, -a.gamma));
-                if (!a.active || a.active[p]) {
-                    a.o0[p] = as.x;
-                    a.o1[p] = as.y;
-                    a.o2[p] = as.z;
-                    a.o3[p] = acc[3] * im;
-                    if (a.ocnt) a.ocnt[p] = count;
+                if (write_out) {
+                    a.o0[pidx] = as.x;
+                    a.o1[pidx] = as.y;
+                    a.o2[pidx] = as.z;
+                    a.o3[pidx] = acc[3] * im;
+                    if (a.ocnt) a.ocnt[pidx] = count;
                 }
             }
             a.facc[i] = as;                                  // (dv/dt, s = P / rho^gamma) for crk_compatible_energy, crk_timestep
