@@ -124,12 +124,14 @@ __device__ __forceinline__ void group_sync(int lg) {
 // A group (WPL warps) serves one leaf at a time and keeps taking leaves from a global counter until none is left; the
 // kernels are launched with as many CTAs as are resident at once.  (One CTA per leaf cost the force sweep 19 % of its time
 // in CTA turnover and 27 % in the dependent loads of the prologue -- measured with clock64 probes, profiles/r02_notes.md.)
-__device__ __forceinline__ long long grab_leaf(const SweepArgs& a) {
+// the counter's answer is only looked at (resolve_slot) when the leaf is needed, one leaf later: no thread waits for the atomic
+__device__ __forceinline__ unsigned int grab_slot(const SweepArgs& a) { return atomicAdd(a.sched, 1u); }
+__device__ __forceinline__ long long resolve_slot(const SweepArgs& a, unsigned int slot) {
     const long long total = a.ids ? a.n_ids : a.nl;
-    const long long slot = (long long)atomicAdd(a.sched, 1u);
-    if (slot >= total) return -1;
-    return a.ids ? (long long)a.ids[slot] : slot;
+    if ((long long)slot >= total) return -1;
+    return a.ids ? (long long)a.ids[slot] : (long long)slot;
 }
+__device__ __forceinline__ long long grab_leaf(const SweepArgs& a) { return resolve_slot(a, grab_slot(a)); }
 // copies the metadata of a leaf's first segment (unit == 0) or of the arena segment `unit` into m; the caller commits
 template <int NT>
 __device__ __forceinline__ void issue_meta(Meta* m, const SweepArgs& a, long long leaf, uint32_t unit, int tg) {
@@ -177,15 +179,20 @@ __device__ __forceinline__ long long sweep_begin(const SweepArgs& a, Meta* m, in
 struct NoInit {
     __device__ __forceinline__ void operator()(uint32_t) const {}
 };
+struct NoHook {
+    __device__ __forceinline__ void operator()() const {}
+};
 // init(tile_s) runs once, after the first segment is staged: slots 0..31 of that tile are the leaf's own particles in lane
 // order (lists.cu), so a sweep can take its i-state from there instead of loading it from global memory.
 // (Measured and not kept, profiles/r02_notes.md: a second, branch-free instantiation of the row loop for segments without
 // boundary-crossing entries -- 172 instead of 190 instructions per pair of k_forces, but ptxas then sinks the shared loads
 // next to their uses and the sweep loses 1.6 ms to short-scoreboard stalls.)
-template <int WPL, int ROWP, int PLANES, bool SYM, int NPRE = 1, typename Pair, typename Init = NoInit>
+// staged() runs once per leaf between the issue of the first segment's copies and B2, i.e. while the copies are in flight and
+// the group has nothing else to do: the place for work that does not need the tile (the previous leaf's epilogue).
+template <int WPL, int ROWP, int PLANES, bool SYM, int NPRE = 1, typename Pair, typename Init = NoInit, typename Hook = NoHook>
 __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4* __restrict__ rows_src, const float4* const* planes,
                                                long long leaf, long long& next_leaf, int lg, int wl, int lane, float4* tile, Meta* m,
-                                               Pair pair, Init init = Init()) {
+                                               Pair pair, Init init = Init(), Hook staged = Hook()) {
     static_assert(ROWP == 0 || ROWP == 2 || ROWP == 8, "row pieces per candidate");
     constexpr int NT = WPL * 32;                                  // threads that serve the leaf
     uint32_t count = 0;
@@ -193,7 +200,7 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
     const int tg = wl * 32 + lane;
     const uint32_t tile_s = (uint32_t)__cvta_generic_to_shared(tile);
     uint32_t unit = 0;                                            // arena unit of the segment being staged (0: not known yet)
-    long long pend = -1;                                          // thread 0: the work item taken for the leaf after next
+    unsigned int pend = 0xffffffffu;                              // thread 0: the work item taken for the leaf after next (raw counter value)
     next_leaf = -1;
 #ifdef CRK_PROBE
     long long pr_stage = 0, pr_t0 = clock64();
@@ -210,11 +217,11 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
             next_leaf = m->next2;
         }
         if (unit == 0u) {                                      // a leaf without a segment (cannot happen for a built leaf)
-            if (tg == 0) pend = (next_leaf >= 0) ? grab_leaf(a) : -1;
+            if (tg == 0 && next_leaf >= 0) pend = grab_slot(a);
             group_sync<WPL>(lg);
             if (next_leaf >= 0) issue_meta<NT>(m, a, next_leaf, 0u, tg);
             cp_async_commit();
-            if (tg == 0) m->next2 = pend;
+            if (tg == 0) m->next2 = (next_leaf >= 0) ? resolve_slot(a, pend) : -1;
             break;
         }
         Seg s;
@@ -296,10 +303,11 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
             e[q] = (k < rows) ? (uint32_t)__ldg(ep + k * 32) : 0u;
         }
         const bool last = (s.next == 0u);
+        if (first) staged();
 #ifdef CRK_PROBE
         const long long pr_s1 = clock64();
 #endif
-        if (last && tg == 0) pend = (next_leaf >= 0) ? grab_leaf(a) : -1;   // consumed at the end of the leaf
+        if (last && tg == 0 && next_leaf >= 0) pend = grab_slot(a);          // looked at when the leaf ends
         group_sync<WPL>(lg);                                   // B2
 #ifdef CRK_PROBE
         if (tg == 0) {
@@ -354,7 +362,7 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
         }
         count += (uint32_t)s.ct;
         if (last) {
-            if (tg == 0) m->next2 = pend;
+            if (tg == 0) m->next2 = (next_leaf >= 0) ? resolve_slot(a, pend) : -1;
             break;
         }
         unit = s.next;
@@ -902,13 +910,58 @@ __device__ __forceinline__ PairF force_pair(const ForceConst& k, const PState& I
 #define CRK_W5_WPL 4
 #endif
 constexpr int W5_WPL = CRK_W5_WPL;
+// The epilogue of a leaf (sum of the W5_WPL partial results in warp order, division by the mass, stores through the
+// permutation) is deferred into the staging window of the group's NEXT leaf, where the warps only wait for their copies: the
+// partial sums and what the stores need travel through this record.  One record is enough: nobody reaches the rows of leaf
+// n + 1 (and so the next write of the record) before the warp that runs epilogue(n) has passed B2 of leaf n + 1.
+template <bool TS>
+struct ForceEpi {
+    float part[W5_WPL][TS ? 6 : 4][32];      // Fx, Fy, Fz, dE (, max approach speed, max Q_i) of warp w
+    float s[32], invm[32];                   // s = P / rho^gamma, 1 / m
+    int32_t pidx[32];                        // caller index of the particle, -1: outputs not wanted (passive or padding)
+    uint32_t cnt[32];
+    long long leaf;                          // -1: nothing pending
+    long long pad;
+};
+template <bool TS>
+__device__ __forceinline__ void force_epilogue(const SweepArgs& a, const ForceEpi<TS>* ep, int lane) {
+    const long long leaf = ep->leaf;
+    if (leaf < 0) return;
+    const int64_t i = leaf * CRK_LEAF + lane;
+    float acc[TS ? 6 : 4];
+#pragma unroll
+    for (int q = 0; q < (TS ? 6 : 4); ++q) acc[q] = ep->part[0][q][lane];
+    for (int w2 = 1; w2 < W5_WPL; ++w2) {
+#pragma unroll
+        for (int q = 0; q < 4; ++q) acc[q] += ep->part[w2][q][lane];
+        if (TS) {
+            acc[4] = fmaxf(acc[4], ep->part[w2][4][lane]);
+            acc[5] = fmaxf(acc[5], ep->part[w2][5][lane]);
+        }
+    }
+    if (TS) a.ts[i] = make_float2(acc[4], acc[5]);
+    const float im = ep->invm[lane];
+    const float4 as = make_float4(acc[0] * im, acc[1] * im, acc[2] * im, ep->s[lane]);
+    const int32_t p = ep->pidx[lane];
+    if (p >= 0) {
+        a.o0[p] = as.x;
+        a.o1[p] = as.y;
+        a.o2[p] = as.z;
+        a.o3[p] = acc[3] * im;
+        if (a.ocnt) a.ocnt[p] = ep->cnt[lane];
+    }
+    a.facc[i] = as;                                      // (dv/dt, s = P / rho^gamma) for crk_compatible_energy, crk_timestep
+}
+
 template <bool TS>   // TS: also reduce the per-particle maxima the time-step criteria need (Eqs. 46, 50)
 __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     const int lane = threadIdx.x & 31, wl = threadIdx.x >> 5;
     float4* tile = (float4*)smem_raw;
     Meta* meta = (Meta*)(smem_raw + FROW * PSTRIDE);
+    ForceEpi<TS>* epi = (ForceEpi<TS>*)(smem_raw + FROW * PSTRIDE + sizeof(Meta));
     const ForceConst fc = {a.L, a.half, 1.0f / a.n_h, a.n_h / 0.2f, a.eps2, a.C_l, a.C_q, a.gamma, a.n_h};
+    if (threadIdx.x == 0) epi->leaf = -1;
     long long leaf = sweep_begin<W5_WPL>(a, meta, 0, wl, lane);
     while (leaf >= 0) {
         const int64_t i = leaf * CRK_LEAF + lane;
@@ -934,27 +987,26 @@ __global__ void __launch_bounds__(W5_WPL * 32, 4) k_forces(SweepArgs a) {
 #pragma unroll
             for (int p = 0; p < FPRE; ++p) pre[p] = lds128(ts + (uint32_t)p * PSTRIDE + (uint32_t)lane * 16u);
             I = load_pstate_shared(fc, ts + (uint32_t)lane * 16u, pre);
+        }, [&]() {
+            if (wl == W5_WPL - 1) force_epilogue<TS>(a, epi, lane);      // of the previous leaf (its record was complete at B1)
         });
-        group_reduce<W5_WPL, 4>(acc, 0, wl, lane, (float*)tile);
-        if (TS) group_reduce<W5_WPL, 2, true>(mx, 0, wl, lane, (float*)tile);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) epi->part[wl][q][lane] = acc[q];
+        if (TS) {
+            epi->part[wl][4][lane] = mx[0];
+            epi->part[wl][5][lane] = mx[1];
+        }
         if (wl == 0) {
-            if (TS) a.ts[i] = make_float2(mx[0], mx[1]);
-            float4 as = make_float4(0.f, 0.f, 0.f, 0.f);
-            if (valid) {
-                const float im = 1.0f / mi;
-                as = make_float4(acc[0] * im, acc[1] * im, acc[2] * im, I.P * __powf(I.rho, -a.gamma));
-                if (write_out) {
-                    a.o0[pidx] = as.x;
-                    a.o1[pidx] = as.y;
-                    a.o2[pidx] = as.z;
-                    a.o3[pidx] = acc[3] * im;
-                    if (a.ocnt) a.ocnt[pidx] = count;
-                }
-            }
-            a.facc[i] = as;                                  // (dv/dt, s = P / rho^gamma) for crk_compatible_energy, crk_timestep
+            epi->s[lane] = valid ? I.P * __powf(I.rho, -a.gamma) : 0.0f;
+            epi->invm[lane] = valid ? 1.0f / mi : 0.0f;
+            epi->pidx[lane] = write_out ? pidx : -1;
+            epi->cnt[lane] = count;
+            if (lane == 0) epi->leaf = leaf;
         }
         leaf = next;
     }
+    group_sync<W5_WPL>(0);
+    if (wl == W5_WPL - 1) force_epilogue<TS>(a, epi, lane);
 }
 
 // ================================================================================ NEXT row 1: compatible energy update
@@ -1140,9 +1192,10 @@ int crk_launch_forces(crk_ctx* c, float* ax, float* ay, float* az, float* dudt, 
     const int64_t items = ids ? n_ids : c->nl;
     if (items == 0) return CRK_OK;
     a.o0 = ax; a.o1 = ay; a.o2 = az; a.o3 = dudt; a.ocnt = pair_count;
-    const int smem = FROW * (int)PSTRIDE + (int)sizeof(Meta);
+    const bool ts_on = (c->prm.flags & CRK_FLAG_TIMESTEP) != 0;
+    const int smem = FROW * (int)PSTRIDE + (int)sizeof(Meta) + (int)(ts_on ? sizeof(ForceEpi<true>) : sizeof(ForceEpi<false>));
     unsigned grid = 0;
-    if (c->prm.flags & CRK_FLAG_TIMESTEP) {
+    if (ts_on) {
         CRK_TRY(crk_ensure(c, c->ts_s, (size_t)np * sizeof(float2)));
         a.ts = (float2*)c->ts_s.p;
         CRK_TRY(persistent_grid(c, k_forces<true>, W5_WPL * 32, smem, 1, items, &grid));
