@@ -374,6 +374,7 @@ def run_ours(args, rank, world, local_rank):
     value = pairs_all / (ms_per_step * 1e-3)
     peaks, peak_kind = load_peaks()
     fp32_meas, _ = crk_measure_fp32_peak(5)
+    fp32_3reg, _ = crk_measure_fp32_peak(5, three_reg=True)
     forces_ms = st["ms_forces"]
     forces_flops = FLOPS_PER_PAIR["forces"] * sym_pairs
     achieved = forces_flops / (forces_ms * 1e-3) / 1e12 if forces_ms > 0 else None
@@ -391,12 +392,18 @@ def run_ours(args, rank, world, local_rank):
                 "peak_measured": fp32_meas / 1e12,
                 "frac_vs_peak_measured": (achieved / (fp32_meas / 1e12)) if achieved and fp32_meas > 0 else None,
                 "peak_measured_source": "crk_measure_fp32_peak: register-resident FFMA chains on every SM, this run",
+                "peak_measured_3reg": fp32_3reg / 1e12,
+                "frac_vs_peak_measured_3reg": (achieved / (fp32_3reg / 1e12)) if achieved and fp32_3reg > 0 else None,
+                "peak_measured_3reg_source": "crk_measure_fp32_peak_3reg: the same loop with three register operands per FFMA "
+                                             "(a = b*c + a, the form of every accumulated pair sum): the register file feeds it at "
+                                             "~61 % of the nominal rate (DESIGN.md section 5.4)",
                 "flops_per_pair": FLOPS_PER_PAIR["forces"], "pairs_per_launch": sym_pairs, "kernel_ms": forces_ms,
                 "traffic": (kf["dram_bytes_read"] + kf["dram_bytes_write"]) if kf else None,
                 "traffic_unit": "bytes per launch (ncu dram__bytes_read.sum + dram__bytes_write.sum; algorithmic minimum 144 B j-state + 16 B outputs per particle)",
                 "traffic_source": (os.path.relpath(NCU_SUMMARY, ROOT) + " <- " + ncu.get("source", "?")) if kf else None,
                 "ncu_fma_pipe_pct": {k: v.get("fma_pipe_pct") for k, v in ncu["kernels"].items()} if ncu else None}
     passes = {k: st[k] for k in ("ms_sort", "ms_tree", "ms_lists", "ms_volumes", "ms_rk", "ms_gradv", "ms_forces")}
+    passes["ms_hydro_prep"] = max(st["ms_hydro"] - st["ms_forces"] - st["ms_gradv"], 0.0)   # pack + permute v, u into the state rows
     alg_flops = (FLOPS_PER_PAIR["volumes"] + FLOPS_PER_PAIR["moments"] + FLOPS_PER_PAIR["gradv"]) * gather_pairs + forces_flops
     sweeps_ms = st["ms_volumes"] + st["ms_rk"] + st["ms_gradv"] + st["ms_forces"]
     sort_bytes = ps.n * (st["sort_passes"] * 32.0 + 16 + 12 + 32 + 16)    # radix passes + pack + gather

@@ -183,6 +183,10 @@ int64_t crk_get_leaf_list(crk_ctx* c, int64_t leaf, uint32_t* host_buf, int64_t 
 /* Measurement aid (not part of the method): runs a register-resident FFMA loop on every SM and returns the achieved
  * FP32 rate in flop/s (FMA = 2 flops) for bench.py's roofline denominator; *ms_out receives the kernel time.  */
 double crk_measure_fp32_peak(void* cuda_stream, int repeats, float* ms_out);
+/* The same loop with three register operands per FFMA (a = b * c + a, the form of every accumulated pair sum).  On B200 the
+ * register file feeds such a stream at about 61 % of the rate of the forms with at most two register operands, so this is
+ * the rate the accumulating part of the pair sweeps can reach; reported by bench.py beside the nominal peak.  */
+double crk_measure_fp32_peak_3reg(void* cuda_stream, int repeats, float* ms_out);
 
 #ifdef __cplusplus
 }

@@ -12,7 +12,7 @@ _LIB_PATH = os.environ.get("CRK_LIB") or os.path.join(_HERE, "libcrk.so")   # CR
 EXPORTED_SYMBOLS = (
     "crk_create", "crk_destroy", "crk_build_cells", "crk_volumes", "crk_rk_coefficients", "crk_hydro_derivs",
     "crk_step_derivs", "crk_step_derivs_host", "crk_hydro_derivs_active", "crk_compatible_energy", "crk_evolve_h", "crk_timestep", "crk_kdk_step", "crk_last_error", "crk_get_perm", "crk_get_gradv", "crk_get_leaf_segments", "crk_get_stats",
-    "crk_reset_stats", "crk_set_timing", "crk_get_leaf_list", "crk_measure_fp32_peak",
+    "crk_reset_stats", "crk_set_timing", "crk_get_leaf_list", "crk_measure_fp32_peak", "crk_measure_fp32_peak_3reg",
 )
 
 _ERR = {0: "CRK_OK", -1: "CRK_EINVAL", -2: "CRK_ERANGE", -3: "CRK_ENOMEM", -4: "CRK_ECUDA", -5: "CRK_ESTATE"}
@@ -86,6 +86,8 @@ def _load():
     L.crk_get_leaf_list.restype = i64
     L.crk_measure_fp32_peak.argtypes = [vp, C.c_int, C.POINTER(C.c_float)]
     L.crk_measure_fp32_peak.restype = C.c_double
+    L.crk_measure_fp32_peak_3reg.argtypes = [vp, C.c_int, C.POINTER(C.c_float)]
+    L.crk_measure_fp32_peak_3reg.restype = C.c_double
     _lib = L
     return L
 
@@ -299,8 +301,10 @@ def crk_step_derivs_host(ctx: Crk, x, y, z, h, vx, vy, vz, m, u, out):
     return ctx.step_derivs_host(x, y, z, h, vx, vy, vz, m, u, out)
 
 
-def crk_measure_fp32_peak(repeats=5):
+def crk_measure_fp32_peak(repeats=5, three_reg=False):
+    """achieved FP32 rate (flop/s) of a register-resident FFMA loop; three_reg: a = b * c + a with three register operands"""
     L = _load()
     ms = C.c_float()
-    f = L.crk_measure_fp32_peak(C.c_void_p(torch.cuda.current_stream().cuda_stream), int(repeats), C.byref(ms))
+    fn = L.crk_measure_fp32_peak_3reg if three_reg else L.crk_measure_fp32_peak
+    f = fn(C.c_void_p(torch.cuda.current_stream().cuda_stream), int(repeats), C.byref(ms))
     return float(f), float(ms.value)
