@@ -1104,15 +1104,22 @@ SweepArgs make_args(crk_ctx* c) {
 // work items; the work counter is zeroed on the stream first.  groups_per_cta = leaves a CTA serves concurrently.
 template <typename K>
 int persistent_grid(crk_ctx* c, K kernel, int threads, int smem, int groups_per_cta, int64_t items, unsigned* grid) {
-    if (smem > 48 * 1024) CRK_CUDA(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    int per_sm = 0, dev = 0, sms = 0;
-    CRK_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, (size_t)smem));
-    CRK_CUDA(c, cudaGetDevice(&dev));
-    CRK_CUDA(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    if (per_sm < 1) {
-        snprintf(c->err, sizeof(c->err), "a sweep kernel does not fit on an SM (%d bytes of shared memory)", smem);
-        return CRK_ECUDA;
+    // occupancy and SM count of a (kernel, shared-memory size) are asked for once per process, not once per launch
+    struct Geo { int smem = -1, per_sm = 0, sms = 0; };
+    static Geo geo;                                       // one instance per kernel (template instantiation)
+    if (geo.smem != smem) {
+        if (smem > 48 * 1024) CRK_CUDA(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        int per_sm = 0, dev = 0, sms = 0;
+        CRK_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, (size_t)smem));
+        CRK_CUDA(c, cudaGetDevice(&dev));
+        CRK_CUDA(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        if (per_sm < 1) {
+            snprintf(c->err, sizeof(c->err), "a sweep kernel does not fit on an SM (%d bytes of shared memory)", smem);
+            return CRK_ECUDA;
+        }
+        geo.smem = smem; geo.per_sm = per_sm; geo.sms = sms;
     }
+    const int per_sm = geo.per_sm, sms = geo.sms;
     const int64_t need = (items + groups_per_cta - 1) / groups_per_cta;
     const int64_t res = (int64_t)per_sm * sms;
     *grid = (unsigned)(need < res ? need : res);
