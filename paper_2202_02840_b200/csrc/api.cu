@@ -90,7 +90,7 @@ void crk_destroy(crk_ctx* c) {
     DevBuf* bufs[] = {&c->keys[0], &c->keys[1], &c->vals[0], &c->vals[1], &c->hist, &c->scan_tmp, &c->posh_orig,
                       &c->posh, &c->leaf_lo, &c->leaf_hi, &c->nbr_cnt, &c->nbr_off, &c->nbr_list, &c->nbr_gcnt,
                       &c->posV, &c->rho_s, &c->coef, &c->fst, &c->u_s, &c->vel_orig, &c->m_s, &c->flag,
-                      &c->host_stage, &c->arena, &c->seg_first, &c->leaf_cnt, &c->cand_first, &c->act_flags, &c->act_offs, &c->act_ids, &c->ts_s, &c->kdk, &c->kick, &c->sched, &c->facc};
+                      &c->host_stage, &c->arena, &c->seg_first, &c->leaf_cnt, &c->cand_first, &c->act_flags, &c->act_offs, &c->act_ids, &c->ts_s, &c->kdk, &c->kick, &c->sched, &c->facc, &c->xv};
     for (DevBuf* b : bufs)
         if (b->p) cudaFree(b->p);
     if (c->h_flag) cudaFreeHost(c->h_flag);

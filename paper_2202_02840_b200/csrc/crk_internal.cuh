@@ -113,6 +113,7 @@ struct crk_ctx {
     DevBuf rho_s;                  // float
     DevBuf coef;                   // 4 planes float4[n]: (A,Bx,By,Bz) (cx,cy,cz,M00) (M01,M02,M10,M11) (M12,M20,M21,M22)
     DevBuf fst;                    // force-sweep state, one 128-byte row per particle (layout at k_rk in pairs.cu)
+    DevBuf xv;                     // float4[2] per particle: (x,y,z,1/h) (vx,vy,vz,V), written by the hydro preparation
     DevBuf facc;                   // float4 (dv/dt, s = P / rho^gamma) per particle, sorted, written by k_forces
     DevBuf ts_s;                   // float2 (max approach speed, max Q_i), sorted; only with CRK_FLAG_TIMESTEP
     DevBuf kick;                   // compatible-energy sweep: (v' - v, s) per particle, sorted

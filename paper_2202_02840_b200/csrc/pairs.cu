@@ -48,6 +48,7 @@ struct SweepArgs {
     float4* __restrict__ coef;            // 4 planes, stride np: (A,B) (c,M0) (M1..M4) (M5..M8)
     float4* __restrict__ fst;             // force-sweep state, one row of FROW float4 per particle (layout at k_rk)
     float4* __restrict__ facc;            // (dv/dt, s = P / rho^gamma) per particle, written by k_forces
+    float4* __restrict__ xv;              // (x,y,z,1/h) (vx,vy,vz,V) per particle, 32 bytes: what the grad v sweep stages
     float* __restrict__ rho_s;
     const float* __restrict__ m_s;
     int64_t np;                           // padded particle count nl*32 (plane stride)
@@ -194,6 +195,7 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
                                                long long leaf, long long& next_leaf, int lg, int wl, int lane, float4* tile, Meta* m,
                                                Pair pair, Init init = Init(), Hook staged = Hook()) {
     static_assert(ROWP == 0 || ROWP == 2 || ROWP == 8, "row pieces per candidate");
+    constexpr int RSTRIDE = ROWP;   // float4 per source row: the compact (x,y,z,1/h)(v,V) array (2) or the full state rows (8 = FROW)
     constexpr int NT = WPL * 32;                                  // threads that serve the leaf
     uint32_t count = 0;
     bool first = true;
@@ -245,7 +247,7 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
 #ifdef CRK_STAGE_PERCAND
             // one candidate per thread, all its pieces: fewer instructions per copy, 32 rows per warp-wide LDGSTS
             for (int c = tg; c < s.C; c += NT) {
-                const float4* src = rows_src + (int64_t)m->cand[c] * FROW;
+                const float4* src = rows_src + (int64_t)m->cand[c] * RSTRIDE;
 #pragma unroll
                 for (int p = 0; p < ROWP; ++p) cp_async16(tile_s + (uint32_t)p * PSTRIDE + (uint32_t)c * 16u, src + p);
             }
@@ -257,7 +259,7 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
 #pragma unroll
                 for (int b = 0; b < SB; ++b) {
                     const int f = f0 + b * NT;
-                    if (f < total) v[b] = __ldg(src0 + (int64_t)m->cand[f >> RS] * FROW);
+                    if (f < total) v[b] = __ldg(src0 + (int64_t)m->cand[f >> RS] * RSTRIDE);
                 }
 #pragma unroll
                 for (int b = 0; b < SB; ++b) {
@@ -274,7 +276,7 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
 #ifdef CRK_EXP_HALFSTAGE
                 if (ROWP == 8 && (c & 1) && c >= 32) continue;
 #endif
-                cp_async16(dst0 + (uint32_t)c * 16u, src0 + (int64_t)j * FROW);
+                cp_async16(dst0 + (uint32_t)c * 16u, src0 + (int64_t)j * RSTRIDE);
             }
 #endif
         }
@@ -497,12 +499,12 @@ __global__ void __launch_bounds__(256) k_hydro_prep(SweepArgs a, const float4* _
     const float4 ph = a.posh[k];
     if (k < a.n) {
         const float4 v = vel_orig[a.perm[k]];
-        a.fst[k * FROW] = make_float4(ph.x, ph.y, ph.z, 1.0f / ph.w);
-        a.fst[k * FROW + 1] = make_float4(v.x, v.y, v.z, a.posV[k].w);
+        a.xv[k * 2] = make_float4(ph.x, ph.y, ph.z, 1.0f / ph.w);
+        a.xv[k * 2 + 1] = make_float4(v.x, v.y, v.z, a.posV[k].w);
         u_s[k] = v.w;
     } else {
-        a.fst[k * FROW] = make_float4(ph.x, ph.y, ph.z, 0.0f);
-        a.fst[k * FROW + 1] = make_float4(0, 0, 0, 0);
+        a.xv[k * 2] = make_float4(ph.x, ph.y, ph.z, 0.0f);
+        a.xv[k * 2 + 1] = make_float4(0, 0, 0, 0);
         u_s[k] = 0.0f;
     }
 }
@@ -573,8 +575,8 @@ template <bool MOM, bool GV>
 __global__ void __launch_bounds__(W2_WPC * 32, (MOM && GV) ? CRK_RK_MINB : (GV ? 8 : 10))
 k_rk(SweepArgs a, const float* __restrict__ u_s, float* __restrict__ gv_full) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    // tile: GV -> the first two pieces of the candidates' force-state rows, (x,y,z,1/h) and (vx,vy,vz,V): one 32-byte sector
-    // each; moments only (crk_rk_coefficients, before the hydro preparation) -> the SoA plane (x,y,z,V)
+    // tile: GV -> the candidates' entries of the compact array xv, (x,y,z,1/h) and (vx,vy,vz,V): one 32-byte sector each;
+    // moments only (crk_rk_coefficients, before the hydro preparation) -> the SoA plane (x,y,z,V)
     constexpr int PL = GV ? 2 : 1;
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     constexpr int WSMEM = PL * (int)PSTRIDE + (int)sizeof(Meta);     // per warp
@@ -590,7 +592,7 @@ k_rk(SweepArgs a, const float* __restrict__ u_s, float* __restrict__ gv_full) {
         const float xi = ph.x, yi = ph.y, zi = ph.z, hi = ph.w;
         const float inv_h = valid ? 1.0f / hi : 0.0f;
         float4 vi = make_float4(0.f, 0.f, 0.f, 0.f);
-        if (GV) vi = a.fst[i * FROW + 1];
+        if (GV) vi = a.xv[i * 2 + 1];
         // moment accumulators: s0; s1[3]; s2[6] (xx,xy,xz,yy,yz,zz); t0[3]; t1[6]; t2[10] (xxx,xxy,xxz,xyy,xyz,xzz,yyy,yyz,yzz,zzz)
         float s0 = 0.f, s1[3] = {0.f, 0.f, 0.f}, s2[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
         float t0[3] = {0.f, 0.f, 0.f}, t1[6] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f}, t2[10] = {0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f};
@@ -604,7 +606,7 @@ k_rk(SweepArgs a, const float* __restrict__ u_s, float* __restrict__ gv_full) {
 #pragma unroll
             for (int r = 0; r < 6; ++r) T2[q][r] = 0.f;
         }
-        leaf_sweep<1, GV ? 2 : 0, GV ? 0 : 1, false>(a, a.fst, planes, leaf, next, w, 0, lane, tile, meta, [&](uint32_t sa, bool wrapped, const float4* pre) {
+        leaf_sweep<1, GV ? 2 : 0, GV ? 0 : 1, false>(a, a.xv, planes, leaf, next, w, 0, lane, tile, meta, [&](uint32_t sa, bool wrapped, const float4* pre) {
             const float4 pj = pre[0];
             float4 vj = make_float4(0.f, 0.f, 0.f, 0.f);
             if (GV) vj = lds128(sa + PSTRIDE);
@@ -775,7 +777,7 @@ k_rk(SweepArgs a, const float* __restrict__ u_s, float* __restrict__ gv_full) {
                     g[3 * al + be] = (float)(-t);
                 }
         }
-        // force-sweep state row (FROW float4 = one 128-byte line per particle; pieces 0 and 1 are written by k_hydro_prep):
+        // force-sweep state row (FROW float4 = one 128-byte line per particle; pieces 0 and 1 repeat the compact array xv):
         //   (x,y,z,1/h) (vx,vy,vz,V) | (A',B) (c',M'0) (M'1..M'4) (M'5..M'8) (gxx,gyy,gzz,P) (gxy+gyx, gxz+gzx, gyz+gzy, rho)
         // with the kernel normalisation folded into the coefficients, A' = -(56/3) sigma/h^5 A, c' = sigma/h^3 c,
         // M' = sigma/h^3 M, so that grad WR_ij = W~ (c' + M' x) + A' s D~ x with the dimensionless W~ = (1-eta)^6 (1+6 eta+35/3 eta^2),
@@ -786,7 +788,9 @@ k_rk(SweepArgs a, const float* __restrict__ u_s, float* __restrict__ gv_full) {
         const float k5f = -C56_3 * (k3f * ihf * ihf);
         const float u = u_s[i], rho = a.rho_s[i], gm = a.gamma;
         const float P = (gm - 1.0f) * rho * u;
-        float4* f = a.fst + i * FROW;
+        float4* f = a.fst + i * FROW;                        // the whole 128-byte line is written here
+        f[0] = make_float4(xi, yi, zi, ihf);
+        f[1] = vi;
         f[2] = make_float4(k5f * o0.x, o0.y, o0.z, o0.w);
         f[3] = make_float4(k3f * o1.x, k3f * o1.y, k3f * o1.z, k3f * o1.w);
         f[4] = make_float4(k3f * o2.x, k3f * o2.y, k3f * o2.z, k3f * o2.w);
@@ -1091,7 +1095,7 @@ SweepArgs make_args(crk_ctx* c) {
     a.cand_first = (const uint32_t*)c->cand_first.p;
     a.perm = c->perm;
     a.posh = (const float4*)c->posh.p; a.posV = (float4*)c->posV.p;
-    a.coef = (float4*)c->coef.p; a.fst = (float4*)c->fst.p; a.facc = (float4*)c->facc.p;
+    a.coef = (float4*)c->coef.p; a.fst = (float4*)c->fst.p; a.facc = (float4*)c->facc.p; a.xv = (float4*)c->xv.p;
     a.rho_s = (float*)c->rho_s.p; a.m_s = (const float*)c->m_s.p;
     a.gamma = c->prm.gamma; a.n_h = c->prm.n_h; a.C_l = c->prm.C_l; a.C_q = c->prm.C_q;
     a.eps2 = c->prm.eps * c->prm.eps;
@@ -1154,6 +1158,7 @@ int crk_launch_hydro_prep(crk_ctx* c, const float* vx, const float* vy, const fl
     CRK_TRY(crk_ensure(c, c->u_s, (size_t)np * sizeof(float)));
     CRK_TRY(crk_ensure(c, c->fst, (size_t)np * FROW * sizeof(float4)));
     CRK_TRY(crk_ensure(c, c->facc, (size_t)np * sizeof(float4)));
+    CRK_TRY(crk_ensure(c, c->xv, (size_t)np * 2 * sizeof(float4)));
     k_pack_vel<<<(unsigned)((c->n + 255) / 256), 256, 0, c->stream>>>(vx, vy, vz, u, c->n, (float4*)c->vel_orig.p);
     CRK_TRY(crk_check_launch(c, "k_pack_vel"));
     SweepArgs a = make_args(c);
