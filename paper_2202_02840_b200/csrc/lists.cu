@@ -82,7 +82,7 @@ __device__ __forceinline__ int test_tile(WarpSmem& S, int* flag, int fill, int C
     uint32_t gp = smem_u32(&S.queue[g][lane]);                  // next entry of this lane (row stride 64 bytes)
     const float2 xi2 = make_float2(xi, xi), yi2 = make_float2(yi, yi), zi2 = make_float2(zi, zi);
     const int C0 = C;
-    uint32_t kept = 0u;
+    uint32_t kept = 0u, bit = 1u, Cu = (uint32_t)C, Cs = (uint32_t)C | CRK_ELL_SYM;
     for (int t0 = 0; t0 < fill; t0 += 2) {
         const float4 pa = S.ta[t0 >> 1], pb = S.tb[t0 >> 1];
         float2 dx = __fadd2_rn(xi2, make_float2(pa.x, pa.y));    // x_i - x_j (the tile holds -x_j)
@@ -96,29 +96,87 @@ __device__ __forceinline__ int test_tile(WarpSmem& S, int* flag, int fill, int C
         }
         const float2 r2v = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
         const float r2[2] = {r2v.x, r2v.y}, hj2[2] = {pb.z, pb.w};
+        if (!SELF) {
+            // one candidate = ten instructions, written out because the compiler turns the conditional increments into add + move
+            // pairs and rebuilds the bit of `kept` with a shift, a select and an or: two compares, the acceptance vote, the
+            // entry word, one predicated 16-bit store, and four predicated updates (queue pointer, kept mask, C, C | SYM)
 #pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            bool ag = r2[u] < hi2;                                         // gather: Eqs. 13-14
-            bool as = ag || (r2[u] < hj2[u]);                              // symmetric: r2 < max(h_i^2, h_j^2), Eqs. 17-18
-            if (SELF) {
-                const bool notself = (t0 + u) != lane;
+            for (int u = 0; u < 2; ++u) {
+                if (WRAP) {
+                    uint32_t hit;
+                    asm volatile(
+                        "{\n"
+                        ".reg .pred pg, ps, pa;\n"
+                        ".reg .b32 e;\n"
+                        ".reg .b16 eh;\n"
+                        "setp.lt.f32 pg, %6, %7;\n"                    // gather: r2 < h_i^2 (Eqs. 13-14)
+                        "setp.lt.or.f32 ps, %6, %8, pg;\n"             // symmetric: r2 < max(h_i^2, h_j^2) (Eqs. 17-18)
+                        "vote.sync.any.pred pa, ps, 0xffffffff;\n"     // a candidate accepted by some lane gets the next slot
+                        "selp.b32 e, %2, %3, pg;\n"
+                        "or.b32 e, e, %9;\n"                           // CRK_ELL_WRAP: the pair crosses the periodic boundary
+                        "cvt.u16.u32 eh, e;\n"
+                        "@ps st.shared.u16 [%0], eh;\n"
+                        "@ps add.u32 %0, %0, 64;\n"
+                        "selp.u32 %5, 1, 0, ps;\n"
+                        "@pa or.b32 %1, %1, %4;\n"
+                        "@pa add.u32 %2, %2, 1;\n"
+                        "@pa add.u32 %3, %3, 1;\n"
+                        "shl.b32 %4, %4, 1;\n"
+                        "}"
+                        : "+r"(gp), "+r"(kept), "+r"(Cu), "+r"(Cs), "+r"(bit), "=r"(hit)
+                        : "f"(r2[u]), "f"(hi2), "f"(hj2[u]), "r"(wr[u] ? CRK_ELL_WRAP : 0u)
+                        : "memory");
+                    wflag = wflag || (wr[u] && hit != 0u);
+                } else {
+                    asm volatile(
+                        "{\n"
+                        ".reg .pred pg, ps, pa;\n"
+                        ".reg .b32 e;\n"
+                        ".reg .b16 eh;\n"
+                        "setp.lt.f32 pg, %5, %6;\n"
+                        "setp.lt.or.f32 ps, %5, %7, pg;\n"
+                        "vote.sync.any.pred pa, ps, 0xffffffff;\n"
+                        "selp.b32 e, %2, %3, pg;\n"
+                        "cvt.u16.u32 eh, e;\n"
+                        "@ps st.shared.u16 [%0], eh;\n"
+                        "@ps add.u32 %0, %0, 64;\n"
+                        "@pa or.b32 %1, %1, %4;\n"
+                        "@pa add.u32 %2, %2, 1;\n"
+                        "@pa add.u32 %3, %3, 1;\n"
+                        "shl.b32 %4, %4, 1;\n"
+                        "}"
+                        : "+r"(gp), "+r"(kept), "+r"(Cu), "+r"(Cs), "+r"(bit)
+                        : "f"(r2[u]), "f"(hi2), "f"(hj2[u])
+                        : "memory");
+                }
+                CRK_CHECK(flag, gp <= smem_u32(&S.queue[CRK_QCAP - 1][31]) + 66u, 0);          // entry queue row < CRK_QCAP
+                CRK_CHECK(flag, Cu <= (uint32_t)CRK_CCAP, 1);                                    // candidate slot < CRK_CCAP
+            }
+        } else {
+#pragma unroll
+            for (int u = 0; u < 2; ++u) {
+                bool ag = r2[u] < hi2;                                         // gather: Eqs. 13-14
+                bool as = ag || (r2[u] < hj2[u]);                              // symmetric: r2 < max(h_i^2, h_j^2), Eqs. 17-18
+                const bool notself = (t0 + u) != lane;                         // the tile is the leaf itself in lane order
                 ag = ag && notself;
                 as = as && notself;
+                uint32_t e = ag ? Cu : Cs;
+                if (WRAP) {
+                    e |= wr[u] ? CRK_ELL_WRAP : 0u;
+                    wflag = wflag || (wr[u] && as);
+                }
+                CRK_CHECK(flag, !as || gp < smem_u32(&S.queue[CRK_QCAP - 1][31]) + 2u, 0);   // entry queue row < CRK_QCAP
+                CRK_CHECK(flag, Cu < (uint32_t)CRK_CCAP, 1);                                   // candidate slot < CRK_CCAP
+                sts_u16_if(gp, e, as);                                         // one predicated store, no branch
+                gp += as ? 64u : 0u;
+                kept |= bit;                                                   // the leaf's own particles always get a slot
+                bit <<= 1;
+                ++Cu;
+                ++Cs;
             }
-            const bool any = SELF || __any_sync(0xffffffffu, as);         // the leaf's own particles always get a slot
-            uint32_t e = ag ? (uint32_t)C : ((uint32_t)C | CRK_ELL_SYM);
-            if (WRAP) {
-                e |= wr[u] ? CRK_ELL_WRAP : 0u;
-                wflag = wflag || (wr[u] && as);
-            }
-            CRK_CHECK(flag, !as || gp < smem_u32(&S.queue[CRK_QCAP - 1][31]) + 2u, 0);   // entry queue row < CRK_QCAP
-            CRK_CHECK(flag, !any || C < CRK_CCAP, 1);                                      // candidate slot < CRK_CCAP
-            sts_u16_if(gp, e, as);                                         // one predicated store, no branch
-            gp += as ? 64u : 0u;
-            kept |= any ? (1u << (t0 + u)) : 0u;
-            C += any ? 1 : 0;
         }
     }
+    C = (int)Cu;
     if (lane < fill && ((kept >> lane) & 1u)) S.cand[C0 + __popc(kept & ((1u << lane) - 1u))] = S.tidx[lane];
     g = (int)((gp - smem_u32(&S.queue[0][lane])) >> 6);
     return C;
