@@ -1,9 +1,11 @@
 // pairs.cu -- steps a1..a5: the four pair sweeps of one CRKSPH derivative evaluation (FP32 pair math on the FMA pipes),
 // and the next rows that ride on them: compatible energy sweep, time-step criteria, evolved smoothing length.
 //
-// All sweeps walk the neighbour lists built once per crk_build_cells (lists.cu).  A leaf (32 particles) is served by WPL
-// warps; lane l of each of them holds particle i = 32*leaf + l in registers.  Per segment of the leaf's chain:
-//   stage   the WPL warps copy the j-state planes of the segment's C candidates into a shared-memory tile, slot = candidate
+// All sweeps walk the neighbour lists built once per crk_build_cells (lists.cu).  A leaf (32 particles) is served by a group
+// of WPL warps; lane l of each of them holds particle i = 32*leaf + l in registers.  The kernels are persistent: a group takes
+// leaves from a work counter until none is left.  Per segment of the leaf's chain:
+//   meta    header, entry counts and candidate indices were copied to shared memory while the previous segment's rows ran
+//   stage   the WPL warps copy the j-state of the segment's C candidates into a shared-memory tile, slot = candidate
 //   drain   warp wl takes rows wl, wl+WPL, ... of the ELL block; row k holds the k-th entry of every lane, so each lane
 //           evaluates one accepted pair per row with j-state fetched from the tile (entries are prefetched 4 rows ahead)
 // and at the end the WPL partial sums of a lane are added in fixed warp order (deterministic) before the epilogue.
@@ -906,10 +908,9 @@ __device__ __forceinline__ PairF force_pair(const ForceConst& k, const PState& I
     return o;
 }
 
-// One CTA = one leaf: W5_WPL warps share the tile of the leaf's candidates and split each lane's entries by rows; four
-// CTAs are resident per SM, so one CTA's staging (header -> candidates -> state, three dependent global loads) overlaps the
-// other three's pair math.  (A persistent, double-buffered variant with 2 x 8 warps per SM was measured slower: 13.1 vs
-// 11.7 ms -- its per-leaf barrier couples all warps of the SM half; profiles/r01_sweeps_v9_ncu_full.md.)
+// One group = one CTA of W5_WPL warps: they share the tile of the leaf's candidates and split each lane's entries by rows;
+// four persistent CTAs are resident per SM, so one group's staging overlaps the other three's pair math (with the copies
+// switched off the sweep is 8 % faster, no more: profiles/r02_notes.md #29).  2 .. 6 warps per leaf were measured (#26).
 #ifndef CRK_W5_WPL
 #define CRK_W5_WPL 4
 #endif

@@ -121,6 +121,102 @@ __global__ void __launch_bounds__(NBR_WARPS * 32) k_leaf_list(const float4* __re
     }
 }
 
+// The same lists, built for the 32 leaves of a level-1 node together: one warp walks the tree ONCE with the node's box and
+// largest h (a superset of what any of its leaves can reach: a leaf's box lies inside the node's, and the gap is evaluated
+// with monotone float operations), collects the candidate leaves in ascending order in shared memory, and then every lane
+// tests the candidates against its own leaf with exactly the arithmetic of k_leaf_list -- same entries, same order, a seventh
+// of the instructions (the upper levels are pruned once per 32 leaves instead of once per leaf).
+constexpr int JOINT_CHUNK = 128;
+__global__ void __launch_bounds__(NBR_WARPS * 32) k_leaf_list_joint(const float4* __restrict__ lo, const float4* __restrict__ hi,
+                                                                    Levels lv, float L, uint32_t cap, uint32_t* __restrict__ cnt,
+                                                                    uint32_t* __restrict__ gcnt, uint32_t* __restrict__ list,
+                                                                    uint32_t* __restrict__ max_cnt) {
+    __shared__ uint32_t stack[NBR_WARPS][NBR_STACK];
+    __shared__ uint32_t chunk[NBR_WARPS][JOINT_CHUNK];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int64_t g = (int64_t)blockIdx.x * NBR_WARPS + w;          // level-1 node = leaves 32 g .. 32 g + 31
+    if (g >= lv.cnt[1]) return;
+    const float4 Qlo = lo[lv.off[1] + g], Qhi = hi[lv.off[1] + g];
+    const float hQ2 = __fmul_rn(Qlo.w, Qlo.w);
+    const int64_t q = g * CRK_BVH_FAN + lane;
+    const bool valid = q < lv.cnt[0];
+    const float inf = __int_as_float(0x7f800000);
+    float4 qlo = make_float4(inf, inf, inf, 0.f), qhi = make_float4(-inf, -inf, -inf, 0.f);
+    if (valid) {
+        qlo = lo[q];
+        qhi = hi[q];
+    }
+    const float hq2 = __fmul_rn(qlo.w, qlo.w);
+    const float half = 0.5f * L;
+    const uint32_t lt = (1u << lane) - 1u;
+    uint32_t n_out = 0, n_gather = 0;
+    const uint64_t base = (uint64_t)q * cap;
+    int fill = 0;
+    // every lane tests the collected candidate leaves against its own leaf (the arithmetic of k_leaf_list)
+    auto drain = [&]() {
+        __syncwarp();
+        for (int t = 0; t < fill; ++t) {
+            const uint32_t b = chunk[w][t];
+            const float4 blo = lo[b], bhi = hi[b];
+            bool wrap = false;
+            const float gx = axis_gap(qlo.x, qhi.x, blo.x, bhi.x, L, half, wrap);
+            const float gy = axis_gap(qlo.y, qhi.y, blo.y, bhi.y, L, half, wrap);
+            const float gz = axis_gap(qlo.z, qhi.z, blo.z, bhi.z, L, half, wrap);
+            const float g2 = __fmaf_rn(gz, gz, __fmaf_rn(gy, gy, __fmul_rn(gx, gx)));
+            const float hb2 = __fmul_rn(blo.w, blo.w);
+            const bool gather = g2 < hq2;
+            const bool pass = valid && (g2 < fmaxf(hq2, hb2));
+            if (pass) {
+                if (n_out < cap) list[base + n_out] = b | (gather ? CRK_FLAG_GATHER : 0u) | (wrap ? CRK_FLAG_WRAP : 0u);
+                ++n_out;
+                n_gather += gather ? 1u : 0u;
+            }
+        }
+        fill = 0;
+        __syncwarp();
+    };
+    int sp = 0;
+    if (lane == 0) stack[w][0] = ((uint32_t)lv.n_levels << 28);   // pseudo-root: children = all nodes of the top level
+    sp = 1;
+    __syncwarp();
+    while (sp > 0) {
+        const uint32_t e = stack[w][sp - 1];
+        --sp;
+        __syncwarp();
+        const int clev = (int)(e >> 28) - 1;
+        const int64_t child = (int64_t)(e & CRK_LEAF_MASK) * CRK_BVH_FAN + lane;
+        bool pass = false, wrap = false;
+        if (child < lv.cnt[clev]) {
+            const float4 blo = lo[lv.off[clev] + child], bhi = hi[lv.off[clev] + child];
+            const float gx = axis_gap(Qlo.x, Qhi.x, blo.x, bhi.x, L, half, wrap);
+            const float gy = axis_gap(Qlo.y, Qhi.y, blo.y, bhi.y, L, half, wrap);
+            const float gz = axis_gap(Qlo.z, Qhi.z, blo.z, bhi.z, L, half, wrap);
+            const float g2 = __fmaf_rn(gz, gz, __fmaf_rn(gy, gy, __fmul_rn(gx, gx)));
+            const float hb2 = __fmul_rn(blo.w, blo.w);
+            pass = g2 < fmaxf(hQ2, hb2);
+        }
+        const uint32_t m = __ballot_sync(0xffffffffu, pass);
+        if (clev == 0) {
+            const int np = __popc(m);
+            if (fill + np > JOINT_CHUNK) drain();
+            if (pass) chunk[w][fill + __popc(m & lt)] = (uint32_t)child;
+            fill += np;
+        } else {
+            // push in descending order so that the lowest child is popped first (candidates come out ascending)
+            if (pass) stack[w][sp + __popc(m & ~lt & ~(1u << lane))] = ((uint32_t)clev << 28) | (uint32_t)child;
+            sp += __popc(m);
+            __syncwarp();
+        }
+    }
+    drain();
+    if (valid) {
+        cnt[q] = n_out;
+        gcnt[q] = n_gather;
+    }
+    const uint32_t mx = __reduce_max_sync(0xffffffffu, n_out);
+    if (lane == 0) atomicMax(max_cnt, mx);
+}
+
 __global__ void k_sum_u32(const uint32_t* __restrict__ a, int64_t n, unsigned long long* __restrict__ out) {
     unsigned long long s = 0;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (int64_t)gridDim.x * blockDim.x) s += a[i];
@@ -158,9 +254,16 @@ int crk_build_tree_and_list(crk_ctx* c) {
     unsigned long long* d_sum2 = (unsigned long long*)((int*)c->flag.p + FW_SUM_ALL);
     if (c->leaf_list_cap < 64) c->leaf_list_cap = 96;
     CRK_TRY(crk_ensure(c, c->nbr_list, ((size_t)nl * c->leaf_list_cap + 1) * sizeof(uint32_t)));
-    k_leaf_list<<<grid, NBR_WARPS * 32, 0, c->stream>>>(lo, hi, lv, c->prm.box, (uint32_t)c->leaf_list_cap,
-                                                        (uint32_t*)c->nbr_cnt.p, (uint32_t*)c->nbr_gcnt.p,
-                                                        (uint32_t*)c->nbr_list.p, d_max);
+    if (c->n_levels >= 2) {
+        const unsigned jgrid = (unsigned)((lv.cnt[1] + NBR_WARPS - 1) / NBR_WARPS);
+        k_leaf_list_joint<<<jgrid, NBR_WARPS * 32, 0, c->stream>>>(lo, hi, lv, c->prm.box, (uint32_t)c->leaf_list_cap,
+                                                                   (uint32_t*)c->nbr_cnt.p, (uint32_t*)c->nbr_gcnt.p,
+                                                                   (uint32_t*)c->nbr_list.p, d_max);
+    } else {   // at most 32 leaves: there is no level above them to share
+        k_leaf_list<<<grid, NBR_WARPS * 32, 0, c->stream>>>(lo, hi, lv, c->prm.box, (uint32_t)c->leaf_list_cap,
+                                                            (uint32_t*)c->nbr_cnt.p, (uint32_t*)c->nbr_gcnt.p,
+                                                            (uint32_t*)c->nbr_list.p, d_max);
+    }
     CRK_TRY(crk_check_launch(c, "k_leaf_list"));
     k_sum_u32<<<148, 256, 0, c->stream>>>((const uint32_t*)c->nbr_gcnt.p, nl, d_sum);
     CRK_TRY(crk_check_launch(c, "k_sum_u32"));
