@@ -49,6 +49,7 @@ enum { FW_ERROR = 0,        // bit 0: input out of range (S13)
        FW_SUM_GATHER = 4,   // u64: leaf pairs with the gather flag
        FW_SUM_ALL = 6,      // u64: leaf pairs
        FW_ARENA = 8,        // u64: arena units the neighbour lists need
+       FW_SETMIXED = 10,    // 1: the supports of the set span more than a factor four (tree.cu: every leaf list built per leaf)
        FW_HOST_ACTIVE = 12, // host side only: crk_select_active
        FW_WORDS = 16 };
 

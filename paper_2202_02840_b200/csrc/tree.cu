@@ -63,14 +63,38 @@ constexpr int NBR_STACK = 32 * (CRK_MAX_LEVELS + 1);
 // One traversal per query leaf.  Leaf q owns slots [q * cap, (q + 1) * cap) of the list; entries beyond cap are counted but
 // not written, and the host re-runs the kernel with a larger cap if the largest count (atomicMax -> *max_cnt) exceeds it
 // (the capacity found is kept in the context, so later builds need one pass and no prefix sum).
-__global__ void __launch_bounds__(NBR_WARPS * 32) k_leaf_list(const float4* __restrict__ lo, const float4* __restrict__ hi,
-                                                              Levels lv, float L, uint32_t cap, uint32_t* __restrict__ cnt,
-                                                              uint32_t* __restrict__ gcnt, uint32_t* __restrict__ list,
-                                                              uint32_t* __restrict__ max_cnt) {
-    __shared__ uint32_t stack[NBR_WARPS][NBR_STACK];
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    const int64_t q = (int64_t)blockIdx.x * NBR_WARPS + w;
-    if (q >= lv.cnt[0]) return;
+// A level-1 node whose supports differ a lot (a background particle of large h among cluster particles) would hand the reach
+// of its largest h to all 32 leaves in the joint traversal: its leaves take the per-leaf traversal instead (clustered 128^3:
+// joint for all nodes 0.26 ms, per leaf 0.18 ms).
+__device__ __forceinline__ bool node_is_mixed(float hmax, float hmin) { return hmax > 1.5f * hmin; }
+// A set whose supports span more than a factor four (the Plummer configurations) is served leaf by leaf altogether: there the
+// joint traversal loses even on the nodes of similar supports.  Decided once per build from the top level of the tree
+// (k_set_mixed -> status word FW_SETMIXED).
+__device__ __forceinline__ bool set_is_mixed(const float4* __restrict__ lo, const float4* __restrict__ hi, const Levels& lv, int lane) {
+    const int top = lv.n_levels - 1;
+    float hmax = 0.f, hmin = __int_as_float(0x7f800000);
+    for (int64_t k = lane; k < lv.cnt[top]; k += 32) {
+        hmax = fmaxf(hmax, lo[lv.off[top] + k].w);
+        hmin = fminf(hmin, hi[lv.off[top] + k].w);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        hmax = fmaxf(hmax, __shfl_xor_sync(0xffffffffu, hmax, o));
+        hmin = fminf(hmin, __shfl_xor_sync(0xffffffffu, hmin, o));
+    }
+    return hmax > 4.0f * hmin;
+}
+
+__global__ void k_set_mixed(const float4* __restrict__ lo, const float4* __restrict__ hi, Levels lv, int* __restrict__ flag) {
+    const bool mixed = set_is_mixed(lo, hi, lv, (int)threadIdx.x);
+    if (threadIdx.x == 0) flag[FW_SETMIXED] = mixed ? 1 : 0;
+}
+
+// one traversal for query leaf q by the whole warp (stack = the warp's shared-memory stack)
+__device__ __forceinline__ void leaf_list_one(const float4* __restrict__ lo, const float4* __restrict__ hi, const Levels& lv, float L,
+                                              uint32_t cap, uint32_t* __restrict__ cnt, uint32_t* __restrict__ gcnt,
+                                              uint32_t* __restrict__ list, uint32_t* __restrict__ max_cnt, uint32_t* stack_w,
+                                              int64_t q, int lane) {
     const float4 qlo = lo[q], qhi = hi[q];
     const float hq2 = __fmul_rn(qlo.w, qlo.w);
     const float half = 0.5f * L;
@@ -78,11 +102,11 @@ __global__ void __launch_bounds__(NBR_WARPS * 32) k_leaf_list(const float4* __re
     uint32_t n_out = 0, n_gather = 0;
     const uint64_t base = (uint64_t)q * cap;
     int sp = 0;
-    if (lane == 0) stack[w][0] = ((uint32_t)lv.n_levels << 28);   // pseudo-root: children = all nodes of the top level
+    if (lane == 0) stack_w[0] = ((uint32_t)lv.n_levels << 28);   // pseudo-root: children = all nodes of the top level
     sp = 1;
     __syncwarp();
     while (sp > 0) {
-        const uint32_t e = stack[w][sp - 1];
+        const uint32_t e = stack_w[sp - 1];
         --sp;
         __syncwarp();
         const int clev = (int)(e >> 28) - 1;
@@ -109,7 +133,7 @@ __global__ void __launch_bounds__(NBR_WARPS * 32) k_leaf_list(const float4* __re
             n_gather += __popc(mg);
         } else {
             // push in descending order so that the lowest child is popped first (list comes out ascending)
-            if (pass) stack[w][sp + __popc(m & ~lt & ~(1u << lane))] = ((uint32_t)clev << 28) | (uint32_t)child;
+            if (pass) stack_w[sp + __popc(m & ~lt & ~(1u << lane))] = ((uint32_t)clev << 28) | (uint32_t)child;
             sp += __popc(m);
             __syncwarp();
         }
@@ -121,6 +145,21 @@ __global__ void __launch_bounds__(NBR_WARPS * 32) k_leaf_list(const float4* __re
     }
 }
 
+__global__ void __launch_bounds__(NBR_WARPS * 32) k_leaf_list(const float4* __restrict__ lo, const float4* __restrict__ hi,
+                                                              Levels lv, float L, uint32_t cap, uint32_t* __restrict__ cnt,
+                                                              uint32_t* __restrict__ gcnt, uint32_t* __restrict__ list,
+                                                              uint32_t* __restrict__ max_cnt, const int* __restrict__ set_mixed) {
+    __shared__ uint32_t stack[NBR_WARPS][NBR_STACK];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int64_t q = (int64_t)blockIdx.x * NBR_WARPS + w;
+    if (q >= lv.cnt[0]) return;
+    if (set_mixed && *set_mixed == 0) {   // the leaves of nodes with similar supports are served by k_leaf_list_joint
+        const int64_t g = q / CRK_BVH_FAN;
+        if (!node_is_mixed(lo[lv.off[1] + g].w, hi[lv.off[1] + g].w)) return;
+    }
+    leaf_list_one(lo, hi, lv, L, cap, cnt, gcnt, list, max_cnt, stack[w], q, lane);
+}
+
 // The same lists, built for the 32 leaves of a level-1 node together: one warp walks the tree ONCE with the node's box and
 // largest h (a superset of what any of its leaves can reach: a leaf's box lies inside the node's, and the gap is evaluated
 // with monotone float operations), collects the candidate leaves in ascending order in shared memory, and then every lane
@@ -130,13 +169,14 @@ constexpr int JOINT_CHUNK = 128;
 __global__ void __launch_bounds__(NBR_WARPS * 32) k_leaf_list_joint(const float4* __restrict__ lo, const float4* __restrict__ hi,
                                                                     Levels lv, float L, uint32_t cap, uint32_t* __restrict__ cnt,
                                                                     uint32_t* __restrict__ gcnt, uint32_t* __restrict__ list,
-                                                                    uint32_t* __restrict__ max_cnt) {
+                                                                    uint32_t* __restrict__ max_cnt, const int* __restrict__ set_mixed) {
     __shared__ uint32_t stack[NBR_WARPS][NBR_STACK];
     __shared__ uint32_t chunk[NBR_WARPS][JOINT_CHUNK];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const int64_t g = (int64_t)blockIdx.x * NBR_WARPS + w;          // level-1 node = leaves 32 g .. 32 g + 31
     if (g >= lv.cnt[1]) return;
     const float4 Qlo = lo[lv.off[1] + g], Qhi = hi[lv.off[1] + g];
+    if (node_is_mixed(Qlo.w, Qhi.w) || *set_mixed != 0) return;     // served leaf by leaf (k_leaf_list)
     const float hQ2 = __fmul_rn(Qlo.w, Qlo.w);
     const int64_t q = g * CRK_BVH_FAN + lane;
     const bool valid = q < lv.cnt[0];
@@ -254,16 +294,22 @@ int crk_build_tree_and_list(crk_ctx* c) {
     unsigned long long* d_sum2 = (unsigned long long*)((int*)c->flag.p + FW_SUM_ALL);
     if (c->leaf_list_cap < 64) c->leaf_list_cap = 96;
     CRK_TRY(crk_ensure(c, c->nbr_list, ((size_t)nl * c->leaf_list_cap + 1) * sizeof(uint32_t)));
-    if (c->n_levels >= 2) {
+    // enough level-1 nodes to fill the GPU with one warp each: the joint traversal for nodes of similar supports, the
+    // per-leaf traversal for the rest; small sets: per leaf only
+    const bool joint = c->n_levels >= 2 && lv.cnt[1] >= 2048;
+    const int* d_mixed = (const int*)c->flag.p + FW_SETMIXED;
+    if (joint) {
+        k_set_mixed<<<1, 32, 0, c->stream>>>(lo, hi, lv, (int*)c->flag.p);
+        CRK_TRY(crk_check_launch(c, "k_set_mixed"));
         const unsigned jgrid = (unsigned)((lv.cnt[1] + NBR_WARPS - 1) / NBR_WARPS);
         k_leaf_list_joint<<<jgrid, NBR_WARPS * 32, 0, c->stream>>>(lo, hi, lv, c->prm.box, (uint32_t)c->leaf_list_cap,
                                                                    (uint32_t*)c->nbr_cnt.p, (uint32_t*)c->nbr_gcnt.p,
-                                                                   (uint32_t*)c->nbr_list.p, d_max);
-    } else {   // at most 32 leaves: there is no level above them to share
-        k_leaf_list<<<grid, NBR_WARPS * 32, 0, c->stream>>>(lo, hi, lv, c->prm.box, (uint32_t)c->leaf_list_cap,
-                                                            (uint32_t*)c->nbr_cnt.p, (uint32_t*)c->nbr_gcnt.p,
-                                                            (uint32_t*)c->nbr_list.p, d_max);
+                                                                   (uint32_t*)c->nbr_list.p, d_max, d_mixed);
+        CRK_TRY(crk_check_launch(c, "k_leaf_list_joint"));
     }
+    k_leaf_list<<<grid, NBR_WARPS * 32, 0, c->stream>>>(lo, hi, lv, c->prm.box, (uint32_t)c->leaf_list_cap,
+                                                        (uint32_t*)c->nbr_cnt.p, (uint32_t*)c->nbr_gcnt.p,
+                                                        (uint32_t*)c->nbr_list.p, d_max, joint ? d_mixed : nullptr);
     CRK_TRY(crk_check_launch(c, "k_leaf_list"));
     k_sum_u32<<<148, 256, 0, c->stream>>>((const uint32_t*)c->nbr_gcnt.p, nl, d_sum);
     CRK_TRY(crk_check_launch(c, "k_sum_u32"));
