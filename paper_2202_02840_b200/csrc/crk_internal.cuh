@@ -25,7 +25,8 @@ enum { EV_BUILD0 = 0, EV_SORTED, EV_TREE1, EV_BUILD1, EV_VOL0, EV_VOL1, EV_RK0, 
 //   cand[c]   = sorted-order index of candidate c (only candidates accepted by at least one lane of the leaf); in a
 //               leaf's first segment cand[0..31] are the leaf's own 32 particles in lane order (always kept)
 //   ell[k][l] = k-th entry of lane l: candidate index | CRK_ELL_SYM (h_i^2 <= r2 < h_j^2: a pair of the symmetric set that
-//               is not in the lane's gather set) | CRK_ELL_WRAP (pair crosses the periodic boundary); lane l owns cnt[l]
+//               is not in the lane's gather set; also the padding of rows beyond cnt[l]: CRK_ELL_SYM | slot 0) | CRK_ELL_WRAP
+//               (pair crosses the periodic boundary); lane l owns cnt[l]
 //               entries; CRK_SEG_WRAP: some entry of the segment may carry CRK_ELL_WRAP
 #define CRK_CCAP 384             // candidates per segment (tile capacity of the sweeps)
 #define CRK_CAND_STRIDE 384      // u32 per leaf in cand_first (the sweeps read it in 16-byte groups)

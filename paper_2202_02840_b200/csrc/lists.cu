@@ -215,8 +215,8 @@ __global__ void __launch_bounds__(LW * 32) k_nbr_lists(ListArgs a) {
         unsigned long long base = 0;
         if (lane == 0) base = atomicAdd(a.counter, units);
         base = __shfl_sync(0xffffffffu, base, 0);
-        // padding of shorter lanes: slot 0 (the sweeps prefetch it, never evaluate it)
-        for (int k = g; k < K; ++k) S.queue[k][lane] = (uint16_t)0;
+        // padding of shorter lanes: slot 0 (the sweeps prefetch it, never evaluate it) with the flag a gather sweep skips
+        for (int k = g; k < K; ++k) S.queue[k][lane] = (uint16_t)CRK_ELL_SYM;
         __syncwarp();
         if (base + units <= a.arena_cap) {
             CRK_CHECK(a.flag, K <= CRK_QCAP && C <= CRK_CCAP && base >= 1, 3);                 // segment sizes

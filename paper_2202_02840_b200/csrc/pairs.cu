@@ -304,7 +304,7 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
             const int k = wl + q * WPL;
-            e[q] = (k < rows) ? (uint32_t)__ldg(ep + k * 32) : 0u;
+            e[q] = (k < rows) ? (uint32_t)__ldg(ep + k * 32) : CRK_ELL_SYM;
         }
         const bool last = (s.next == 0u);
         if (first) staged();
@@ -333,31 +333,41 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
         }
         // plane 0 of the next pair's candidate is fetched one pair ahead: the pair math starts without waiting for shared
         // memory, and the loads of the remaining planes are covered by the arithmetic that needs plane 0 only
+        // Padding entries (rows beyond a lane's count) are CRK_ELL_SYM | slot 0: a gather sweep skips them with the test it makes
+        // anyway, a symmetric sweep compares the row with the lane's count.
+        auto slot_addr = [&](uint32_t ent) {
+            uint32_t ad;
+            asm("mad.lo.u32 %0, %1, 16, %2;" : "=r"(ad) : "r"(ent & CRK_ELL_MASK), "r"(tile_s));
+            return ad;
+        };
         float4 cur[NPRE];
+        uint32_t sa = slot_addr(e[0]);
 #pragma unroll
-        for (int p = 0; p < NPRE; ++p) cur[p] = lds128(tile_s + (uint32_t)p * PSTRIDE + (e[0] & CRK_ELL_MASK) * 16u);
+        for (int p = 0; p < NPRE; ++p) cur[p] = lds128(sa + (uint32_t)p * PSTRIDE);
         for (int k0 = wl; k0 < rows; k0 += 4 * WPL) {
             uint32_t nx[4];
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const int k = k0 + (4 + q) * WPL;
-                nx[q] = (k < rows) ? (uint32_t)__ldg(ep + k * 32) : 0u;
+                nx[q] = (k < rows) ? (uint32_t)__ldg(ep + k * 32) : CRK_ELL_SYM;
             }
 #pragma unroll
             for (int q = 0; q < 4; ++q) {
                 const int k = k0 + q * WPL;
                 const uint32_t en = (q < 3) ? e[(q + 1) & 3] : nx[0];
+                const uint32_t san = slot_addr(en);
                 float4 nxt[NPRE];
 #pragma unroll
-                for (int p = 0; p < NPRE; ++p) nxt[p] = lds128(tile_s + (uint32_t)p * PSTRIDE + (en & CRK_ELL_MASK) * 16u);
+                for (int p = 0; p < NPRE; ++p) nxt[p] = lds128(san + (uint32_t)p * PSTRIDE);
                 CRK_CHECK(a.flag, k >= mine || (int)(e[q] & CRK_ELL_MASK) < s.C, 10);       // entry -> staged slot
+                CRK_CHECK(a.flag, SYM || k < mine || (e[q] & CRK_ELL_SYM) != 0u, 11);       // padding carries the skip flag
 #ifdef CRK_EXP_NOCONFLICT   // timing experiment only (wrong results): every lane of a quarter-warp reads a different bank group
                 if (k < mine && (SYM || !(e[q] & CRK_ELL_SYM)))
                     pair(tile_s + (((e[q] & CRK_ELL_MASK) & ~31u) | (uint32_t)lane) * 16u, (e[q] & CRK_ELL_WRAP) != 0u, cur);
 #else
-                if (k < mine && (SYM || !(e[q] & CRK_ELL_SYM)))
-                    pair(tile_s + (e[q] & CRK_ELL_MASK) * 16u, (e[q] & CRK_ELL_WRAP) != 0u, cur);
+                if (SYM ? (k < mine) : !(e[q] & CRK_ELL_SYM)) pair(sa, (e[q] & CRK_ELL_WRAP) != 0u, cur);
 #endif
+                sa = san;
 #pragma unroll
                 for (int p = 0; p < NPRE; ++p) cur[p] = nxt[p];
             }
