@@ -52,7 +52,8 @@ struct SweepArgs {
     float4* __restrict__ facc;            // (dv/dt, s = P / rho^gamma) per particle, written by k_forces
     float4* __restrict__ xv;              // (x,y,z,1/h) (vx,vy,vz,V) per particle, 32 bytes: what the grad v sweep stages
     float* __restrict__ rho_s;
-    const float* __restrict__ m_s;
+    float* __restrict__ m_s;              // masses in sorted order (written by k_volumes)
+    const float* __restrict__ m_in;       // masses in caller order (crk_volumes)
     int64_t np;                           // padded particle count nl*32 (plane stride)
     float gamma, n_h, C_l, C_q, eps2;
     // outputs in caller order (may be null)
@@ -482,17 +483,19 @@ __global__ void __launch_bounds__(W1_WPC * 32) k_volumes(SweepArgs a) {
             const float k3 = SIGMA_C4 * inv_h * inv_h * inv_h;
             const float ni = k3 * (acc + 1.0f);              // self term W~(0) = 1
             const float V = 1.0f / ni;
-            const float mi = a.m_s[i];
+            const int32_t p = a.perm[i];
+            const float mi = a.m_in[p];
+            a.m_s[i] = mi;
             const float rho = mi * ni;
             a.posV[i] = make_float4(xi, yi, zi, V);
             a.rho_s[i] = rho;
-            const int32_t p = a.perm[i];
             if (a.o0) a.o0[p] = V;
             if (a.o1) a.o1[p] = rho;
             if (a.ocnt) a.ocnt[p] = count;
         } else {
             a.posV[i] = make_float4(pi.x, pi.y, pi.z, 0.0f);
             a.rho_s[i] = 0.0f;
+            a.m_s[i] = 1.0f;
         }
         leaf = next;
     }
@@ -1091,12 +1094,6 @@ __global__ void __launch_bounds__(W5_WPL * 32, 4) k_compat(SweepArgs a, float dt
     }
 }
 
-__global__ void __launch_bounds__(256) k_gather_f32(const float* __restrict__ in, const int32_t* __restrict__ perm,
-                                                    int64_t n, int64_t np, float* __restrict__ out) {
-    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (k < np) out[k] = (k < n) ? in[perm[k]] : 1.0f;
-}
-
 SweepArgs make_args(crk_ctx* c) {
     SweepArgs a;
     memset(&a, 0, sizeof(a));
@@ -1107,7 +1104,7 @@ SweepArgs make_args(crk_ctx* c) {
     a.perm = c->perm;
     a.posh = (const float4*)c->posh.p; a.posV = (float4*)c->posV.p;
     a.coef = (float4*)c->coef.p; a.fst = (float4*)c->fst.p; a.facc = (float4*)c->facc.p; a.xv = (float4*)c->xv.p;
-    a.rho_s = (float*)c->rho_s.p; a.m_s = (const float*)c->m_s.p;
+    a.rho_s = (float*)c->rho_s.p; a.m_s = (float*)c->m_s.p;
     a.gamma = c->prm.gamma; a.n_h = c->prm.n_h; a.C_l = c->prm.C_l; a.C_q = c->prm.C_q;
     a.eps2 = c->prm.eps * c->prm.eps;
     a.flag = (int*)c->flag.p;
@@ -1150,9 +1147,8 @@ int crk_launch_volumes(crk_ctx* c, const float* m, float* V, float* rho, uint32_
     CRK_TRY(crk_ensure(c, c->posV, (size_t)np * sizeof(float4)));
     CRK_TRY(crk_ensure(c, c->rho_s, (size_t)np * sizeof(float)));
     CRK_TRY(crk_ensure(c, c->m_s, (size_t)np * sizeof(float)));
-    k_gather_f32<<<(unsigned)((np + 255) / 256), 256, 0, c->stream>>>(m, c->perm, c->n, np, (float*)c->m_s.p);
-    CRK_TRY(crk_check_launch(c, "k_gather_f32"));
     SweepArgs a = make_args(c);
+    a.m_in = m;
     a.o0 = V; a.o1 = rho; a.ocnt = nbr_count;
     const int smem = W1_WPC * W1_SMEM;
     unsigned grid = 0;
