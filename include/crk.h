@@ -58,7 +58,7 @@ typedef struct {
     float eps;        /* 0.1; enters Eq. 25 as eps^2 * hhat^2                                                 */
     int   leaf_size;  /* particles per leaf bucket; must be 32 in this version (one warp lane per particle)   */
     int   flags;      /* 0 or an OR of CRK_FLAG_TIMESTEP (the momentum sweep also reduces what crk_timestep needs),
-                         CRK_FLAG_KDK_REUSE and CRK_FLAG_KDK_COMPATIBLE (both about crk_kdk_step), defined below       */
+                         CRK_FLAG_KDK_REUSE and CRK_FLAG_KDK_COMPATIBLE (both about crk_kdk_step), CRK_FLAG_TREE_PER_LEAF, defined below */
 } crk_params;
 
 typedef struct {
@@ -134,6 +134,10 @@ int  crk_compatible_energy(crk_ctx* c, float dt, float* delta_u);
  * its own velocity change and pair accelerations, reading S20) instead of Eq. 18's rate: total energy is then
  * conserved to roundoff -- the paper's fiducial energy integration.  Two more pair sweeps per step.     */
 #define CRK_FLAG_KDK_COMPATIBLE 4
+/* CRK_FLAG_TREE_PER_LEAF: crk_build_cells builds every leaf interaction list with the per-leaf tree walk.  Without it, sets of
+ * 2048 or more level-1 nodes whose supports span less than a factor four walk the tree once per node of 32 leaves (same
+ * entries in the same order; tests compare the two).  */
+#define CRK_FLAG_TREE_PER_LEAF 8
 int  crk_kdk_step(crk_ctx* c, int64_t n, float* x, float* y, float* z, const float* h, float* vx, float* vy, float* vz,
                   const float* m, float* u, float dt);
 

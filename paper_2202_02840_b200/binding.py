@@ -105,12 +105,14 @@ def _opt(t, dtype=torch.float32):
 class Crk:
     """One library context (crk_ctx) bound to the current torch CUDA stream."""
 
-    def __init__(self, box=1.0, gamma=5.0 / 3.0, n_h=2.4, C_l=2.0, C_q=1.0, eps=0.1, stream=None, timestep=False, kdk_reuse=False, kdk_compatible=False):
+    def __init__(self, box=1.0, gamma=5.0 / 3.0, n_h=2.4, C_l=2.0, C_q=1.0, eps=0.1, stream=None, timestep=False, kdk_reuse=False, kdk_compatible=False,
+                 tree_per_leaf=False):
         L = _load()
         if not torch.cuda.is_available():
             raise RuntimeError("libcrk needs a CUDA device; there is no CPU fallback")
         self._L = L
-        self._p = _Params(box, gamma, n_h, C_l, C_q, eps, 32, (1 if timestep else 0) | (2 if kdk_reuse else 0) | (4 if kdk_compatible else 0))   # CRK_FLAG_TIMESTEP | _KDK_REUSE | _KDK_COMPATIBLE
+        self._p = _Params(box, gamma, n_h, C_l, C_q, eps, 32, (1 if timestep else 0) | (2 if kdk_reuse else 0) | (4 if kdk_compatible else 0)
+                          | (8 if tree_per_leaf else 0))   # CRK_FLAG_TIMESTEP | _KDK_REUSE | _KDK_COMPATIBLE | _TREE_PER_LEAF
         self.stream = stream if stream is not None else torch.cuda.current_stream()
         h = C.c_void_p()
         rc = L.crk_create(C.byref(h), C.byref(self._p), C.c_void_p(self.stream.cuda_stream))

@@ -296,7 +296,7 @@ int crk_build_tree_and_list(crk_ctx* c) {
     CRK_TRY(crk_ensure(c, c->nbr_list, ((size_t)nl * c->leaf_list_cap + 1) * sizeof(uint32_t)));
     // enough level-1 nodes to fill the GPU with one warp each: the joint traversal for nodes of similar supports, the
     // per-leaf traversal for the rest; small sets: per leaf only
-    const bool joint = c->n_levels >= 2 && lv.cnt[1] >= 2048;
+    const bool joint = c->n_levels >= 2 && lv.cnt[1] >= 2048 && !(c->prm.flags & CRK_FLAG_TREE_PER_LEAF);
     const int* d_mixed = (const int*)c->flag.p + FW_SETMIXED;
     if (joint) {
         k_set_mixed<<<1, 32, 0, c->stream>>>(lo, hi, lv, (int*)c->flag.p);

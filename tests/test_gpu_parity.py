@@ -117,6 +117,31 @@ def test_sort_tree_and_leaf_lists_cover_every_neighbour(oracle_mod):
             assert set(lj[fi].tolist()) <= gather, "a gather neighbour's leaf lacks the gather flag"
 
 
+def test_joint_tree_walk_builds_the_lists_of_the_per_leaf_walk():
+    """cosmo 128^3 = 2048 level-1 nodes of similar supports: crk_build_cells walks the tree once per node of 32 leaves; with
+    CRK_FLAG_TREE_PER_LEAF once per leaf.  Same entries, same order, same flags -- and so the same bits downstream."""
+    import torch
+    from paper_2202_02840_b200 import Crk
+    ps = wl.make_config("cosmo", 128)
+    dev = torch.device("cuda:0")
+    t = [torch.from_numpy(np.ascontiguousarray(getattr(ps, k))).to(dev) for k in ("x", "y", "z", "h", "vx", "vy", "vz", "m", "u")]
+    outs = []
+    lists = []
+    for per_leaf in (False, True):
+        ctx = Crk(box=ps.box, gamma=ps.gamma, n_h=ps.n_h, tree_per_leaf=per_leaf)
+        out = ctx.step_derivs(*t)
+        torch.cuda.synchronize()
+        st = ctx.stats()
+        rng = np.random.default_rng(1)
+        lists.append((st["n_leaf_pairs"], st["n_leaf_pairs_gather"], [ctx.leaf_list(int(q)) for q in rng.integers(0, st["n_leaves"], 200)]))
+        outs.append([o.cpu().numpy() for o in out])
+    assert lists[0][0] == lists[1][0] and lists[0][1] == lists[1][1], "leaf pair totals differ"
+    for a, b in zip(lists[0][2], lists[1][2]):
+        assert np.array_equal(a, b), "a leaf interaction list differs between the two walks"
+    for a, b in zip(outs[0], outs[1]):
+        assert np.array_equal(a.view(np.uint32), b.view(np.uint32)), "derivatives differ in some bit"
+
+
 # ------------------------------------------------------------------------------------------------ small configs
 @pytest.mark.parametrize("name,n_side", [("tiny_uniform", 16), ("blast_wave", 24), ("clustered", 24), ("cosmo", 32)])
 def test_parity_small(name, n_side, oracle_mod):
