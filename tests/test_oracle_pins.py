@@ -881,3 +881,119 @@ def test_active_mask_restricts_the_sums_and_nothing_else(clustered):
     for a, b, f in zip(r1, r2, full):
         assert np.array_equal(a[on], b[on]) and np.array_equal(a[on], f[on])
         assert np.isnan(a[~on]).all()
+
+
+# --------------------------------------------------------------------------- S14: the degenerate-neighbourhood branch
+def _s14_oracle(oracle_mod, pts, h, n_h=2.4):
+    """pts: float64 [n,3] inside a unit box; one support radius h for all.  Returns the oracle after rk_coefficients."""
+    pts = np.asarray(pts, dtype=np.float64)
+    x, y, z = (np.ascontiguousarray(pts[:, a], dtype=np.float32) for a in range(3))
+    hh = np.full(pts.shape[0], h, dtype=np.float32)
+    o = oracle_mod.Oracle(1.0, 5.0 / 3.0, n_h)
+    o.build(x, y, z, hh)
+    o.volumes(np.ones(pts.shape[0], dtype=np.float32))
+    A, B, gA, gB = o.rk_coefficients()
+    return o, (x, y, z, hh), (A, B, gA, gB)
+
+
+def _m2_ratio(o):
+    """det m2 / (tr m2 / 3)^3 of every particle, from the oracle's raw moments (1 for an isotropic m2, 0 for a flat one)"""
+    m0, m1, m2 = o.moments()
+    M = m2.T.reshape(-1, 3, 3)
+    tr3 = np.trace(M, axis1=1, axis2=2) / 3.0
+    with np.errstate(divide="ignore", invalid="ignore"):
+        return np.linalg.det(M) / tr3 ** 3
+
+
+def _flat_sets():
+    """neighbourhoods that span fewer than three dimensions: 1, 2, 3 points, four coplanar points, a coplanar disc of 20"""
+    rng = np.random.default_rng(1404)
+    c = np.array([0.5, 0.5, 0.5])
+    h = 0.2
+    disc = np.c_[0.09 * rng.uniform(-1, 1, (20, 2)), np.zeros(20)]
+    sets = {
+        "one": np.zeros((1, 3)),
+        "two": np.array([[0, 0, 0], [0.05, 0.02, -0.03]]),
+        "three": np.array([[0, 0, 0], [0.05, 0.02, -0.03], [-0.04, 0.06, 0.01]]),       # a plane through three points
+        "four_coplanar": np.array([[0, 0, 0], [0.06, 0, 0], [0, 0.05, 0], [0.05, 0.04, 0]]),
+        "disc20": disc,
+    }
+    return {k: (c + v, h) for k, v in sets.items()}
+
+
+@pytest.mark.parametrize("name", ["one", "two", "three", "four_coplanar", "disc20"])
+def test_S14_zeroth_moment_constraint_survives_a_singular_m2(name, oracle_mod):
+    """PAPER.md:116 ('enforcing the zeroth ... moments of WR integrate to 1'): where m2 cannot be inverted the linear
+    correction is dropped (B = 0, reading S14) but sum_j V_j WR_ij = 1 must still hold identically in x_i, so its gradient
+    sum_j V_j grad WR_ij = 0 too -- which fixes grad A = -A^2 grad m0, sign included -- and grad A is the derivative of A."""
+    pts, h = _flat_sets()[name]
+    o, (x, y, z, hh), (A, B, gA, gB) = _s14_oracle(oracle_mod, pts, h)
+    assert np.all(B == 0.0) and np.all(gB == 0.0), "these sets must take the fallback"
+    S0, S1, G0, G1 = o.rk_sums()
+    assert np.abs(S0 - 1).max() < 1e-12
+    assert (np.abs(G0) * h).max() < 1e-11
+    if name != "one":
+        assert (np.abs(gA).max(axis=0) > 1e-3 * A / h).any(), "a test of the sign needs a gradient that is not zero"
+    # grad A against central differences of A at displaced evaluation points (same branch: a displacement of 1e-5 h leaves
+    # det m2 / (tr m2 / 3)^3 below 1e-9)
+    h = float(hh[0])                    # the support radius as the oracle holds it (float32)
+    dl = 1e-5 * h
+    for i in range(pts.shape[0]):
+        p = np.array([x[i], y[i], z[i]], dtype=np.float64)
+        A0, B0 = o.eval_AB_at(p, h)
+        assert A0 == pytest.approx(A[i], rel=1e-9) and np.all(B0 == 0.0)
+        for c in range(3):
+            e = np.zeros(3); e[c] = dl
+            fd = (o.eval_AB_at(p + e, h)[0] - o.eval_AB_at(p - e, h)[0]) / (2 * dl)
+            assert fd == pytest.approx(gA[c, i], rel=1e-5, abs=1e-7 * A[i] / h)
+
+
+def test_S14_threshold_sits_where_the_first_moment_condition_is_given_up(oracle_mod):
+    """Reading S14: m2 counts as singular when det m2 <= 1e-4 (tr m2 / 3)^3.  The paper's constraint decides what
+    each side of that line must look like: above it sum_j V_j x_ij WR_ij = 0 holds (first moment), below it
+    only the zeroth moment does and the first-moment sum is what B = 0 leaves, A m1.  A disc of 20 points is walked off its
+    plane in 41 steps so that particles land on both sides of the line within a factor ten of it: a threshold ten times
+    larger or smaller puts some of them on the wrong side of this test."""
+    rng = np.random.default_rng(1405)
+    h = 0.2
+    disc = 0.09 * rng.uniform(-1, 1, (20, 2))
+    xi = rng.uniform(-1, 1, 20)
+    below, above = 0, 0
+    lo_r, hi_r = [], []
+    for eps in np.logspace(-3.5, -1.5, 41):                 # thickness / radius of the disc
+        pts = np.array([0.5, 0.5, 0.5]) + np.c_[disc, 0.09 * eps * xi]
+        o, (x, y, z, hh), (A, B, gA, gB) = _s14_oracle(oracle_mod, pts, h)
+        ratio = _m2_ratio(o)
+        m0, m1, m2 = o.moments()
+        S0, S1, G0, G1 = o.rk_sums()
+        assert np.abs(S0 - 1).max() < 1e-12
+        for i in range(20):
+            if not (1e-5 < ratio[i] < 1e-3) or abs(ratio[i] / 1e-4 - 1) < 1e-6:
+                continue
+            first = np.abs(S1[:, i]).max() / h
+            if ratio[i] <= 1e-4:
+                below += 1
+                lo_r.append(ratio[i])
+                assert np.all(B[:, i] == 0.0)
+                assert np.allclose(S1[:, i], A[i] * m1[:, i], rtol=1e-10, atol=1e-14)
+                assert first > 1e-6, "the neighbourhood is lopsided, so without B the first moment cannot vanish"
+            else:
+                above += 1
+                hi_r.append(ratio[i])
+                assert np.any(B[:, i] != 0.0)
+                assert first < 1e-9, f"first-moment condition broken at ratio {ratio[i]:.3e}"
+    # both decades next to the line are populated, close to it as well as far from it
+    assert below >= 20 and above >= 20
+    assert min(lo_r) < 2e-5 and max(lo_r) > 5e-5 and min(hi_r) < 2e-4 and max(hi_r) > 5e-4
+
+
+def test_S14_fixture_ratios_are_what_DESIGN_says(tiny, clustered):
+    """DESIGN.md S14 quotes the smallest det m2 / (tr m2 / 3)^3 of the CPU fixtures; keep those numbers honest.  The lattice-like
+    set is nearly isotropic; the 18^3 Plummer fixture has particles at the rim of the sphere with one-sided neighbourhoods."""
+    r_tiny = _m2_ratio(tiny[1])
+    r_cl = _m2_ratio(clustered[1])
+    print(f"[S14] min ratio tiny_uniform 16^3: {r_tiny.min():.3e}; clustered 18^3: {r_cl.min():.3e}, "
+          f"below 1e-3: {(r_cl < 1e-3).sum()}, below 1e-4 (fallback): {(r_cl <= 1e-4).sum()} of {r_cl.size}")
+    assert r_tiny.min() > 0.3
+    assert r_cl.min() > 1e-5
+    assert ((clustered[2]["B"] == 0).all(axis=0) == (r_cl <= 1e-4)).all()
