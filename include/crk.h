@@ -169,6 +169,43 @@ int  crk_evolve_h(crk_ctx* c, float* h_new);
 int  crk_hydro_derivs_active(crk_ctx* c, const uint8_t* active, const float* vx, const float* vy, const float* vz,
                              const float* u, float* ax, float* ay, float* az, float* dudt);
 
+/* ---- for callers that must not allocate device memory: the space-filling-curve order without a context ----------------
+ * Who this is for.  A simulation code that claims nearly all of the device memory for its own arena at start-up (HACC-style
+ * hosts do) leaves nothing for a library's cudaMalloc later on, and a time step that has gravity and hydro kernels in
+ * flight on several streams cannot afford one either: cudaMalloc and cudaFree stall the whole device until everything
+ * queued has drained.  Every other entry point of this header works on a crk_ctx, which grows its scratch buffers with
+ * cudaMalloc on demand.  This one does not: it needs no context and makes no cudaMalloc / cudaFree / cudaMallocHost call,
+ * now or later.
+ * What it does.  The first half of crk_build_cells (section 3.3): validates the input as crk_build_cells
+ * does, forms the Hilbert keys on the grid whose cells are half the smallest h (at most 16 bits per axis), sorts them
+ * with the library's stable 8-bit LSD radix sort, and writes perm[k] = caller index of the k-th particle along the curve
+ * -- bit for bit what crk_get_perm returns after a crk_build_cells of the same x, y, z, h on a fresh context with the same
+ * box.  A caller can use it to put its own arrays in the order in which 32 consecutive particles form a compact leaf.
+ * Arguments.  x, y, z, h: device float[n], read only.  perm: device int32[n], written.  box as in crk_params.  n from 0
+ * (nothing is done) to CRK_NOALLOC_MAX_N; a larger n is refused with CRK_EINVAL before anything is launched.  errbuf:
+ * host char[errbuf_len] or NULL; receives a one-line message when the return value is not CRK_OK.
+ * Where the scratch lives.  The sort's working set (two key and two index buffers, the packed copy of the input that the
+ * key kernel writes, the digit histograms and their scan, two status words; CRK_NOALLOC_SCRATCH_BYTES = about 10.3 MB for
+ * CRK_NOALLOC_MAX_N = 262 144 particles) is a fixed array inside the library's device image.  Every GPU onto which the
+ * library's device code is loaded holds those bytes until the process exits, whether or not this function is ever called
+ * there.
+ * First call on a device.  The first call made with a given device current looks up the device address of that array
+ * (cudaGetSymbolAddress) and remembers it for that device; make this first call outside any stream capture, e.g. once
+ * during start-up with n = 0.  Later calls on that device only launch kernels, two small device-to-host copies and one
+ * device-to-device copy on `cuda_stream`.
+ * Sharing.  All calls on one device use the same array, and it still holds what the previous call left there.  The function
+ * clears the two status words it needs at zero itself, on the stream, at the start of each call; everything else is
+ * overwritten before it is read.  Two calls whose GPU work can overlap (different streams, or different host threads) race
+ * on the array and give garbage: serialise them.
+ * Synchronisation and errors.  Synchronises `cuda_stream` twice (after measuring the smallest h, and at the end to read
+ * the range flag), so perm is complete on return.  CRK_EINVAL: null pointer with n > 0, n < 0, n > CRK_NOALLOC_MAX_N or box
+ * <= 0; CRK_ERANGE: a position outside [0, box) or an h outside (0, box/2) (perm is then unspecified); CRK_ECUDA: a CUDA call
+ * failed.                                                                                                              */
+#define CRK_NOALLOC_MAX_N 262144
+#define CRK_NOALLOC_SCRATCH_BYTES 10765056
+int  crk_sfc_order_noalloc(void* cuda_stream, int64_t n, const float* x, const float* y, const float* z, const float* h,
+                           float box, int32_t* perm, char* errbuf, int errbuf_len);
+
 /* ---- diagnostics ---- */
 const char* crk_last_error(const crk_ctx* c);
 int  crk_get_perm(crk_ctx* c, int32_t* perm);        /* device int32[n]: perm[k] = caller index of sorted slot k   */

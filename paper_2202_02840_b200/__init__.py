@@ -16,6 +16,8 @@ from .binding import (  # noqa: F401
     crk_step_derivs,
     crk_step_derivs_host,
     crk_measure_fp32_peak,
+    crk_sfc_order_noalloc,
+    NOALLOC_MAX_N,
     library_path,
     EXPORTED_SYMBOLS,
 )

@@ -13,7 +13,9 @@ EXPORTED_SYMBOLS = (
     "crk_create", "crk_destroy", "crk_build_cells", "crk_volumes", "crk_rk_coefficients", "crk_hydro_derivs",
     "crk_step_derivs", "crk_step_derivs_host", "crk_hydro_derivs_active", "crk_compatible_energy", "crk_evolve_h", "crk_timestep", "crk_kdk_step", "crk_last_error", "crk_get_perm", "crk_get_gradv", "crk_get_leaf_segments", "crk_get_stats",
     "crk_reset_stats", "crk_set_timing", "crk_get_leaf_list", "crk_measure_fp32_peak", "crk_measure_fp32_peak_3reg",
+    "crk_sfc_order_noalloc",
 )
+NOALLOC_MAX_N = 262144       # CRK_NOALLOC_MAX_N of include/crk.h
 
 _ERR = {0: "CRK_OK", -1: "CRK_EINVAL", -2: "CRK_ERANGE", -3: "CRK_ENOMEM", -4: "CRK_ECUDA", -5: "CRK_ESTATE"}
 
@@ -88,6 +90,7 @@ def _load():
     L.crk_measure_fp32_peak.restype = C.c_double
     L.crk_measure_fp32_peak_3reg.argtypes = [vp, C.c_int, C.POINTER(C.c_float)]
     L.crk_measure_fp32_peak_3reg.restype = C.c_double
+    L.crk_sfc_order_noalloc.argtypes = [vp, i64, vp, vp, vp, vp, C.c_float, vp, C.c_char_p, C.c_int]
     _lib = L
     return L
 
@@ -301,6 +304,33 @@ def crk_step_derivs(ctx: Crk, x, y, z, h, vx, vy, vz, m, u):
 
 def crk_step_derivs_host(ctx: Crk, x, y, z, h, vx, vy, vz, m, u, out):
     return ctx.step_derivs_host(x, y, z, h, vx, vy, vz, m, u, out)
+
+
+def crk_sfc_order_noalloc(x, y, z, h, box: float, perm, stream=None):
+    """Curve order of up to NOALLOC_MAX_N particles for callers that must not allocate device memory (a host code whose own
+    arena already holds the whole GPU, or one that cannot take the device-wide stall of a cudaMalloc inside a time step):
+    the library works in a fixed array that is part of its device image instead of cudaMalloc'ed buffers.  x, y, z, h:
+    float32 CUDA tensors of one length n; perm: an int32 CUDA tensor of n elements that the CALLER provides (this wrapper
+    makes no tensor either) and that receives what Crk.perm() gives after build_cells of the same input.  Calls share the
+    array: do not let two of them overlap on the GPU.  The first call on a device looks the array up; make it outside any
+    stream capture.  Raises CrkError with the library's message (n too large, input out of range, CUDA failure)."""
+    L = _load()
+    if not torch.cuda.is_available():
+        raise RuntimeError("libcrk needs a CUDA device; there is no CPU fallback")
+    n = int(x.numel())
+    for t in (y, z, h, perm):
+        if int(t.numel()) != n:
+            raise ValueError("x, y, z, h and perm must have one length")
+    st = stream if stream is not None else torch.cuda.current_stream()
+    msg = C.create_string_buffer(256)
+    if n == 0:
+        args = [None] * 4 + [C.c_float(box), None]
+    else:
+        args = [_dev(t) for t in (x, y, z, h)] + [C.c_float(box), _dev(perm, torch.int32)]
+    rc = L.crk_sfc_order_noalloc(C.c_void_p(st.cuda_stream), n, *args, msg, len(msg))
+    if rc != 0:
+        raise CrkError(rc, msg.value.decode())
+    return perm
 
 
 def crk_measure_fp32_peak(repeats=5, three_reg=False):

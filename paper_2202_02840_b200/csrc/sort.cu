@@ -5,6 +5,8 @@
 // the sorted sequence into contiguous 32-particle leaves (tree.cu).  Every kernel here streams keys/payload once per pass.
 #include "crk_internal.cuh"
 #include <algorithm>
+#include <mutex>
+#include <stdarg.h>
 
 namespace {
 
@@ -401,4 +403,153 @@ int crk_sort_particles(crk_ctx* c, const float* x, const float* y, const float* 
         (const float4*)c->posh_orig.p, (const uint32_t*)c->perm, n, nl, (float4*)c->posh.p, (float4*)c->leaf_lo.p,
         (float4*)c->leaf_hi.p);
     return crk_check_launch(c, "k_gather_leaves");
+}
+
+// ---- crk_sfc_order_noalloc (include/crk.h): the sort above for callers that must not allocate --------------------------
+// Hosts that hand the whole device to their own arena at start-up, or that cannot take the device-wide stall of a
+// cudaMalloc in the middle of a time step, get the curve order from here: same kernels, same launch order as
+// crk_measure_hmin + crk_sort_particles, but every buffer the sort needs is a slice of ONE array that is part of the
+// library's device image.  Nothing below calls cudaMalloc, cudaFree, cudaMallocHost or anything that does.
+namespace {
+
+constexpr size_t na_al(size_t b) { return (b + 255) & ~(size_t)255; }
+constexpr size_t NA_N = CRK_NOALLOC_MAX_N;
+constexpr size_t NA_NBLK = (NA_N + SORT_TILE - 1) / SORT_TILE;
+constexpr size_t NA_HIST_WORDS = (size_t)RADIX * NA_NBLK + 1;      // digit-major histogram; its scan has one entry more
+constexpr size_t NA_SCAN_WORDS = 4096;                             // block sums of the scan (40 words at the maximal n)
+constexpr size_t NA_OFF_FLAG = 0;                                  // FW_WORDS status words; FW_ERROR and FW_HMIN are used
+constexpr size_t NA_OFF_KEYS0 = NA_OFF_FLAG + na_al(FW_WORDS * sizeof(int));
+constexpr size_t NA_OFF_KEYS1 = NA_OFF_KEYS0 + na_al(NA_N * sizeof(uint64_t));
+constexpr size_t NA_OFF_VALS0 = NA_OFF_KEYS1 + na_al(NA_N * sizeof(uint64_t));
+constexpr size_t NA_OFF_VALS1 = NA_OFF_VALS0 + na_al(NA_N * sizeof(uint32_t));
+constexpr size_t NA_OFF_POSH = NA_OFF_VALS1 + na_al(NA_N * sizeof(uint32_t));
+constexpr size_t NA_OFF_HIST = NA_OFF_POSH + na_al(NA_N * sizeof(float4));
+constexpr size_t NA_OFF_OFFS = NA_OFF_HIST + na_al(NA_HIST_WORDS * sizeof(uint32_t));
+constexpr size_t NA_OFF_SCAN = NA_OFF_OFFS + na_al(NA_HIST_WORDS * sizeof(uint32_t));
+constexpr size_t NA_BYTES = NA_OFF_SCAN + na_al(NA_SCAN_WORDS * sizeof(uint32_t));
+static_assert(NA_BYTES == CRK_NOALLOC_SCRATCH_BYTES, "include/crk.h states the size of the fixed scratch array");
+
+// The scratch itself.  In HOST code this name is only a handle for the runtime's symbol calls -- it is not a device
+// address, and a kernel handed `na_scratch` directly would fault (or, on a system where the GPU can reach host memory,
+// quietly work on the wrong bytes).  Host code therefore asks cudaGetSymbolAddress for the device's copy, once per device.
+static __device__ __align__(256) unsigned char na_scratch[NA_BYTES];
+
+constexpr int NA_MAX_DEVICES = 64;
+unsigned char* na_dev_ptr[NA_MAX_DEVICES] = {};   // device address of na_scratch on device d, 0 = not looked up yet
+std::mutex na_mu;                                  // guards na_dev_ptr (set-up only; it does not serialise the GPU work)
+
+int na_fail(char* errbuf, int errbuf_len, int code, const char* fmt, ...) {
+    if (errbuf && errbuf_len > 0) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(errbuf, (size_t)errbuf_len, fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+// device address of the scratch array on the CURRENT device; looked up on the first call made with that device current
+int na_scratch_for_current_device(unsigned char** out, char* errbuf, int errbuf_len) {
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return na_fail(errbuf, errbuf_len, CRK_ECUDA, "cudaGetDevice: %s", cudaGetErrorString(e));
+    if (dev < 0 || dev >= NA_MAX_DEVICES)
+        return na_fail(errbuf, errbuf_len, CRK_ECUDA, "crk_sfc_order_noalloc: device ordinal %d is beyond the %d this entry point keeps track of", dev, NA_MAX_DEVICES);
+    std::lock_guard<std::mutex> lock(na_mu);
+    if (!na_dev_ptr[dev]) {
+        unsigned char* p = nullptr;
+        e = cudaGetSymbolAddress((void**)&p, na_scratch);
+        if (e != cudaSuccess || !p) {
+            cudaGetLastError();
+            return na_fail(errbuf, errbuf_len, CRK_ECUDA, "cudaGetSymbolAddress(fixed scratch array) on device %d: %s", dev, cudaGetErrorString(e));
+        }
+        na_dev_ptr[dev] = p;
+    }
+    *out = na_dev_ptr[dev];
+    return CRK_OK;
+}
+
+#define NA_CUDA(call)                                                                                                   \
+    do {                                                                                                                \
+        cudaError_t e__ = (call);                                                                                       \
+        if (e__ != cudaSuccess) return na_fail(errbuf, errbuf_len, CRK_ECUDA, "crk_sfc_order_noalloc: %s: %s", #call, cudaGetErrorString(e__)); \
+    } while (0)
+
+}  // namespace
+
+extern "C" int crk_sfc_order_noalloc(void* cuda_stream, int64_t n, const float* x, const float* y, const float* z, const float* h,
+                                     float box, int32_t* perm, char* errbuf, int errbuf_len) {
+    if (errbuf && errbuf_len > 0) errbuf[0] = 0;
+    if (n < 0) return na_fail(errbuf, errbuf_len, CRK_EINVAL, "crk_sfc_order_noalloc: n = %lld is negative", (long long)n);
+    if (n > (int64_t)NA_N)
+        return na_fail(errbuf, errbuf_len, CRK_EINVAL,
+                       "crk_sfc_order_noalloc: n = %lld exceeds CRK_NOALLOC_MAX_N = %lld, the capacity of the fixed scratch array; "
+                       "use crk_build_cells + crk_get_perm (which allocate) for larger sets",
+                       (long long)n, (long long)NA_N);
+    if (!(box > 0.f)) return na_fail(errbuf, errbuf_len, CRK_EINVAL, "crk_sfc_order_noalloc: box must be positive");
+    if (n > 0 && (!x || !y || !z || !h || !perm)) return na_fail(errbuf, errbuf_len, CRK_EINVAL, "crk_sfc_order_noalloc: null pointer");
+    // set-up of this device (first call only): also with n = 0, so that a start-up call outside any capture does it
+    unsigned char* S = nullptr;
+    CRK_TRY(na_scratch_for_current_device(&S, errbuf, errbuf_len));
+    if (n == 0) return CRK_OK;
+
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    int* flag = (int*)(S + NA_OFF_FLAG);
+    uint64_t* keys[2] = {(uint64_t*)(S + NA_OFF_KEYS0), (uint64_t*)(S + NA_OFF_KEYS1)};
+    uint32_t* vals[2] = {(uint32_t*)(S + NA_OFF_VALS0), (uint32_t*)(S + NA_OFF_VALS1)};
+    float4* posh_orig = (float4*)(S + NA_OFF_POSH);
+    uint32_t* hist = (uint32_t*)(S + NA_OFF_HIST);
+    uint32_t* offs = (uint32_t*)(S + NA_OFF_OFFS);
+    uint32_t* scan_tmp = (uint32_t*)(S + NA_OFF_SCAN);
+
+    // launch bookkeeping of the helpers above goes through a context object; this one lives on the host stack, owns nothing
+    // and is never passed to anything that allocates
+    crk_ctx tmp;
+    tmp.stream = st;
+    tmp.prm.box = box;
+    tmp.n = n;
+    tmp.err[0] = 0;
+
+    // the array keeps what the last call left in it: the two status words (range flag, encoded smallest h) must start at zero
+    NA_CUDA(cudaMemsetAsync(flag, 0, FW_WORDS * sizeof(int), st));
+    k_h_min<<<(unsigned)std::min<int64_t>((n + 255) / 256, 1184), 256, 0, st>>>(h, n, flag);
+    NA_CUDA(cudaGetLastError());
+    int enc_host = 0;
+    NA_CUDA(cudaMemcpyAsync(&enc_host, flag + FW_HMIN, sizeof(int), cudaMemcpyDeviceToHost, st));
+    NA_CUDA(cudaStreamSynchronize(st));
+    const int bits = crk_key_bits_from_hmin(&tmp, (uint32_t)enc_host);     // as the first crk_build_cells of a context
+
+    const int nblk = (int)((n + SORT_TILE - 1) / SORT_TILE);
+    {   // block sums of the scan must fit their slice (they do for every n <= CRK_NOALLOC_MAX_N; checked, not assumed)
+        size_t need = 0;
+        for (int64_t m = (int64_t)RADIX * nblk + 1; m > 1;) {
+            const int64_t nb = (m + SCAN_TILE - 1) / SCAN_TILE;
+            need += (size_t)(2 * nb + 2);
+            if (nb <= 1) break;
+            m = nb + 1;
+        }
+        if (need > NA_SCAN_WORDS || (size_t)RADIX * nblk + 1 > NA_HIST_WORDS)
+            return na_fail(errbuf, errbuf_len, CRK_EINVAL, "crk_sfc_order_noalloc: n = %lld does not fit the fixed scratch array", (long long)n);
+    }
+    k_keys_pack<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(x, y, z, h, n, box, bits, keys[0], vals[0], posh_orig, flag);
+    NA_CUDA(cudaGetLastError());
+    NA_CUDA(cudaFuncSetAttribute(k_radix_scatter, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sizeof(ScatterSmem)));
+    int cur = 0;
+    for (int shift = 0; shift < 3 * bits; shift += RADIX_BITS) {
+        k_radix_hist<<<nblk, SORT_THREADS, 0, st>>>(keys[cur], n, shift, hist, nblk);      // writes every entry it owns: no clearing
+        NA_CUDA(cudaGetLastError());
+        if (scan_rec(&tmp, hist, offs, (int64_t)RADIX * nblk, (int64_t)RADIX * nblk + 1, scan_tmp) != CRK_OK)
+            return na_fail(errbuf, errbuf_len, CRK_ECUDA, "crk_sfc_order_noalloc: %s", tmp.err);
+        k_radix_scatter<<<nblk, SORT_THREADS, sizeof(ScatterSmem), st>>>(keys[cur], vals[cur], keys[cur ^ 1], vals[cur ^ 1], n, shift,
+                                                                         offs, nblk);
+        NA_CUDA(cudaGetLastError());
+        cur ^= 1;
+    }
+    NA_CUDA(cudaMemcpyAsync(perm, vals[cur], (size_t)n * sizeof(int32_t), cudaMemcpyDeviceToDevice, st));
+    int err_host = 0;
+    NA_CUDA(cudaMemcpyAsync(&err_host, flag + FW_ERROR, sizeof(int), cudaMemcpyDeviceToHost, st));
+    NA_CUDA(cudaStreamSynchronize(st));
+    if (err_host & 1)
+        return na_fail(errbuf, errbuf_len, CRK_ERANGE, "input out of range: need 0 <= x,y,z < box and 0 < h < box/2");
+    return CRK_OK;
 }
