@@ -33,7 +33,7 @@ def build(force: bool = False, verbose: bool = False, checked: bool = False) -> 
     if not force and os.path.exists(lib) and os.path.getmtime(lib) >= _newest_dep():
         return lib
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    flags = list(NVCC_FLAGS) + (["-Xptxas", "-v"] if verbose else []) + (["-DCRK_CHECKED"] if checked else []) + os.environ.get("CRK_NVCC_EXTRA", "").split()
+    flags = list(NVCC_FLAGS) + (["-Xptxas", "-v"] if verbose else []) + (["-DCRK_CHECKED"] if checked else [])
     objs = []
 
     def compile_one(src):

@@ -27,7 +27,8 @@ enum { EV_BUILD0 = 0, EV_SORTED, EV_TREE1, EV_BUILD1, EV_VOL0, EV_VOL1, EV_RK0, 
 //   ell[k][l] = k-th entry of lane l: candidate index | CRK_ELL_SYM (h_i^2 <= r2 < h_j^2: a pair of the symmetric set that
 //               is not in the lane's gather set; also the padding of rows beyond cnt[l]: CRK_ELL_SYM | slot 0) | CRK_ELL_WRAP
 //               (pair crosses the periodic boundary); lane l owns cnt[l]
-//               entries; CRK_SEG_WRAP: some entry of the segment may carry CRK_ELL_WRAP
+//               entries; CRK_SEG_WRAP: some entry of the segment may carry CRK_ELL_WRAP (a diagnostic of the builder, shown by
+//               crk_get_leaf_segments; the sweeps test the per-entry flag and do not read it)
 #define CRK_CCAP 384             // candidates per segment (tile capacity of the sweeps)
 #define CRK_CAND_STRIDE 384      // u32 per leaf in cand_first (the sweeps read it in 16-byte groups)
 #define CRK_QCAP 128             // entries per lane per segment

@@ -13,17 +13,6 @@
 // Equation numbers refer to /root/reference/PAPER.md; the closed forms of A, B, grad A, grad B are derived in DESIGN.md.
 #include "crk_internal.cuh"
 
-#ifdef CRK_PROBE
-// development probe (never in the product build): per sweep (index = planes in the tile) the summed cycles a group spends
-// staging, the summed cycles of its whole leaf sweep, and the number of leaves
-__device__ unsigned long long crk_probe[48];
-extern "C" int crk_probe_read(unsigned long long* out, int reset) {
-    cudaDeviceSynchronize();
-    cudaMemcpyFromSymbol(out, crk_probe, sizeof(crk_probe));
-    if (reset) { unsigned long long z[48] = {0}; cudaMemcpyToSymbol(crk_probe, z, sizeof(z)); }
-    return 0;
-}
-#endif
 
 namespace {
 
@@ -70,7 +59,6 @@ struct SweepArgs {
 struct Seg {
     const uint16_t* ell;
     int C, K, ct;
-    bool wrap;               // some entry of the segment may cross the periodic boundary
     uint32_t next;
 };
 
@@ -127,7 +115,7 @@ __device__ __forceinline__ void group_sync(int lg) {
 // ---- persistent groups: work distribution and metadata prefetch --------------------------------------------------------
 // A group (WPL warps) serves one leaf at a time and keeps taking leaves from a global counter until none is left; the
 // kernels are launched with as many CTAs as are resident at once.  (One CTA per leaf cost the force sweep 19 % of its time
-// in CTA turnover and 27 % in the dependent loads of the prologue -- measured with clock64 probes, profiles/r02_notes.md.)
+// in CTA turnover and 27 % in the dependent loads of the prologue -- measured with clock64 probes in round 2.)
 // the counter's answer is only looked at (resolve_slot) when the leaf is needed, one leaf later: no thread waits for the atomic
 __device__ __forceinline__ unsigned int grab_slot(const SweepArgs& a) { return atomicAdd(a.sched, 1u); }
 __device__ __forceinline__ long long resolve_slot(const SweepArgs& a, unsigned int slot) {
@@ -188,7 +176,7 @@ struct NoHook {
 };
 // init(tile_s) runs once, after the first segment is staged: slots 0..31 of that tile are the leaf's own particles in lane
 // order (lists.cu), so a sweep can take its i-state from there instead of loading it from global memory.
-// (Measured and not kept, profiles/r02_notes.md: a second, branch-free instantiation of the row loop for segments without
+// (Measured in round 2 and not kept: a second, branch-free instantiation of the row loop for segments without
 // boundary-crossing entries -- 172 instead of 190 instructions per pair of k_forces, but ptxas then sinks the shared loads
 // next to their uses and the sweep loses 1.6 ms to short-scoreboard stalls.)
 // staged() runs once per leaf between the issue of the first segment's copies and B2, i.e. while the copies are in flight and
@@ -207,15 +195,9 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
     uint32_t unit = 0;                                            // arena unit of the segment being staged (0: not known yet)
     unsigned int pend = 0xffffffffu;                              // thread 0: the work item taken for the leaf after next (raw counter value)
     next_leaf = -1;
-#ifdef CRK_PROBE
-    long long pr_stage = 0, pr_t0 = clock64();
-#endif
     for (;;) {
         asm volatile("cp.async.wait_all;" ::: "memory");
         group_sync<WPL>(lg);                                   // B1
-#ifdef CRK_PROBE
-        const long long pr_s0 = clock64();
-#endif
         const uint4 h0 = m->hdr;
         if (first) {
             unit = h0.w;
@@ -232,7 +214,6 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
         Seg s;
         s.next = h0.x;
         s.C = (int)(h0.y & 0x7fffu);
-        s.wrap = (h0.y & CRK_SEG_WRAP) != 0u;
         s.K = (int)(h0.y >> 16);
         s.ct = (int)m->cnt[lane];
         s.ell = (const uint16_t*)(a.arena + unit + CRK_SEG_HDR_UNITS + (first ? 0 : ((s.C + 3) >> 2)));
@@ -247,41 +228,13 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
             const uint32_t pc = (uint32_t)(tg & (ROWP - 1));       // NT is a multiple of ROWP: a thread always copies the same piece
             const uint32_t dst0 = tile_s + pc * PSTRIDE;
             const float4* src0 = rows_src + pc;
-#ifdef CRK_STAGE_PERCAND
-            // one candidate per thread, all its pieces: fewer instructions per copy, 32 rows per warp-wide LDGSTS
-            for (int c = tg; c < s.C; c += NT) {
-                const float4* src = rows_src + (int64_t)m->cand[c] * RSTRIDE;
-#pragma unroll
-                for (int p = 0; p < ROWP; ++p) cp_async16(tile_s + (uint32_t)p * PSTRIDE + (uint32_t)c * 16u, src + p);
-            }
-#elif defined(CRK_STAGE_LDG)
-            // through registers: a warp-wide LDG.128 of 32 / ROWP full rows is served line by line, an LDGSTS thread by thread
-            constexpr int SB = 5;
-            for (int f0 = tg; f0 < total; f0 += NT * SB) {
-                float4 v[SB];
-#pragma unroll
-                for (int b = 0; b < SB; ++b) {
-                    const int f = f0 + b * NT;
-                    if (f < total) v[b] = __ldg(src0 + (int64_t)m->cand[f >> RS] * RSTRIDE);
-                }
-#pragma unroll
-                for (int b = 0; b < SB; ++b) {
-                    const int f = f0 + b * NT;
-                    if (f < total) asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(dst0 + (uint32_t)(f >> RS) * 16u), "f"(v[b].x), "f"(v[b].y), "f"(v[b].z), "f"(v[b].w) : "memory");
-                }
-            }
-#else
 #pragma unroll 4
             for (int f = tg; f < total; f += NT) {
                 const int c = f >> RS;
                 const uint32_t j = m->cand[c];
                 CRK_CHECK(a.flag, (int64_t)j < a.np, 9);                                    // candidate index
-#ifdef CRK_EXP_HALFSTAGE
-                if (ROWP == 8 && (c & 1) && c >= 32) continue;
-#endif
                 cp_async16(dst0 + (uint32_t)c * 16u, src0 + (int64_t)j * RSTRIDE);
             }
-#endif
         }
         if (PLANES > 0) {
             for (int c0 = 0; c0 < s.C; c0 += NT * 2) {
@@ -309,25 +262,13 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
         }
         const bool last = (s.next == 0u);
         if (first) staged();
-#ifdef CRK_PROBE
-        const long long pr_s1 = clock64();
-#endif
         if (last && tg == 0 && next_leaf >= 0) pend = grab_slot(a);          // looked at when the leaf ends
         group_sync<WPL>(lg);                                   // B2
-#ifdef CRK_PROBE
-        if (tg == 0) {
-            atomicAdd(&crk_probe[(ROWP + PLANES) * 4 + 3], (unsigned long long)(pr_s1 - pr_s0));
-            atomicAdd(&crk_probe[40 + ((ROWP + PLANES) & 7)], (unsigned long long)(clock64() - pr_s1));
-        }
-#endif
         if (!last) issue_meta<NT>(m, a, 0, s.next, tg);
         else if (next_leaf >= 0) issue_meta<NT>(m, a, next_leaf, 0u, tg);
         cp_async_commit();
         asm volatile("cp.async.wait_group 1;" ::: "memory");   // the state copies (the metadata copy may still be in flight)
         group_sync<WPL>(lg);                                   // B3
-#ifdef CRK_PROBE
-        pr_stage += clock64() - pr_s0;
-#endif
         if (first) {
             init(tile_s);
             first = false;
@@ -362,12 +303,7 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
                 for (int p = 0; p < NPRE; ++p) nxt[p] = lds128(san + (uint32_t)p * PSTRIDE);
                 CRK_CHECK(a.flag, k >= mine || (int)(e[q] & CRK_ELL_MASK) < s.C, 10);       // entry -> staged slot
                 CRK_CHECK(a.flag, SYM || k < mine || (e[q] & CRK_ELL_SYM) != 0u, 11);       // padding carries the skip flag
-#ifdef CRK_EXP_NOCONFLICT   // timing experiment only (wrong results): every lane of a quarter-warp reads a different bank group
-                if (k < mine && (SYM || !(e[q] & CRK_ELL_SYM)))
-                    pair(tile_s + (((e[q] & CRK_ELL_MASK) & ~31u) | (uint32_t)lane) * 16u, (e[q] & CRK_ELL_WRAP) != 0u, cur);
-#else
                 if (SYM ? (k < mine) : !(e[q] & CRK_ELL_SYM)) pair(sa, (e[q] & CRK_ELL_WRAP) != 0u, cur);
-#endif
                 sa = san;
 #pragma unroll
                 for (int p = 0; p < NPRE; ++p) cur[p] = nxt[p];
@@ -382,13 +318,6 @@ __device__ __forceinline__ uint32_t leaf_sweep(const SweepArgs& a, const float4*
         }
         unit = s.next;
     }
-#ifdef CRK_PROBE
-    if (tg == 0) {
-        atomicAdd(&crk_probe[(ROWP + PLANES) * 4 + 0], (unsigned long long)pr_stage);
-        atomicAdd(&crk_probe[(ROWP + PLANES) * 4 + 1], (unsigned long long)(clock64() - pr_t0));
-        atomicAdd(&crk_probe[(ROWP + PLANES) * 4 + 2], 1ull);
-    }
-#endif
     return count;
 }
 
@@ -582,12 +511,10 @@ __device__ __forceinline__ void wendland_folded(float eta, float& Wt, float& Dt)
 // the compiler to contract differently), so the staged calls and crk_step_derivs produce identical bits.
 // The epilogue with GV also forms P = (gamma-1) rho u (Eq. 4, unclamped) and c_s = sqrt(gamma (gamma-1) max(u,0)) (S12) and
 // writes the packed force-sweep state of the particle.
-#ifndef CRK_RK_MINB
-#define CRK_RK_MINB 8
-#endif
 constexpr int W2_WPC = 2;
+constexpr int RK_MINB = 8;        // resident CTAs per SM the merged moments + grad v sweep is compiled for
 template <bool MOM, bool GV>
-__global__ void __launch_bounds__(W2_WPC * 32, (MOM && GV) ? CRK_RK_MINB : (GV ? 8 : 10))
+__global__ void __launch_bounds__(W2_WPC * 32, (MOM && GV) ? RK_MINB : (GV ? 8 : 10))
 k_rk(SweepArgs a, const float* __restrict__ u_s, float* __restrict__ gv_full) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
     // tile: GV -> the candidates' entries of the compact array xv, (x,y,z,1/h) and (vx,vy,vz,V): one 32-byte sector each;
@@ -923,11 +850,8 @@ __device__ __forceinline__ PairF force_pair(const ForceConst& k, const PState& I
 
 // One group = one CTA of W5_WPL warps: they share the tile of the leaf's candidates and split each lane's entries by rows;
 // four persistent CTAs are resident per SM, so one group's staging overlaps the other three's pair math (with the copies
-// switched off the sweep is 8 % faster, no more: profiles/r02_notes.md #29).  2 .. 6 warps per leaf were measured (#26).
-#ifndef CRK_W5_WPL
-#define CRK_W5_WPL 4
-#endif
-constexpr int W5_WPL = CRK_W5_WPL;
+// switched off the sweep is 8 % faster, no more).  2 .. 6 warps per leaf were measured in round 2.
+constexpr int W5_WPL = 4;
 // The epilogue of a leaf (sum of the W5_WPL partial results in warp order, division by the mass, stores through the
 // permutation) is deferred into the staging window of the group's NEXT leaf, where the warps only wait for their copies: the
 // partial sums and what the stores need travel through this record.  One record is enough: nobody reaches the rows of leaf
