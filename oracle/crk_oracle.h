@@ -16,9 +16,15 @@
  * grad v, momentum/energy pair antisymmetry are pinned by invariants; the limiter (phi_VL off r = 1, phi_ad), mu, Q and
  * the pair terms of Eqs. 17-18 are pinned against the paper's PRINTED forms rebuilt in numpy with the golden constants
  * (C_l, C_q, eps, eta_fold/eta_crit), incl. closed-form pairs (head-on approach, close approach in a linear flow).
+ * The zeroth-order fallback of solve_coef for a singular m2 (S14: B = 0, A = 1/m0, grad A = -A^2 grad m0) is pinned against
+ * the zeroth-moment constraint of PAPER.md:116, its gradient and finite differences of A on sets that span fewer than three
+ * dimensions; the position of the singularity line is pinned from both sides (first-moment condition holds above it, equals
+ * A m1 below it) within a factor ten (test_S14_*).
  * PARITY UNPINNED
  * (fixed by DESIGN.md readings only): Eq. 18 P_j-vs-P_i choice (S6), rho = m/V for unequal masses (S2),
- * c_s clamp max(u,0) (S12).
+ * c_s clamp max(u,0) (S12), and the VALUE 1e-4 of S14's threshold det m2 <= 1e-4 (tr m2 / 3)^3: the paper gives no number.
+ * A particle whose ratio lies within FP32 rounding of the line can take different branches here (FP64 sums) and in the CUDA
+ * library (FP32 sums); the parity fixtures stay a factor two away from it (smallest ratio 2.0e-4).
  */
 #ifndef CRK_ORACLE_H
 #define CRK_ORACLE_H
