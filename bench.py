@@ -229,6 +229,7 @@ def run_ours(args, rank, world, local_rank):
     sym_pairs = float(res[4].to(torch.int64).sum().item())
     pairs_per_step = 3.0 * gather_pairs + sym_pairs
     wstats = workload_stats(ps, cnt.cpu().numpy(), res[4].cpu().numpy(), ctx.leaf_segments().cpu().numpy().astype(np.uint32))
+    wstats["s14_fallback_particles"] = int(ctx.stats()["n_fallback"])     # particles with a singular m2 (S14)
     del cnt, res
     big = ps.n > 40_000_000 or args.no_next_rows        # 512^3: skip the next-row extras (they need copies of the state)
 

@@ -78,7 +78,9 @@ typedef struct {
     int64_t  n_active_leaves, n_halo_leaves;   /* of the last crk_hydro_derivs_active                                 */
     int32_t  rebuilds;        /* builds repeated since crk_create because the data outgrew the key width, the leaf-list
                                  capacity or the list arena the previous build had found (see crk_build_cells)        */
-    int32_t  reserved;
+    int32_t  n_fallback;      /* particles of the last crk_rk_coefficients whose second moment counted as singular, det m2 <=
+                                 1e-4 (tr m2 / 3)^3 (fewer than three dimensions spanned: thin sheets, n <= 3), and that therefore
+                                 got the zeroth-order correction only (B = 0; reading S14).  0 before that call       */
 } crk_stats;
 
 /* stream: a cudaStream_t (0 = default stream).  Returns CRK_OK and *out, or an error.                       */
@@ -220,7 +222,7 @@ int  crk_get_gradv(crk_ctx* c, float* gradv);         /* device float[9][n], ind
  * crosses the periodic boundary | K << 16, 0, arena unit}; C = candidate slots, K = rows of the entry block (layout:
  * csrc/crk_internal.cuh)                                                                                       */
 int  crk_get_leaf_segments(crk_ctx* c, uint32_t* seg);
-int  crk_get_stats(crk_ctx* c, crk_stats* out);       /* host struct                                                */
+int  crk_get_stats(crk_ctx* c, crk_stats* out);       /* host struct; synchronises the stream (reads n_fallback, the timings) */
 int  crk_reset_stats(crk_ctx* c);
 int  crk_set_timing(crk_ctx* c, int on);              /* record CUDA events around each pass (adds stream syncs when read) */
 /* leaf interaction list of leaf `leaf` (host buffer): entries leaf_index | bit31 (gather) | bit30 (periodic wrap);

@@ -37,7 +37,7 @@ class Stats(C.Structure):
                 ("ms_build", C.c_float), ("ms_volumes", C.c_float), ("ms_rk", C.c_float), ("ms_hydro", C.c_float),
                 ("ms_sort", C.c_float), ("ms_tree", C.c_float), ("ms_gradv", C.c_float), ("ms_forces", C.c_float),
                 ("ms_lists", C.c_float), ("timed_steps", C.c_int32), ("sort_passes", C.c_int32),
-                ("n_active_leaves", C.c_int64), ("n_halo_leaves", C.c_int64), ("rebuilds", C.c_int32), ("reserved", C.c_int32)]
+                ("n_active_leaves", C.c_int64), ("n_halo_leaves", C.c_int64), ("rebuilds", C.c_int32), ("n_fallback", C.c_int32)]
 
     def as_dict(self):
         return {k: getattr(self, k) for k, _ in self._fields_}

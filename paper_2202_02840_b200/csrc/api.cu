@@ -508,6 +508,11 @@ int crk_get_stats(crk_ctx* c, crk_stats* out) {
     out->n_active_leaves = c->n_active_leaves;
     out->n_halo_leaves = c->n_halo_leaves;
     out->rebuilds = c->st.rebuilds;
+    if (c->stage >= 3 && c->n > 0) {   // the coefficient sweep counted the particles that took the S14 fallback
+        CRK_CUDA(c, cudaMemcpyAsync(c->h_flag + FW_FALLBACK, (int*)c->flag.p + FW_FALLBACK, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+        CRK_CUDA(c, cudaStreamSynchronize(c->stream));
+        out->n_fallback = c->h_flag[FW_FALLBACK];
+    }
     if (c->timing && c->n > 0) {
         // mean over the completed steps still held in the event ring (all steps since crk_reset_stats if <= 64)
         CRK_CUDA(c, cudaStreamSynchronize(c->stream));

@@ -53,6 +53,7 @@ enum { FW_ERROR = 0,        // bit 0: input out of range (S13)
        FW_ARENA = 8,        // u64: arena units the neighbour lists need
        FW_SETMIXED = 10,    // 1: the supports of the set span more than a factor four (tree.cu: every leaf list built per leaf)
        FW_HOST_ACTIVE = 12, // host side only: crk_select_active
+       FW_FALLBACK = 13,    // particles whose m2 counted as singular in the last coefficient sweep (S14), pairs.cu k_rk
        FW_WORDS = 16 };
 
 // CRK_CHECKED builds (python -m paper_2202_02840_b200.build --checked -> libcrk_checked.so): every index the list builder and the
@@ -128,6 +129,11 @@ struct crk_ctx {
     DevBuf sched;                  // work counter of the persistent sweeps (pairs.cu)
     DevBuf host_stage;             // device staging for crk_step_derivs_host (13 float arrays)
     int* h_flag = nullptr;         // pinned host mirror
+    // launch geometry of the persistent sweeps (pairs.cu: persistent_grid), one entry per (kernel, shared memory, threads, device)
+    struct GridGeo { const void* kernel = nullptr; int smem = 0, threads = 0, dev = 0, per_sm = 0, sms = 0; };
+    static constexpr int GEO_CAP = 16;
+    GridGeo geo[GEO_CAP];
+    int n_geo = 0;
 };
 
 #define CRK_CUDA(c, call)                                                                          \

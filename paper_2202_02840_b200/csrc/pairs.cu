@@ -657,6 +657,7 @@ k_rk(SweepArgs a, const float* __restrict__ u_s, float* __restrict__ gv_full) {
                         for (int p = 0; p < 3; ++p) dB[c][p] = -(inv[p][0] * rhs[0] + inv[p][1] * rhs[1] + inv[p][2] * rhs[2]);
                     }
                 } else {   // S14: degenerate neighbourhood -> zeroth-order correction only
+                    atomicAdd((unsigned int*)a.flag + FW_FALLBACK, 1u);   // reported by crk_get_stats (rare: none on the BASELINE configs)
                     A = 1.0 / m0;
 #pragma unroll
                     for (int c = 0; c < 3; ++c) {
@@ -1040,22 +1041,28 @@ SweepArgs make_args(crk_ctx* c) {
 // work items; the work counter is zeroed on the stream first.  groups_per_cta = leaves a CTA serves concurrently.
 template <typename K>
 int persistent_grid(crk_ctx* c, K kernel, int threads, int smem, int groups_per_cta, int64_t items, unsigned* grid) {
-    // occupancy and SM count of a (kernel, shared-memory size) are asked for once per process, not once per launch
-    struct Geo { int smem = -1, per_sm = 0, sms = 0; };
-    static Geo geo;                                       // one instance per kernel (template instantiation)
-    if (geo.smem != smem) {
+    // occupancy and SM count of a (kernel, shared-memory size, device) are asked for once per context, not once per launch.
+    // The key is the kernel's ADDRESS: the template parameter K is only its function-pointer type, which k_volumes and both
+    // k_forces instantiations share, as do the three k_rk instantiations.
+    int dev = 0;
+    CRK_CUDA(c, cudaGetDevice(&dev));
+    const void* key = (const void*)kernel;
+    crk_ctx::GridGeo* g = nullptr;
+    for (int q = 0; q < c->n_geo; ++q)
+        if (c->geo[q].kernel == key && c->geo[q].smem == smem && c->geo[q].threads == threads && c->geo[q].dev == dev) g = &c->geo[q];
+    if (!g) {
         if (smem > 48 * 1024) CRK_CUDA(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        int per_sm = 0, dev = 0, sms = 0;
+        int per_sm = 0, sms = 0;
         CRK_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, (size_t)smem));
-        CRK_CUDA(c, cudaGetDevice(&dev));
         CRK_CUDA(c, cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
         if (per_sm < 1) {
             snprintf(c->err, sizeof(c->err), "a sweep kernel does not fit on an SM (%d bytes of shared memory)", smem);
             return CRK_ECUDA;
         }
-        geo.smem = smem; geo.per_sm = per_sm; geo.sms = sms;
+        g = &c->geo[c->n_geo < crk_ctx::GEO_CAP ? c->n_geo++ : crk_ctx::GEO_CAP - 1];   // a full table reuses its last entry
+        g->kernel = key; g->smem = smem; g->threads = threads; g->dev = dev; g->per_sm = per_sm; g->sms = sms;
     }
-    const int per_sm = geo.per_sm, sms = geo.sms;
+    const int per_sm = g->per_sm, sms = g->sms;
     const int64_t need = (items + groups_per_cta - 1) / groups_per_cta;
     const int64_t res = (int64_t)per_sm * sms;
     *grid = (unsigned)(need < res ? need : res);
@@ -1110,6 +1117,7 @@ int crk_launch_rk(crk_ctx* c, bool mom, bool gv, float* A, float* B, float* grad
     const int smem = W2_WPC * ((gv ? 2 : 1) * (int)PSTRIDE + (int)sizeof(Meta));
     const float* us = (const float*)c->u_s.p;
     unsigned grid = 0;
+    if (mom && !ids) CRK_CUDA(c, cudaMemsetAsync((int*)c->flag.p + FW_FALLBACK, 0, sizeof(int), c->stream));   // counts this sweep only
     if (mom && gv) {
         CRK_TRY(persistent_grid(c, k_rk<true, true>, W2_WPC * 32, smem, W2_WPC, items, &grid));
         a.sched = (unsigned int*)c->sched.p;
