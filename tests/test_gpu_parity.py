@@ -14,6 +14,7 @@ pytestmark = pytest.mark.gpu
 
 TOL_DERIV = 1e-4
 TOL_INV = 1e-5
+TOL_WORST = 1e-3       # per particle: |dv/dt error| against the particle's own scale (check_parity)
 TOL_SCALAR = 4e-6      # max-norm on V, rho, A.  Measured maxima over every case of this file (printed as [scalars]): V 1.3e-6,
                        # rho 1.3e-6 (n_h = 4, 268-term FP32 sums), A 1.8e-6 (non-default parameters); the bar is 2x the worst.
                        # Source: FP32 accumulation of 60-268 kernel terms, each through rsqrt.approx (2^-22) -- DESIGN.md 5.3
@@ -57,6 +58,8 @@ def gpu_eval(ps, stages=False):
 def check_parity(ps, g, o, oracle_gv=None, mask=None, label=""):
     """g: GPU outputs, o: oracle outputs (dicts).  mask: compare only these particles (windowed oracle)."""
     sel = slice(None) if mask is None else mask
+    if mask is None and "stats" in g:     # both sides took the S14 branch (singular m2 -> B = 0 exactly) for the same number of particles
+        assert g["stats"]["n_fallback"] == int((np.asarray(o["B"]) == 0.0).all(axis=0).sum()), label + " S14 fallback count"
     assert np.array_equal(g["nbr_count"][sel].astype(np.int64), o["nbr_count"][sel].astype(np.int64)), label + " nbr_count"
     assert np.array_equal(g["pair_count"][sel].astype(np.int64), o["pair_count"][sel].astype(np.int64)), label + " pair_count"
     e_s = [float(np.max(np.abs(g[k][sel] / o[k][sel] - 1))) for k in ("V", "rho", "A")]
@@ -75,6 +78,15 @@ def check_parity(ps, g, o, oracle_gv=None, mask=None, label=""):
     e_u = rel_l2(g["dudt"][sel], o["dudt"][sel])
     assert e_a < TOL_DERIV, f"{label} dv/dt rel L2 {e_a:.3e}"
     assert e_u < TOL_DERIV, f"{label} du/dt rel L2 {e_u:.3e}"
+    # a global norm is dominated by the particles with the largest derivatives (the cores of a clustered set): every particle
+    # is also held to TOL_WORST of its OWN scale -- the larger of its acceleration and the pressure-gradient scale
+    # (gamma - 1) u_i / h_i of a single pair term -- so that a wrong particle in a void cannot hide under the rms of the cores
+    scale = np.maximum(np.sqrt((acc_o.astype(np.float64) ** 2).sum(0)),
+                       (ps.gamma - 1.0) * np.abs(ps.u[sel].astype(np.float64)) / ps.h[sel].astype(np.float64))
+    err = np.sqrt(((acc_g.astype(np.float64) - acc_o) ** 2).sum(0))
+    worst = float((err / scale).max()) if err.size else 0.0
+    print(f"[worst particle] {label}: |dv/dt error| / max(|dv/dt|, (gamma-1) u/h) = {worst:.2e}")
+    assert worst < TOL_WORST, f"{label} worst particle {worst:.3e}"
     return e_a, e_u
 
 
@@ -207,6 +219,7 @@ def test_parity_singular_m2_fallback(n, oracle_mod):
     g = gpu_eval(ps)
     assert np.abs(od["B"]).max() == 0.0 and np.abs(od["gradB"]).max() == 0.0, "the oracle did not take the S14 branch"
     assert np.abs(g["B"]).max() == 0.0 and np.abs(g["gradB"]).max() == 0.0, "the kernel did not take the S14 branch"
+    assert g["stats"]["n_fallback"] == n, "crk_stats.n_fallback counts the particles that took it"
     assert np.array_equal(g["nbr_count"].astype(np.int64), od["nbr_count"].astype(np.int64))
     assert np.array_equal(g["pair_count"].astype(np.int64), od["pair_count"].astype(np.int64))
     assert np.allclose(g["V"], od["V"], rtol=TOL_SCALAR) and np.allclose(g["A"], od["A"], rtol=TOL_SCALAR)
@@ -674,11 +687,16 @@ def test_parity_config5_clustered_large(oracle_mod):
     Plummer generator at 512^3 = 134 M particles (32768 spheres), k-th-neighbour h with a range of ~50x.  Windows around the
     densest core, the emptiest void, the box centre and a box corner against the brute-force oracle, invariants on the
     full output.  (No all-particle count check: the oracle's uniform grid is quadratic in the densest cell of a clustered
-    set.)  Opt-in (CRK_TEST_LARGE=1): the generator's k-d-tree pass over 134 M points takes ~10 minutes of host time; the
-    output of the last run is kept in profiles/r02_config5_clustered_large.md."""
+    set.)  Runs by default (about five and a half minutes, most of it the generator's k-d-tree pass over 134 M points on the
+    host); CRK_TEST_LARGE=0 leaves it out, and it is skipped where the host or the GPU is too small to hold the configuration.
+    The output of the round-2 run is kept in profiles/r02_config5_clustered_large.md."""
     import os
-    if os.environ.get("CRK_TEST_LARGE", "0") != "1":
-        pytest.skip("set CRK_TEST_LARGE=1 to run the 134 M-particle clustered configuration")
+    if os.environ.get("CRK_TEST_LARGE", "1") == "0":
+        pytest.skip("CRK_TEST_LARGE=0: the 134 M-particle clustered configuration was left out on request")
+    torch = _torch()
+    import psutil
+    if psutil.virtual_memory().available < 60e9 or torch.cuda.get_device_properties(0).total_memory < 150e9:
+        pytest.skip("the 134 M-particle clustered configuration needs ~60 GB of host memory and ~100 GB on the GPU")
     _large_config_check(wl.make_config("clustered_large"), oracle_mod, "clustered512", full_counts=False)
 
 
@@ -823,16 +841,18 @@ def test_kdk_step_parity(name, n_side, dt, steps, oracle_mod):
 
 
 # ------------------------------------------------------------------------------- NEXT row 4: paper-default resolution n_h = 4
-@pytest.mark.parametrize("name,n_side", [("tiny_uniform", 16), ("cosmo", 24)])
-def test_parity_paper_default_resolution_nh4(name, n_side, oracle_mod):
+@pytest.mark.parametrize("name,n_side,grid", [("tiny_uniform", 16, False), ("cosmo", 24, False), ("cosmo", 64, True), ("cosmo", 128, True)])
+def test_parity_paper_default_resolution_nh4(name, n_side, grid, oracle_mod):
     """n_h = 4 (N_res = 268 neighbours): every leaf needs a chain of neighbour-list segments (~900
-    candidates against 352 slots), which exercises the multi-segment path of the builder and of all sweeps."""
+    candidates against 352 slots), which exercises the multi-segment path of the builder and of all sweeps.  The two larger
+    cases (262 144 and 2 097 152 particles) compare EVERY particle -- counts bit for bit, all coefficients and derivatives --
+    with the oracle run through its grid neighbour search (bit-identical to the brute-force build, tests/test_oracle_pins.py)."""
     ps = wl.make_config(name, n_side)
     ps.h[:] = (ps.h * (4.0 / ps.n_h)).astype(np.float32)
     ps.n_h = 4.0
     assert float(ps.h.max()) < 0.5 * ps.box
     o = oracle_mod.Oracle(ps.box, ps.gamma, ps.n_h)
-    od = o.step_derivs(ps)
+    od = o.step_derivs(ps, grid=grid)
     g = gpu_eval(ps)
     e_a, e_u = check_parity(ps, g, od, oracle_gv=o.gradv(), label=name + " n_h=4")
     mom, en = check_invariants(ps, g, label=name + " n_h=4")
